@@ -1,0 +1,148 @@
+"""Pins for oracle/network.py (O-5; readings B1-B8)."""
+import numpy as np
+import pytest
+import torch
+import torch.nn.functional as F
+
+from oracle import network as onet
+from synthdata import weights as sw
+
+RNG = np.random.default_rng(17)
+
+
+@pytest.mark.parametrize("c_in,c_out,k,stride,pad,t", [
+    (2, 3, 7, 2, 3, 19), (3, 4, 3, 1, 1, 11), (3, 4, 3, 2, 1, 12), (4, 2, 1, 2, 0, 9), (1, 1, 3, 2, 1, 7)])
+def test_conv_matmul_form_equals_brute_force_definition(c_in, c_out, k, stride, pad, t):
+    x = RNG.standard_normal((2, c_in, t))
+    w = RNG.standard_normal((c_out, c_in, k))
+    fast = onet.conv1d(x, w, stride, pad)
+    for b in range(2):
+        np.testing.assert_allclose(fast[b], onet.conv1d_direct(x[b], w, stride, pad), atol=1e-13)
+
+
+def test_conv_asymmetric_kernel_orientation():
+    # cross-correlation orientation: a single tap at d=0 reads in[t*stride - pad]
+    x = np.arange(10.0)[None, None, :]
+    w = np.zeros((1, 1, 3)); w[0, 0, 0] = 1.0
+    y = onet.conv1d(x, w, 1, 1)[0, 0]
+    np.testing.assert_array_equal(y, np.concatenate([[0.0], np.arange(9.0)]))
+
+
+@pytest.mark.parametrize("k,stride,pad,t", [(7, 2, 3, 64), (3, 1, 1, 33), (3, 2, 1, 32), (1, 2, 0, 31)])
+def test_conv_equals_torch_library(k, stride, pad, t):
+    x = RNG.standard_normal((3, 5, t)); w = RNG.standard_normal((6, 5, k))
+    ref = F.conv1d(torch.from_numpy(x), torch.from_numpy(w), stride=stride, padding=pad).numpy()
+    np.testing.assert_allclose(onet.conv1d(x, w, stride, pad), ref, atol=1e-12)
+
+
+def test_maxpool_equals_torch_library_and_padding_never_wins():
+    x = RNG.standard_normal((2, 3, 17)) - 5.0        # all negative: zero padding would win if used
+    ref = F.max_pool1d(torch.from_numpy(x), 3, 2, 1).numpy()
+    np.testing.assert_array_equal(onet.maxpool1d(x, 3, 2, 1), ref)
+
+
+def _net(cfg):
+    return onet.parse_blob(sw.make_weight_blob(**cfg))
+
+
+def test_fold_is_identity_tiny_and_full_shapes():
+    tiny = _net(sw.tiny_config())
+    x = RNG.standard_normal((2, 2, 256))
+    np.testing.assert_allclose(onet.forward(tiny, x, folded=True), onet.forward(tiny, x, folded=False), rtol=1e-12)
+    # group statistics (config-1 style) on a narrow net so it runs fast
+    cfg = dict(table=sw.resnet_layer_table(2, 16, 7, [1, 1], [16, 32]), norm_kind=sw.NORM_GROUP, n_groups=8, seed=3)
+    net = _net(cfg)
+    np.testing.assert_allclose(onet.forward(net, x, folded=True), onet.forward(net, x, folded=False), rtol=1e-12)
+
+
+def test_per_channel_norm_equals_torch_batchnorm_eval():
+    net = _net(sw.tiny_config())
+    l = net["layers"][0]
+    x = RNG.standard_normal((2, 2, 64))
+    z = F.conv1d(torch.from_numpy(x), torch.from_numpy(l["W"].copy()), stride=l["stride"], padding=l["pad"])
+    ref = F.batch_norm(z, torch.from_numpy(l["mean"].copy()), torch.from_numpy(l["var"].copy()),
+                       torch.from_numpy(l["gamma"].copy()), torch.from_numpy(l["beta"].copy()),
+                       training=False, eps=net["eps"]).numpy()
+    w, b = onet.fold_norm(l, net["norm_kind"], net["n_groups"], net["eps"])
+    np.testing.assert_allclose(onet.conv1d(x, w, l["stride"], l["pad"]) + b[None, :, None], ref, atol=1e-12)
+
+
+def test_group_statistics_index():
+    np.testing.assert_array_equal(onet.stat_index(64, 1, 8), np.repeat(np.arange(8), 8))
+    np.testing.assert_array_equal(onet.stat_index(8, 0, 0), np.arange(8))
+
+
+def _torch_forward(net, x):
+    """Independent re-assembly of the network from torch library ops (conv1d, max_pool1d)."""
+    outs, x0 = [], torch.from_numpy(x)
+    for l in net["layers"]:
+        src = x0 if l["input_from"] < 0 else outs[l["input_from"]]
+        if l["kind"] == 0:
+            g = onet.stat_index(l["c_out"], net["norm_kind"], net["n_groups"])
+            z = F.conv1d(src, torch.from_numpy(l["W"].copy()), stride=l["stride"], padding=l["pad"])
+            y = F.batch_norm(z, torch.from_numpy(l["mean"][g].copy()), torch.from_numpy(l["var"][g].copy()),
+                             torch.from_numpy(l["gamma"].copy()), torch.from_numpy(l["beta"].copy()),
+                             training=False, eps=net["eps"])
+            if l["residual_from"] >= 0:
+                y = y + outs[l["residual_from"]]
+            if l["relu"]:
+                y = F.relu(y)
+        elif l["kind"] == 1:
+            y = F.max_pool1d(src, l["k"], l["stride"], l["pad"])
+        else:
+            y = F.adaptive_avg_pool1d(src, 1)[:, :, 0] @ torch.from_numpy(l["w"].copy()) + l["b"]
+        outs.append(y)
+    return outs[-1].numpy()
+
+
+def test_forward_equals_torch_library_assembly_tiny():
+    net = _net(sw.tiny_config())
+    x = RNG.standard_normal((3, 2, 2048))
+    np.testing.assert_allclose(onet.forward(net, x), _torch_forward(net, x), rtol=1e-10)
+
+
+def test_full_network_shape_closed_forms():
+    cfg = sw.full_config()
+    net = _net(cfg)
+    convs = [l for l in net["layers"] if l["kind"] == 0]
+    assert len(convs) == 36                                        # 1 stem + 32 + 3 shortcuts (B1)
+    n_params = sum(l["W"].size + l["c_out"] for l in convs) + 512 + 1
+    assert n_params == 7_210_689
+    lens = onet.output_length(net, 3072)
+    assert lens[0] == 1536 and lens[1] == 768 and lens[-2] == 96   # B2: 3072 -> 1536 -> 768 ... -> 96
+    macs = sum(l["W"].size * lens[i] for i, l in enumerate(net["layers"]) if l["kind"] == 0) + 512
+    assert abs(macs / 1e6 - 1070.92) < 0.01
+    tiny = _net(sw.tiny_config())
+    tl = onet.output_length(tiny, 2048)
+    assert tl[0] == 1024 and tl[1] == 512 and tl[-2] == 64
+    tconvs = [l for l in tiny["layers"] if l["kind"] == 0]
+    assert sum(l["W"].size + l["c_out"] for l in tconvs) + 64 + 1 == 27_801
+
+
+def test_he_normal_variance_and_head():
+    net = _net(sw.full_config())
+    l = [l for l in net["layers"] if l["kind"] == 0 and l["c_in"] == 256 and l["k"] == 3][0]
+    np.testing.assert_allclose(l["W"].var(), 2.0 / (256 * 3), rtol=0.02)
+    head = net["layers"][-1]
+    np.testing.assert_allclose(head["w"].var(), 1.0 / 512, rtol=0.2)
+    assert head["b"] == 0.0
+
+
+def test_residual_is_added_before_relu():
+    # hand-built 2-layer net: y = relu(conv_b(relu(conv_a(x))) + x); identity-free closed form on 1 channel
+    table = [sw.LayerSpec(0, 1, 1, 1, 1, 0, 1, -1, -1), sw.LayerSpec(0, 1, 1, 1, 1, 0, 1, 0, 0),
+             sw.LayerSpec(2, 1, 1, 1, 1, 0, 0, 1, -1)]
+    net = onet.parse_blob(sw.make_weight_blob(table, 0, 0, seed=5, in_channels=1))
+    for l in net["layers"][:2]:
+        l["W"][:] = -1.0; l["gamma"][:] = 1.0; l["beta"][:] = 0.0; l["mean"][:] = 0.0; l["var"][:] = 1.0 - net["eps"]
+    net["layers"][2]["w"][:] = 1.0
+    x = np.array([[[-2.0, 3.0]]])
+    # conv_a: -x = [2,-3] -> relu [2,0]; conv_b: -[2,0] = [-2,0]; + residual [2,0] -> [0,0]; mean 0
+    # if the residual were added after the ReLU the result would be mean([2,0]) = 1
+    np.testing.assert_allclose(onet.forward(net, x), [0.0], atol=1e-12)
+
+
+def test_round_bf16_matches_torch():
+    x = RNG.standard_normal(1000) * 10
+    ref = torch.from_numpy(x).float().bfloat16().double().numpy()
+    np.testing.assert_array_equal(onet.round_bf16(x), ref)
