@@ -1,0 +1,152 @@
+/* aframe.h -- C ABI of the B200-native (sm_100a) Aframe streaming detection statistic.
+ *
+ * Method: arXiv 2403.18661 (Marx et al. 2024), cited below as P:<line of PAPER.md>.
+ *   strain [2][N] @ 2048 Hz  ->  Welch PSD  ->  whitening filter  ->  whitened stream
+ *   ->  overlapping windows  ->  1D ResNet  ->  one scalar per window
+ * (Sec. II network; Sec. IV.B "PSD estimation, filter construction, and whitening";
+ *  P:170-172 Sec. VI snapshotter -> whitener -> network; Sec. IX timeslides.)
+ * The parameters the paper leaves open are the readings A1..C3 of DESIGN.md.
+ *
+ * Conventions
+ *  - Pointers named d_* are DEVICE pointers owned by the caller; the library never frees or
+ *    reallocates them.  Pointers named h_* / `host_*` are HOST pointers.
+ *  - All work is enqueued on the CUDA stream given to aframe_create.  No call synchronises the
+ *    stream except aframe_create / aframe_destroy / aframe_weights_load / *_create / *_destroy
+ *    and a call that has to grow the context's internal workspace (first use at a larger size).
+ *  - Every call returns an aframe_status; none throws, aborts or prints.  aframe_last_error
+ *    returns a context-owned, NUL-terminated description of the last failure.
+ *  - No CPU fallback exists: on a device that is not compute capability 10.x aframe_create
+ *    returns AFRAME_EUNSUPPORTED.
+ *  - NaN/Inf in the inputs propagate to the outputs; they are not trapped.
+ *  - Strain is pre-scaled on load by the exact power of two 2^strain_scale_log2 (reading A9:
+ *    a PSD of ~1e-46 is below the smallest fp32 denormal).  PSDs handed out by the library are
+ *    in SCALED units: true PSD * 2^(2*strain_scale_log2).  Whitened output is unit-free and
+ *    unaffected.
+ */
+#ifndef AFRAME_H_
+#define AFRAME_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  AFRAME_OK = 0,
+  AFRAME_EINVAL = 1,       /* bad parameter value (NULL pointer, non power-of-two FFT length, ...) */
+  AFRAME_ESHAPE = 2,       /* sizes inconsistent with the configuration / layer table          */
+  AFRAME_ENOMEM = 3,       /* host or device allocation failed                                  */
+  AFRAME_ECUDA = 4,        /* a CUDA call failed; aframe_last_error holds the CUDA string       */
+  AFRAME_ESTATE = 5,       /* object used in a state that does not allow the call               */
+  AFRAME_EUNSUPPORTED = 6  /* device is not sm_100, or the layer table needs an unsupported op  */
+} aframe_status;
+
+typedef enum { AFRAME_FP32 = 0, AFRAME_BF16 = 1 } aframe_precision;
+
+/* POD configuration, versioned by .size (= sizeof(aframe_config)).  Defaults in comments are
+ * BASELINE.json configs[1..4]; configs[0] uses n_design 4096, kernel_len 2048. */
+typedef struct {
+  uint32_t size;
+  int32_t  n_channels;        /* 2: channel 0 = H1, 1 = L1                         */
+  double   fs;                /* 2048 Hz                                                  */
+  int32_t  welch_nfft;        /* 4096 = 2 s Welch segment (reading A1); power of two, 1024..8192 */
+  int32_t  welch_hop;         /* 2048 = 50 % overlap; must equal welch_nfft/2                    */
+  int32_t  filter_len;        /* L = 2048 = 1 s: 0.5 s corrupted per edge; <= 4096*/
+  int32_t  n_design;          /* N_d design-grid FFT length (reading A4): power of two, <= 8192  */
+  double   f_lo, f_hi;        /* 20, 1000 Hz inclusive band (reading A3)                         */
+  int32_t  kernel_len;        /* K = 3072 = 1.5 s window                                 */
+  int32_t  stride;            /* s = 128 samples = 16 Hz inference rate (paper: 512 = 4 Hz)*/
+  int64_t  psd_len;           /* 131072 = 64 s of PSD history; multiple of welch_hop     */
+  int64_t  psd_update;        /* 16384 = new PSD every 8 s (BASELINE.json configs[2])            */
+  int32_t  strain_scale_log2; /* 70                                                              */
+  int32_t  precision;         /* aframe_precision of the network path                            */
+} aframe_config;
+
+typedef struct aframe_ctx aframe_ctx;
+typedef struct aframe_weights aframe_weights;
+typedef struct aframe_stream_state aframe_stream_state;
+
+/* Fill *cfg with the defaults above (size set).  Never fails for cfg != NULL. */
+aframe_status aframe_config_default(aframe_config* cfg);
+
+/* Create a context bound to the current CUDA device and to `cuda_stream` (a cudaStream_t; NULL = the
+ * legacy default stream).  Validates cfg on the host (AFRAME_EINVAL / AFRAME_ESHAPE), checks the
+ * device (AFRAME_EUNSUPPORTED) and uploads twiddle/window tables.  Synchronises. */
+aframe_status aframe_create(const aframe_config* cfg, void* cuda_stream, aframe_ctx** out);
+void          aframe_destroy(aframe_ctx* ctx);
+const char*   aframe_last_error(const aframe_ctx* ctx);   /* ctx may be NULL: returns a static string */
+
+/* ---- O-1  Welch PSD ("The first 8 s is used to estimate the PSD"; reading A1) -------
+ * d_strain: [C][ld] fp32 raw strain, channel c at d_strain + c*ld, n_samples valid per channel
+ *           (n_samples >= welch_nfft, else AFRAME_ESHAPE).
+ * d_psd   : [C][welch_nfft/2+1] fp32, one-sided density, SCALED units, mean over the
+ *           floor((n_samples-nfft)/hop)+1 Hann-windowed, mean-detrended segments. */
+aframe_status aframe_psd_welch(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
+                               float* d_psd);
+
+/* ---- O-2/O-3  filter design + whitening (readings A3-A6) -----------------------------
+ * Designs the L-tap zero-phase FIR whitening filter from d_psd (as returned by aframe_psd_welch) and
+ * applies it to a contiguous segment by FFT overlap-save.  Output has n_samples - filter_len samples
+ * per channel: out[c][m] corresponds to input sample m + filter_len/2 (0.5 s cropped per edge).
+ * d_out: [C][ld_out] of fp32 or bf16 (out_dtype).  n_samples <= filter_len writes nothing (OK). */
+aframe_status aframe_whiten(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
+                            const float* d_psd, void* d_out, int64_t ld_out, aframe_precision out_dtype);
+
+/* Optional read-back of the taps designed by the last aframe_whiten call on this context:
+ * d_taps [C][filter_len+1] fp32, h[j + L/2], j = -L/2..L/2 (used by the parity tests of O-2). */
+aframe_status aframe_filter_taps(aframe_ctx* ctx, float* d_taps);
+
+/* ---- O-6  rolling-PSD whitening of a long segment (BASELINE.json configs[2], [3]) -----------------
+ * Same result, sample for sample, as feeding the segment through aframe_stream_step: a new PSD every
+ * psd_update samples from the trailing psd_len samples, each whitened sample m using the filter of
+ * epoch floor((stride*(floor((m+L/2)/stride)+1) - psd_len)/psd_update).  The first output corresponds
+ * to raw sample psd_len - stride - L/2; *h_n_out (HOST pointer) receives the samples written per
+ * channel (0 if n_samples < psd_len).  d_out: [C][ld_out]. */
+aframe_status aframe_whiten_rolling(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
+                                    void* d_out, int64_t ld_out, aframe_precision out_dtype,
+                                    int64_t* h_n_out);
+
+/* ---- weights (readings B1-B7) ----------------------------------------------------------
+ * host_blob: the version-1 blob documented in synthdata/weights.py (header, layer table, UNFOLDED
+ * fp32 parameters).  The library validates the table against cfg (AFRAME_ESHAPE), folds the frozen
+ * norm into (W', b') in double precision, and uploads fp32 and bf16 (K-major) copies.  Synchronises. */
+aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob, size_t bytes, aframe_weights** out);
+void          aframe_weights_free(aframe_weights* w);
+
+/* ---- O-5  network forward ------------------------------------------------------------------------------
+ * d_windows: [B][C][kernel_len] fp32, already whitened.  d_scores: [B] fp32 raw logits (no sigmoid, B8).
+ * B <= 0 is AFRAME_EINVAL.  Precision follows cfg.precision (bf16: tcgen05 tensor-core path with fp32
+ * accumulation, reading B10; fp32: CUDA-core FFMA path). */
+aframe_status aframe_forward(aframe_ctx* ctx, const aframe_weights* w, const float* d_windows, int64_t B,
+                             float* d_scores);
+
+/* Same network, windows taken in place from a whitened stream (O-4, no unfold copy; timeslides C3):
+ * window i, channel c = d_white[c*ld + first + i*stride + chan_shift[c] + (0..kernel_len)).
+ * dtype is the element type of d_white; chan_shift is a HOST array of n_channels entries (NULL = 0). */
+aframe_status aframe_forward_strided(aframe_ctx* ctx, const aframe_weights* w, const void* d_white,
+                                     aframe_precision dtype, int64_t ld, int64_t first,
+                                     const int64_t* chan_shift, int64_t B, float* d_scores);
+
+/* ---- O-6  streaming ("snapshotting") -------------------------------------------------
+ * The state (raw ring, cached periodograms, PSD, filter, whitened ring, activations) is an opaque
+ * device-resident object owned by the library. */
+aframe_status aframe_stream_create(aframe_ctx* ctx, const aframe_weights* w, aframe_stream_state** out);
+aframe_status aframe_stream_reset(aframe_stream_state* st);
+void          aframe_stream_destroy(aframe_stream_state* st);
+
+/* One update: d_new_samples [C][stride] fp32 raw strain.  Writes d_n_scores[0] (0 during warm-up,
+ * else 1) and, when 1, d_scores[0].  CUDA-graph capturable: no allocation, no host-side control flow
+ * that depends on device data; the update counter lives on the device, so a captured graph can be
+ * replayed for every update. */
+aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samples, aframe_stream_state* st,
+                                 float* d_scores, int32_t* d_n_scores);
+
+/* Number of kernels the library has launched on this context since creation (for bench accounting). */
+int64_t aframe_launch_count(const aframe_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFRAME_H_ */

@@ -1,0 +1,243 @@
+"""Thin ctypes binding of include/aframe.h: argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libaframe_b200.so; torch is used for device
+memory and streams.  There is no CPU fallback: if the shared library is missing or no sm_100 device
+is present, calls fail loudly.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libaframe_b200.so")
+
+OK, EINVAL, ESHAPE, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED = range(7)
+FP32, BF16 = 0, 1
+_STATUS = {0: "AFRAME_OK", 1: "AFRAME_EINVAL", 2: "AFRAME_ESHAPE", 3: "AFRAME_ENOMEM", 4: "AFRAME_ECUDA",
+           5: "AFRAME_ESTATE", 6: "AFRAME_EUNSUPPORTED"}
+
+
+class AframeError(RuntimeError):
+    def __init__(self, status, msg=""):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class aframe_config(C.Structure):
+    _fields_ = [("size", C.c_uint32), ("n_channels", C.c_int32), ("fs", C.c_double),
+                ("welch_nfft", C.c_int32), ("welch_hop", C.c_int32), ("filter_len", C.c_int32),
+                ("n_design", C.c_int32), ("f_lo", C.c_double), ("f_hi", C.c_double),
+                ("kernel_len", C.c_int32), ("stride", C.c_int32), ("psd_len", C.c_int64),
+                ("psd_update", C.c_int64), ("strain_scale_log2", C.c_int32), ("precision", C.c_int32)]
+
+
+EXPORTS = {
+    "aframe_config_default": (C.c_int, [C.POINTER(aframe_config)]),
+    "aframe_create": (C.c_int, [C.POINTER(aframe_config), C.c_void_p, C.POINTER(C.c_void_p)]),
+    "aframe_destroy": (None, [C.c_void_p]),
+    "aframe_last_error": (C.c_char_p, [C.c_void_p]),
+    "aframe_psd_welch": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]),
+    "aframe_whiten": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_int64, C.c_int]),
+    "aframe_filter_taps": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "aframe_whiten_rolling": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_int64, C.c_int,
+                                        C.POINTER(C.c_int64)]),
+    "aframe_weights_load": (C.c_int, [C.c_void_p, C.c_char_p, C.c_size_t, C.POINTER(C.c_void_p)]),
+    "aframe_weights_free": (None, [C.c_void_p]),
+    "aframe_forward": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]),
+    "aframe_forward_strided": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64,
+                                         C.POINTER(C.c_int64), C.c_int64, C.c_void_p]),
+    "aframe_stream_create": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p)]),
+    "aframe_stream_reset": (C.c_int, [C.c_void_p]),
+    "aframe_stream_destroy": (None, [C.c_void_p]),
+    "aframe_stream_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "aframe_launch_count": (C.c_int64, [C.c_void_p]),
+}
+
+_lib = None
+
+
+def load_library():
+    """dlopen the C-ABI library and declare every prototype of include/aframe.h."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2403_18661_b200.build` "
+                              "(or __graft_entry__.build()); there is no fallback path")
+        lib = C.CDLL(LIB_PATH)
+        for name, (res, args) in EXPORTS.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def default_config(**overrides) -> aframe_config:
+    cfg = aframe_config()
+    load_library().aframe_config_default(C.byref(cfg))
+    for k, v in overrides.items():
+        if not hasattr(cfg, k):
+            raise AttributeError(k)
+        setattr(cfg, k, v)
+    return cfg
+
+
+def _ptr(t: torch.Tensor):
+    return C.c_void_p(t.data_ptr())
+
+
+def _need(t, dtype, what):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError(f"{what}: expected a contiguous CUDA tensor of {dtype}")
+
+
+class Weights:
+    def __init__(self, ctx, handle):
+        self.ctx, self.handle = ctx, handle
+
+    def free(self):
+        if self.handle:
+            load_library().aframe_weights_free(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+class Context:
+    """aframe_ctx bound to a torch CUDA stream (default: the current stream)."""
+
+    def __init__(self, cfg: aframe_config | None = None, stream: torch.cuda.Stream | None = None, **overrides):
+        self.lib = load_library()
+        self.cfg = cfg if cfg is not None else default_config(**overrides)
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        h = C.c_void_p()
+        st = self.lib.aframe_create(C.byref(self.cfg), C.c_void_p(self.stream.cuda_stream), C.byref(h))
+        if st != OK:
+            raise AframeError(st, "aframe_create")
+        self.handle = h
+
+    def close(self):
+        if getattr(self, "handle", None):
+            self.lib.aframe_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st):
+        if st != OK:
+            raise AframeError(st, self.lib.aframe_last_error(self.handle).decode())
+
+    @property
+    def n_freq(self):
+        return self.cfg.welch_nfft // 2 + 1
+
+    def launch_count(self):
+        return int(self.lib.aframe_launch_count(self.handle))
+
+    # ---- O-1
+    def psd_welch(self, strain: torch.Tensor, out: torch.Tensor | None = None):
+        _need(strain, torch.float32, "strain")
+        c, n = strain.shape
+        if out is None:
+            out = torch.empty((c, self.n_freq), dtype=torch.float32, device=strain.device)
+        self._check(self.lib.aframe_psd_welch(self.handle, _ptr(strain), n, strain.stride(0), _ptr(out)))
+        return out
+
+    # ---- O-2 / O-3
+    def whiten(self, strain, psd, out=None, out_dtype=torch.float32):
+        _need(strain, torch.float32, "strain"); _need(psd, torch.float32, "psd")
+        c, n = strain.shape
+        n_out = max(n - self.cfg.filter_len, 0)
+        if out is None:
+            out = torch.empty((c, max(n_out, 1)), dtype=out_dtype, device=strain.device)
+        prec = BF16 if out.dtype == torch.bfloat16 else FP32
+        self._check(self.lib.aframe_whiten(self.handle, _ptr(strain), n, strain.stride(0), _ptr(psd), _ptr(out),
+                                           out.stride(0), prec))
+        return out[:, :n_out]
+
+    def filter_taps(self):
+        out = torch.empty((self.cfg.n_channels, self.cfg.filter_len + 1), dtype=torch.float32, device="cuda")
+        self._check(self.lib.aframe_filter_taps(self.handle, _ptr(out)))
+        return out
+
+    def whiten_rolling(self, strain, out=None, out_dtype=torch.float32):
+        _need(strain, torch.float32, "strain")
+        c, n = strain.shape
+        if out is None:
+            out = torch.empty((c, max(n, 1)), dtype=out_dtype, device=strain.device)
+        prec = BF16 if out.dtype == torch.bfloat16 else FP32
+        n_out = C.c_int64(0)
+        self._check(self.lib.aframe_whiten_rolling(self.handle, _ptr(strain), n, strain.stride(0), _ptr(out),
+                                                   out.stride(0), prec, C.byref(n_out)))
+        return out[:, : n_out.value]
+
+    # ---- weights / O-5
+    def load_weights(self, blob: bytes) -> Weights:
+        h = C.c_void_p()
+        self._check(self.lib.aframe_weights_load(self.handle, blob, len(blob), C.byref(h)))
+        return Weights(self, h)
+
+    def forward(self, weights: Weights, windows, scores=None):
+        _need(windows, torch.float32, "windows")
+        b = windows.shape[0]
+        if scores is None:
+            scores = torch.empty((b,), dtype=torch.float32, device=windows.device)
+        self._check(self.lib.aframe_forward(self.handle, weights.handle, _ptr(windows), b, _ptr(scores)))
+        return scores
+
+    def forward_strided(self, weights: Weights, white, first, n_windows, chan_shift=None, scores=None):
+        if not (white.is_cuda and white.is_contiguous() and white.dtype in (torch.float32, torch.bfloat16)):
+            raise TypeError("white: expected a contiguous CUDA tensor of float32 or bfloat16")
+        if scores is None:
+            scores = torch.empty((n_windows,), dtype=torch.float32, device=white.device)
+        shifts = None
+        if chan_shift is not None:
+            shifts = (C.c_int64 * self.cfg.n_channels)(*[int(v) for v in chan_shift])
+        prec = BF16 if white.dtype == torch.bfloat16 else FP32
+        self._check(self.lib.aframe_forward_strided(self.handle, weights.handle, _ptr(white), prec, white.stride(0),
+                                                    int(first), shifts, int(n_windows), _ptr(scores)))
+        return scores
+
+    # ---- O-6
+    def stream_create(self, weights: Weights):
+        return Stream(self, weights)
+
+
+class Stream:
+    def __init__(self, ctx: Context, weights: Weights):
+        self.ctx, self.weights = ctx, weights
+        h = C.c_void_p()
+        ctx._check(ctx.lib.aframe_stream_create(ctx.handle, weights.handle, C.byref(h)))
+        self.handle = h
+        self.score = torch.zeros(1, dtype=torch.float32, device="cuda")
+        self.n_scores = torch.zeros(1, dtype=torch.int32, device="cuda")
+
+    def reset(self):
+        self.ctx._check(self.ctx.lib.aframe_stream_reset(self.handle))
+
+    def step(self, new_samples: torch.Tensor):
+        """Enqueue one update; results land in self.score / self.n_scores (device tensors)."""
+        _need(new_samples, torch.float32, "new_samples")
+        self.ctx._check(self.ctx.lib.aframe_stream_step(self.ctx.handle, _ptr(new_samples), self.handle,
+                                                        _ptr(self.score), _ptr(self.n_scores)))
+
+    def close(self):
+        if getattr(self, "handle", None):
+            self.ctx.lib.aframe_stream_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

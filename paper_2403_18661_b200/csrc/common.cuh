@@ -1,0 +1,120 @@
+// Shared host/device helpers of the aframe B200 library (not shared with oracle/).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string>
+#include <vector>
+
+#include "../../include/aframe.h"
+
+#define AF_MAX_CH 8
+#if defined(__GNUC__)
+#define AF_API extern "C" __attribute__((visibility("default")))
+#else
+#define AF_API extern "C"
+#endif
+
+struct LayerDesc {
+  int kind, c_in, c_out, k, stride, pad, relu, input_from, residual_from;
+  int t_in, t_out;
+};
+
+// Folded network on the device.
+struct aframe_weights {
+  aframe_ctx* ctx = nullptr;
+  std::vector<LayerDesc> layers;
+  int in_channels = 0;
+  int kernel_len = 0;
+  // per conv layer (index = layer index; null for other kinds)
+  std::vector<float*> d_w32;          // [k][c_in][c_out] fp32 (N contiguous) for the CUDA-core path
+  std::vector<__nv_bfloat16*> d_w16;  // [k][c_out][c_in] bf16 (K-major) for the tcgen05 path
+  std::vector<float*> d_bias;         // [c_out] fp32 folded bias
+  float* d_head_w = nullptr;          // [c_in]
+  float head_b = 0.f;
+  int head_layer = -1;
+  bool tc_ok = false;                 // bf16 tensor-core path available for this table
+  std::string tc_reason;
+};
+
+struct Workspace {
+  void* ptr = nullptr;
+  size_t bytes = 0;
+};
+
+struct aframe_ctx {
+  aframe_config cfg;
+  cudaStream_t stream = nullptr;
+  int device = 0;
+  int n_sms = 148;
+  char err[512];
+  int64_t launches = 0;
+  // tables
+  float2* d_tw32 = nullptr;    // exp(-2 pi i q / 8192), q < 8192
+  double2* d_tw64 = nullptr;
+  // scratch
+  Workspace ws_psd;            // periodograms
+  Workspace ws_filt;           // PSD / H / taps per epoch
+  Workspace ws_act;            // network activations
+  float* d_taps_last = nullptr;   // [C][L+1] of the last aframe_whiten call
+  void* encode_tiled = nullptr;   // cuTensorMapEncodeTiled entry point
+};
+
+#define AF_TW_N 8192
+#define AF_NOS 8192   // overlap-save block (real samples)
+
+static inline aframe_status af_fail(aframe_ctx* ctx, aframe_status st, const char* fmt, const char* a = "") {
+  if (ctx) snprintf(ctx->err, sizeof(ctx->err), fmt, a);
+  return st;
+}
+
+#define AF_CUDA(ctx, call)                                                                  \
+  do {                                                                                      \
+    cudaError_t e_ = (call);                                                                \
+    if (e_ != cudaSuccess) {                                                                \
+      if (ctx) snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d %s: %s", __FILE__, __LINE__, \
+                        #call, cudaGetErrorString(e_));                                     \
+      return AFRAME_ECUDA;                                                                  \
+    }                                                                                       \
+  } while (0)
+
+#define AF_LAUNCH_CHECK(ctx)                 \
+  do {                                       \
+    (ctx)->launches++;                       \
+    AF_CUDA(ctx, cudaGetLastError());        \
+  } while (0)
+
+aframe_status af_ws_reserve(aframe_ctx* ctx, Workspace& ws, size_t bytes);
+
+// Device-side gate of the streaming path (O-6): the update counter lives on the device so that one
+// captured CUDA graph serves every update; gated kernels return at once on updates that need no work.
+struct StreamGate {
+  const int64_t* d_n = nullptr;   // samples received so far (after this update's append); null = ungated
+  int* d_has_filter = nullptr;
+  int64_t ring_len = 0;           // raw ring length in samples
+  int64_t psd_len = 0, psd_update = 0;
+  __host__ __device__ bool psd_due() const {
+    const int64_t n = *d_n;
+    return n >= psd_len && ((n - psd_len) % psd_update) == 0;
+  }
+};
+
+// ---- kernels' host entry points (defined in the .cu files) ------------------------------------
+aframe_status af_launch_welch_periodograms(aframe_ctx* ctx, const float* d_strain, int64_t ld, int64_t first_seg,
+                                           int64_t n_seg, float* d_pgram /*[C][n_seg][F]*/, const StreamGate* gate = nullptr);
+aframe_status af_launch_psd_mean(aframe_ctx* ctx, const float* d_pgram, int64_t n_seg_total, int64_t seg0_stride,
+                                 int64_t n_epochs, int64_t n_avg, float* d_psd /*[n_epochs][C][F]*/, const StreamGate* gate = nullptr);
+aframe_status af_launch_filter_design(aframe_ctx* ctx, const float* d_psd, int64_t n_epochs, float* d_H /*[E][C][NOS/2+1]*/,
+                                      float* d_taps /*[E][C][L+1] or null*/, const StreamGate* gate = nullptr);
+aframe_status af_launch_whiten_os(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
+                                  const float* d_H, int64_t in0, int64_t out_total, int64_t epoch_len, int64_t n_epochs,
+                                  void* d_out, int64_t ld_out, int out_bf16);
+
+aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_bf16,
+                              int64_t sB, int64_t sT, const int64_t* choff, int64_t B, float* d_scores);
+aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_bf16,
+                              int64_t sB, int64_t sT, const int64_t* choff, int64_t B, float* d_scores);
+aframe_status af_tc_check(aframe_ctx* ctx, aframe_weights* w);
+void af_tc_forget(aframe_ctx* ctx);

@@ -1,0 +1,198 @@
+// Host side of the bf16 tensor-core network path: TMA tensor maps, per-layer launches, forward driver.
+#include <stdlib.h>
+#include <map>
+
+#include "conv_tc_kernel.cuh"
+#include "common.cuh"
+#include "net_plan.h"
+#include "stem.h"
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static bool encode_map(aframe_ctx* ctx, CUtensorMap* m, const void* ptr, int rank, const uint64_t* dims,
+                       const uint64_t* strides_bytes /*rank-1*/, const uint32_t* box) {
+  cuuint64_t gd[5], gs[4];
+  cuuint32_t bx[5], es[5];
+  for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; es[i] = 1; }
+  for (int i = 0; i < rank - 1; ++i) gs[i] = strides_bytes[i];
+  EncodeTiledFn fn = reinterpret_cast<EncodeTiledFn>(ctx->encode_tiled);
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, const_cast<void*>(ptr), gd, gs, bx, es,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(ctx->err, sizeof(ctx->err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return false;
+  }
+  return true;
+}
+
+struct TcLaunch {
+  CUtensorMap tm_in, tm_w, tm_out, tm_res;
+  TcConvParams p;
+  int BN, grid;
+};
+
+static int tile_t_box(int t_out) {
+  if (t_out % 128 == 0) return 128;
+  int tb = 1;
+  while (tb < 128 && t_out % (tb * 2) == 0) tb *= 2;
+  return tb;
+}
+
+// A conv layer runs on the tensor-core kernel if its channel counts tile into 64-wide K blocks / 64..256-wide N.
+static bool tc_layer_ok(const LayerDesc& l, std::string& why) {
+  if (l.c_in % 64) { why = "conv c_in not a multiple of 64"; return false; }
+  if (!(l.c_out == 64 || l.c_out == 128 || l.c_out % 256 == 0)) { why = "conv c_out not 64, 128 or a multiple of 256"; return false; }
+  if (!((l.k == 3 && l.pad == 1) || (l.k == 1 && l.pad == 0))) { why = "conv kernel/padding other than k3p1 / k1p0"; return false; }
+  if (l.stride != 1 && l.stride != 2) { why = "conv stride other than 1 or 2"; return false; }
+  if (l.t_in % l.stride) { why = "conv input length not divisible by its stride"; return false; }
+  if (l.t_out * l.stride != l.t_in) { why = "conv output length != input length / stride"; return false; }
+  if (tile_t_box(l.t_out) < 8) { why = "conv output length has no power-of-two factor >= 8"; return false; }
+  return true;
+}
+
+aframe_status af_tc_check(aframe_ctx* ctx, aframe_weights* w) {
+  w->tc_ok = false;
+  const int n = (int)w->layers.size();
+  if (!ctx->encode_tiled) { w->tc_reason = "cuTensorMapEncodeTiled entry point not found"; return AFRAME_OK; }
+  if (n < 3 || w->layers[0].kind != 0 || w->layers[0].input_from != -1 || w->layers[1].kind != 1 ||
+      w->layers[1].input_from != 0) { w->tc_reason = "table does not start with stem conv + max-pool"; return AFRAME_OK; }
+  const LayerDesc& s = w->layers[0];
+  const LayerDesc& q = w->layers[1];
+  if (!(s.k == 7 && s.c_in == 2 && s.c_out == 64 && s.stride == 2 && s.pad == 3 && s.relu && s.residual_from < 0 &&
+        q.k == 3 && q.stride == 2 && q.pad == 1)) { w->tc_reason = "stem is not conv(2->64,k7,s2,p3)+ReLU+maxpool(k3,s2,p1)"; return AFRAME_OK; }
+  for (int i = 2; i < n; ++i) {
+    const LayerDesc& l = w->layers[i];
+    if (l.input_from == 0 || l.residual_from == 0 || l.input_from < 0) { w->tc_reason = "a layer reads the pre-pool stem output or the raw input"; return AFRAME_OK; }
+    if (l.kind == 1) { w->tc_reason = "max-pool after the stem is not built on the bf16 path"; return AFRAME_OK; }
+    if (l.kind == 0 && !tc_layer_ok(l, w->tc_reason)) return AFRAME_OK;
+  }
+  w->tc_ok = true;
+  return AFRAME_OK;
+}
+
+static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const __nv_bfloat16* in,
+                         const __nv_bfloat16* res, __nv_bfloat16* out, int64_t nb, TcLaunch& L) {
+  const LayerDesc& l = w->layers[li];
+  const int BN = l.c_out >= 256 ? 256 : l.c_out;
+  const int T_box = tile_t_box(l.t_out), B_box = 128 / T_box;
+  const int P = l.stride;
+  {
+    const uint64_t dims[4] = {(uint64_t)l.c_in, (uint64_t)P, (uint64_t)(l.t_in / P), (uint64_t)nb};
+    const uint64_t str[3] = {(uint64_t)l.c_in * 2, (uint64_t)P * l.c_in * 2, (uint64_t)l.t_in * l.c_in * 2};
+    const uint32_t box[4] = {64, 1, (uint32_t)T_box, (uint32_t)B_box};
+    if (!encode_map(ctx, &L.tm_in, in, 4, dims, str, box)) return false;
+  }
+  {
+    const uint64_t dims[3] = {(uint64_t)l.c_in, (uint64_t)l.c_out, (uint64_t)l.k};
+    const uint64_t str[2] = {(uint64_t)l.c_in * 2, (uint64_t)l.c_out * l.c_in * 2};
+    const uint32_t box[3] = {64, (uint32_t)BN, 1};
+    if (!encode_map(ctx, &L.tm_w, w->d_w16[li], 3, dims, str, box)) return false;
+  }
+  {
+    const uint64_t dims[4] = {(uint64_t)l.c_out, 1, (uint64_t)l.t_out, (uint64_t)nb};
+    const uint64_t str[3] = {(uint64_t)l.c_out * 2, (uint64_t)l.c_out * 2, (uint64_t)l.t_out * l.c_out * 2};
+    const uint32_t box[4] = {64, 1, (uint32_t)T_box, (uint32_t)B_box};
+    if (!encode_map(ctx, &L.tm_out, out, 4, dims, str, box)) return false;
+    if (!encode_map(ctx, &L.tm_res, res ? res : out, 4, dims, str, box)) return false;
+  }
+  TcConvParams& p = L.p;
+  p.bias = w->d_bias[li];
+  p.taps = l.k; p.pad = l.pad; p.P = P;
+  p.kblocks = l.c_in / 64;
+  p.n_tiles = l.c_out / BN;
+  p.T_box = T_box; p.B_box = B_box;
+  p.t_blks = l.t_out / T_box;
+  const int64_t b_blks = (nb + B_box - 1) / B_box;
+  p.num_tiles = (int)(b_blks * p.t_blks * p.n_tiles);
+  p.relu = l.relu; p.has_res = res != nullptr;
+  L.BN = BN;
+  L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
+  return true;
+}
+
+template <int BN> static cudaError_t launch_bn(const TcLaunch& L, cudaStream_t s) {
+  static bool attr = false;
+  if (!attr) {
+    cudaError_t e = cudaFuncSetAttribute(conv_tc_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<BN>::SMEM);
+    if (e != cudaSuccess) return e;
+    attr = true;
+  }
+  conv_tc_kernel<BN><<<L.grid, 192, TcCfg<BN>::SMEM, s>>>(L.tm_in, L.tm_w, L.tm_out, L.tm_res, L.p);
+  return cudaGetLastError();
+}
+
+struct TcPlanCache {
+  const aframe_weights* w = nullptr;
+  void* base = nullptr;
+  int64_t nb = 0;
+  size_t slot_bytes = 0;
+  std::vector<TcLaunch> launches;   // indexed by layer
+};
+static std::map<aframe_ctx*, std::vector<TcPlanCache>> g_cache;
+
+void af_tc_forget(aframe_ctx* ctx) { g_cache.erase(ctx); }
+
+static int64_t tc_chunk_windows() {
+  static int64_t v = 0;
+  if (v == 0) {
+    const char* e = getenv("AFRAME_CHUNK_B");
+    v = e ? atoll(e) : 512;
+    if (v < 1) v = 512;
+  }
+  return v;
+}
+
+aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_bf16, int64_t sB,
+                              int64_t sT, const int64_t* choff, int64_t B, float* d_scores) {
+  (void)sT;
+  NetPlan plan;
+  af_make_plan(w, true, plan);
+  const int64_t chunk = tc_chunk_windows() < B ? tc_chunk_windows() : B;
+  const size_t slot_bytes = ((plan.slot_elems * 2 * (size_t)chunk) + 1023) & ~(size_t)1023;
+  aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots);
+  if (st != AFRAME_OK) return st;
+  char* base = reinterpret_cast<char*>(ctx->ws_act.ptr);
+  const int n = (int)w->layers.size();
+  auto slot_ptr = [&](int layer) { return reinterpret_cast<__nv_bfloat16*>(base + slot_bytes * plan.slot[layer]); };
+  std::vector<TcPlanCache>& caches = g_cache[ctx];
+
+  for (int64_t b0 = 0; b0 < B; b0 += chunk) {
+    const int64_t nb = (B - b0 < chunk) ? (B - b0) : chunk;
+    TcPlanCache* pc = nullptr;
+    for (auto& c : caches)
+      if (c.w == w && c.base == base && c.nb == nb && c.slot_bytes == slot_bytes) { pc = &c; break; }
+    if (!pc) {
+      if (caches.size() > 8) caches.clear();
+      caches.emplace_back();
+      pc = &caches.back();
+      pc->w = w; pc->base = base; pc->nb = nb; pc->slot_bytes = slot_bytes;
+      pc->launches.resize(n);
+      for (int i = 2; i < n; ++i) {
+        const LayerDesc& l = w->layers[i];
+        if (l.kind != 0) continue;
+        if (!build_launch(ctx, w, i, slot_ptr(l.input_from), l.residual_from >= 0 ? slot_ptr(l.residual_from) : nullptr,
+                          slot_ptr(i), nb, pc->launches[i])) { caches.pop_back(); return AFRAME_ECUDA; }
+      }
+    }
+    const size_t esz = in_bf16 ? 2 : 4;
+    st = af_launch_stem_bf16(ctx, w->layers[0], w->layers[1], reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz,
+                             in_bf16, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1));
+    if (st != AFRAME_OK) return st;
+    for (int i = 2; i < n; ++i) {
+      const LayerDesc& l = w->layers[i];
+      if (l.kind == 0) {
+        const TcLaunch& L = pc->launches[i];
+        cudaError_t e = L.BN == 256 ? launch_bn<256>(L, ctx->stream) : (L.BN == 128 ? launch_bn<128>(L, ctx->stream) : launch_bn<64>(L, ctx->stream));
+        ctx->launches++;
+        if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
+      } else if (l.kind == 2) {
+        st = af_launch_head(ctx, slot_ptr(l.input_from), 1, w->d_head_w, w->head_b, l.t_in, l.c_in, nb, d_scores + b0);
+        if (st != AFRAME_OK) return st;
+      }
+    }
+  }
+  return AFRAME_OK;
+}
