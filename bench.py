@@ -1,0 +1,395 @@
+#!/usr/bin/env python
+"""bench.py -- throughput / latency of the B200-native Aframe detection-statistic path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Workload (BASELINE.json configs[3], "offline background throughput"): a 1e5 s two-detector record of
+synthetic coloured noise is analysed in time blocks of --block-seconds (default 4096 s).  ONE STEP = one
+block through the whole hot path: raw strain -> rolling Welch PSD (64 s, new every
+8 s) -> filter design -> overlap-save whitening (once per detector) -> 8 timeslides (L1 shifted 1..8 s)
+of 1.5 s windows at stride 128, 4096 windows per launch sequence -> bf16 tcgen05 ResNet -> one score per
+window.  Each step takes a different block (its own seeded noise), so nothing is reused between steps.
+
+    value = analysed livetime per second = sum_slides windows * stride / fs / wall   [strain-seconds/s]
+
+Multi-GPU: blocks are independent; rank r takes its own blocks, no collective on the data
+path ("scaling": "weak").  The time is the max over ranks of the CUDA-event time of the K steps.
+
+The JSON line also carries: "e2e" (same steps through aframe_score_timeslides_host: pinned host strain
+in, scores out, copies inside the timed region), "roofline" of the dominant kernel family (conv_tc_kernel,
+tensor-bound) from CUDA events recorded by the library on its own stream, "stages" (per-stage device
+time), "latency" (configs[4]: per-update p50/p99 of aframe_stream_step) and "cpu_baseline" (the float64
+oracle timed on this box's host cores on a bounded sample).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FS = 2048
+STRIDE = 128
+KERNEL = 3072
+FILTER = 2048
+PSD_LEN = 131072
+N_SLIDES = 8
+MMAC_CONV = 1069.5e6      # residual-stage MACs per window
+MMAC_TOTAL = 1070.92e6    # incl. stem and head
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=4)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--block-seconds", type=int, default=4096, help="strain seconds analysed per slide per step")
+    ap.add_argument("--batch", type=int, default=4096, help="windows per launch sequence (configs[3]: 4096)")
+    ap.add_argument("--latency-updates", type=int, default=10000, help="configs[4] timed updates (0 = skip)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def block_geometry(block_seconds):
+    """Raw samples a block needs so that n_win windows per slide fit for shifts up to N_SLIDES seconds."""
+    n_win = block_seconds * FS // STRIDE
+    m0 = PSD_LEN - STRIDE - FILTER // 2                       # raw index of whitened sample 0 (reading C1)
+    n_white = (n_win - 1) * STRIDE + N_SLIDES * FS + KERNEL   # whitened samples the windows reach
+    n_raw = m0 + n_white + FILTER // 2
+    n_raw = -(-n_raw // STRIDE) * STRIDE
+    return n_win, n_raw
+
+
+def make_block(index, n_raw):
+    from synthdata import coloured_noise
+    seed = int(np.random.SeedSequence([1003, index]).generate_state(1)[0])
+    return coloured_noise(n_raw, seed=seed)
+
+
+class ClockSampler:
+    """nvidia-smi SM clock / throttle-reason samples during the timed region (B200_PROFILING.md)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows, self.proc, self.gpu = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([v.strip() for v in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------------
+# the oracle on the host cores: cpu_baseline leg and --impl reference
+# ------------------------------------------------------------------------------------------------------
+def oracle_sample(n_windows, seg_seconds=66):
+    """Time the float64 oracle, as it stands, on a bounded sample of the workload: Welch PSD + filter
+    design + FFT whitening of `seg_seconds` s x 2 channels, then the network forward on n_windows windows
+    taken from that whitened stream at stride 128.  Returns the combined rate for N_SLIDES timeslides."""
+    from oracle import network as onet, psd as opsd, whiten as owh
+    from synthdata import coloured_noise, full_config, make_weight_blob
+    x = coloured_noise(seg_seconds * FS, seed=1003).astype(np.float64)
+    net = onet.parse_blob(make_weight_blob(**full_config()))
+    t0 = time.perf_counter()
+    y = np.stack([owh.whiten_fft(x[c], owh.design_filter(opsd.welch(x[c, :PSD_LEN]))) for c in range(2)])
+    t_wh = time.perf_counter() - t0
+    wins = np.stack([y[:, i * STRIDE: i * STRIDE + KERNEL] for i in range(n_windows)])
+    t0 = time.perf_counter()
+    scores = onet.forward(net, wins)
+    t_net = time.perf_counter() - t0
+    assert np.all(np.isfinite(scores))
+    whiten_rate = (seg_seconds - 1) / t_wh                  # whitened strain-seconds (both detectors) per second
+    win_rate = n_windows / t_net
+    per_second = 1.0 / whiten_rate + N_SLIDES * (FS / STRIDE) / win_rate   # CPU seconds per second of record
+    return {"value": N_SLIDES / per_second, "windows_per_s": win_rate, "whiten_strain_s_per_s": whiten_rate,
+            "seconds": t_wh + t_net}
+
+
+def host_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
+    except Exception:
+        n = 1
+    return int(min(n, len(os.sched_getaffinity(0))))
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_windows = 64
+    for _ in range(args.warmup):
+        oracle_sample(8, seg_seconds=66)
+    t0 = time.perf_counter()
+    vals = [oracle_sample(n_windows) for _ in range(args.steps)]
+    dt = time.perf_counter() - t0
+    v = float(np.mean([r["value"] for r in vals]))
+    sample = (f"per step: Welch+design+whitening of 66 s x 2 ch and the float64 ResNet forward on {n_windows} windows "
+              f"of configs[3]'s stream; rates combined for {N_SLIDES} timeslides")
+    print(json.dumps({
+        "impl": "reference", "metric": "analysed strain-seconds per second (whitened + scored, all timeslides)",
+        "value": v, "unit": "strain-s/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[3] offline background (bounded sample, float64 CPU oracle)", "sample": sample},
+        "windows_per_s": float(np.mean([r["windows_per_s"] for r in vals])),
+        "cpu_baseline": {"value": v, "unit": "strain-s/s", "cores": host_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "strain-s/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ------------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------------
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return {"bf16_burst": d["bf16_tflops"], "bf16_sustained": d["bf16_tflops_sustained"], "hbm": d["hbm_gbs"],
+                "source": "MEASURED_PEAKS.json"}
+    return {"bf16_burst": 1590.0, "bf16_sustained": 1400.0, "hbm": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+def latency_run(af, torch, ctx_stream, weights_blob, n_updates, n_warm_scored=100):
+    """configs[4]: one update of 128 new samples per detector, batch 1, over a 1.5 s ring with incremental
+    whitening.  Host wall-clock from the call to the score being readable on the host, and device time."""
+    from synthdata import coloured_noise
+    ctx = af.Context(precision=af.BF16, stream=ctx_stream)
+    w = ctx.load_weights(weights_blob)
+    st = ctx.stream_create(w)
+    n_fill = PSD_LEN // STRIDE + KERNEL // STRIDE           # updates before the first score (reading C1)
+    total = n_fill + n_warm_scored + n_updates
+    x = coloured_noise(total * STRIDE, seed=1002)
+    # [update][channel][stride], pinned; each update's H2D copy (1 KiB) is inside the timed call
+    upd = torch.from_numpy(np.ascontiguousarray(x.reshape(2, total, STRIDE).transpose(1, 0, 2))).pin_memory()
+    dev_in = torch.empty((2, STRIDE), dtype=torch.float32, device="cuda")
+    host_out = torch.zeros(2, dtype=torch.float32).pin_memory()
+    wall, dev = [], []
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(ctx_stream):
+        for u in range(total):
+            timed = u >= n_fill + n_warm_scored
+            t0 = time.perf_counter()
+            dev_in.copy_(upd[u], non_blocking=True)
+            if timed:
+                ev0.record(ctx_stream)
+            st.step(dev_in)
+            if timed:
+                ev1.record(ctx_stream)
+            host_out[0:1].copy_(st.score, non_blocking=True)
+            ctx_stream.synchronize()
+            if timed:
+                wall.append(time.perf_counter() - t0)
+                dev.append(ev0.elapsed_time(ev1) * 1e-3)
+    n_scored = int(st.n_scores.item())
+    assert n_scored == 1 and np.isfinite(float(host_out[0]))
+    wall, dev = np.asarray(wall) * 1e3, np.asarray(dev) * 1e3
+    out = {"workload": "configs[4]: 128 new samples/detector per update, batch 1, bf16 config-1 network",
+           "updates": int(n_updates), "p50_ms": float(np.percentile(wall, 50)), "p99_ms": float(np.percentile(wall, 99)),
+           "device_p50_ms": float(np.percentile(dev, 50)), "device_p99_ms": float(np.percentile(dev, 99)),
+           "mean_ms": float(wall.mean()), "timing": "host wall-clock: pinned H2D of the update + aframe_stream_step + "
+           "D2H of the score + stream sync; device: CUDA events around aframe_stream_step",
+           "graph": bool(getattr(st, "uses_graph", False)),
+           "realtime_factor": float((STRIDE / FS) / (wall.mean() * 1e-3))}
+    st.close(); w.free(); ctx.close()
+    return out
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as ge
+    import paper_2403_18661_b200 as af
+    from synthdata import full_config, make_weight_blob
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    if not os.path.exists(af.LIB_PATH):
+        ge.build()
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    stream = torch.cuda.Stream()
+    blob = make_weight_blob(**full_config())
+    n_win, n_raw = block_geometry(args.block_seconds)
+    shifts = [k * FS for k in range(1, N_SLIDES + 1)]
+    n_blocks = args.warmup + args.steps
+    blocks_host = [torch.from_numpy(make_block(rank * 1000 + j, n_raw)).pin_memory() for j in range(n_blocks)]
+    blocks_dev = [b.cuda() for b in blocks_host]
+    scores_dev = torch.empty((N_SLIDES, n_win), dtype=torch.float32, device="cuda")
+    scores_host = torch.empty((N_SLIDES, n_win), dtype=torch.float32).pin_memory()
+    torch.cuda.synchronize()
+
+    with torch.cuda.stream(stream):
+        ctx = af.Context(precision=af.BF16, stream=stream)
+        w = ctx.load_weights(blob)
+
+        def step_dev(j):
+            ctx.score_timeslides(w, blocks_dev[j], 0, n_win, shifts, batch=args.batch, scores=scores_dev)
+
+        def step_host(j):
+            ctx.score_timeslides(w, blocks_host[j], 0, n_win, shifts, batch=args.batch, scores=scores_host)
+
+        # ---- device-resident timing -----------------------------------------------------------------
+        for j in range(args.warmup):
+            step_dev(j)
+        barrier()
+        launches0 = ctx.launch_count()
+        ctx.profile(True)
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for j in range(args.steps):
+            step_dev(args.warmup + j)
+        e1.record(stream)
+        barrier()
+        clocks = sampler.stop()
+        ms_total = e0.elapsed_time(e1)
+        stages = ctx.profile_read()
+        ctx.profile(False)
+        launches = ctx.launch_count() - launches0
+        assert torch.isfinite(scores_dev).all()
+
+        # ---- end to end: pinned host strain in, scores out, copies inside the timed region -------------
+        e2e = None
+        if not args.no_e2e:
+            step_host(0)
+            barrier()
+            t0 = time.perf_counter()
+            for j in range(args.steps):
+                step_host(args.warmup + j)     # synchronises inside (scores are on the host when it returns)
+            barrier()
+            e2e_s = time.perf_counter() - t0
+            assert torch.isfinite(scores_host).all()
+
+    t = torch.tensor([ms_total, (e2e_s if not args.no_e2e else 0.0) * 1e3], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, e2e_ms = float(t[0]), float(t[1])
+    livetime = world * args.steps * N_SLIDES * n_win * STRIDE / FS        # strain-seconds, all ranks
+    windows = world * args.steps * N_SLIDES * n_win
+    value = livetime / (ms_total * 1e-3)
+    if not args.no_e2e:
+        e2e = {"value": livetime / (e2e_ms * 1e-3), "unit": "strain-s/s",
+               "h2d_bytes_per_step": int(blocks_host[0].numel() * 4), "d2h_bytes_per_step": int(scores_host.numel() * 4),
+               "api": "aframe_score_timeslides_host (pinned host buffers; H2D + D2H inside the call)"}
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = measured_peaks()
+    conv_ms, conv_launches = stages["conv"]
+    win_rank = args.steps * N_SLIDES * n_win
+    conv_tflops = 2.0 * MMAC_CONV * win_rank / (conv_ms * 1e-3) / 1e12 if conv_ms > 0 else 0.0
+    out = {
+        "metric": "analysed strain-seconds per second (whitened + scored, all timeslides)",
+        "value": value, "unit": "strain-s/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": f"configs[3] offline background: {N_SLIDES} timeslides, {args.batch} windows/launch sequence, "
+                               f"1.5 s windows at stride 128, config-1 ResNet bf16; record analysed in blocks of "
+                               f"{args.block_seconds} s, one block per step",
+                   "block_seconds": args.block_seconds, "windows_per_step": N_SLIDES * n_win, "batch": args.batch,
+                   "l2": "each step reads a different block; per-launch activations (>= 400 MB) exceed the 126 MB L2",
+                   "chunk_windows": int(os.environ.get("AFRAME_CHUNK_B", "0")) or "library default"},
+        "windows_per_s": windows / (ms_total * 1e-3),
+        "end_to_end_tflops": 2.0 * MMAC_TOTAL * windows / (ms_total * 1e-3) / 1e12,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+        "roofline": {"kernel": "conv_tc_kernel<BN> (35 residual-stage convolutions, tcgen05 implicit GEMM)",
+                     "bound": "tensor", "achieved": conv_tflops, "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
+                     "frac": conv_tflops / peaks["bf16_sustained"], "traffic": None,
+                     "peak_kind": "sustained bf16 cuBLAS, " + peaks["source"], "launches": int(conv_launches),
+                     "avg_launch_ms": conv_ms / max(conv_launches, 1),
+                     "algorithmic": "2 x 1069.5 MMAC per window x windows scored, over the summed CUDA-event time of "
+                                    "the conv launches on the library's stream"},
+        "stages": {k: {"ms": v[0], "launches": v[1], "share": v[0] / ms_total} for k, v in stages.items()},
+    }
+    wh_ms = stages["whiten"][0]
+    if wh_ms > 0:
+        n_out_block = n_raw - (PSD_LEN - STRIDE - FILTER // 2) - FILTER // 2
+        gbs = args.steps * 2 * n_out_block * (4 + 2) / (wh_ms * 1e-3) / 1e9      # fp32 in + bf16 out per sample
+        out["roofline_whiten"] = {"kernel": "whiten_os_kernel", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"],
+                                  "unit": "GB/s", "frac": gbs / peaks["hbm"], "traffic": None,
+                                  "algorithmic": "4 B in + 2 B (bf16) out per whitened sample per channel"}
+    if args.latency_updates > 0 and world == 1:
+        out["latency"] = latency_run(af, torch, stream, blob, args.latency_updates)
+    if not args.no_cpu_baseline:
+        r = oracle_sample(256)
+        out["cpu_baseline"] = {"value": r["value"], "unit": "strain-s/s", "cores": host_threads(), "kind": "oracle",
+                               "windows_per_s": r["windows_per_s"], "whiten_strain_s_per_s": r["whiten_strain_s_per_s"],
+                               "sample": "float64 oracle: Welch+design+whitening of 66 s x 2 ch and the ResNet forward on "
+                                         "256 windows of the same stream; rates combined for 8 timeslides"}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -143,8 +143,49 @@ void          aframe_stream_destroy(aframe_stream_state* st);
 aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samples, aframe_stream_state* st,
                                  float* d_scores, int32_t* d_n_scores);
 
+/* ---- O-3..O-6 in one call: offline background analysis of a stored segment (C3) ---------
+ * BASELINE.json configs[3]: the segment is whitened once per detector with the rolling-PSD rule
+ * (aframe_whiten_rolling; output kept in the context's workspace in the network's input precision),
+ * then n_slides timeslides are scored: window i of slide k takes channel 0 (H1, held fixed) at whitened
+ * index first + i*stride and every other channel at first + i*stride + slide_shifts[k] ("the Livingston
+ * data is shifted in 1 s increments"; shifts in SAMPLES, applied to the whitened stream, C3).
+ * Whitened index 0 is raw sample psd_len - stride - filter_len/2 of the segment.  Windows are scored
+ * `batch` per launch sequence (configs[3]: 4096).  scores: [n_slides][n_windows] fp32 logits.
+ * h_slide_shifts is a HOST array.  AFRAME_ESHAPE if any window reaches outside the whitened segment.
+ *
+ * aframe_score_timeslides      : d_strain / d_scores are DEVICE pointers; asynchronous on the stream.
+ * aframe_score_timeslides_host : h_strain / h_scores are HOST pointers (pinned memory makes the copies
+ *   asynchronous); the call copies the segment to the device, runs the same path, copies the scores back
+ *   and synchronises the stream before returning. */
+aframe_status aframe_score_timeslides(aframe_ctx* ctx, const aframe_weights* w, const float* d_strain,
+                                      int64_t n_samples, int64_t ld, int64_t first, int64_t n_windows,
+                                      const int64_t* h_slide_shifts, int32_t n_slides, int64_t batch,
+                                      float* d_scores);
+aframe_status aframe_score_timeslides_host(aframe_ctx* ctx, const aframe_weights* w, const float* h_strain,
+                                           int64_t n_samples, int64_t ld, int64_t first, int64_t n_windows,
+                                           const int64_t* h_slide_shifts, int32_t n_slides, int64_t batch,
+                                           float* h_scores);
+
 /* Number of kernels the library has launched on this context since creation (for bench accounting). */
 int64_t aframe_launch_count(const aframe_ctx* ctx);
+
+/* ---- per-stage device timing (measurement aid) ------------------------------------------
+ * aframe_profile(ctx, 1) clears the counters and makes every later call bracket each stage of the path
+ * with a pair of CUDA events on the context's stream; aframe_profile(ctx, 0) stops.  aframe_profile_read
+ * synchronises the stream and returns, per stage kind, the summed device time in milliseconds and the
+ * number of kernel launches it covered (arrays of AFRAME_PROF_KINDS entries, HOST pointers). */
+enum {
+  AFRAME_PROF_WELCH = 0,    /* periodograms + PSD mean (a-2)            */
+  AFRAME_PROF_DESIGN = 1,   /* whitening-filter design (a-3)            */
+  AFRAME_PROF_WHITEN = 2,   /* overlap-save / FIR whitening (a-4)       */
+  AFRAME_PROF_STEM = 3,     /* window assembly + stem + max-pool (a-5/6)*/
+  AFRAME_PROF_CONV = 4,     /* residual-stage convolutions (a-7)        */
+  AFRAME_PROF_HEAD = 5,     /* pool + linear head (a-8)                 */
+  AFRAME_PROF_STREAM = 6,   /* ring-buffer bookkeeping (a-9)            */
+  AFRAME_PROF_KINDS = 8
+};
+aframe_status aframe_profile(aframe_ctx* ctx, int enable);
+aframe_status aframe_profile_read(aframe_ctx* ctx, double* h_ms, int64_t* h_launches);
 
 #ifdef __cplusplus
 }

@@ -54,7 +54,14 @@ EXPORTS = {
     "aframe_stream_destroy": (None, [C.c_void_p]),
     "aframe_stream_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "aframe_launch_count": (C.c_int64, [C.c_void_p]),
+    "aframe_score_timeslides": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_int64,
+                                          C.POINTER(C.c_int64), C.c_int32, C.c_int64, C.c_void_p]),
+    "aframe_score_timeslides_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64,
+                                               C.c_int64, C.POINTER(C.c_int64), C.c_int32, C.c_int64, C.c_void_p]),
+    "aframe_profile": (C.c_int, [C.c_void_p, C.c_int]),
+    "aframe_profile_read": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
 }
+PROF_KINDS = ("welch", "design", "whiten", "stem", "conv", "head", "stream", "reserved")
 
 _lib = None
 
@@ -207,6 +214,33 @@ class Context:
         self._check(self.lib.aframe_forward_strided(self.handle, weights.handle, _ptr(white), prec, white.stride(0),
                                                     int(first), shifts, int(n_windows), _ptr(scores)))
         return scores
+
+    # ---- configs[3]: whiten once, score every timeslide
+    def score_timeslides(self, weights: Weights, strain, first, n_windows, slide_shifts, batch=4096, scores=None):
+        """strain: CUDA tensor (device entry point) or pinned/pageable CPU tensor (host entry point,
+        copies inside the call, synchronises).  Returns scores [n_slides][n_windows] on the same side."""
+        if not (isinstance(strain, torch.Tensor) and strain.dtype == torch.float32 and strain.stride(1) == 1):
+            raise TypeError("strain: expected a float32 tensor [C][N] with unit inner stride")
+        c, n = strain.shape
+        ns = len(slide_shifts)
+        sh = (C.c_int64 * ns)(*[int(v) for v in slide_shifts])
+        if scores is None:
+            scores = torch.empty((ns, n_windows), dtype=torch.float32, device=strain.device,
+                                 pin_memory=not strain.is_cuda)
+        fn = self.lib.aframe_score_timeslides if strain.is_cuda else self.lib.aframe_score_timeslides_host
+        self._check(fn(self.handle, weights.handle, _ptr(strain), n, strain.stride(0), int(first), int(n_windows), sh, ns,
+                       int(batch), _ptr(scores)))
+        return scores
+
+    # ---- per-stage device timing
+    def profile(self, enable: bool):
+        self._check(self.lib.aframe_profile(self.handle, 1 if enable else 0))
+
+    def profile_read(self):
+        ms = (C.c_double * 8)()
+        nl = (C.c_int64 * 8)()
+        self._check(self.lib.aframe_profile_read(self.handle, ms, nl))
+        return {k: (ms[i], int(nl[i])) for i, k in enumerate(PROF_KINDS) if k != "reserved"}
 
     # ---- O-6
     def stream_create(self, weights: Weights):

@@ -127,6 +127,10 @@ AF_API void aframe_destroy(aframe_ctx* ctx) {
   af_tc_forget(ctx);
   cudaFree(ctx->d_tw32); cudaFree(ctx->d_tw64); cudaFree(ctx->d_taps_last);
   cudaFree(ctx->ws_psd.ptr); cudaFree(ctx->ws_filt.ptr); cudaFree(ctx->ws_act.ptr);
+  cudaFree(ctx->ws_white.ptr); cudaFree(ctx->ws_stage.ptr);
+  for (ProfSpan& s : ctx->prof_spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+  for (cudaEvent_t e : ctx->prof_pool) cudaEventDestroy(e);
+  for (int k = 0; k < AFRAME_PROF_KINDS; ++k) if (ctx->prof_open[k]) cudaEventDestroy(ctx->prof_open[k]);
   cudaGetLastError();
   delete ctx;
 }
@@ -374,4 +378,131 @@ AF_API aframe_status aframe_forward_strided(aframe_ctx* ctx, const aframe_weight
     choff[c] = (int64_t)c * ld + first + sh;
   }
   return forward_common(ctx, w, d_white, dtype == AFRAME_BF16, ctx->cfg.stride, choff, B, d_scores);
+}
+
+// ---- per-stage device timing --------------------------------------------------------------------------
+static cudaEvent_t prof_event(aframe_ctx* ctx) {
+  cudaEvent_t e = nullptr;
+  if (!ctx->prof_pool.empty()) { e = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); return e; }
+  if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return e;
+}
+
+void af_prof_begin(aframe_ctx* ctx, int kind) {
+  if (!ctx->prof_on || ctx->prof_open[kind]) return;
+  cudaEvent_t e = prof_event(ctx);
+  if (!e) return;
+  cudaEventRecord(e, ctx->stream);
+  ctx->prof_open[kind] = e;
+}
+
+void af_prof_end(aframe_ctx* ctx, int kind, int launches) {
+  if (!ctx->prof_on || !ctx->prof_open[kind]) return;
+  cudaEvent_t e = prof_event(ctx);
+  if (!e) return;
+  cudaEventRecord(e, ctx->stream);
+  ctx->prof_spans.push_back(ProfSpan{ctx->prof_open[kind], e, kind, launches});
+  ctx->prof_open[kind] = nullptr;
+}
+
+static void prof_clear(aframe_ctx* ctx) {
+  for (ProfSpan& s : ctx->prof_spans) { ctx->prof_pool.push_back(s.a); ctx->prof_pool.push_back(s.b); }
+  ctx->prof_spans.clear();
+  for (int k = 0; k < AFRAME_PROF_KINDS; ++k)
+    if (ctx->prof_open[k]) { ctx->prof_pool.push_back(ctx->prof_open[k]); ctx->prof_open[k] = nullptr; }
+}
+
+AF_API aframe_status aframe_profile(aframe_ctx* ctx, int enable) {
+  if (!ctx) return AFRAME_EINVAL;
+  AF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  prof_clear(ctx);
+  ctx->prof_on = enable != 0;
+  return AFRAME_OK;
+}
+
+AF_API aframe_status aframe_profile_read(aframe_ctx* ctx, double* h_ms, int64_t* h_launches) {
+  if (!ctx) return AFRAME_EINVAL;
+  if (!h_ms || !h_launches) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
+  AF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  for (int k = 0; k < AFRAME_PROF_KINDS; ++k) { h_ms[k] = 0.0; h_launches[k] = 0; }
+  for (const ProfSpan& s : ctx->prof_spans) {
+    float ms = 0.f;
+    AF_CUDA(ctx, cudaEventElapsedTime(&ms, s.a, s.b));
+    h_ms[s.kind] += (double)ms;
+    h_launches[s.kind] += s.launches;
+  }
+  return AFRAME_OK;
+}
+
+// ---- offline background analysis: whiten once, score every timeslide (configs[3]) ---------------------
+static aframe_status score_timeslides_dev(aframe_ctx* ctx, const aframe_weights* w, const float* d_strain,
+                                          int64_t n_samples, int64_t ld, int64_t first, int64_t n_windows,
+                                          const int64_t* h_slide_shifts, int32_t n_slides, int64_t batch,
+                                          float* d_scores) {
+  const aframe_config& cfg = ctx->cfg;
+  const int C = cfg.n_channels;
+  if (n_windows <= 0 || n_slides <= 0 || batch <= 0) return af_fail(ctx, AFRAME_EINVAL, "n_windows, n_slides, batch must be positive");
+  if (first < 0) return af_fail(ctx, AFRAME_EINVAL, "first must be non-negative");
+  if (w->ctx != ctx) return af_fail(ctx, AFRAME_ESTATE, "weights belong to another context");
+  const int bf16 = cfg.precision == AFRAME_BF16;
+  const size_t esz = bf16 ? 2 : 4;
+  const int64_t ld_w = (n_samples + 63) & ~(int64_t)63;
+  aframe_status st = af_ws_reserve(ctx, ctx->ws_white, esz * (size_t)C * ld_w);
+  if (st != AFRAME_OK) return st;
+  int64_t n_out = 0;
+  st = aframe_whiten_rolling(ctx, d_strain, n_samples, ld, ctx->ws_white.ptr, ld_w, bf16 ? AFRAME_BF16 : AFRAME_FP32, &n_out);
+  if (st != AFRAME_OK) return st;
+  int64_t sh_min = 0, sh_max = 0;
+  for (int k = 0; k < n_slides; ++k) {
+    if (h_slide_shifts[k] < sh_min) sh_min = h_slide_shifts[k];
+    if (h_slide_shifts[k] > sh_max) sh_max = h_slide_shifts[k];
+  }
+  if (first + sh_min < 0 || first + sh_max + (n_windows - 1) * cfg.stride + cfg.kernel_len > n_out)
+    return af_fail(ctx, AFRAME_ESHAPE, "timeslide windows reach outside the whitened segment");
+  for (int k = 0; k < n_slides; ++k) {
+    int64_t shifts[AF_MAX_CH];
+    shifts[0] = 0;
+    for (int c = 1; c < C; ++c) shifts[c] = h_slide_shifts[k];
+    for (int64_t i0 = 0; i0 < n_windows; i0 += batch) {
+      const int64_t nb = n_windows - i0 < batch ? n_windows - i0 : batch;
+      st = aframe_forward_strided(ctx, w, ctx->ws_white.ptr, bf16 ? AFRAME_BF16 : AFRAME_FP32, ld_w,
+                                  first + i0 * cfg.stride, shifts, nb, d_scores + (int64_t)k * n_windows + i0);
+      if (st != AFRAME_OK) return st;
+    }
+  }
+  return AFRAME_OK;
+}
+
+AF_API aframe_status aframe_score_timeslides(aframe_ctx* ctx, const aframe_weights* w, const float* d_strain,
+                                             int64_t n_samples, int64_t ld, int64_t first, int64_t n_windows,
+                                             const int64_t* h_slide_shifts, int32_t n_slides, int64_t batch,
+                                             float* d_scores) {
+  if (!ctx) return AFRAME_EINVAL;
+  if (!w || !d_strain || !h_slide_shifts || !d_scores) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
+  return score_timeslides_dev(ctx, w, d_strain, n_samples, ld, first, n_windows, h_slide_shifts, n_slides, batch, d_scores);
+}
+
+AF_API aframe_status aframe_score_timeslides_host(aframe_ctx* ctx, const aframe_weights* w, const float* h_strain,
+                                                  int64_t n_samples, int64_t ld, int64_t first, int64_t n_windows,
+                                                  const int64_t* h_slide_shifts, int32_t n_slides, int64_t batch,
+                                                  float* h_scores) {
+  if (!ctx) return AFRAME_EINVAL;
+  if (!w || !h_strain || !h_slide_shifts || !h_scores) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
+  if (n_samples <= 0 || ld < n_samples) return af_fail(ctx, AFRAME_ESHAPE, "ld < n_samples");
+  if (n_windows <= 0 || n_slides <= 0) return af_fail(ctx, AFRAME_EINVAL, "n_windows, n_slides must be positive");
+  const int C = ctx->cfg.n_channels;
+  const int64_t ld_d = (n_samples + 63) & ~(int64_t)63;
+  const size_t strain_bytes = sizeof(float) * (size_t)C * ld_d;
+  const size_t score_bytes = sizeof(float) * (size_t)n_slides * n_windows;
+  aframe_status st = af_ws_reserve(ctx, ctx->ws_stage, strain_bytes + score_bytes);
+  if (st != AFRAME_OK) return st;
+  float* d_strain = reinterpret_cast<float*>(ctx->ws_stage.ptr);
+  float* d_scores = reinterpret_cast<float*>(reinterpret_cast<char*>(ctx->ws_stage.ptr) + strain_bytes);
+  AF_CUDA(ctx, cudaMemcpy2DAsync(d_strain, sizeof(float) * ld_d, h_strain, sizeof(float) * ld, sizeof(float) * n_samples, C,
+                                 cudaMemcpyHostToDevice, ctx->stream));
+  st = score_timeslides_dev(ctx, w, d_strain, n_samples, ld_d, first, n_windows, h_slide_shifts, n_slides, batch, d_scores);
+  if (st != AFRAME_OK) return st;
+  AF_CUDA(ctx, cudaMemcpyAsync(h_scores, d_scores, score_bytes, cudaMemcpyDeviceToHost, ctx->stream));
+  AF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  return AFRAME_OK;
 }

@@ -39,6 +39,11 @@ struct aframe_weights {
   std::string tc_reason;
 };
 
+struct ProfSpan {
+  cudaEvent_t a, b;
+  int kind, launches;
+};
+
 struct Workspace {
   void* ptr = nullptr;
   size_t bytes = 0;
@@ -60,7 +65,19 @@ struct aframe_ctx {
   Workspace ws_act;            // network activations
   float* d_taps_last = nullptr;   // [C][L+1] of the last aframe_whiten call
   void* encode_tiled = nullptr;   // cuTensorMapEncodeTiled entry point
+  Workspace ws_white;          // whitened stream of aframe_score_timeslides
+  Workspace ws_stage;          // device staging of the *_host entry points
+  // optional per-stage device timing (aframe_profile): CUDA-event pairs on ctx->stream
+  bool prof_on = false;
+  std::vector<ProfSpan> prof_spans;
+  std::vector<cudaEvent_t> prof_pool;
+  cudaEvent_t prof_open[AFRAME_PROF_KINDS] = {};
 };
+
+// Stage timing: af_prof_begin records an event before the first launch of a stage, af_prof_end one after
+// its last launch; aframe_profile_read sums the elapsed times per stage.  No-ops unless profiling is on.
+void af_prof_begin(aframe_ctx* ctx, int kind);
+void af_prof_end(aframe_ctx* ctx, int kind, int launches);
 
 #define AF_TW_N 8192
 #define AF_NOS 8192   // overlap-save block (real samples)

@@ -178,18 +178,27 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       }
     }
     const size_t esz = in_bf16 ? 2 : 4;
+    af_prof_begin(ctx, AFRAME_PROF_STEM);
     st = af_launch_stem_bf16(ctx, w->layers[0], w->layers[1], reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz,
                              in_bf16, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1));
+    af_prof_end(ctx, AFRAME_PROF_STEM, 1);
     if (st != AFRAME_OK) return st;
+    int n_conv = 0;
     for (int i = 2; i < n; ++i) {
       const LayerDesc& l = w->layers[i];
       if (l.kind == 0) {
         const TcLaunch& L = pc->launches[i];
+        af_prof_begin(ctx, AFRAME_PROF_CONV);
+        ++n_conv;
         cudaError_t e = L.BN == 256 ? launch_bn<256>(L, ctx->stream) : (L.BN == 128 ? launch_bn<128>(L, ctx->stream) : launch_bn<64>(L, ctx->stream));
         ctx->launches++;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
       } else if (l.kind == 2) {
+        af_prof_end(ctx, AFRAME_PROF_CONV, n_conv);
+        n_conv = 0;
+        af_prof_begin(ctx, AFRAME_PROF_HEAD);
         st = af_launch_head(ctx, slot_ptr(l.input_from), 1, w->d_head_w, w->head_b, l.t_in, l.c_in, nb, d_scores + b0);
+        af_prof_end(ctx, AFRAME_PROF_HEAD, 1);
         if (st != AFRAME_OK) return st;
       }
     }

@@ -202,6 +202,8 @@ aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const vo
         a.T_in = l.t_in; a.T_out = l.t_out; a.C_in = l.c_in; a.C_out = l.c_out;
         a.k = l.k; a.stride = l.stride; a.pad = l.pad; a.relu = l.relu;
         dim3 grid((unsigned)((a.rows + 63) / 64), (unsigned)((l.c_out + 63) / 64));
+        const int pk = l.input_from < 0 ? AFRAME_PROF_STEM : AFRAME_PROF_CONV;
+        af_prof_begin(ctx, pk);
         if (l.input_from < 0) {
           const size_t esz = in_bf16 ? 2 : 4;
           a.in = reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz;
@@ -213,16 +215,21 @@ aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const vo
           a.in = src; a.in_sB = (int64_t)l.t_in * l.c_in; a.in_sT = l.c_in; a.in_sC = 1; a.use_choff = 0;
           conv_fp32_kernel<false><<<grid, 256, 0, ctx->stream>>>(a);
         }
+        af_prof_end(ctx, pk, 1);
         AF_LAUNCH_CHECK(ctx);
       } else if (l.kind == 1) {
         if (!src) return af_fail(ctx, AFRAME_EUNSUPPORTED, "max-pool directly on the network input is not supported");
         const int64_t total = nb * l.t_out * l.c_out;
+        af_prof_begin(ctx, AFRAME_PROF_STEM);
         maxpool_fp32_kernel<<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(src, dst, total, l.t_in, l.t_out,
                                                                                       l.c_out, l.k, l.stride, l.pad);
+        af_prof_end(ctx, AFRAME_PROF_STEM, 1);
         AF_LAUNCH_CHECK(ctx);
       } else {
         if (!src) return af_fail(ctx, AFRAME_EUNSUPPORTED, "head directly on the network input is not supported");
+        af_prof_begin(ctx, AFRAME_PROF_HEAD);
         st = af_launch_head(ctx, src, 0, w->d_head_w, w->head_b, l.t_in, l.c_in, nb, d_scores + b0);
+        af_prof_end(ctx, AFRAME_PROF_HEAD, 1);
         if (st != AFRAME_OK) return st;
       }
     }

@@ -263,6 +263,7 @@ aframe_status af_launch_welch_periodograms(aframe_ctx* ctx, const float* d_strai
   const double sum_w2 = 0.375 * nfft;                 // sum of the periodic Hann window squared
   const float norm = (float)(1.0 / (cfg.fs * sum_w2));
   dim3 grid((unsigned)(gate_in ? 1 : n_seg), (unsigned)cfg.n_channels);
+  af_prof_begin(ctx, AFRAME_PROF_WELCH);
 #define AF_WELCH_CASE(N)                                                                                            \
   case N:                                                                                                           \
     welch_periodogram_kernel<N><<<grid, N / 32, 0, ctx->stream>>>(d_strain, ld, cfg.welch_hop, first_seg, n_seg,    \
@@ -273,6 +274,7 @@ aframe_status af_launch_welch_periodograms(aframe_ctx* ctx, const float* d_strai
     default: return af_fail(ctx, AFRAME_EINVAL, "welch_nfft must be a power of two in 1024..8192");
   }
 #undef AF_WELCH_CASE
+  af_prof_end(ctx, AFRAME_PROF_WELCH, 1);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }
@@ -283,7 +285,9 @@ aframe_status af_launch_psd_mean(aframe_ctx* ctx, const float* d_pgram, int64_t 
   if (n_epochs <= 0) return AFRAME_OK;
   const int F = ctx->cfg.welch_nfft / 2 + 1;
   dim3 grid((F + 127) / 128, (unsigned)n_epochs, (unsigned)ctx->cfg.n_channels);
+  af_prof_begin(ctx, AFRAME_PROF_WELCH);
   psd_mean_kernel<<<grid, 128, 0, ctx->stream>>>(d_pgram, n_seg_total, seg_step, (int)n_avg, F, ctx->cfg.n_channels, d_psd, gate);
+  af_prof_end(ctx, AFRAME_PROF_WELCH, 1);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }
@@ -298,6 +302,7 @@ aframe_status af_launch_filter_design(aframe_ctx* ctx, const float* d_psd, int64
   const size_t smem = filter_design_smem(cfg.filter_len);
   dim3 grid((unsigned)n_epochs, (unsigned)cfg.n_channels);
   const int F_w = cfg.welch_nfft / 2 + 1;
+  af_prof_begin(ctx, AFRAME_PROF_DESIGN);
 #define AF_FD_CASE(N)                                                                                                \
   case N: {                                                                                                          \
     static bool attr_set = false;                                                                                    \
@@ -313,6 +318,7 @@ aframe_status af_launch_filter_design(aframe_ctx* ctx, const float* d_psd, int64
     default: return af_fail(ctx, AFRAME_EINVAL, "n_design must be a power of two in 1024..8192");
   }
 #undef AF_FD_CASE
+  af_prof_end(ctx, AFRAME_PROF_DESIGN, 1);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }
@@ -326,12 +332,14 @@ aframe_status af_launch_whiten_os(aframe_ctx* ctx, const float* d_strain, int64_
   const int bpe = (int)((epoch_len + valid - 1) / valid);
   const float scale = ldexpf(1.0f, cfg.strain_scale_log2);
   dim3 grid((unsigned)(n_epochs * bpe), (unsigned)cfg.n_channels);
+  af_prof_begin(ctx, AFRAME_PROF_WHITEN);
   if (out_bf16)
     whiten_os_kernel<true><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, cfg.n_channels, in0, out_total,
                                                           epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
   else
     whiten_os_kernel<false><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, cfg.n_channels, in0, out_total,
                                                            epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
+  af_prof_end(ctx, AFRAME_PROF_WHITEN, 1);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }
