@@ -31,8 +31,24 @@ static bool encode_map(aframe_ctx* ctx, CUtensorMap* m, const void* ptr, int ran
 struct TcLaunch {
   CUtensorMap tm_in, tm_w, tm_out, tm_res;
   TcConvParams p;
-  int BN, grid;
+  int BN, grid, smem;
+  bool head;
 };
+
+// score[b] = (sum of the fused-head partials of window b) / T + bias   (deterministic: fixed summation order)
+__global__ void head_finish_kernel(const float* __restrict__ part, int n_part, float inv_t, float bias, int64_t B,
+                                   float* __restrict__ scores) {
+  const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= B) return;
+  float s = 0.f;
+  for (int i = 0; i < n_part; ++i) s += part[b * n_part + i];
+  scores[b] = s * inv_t + bias;
+}
+
+static int env_int(const char* name, int dflt) {
+  const char* e = getenv(name);
+  return e ? atoi(e) : dflt;
+}
 
 static int tile_t_box(int t_out) {
   if (t_out % 128 == 0) return 128;
@@ -74,7 +90,8 @@ aframe_status af_tc_check(aframe_ctx* ctx, aframe_weights* w) {
 }
 
 static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const __nv_bfloat16* in,
-                         const __nv_bfloat16* res, __nv_bfloat16* out, int64_t nb, TcLaunch& L) {
+                         const __nv_bfloat16* res, __nv_bfloat16* out, int64_t nb, bool head, float* head_part,
+                         TcLaunch& L) {
   const LayerDesc& l = w->layers[li];
   const int BN = l.c_out >= 256 ? 256 : l.c_out;
   const int T_box = tile_t_box(l.t_out), B_box = 128 / T_box;
@@ -108,20 +125,37 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   const int64_t b_blks = (nb + B_box - 1) / B_box;
   p.num_tiles = (int)(b_blks * p.t_blks * p.n_tiles);
   p.relu = l.relu; p.has_res = res != nullptr;
+  p.c_out = l.c_out;
+  p.head_w = head ? w->d_head_w : nullptr;
+  p.head_part = head ? head_part : nullptr;
+  p.head_slabs = l.t_out / 32;
+  p.nb = nb;
+  // shared-memory plan (227 KB per CTA): main-loop ring depth vs epilogue staging / residual prefetch buffers
+  if (BN == 256)      { p.stages = p.has_res ? 3 : 4; p.nbuf = p.has_res ? 4 : 2; p.pf = p.has_res ? 2 : 0; }
+  else if (BN == 128) { p.stages = p.has_res ? 3 : 4; p.nbuf = p.has_res ? 3 : 2; p.pf = p.has_res ? 1 : 0; }
+  else                { p.stages = 5;                 p.nbuf = 3;                 p.pf = p.has_res ? 1 : 0; }
   L.BN = BN;
+  L.head = head;
+  L.smem = BN == 256 ? TcCfg<256>::smem(p.stages, p.nbuf, head) : (BN == 128 ? TcCfg<128>::smem(p.stages, p.nbuf, head)
+                                                                            : TcCfg<64>::smem(p.stages, p.nbuf, head));
   L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
   return true;
 }
 
-template <int BN> static cudaError_t launch_bn(const TcLaunch& L, cudaStream_t s) {
+template <int BN, bool HEAD> static cudaError_t launch_bn(const TcLaunch& L, cudaStream_t s) {
   static bool attr = false;
   if (!attr) {
-    cudaError_t e = cudaFuncSetAttribute(conv_tc_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<BN>::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(conv_tc_kernel<BN, HEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448);
     if (e != cudaSuccess) return e;
     attr = true;
   }
-  conv_tc_kernel<BN><<<L.grid, 192, TcCfg<BN>::SMEM, s>>>(L.tm_in, L.tm_w, L.tm_out, L.tm_res, L.p);
+  conv_tc_kernel<BN, HEAD><<<L.grid, TcCfg<BN>::THREADS, L.smem, s>>>(L.tm_in, L.tm_w, L.tm_out, L.tm_res, L.p);
   return cudaGetLastError();
+}
+
+static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s) {
+  if (L.head) return launch_bn<256, true>(L, s);
+  return L.BN == 256 ? launch_bn<256, false>(L, s) : (L.BN == 128 ? launch_bn<128, false>(L, s) : launch_bn<64, false>(L, s));
 }
 
 struct TcPlanCache {
@@ -139,8 +173,8 @@ static int64_t tc_chunk_windows() {
   static int64_t v = 0;
   if (v == 0) {
     const char* e = getenv("AFRAME_CHUNK_B");
-    v = e ? atoll(e) : 512;
-    if (v < 1) v = 512;
+    v = e ? atoll(e) : 592;     // 4 x 148 SMs: every layer's tile count is then a whole number of waves
+    if (v < 1) v = 592;
   }
   return v;
 }
@@ -152,10 +186,26 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   af_make_plan(w, true, plan);
   const int64_t chunk = tc_chunk_windows() < B ? tc_chunk_windows() : B;
   const size_t slot_bytes = ((plan.slot_elems * 2 * (size_t)chunk) + 1023) & ~(size_t)1023;
-  aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots);
+  const int n = (int)w->layers.size();
+  // fused head: the conv feeding the head (and nothing else) pools + dots in its epilogue and stores nothing
+  int fuse = -1, n_part = 0;
+  {
+    const LayerDesc& h = w->layers[n - 1];
+    const int src = h.input_from;
+    bool only_consumer = src >= 2 && w->layers[src].kind == 0;
+    for (int i = 0; only_consumer && i < n - 1; ++i)
+      if (w->layers[i].input_from == src || w->layers[i].residual_from == src) only_consumer = false;
+    if (only_consumer && w->layers[src].c_out % 256 == 0 && w->layers[src].c_out <= 512 && tile_t_box(w->layers[src].t_out) % 32 == 0 &&
+        env_int("AFRAME_FUSE_HEAD", 1)) {
+      fuse = src;
+      n_part = (w->layers[src].t_out / 32) * (w->layers[src].c_out / 64);
+    }
+  }
+  const size_t part_bytes = (sizeof(float) * (size_t)n_part * chunk + 1023) & ~(size_t)1023;
+  aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots + part_bytes);
   if (st != AFRAME_OK) return st;
   char* base = reinterpret_cast<char*>(ctx->ws_act.ptr);
-  const int n = (int)w->layers.size();
+  float* head_part = reinterpret_cast<float*>(base + slot_bytes * plan.n_slots);
   auto slot_ptr = [&](int layer) { return reinterpret_cast<__nv_bfloat16*>(base + slot_bytes * plan.slot[layer]); };
   std::vector<TcPlanCache>& caches = g_cache[ctx];
 
@@ -174,7 +224,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         const LayerDesc& l = w->layers[i];
         if (l.kind != 0) continue;
         if (!build_launch(ctx, w, i, slot_ptr(l.input_from), l.residual_from >= 0 ? slot_ptr(l.residual_from) : nullptr,
-                          slot_ptr(i), nb, pc->launches[i])) { caches.pop_back(); return AFRAME_ECUDA; }
+                          slot_ptr(i), nb, i == fuse, head_part, pc->launches[i])) { caches.pop_back(); return AFRAME_ECUDA; }
       }
     }
     const size_t esz = in_bf16 ? 2 : 4;
@@ -190,14 +240,21 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         const TcLaunch& L = pc->launches[i];
         af_prof_begin(ctx, AFRAME_PROF_CONV);
         ++n_conv;
-        cudaError_t e = L.BN == 256 ? launch_bn<256>(L, ctx->stream) : (L.BN == 128 ? launch_bn<128>(L, ctx->stream) : launch_bn<64>(L, ctx->stream));
+        cudaError_t e = launch_conv(L, ctx->stream);
         ctx->launches++;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
       } else if (l.kind == 2) {
         af_prof_end(ctx, AFRAME_PROF_CONV, n_conv);
         n_conv = 0;
         af_prof_begin(ctx, AFRAME_PROF_HEAD);
-        st = af_launch_head(ctx, slot_ptr(l.input_from), 1, w->d_head_w, w->head_b, l.t_in, l.c_in, nb, d_scores + b0);
+        if (fuse >= 0) {
+          head_finish_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, ctx->stream>>>(head_part, n_part, 1.0f / l.t_in, w->head_b, nb,
+                                                                                  d_scores + b0);
+          ctx->launches++;
+          if (cudaGetLastError() != cudaSuccess) return af_fail(ctx, AFRAME_ECUDA, "head_finish launch failed");
+        } else {
+          st = af_launch_head(ctx, slot_ptr(l.input_from), 1, w->d_head_w, w->head_b, l.t_in, l.c_in, nb, d_scores + b0);
+        }
         af_prof_end(ctx, AFRAME_PROF_HEAD, 1);
         if (st != AFRAME_OK) return st;
       }

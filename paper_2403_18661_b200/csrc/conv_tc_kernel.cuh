@@ -9,9 +9,12 @@
 //                               per window, so rows never bleed between windows.  Stride 2 = parity dim.
 //   B tile (BN x 64 ch)       : TMA box of the folded bf16 weights [taps][C_out][C_in] (K-major).
 //   tcgen05.mma M=128, N=BN, K=16, fp32 accumulators in TMEM (two stages of BN columns).
-//   Epilogue: tcgen05.ld -> +bias (+residual via TMA) -> ReLU -> bf16 -> swizzled smem -> TMA store.
+//   Epilogue: tcgen05.ld -> +bias (+residual, prefetched by TMA) -> ReLU -> bf16 -> swizzled smem -> TMA store,
+//   or (HEAD) the fused global-average-pool + linear head: per-(window, slab) partial dot products.
 //
-// Warp roles (192 threads): warp 0 TMA producer, warp 1 MMA issuer (+TMEM alloc), warps 2-5 epilogue.
+// Warp roles: warp 0 TMA producer, warp 1 MMA issuer (+TMEM alloc), then EG epilogue groups of 4 warps.
+// With EG = 2 the groups take alternate tiles (group g <-> TMEM accumulator stage g), which doubles the
+// epilogue rate of the small-K layers whose epilogue, not the MMA, is the critical path.
 // Persistent: CTA i handles tiles i, i + grid, ...
 #pragma once
 #include "tc_ptx.cuh"
@@ -25,49 +28,78 @@ struct TcConvParams {
   int t_blks, T_box, B_box;  // tile = T_box rows of B_box windows (T_box * B_box = 128)
   int num_tiles;
   int relu, has_res;
+  int stages;                // smem ring depth of the main loop
+  int nbuf, pf;              // output/residual staging buffers per epilogue group, residual prefetch distance
+  int c_out;
+  // fused head (HEAD variant): partial[b][slab][chunk] = sum_{t in slab, c in chunk} bf16(out[b][t][c]) * head_w[c]
+  const float* head_w;
+  float* head_part;
+  int head_slabs;            // T_out / T_box
+  int64_t nb;                // windows in this launch (head variant bounds check)
 };
+
+// shared-memory carve-up (bytes from the 1024-aligned start of dynamic shared memory):
+//   [0, 256) mbarriers + TMEM base slot | [256, 2304) bias[c_out <= 512] | HEAD only: [3072, 5120) head_w
+//   then the main-loop ring (1024-aligned stages) and the epilogue staging buffers
+#define TC_BAR_BYTES 256
+#define TC_OUT_BYTES (128 * 128)    // one 64-channel chunk of the output tile
+__host__ __device__ constexpr int tc_fixed_bytes(bool head) { return head ? 5120 : 3072; }
 
 template <int BN> struct TcCfg {
   static constexpr int A_BYTES = 128 * 128;
   static constexpr int B_BYTES = BN * 128;
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int OUT_BYTES = 128 * 128;                 // one 64-channel chunk of the output tile
-  static constexpr int STAGES = (BN == 256) ? 4 : (BN == 128 ? 6 : 8);
-  static constexpr int SMEM = STAGES * STAGE_BYTES + 2 * OUT_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+  static constexpr int EG = (BN == 256) ? 1 : 2;
+  static constexpr int THREADS = 64 + 128 * EG;
+  static constexpr int smem(int stages, int nbuf, bool head) {
+    return tc_fixed_bytes(head) + stages * STAGE_BYTES + EG * nbuf * TC_OUT_BYTES;
+  }
 };
 
 __device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 
-template <int BN>
-__global__ void __launch_bounds__(192, 1)
+template <int BN, bool HEAD>
+__global__ void __launch_bounds__(TcCfg<BN>::THREADS, 1)
 conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_w,
                const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_res,
                const TcConvParams p) {
   using Cfg = TcCfg<BN>;
-  constexpr int STAGES = Cfg::STAGES;
-  extern __shared__ unsigned char smem_raw[];
-  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t out_base = base + STAGES * Cfg::STAGE_BYTES;
-  const uint32_t bar_base = out_base + 2 * Cfg::OUT_BYTES;
-  // barriers (8 B each): full[STAGES], empty[STAGES], tmem_full[2], tmem_empty[2], res_full[2]; then tmem ptr
-  auto full_bar = [&](int s) { return bar_base + 8u * s; };
-  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
-  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + a); };
-  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + 2 + a); };
-  auto res_bar = [&](int b) { return bar_base + 8u * (2 * STAGES + 4 + b); };
-  const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 6);
-  unsigned char* gen_base = smem_raw + (base - smem_u32(smem_raw));
+  constexpr int EG = Cfg::EG;
+  constexpr int MAXBUF = 4;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const uint32_t base = smem_u32(smem_raw);
+  if (base & 1023u) __trap();                      // SWIZZLE_128B tiles need 1024-byte alignment
+  unsigned char* gen_base = smem_raw;
+  const int STAGES = p.stages;
+  // barriers (8 B each): full[S], empty[S], tfull[2], tempty[2], res[EG][MAXBUF]; then the TMEM base slot
+  auto full_bar = [&](int s) { return base + 8u * s; };
+  auto empty_bar = [&](int s) { return base + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int a) { return base + 8u * (2 * STAGES + a); };
+  auto tempty_bar = [&](int a) { return base + 8u * (2 * STAGES + 2 + a); };
+  auto res_bar = [&](int g, int b) { return base + 8u * (2 * STAGES + 4 + g * MAXBUF + b); };
+  const uint32_t tmem_slot = base + 8u * (2 * STAGES + 4 + EG * MAXBUF);
+  float* s_bias = reinterpret_cast<float*>(gen_base + TC_BAR_BYTES);
+  float* s_headw = reinterpret_cast<float*>(gen_base + 3072);
+  const uint32_t stage_base = base + tc_fixed_bytes(HEAD);
+  const uint32_t out_base = stage_base + STAGES * Cfg::STAGE_BYTES;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
-    tma_prefetch_desc(&tm_in); tma_prefetch_desc(&tm_w); tma_prefetch_desc(&tm_out);
+    tma_prefetch_desc(&tm_in); tma_prefetch_desc(&tm_w);
+    if (!HEAD) tma_prefetch_desc(&tm_out);
     if (p.has_res) tma_prefetch_desc(&tm_res);
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 128); mbar_init(res_bar(a), 1); }
+    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 128); }
+    for (int g = 0; g < EG; ++g)
+      for (int b = 0; b < MAXBUF; ++b) mbar_init(res_bar(g, b), 1);
     fence_mbar_init();
   }
   if (warp == 1) tmem_alloc(tmem_slot, 512);
+  for (int i = threadIdx.x; i < p.c_out; i += blockDim.x) {
+    s_bias[i] = p.bias[i];
+    if (HEAD) s_headw[i] = p.head_w[i];
+  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -89,7 +121,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
           for (int kb = 0; kb < p.kblocks; ++kb) {
             mbar_wait(empty_bar(stage), phase ^ 1u);
             mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
-            const uint32_t sa = base + stage * Cfg::STAGE_BYTES;
+            const uint32_t sa = stage_base + stage * Cfg::STAGE_BYTES;
             tma_load_4d(sa, &tm_in, full_bar(stage), kb * 64, par, t0 + toff, b0);
             tma_load_3d(sa + Cfg::A_BYTES, &tm_w, full_bar(stage), kb * 64, n0, d);
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
@@ -110,7 +142,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
         for (int it = 0; it < kiters; ++it) {
           mbar_wait(full_bar(stage), phase);
           tc_fence_after();
-          const uint32_t sa = base + stage * Cfg::STAGE_BYTES;
+          const uint32_t sa = stage_base + stage * Cfg::STAGE_BYTES;
           const uint64_t da = umma_desc_sw128(sa), db = umma_desc_sw128(sa + Cfg::A_BYTES);
 #pragma unroll
           for (int k = 0; k < 4; ++k)   // 4 x (K = 16 bf16 = 32 B) inside the 128-byte swizzle row
@@ -123,50 +155,79 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
       }
     }
   } else {
-    // ===== epilogue: 4 warps, thread <-> one output row =====
+    // ===== epilogue: EG groups of 4 warps, thread <-> one output row =====
+    const int ew = warp - 2;
+    const int g = ew >> 2;                         // epilogue group: takes this CTA's tiles g, g + EG, ...
     const int q = warp & 3;                        // TMEM lane quadrant this warp may access
     const int row = q * 32 + lane;
-    const bool leader = (threadIdx.x == 64);
-    int acc = 0; uint32_t acc_phase = 0;
-    uint32_t chunk_ctr = 0;
-    for (int tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+    const bool leader = ((ew & 3) == 0) && lane == 0;
+    const int NBUF = p.nbuf, PF = p.pf;
+    const uint32_t gbuf = out_base + (uint32_t)(g * NBUF) * TC_OUT_BYTES;
+    constexpr int CH = BN / 64;
+    const int tile_step = EG * gridDim.x;
+
+    // residual prefetch cursor (leader only): chunk pf_j of this group's chunk sequence
+    int pf_tile = blockIdx.x + g * gridDim.x, pf_c = 0;
+    uint32_t pf_j = 0;
+    auto issue_res = [&]() {
+      if (pf_tile < p.num_tiles) {
+        const int n_idx = pf_tile % p.n_tiles, m_idx = pf_tile / p.n_tiles;
+        const int t0 = (m_idx % p.t_blks) * p.T_box, b0 = (m_idx / p.t_blks) * p.B_box, n0 = n_idx * BN;
+        const int buf = pf_j % NBUF;
+        mbar_arrive_expect_tx(res_bar(g, buf), TC_OUT_BYTES);
+        tma_load_4d(gbuf + buf * TC_OUT_BYTES, &tm_res, res_bar(g, buf), n0 + pf_c * 64, 0, t0, b0);
+      }
+      ++pf_j;
+      if (++pf_c == CH) { pf_c = 0; pf_tile += tile_step; }
+    };
+    if (leader && p.has_res)
+      for (int i = 0; i < PF; ++i) issue_res();
+
+    uint32_t j = 0;                                // chunk counter of this group
+    uint32_t seq = g;                              // this CTA's tile sequence number
+    for (int tile = blockIdx.x + g * gridDim.x; tile < p.num_tiles; tile += tile_step, seq += EG) {
+      const int acc = seq & 1;
+      const uint32_t acc_phase = (seq >> 1) & 1u;
       const int n_idx = tile % p.n_tiles, m_idx = tile / p.n_tiles;
       const int t0 = (m_idx % p.t_blks) * p.T_box, b0 = (m_idx / p.t_blks) * p.B_box, n0 = n_idx * BN;
       mbar_wait(tfull_bar(acc), acc_phase);
       tc_fence_after();
+      float head_acc = 0.f;
 #pragma unroll 1
-      for (int c = 0; c < BN / 64; ++c, ++chunk_ctr) {
-        const int buf = chunk_ctr & 1u;
-        const uint32_t sbuf = out_base + buf * Cfg::OUT_BYTES;
+      for (int c = 0; c < CH; ++c, ++j) {
+        const int buf = j % NBUF;
+        const uint32_t sbuf = gbuf + buf * TC_OUT_BYTES;
         if (leader) {
-          tma_store_wait_read<1>();                // the store that last used this buffer has read it
           if (p.has_res) {
-            mbar_arrive_expect_tx(res_bar(buf), Cfg::OUT_BYTES);
-            tma_load_4d(sbuf, &tm_res, res_bar(buf), n0 + c * 64, 0, t0, b0);
+            if (!HEAD) tma_store_wait_read_n(NBUF - PF - 1);   // buffer of chunk j + PF is free again
+            issue_res();
+          } else if (!HEAD) {
+            tma_store_wait_read_n(NBUF - 1);                   // buffer of this chunk is free again
           }
         }
-        named_bar_sync(1, 128);
+        named_bar_sync(1 + g, 128);
         uint32_t v[64];
         const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256 + c * 64);
         tmem_ld32(taddr, v);
         tmem_ld32(taddr + 32, v + 32);
         tmem_ld_wait();
-        if (c == BN / 64 - 1) {                    // accumulator drained: hand it back to the MMA warp
+        if (c == CH - 1) {                         // accumulator drained: hand it back to the MMA warp
           tc_fence_before();
           mbar_arrive(tempty_bar(acc));
         }
-        if (p.has_res) mbar_wait(res_bar(buf), (chunk_ctr >> 1) & 1u);
-        const float4* bias4 = reinterpret_cast<const float4*>(p.bias + n0 + c * 64);
+        if (p.has_res) mbar_wait(res_bar(g, buf), (j / NBUF) & 1u);
+        const float4* bias4 = reinterpret_cast<const float4*>(s_bias + n0 + c * 64);
+        const float4* hw4 = reinterpret_cast<const float4*>(s_headw + n0 + c * 64);
         unsigned char* rowp = gen_base + (sbuf - base) + row * 128;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {              // 8 pieces of 8 channels (16 B of bf16)
-          const float4 bA = __ldg(bias4 + 2 * j), bB = __ldg(bias4 + 2 * j + 1);
+        for (int jj = 0; jj < 8; ++jj) {           // 8 pieces of 8 channels (16 B of bf16)
+          const float4 bA = bias4[2 * jj], bB = bias4[2 * jj + 1];
           float f[8];
-          f[0] = __uint_as_float(v[8 * j + 0]) + bA.x; f[1] = __uint_as_float(v[8 * j + 1]) + bA.y;
-          f[2] = __uint_as_float(v[8 * j + 2]) + bA.z; f[3] = __uint_as_float(v[8 * j + 3]) + bA.w;
-          f[4] = __uint_as_float(v[8 * j + 4]) + bB.x; f[5] = __uint_as_float(v[8 * j + 5]) + bB.y;
-          f[6] = __uint_as_float(v[8 * j + 6]) + bB.z; f[7] = __uint_as_float(v[8 * j + 7]) + bB.w;
-          uint4* sp = reinterpret_cast<uint4*>(rowp + ((j ^ (row & 7)) << 4));   // 128B-swizzle position
+          f[0] = __uint_as_float(v[8 * jj + 0]) + bA.x; f[1] = __uint_as_float(v[8 * jj + 1]) + bA.y;
+          f[2] = __uint_as_float(v[8 * jj + 2]) + bA.z; f[3] = __uint_as_float(v[8 * jj + 3]) + bA.w;
+          f[4] = __uint_as_float(v[8 * jj + 4]) + bB.x; f[5] = __uint_as_float(v[8 * jj + 5]) + bB.y;
+          f[6] = __uint_as_float(v[8 * jj + 6]) + bB.z; f[7] = __uint_as_float(v[8 * jj + 7]) + bB.w;
+          uint4* sp = reinterpret_cast<uint4*>(rowp + ((jj ^ (row & 7)) << 4));   // 128B-swizzle position
           if (p.has_res) {
             const uint4 r = *sp;
             const __nv_bfloat162* rb = reinterpret_cast<const __nv_bfloat162*>(&r);
@@ -184,18 +245,41 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
           __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(&o);
 #pragma unroll
           for (int e = 0; e < 4; ++e) ob[e] = __floats2bfloat162_rn(f[2 * e], f[2 * e + 1]);
-          *sp = o;
+          if (HEAD) {
+            const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
+            const float2 o0 = __bfloat1622float2(ob[0]), o1 = __bfloat1622float2(ob[1]);
+            const float2 o2 = __bfloat1622float2(ob[2]), o3 = __bfloat1622float2(ob[3]);
+            head_acc = fmaf(o0.x, hA.x, head_acc); head_acc = fmaf(o0.y, hA.y, head_acc);
+            head_acc = fmaf(o1.x, hA.z, head_acc); head_acc = fmaf(o1.y, hA.w, head_acc);
+            head_acc = fmaf(o2.x, hB.x, head_acc); head_acc = fmaf(o2.y, hB.y, head_acc);
+            head_acc = fmaf(o3.x, hB.z, head_acc); head_acc = fmaf(o3.y, hB.w, head_acc);
+          } else {
+            *sp = o;
+          }
         }
-        fence_proxy_async_smem();                  // generic-proxy writes -> visible to the TMA store
-        named_bar_sync(1, 128);
-        if (leader) {
-          tma_store_4d(&tm_out, sbuf, n0 + c * 64, 0, t0, b0);
-          tma_store_commit();
+        if (HEAD) {
+          // the warp's 32 rows are one 32-row slab of one window (T_box % 32 == 0): reduce and emit a partial
+          float s = head_acc;
+          head_acc = 0.f;
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+          const int r0 = q * 32;
+          const int64_t b = b0 + r0 / p.T_box;
+          const int slab = (t0 + r0 % p.T_box) >> 5;
+          if (lane == 0 && b < p.nb)
+            p.head_part[(b * p.head_slabs + slab) * (p.c_out >> 6) + n_idx * CH + c] = s;
+          named_bar_sync(1 + g, 128);              // residual buffer fully read before it is refilled
+        } else {
+          fence_proxy_async_smem();                // generic-proxy writes -> visible to the TMA store
+          named_bar_sync(1 + g, 128);
+          if (leader) {
+            tma_store_4d(&tm_out, sbuf, n0 + c * 64, 0, t0, b0);
+            tma_store_commit();
+          }
         }
       }
-      if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
     }
-    if (leader) tma_store_wait_all<0>();
+    if (leader && !HEAD) tma_store_wait_all<0>();
   }
   tc_fence_before();
   __syncthreads();

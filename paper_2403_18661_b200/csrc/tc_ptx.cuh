@@ -115,3 +115,13 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
+
+// cp.async.bulk.wait_group.read takes an immediate: dispatch the small run-time values the kernels use.
+__device__ __forceinline__ void tma_store_wait_read_n(int n) {
+  switch (n) {
+    case 0: tma_store_wait_read<0>(); break;
+    case 1: tma_store_wait_read<1>(); break;
+    case 2: tma_store_wait_read<2>(); break;
+    default: tma_store_wait_read<3>(); break;
+  }
+}
