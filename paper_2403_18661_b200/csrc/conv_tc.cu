@@ -32,7 +32,7 @@ struct TcLaunch {
   CUtensorMap tm_in, tm_w, tm_out, tm_res;
   TcConvParams p;
   int BN, grid, smem;
-  bool head;
+  bool head, cg2;
 };
 
 // score[b] = (sum of the fused-head partials of window b) / T + bias   (deterministic: fixed summation order)
@@ -94,6 +94,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
                          TcLaunch& L) {
   const LayerDesc& l = w->layers[li];
   const int BN = l.c_out >= 256 ? 256 : l.c_out;
+  const bool cg2 = BN == 256 && env_int("AFRAME_CG2", 1) != 0;   // CTA pairs (cta_group::2) for the N = 256 layers
   const int T_box = tile_t_box(l.t_out), B_box = 128 / T_box;
   const int P = l.stride;
   {
@@ -105,7 +106,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   {
     const uint64_t dims[3] = {(uint64_t)l.c_in, (uint64_t)l.c_out, (uint64_t)l.k};
     const uint64_t str[2] = {(uint64_t)l.c_in * 2, (uint64_t)l.c_out * l.c_in * 2};
-    const uint32_t box[3] = {64, (uint32_t)BN, 1};
+    const uint32_t box[3] = {64, (uint32_t)(cg2 ? BN / 2 : BN), 1};
     if (!encode_map(ctx, &L.tm_w, w->d_w16[li], 3, dims, str, box)) return false;
   }
   {
@@ -123,7 +124,8 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.T_box = T_box; p.B_box = B_box;
   p.t_blks = l.t_out / T_box;
   const int64_t b_blks = (nb + B_box - 1) / B_box;
-  p.num_tiles = (int)(b_blks * p.t_blks * p.n_tiles);
+  const int64_t m_tiles = b_blks * p.t_blks;
+  p.num_tiles = (int)((cg2 ? (m_tiles + 1) / 2 : m_tiles) * p.n_tiles);
   p.relu = l.relu; p.has_res = res != nullptr;
   p.c_out = l.c_out;
   p.head_w = head ? w->d_head_w : nullptr;
@@ -131,31 +133,45 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.head_slabs = l.t_out / 32;
   p.nb = nb;
   // shared-memory plan (227 KB per CTA): main-loop ring depth vs epilogue staging / residual prefetch buffers
-  if (BN == 256)      { p.stages = p.has_res ? 3 : 4; p.nbuf = p.has_res ? 4 : 2; p.pf = p.has_res ? 2 : 0; }
+  if (cg2)            { p.stages = p.has_res ? 5 : 6; p.nbuf = p.has_res ? (head ? 3 : 4) : 2; p.pf = p.has_res ? 2 : 0; }
+  else if (BN == 256) { p.stages = p.has_res ? 3 : 4; p.nbuf = p.has_res ? 4 : 2; p.pf = p.has_res ? 2 : 0; }
   else if (BN == 128) { p.stages = p.has_res ? 3 : 4; p.nbuf = p.has_res ? 3 : 2; p.pf = p.has_res ? 1 : 0; }
   else                { p.stages = 5;                 p.nbuf = 3;                 p.pf = p.has_res ? 1 : 0; }
   L.BN = BN;
   L.head = head;
-  L.smem = BN == 256 ? TcCfg<256>::smem(p.stages, p.nbuf, head) : (BN == 128 ? TcCfg<128>::smem(p.stages, p.nbuf, head)
+  L.cg2 = cg2;
+  L.smem = cg2 ? TcCfg<256, true>::smem(p.stages, p.nbuf, head) : BN == 256 ? TcCfg<256>::smem(p.stages, p.nbuf, head) : (BN == 128 ? TcCfg<128>::smem(p.stages, p.nbuf, head)
                                                                             : TcCfg<64>::smem(p.stages, p.nbuf, head));
-  L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
+  if (cg2) L.grid = 2 * (p.num_tiles < ctx->n_sms / 2 ? p.num_tiles : ctx->n_sms / 2);
+  else L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
   return true;
 }
 
-template <int BN, bool HEAD> static cudaError_t launch_bn(const TcLaunch& L, cudaStream_t s) {
+template <int BN, bool HEAD, bool CG2> static cudaError_t launch_bn(const TcLaunch& L, cudaStream_t s) {
   static bool attr = false;
+  auto kern = conv_tc_kernel<BN, HEAD, CG2>;
   if (!attr) {
-    cudaError_t e = cudaFuncSetAttribute(conv_tc_kernel<BN, HEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448);
     if (e != cudaSuccess) return e;
     attr = true;
   }
-  conv_tc_kernel<BN, HEAD><<<L.grid, TcCfg<BN>::THREADS, L.smem, s>>>(L.tm_in, L.tm_w, L.tm_out, L.tm_res, L.p);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)L.grid);
+  cfg.blockDim = dim3((unsigned)TcCfg<BN, CG2>::THREADS);
+  cfg.dynamicSmemBytes = (size_t)L.smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = CG2 ? 2 : 1; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, L.tm_in, L.tm_w, L.tm_out, L.tm_res, L.p);
 }
 
 static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s) {
-  if (L.head) return launch_bn<256, true>(L, s);
-  return L.BN == 256 ? launch_bn<256, false>(L, s) : (L.BN == 128 ? launch_bn<128, false>(L, s) : launch_bn<64, false>(L, s));
+  if (L.cg2) return L.head ? launch_bn<256, true, true>(L, s) : launch_bn<256, false, true>(L, s);
+  if (L.head) return launch_bn<256, true, false>(L, s);
+  return L.BN == 256 ? launch_bn<256, false, false>(L, s)
+                     : (L.BN == 128 ? launch_bn<128, false, false>(L, s) : launch_bn<64, false, false>(L, s));
 }
 
 struct TcPlanCache {

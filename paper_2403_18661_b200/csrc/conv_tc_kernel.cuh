@@ -45,9 +45,10 @@ struct TcConvParams {
 #define TC_OUT_BYTES (128 * 128)    // one 64-channel chunk of the output tile
 __host__ __device__ constexpr int tc_fixed_bytes(bool head) { return head ? 5120 : 3072; }
 
-template <int BN> struct TcCfg {
+template <int BN, bool CG2 = false> struct TcCfg {
   static constexpr int A_BYTES = 128 * 128;
-  static constexpr int B_BYTES = BN * 128;
+  static constexpr int B_ROWS = CG2 ? BN / 2 : BN;   // CTA pair: each CTA stages half of the B tile
+  static constexpr int B_BYTES = B_ROWS * 128;
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
   static constexpr int EG = (BN == 256) ? 1 : 2;
   static constexpr int THREADS = 64 + 128 * EG;
@@ -58,13 +59,17 @@ template <int BN> struct TcCfg {
 
 __device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 
-template <int BN, bool HEAD>
-__global__ void __launch_bounds__(TcCfg<BN>::THREADS, 1)
+template <int BN, bool HEAD, bool CG2>
+__global__ void __launch_bounds__(TcCfg<BN, CG2>::THREADS, 1)
 conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_w,
                const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_res,
                const TcConvParams p) {
-  using Cfg = TcCfg<BN>;
+  using Cfg = TcCfg<BN, CG2>;
   constexpr int EG = Cfg::EG;
+  // CTA pair (CG2): cluster of 2 CTAs = one M = 256 tile (rows [0,128) in the leader, [128,256) in its peer).
+  const uint32_t rank = CG2 ? cluster_ctarank() : 0u;
+  const int n_workers = CG2 ? (int)(gridDim.x >> 1) : (int)gridDim.x;   // tile loops step by this
+  const int worker = CG2 ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
   constexpr int MAXBUF = 4;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const uint32_t base = smem_u32(smem_raw);
@@ -90,18 +95,19 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
     if (!HEAD) tma_prefetch_desc(&tm_out);
     if (p.has_res) tma_prefetch_desc(&tm_res);
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 128); }
+    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), CG2 ? 8 : 4); }   // one arrival per epilogue warp
     for (int g = 0; g < EG; ++g)
       for (int b = 0; b < MAXBUF; ++b) mbar_init(res_bar(g, b), 1);
     fence_mbar_init();
   }
-  if (warp == 1) tmem_alloc(tmem_slot, 512);
+  if (warp == 1) { if (CG2) tmem_alloc_cg2(tmem_slot, 512); else tmem_alloc(tmem_slot, 512); }
   for (int i = threadIdx.x; i < p.c_out; i += blockDim.x) {
     s_bias[i] = p.bias[i];
     if (HEAD) s_headw[i] = p.head_w[i];
   }
   tc_fence_before();
   __syncthreads();
+  if (CG2) cluster_sync_all();                     // the peer's barriers exist before any remote arrive / complete_tx
   tc_fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(gen_base + (tmem_slot - base));
 
@@ -111,8 +117,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
     // ===== TMA producer =====
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      for (int tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
-        const int n_idx = tile % p.n_tiles, m_idx = tile / p.n_tiles;
+      for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
+        const int n_idx = tile % p.n_tiles, m_idx = (tile / p.n_tiles) * (CG2 ? 2 : 1) + (int)rank;
         const int t0 = (m_idx % p.t_blks) * p.T_box, b0 = (m_idx / p.t_blks) * p.B_box, n0 = n_idx * BN;
         for (int d = 0; d < p.taps; ++d) {
           const int sft = d - p.pad;
@@ -120,10 +126,18 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
           const int par = sft - toff * p.P;
           for (int kb = 0; kb < p.kblocks; ++kb) {
             mbar_wait(empty_bar(stage), phase ^ 1u);
-            mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
             const uint32_t sa = stage_base + stage * Cfg::STAGE_BYTES;
-            tma_load_4d(sa, &tm_in, full_bar(stage), kb * 64, par, t0 + toff, b0);
-            tma_load_3d(sa + Cfg::A_BYTES, &tm_w, full_bar(stage), kb * 64, n0, d);
+            if (CG2) {
+              // both CTAs load their own A rows and their half of B; all bytes are counted on the leader's barrier
+              if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * Cfg::STAGE_BYTES);
+              const uint32_t lbar = mapa_cluster(full_bar(stage), 0);
+              tma_load_4d_cg2(sa, &tm_in, lbar, kb * 64, par, t0 + toff, b0);
+              tma_load_3d_cg2(sa + Cfg::A_BYTES, &tm_w, lbar, kb * 64, n0 + (int)rank * Cfg::B_ROWS, d);
+            } else {
+              mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
+              tma_load_4d(sa, &tm_in, full_bar(stage), kb * 64, par, t0 + toff, b0);
+              tma_load_3d(sa + Cfg::A_BYTES, &tm_w, full_bar(stage), kb * 64, n0, d);
+            }
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
           }
         }
@@ -131,11 +145,11 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
     }
   } else if (warp == 1) {
     // ===== MMA issuer (one thread) =====
-    if (lane == 0) {
-      constexpr uint32_t idesc = umma_idesc_bf16(BN);
+    if (lane == 0 && rank == 0) {
+      constexpr uint32_t idesc = umma_idesc_bf16_mn(CG2 ? 256 : 128, BN);
       int stage = 0; uint32_t phase = 0;
       int acc = 0; uint32_t acc_phase = 0;
-      for (int tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+      for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(acc * 256);
@@ -145,12 +159,16 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
           const uint32_t sa = stage_base + stage * Cfg::STAGE_BYTES;
           const uint64_t da = umma_desc_sw128(sa), db = umma_desc_sw128(sa + Cfg::A_BYTES);
 #pragma unroll
-          for (int k = 0; k < 4; ++k)   // 4 x (K = 16 bf16 = 32 B) inside the 128-byte swizzle row
-            umma_bf16(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
-          umma_commit(empty_bar(stage));           // frees the smem slot when these MMAs retire
+          for (int k = 0; k < 4; ++k) { // 4 x (K = 16 bf16 = 32 B) inside the 128-byte swizzle row
+            if (CG2) umma_bf16_cg2(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
+            else umma_bf16(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
+          }
+          if (CG2) umma_commit_cg2(empty_bar(stage), 3);   // frees the smem slot in BOTH CTAs when these MMAs retire
+          else umma_commit(empty_bar(stage));
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
-        umma_commit(tfull_bar(acc));               // accumulator complete -> epilogue
+        if (CG2) umma_commit_cg2(tfull_bar(acc), 3);   // accumulator complete -> both CTAs' epilogues
+        else umma_commit(tfull_bar(acc));
         if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
       }
     }
@@ -164,14 +182,15 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
     const int NBUF = p.nbuf, PF = p.pf;
     const uint32_t gbuf = out_base + (uint32_t)(g * NBUF) * TC_OUT_BYTES;
     constexpr int CH = BN / 64;
-    const int tile_step = EG * gridDim.x;
+    const int tile_step = EG * n_workers;
+    const uint32_t tempty_leader0 = CG2 ? mapa_cluster(tempty_bar(0), 0) : tempty_bar(0);
 
     // residual prefetch cursor (leader only): chunk pf_j of this group's chunk sequence
-    int pf_tile = blockIdx.x + g * gridDim.x, pf_c = 0;
+    int pf_tile = worker + g * n_workers, pf_c = 0;
     uint32_t pf_j = 0;
     auto issue_res = [&]() {
       if (pf_tile < p.num_tiles) {
-        const int n_idx = pf_tile % p.n_tiles, m_idx = pf_tile / p.n_tiles;
+        const int n_idx = pf_tile % p.n_tiles, m_idx = (pf_tile / p.n_tiles) * (CG2 ? 2 : 1) + (int)rank;
         const int t0 = (m_idx % p.t_blks) * p.T_box, b0 = (m_idx / p.t_blks) * p.B_box, n0 = n_idx * BN;
         const int buf = pf_j % NBUF;
         mbar_arrive_expect_tx(res_bar(g, buf), TC_OUT_BYTES);
@@ -185,10 +204,10 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
 
     uint32_t j = 0;                                // chunk counter of this group
     uint32_t seq = g;                              // this CTA's tile sequence number
-    for (int tile = blockIdx.x + g * gridDim.x; tile < p.num_tiles; tile += tile_step, seq += EG) {
+    for (int tile = worker + g * n_workers; tile < p.num_tiles; tile += tile_step, seq += EG) {
       const int acc = seq & 1;
       const uint32_t acc_phase = (seq >> 1) & 1u;
-      const int n_idx = tile % p.n_tiles, m_idx = tile / p.n_tiles;
+      const int n_idx = tile % p.n_tiles, m_idx = (tile / p.n_tiles) * (CG2 ? 2 : 1) + (int)rank;
       const int t0 = (m_idx % p.t_blks) * p.T_box, b0 = (m_idx / p.t_blks) * p.B_box, n0 = n_idx * BN;
       mbar_wait(tfull_bar(acc), acc_phase);
       tc_fence_after();
@@ -211,9 +230,13 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
         tmem_ld32(taddr, v);
         tmem_ld32(taddr + 32, v + 32);
         tmem_ld_wait();
-        if (c == CH - 1) {                         // accumulator drained: hand it back to the MMA warp
+        if (c == CH - 1) {                         // accumulator drained: hand it back to the (leader's) MMA warp
           tc_fence_before();
-          mbar_arrive(tempty_bar(acc));
+          __syncwarp();
+          if (lane == 0) {
+            if (CG2) mbar_arrive_cluster(tempty_leader0 + 8u * acc);
+            else mbar_arrive(tempty_bar(acc));
+          }
         }
         if (p.has_res) mbar_wait(res_bar(g, buf), (j / NBUF) & 1u);
         const float4* bias4 = reinterpret_cast<const float4*>(s_bias + n0 + c * 64);
@@ -283,5 +306,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem_base, 512); }
+  if (CG2) cluster_sync_all();                     // the peer has drained its half of the accumulators
+  if (warp == 1) {
+    tc_fence_after();
+    if (CG2) tmem_dealloc_cg2(tmem_base, 512); else tmem_dealloc(tmem_base, 512);
+  }
 }
