@@ -185,6 +185,11 @@ enum {
   AFRAME_PROF_KINDS = 8
 };
 aframe_status aframe_profile(aframe_ctx* ctx, int enable);
+/* One forward pass of aframe_forward on d_windows [B][C][kernel_len] with a CUDA-event pair around every layer's
+ * launch (bf16 path; B at most one internal chunk).  h_ms: HOST array of n_layers floats (layer-table order; the stem's
+ * conv + max-pool are reported on entry 0, the head on the last entry).  Synchronises. */
+aframe_status aframe_profile_layers(aframe_ctx* ctx, const aframe_weights* w, const float* d_windows, int64_t B,
+                                    float* d_scores, float* h_ms, int32_t n_layers);
 aframe_status aframe_profile_read(aframe_ctx* ctx, double* h_ms, int64_t* h_launches);
 
 #ifdef __cplusplus

@@ -59,6 +59,7 @@ EXPORTS = {
     "aframe_score_timeslides_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64,
                                                C.c_int64, C.POINTER(C.c_int64), C.c_int32, C.c_int64, C.c_void_p]),
     "aframe_profile": (C.c_int, [C.c_void_p, C.c_int]),
+    "aframe_profile_layers": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.POINTER(C.c_float), C.c_int32]),
     "aframe_profile_read": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
 }
 PROF_KINDS = ("welch", "design", "whiten", "stem", "conv", "head", "stream", "reserved")
@@ -235,6 +236,14 @@ class Context:
     # ---- per-stage device timing
     def profile(self, enable: bool):
         self._check(self.lib.aframe_profile(self.handle, 1 if enable else 0))
+
+    def profile_layers(self, weights, windows, n_layers):
+        _need(windows, torch.float32, "windows")
+        scores = torch.empty((windows.shape[0],), dtype=torch.float32, device=windows.device)
+        ms = (C.c_float * n_layers)()
+        self._check(self.lib.aframe_profile_layers(self.handle, weights.handle, _ptr(windows), windows.shape[0], _ptr(scores),
+                                                   ms, n_layers))
+        return list(ms), scores
 
     def profile_read(self):
         ms = (C.c_double * 8)()

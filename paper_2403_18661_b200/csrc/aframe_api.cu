@@ -506,3 +506,16 @@ AF_API aframe_status aframe_score_timeslides_host(aframe_ctx* ctx, const aframe_
   AF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
   return AFRAME_OK;
 }
+
+AF_API aframe_status aframe_profile_layers(aframe_ctx* ctx, const aframe_weights* w, const float* d_windows, int64_t B,
+                                           float* d_scores, float* h_ms, int32_t n_layers) {
+  if (!ctx) return AFRAME_EINVAL;
+  if (!w || !d_windows || !d_scores || !h_ms) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
+  if (n_layers != (int32_t)w->layers.size()) return af_fail(ctx, AFRAME_ESHAPE, "n_layers does not match the layer table");
+  if (ctx->cfg.precision != AFRAME_BF16) return af_fail(ctx, AFRAME_EUNSUPPORTED, "per-layer timing is built for the bf16 path");
+  for (int i = 0; i < n_layers; ++i) h_ms[i] = 0.f;
+  ctx->layer_ms = h_ms;
+  aframe_status st = aframe_forward(ctx, w, d_windows, B, d_scores);
+  ctx->layer_ms = nullptr;
+  return st;
+}

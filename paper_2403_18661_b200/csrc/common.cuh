@@ -72,6 +72,7 @@ struct aframe_ctx {
   std::vector<ProfSpan> prof_spans;
   std::vector<cudaEvent_t> prof_pool;
   cudaEvent_t prof_open[AFRAME_PROF_KINDS] = {};
+  float* layer_ms = nullptr;   // aframe_profile_layers: per-layer device time of the next forward (host array), else null
 };
 
 // Stage timing: af_prof_begin records an event before the first launch of a stage, af_prof_end one after

@@ -119,6 +119,11 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   TcConvParams& p = L.p;
   p.bias = w->d_bias[li];
   p.taps = l.k; p.pad = l.pad; p.P = P;
+  for (int d = 0; d < 3; ++d) {
+    const int sft = d - l.pad;
+    const int toff = sft >= 0 ? sft / P : -((-sft + P - 1) / P);
+    p.tap_toff[d] = toff; p.tap_par[d] = sft - toff * P;
+  }
   p.kblocks = l.c_in / 64;
   p.n_tiles = l.c_out / BN;
   p.T_box = T_box; p.B_box = B_box;
@@ -126,17 +131,24 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   const int64_t b_blks = (nb + B_box - 1) / B_box;
   const int64_t m_tiles = b_blks * p.t_blks;
   p.num_tiles = (int)((cg2 ? (m_tiles + 1) / 2 : m_tiles) * p.n_tiles);
+  p.div_n = tc_fastdiv((uint32_t)p.n_tiles);
+  p.div_t = tc_fastdiv((uint32_t)p.t_blks);
   p.relu = l.relu; p.has_res = res != nullptr;
   p.c_out = l.c_out;
   p.head_w = head ? w->d_head_w : nullptr;
   p.head_part = head ? head_part : nullptr;
   p.head_slabs = l.t_out / 32;
   p.nb = nb;
+  p.dbg = env_int("AFRAME_TC_DBG", 0);
   // shared-memory plan (227 KB per CTA): main-loop ring depth vs epilogue staging / residual prefetch buffers
-  if (cg2)            { p.stages = p.has_res ? 5 : 6; p.nbuf = p.has_res ? (head ? 3 : 4) : 2; p.pf = p.has_res ? 2 : 0; }
-  else if (BN == 256) { p.stages = p.has_res ? 3 : 4; p.nbuf = p.has_res ? 4 : 2; p.pf = p.has_res ? 2 : 0; }
-  else if (BN == 128) { p.stages = p.has_res ? 3 : 4; p.nbuf = p.has_res ? 3 : 2; p.pf = p.has_res ? 1 : 0; }
-  else                { p.stages = 5;                 p.nbuf = 3;                 p.pf = p.has_res ? 1 : 0; }
+  // (two epilogue groups: EG * nbuf staging buffers of 16 KB)
+  if (cg2) {
+    if (head)           { p.stages = 4; p.nbuf = 2; p.pf = 1; }
+    else if (p.has_res) { p.stages = 4; p.nbuf = 3; p.pf = 1; }
+    else                { p.stages = 5; p.nbuf = 2; p.pf = 0; }
+  } else if (BN == 256) { p.stages = 3; p.nbuf = 2; p.pf = p.has_res ? 1 : 0; }
+  else if (BN == 128)   { p.stages = p.has_res ? 3 : 4; p.nbuf = p.has_res ? 3 : 2; p.pf = p.has_res ? 1 : 0; }
+  else                  { p.stages = 5;                 p.nbuf = 3;                 p.pf = p.has_res ? 1 : 0; }
   L.BN = BN;
   L.head = head;
   L.cg2 = cg2;
@@ -244,14 +256,22 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       }
     }
     const size_t esz = in_bf16 ? 2 : 4;
+    std::vector<cudaEvent_t> lev;
+    if (ctx->layer_ms) {
+      lev.resize(n + 1);
+      for (auto& e : lev) cudaEventCreate(&e);
+      cudaEventRecord(lev[0], ctx->stream);
+    }
     af_prof_begin(ctx, AFRAME_PROF_STEM);
     st = af_launch_stem_bf16(ctx, w->layers[0], w->layers[1], reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz,
                              in_bf16, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1));
     af_prof_end(ctx, AFRAME_PROF_STEM, 1);
     if (st != AFRAME_OK) return st;
     int n_conv = 0;
+    if (ctx->layer_ms) { cudaEventRecord(lev[1], ctx->stream); cudaEventRecord(lev[2], ctx->stream); }
     for (int i = 2; i < n; ++i) {
       const LayerDesc& l = w->layers[i];
+      struct Rec { aframe_ctx* c; std::vector<cudaEvent_t>& v; int i; ~Rec() { if (c->layer_ms) cudaEventRecord(v[i + 1], c->stream); } } rec{ctx, lev, i};
       if (l.kind == 0) {
         const TcLaunch& L = pc->launches[i];
         af_prof_begin(ctx, AFRAME_PROF_CONV);
@@ -274,6 +294,15 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         af_prof_end(ctx, AFRAME_PROF_HEAD, 1);
         if (st != AFRAME_OK) return st;
       }
+    }
+    if (ctx->layer_ms) {
+      cudaStreamSynchronize(ctx->stream);
+      for (int i = 0; i < n; ++i) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, lev[i], lev[i + 1]);
+        ctx->layer_ms[i] += ms;
+      }
+      for (auto& e : lev) cudaEventDestroy(e);
     }
   }
   return AFRAME_OK;

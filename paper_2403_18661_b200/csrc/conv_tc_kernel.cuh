@@ -20,8 +20,27 @@
 #include "tc_ptx.cuh"
 #include <cuda_bf16.h>
 
+// Division by a run-time constant without the ~200-cycle integer-divide sequence (the tile loops of the producer,
+// MMA and epilogue roles are single dependent instruction streams): q = (umulhi(x, mul) + x) >> shr, exact for
+// 0 <= x < 2^31 (Granlund-Montgomery round-up method; mul, shr computed on the host by tc_fastdiv).
+struct TcFastDiv {
+  uint32_t mul, shr, d;
+  __device__ __forceinline__ void divmod(int x, int& q, int& r) const {
+    q = (int)(((uint64_t)__umulhi((uint32_t)x, mul) + (uint32_t)x) >> shr);
+    r = x - q * (int)d;
+  }
+};
+static inline TcFastDiv tc_fastdiv(uint32_t d) {
+  TcFastDiv f; f.d = d; f.shr = 0;
+  while ((1ull << f.shr) < d) ++f.shr;
+  f.mul = (uint32_t)((((1ull << f.shr) - d) << 32) / d + 1);
+  return f;
+}
+
 struct TcConvParams {
   const float* bias;
+  TcFastDiv div_n, div_t;    // by n_tiles and by t_blks
+  int tap_toff[3], tap_par[3];   // per tap: row offset and parity plane of the strided input view
   int taps, pad, P;          // kernel taps, left padding, stride
   int kblocks;               // C_in / 64
   int n_tiles;               // C_out / BN
@@ -36,12 +55,13 @@ struct TcConvParams {
   float* head_part;
   int head_slabs;            // T_out / T_box
   int64_t nb;                // windows in this launch (head variant bounds check)
+  int dbg;                   // timing experiments only (wrong results): 1 = no TMA loads, 2 = epilogue drains TMEM only
 };
 
 // shared-memory carve-up (bytes from the 1024-aligned start of dynamic shared memory):
-//   [0, 256) mbarriers + TMEM base slot | [256, 2304) bias[c_out <= 512] | HEAD only: [3072, 5120) head_w
+//   [0, 512) mbarriers + TMEM base slot | [512, 2560) bias[c_out <= 512] | HEAD only: [3072, 5120) head_w
 //   then the main-loop ring (1024-aligned stages) and the epilogue staging buffers
-#define TC_BAR_BYTES 256
+#define TC_BAR_BYTES 512
 #define TC_OUT_BYTES (128 * 128)    // one 64-channel chunk of the output tile
 __host__ __device__ constexpr int tc_fixed_bytes(bool head) { return head ? 5120 : 3072; }
 
@@ -50,7 +70,10 @@ template <int BN, bool CG2 = false> struct TcCfg {
   static constexpr int B_ROWS = CG2 ? BN / 2 : BN;   // CTA pair: each CTA stages half of the B tile
   static constexpr int B_BYTES = B_ROWS * 128;
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int EG = (BN == 256) ? 1 : 2;
+  static constexpr int EG = 2;                       // epilogue groups of 4 warps
+  static constexpr bool SPLIT = (BN == 256);         // true: both groups drain every tile (alternate 64-column chunks);
+                                                     // false: the groups take alternate tiles
+  static constexpr int NACC = 512 / BN;              // TMEM accumulator stages (512 columns)
   static constexpr int THREADS = 64 + 128 * EG;
   static constexpr int smem(int stages, int nbuf, bool head) {
     return tc_fixed_bytes(head) + stages * STAGE_BYTES + EG * nbuf * TC_OUT_BYTES;
@@ -66,6 +89,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
                const TcConvParams p) {
   using Cfg = TcCfg<BN, CG2>;
   constexpr int EG = Cfg::EG;
+  constexpr bool SPLIT = Cfg::SPLIT;
+  constexpr int NACC = Cfg::NACC;
   // CTA pair (CG2): cluster of 2 CTAs = one M = 256 tile (rows [0,128) in the leader, [128,256) in its peer).
   const uint32_t rank = CG2 ? cluster_ctarank() : 0u;
   const int n_workers = CG2 ? (int)(gridDim.x >> 1) : (int)gridDim.x;   // tile loops step by this
@@ -76,13 +101,13 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
   if (base & 1023u) __trap();                      // SWIZZLE_128B tiles need 1024-byte alignment
   unsigned char* gen_base = smem_raw;
   const int STAGES = p.stages;
-  // barriers (8 B each): full[S], empty[S], tfull[2], tempty[2], res[EG][MAXBUF]; then the TMEM base slot
+  // barriers (8 B each): full[S], empty[S], tfull[NACC], tempty[NACC], res[EG][MAXBUF]; then the TMEM base slot
   auto full_bar = [&](int s) { return base + 8u * s; };
   auto empty_bar = [&](int s) { return base + 8u * (STAGES + s); };
   auto tfull_bar = [&](int a) { return base + 8u * (2 * STAGES + a); };
-  auto tempty_bar = [&](int a) { return base + 8u * (2 * STAGES + 2 + a); };
-  auto res_bar = [&](int g, int b) { return base + 8u * (2 * STAGES + 4 + g * MAXBUF + b); };
-  const uint32_t tmem_slot = base + 8u * (2 * STAGES + 4 + EG * MAXBUF);
+  auto tempty_bar = [&](int a) { return base + 8u * (2 * STAGES + NACC + a); };
+  auto res_bar = [&](int g, int b) { return base + 8u * (2 * STAGES + 2 * NACC + g * MAXBUF + b); };
+  const uint32_t tmem_slot = base + 8u * (2 * STAGES + 2 * NACC + EG * MAXBUF);
   float* s_bias = reinterpret_cast<float*>(gen_base + TC_BAR_BYTES);
   float* s_headw = reinterpret_cast<float*>(gen_base + 3072);
   const uint32_t stage_base = base + tc_fixed_bytes(HEAD);
@@ -95,7 +120,10 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
     if (!HEAD) tma_prefetch_desc(&tm_out);
     if (p.has_res) tma_prefetch_desc(&tm_res);
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), CG2 ? 8 : 4); }   // one arrival per epilogue warp
+    for (int a = 0; a < NACC; ++a) {               // tempty: one arrival per epilogue warp that drains the stage
+      mbar_init(tfull_bar(a), 1);
+      mbar_init(tempty_bar(a), (SPLIT ? 8 : 4) * (CG2 ? 2 : 1));
+    }
     for (int g = 0; g < EG; ++g)
       for (int b = 0; b < MAXBUF; ++b) mbar_init(res_bar(g, b), 1);
     fence_mbar_init();
@@ -112,22 +140,31 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(gen_base + (tmem_slot - base));
 
   const int kiters = p.taps * p.kblocks;
+  // tile -> (n0, t0, b0): n fastest, then the T_box-row block inside a window group, then the window group
+  auto decode = [&](int tile, int& n_idx, int& t0, int& b0) {
+    int mp, tb, bb;
+    p.div_n.divmod(tile, mp, n_idx);
+    const int m_idx = mp * (CG2 ? 2 : 1) + (int)rank;
+    p.div_t.divmod(m_idx, bb, tb);
+    t0 = tb * p.T_box; b0 = bb * p.B_box;
+  };
 
   if (warp == 0) {
     // ===== TMA producer =====
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
-        const int n_idx = tile % p.n_tiles, m_idx = (tile / p.n_tiles) * (CG2 ? 2 : 1) + (int)rank;
-        const int t0 = (m_idx % p.t_blks) * p.T_box, b0 = (m_idx / p.t_blks) * p.B_box, n0 = n_idx * BN;
+        int n_idx, t0, b0;
+        decode(tile, n_idx, t0, b0);
+        const int n0 = n_idx * BN;
         for (int d = 0; d < p.taps; ++d) {
-          const int sft = d - p.pad;
-          const int toff = floor_div(sft, p.P);
-          const int par = sft - toff * p.P;
+          const int toff = p.tap_toff[d], par = p.tap_par[d];
           for (int kb = 0; kb < p.kblocks; ++kb) {
             mbar_wait(empty_bar(stage), phase ^ 1u);
             const uint32_t sa = stage_base + stage * Cfg::STAGE_BYTES;
-            if (CG2) {
+            if (p.dbg & 1) {
+              if (rank == 0) mbar_arrive(full_bar(stage));
+            } else if (CG2) {
               // both CTAs load their own A rows and their half of B; all bytes are counted on the leader's barrier
               if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * Cfg::STAGE_BYTES);
               const uint32_t lbar = mapa_cluster(full_bar(stage), 0);
@@ -152,7 +189,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
         tc_fence_after();
-        const uint32_t d_tmem = tmem_base + (uint32_t)(acc * 256);
+        const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
         for (int it = 0; it < kiters; ++it) {
           mbar_wait(full_bar(stage), phase);
           tc_fence_after();
@@ -160,6 +197,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
           const uint64_t da = umma_desc_sw128(sa), db = umma_desc_sw128(sa + Cfg::A_BYTES);
 #pragma unroll
           for (int k = 0; k < 4; ++k) { // 4 x (K = 16 bf16 = 32 B) inside the 128-byte swizzle row
+            if (p.dbg & 8) continue;
             if (CG2) umma_bf16_cg2(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
             else umma_bf16(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
           }
@@ -169,7 +207,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
         }
         if (CG2) umma_commit_cg2(tfull_bar(acc), 3);   // accumulator complete -> both CTAs' epilogues
         else umma_commit(tfull_bar(acc));
-        if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+        if (++acc == NACC) { acc = 0; acc_phase ^= 1u; }
       }
     }
   } else {
@@ -182,38 +220,44 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
     const int NBUF = p.nbuf, PF = p.pf;
     const uint32_t gbuf = out_base + (uint32_t)(g * NBUF) * TC_OUT_BYTES;
     constexpr int CH = BN / 64;
-    const int tile_step = EG * n_workers;
+    const int tile_step = (SPLIT ? 1 : EG) * n_workers;     // this group's tiles ...
+    const int tile_first = worker + (SPLIT ? 0 : g) * n_workers;
+    constexpr int C_STEP = SPLIT ? 2 : 1;                   // ... and its chunks of each tile
+    const int c_first = SPLIT ? g : 0;
     const uint32_t tempty_leader0 = CG2 ? mapa_cluster(tempty_bar(0), 0) : tempty_bar(0);
 
     // residual prefetch cursor (leader only): chunk pf_j of this group's chunk sequence
-    int pf_tile = worker + g * n_workers, pf_c = 0;
+    int pf_tile = tile_first, pf_c = c_first;
     uint32_t pf_j = 0;
     auto issue_res = [&]() {
       if (pf_tile < p.num_tiles) {
-        const int n_idx = pf_tile % p.n_tiles, m_idx = (pf_tile / p.n_tiles) * (CG2 ? 2 : 1) + (int)rank;
-        const int t0 = (m_idx % p.t_blks) * p.T_box, b0 = (m_idx / p.t_blks) * p.B_box, n0 = n_idx * BN;
+        int n_idx, t0, b0;
+        decode(pf_tile, n_idx, t0, b0);
+        const int n0 = n_idx * BN;
         const int buf = pf_j % NBUF;
         mbar_arrive_expect_tx(res_bar(g, buf), TC_OUT_BYTES);
         tma_load_4d(gbuf + buf * TC_OUT_BYTES, &tm_res, res_bar(g, buf), n0 + pf_c * 64, 0, t0, b0);
       }
       ++pf_j;
-      if (++pf_c == CH) { pf_c = 0; pf_tile += tile_step; }
+      pf_c += C_STEP;
+      if (pf_c >= CH) { pf_c = c_first; pf_tile += tile_step; }
     };
     if (leader && p.has_res)
       for (int i = 0; i < PF; ++i) issue_res();
 
     uint32_t j = 0;                                // chunk counter of this group
-    uint32_t seq = g;                              // this CTA's tile sequence number
-    for (int tile = worker + g * n_workers; tile < p.num_tiles; tile += tile_step, seq += EG) {
-      const int acc = seq & 1;
-      const uint32_t acc_phase = (seq >> 1) & 1u;
-      const int n_idx = tile % p.n_tiles, m_idx = (tile / p.n_tiles) * (CG2 ? 2 : 1) + (int)rank;
-      const int t0 = (m_idx % p.t_blks) * p.T_box, b0 = (m_idx / p.t_blks) * p.B_box, n0 = n_idx * BN;
+    uint32_t seq = SPLIT ? 0 : g;                  // this CTA's tile sequence number
+    for (int tile = tile_first; tile < p.num_tiles; tile += tile_step, seq += (SPLIT ? 1 : EG)) {
+      const int acc = seq % NACC;
+      const uint32_t acc_phase = (seq / NACC) & 1u;
+      int n_idx, t0, b0;
+      decode(tile, n_idx, t0, b0);
+      const int n0 = n_idx * BN;
       mbar_wait(tfull_bar(acc), acc_phase);
       tc_fence_after();
       float head_acc = 0.f;
 #pragma unroll 1
-      for (int c = 0; c < CH; ++c, ++j) {
+      for (int c = c_first; c < CH; c += C_STEP, ++j) {
         const int buf = j % NBUF;
         const uint32_t sbuf = gbuf + buf * TC_OUT_BYTES;
         if (leader) {
@@ -226,11 +270,11 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
         }
         named_bar_sync(1 + g, 128);
         uint32_t v[64];
-        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * 256 + c * 64);
+        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN + c * 64);
         tmem_ld32(taddr, v);
         tmem_ld32(taddr + 32, v + 32);
         tmem_ld_wait();
-        if (c == CH - 1) {                         // accumulator drained: hand it back to the (leader's) MMA warp
+        if (c + C_STEP >= CH) {                    // this group's part of the accumulator is drained: hand it back to the (leader's) MMA warp
           tc_fence_before();
           __syncwarp();
           if (lane == 0) {
@@ -238,6 +282,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
             else mbar_arrive(tempty_bar(acc));
           }
         }
+        if (p.dbg & 2) { if (p.has_res) mbar_wait(res_bar(g, buf), (j / NBUF) & 1u); named_bar_sync(1 + g, 128); continue; }
         if (p.has_res) mbar_wait(res_bar(g, buf), (j / NBUF) & 1u);
         const float4* bias4 = reinterpret_cast<const float4*>(s_bias + n0 + c * 64);
         const float4* hw4 = reinterpret_cast<const float4*>(s_headw + n0 + c * 64);
@@ -260,14 +305,15 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
               f[2 * e] += rf.x; f[2 * e + 1] += rf.y;
             }
           }
-          if (p.relu) {
-#pragma unroll
-            for (int e = 0; e < 8; ++e) f[e] = fmaxf(f[e], 0.f);
-          }
           uint4 o;
           __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(&o);
 #pragma unroll
           for (int e = 0; e < 4; ++e) ob[e] = __floats2bfloat162_rn(f[2 * e], f[2 * e + 1]);
+          if (p.relu) {                            // ReLU commutes with the rounding: one packed max per channel pair
+            const __nv_bfloat162 z2 = __float2bfloat162_rn(0.f);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) ob[e] = __hmax2(ob[e], z2);
+          }
           if (HEAD) {
             const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
             const float2 o0 = __bfloat1622float2(ob[0]), o1 = __bfloat1622float2(ob[1]);
@@ -295,7 +341,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
         } else {
           fence_proxy_async_smem();                // generic-proxy writes -> visible to the TMA store
           named_bar_sync(1 + g, 128);
-          if (leader) {
+          if (leader && !(p.dbg & 4)) {
             tma_store_4d(&tm_out, sbuf, n0 + c * 64, 0, t0, b0);
             tma_store_commit();
           }
