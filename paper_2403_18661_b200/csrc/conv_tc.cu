@@ -32,7 +32,7 @@ struct TcLaunch {
   CUtensorMap tm_in, tm_w, tm_out, tm_res;
   TcConvParams p;
   int BN, grid, smem;
-  bool head, cg2;
+  bool head, cg2, halo;
 };
 
 // score[b] = (sum of the fused-head partials of window b) / T + bias   (deterministic: fixed summation order)
@@ -97,10 +97,14 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   const bool cg2 = BN == 256 && env_int("AFRAME_CG2", 1) != 0;   // CTA pairs (cta_group::2) for the N = 256 layers
   const int T_box = tile_t_box(l.t_out), B_box = 128 / T_box;
   const int P = l.stride;
+  const bool has_res = res != nullptr;
+  // resident weights + one halo box per tile (see TcConvParams): stride-1 k3 layers whose tiles stay inside a window
+  bool halo = !head && !cg2 && l.k == 3 && l.stride == 1 && l.pad == 1 && T_box == 128 && BN == l.c_out && BN <= 128 &&
+              env_int("AFRAME_HALO", 1) != 0;
   {
     const uint64_t dims[4] = {(uint64_t)l.c_in, (uint64_t)P, (uint64_t)(l.t_in / P), (uint64_t)nb};
     const uint64_t str[3] = {(uint64_t)l.c_in * 2, (uint64_t)P * l.c_in * 2, (uint64_t)l.t_in * l.c_in * 2};
-    const uint32_t box[4] = {64, 1, (uint32_t)T_box, (uint32_t)B_box};
+    const uint32_t box[4] = {64, 1, (uint32_t)(halo ? T_box + 2 : T_box), (uint32_t)B_box};
     if (!encode_map(ctx, &L.tm_in, in, 4, dims, str, box)) return false;
   }
   {
@@ -140,28 +144,41 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.head_slabs = l.t_out / 32;
   p.nb = nb;
   p.dbg = env_int("AFRAME_TC_DBG", 0);
+  p.dbg_out = nullptr;
+  if (env_int("AFRAME_TC_PROF", 0)) {       // experiment: per-role cycle counters, 32 slots per layer, read back by the caller
+    static long long* d_prof = nullptr;
+    if (!d_prof) { cudaMalloc(&d_prof, sizeof(long long) * 32 * 64); cudaMemset(d_prof, 0, sizeof(long long) * 32 * 64); }
+    p.dbg_out = d_prof + 32 * li;
+    if (const char* f = getenv("AFRAME_TC_PROF_PTR")) { FILE* fp = fopen(f, "w"); if (fp) { fprintf(fp, "%llu\n", (unsigned long long)(uintptr_t)d_prof); fclose(fp); } }
+  }
   // shared-memory plan (227 KB per CTA): main-loop ring depth vs epilogue staging / residual prefetch buffers
-  // (two epilogue groups: EG * nbuf staging buffers of 16 KB)
-  if (cg2) {
-    if (head)           { p.stages = 4; p.nbuf = 2; p.pf = 1; }
-    else if (p.has_res) { p.stages = 4; p.nbuf = 3; p.pf = 1; }
-    else                { p.stages = 5; p.nbuf = 2; p.pf = 0; }
-  } else if (BN == 256) { p.stages = 3; p.nbuf = 2; p.pf = p.has_res ? 1 : 0; }
-  else if (BN == 128)   { p.stages = p.has_res ? 3 : 4; p.nbuf = p.has_res ? 3 : 2; p.pf = p.has_res ? 1 : 0; }
-  else                  { p.stages = 5;                 p.nbuf = 3;                 p.pf = p.has_res ? 1 : 0; }
+  // (two epilogue groups: EG * nbuf staging buffers of 16 KB; a residual tile is prefetched pf chunks ahead into the
+  //  buffer its chunk's output is staged in)
+  const bool r = p.has_res;
+  if (cg2)                    { p.stages = r ? 4 : 5; p.nbuf = r ? (head ? 2 : 3) : 2; p.pf = r ? 1 : 0; }
+  else if (BN == 256)         { p.stages = 3; p.nbuf = 2; p.pf = r ? 1 : 0; }
+  else if (halo && BN == 128) { p.stages = 2; p.nbuf = 1; p.pf = 0; }
+  else if (halo)              { p.stages = r ? 6 : 8; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
+  else if (BN == 128)         { p.stages = r ? 4 : 5; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
+  else                        { p.stages = r ? 5 : 6; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
+  p.w_bytes = halo ? l.k * p.kblocks * BN * 128 : 0;
+  p.stage_bytes = halo ? p.kblocks * TcCfg<64>::HALO_A_BYTES : 0;
+  p.desc_base_offset = env_int("AFRAME_DESC_BO", 0);
   L.BN = BN;
   L.head = head;
   L.cg2 = cg2;
-  L.smem = cg2 ? TcCfg<256, true>::smem(p.stages, p.nbuf, head) : BN == 256 ? TcCfg<256>::smem(p.stages, p.nbuf, head) : (BN == 128 ? TcCfg<128>::smem(p.stages, p.nbuf, head)
+  L.halo = halo;
+  L.smem = halo ? (BN == 128 ? TcCfg<128>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks) : TcCfg<64>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks))
+         : cg2 ? TcCfg<256, true>::smem(p.stages, p.nbuf, head) : BN == 256 ? TcCfg<256>::smem(p.stages, p.nbuf, head) : (BN == 128 ? TcCfg<128>::smem(p.stages, p.nbuf, head)
                                                                             : TcCfg<64>::smem(p.stages, p.nbuf, head));
   if (cg2) L.grid = 2 * (p.num_tiles < ctx->n_sms / 2 ? p.num_tiles : ctx->n_sms / 2);
   else L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
   return true;
 }
 
-template <int BN, bool HEAD, bool CG2> static cudaError_t launch_bn(const TcLaunch& L, cudaStream_t s) {
+template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t launch_bn(const TcLaunch& L, cudaStream_t s) {
   static bool attr = false;
-  auto kern = conv_tc_kernel<BN, HEAD, CG2>;
+  auto kern = conv_tc_kernel<BN, HEAD, CG2, HALO>;
   if (!attr) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448);
     if (e != cudaSuccess) return e;
@@ -182,6 +199,7 @@ template <int BN, bool HEAD, bool CG2> static cudaError_t launch_bn(const TcLaun
 static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s) {
   if (L.cg2) return L.head ? launch_bn<256, true, true>(L, s) : launch_bn<256, false, true>(L, s);
   if (L.head) return launch_bn<256, true, false>(L, s);
+  if (L.halo) return L.BN == 128 ? launch_bn<128, false, false, true>(L, s) : launch_bn<64, false, false, true>(L, s);
   return L.BN == 256 ? launch_bn<256, false, false>(L, s)
                      : (L.BN == 128 ? launch_bn<128, false, false>(L, s) : launch_bn<64, false, false>(L, s));
 }

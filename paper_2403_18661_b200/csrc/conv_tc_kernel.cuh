@@ -55,6 +55,13 @@ struct TcConvParams {
   float* head_part;
   int head_slabs;            // T_out / T_box
   int64_t nb;                // windows in this launch (head variant bounds check)
+  // HALO variant (k = 3, stride 1, whole 128-row tiles inside one window): the folded weights of the layer stay resident
+  // in shared memory (w_bytes) and ONE (128 + 2)-row input box per 64-channel block serves all three taps: tap d reads
+  // the tile through a shared-memory descriptor whose start address is shifted by d rows (d * 128 B).
+  int w_bytes;               // resident weight region (0 unless HALO)
+  int stage_bytes;           // bytes per main-loop stage
+  int desc_base_offset;      // experiment: set the descriptor's base-offset field to the row shift (d & 7)
+  long long* dbg_out;        // timing experiments: per-role cycle counters of CTA 0 (null = off)
   int dbg;                   // timing experiments only (wrong results): 1 = no TMA loads, 2 = epilogue drains TMEM only
 };
 
@@ -78,13 +85,17 @@ template <int BN, bool CG2 = false> struct TcCfg {
   static constexpr int smem(int stages, int nbuf, bool head) {
     return tc_fixed_bytes(head) + stages * STAGE_BYTES + EG * nbuf * TC_OUT_BYTES;
   }
+  static constexpr int HALO_A_BYTES = 17 * 1024;     // 130 rows x 128 B, padded to the 1024-byte swizzle period
+  static constexpr int smem_halo(int stages, int nbuf, int taps, int kblocks) {
+    return tc_fixed_bytes(false) + taps * kblocks * BN * 128 + stages * kblocks * HALO_A_BYTES + EG * nbuf * TC_OUT_BYTES;
+  }
 };
 
 __device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 
-template <int BN, bool HEAD, bool CG2>
+template <int BN, bool HEAD, bool CG2, bool HALO>
 __global__ void __launch_bounds__(TcCfg<BN, CG2>::THREADS, 1)
-conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_w,
+conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 rows */, const __grid_constant__ CUtensorMap tm_w,
                const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_res,
                const TcConvParams p) {
   using Cfg = TcCfg<BN, CG2>;
@@ -95,37 +106,42 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
   const uint32_t rank = CG2 ? cluster_ctarank() : 0u;
   const int n_workers = CG2 ? (int)(gridDim.x >> 1) : (int)gridDim.x;   // tile loops step by this
   const int worker = CG2 ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
-  constexpr int MAXBUF = 4;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const uint32_t base = smem_u32(smem_raw);
   if (base & 1023u) __trap();                      // SWIZZLE_128B tiles need 1024-byte alignment
   unsigned char* gen_base = smem_raw;
   const int STAGES = p.stages;
-  // barriers (8 B each): full[S], empty[S], tfull[NACC], tempty[NACC], res[EG][MAXBUF]; then the TMEM base slot
+  // barriers (8 B each): full[S], empty[S], tfull[NACC], tempty[NACC], res[EG][MAXBUF], w_bar; then the TMEM base slot
   auto full_bar = [&](int s) { return base + 8u * s; };
   auto empty_bar = [&](int s) { return base + 8u * (STAGES + s); };
   auto tfull_bar = [&](int a) { return base + 8u * (2 * STAGES + a); };
   auto tempty_bar = [&](int a) { return base + 8u * (2 * STAGES + NACC + a); };
+  constexpr int MAXBUF = 4;
   auto res_bar = [&](int g, int b) { return base + 8u * (2 * STAGES + 2 * NACC + g * MAXBUF + b); };
-  const uint32_t tmem_slot = base + 8u * (2 * STAGES + 2 * NACC + EG * MAXBUF);
+  const uint32_t w_bar = base + 8u * (2 * STAGES + 2 * NACC + EG * MAXBUF);
+  const uint32_t tmem_slot = w_bar + 8u;
   float* s_bias = reinterpret_cast<float*>(gen_base + TC_BAR_BYTES);
   float* s_headw = reinterpret_cast<float*>(gen_base + 3072);
-  const uint32_t stage_base = base + tc_fixed_bytes(HEAD);
-  const uint32_t out_base = stage_base + STAGES * Cfg::STAGE_BYTES;
+  static_assert(!HALO || (!CG2 && !HEAD), "HALO is a single-CTA, storing variant");
+  const uint32_t w_base = base + tc_fixed_bytes(HEAD);           // HALO: resident weights [tap][kblock][BN rows][128 B]
+  const uint32_t stage_base = w_base + (HALO ? p.w_bytes : 0);
+  const int STAGE_BYTES = HALO ? p.stage_bytes : Cfg::STAGE_BYTES;
+  const uint32_t out_base = stage_base + STAGES * STAGE_BYTES;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tm_in); tma_prefetch_desc(&tm_w);
     if (!HEAD) tma_prefetch_desc(&tm_out);
-    if (p.has_res) tma_prefetch_desc(&tm_res);
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     for (int a = 0; a < NACC; ++a) {               // tempty: one arrival per epilogue warp that drains the stage
       mbar_init(tfull_bar(a), 1);
       mbar_init(tempty_bar(a), (SPLIT ? 8 : 4) * (CG2 ? 2 : 1));
     }
+    mbar_init(w_bar, 1);
     for (int g = 0; g < EG; ++g)
       for (int b = 0; b < MAXBUF; ++b) mbar_init(res_bar(g, b), 1);
+    if (p.has_res) tma_prefetch_desc(&tm_res);
     fence_mbar_init();
   }
   if (warp == 1) { if (CG2) tmem_alloc_cg2(tmem_slot, 512); else tmem_alloc(tmem_slot, 512); }
@@ -140,6 +156,11 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(gen_base + (tmem_slot - base));
 
   const int kiters = p.taps * p.kblocks;
+  // cycle accounting for experiments (CTA 0 only): T(slot) adds the cycles since the previous T() of this thread
+  const bool prof = p.dbg_out != nullptr && blockIdx.x == 0;
+  long long tprev = prof ? clock64() : 0, tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  auto T = [&](int slot) { if (prof) { const long long t = clock64(); tacc[slot] += t - tprev; tprev = t; } };
+  auto Tflush = [&](int role) { if (prof) for (int i = 0; i < 8; ++i) p.dbg_out[role * 8 + i] = tacc[i]; };
   // tile -> (n0, t0, b0): n fastest, then the T_box-row block inside a window group, then the window group
   auto decode = [&](int tile, int& n_idx, int& t0, int& b0) {
     int mp, tb, bb;
@@ -151,7 +172,28 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
 
   if (warp == 0) {
     // ===== TMA producer =====
-    if (lane == 0) {
+    if (lane == 0 && HALO) {
+      // resident weights, once per CTA (n_tiles == 1: BN == C_out)
+      mbar_arrive_expect_tx(w_bar, (uint32_t)p.w_bytes);
+      for (int d = 0; d < p.taps; ++d)
+        for (int kb = 0; kb < p.kblocks; ++kb)
+          tma_load_3d(w_base + (uint32_t)((d * p.kblocks + kb) * BN * 128), &tm_w, w_bar, kb * 64, 0, d);
+      int stage = 0; uint32_t phase = 0;
+      for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
+        int n_idx, t0, b0;
+        decode(tile, n_idx, t0, b0);
+        T(0);
+        mbar_wait(empty_bar(stage), phase ^ 1u);
+        T(1);
+        mbar_arrive_expect_tx(full_bar(stage), (uint32_t)(p.kblocks * 130 * 128));
+        const uint32_t sa = stage_base + stage * STAGE_BYTES;
+        for (int kb = 0; kb < p.kblocks; ++kb)     // rows t0 - 1 .. t0 + 128 of the window; out-of-range rows are zero-filled
+          tma_load_4d(sa + kb * Cfg::HALO_A_BYTES, &tm_in, full_bar(stage), kb * 64, 0, t0 - 1, b0);
+        if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        T(2);
+      }
+      Tflush(0);
+    } else if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         int n_idx, t0, b0;
@@ -160,8 +202,10 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
         for (int d = 0; d < p.taps; ++d) {
           const int toff = p.tap_toff[d], par = p.tap_par[d];
           for (int kb = 0; kb < p.kblocks; ++kb) {
+            T(0);
             mbar_wait(empty_bar(stage), phase ^ 1u);
-            const uint32_t sa = stage_base + stage * Cfg::STAGE_BYTES;
+            T(1);
+            const uint32_t sa = stage_base + stage * STAGE_BYTES;
             if (p.dbg & 1) {
               if (rank == 0) mbar_arrive(full_bar(stage));
             } else if (CG2) {
@@ -176,25 +220,58 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
               tma_load_3d(sa + Cfg::A_BYTES, &tm_w, full_bar(stage), kb * 64, n0, d);
             }
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+            T(2);
           }
         }
       }
+      Tflush(0);
     }
   } else if (warp == 1) {
-    // ===== MMA issuer (one thread) =====
-    if (lane == 0 && rank == 0) {
+    // ===== MMA issuer: the whole warp runs the (uniform) loop, one elected lane issues =====
+    if (rank == 0) {
       constexpr uint32_t idesc = umma_idesc_bf16_mn(CG2 ? 256 : 128, BN);
       int stage = 0; uint32_t phase = 0;
       int acc = 0; uint32_t acc_phase = 0;
+      if (HALO) mbar_wait(w_bar, 0);
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
+        T(0);
         mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
+        T(1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
-        for (int it = 0; it < kiters; ++it) {
+        if (HALO) {
           mbar_wait(full_bar(stage), phase);
+          T(2);
           tc_fence_after();
-          const uint32_t sa = stage_base + stage * Cfg::STAGE_BYTES;
+          const uint32_t sa = stage_base + stage * STAGE_BYTES;
+          uint32_t first = 0;
+          if (elect_one()) {
+          for (int d = 0; d < p.taps; ++d)
+            for (int kb = 0; kb < p.kblocks; ++kb) {
+              // tap d: rows d .. d + 127 of the 130-row box = descriptor start shifted by d rows of 128 B
+              uint64_t da = umma_desc_sw128(sa + kb * Cfg::HALO_A_BYTES + d * 128);
+              if (p.desc_base_offset) da |= (uint64_t)(d & 7) << 49;
+              const uint64_t db = umma_desc_sw128(w_base + (uint32_t)((d * p.kblocks + kb) * BN * 128));
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                umma_bf16(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, first);
+                first = 1u;
+              }
+            }
+          umma_commit(empty_bar(stage));
+          }
+          __syncwarp();
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+          T(3);
+        }
+        for (int it = 0; it < (HALO ? 0 : kiters); ++it) {
+          T(0);
+          mbar_wait(full_bar(stage), phase);
+          T(2);
+          tc_fence_after();
+          const uint32_t sa = stage_base + stage * STAGE_BYTES;
           const uint64_t da = umma_desc_sw128(sa), db = umma_desc_sw128(sa + Cfg::A_BYTES);
+          if (elect_one()) {
 #pragma unroll
           for (int k = 0; k < 4; ++k) { // 4 x (K = 16 bf16 = 32 B) inside the 128-byte swizzle row
             if (p.dbg & 8) continue;
@@ -203,12 +280,20 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
           }
           if (CG2) umma_commit_cg2(empty_bar(stage), 3);   // frees the smem slot in BOTH CTAs when these MMAs retire
           else umma_commit(empty_bar(stage));
+          }
+          __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+          T(3);
         }
-        if (CG2) umma_commit_cg2(tfull_bar(acc), 3);   // accumulator complete -> both CTAs' epilogues
-        else umma_commit(tfull_bar(acc));
+        if (elect_one()) {
+          if (CG2) umma_commit_cg2(tfull_bar(acc), 3);   // accumulator complete -> both CTAs' epilogues
+          else umma_commit(tfull_bar(acc));
+        }
+        __syncwarp();
         if (++acc == NACC) { acc = 0; acc_phase ^= 1u; }
+        T(4);
       }
+      if (lane == 0) Tflush(1);
     }
   } else {
     // ===== epilogue: EG groups of 4 warps, thread <-> one output row =====
@@ -217,7 +302,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
     const int q = warp & 3;                        // TMEM lane quadrant this warp may access
     const int row = q * 32 + lane;
     const bool leader = ((ew & 3) == 0) && lane == 0;
-    const int NBUF = p.nbuf, PF = p.pf;
+    const int NBUF = p.nbuf > 0 ? p.nbuf : 1;      // (the fused head stages nothing)
     const uint32_t gbuf = out_base + (uint32_t)(g * NBUF) * TC_OUT_BYTES;
     constexpr int CH = BN / 64;
     const int tile_step = (SPLIT ? 1 : EG) * n_workers;     // this group's tiles ...
@@ -226,17 +311,18 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
     const int c_first = SPLIT ? g : 0;
     const uint32_t tempty_leader0 = CG2 ? mapa_cluster(tempty_bar(0), 0) : tempty_bar(0);
 
-    // residual prefetch cursor (leader only): chunk pf_j of this group's chunk sequence
+    // residual prefetch cursor (leader only): item pf_j of this group's (tile, chunk) sequence; the residual tile lands
+    // in the staging buffer the chunk's output will be written to (added in place)
     int pf_tile = tile_first, pf_c = c_first;
     uint32_t pf_j = 0;
+    const int PF = p.pf;
     auto issue_res = [&]() {
       if (pf_tile < p.num_tiles) {
         int n_idx, t0, b0;
         decode(pf_tile, n_idx, t0, b0);
-        const int n0 = n_idx * BN;
         const int buf = pf_j % NBUF;
         mbar_arrive_expect_tx(res_bar(g, buf), TC_OUT_BYTES);
-        tma_load_4d(gbuf + buf * TC_OUT_BYTES, &tm_res, res_bar(g, buf), n0 + pf_c * 64, 0, t0, b0);
+        tma_load_4d(gbuf + buf * TC_OUT_BYTES, &tm_res, res_bar(g, buf), n_idx * BN + pf_c * 64, 0, t0, b0);
       }
       ++pf_j;
       pf_c += C_STEP;
@@ -253,7 +339,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
       int n_idx, t0, b0;
       decode(tile, n_idx, t0, b0);
       const int n0 = n_idx * BN;
+      T(0);
       mbar_wait(tfull_bar(acc), acc_phase);
+      T(1);
       tc_fence_after();
       float head_acc = 0.f;
 #pragma unroll 1
@@ -268,12 +356,15 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
             tma_store_wait_read_n(NBUF - 1);                   // buffer of this chunk is free again
           }
         }
+        T(2);
         named_bar_sync(1 + g, 128);
+        T(3);
         uint32_t v[64];
         const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN + c * 64);
         tmem_ld32(taddr, v);
         tmem_ld32(taddr + 32, v + 32);
         tmem_ld_wait();
+        T(4);
         if (c + C_STEP >= CH) {                    // this group's part of the accumulator is drained: hand it back to the (leader's) MMA warp
           tc_fence_before();
           __syncwarp();
@@ -284,6 +375,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
         }
         if (p.dbg & 2) { if (p.has_res) mbar_wait(res_bar(g, buf), (j / NBUF) & 1u); named_bar_sync(1 + g, 128); continue; }
         if (p.has_res) mbar_wait(res_bar(g, buf), (j / NBUF) & 1u);
+        T(5);
         const float4* bias4 = reinterpret_cast<const float4*>(s_bias + n0 + c * 64);
         const float4* hw4 = reinterpret_cast<const float4*>(s_headw + n0 + c * 64);
         unsigned char* rowp = gen_base + (sbuf - base) + row * 128;
@@ -339,15 +431,18 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
             p.head_part[(b * p.head_slabs + slab) * (p.c_out >> 6) + n_idx * CH + c] = s;
           named_bar_sync(1 + g, 128);              // residual buffer fully read before it is refilled
         } else {
+          T(6);
           fence_proxy_async_smem();                // generic-proxy writes -> visible to the TMA store
           named_bar_sync(1 + g, 128);
           if (leader && !(p.dbg & 4)) {
             tma_store_4d(&tm_out, sbuf, n0 + c * 64, 0, t0, b0);
             tma_store_commit();
           }
+          T(7);
         }
       }
     }
+    if (leader) Tflush(2 + g);
     if (leader && !HEAD) tma_store_wait_all<0>();
   }
   tc_fence_before();

@@ -143,7 +143,14 @@ __device__ __forceinline__ uint32_t mapa_cluster(uint32_t local_addr, uint32_t r
   return r;
 }
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// one lane of a converged warp (the idiom keeps the surrounding code warp-uniform, so the compiler can hold
+// descriptors and coordinates in uniform registers instead of moving them there per instruction)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{ .reg .pred p; elect.sync _|p, 0xffffffff; selp.u32 %0, 1, 0, p; }" : "=r"(pred));
+  return pred != 0;
 }
 // TMA loads of a CTA pair: data lands in the issuing CTA's smem, the bytes are counted on the LEADER's mbarrier
 __device__ __forceinline__ void tma_load_4d_cg2(uint32_t dst, const CUtensorMap* m, uint32_t bar_cluster, int c0, int c1, int c2, int c3) {
@@ -177,4 +184,11 @@ __device__ __forceinline__ void umma_commit_cg2(uint32_t bar, uint16_t cta_mask)
 // kind::f16 instruction descriptor with M = m (128: one CTA; 256: CTA pair), N = n
 __host__ __device__ constexpr uint32_t umma_idesc_bf16_mn(int m, int n) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
+}
+
+__device__ __forceinline__ uint4 ld_nc_v4(const uint4* ptr) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(ptr));
+  return r;
 }
