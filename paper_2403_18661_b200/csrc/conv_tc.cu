@@ -155,7 +155,9 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   // (two epilogue groups: EG * nbuf staging buffers of 16 KB; a residual tile is prefetched pf chunks ahead into the
   //  buffer its chunk's output is staged in)
   const bool r = p.has_res;
-  if (cg2)                    { p.stages = r ? 4 : 5; p.nbuf = r ? (head ? 2 : 3) : 2; p.pf = r ? 1 : 0; }
+  if (cg2 && head)            { p.stages = 5; p.nbuf = 1; p.pf = 0; }
+  else if (cg2 && l.k * p.kblocks < 12) { p.stages = 5; p.nbuf = 2; p.pf = r ? 1 : 0; }   // short K: the epilogue is the critical path
+  else if (cg2)               { p.stages = r ? 5 : 6; p.nbuf = r ? 2 : 1; p.pf = r ? 1 : 0; }
   else if (BN == 256)         { p.stages = 3; p.nbuf = 2; p.pf = r ? 1 : 0; }
   else if (halo && BN == 128) { p.stages = 2; p.nbuf = 1; p.pf = 0; }
   else if (halo)              { p.stages = r ? 6 : 8; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
@@ -219,8 +221,11 @@ static int64_t tc_chunk_windows() {
   static int64_t v = 0;
   if (v == 0) {
     const char* e = getenv("AFRAME_CHUNK_B");
-    v = e ? atoll(e) : 592;     // 4 x 148 SMs: every layer's tile count is then a whole number of waves
-    if (v < 1) v = 592;
+    // windows per internal launch sequence.  Measured on B200: every layer launch carries ~12 us of launch gap, prologue
+    // (TMEM/barriers/first loads from HBM) and drain, so large chunks win (592: 869, 1184: 922, 4096: 994 TFLOP/s);
+    // the three live activation tensors leave the 126 MB L2 from ~300 windows on anyway.
+    v = e ? atoll(e) : 4096;
+    if (v < 1) v = 4096;
   }
   return v;
 }

@@ -172,12 +172,16 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
 
   if (warp == 0) {
     // ===== TMA producer =====
-    if (lane == 0 && HALO) {
+    // (the whole warp runs the uniform loops; one elected lane issues, so operands stay in uniform registers)
+    if (HALO) {
       // resident weights, once per CTA (n_tiles == 1: BN == C_out)
-      mbar_arrive_expect_tx(w_bar, (uint32_t)p.w_bytes);
-      for (int d = 0; d < p.taps; ++d)
-        for (int kb = 0; kb < p.kblocks; ++kb)
-          tma_load_3d(w_base + (uint32_t)((d * p.kblocks + kb) * BN * 128), &tm_w, w_bar, kb * 64, 0, d);
+      if (elect_one()) {
+        mbar_arrive_expect_tx(w_bar, (uint32_t)p.w_bytes);
+        for (int d = 0; d < p.taps; ++d)
+          for (int kb = 0; kb < p.kblocks; ++kb)
+            tma_load_3d(w_base + (uint32_t)((d * p.kblocks + kb) * BN * 128), &tm_w, w_bar, kb * 64, 0, d);
+      }
+      __syncwarp();
       int stage = 0; uint32_t phase = 0;
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         int n_idx, t0, b0;
@@ -185,15 +189,19 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         T(0);
         mbar_wait(empty_bar(stage), phase ^ 1u);
         T(1);
-        mbar_arrive_expect_tx(full_bar(stage), (uint32_t)(p.kblocks * 130 * 128));
         const uint32_t sa = stage_base + stage * STAGE_BYTES;
-        for (int kb = 0; kb < p.kblocks; ++kb)     // rows t0 - 1 .. t0 + 128 of the window; out-of-range rows are zero-filled
-          tma_load_4d(sa + kb * Cfg::HALO_A_BYTES, &tm_in, full_bar(stage), kb * 64, 0, t0 - 1, b0);
+        if (elect_one()) {
+          mbar_arrive_expect_tx(full_bar(stage), (uint32_t)(p.kblocks * 130 * 128));
+          for (int kb = 0; kb < p.kblocks; ++kb)   // rows t0 - 1 .. t0 + 128 of the window; out-of-range rows are zero-filled
+            tma_load_4d(sa + kb * Cfg::HALO_A_BYTES, &tm_in, full_bar(stage), kb * 64, 0, t0 - 1, b0);
+        }
+        __syncwarp();
         if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         T(2);
       }
-      Tflush(0);
-    } else if (lane == 0) {
+      if (lane == 0) Tflush(0);
+    } else {
+      const uint32_t lfull0 = CG2 ? mapa_cluster(full_bar(0), 0) : full_bar(0);   // leader's full barriers
       int stage = 0; uint32_t phase = 0;
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         int n_idx, t0, b0;
@@ -206,25 +214,28 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             mbar_wait(empty_bar(stage), phase ^ 1u);
             T(1);
             const uint32_t sa = stage_base + stage * STAGE_BYTES;
-            if (p.dbg & 1) {
-              if (rank == 0) mbar_arrive(full_bar(stage));
-            } else if (CG2) {
-              // both CTAs load their own A rows and their half of B; all bytes are counted on the leader's barrier
-              if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * Cfg::STAGE_BYTES);
-              const uint32_t lbar = mapa_cluster(full_bar(stage), 0);
-              tma_load_4d_cg2(sa, &tm_in, lbar, kb * 64, par, t0 + toff, b0);
-              tma_load_3d_cg2(sa + Cfg::A_BYTES, &tm_w, lbar, kb * 64, n0 + (int)rank * Cfg::B_ROWS, d);
-            } else {
-              mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
-              tma_load_4d(sa, &tm_in, full_bar(stage), kb * 64, par, t0 + toff, b0);
-              tma_load_3d(sa + Cfg::A_BYTES, &tm_w, full_bar(stage), kb * 64, n0, d);
+            if (elect_one()) {
+              if (p.dbg & 1) {
+                if (rank == 0) mbar_arrive(full_bar(stage));
+              } else if (CG2) {
+                // both CTAs load their own A rows and their half of B; all bytes are counted on the leader's barrier
+                if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * Cfg::STAGE_BYTES);
+                const uint32_t lbar = lfull0 + 8u * stage;
+                tma_load_4d_cg2(sa, &tm_in, lbar, kb * 64, par, t0 + toff, b0);
+                tma_load_3d_cg2(sa + Cfg::A_BYTES, &tm_w, lbar, kb * 64, n0 + (int)rank * Cfg::B_ROWS, d);
+              } else {
+                mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
+                tma_load_4d(sa, &tm_in, full_bar(stage), kb * 64, par, t0 + toff, b0);
+                tma_load_3d(sa + Cfg::A_BYTES, &tm_w, full_bar(stage), kb * 64, n0, d);
+              }
             }
+            __syncwarp();
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             T(2);
           }
         }
       }
-      Tflush(0);
+      if (lane == 0) Tflush(0);
     }
   } else if (warp == 1) {
     // ===== MMA issuer: the whole warp runs the (uniform) loop, one elected lane issues =====
