@@ -1,0 +1,141 @@
+"""GPU parity (through the C ABI) of the streaming state (O-6, BASELINE.json configs[2]/[4]) and of the offline
+timeslide driver (configs[3]) against the float64 oracle."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import network as onet
+from oracle import stream as ost
+from synthdata import coloured_noise, make_weight_blob, tiny_config, full_config
+
+pytestmark = pytest.mark.gpu
+FS = 2048
+S = 128
+
+
+@pytest.fixture(scope="module")
+def af():
+    import __graft_entry__ as ge
+    ge.build()
+    import paper_2403_18661_b200 as af
+    return af
+
+
+def rel_err(g, o):
+    g, o = np.asarray(g, np.float64), np.asarray(o, np.float64)
+    return float(np.max(np.abs(g - o) / np.maximum(np.abs(o), 1e-3 * np.abs(o).max())))
+
+
+def _run_stream(af, ctx, w, x, n_updates):
+    st = ctx.stream_create(w)
+    upd = torch.from_numpy(np.ascontiguousarray(x[:, : n_updates * S].reshape(2, n_updates, S).transpose(1, 0, 2))).cuda()
+    flags, scores = [], []
+    for u in range(n_updates):
+        st.step(upd[u])
+        flags.append(int(st.n_scores.item()))
+        scores.append(float(st.score.item()))
+    st.close()
+    return np.asarray(flags), np.asarray(scores)
+
+
+def test_stream_fp32_matches_oracle_through_warmup_and_a_psd_update(af):
+    """configs[2]/[4] geometry (64 s PSD, update every 8 s, stride 128) with the tiny network in fp32: warm-up flags
+    (reading C1), every score up to and across the second PSD epoch (reading C2), rule T2."""
+    tc = tiny_config()
+    n_updates = (131072 + 16384) // S + 12                      # past the second PSD (n = 147456)
+    x = coloured_noise(n_updates * S, seed=1002)
+    cfg = ost.StreamConfig(kernel_len=tc["kernel_len"], n_design=4096)
+    blob = make_weight_blob(**tc)
+    so = ost.StreamOracle(cfg, net=onet.parse_blob(blob))
+    ref = [so.step(x[:, u * S:(u + 1) * S].astype(np.float64)) for u in range(n_updates)]
+    assert so.n_psd_updates == 2
+
+    ctx = af.Context(n_design=4096, kernel_len=tc["kernel_len"], precision=af.FP32)
+    w = ctx.load_weights(blob)
+    flags, scores = _run_stream(af, ctx, w, x, n_updates)
+    exp_flags = np.array([0 if r is None else 1 for r in ref])
+    np.testing.assert_array_equal(flags, exp_flags)
+    first = int(np.argmax(exp_flags))
+    assert first == 131072 // S - 1 + tc["kernel_len"] // S - 1   # first PSD at update 1023, window full 15 updates later
+    got = scores[first:]
+    want = np.array([r for r in ref if r is not None])
+    assert rel_err(got, want) <= 1e-4
+
+
+def test_stream_bf16_full_network_scores(af):
+    """configs[4]: config-1 network in bf16 at batch 1; rule T3 on the first scored updates."""
+    fc = full_config()
+    n_updates = 131072 // S + 3072 // S + 6
+    x = coloured_noise(n_updates * S, seed=1002)
+    blob = make_weight_blob(**fc)
+    so = ost.StreamOracle(ost.StreamConfig(), net=onet.parse_blob(blob))
+    ref = [so.step(x[:, u * S:(u + 1) * S].astype(np.float64)) for u in range(n_updates)]
+    ctx = af.Context(precision=af.BF16)
+    w = ctx.load_weights(blob)
+    flags, scores = _run_stream(af, ctx, w, x, n_updates)
+    np.testing.assert_array_equal(flags, [0 if r is None else 1 for r in ref])
+    want = np.array([r for r in ref if r is not None])
+    assert len(want) == n_updates - (131072 // S - 1 + 3072 // S - 1)
+    assert rel_err(scores[flags == 1], want) <= 2e-2
+
+
+def test_stream_reset_reproduces_the_same_scores(af):
+    tc = tiny_config()
+    n_updates = 131072 // S + tc["kernel_len"] // S + 3
+    x = coloured_noise(n_updates * S, seed=5)
+    ctx = af.Context(n_design=4096, kernel_len=tc["kernel_len"], precision=af.FP32)
+    w = ctx.load_weights(make_weight_blob(**tc))
+    st = ctx.stream_create(w)
+    upd = torch.from_numpy(np.ascontiguousarray(x.reshape(2, n_updates, S).transpose(1, 0, 2))).cuda()
+    runs = []
+    for _ in range(2):
+        out = []
+        for u in range(n_updates):
+            st.step(upd[u])
+            if u >= n_updates - 3:
+                out.append((int(st.n_scores.item()), float(st.score.item())))
+        runs.append(out)
+        st.reset()
+    assert runs[0] == runs[1] and all(f == 1 for f, _ in runs[0])
+
+
+def test_score_timeslides_device_host_and_oracle(af):
+    """configs[3] in one call: whiten once, score every timeslide.  (a) equals aframe_forward_strided on the rolling-
+    whitened stream, bit for bit; (b) the host-buffer entry point returns the same bits; (c) sampled windows match the
+    float64 oracle (rolling whitening + network) within rule T3; (d) windows past the segment are refused."""
+    fc = full_config()
+    n_win, shifts, batch = 200, [2048, 3 * 2048], 96           # ragged last batch
+    m0 = 131072 - S - 1024
+    n_white = (n_win - 1) * S + max(shifts) + 3072
+    n_raw = -(-(m0 + n_white + 1024) // S) * S + 16384          # crosses a PSD epoch
+    x = coloured_noise(n_raw, seed=1003)
+    blob = make_weight_blob(**fc)
+    ctx = af.Context(precision=af.BF16)
+    w = ctx.load_weights(blob)
+    xd = torch.from_numpy(x).cuda()
+    dev = ctx.score_timeslides(w, xd, 0, n_win, shifts, batch=batch)
+    assert dev.shape == (2, n_win) and dev.is_cuda
+    white = ctx.whiten_rolling(xd, out_dtype=torch.bfloat16).contiguous()
+    for k, sh in enumerate(shifts):
+        ref = ctx.forward_strided(w, white, 0, n_win, chan_shift=[0, sh])
+        assert torch.equal(dev[k], ref)
+    host = ctx.score_timeslides(w, torch.from_numpy(x).pin_memory(), 0, n_win, shifts, batch=batch)
+    assert not host.is_cuda and torch.equal(host, dev.cpu())
+
+    cfg = ost.StreamConfig()
+    net = onet.parse_blob(blob)
+    x64 = x.astype(np.float64)
+    picks = [(0, 0), (0, n_win - 1), (1, 17), (1, n_win - 1), (1, 128)]
+    wins = []
+    for k, i in picks:
+        a = m0 + i * S
+        h1, _ = ost.whiten_rolling(x64[0], cfg, m_lo=a, m_hi=a + 3072)
+        l1, _ = ost.whiten_rolling(x64[1], cfg, m_lo=a + shifts[k], m_hi=a + shifts[k] + 3072)
+        wins.append(np.stack([h1, l1]))
+    want = onet.forward(net, np.stack(wins))
+    got = np.array([float(dev[k, i]) for k, i in picks])
+    assert rel_err(got, want) <= 2e-2
+
+    with pytest.raises(af.AframeError) as e:
+        ctx.score_timeslides(w, xd, 0, n_win + 2000, shifts, batch=batch)
+    assert e.value.status == af.ESHAPE
