@@ -166,6 +166,10 @@ aframe_status aframe_score_timeslides_host(aframe_ctx* ctx, const aframe_weights
                                            const int64_t* h_slide_shifts, int32_t n_slides, int64_t batch,
                                            float* h_scores);
 
+/* How many updates of this state were served by replaying the captured CUDA graph (0 if graphs are switched off with
+ * the environment variable AFRAME_STREAM_GRAPH=0, or while aframe_profile is on). */
+int64_t aframe_stream_graph_replays(const aframe_stream_state* st);
+
 /* Number of kernels the library has launched on this context since creation (for bench accounting). */
 int64_t aframe_launch_count(const aframe_ctx* ctx);
 

@@ -54,6 +54,7 @@ EXPORTS = {
     "aframe_stream_destroy": (None, [C.c_void_p]),
     "aframe_stream_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "aframe_launch_count": (C.c_int64, [C.c_void_p]),
+    "aframe_stream_graph_replays": (C.c_int64, [C.c_void_p]),
     "aframe_score_timeslides": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_int64,
                                           C.POINTER(C.c_int64), C.c_int32, C.c_int64, C.c_void_p]),
     "aframe_score_timeslides_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64,
@@ -267,6 +268,10 @@ class Stream:
 
     def reset(self):
         self.ctx._check(self.ctx.lib.aframe_stream_reset(self.handle))
+
+    @property
+    def uses_graph(self):
+        return int(self.ctx.lib.aframe_stream_graph_replays(self.handle)) > 0
 
     def step(self, new_samples: torch.Tensor):
         """Enqueue one update; results land in self.score / self.n_scores (device tensors)."""

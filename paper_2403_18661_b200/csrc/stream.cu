@@ -2,6 +2,7 @@
 // Every kernel of an update takes its decisions from a device-resident counter, so the same launch
 // sequence (and hence one captured CUDA graph) serves every update.
 #include <new>
+#include <stdlib.h>
 #include "common.cuh"
 
 struct aframe_stream_state {
@@ -20,6 +21,13 @@ struct aframe_stream_state {
   float* d_taps = nullptr;       // [C][L+1]
   float* d_white = nullptr;      // [C][K] newest K whitened samples, oldest first
   float* d_new = nullptr;        // [C][stride]
+  // One update = one CUDA graph launch: the launch sequence is captured the first time a given triple of caller
+  // pointers is seen and replayed afterwards (every decision of an update is taken on the device from the counters,
+  // so the same graph serves every update).
+  cudaGraphExec_t graph = nullptr;
+  const float* g_in = nullptr; float* g_scores = nullptr; int32_t* g_n = nullptr;
+  int64_t g_launches = 0;        // kernels per replay
+  int64_t replays = 0;
 };
 
 // Append `stride` samples per channel to the ring and advance the counter.  One CTA.
@@ -101,6 +109,7 @@ AF_API aframe_status aframe_stream_reset(aframe_stream_state* st) {
 AF_API void aframe_stream_destroy(aframe_stream_state* st) {
   if (!st) return;
   if (st->ctx) cudaStreamSynchronize(st->ctx->stream);
+  if (st->graph) cudaGraphExecDestroy(st->graph);
   cudaFree(st->blob);
   cudaGetLastError();
   st->ctx = nullptr;
@@ -152,11 +161,53 @@ AF_API aframe_status aframe_stream_create(aframe_ctx* ctx, const aframe_weights*
   return AFRAME_OK;
 }
 
+static aframe_status stream_step_enqueue(aframe_ctx* ctx, const float* d_new_samples, aframe_stream_state* st,
+                                         float* d_scores, int32_t* d_n_scores);
+
+static bool stream_graph_enabled() {
+  static int v = -1;
+  if (v < 0) { const char* e = getenv("AFRAME_STREAM_GRAPH"); v = e ? (atoi(e) != 0) : 1; }
+  return v != 0;
+}
+
+AF_API int64_t aframe_stream_graph_replays(const aframe_stream_state* st) { return st ? st->replays : 0; }
+
 AF_API aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samples, aframe_stream_state* st,
                                         float* d_scores, int32_t* d_n_scores) {
   if (!ctx) return AFRAME_EINVAL;
   if (!st || st->ctx != ctx) return af_fail(ctx, AFRAME_ESTATE, "stream state is destroyed or belongs to another context");
   if (!d_new_samples || !d_scores || !d_n_scores) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(ctx->stream, &cap);
+  // direct launches when the caller is capturing the stream itself, when stage timing is on, or when switched off
+  // (the legacy default stream cannot be captured: a context bound to it launches directly as well)
+  if (!stream_graph_enabled() || ctx->prof_on || ctx->layer_ms || cap != cudaStreamCaptureStatusNone ||
+      ctx->stream == nullptr || ctx->stream == cudaStreamLegacy)
+    return stream_step_enqueue(ctx, d_new_samples, st, d_scores, d_n_scores);
+  if (!st->graph || st->g_in != d_new_samples || st->g_scores != d_scores || st->g_n != d_n_scores) {
+    if (st->graph) { cudaGraphExecDestroy(st->graph); st->graph = nullptr; }
+    const int64_t l0 = ctx->launches;
+    AF_CUDA(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+    aframe_status rs = stream_step_enqueue(ctx, d_new_samples, st, d_scores, d_n_scores);
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
+    st->g_launches = ctx->launches - l0;
+    ctx->launches = l0;
+    if (rs != AFRAME_OK) { if (g) cudaGraphDestroy(g); cudaGetLastError(); return rs; }
+    if (e != cudaSuccess || !g) { cudaGetLastError(); return af_fail(ctx, AFRAME_ECUDA, "stream capture failed: %s", cudaGetErrorString(e)); }
+    e = cudaGraphInstantiate(&st->graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { st->graph = nullptr; cudaGetLastError(); return af_fail(ctx, AFRAME_ECUDA, "graph instantiation failed: %s", cudaGetErrorString(e)); }
+    st->g_in = d_new_samples; st->g_scores = d_scores; st->g_n = d_n_scores;
+  }
+  AF_CUDA(ctx, cudaGraphLaunch(st->graph, ctx->stream));
+  ctx->launches += st->g_launches;
+  st->replays++;
+  return AFRAME_OK;
+}
+
+static aframe_status stream_step_enqueue(aframe_ctx* ctx, const float* d_new_samples, aframe_stream_state* st,
+                                         float* d_scores, int32_t* d_n_scores) {
   const aframe_config& cfg = ctx->cfg;
   const int C = cfg.n_channels, L = cfg.filter_len, K = cfg.kernel_len, s = cfg.stride;
   stream_ingest_kernel<<<1, 256, 0, ctx->stream>>>(d_new_samples, C, s, st->d_raw, st->ring_len, st->d_n);

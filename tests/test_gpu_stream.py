@@ -99,6 +99,35 @@ def test_stream_reset_reproduces_the_same_scores(af):
     assert runs[0] == runs[1] and all(f == 1 for f, _ in runs[0])
 
 
+def test_stream_graph_replay_equals_direct_launches(af):
+    """On a non-default stream one update is one CUDA-graph launch (configs[4]); the scores must be the same bits as
+    the direct launch sequence of a context bound to the default stream."""
+    fc = full_config()
+    n_updates = 131072 // S + 3072 // S + 4
+    x = coloured_noise(n_updates * S, seed=11)
+    blob = make_weight_blob(**fc)
+    upd = torch.from_numpy(np.ascontiguousarray(x.reshape(2, n_updates, S).transpose(1, 0, 2))).cuda()
+    buf = torch.empty((2, S), dtype=torch.float32, device="cuda")
+    out = {}
+    for name, stream in (("direct", None), ("graph", torch.cuda.Stream())):
+        ctx = af.Context(precision=af.BF16, stream=stream)
+        w = ctx.load_weights(blob)
+        st = ctx.stream_create(w)
+        scores = []
+        with torch.cuda.stream(stream if stream is not None else torch.cuda.current_stream()):
+            for u in range(n_updates):
+                buf.copy_(upd[u], non_blocking=True)           # same device buffer every update -> one captured graph
+                st.step(buf)
+                if u >= n_updates - 5:
+                    torch.cuda.current_stream().synchronize()
+                    scores.append((int(st.n_scores.item()), float(st.score.item())))
+            torch.cuda.current_stream().synchronize()
+        out[name] = (scores, st.uses_graph)
+        st.close()
+    assert out["graph"][1] and not out["direct"][1]
+    assert out["graph"][0] == out["direct"][0] and all(f == 1 for f, _ in out["graph"][0])
+
+
 def test_score_timeslides_device_host_and_oracle(af):
     """configs[3] in one call: whiten once, score every timeslide.  (a) equals aframe_forward_strided on the rolling-
     whitened stream, bit for bit; (b) the host-buffer entry point returns the same bits; (c) sampled windows match the
