@@ -191,10 +191,13 @@ template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t lau
   cfg.blockDim = dim3((unsigned)TcCfg<BN, CG2>::THREADS);
   cfg.dynamicSmemBytes = (size_t)L.smem;
   cfg.stream = s;
-  cudaLaunchAttribute at[1];
+  cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeClusterDimension;
   at[0].val.clusterDim.x = CG2 ? 2 : 1; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-  cfg.attrs = at; cfg.numAttrs = 1;
+  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // the kernel orders itself with griddepcontrol.wait
+  at[1].val.programmaticStreamSerializationAllowed = 1;
+  static const int pdl = env_int("AFRAME_PDL", 1);
+  cfg.attrs = at; cfg.numAttrs = pdl ? 2 : 1;
   return cudaLaunchKernelEx(&cfg, kern, L.tm_in, L.tm_w, L.tm_out, L.tm_res, L.p);
 }
 

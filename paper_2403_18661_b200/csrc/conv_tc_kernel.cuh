@@ -155,6 +155,11 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
   tc_fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(gen_base + (tmem_slot - base));
 
+  // Programmatic dependent launch: the next layer's CTAs may start their prologue (barriers, TMEM, bias, resident
+  // weights) while this grid is still running; everything that reads the previous layer's output comes after pdl_wait().
+  pdl_launch_dependents();
+  if (!(HALO && warp == 0)) pdl_wait();            // (the halo producer first issues its weight loads, see below)
+
   const int kiters = p.taps * p.kblocks;
   // cycle accounting for experiments (CTA 0 only): T(slot) adds the cycles since the previous T() of this thread
   const bool prof = p.dbg_out != nullptr && blockIdx.x == 0;
@@ -182,6 +187,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             tma_load_3d(w_base + (uint32_t)((d * p.kblocks + kb) * BN * 128), &tm_w, w_bar, kb * 64, 0, d);
       }
       __syncwarp();
+      pdl_wait();                                  // the activations below are the previous layer's output
       int stage = 0; uint32_t phase = 0;
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         int n_idx, t0, b0;

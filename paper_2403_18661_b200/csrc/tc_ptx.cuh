@@ -192,3 +192,7 @@ __device__ __forceinline__ uint4 ld_nc_v4(const uint4* ptr) {
                : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(ptr));
   return r;
 }
+
+// Programmatic dependent launch (griddepcontrol): see conv_tc_kernel
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
