@@ -93,6 +93,48 @@ template <int BN, bool CG2 = false> struct TcCfg {
 
 __device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 
+// One 64-channel chunk of one output row: + bias (+ residual read from the staging buffer) -> bf16 -> max(., lo)
+// (lo = 0: ReLU, which commutes with the rounding; lo = -inf: none) -> staging buffer, or the fused head's dot product.
+template <bool RES, bool HEAD>
+__device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4* bias4, const float4* hw4,
+                                                 unsigned char* rowp, int row, __nv_bfloat162 lo2, float& head_acc) {
+  float hacc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int jj = 0; jj < 8; ++jj) {                 // 8 pieces of 8 channels (16 B of bf16)
+    const float4 bA = bias4[2 * jj], bB = bias4[2 * jj + 1];
+    float f[8];
+    f[0] = __uint_as_float(v[8 * jj + 0]) + bA.x; f[1] = __uint_as_float(v[8 * jj + 1]) + bA.y;
+    f[2] = __uint_as_float(v[8 * jj + 2]) + bA.z; f[3] = __uint_as_float(v[8 * jj + 3]) + bA.w;
+    f[4] = __uint_as_float(v[8 * jj + 4]) + bB.x; f[5] = __uint_as_float(v[8 * jj + 5]) + bB.y;
+    f[6] = __uint_as_float(v[8 * jj + 6]) + bB.z; f[7] = __uint_as_float(v[8 * jj + 7]) + bB.w;
+    uint4* sp = reinterpret_cast<uint4*>(rowp + ((jj ^ (row & 7)) << 4));   // 128B-swizzle position
+    if (RES) {
+      const uint4 r = *sp;
+      const uint32_t rw[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {                // bf16 pair -> two fp32 (exact): low half << 16, high half masked
+        f[2 * e] += __uint_as_float(rw[e] << 16);
+        f[2 * e + 1] += __uint_as_float(rw[e] & 0xffff0000u);
+      }
+    }
+    uint4 o;
+    __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(&o);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) ob[e] = __hmax2(__floats2bfloat162_rn(f[2 * e], f[2 * e + 1]), lo2);
+    if (HEAD) {
+      const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
+      const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
+      hacc[0] = fmaf(__uint_as_float(ow[0] << 16), hA.x, hacc[0]); hacc[1] = fmaf(__uint_as_float(ow[0] & 0xffff0000u), hA.y, hacc[1]);
+      hacc[2] = fmaf(__uint_as_float(ow[1] << 16), hA.z, hacc[2]); hacc[3] = fmaf(__uint_as_float(ow[1] & 0xffff0000u), hA.w, hacc[3]);
+      hacc[0] = fmaf(__uint_as_float(ow[2] << 16), hB.x, hacc[0]); hacc[1] = fmaf(__uint_as_float(ow[2] & 0xffff0000u), hB.y, hacc[1]);
+      hacc[2] = fmaf(__uint_as_float(ow[3] << 16), hB.z, hacc[2]); hacc[3] = fmaf(__uint_as_float(ow[3] & 0xffff0000u), hB.w, hacc[3]);
+    } else {
+      *sp = o;
+    }
+  }
+  if (HEAD) head_acc += (hacc[0] + hacc[1]) + (hacc[2] + hacc[3]);
+}
+
 template <int BN, bool HEAD, bool CG2, bool HALO>
 __global__ void __launch_bounds__(TcCfg<BN, CG2>::THREADS, 1)
 conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 rows */, const __grid_constant__ CUtensorMap tm_w,
@@ -396,45 +438,10 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         const float4* bias4 = reinterpret_cast<const float4*>(s_bias + n0 + c * 64);
         const float4* hw4 = reinterpret_cast<const float4*>(s_headw + n0 + c * 64);
         unsigned char* rowp = gen_base + (sbuf - base) + row * 128;
-#pragma unroll
-        for (int jj = 0; jj < 8; ++jj) {           // 8 pieces of 8 channels (16 B of bf16)
-          const float4 bA = bias4[2 * jj], bB = bias4[2 * jj + 1];
-          float f[8];
-          f[0] = __uint_as_float(v[8 * jj + 0]) + bA.x; f[1] = __uint_as_float(v[8 * jj + 1]) + bA.y;
-          f[2] = __uint_as_float(v[8 * jj + 2]) + bA.z; f[3] = __uint_as_float(v[8 * jj + 3]) + bA.w;
-          f[4] = __uint_as_float(v[8 * jj + 4]) + bB.x; f[5] = __uint_as_float(v[8 * jj + 5]) + bB.y;
-          f[6] = __uint_as_float(v[8 * jj + 6]) + bB.z; f[7] = __uint_as_float(v[8 * jj + 7]) + bB.w;
-          uint4* sp = reinterpret_cast<uint4*>(rowp + ((jj ^ (row & 7)) << 4));   // 128B-swizzle position
-          if (p.has_res) {
-            const uint4 r = *sp;
-            const __nv_bfloat162* rb = reinterpret_cast<const __nv_bfloat162*>(&r);
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const float2 rf = __bfloat1622float2(rb[e]);
-              f[2 * e] += rf.x; f[2 * e + 1] += rf.y;
-            }
-          }
-          uint4 o;
-          __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(&o);
-#pragma unroll
-          for (int e = 0; e < 4; ++e) ob[e] = __floats2bfloat162_rn(f[2 * e], f[2 * e + 1]);
-          if (p.relu) {                            // ReLU commutes with the rounding: one packed max per channel pair
-            const __nv_bfloat162 z2 = __float2bfloat162_rn(0.f);
-#pragma unroll
-            for (int e = 0; e < 4; ++e) ob[e] = __hmax2(ob[e], z2);
-          }
-          if (HEAD) {
-            const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
-            const float2 o0 = __bfloat1622float2(ob[0]), o1 = __bfloat1622float2(ob[1]);
-            const float2 o2 = __bfloat1622float2(ob[2]), o3 = __bfloat1622float2(ob[3]);
-            head_acc = fmaf(o0.x, hA.x, head_acc); head_acc = fmaf(o0.y, hA.y, head_acc);
-            head_acc = fmaf(o1.x, hA.z, head_acc); head_acc = fmaf(o1.y, hA.w, head_acc);
-            head_acc = fmaf(o2.x, hB.x, head_acc); head_acc = fmaf(o2.y, hB.y, head_acc);
-            head_acc = fmaf(o3.x, hB.z, head_acc); head_acc = fmaf(o3.y, hB.w, head_acc);
-          } else {
-            *sp = o;
-          }
-        }
+        // straight-line code per variant (no run-time branches inside the unrolled loop, so the 8 pieces interleave)
+        const __nv_bfloat162 lo2 = __float2bfloat162_rn(p.relu ? 0.f : -INFINITY);
+        if (p.has_res) tc_epilogue_math<true, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc);
+        else tc_epilogue_math<false, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc);
         if (HEAD) {
           // the warp's 32 rows are one 32-row slab of one window (T_box % 32 == 0): reduce and emit a partial
           float s = head_acc;
