@@ -370,6 +370,14 @@ def run_ours(args):
         out["roofline_whiten"] = {"kernel": "whiten_os_kernel", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"],
                                   "unit": "GB/s", "frac": gbs / peaks["hbm"], "traffic": None,
                                   "algorithmic": "4 B in + 2 B (bf16) out per whitened sample per channel"}
+    we_ms = stages["welch"][0]
+    if we_ms > 0:
+        gbs = args.steps * 2 * n_raw * 4 / (we_ms * 1e-3) / 1e9                   # every raw sample enters the PSD once
+        out["roofline_welch"] = {"kernel": "welch_periodogram_kernel + psd_mean_kernel", "bound": "hbm", "achieved": gbs,
+                                 "peak": peaks["hbm"], "unit": "GB/s", "frac": gbs / peaks["hbm"], "traffic": None,
+                                 "algorithmic": "4 B per raw sample per channel (each sample is in two 50 %-overlapped "
+                                                "segments; the second read is an L2 hit); DESIGN.md section 5 derives the fp32-ALU "
+                                                "bound that caps both FFT kernels below the HBM roofline"}
     if args.latency_updates > 0 and world == 1:
         out["latency"] = latency_run(af, torch, stream, blob, args.latency_updates)
     if not args.no_cpu_baseline:

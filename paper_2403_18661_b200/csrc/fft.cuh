@@ -85,9 +85,24 @@ __device__ __forceinline__ void fft_pass(T2* s, const T2* __restrict__ tw, int t
 #pragma unroll
       for (int r = 0; r < R; ++r) v[jj][r] = s[fft_pad(j + r * J)];
       if (NS > 1) {
+        // twiddles w^r, r = 1..R-1, w = exp(-2 pi i (j % NS) / (NS R)): ONE table load, the powers by a depth-4
+        // product tree (w2 = w w, w4 = w2 w2, w8 = w4 w4, the rest as products of two of those): the table loads of all
+        // R-1 powers made this pass wait on L1/L2 (long-scoreboard stalls); the tree costs R-2 complex multiplies and
+        // loses < R ulp.
         const int q = (j % NS) * (AF_TW_N / (NS * R));
+        T2 w[R];
+        w[1] = tw[q];
+        if (R > 2) w[2] = cmul(w[1], w[1]);
+        if (R > 4) w[4] = cmul(w[2], w[2]);
+        if (R > 8) w[8] = cmul(w[4], w[4]);
 #pragma unroll
-        for (int r = 1; r < R; ++r) v[jj][r] = cmul(v[jj][r], tw[r * q]);
+        for (int r = 3; r < R; ++r)
+          if ((r & (r - 1)) != 0) {                 // not a power of two: highest set bit times the rest
+            const int hb = r >= 8 ? 8 : (r >= 4 ? 4 : 2);
+            w[r] = cmul(w[hb], w[r - hb]);
+          }
+#pragma unroll
+        for (int r = 1; r < R; ++r) v[jj][r] = cmul(v[jj][r], w[r]);
       }
       RegFFT<R, T2>::run(v[jj]);
     }

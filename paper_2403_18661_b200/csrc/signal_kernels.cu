@@ -161,7 +161,7 @@ filter_design_kernel(const float* __restrict__ psd, int F_w, int C, double fs, d
 // FFT -> untangle, multiply by real H, re-tangle -> inverse FFT (conjugation trick) -> store valid part.
 // --------------------------------------------------------------------------------------------------
 template <bool OUT_BF16>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 3)
 whiten_os_kernel(const float* __restrict__ strain, int64_t n_samples, int64_t ld, const float* __restrict__ H, int C,
                  int64_t in0, int64_t out_total, int64_t epoch_len, int blocks_per_epoch, int L, float scale,
                  const float2* __restrict__ tw, void* __restrict__ out_v, int64_t ld_out) {
@@ -227,11 +227,16 @@ whiten_os_kernel(const float* __restrict__ strain, int64_t n_samples, int64_t ld
   const int half = L / 2;
   if (OUT_BF16) {
     __nv_bfloat16* o = reinterpret_cast<__nv_bfloat16*>(out_v) + (int64_t)c * ld_out + out0;
+    const bool st_vec = ((((uintptr_t)o) & 3) == 0) && ((half & 1) == 0);
     for (int n = tid; n < M; n += NT) {
       const float2 r = s[fft_pad(n)];
       const int64_t i0 = 2 * n - half;
-      if (i0 >= 0 && i0 < n_valid) o[i0] = __float2bfloat16_rn(r.x);
-      if (i0 + 1 >= 0 && i0 + 1 < n_valid) o[i0 + 1] = __float2bfloat16_rn(-r.y);
+      if (st_vec && i0 >= 0 && i0 + 1 < n_valid) {
+        *reinterpret_cast<__nv_bfloat162*>(o + i0) = __floats2bfloat162_rn(r.x, -r.y);
+      } else {
+        if (i0 >= 0 && i0 < n_valid) o[i0] = __float2bfloat16_rn(r.x);
+        if (i0 + 1 >= 0 && i0 + 1 < n_valid) o[i0 + 1] = __float2bfloat16_rn(-r.y);
+      }
     }
   } else {
     float* o = reinterpret_cast<float*>(out_v) + (int64_t)c * ld_out + out0;
