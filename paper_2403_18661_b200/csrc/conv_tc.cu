@@ -3,6 +3,7 @@
 #include <map>
 
 #include "conv_tc_kernel.cuh"
+#include "conv_block_kernel.cuh"
 #include "common.cuh"
 #include "net_plan.h"
 #include "stem.h"
@@ -209,12 +210,86 @@ static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s) {
                      : (L.BN == 128 ? launch_bn<128, false, false>(L, s) : launch_bn<64, false, false>(L, s));
 }
 
+// fused basic block (conv_block_kernel): layers a (conv) and b (conv + residual from a's input)
+struct TcBlockLaunch {
+  CUtensorMap tm_x, tm_wa, tm_wb, tm_out;
+  TcBlockParams p;
+  int grid = 0, smem = 0;
+};
+
+// Layer i is the first conv of a basic block the fused kernel can run: 64 -> 64 -> 64 channels, k3 s1 p1, ReLU after each,
+// the second conv adds the block input, and nothing else reads the intermediate tensor.
+static int fusable_block(const aframe_weights* w, int i) {
+  const int n = (int)w->layers.size();
+  if (i < 2 || i + 1 >= n) return -1;
+  const LayerDesc& a = w->layers[i];
+  const LayerDesc& b = w->layers[i + 1];
+  auto conv3 = [](const LayerDesc& l) { return l.kind == 0 && l.k == 3 && l.stride == 1 && l.pad == 1 && l.relu && l.c_in == 64 && l.c_out == 64; };
+  if (!conv3(a) || !conv3(b) || a.residual_from >= 0 || b.input_from != i || b.residual_from != a.input_from) return -1;
+  for (int j = 0; j < n; ++j)
+    if (j != i + 1 && (w->layers[j].input_from == i || w->layers[j].residual_from == i)) return -1;
+  return i + 1;
+}
+
+static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia, int ib, const __nv_bfloat16* x,
+                               __nv_bfloat16* out, int64_t nb, TcBlockLaunch& L) {
+  const LayerDesc& a = w->layers[ia];
+  const int T = a.t_out;
+  const uint64_t dims[3] = {64, (uint64_t)T, (uint64_t)nb};
+  const uint64_t str[2] = {128, (uint64_t)T * 128};
+  const uint32_t box_x[3] = {64, 130, 1}, box_o[3] = {64, TCB_ROWS, 1}, box_w[3] = {64, 64, 1};
+  const uint64_t wd[3] = {64, 64, 3};
+  const uint64_t ws[2] = {128, 64 * 128};
+  if (!encode_map(ctx, &L.tm_x, x, 3, dims, str, box_x) || !encode_map(ctx, &L.tm_out, out, 3, dims, str, box_o) ||
+      !encode_map(ctx, &L.tm_wa, w->d_w16[ia], 3, wd, ws, box_w) || !encode_map(ctx, &L.tm_wb, w->d_w16[ib], 3, wd, ws, box_w))
+    return false;
+  TcBlockParams& p = L.p;
+  p.bias_a = w->d_bias[ia]; p.bias_b = w->d_bias[ib];
+  p.T = T;
+  p.tiles_per_win = (T + TCB_ROWS - 1) / TCB_ROWS;
+  p.num_tiles = (int)(nb * p.tiles_per_win);
+  p.div_tw = tc_fastdiv((uint32_t)p.tiles_per_win);
+  p.nx = 6; p.ny = 2; p.no = 1;
+  p.dbg_out = nullptr;
+  if (env_int("AFRAME_TC_PROF", 0)) {
+    static long long* d_prof = nullptr;
+    if (!d_prof) { cudaMalloc(&d_prof, sizeof(long long) * 64 * 8); cudaMemset(d_prof, 0, sizeof(long long) * 64 * 8); }
+    p.dbg_out = d_prof + 48 * (ib % 8);
+    if (const char* f = getenv("AFRAME_TCB_PROF_PTR")) { FILE* fp = fopen(f, "w"); if (fp) { fprintf(fp, "%llu\n", (unsigned long long)(uintptr_t)d_prof); fclose(fp); } }
+  }
+  L.smem = tcb_smem(p.nx, p.ny, p.no);
+  L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
+  return true;
+}
+
+static cudaError_t launch_block(const TcBlockLaunch& L, cudaStream_t s) {
+  static bool attr = false;
+  if (!attr) {
+    cudaError_t e = cudaFuncSetAttribute(conv_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448);
+    if (e != cudaSuccess) return e;
+    attr = true;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)L.grid);
+  cfg.blockDim = dim3(576);
+  cfg.dynamicSmemBytes = (size_t)L.smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  static const int pdl = env_int("AFRAME_PDL", 1);
+  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, conv_block_kernel, L.tm_x, L.tm_wa, L.tm_wb, L.tm_out, L.p);
+}
+
 struct TcPlanCache {
   const aframe_weights* w = nullptr;
   void* base = nullptr;
   int64_t nb = 0;
   size_t slot_bytes = 0;
   std::vector<TcLaunch> launches;   // indexed by layer
+  std::vector<TcBlockLaunch> blocks;  // indexed by the block's SECOND layer
+  std::vector<int> fused_with;        // per layer: index of the partner layer if the pair runs fused, else -1
 };
 static std::map<aframe_ctx*, std::vector<TcPlanCache>> g_cache;
 
@@ -274,9 +349,18 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       pc = &caches.back();
       pc->w = w; pc->base = base; pc->nb = nb; pc->slot_bytes = slot_bytes;
       pc->launches.resize(n);
+      pc->blocks.resize(n);
+      pc->fused_with.assign(n, -1);
+      if (env_int("AFRAME_FUSE_BLOCK", 1))
+        for (int i = 2; i < n; ++i) {
+          const int ib = pc->fused_with[i] < 0 ? fusable_block(w, i) : -1;
+          if (ib < 0) continue;
+          if (!build_block_launch(ctx, w, i, ib, slot_ptr(w->layers[i].input_from), slot_ptr(ib), nb, pc->blocks[ib])) { caches.pop_back(); return AFRAME_ECUDA; }
+          pc->fused_with[i] = ib; pc->fused_with[ib] = i;
+        }
       for (int i = 2; i < n; ++i) {
         const LayerDesc& l = w->layers[i];
-        if (l.kind != 0) continue;
+        if (l.kind != 0 || pc->fused_with[i] >= 0) continue;
         if (!build_launch(ctx, w, i, slot_ptr(l.input_from), l.residual_from >= 0 ? slot_ptr(l.residual_from) : nullptr,
                           slot_ptr(i), nb, i == fuse, head_part, pc->launches[i])) { caches.pop_back(); return AFRAME_ECUDA; }
       }
@@ -298,11 +382,19 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     for (int i = 2; i < n; ++i) {
       const LayerDesc& l = w->layers[i];
       struct Rec { aframe_ctx* c; std::vector<cudaEvent_t>& v; int i; ~Rec() { if (c->layer_ms) cudaEventRecord(v[i + 1], c->stream); } } rec{ctx, lev, i};
+      if (l.kind == 0 && pc->fused_with[i] > i) continue;      // first conv of a fused block: runs with its partner
       if (l.kind == 0) {
+        // Alternate the direction in which consecutive launches walk their tiles: a layer then starts with the rows its
+        // producer wrote LAST, which are still in L2 (walking every layer forwards evicts exactly the lines that are
+        // about to be read).
+        static const int alt = env_int("AFRAME_ALT_DIR", 1);
+        const int rev = alt ? (n_conv & 1) : 0;
+        pc->launches[i].p.reverse = rev;
+        pc->blocks[i].p.reverse = rev;
         const TcLaunch& L = pc->launches[i];
         af_prof_begin(ctx, AFRAME_PROF_CONV);
         ++n_conv;
-        cudaError_t e = launch_conv(L, ctx->stream);
+        cudaError_t e = pc->fused_with[i] >= 0 ? launch_block(pc->blocks[i], ctx->stream) : launch_conv(L, ctx->stream);
         ctx->launches++;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
       } else if (l.kind == 2) {

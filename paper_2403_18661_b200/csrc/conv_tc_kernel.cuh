@@ -46,6 +46,7 @@ struct TcConvParams {
   int n_tiles;               // C_out / BN
   int t_blks, T_box, B_box;  // tile = T_box rows of B_box windows (T_box * B_box = 128)
   int num_tiles;
+  int reverse;               // walk the tiles from the last to the first (see af_forward_bf16: L2 reuse between layers)
   int relu, has_res;
   int stages;                // smem ring depth of the main loop
   int nbuf, pf;              // output/residual staging buffers per epilogue group, residual prefetch distance
@@ -211,6 +212,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
   // tile -> (n0, t0, b0): n fastest, then the T_box-row block inside a window group, then the window group
   auto decode = [&](int tile, int& n_idx, int& t0, int& b0) {
     int mp, tb, bb;
+    if (p.reverse) tile = p.num_tiles - 1 - tile;
     p.div_n.divmod(tile, mp, n_idx);
     const int m_idx = mp * (CG2 ? 2 : 1) + (int)rank;
     p.div_t.divmod(m_idx, bb, tb);

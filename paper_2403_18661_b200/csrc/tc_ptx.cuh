@@ -196,3 +196,27 @@ __device__ __forceinline__ uint4 ld_nc_v4(const uint4* ptr) {
 // Programmatic dependent launch (griddepcontrol): see conv_tc_kernel
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
+               ::"l"(m), "r"(src), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+// non-blocking probe of an mbarrier phase
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile("{ .reg .pred p; mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+               : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  return done != 0;
+}
+
+// Descriptor halves for the issue loops: the high word of a K-major SWIZZLE_128B descriptor is constant, the low word is
+// (address >> 4) | (1 << 16); a row / K shift is a plain 32-bit add on the low word (the 14-bit address field cannot
+// carry for shared-memory addresses), which keeps the per-MMA uniform-datapath work to one add per operand.
+__host__ __device__ constexpr uint32_t umma_desc_hi_sw128() { return (uint32_t)(1024 >> 4) | (1u << 14) | (2u << 29); }
+__device__ __forceinline__ uint32_t umma_desc_lo(uint32_t smem_addr) { return ((smem_addr & 0x3FFFFu) >> 4) | (1u << 16); }
+template <bool ACC>
+__device__ __forceinline__ void umma_bf16_lohi(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc) {
+  asm volatile(
+      "{ .reg .pred p; .reg .b64 da, db; setp.ne.b32 p, %4, 0; mov.b64 da, {%1, %5}; mov.b64 db, {%2, %5};\n"
+      "  tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, p; }"
+      ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(ACC ? 1u : 0u), "r"(umma_desc_hi_sw128()) : "memory");
+}
