@@ -127,7 +127,7 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
     }
     if (lane == 0) Tflush(0);
   } else if (warp == 1) {
-    // ===== MMA issuer: A(i) then B(i - 1), so epilogue A of tile i runs under the MMAs of B(i - 1) =====
+    // ===== MMA issuer (whole warp runs the uniform loop, one elected lane issues) =====
     constexpr uint32_t idesc = umma_idesc_bf16_mn(128, 64);
     mbar_wait(w_bar, 0);
     int n_my = 0;
