@@ -14,6 +14,7 @@ psd      O-1  Welch PSD ("estimate the PSD"; reading A1, A2)
 whiten   O-2  whitening-filter design, O-3 FIR whitening (A3-A6)
 network  O-5  1D ResNet forward from the layer table (B1-B8)
 stream   O-4  window unfold, O-6 streaming / rolling-PSD rule, timeslides
+postprocess  NEXT-1  1 s top-hat integration of the scores, 8 s clustering -> triggers (readings D1-D3)
 
 Parity pins: every function above is pinned in tests/test_oracle_*.py against a closed
 form, a library routine (numpy.fft, scipy.signal.welch, scipy.signal.lfilter/torch conv)
