@@ -71,6 +71,19 @@ def block_geometry(block_seconds):
     return n_win, n_raw
 
 
+def rank_block_ids(rank, n_blocks):
+    """Block indices of the record analysed by `rank`: disjoint across ranks (each block is an independent time shard)."""
+    return [rank * 1000 + j for j in range(n_blocks)]
+
+
+def max_over_ranks(t, world):
+    """Element-wise max over ranks of a float64 tensor (the only collective of the run; timing, not data)."""
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t
+
+
 def make_block(index, n_raw):
     from synthdata import coloured_noise
     seed = int(np.random.SeedSequence([1003, index]).generate_state(1)[0])
@@ -271,7 +284,7 @@ def run_ours(args):
     n_win, n_raw = block_geometry(args.block_seconds)
     shifts = [k * FS for k in range(1, N_SLIDES + 1)]
     n_blocks = args.warmup + args.steps
-    blocks_host = [torch.from_numpy(make_block(rank * 1000 + j, n_raw)).pin_memory() for j in range(n_blocks)]
+    blocks_host = [torch.from_numpy(make_block(b, n_raw)).pin_memory() for b in rank_block_ids(rank, n_blocks)]
     blocks_dev = [b.cuda() for b in blocks_host]
     scores_dev = torch.empty((N_SLIDES, n_win), dtype=torch.float32, device="cuda")
     scores_host = torch.empty((N_SLIDES, n_win), dtype=torch.float32).pin_memory()
@@ -321,8 +334,7 @@ def run_ours(args):
             assert torch.isfinite(scores_host).all()
 
     t = torch.tensor([ms_total, (e2e_s if not args.no_e2e else 0.0) * 1e3], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    t = max_over_ranks(t, world)
     ms_total, e2e_ms = float(t[0]), float(t[1])
     livetime = world * args.steps * N_SLIDES * n_win * STRIDE / FS        # strain-seconds, all ranks
     windows = world * args.steps * N_SLIDES * n_win

@@ -166,6 +166,17 @@ aframe_status aframe_score_timeslides_host(aframe_ctx* ctx, const aframe_weights
                                            const int64_t* h_slide_shifts, int32_t n_slides, int64_t batch,
                                            float* h_scores);
 
+/* ---- NEXT-1  post-processing of the score series (readings D1-D3 of DESIGN.md) -------------------------
+ * d_scores [n_series][ld] fp32 (e.g. the [n_slides][n_windows] output of aframe_score_timeslides), n valid per series.
+ * d_integrated [n_series][n]: 1 s top hat = mean of the trailing n_int scores (n_int = inference rate x 1 s = 16;
+ *   the first n_int - 1 entries average the scores that exist), float32 sums in index order.
+ * Triggers: one per consecutive window of n_cluster integrated values (8 s = 128; a trailing partial window counts):
+ *   d_trig_value [n_series][n_trig] = the maximum, d_trig_index [n_series][n_trig] = index of its first occurrence.
+ *   *h_n_trig (HOST) = ceil(n / n_cluster).  The caller sizes the trigger arrays for that. */
+aframe_status aframe_postprocess(aframe_ctx* ctx, const float* d_scores, int64_t n_series, int64_t n, int64_t ld,
+                                 int32_t n_int, int32_t n_cluster, float* d_integrated, float* d_trig_value,
+                                 int64_t* d_trig_index, int64_t* h_n_trig);
+
 /* How many updates of this state were served by replaying the captured CUDA graph (0 if graphs are switched off with
  * the environment variable AFRAME_STREAM_GRAPH=0, or while aframe_profile is on). */
 int64_t aframe_stream_graph_replays(const aframe_stream_state* st);

@@ -54,6 +54,8 @@ EXPORTS = {
     "aframe_stream_destroy": (None, [C.c_void_p]),
     "aframe_stream_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "aframe_launch_count": (C.c_int64, [C.c_void_p]),
+    "aframe_postprocess": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_int32, C.c_int32,
+                                     C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]),
     "aframe_stream_graph_replays": (C.c_int64, [C.c_void_p]),
     "aframe_score_timeslides": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_int64,
                                           C.POINTER(C.c_int64), C.c_int32, C.c_int64, C.c_void_p]),
@@ -233,6 +235,22 @@ class Context:
         self._check(fn(self.handle, weights.handle, _ptr(strain), n, strain.stride(0), int(first), int(n_windows), sh, ns,
                        int(batch), _ptr(scores)))
         return scores
+
+    # ---- NEXT-1: top-hat integration + clustering
+    def postprocess(self, scores, n_int=16, n_cluster=128):
+        """scores [n_series][n] (or [n]) float32 CUDA -> (integrated [n_series][n], trig_value, trig_index [n_series][n_trig])."""
+        _need(scores, torch.float32, "scores")
+        s2 = scores if scores.dim() == 2 else scores[None]
+        ns, n = s2.shape
+        n_trig = -(-n // n_cluster)
+        integ = torch.empty((ns, n), dtype=torch.float32, device=scores.device)
+        val = torch.empty((ns, n_trig), dtype=torch.float32, device=scores.device)
+        idx = torch.empty((ns, n_trig), dtype=torch.int64, device=scores.device)
+        nt = C.c_int64(0)
+        self._check(self.lib.aframe_postprocess(self.handle, _ptr(s2), ns, n, s2.stride(0), int(n_int), int(n_cluster),
+                                                _ptr(integ), _ptr(val), _ptr(idx), C.byref(nt)))
+        assert nt.value == n_trig
+        return integ, val, idx
 
     # ---- per-stage device timing
     def profile(self, enable: bool):
