@@ -95,7 +95,8 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
                          TcLaunch& L) {
   const LayerDesc& l = w->layers[li];
   const int BN = l.c_out >= 256 ? 256 : l.c_out;
-  const bool cg2 = BN == 256 && env_int("AFRAME_CG2", 1) != 0;   // CTA pairs (cta_group::2) for the N = 256 layers
+  const int cg2_mode = env_int("AFRAME_CG2", 1);                 // 1: CTA pairs (cta_group::2) for the N = 256 layers; 2: also N = 128
+  const bool cg2 = (BN == 256 && cg2_mode != 0) || (BN == 128 && cg2_mode >= 2);
   const int T_box = tile_t_box(l.t_out), B_box = 128 / T_box;
   const int P = l.stride;
   const bool has_res = res != nullptr;
@@ -157,21 +158,22 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   //  buffer its chunk's output is staged in)
   const bool r = p.has_res;
   if (cg2 && head)            { p.stages = 5; p.nbuf = 1; p.pf = 0; }
+  else if (cg2 && BN == 128)  { p.stages = r ? 5 : 6; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }   // 24 KB stages
   else if (cg2 && l.k * p.kblocks < 12) { p.stages = 5; p.nbuf = 2; p.pf = r ? 1 : 0; }   // short K: the epilogue is the critical path
   else if (cg2)               { p.stages = r ? 5 : 6; p.nbuf = r ? 2 : 1; p.pf = r ? 1 : 0; }
   else if (BN == 256)         { p.stages = 3; p.nbuf = 2; p.pf = r ? 1 : 0; }
-  else if (halo && BN == 128) { p.stages = 2; p.nbuf = 1; p.pf = 0; }
+  else if (halo && BN == 128) { p.stages = 3; p.nbuf = 2; p.pf = r ? 1 : 0; }   // 96 KB of weights + 3 x 17 KB + 4 x 16 KB
   else if (halo)              { p.stages = r ? 6 : 8; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
   else if (BN == 128)         { p.stages = r ? 4 : 5; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
   else                        { p.stages = r ? 5 : 6; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
   p.w_bytes = halo ? l.k * p.kblocks * BN * 128 : 0;
-  p.stage_bytes = halo ? p.kblocks * TcCfg<64>::HALO_A_BYTES : 0;
+  p.stage_bytes = halo ? TcCfg<64>::HALO_A_BYTES : 0;     // one stage = one 64-channel block
   p.desc_base_offset = env_int("AFRAME_DESC_BO", 0);
   L.BN = BN;
   L.head = head;
   L.cg2 = cg2;
   L.halo = halo;
-  L.smem = halo ? (BN == 128 ? TcCfg<128>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks) : TcCfg<64>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks))
+  L.smem = (cg2 && BN == 128) ? TcCfg<128, true>::smem(p.stages, p.nbuf, false) : halo ? (BN == 128 ? TcCfg<128>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks) : TcCfg<64>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks))
          : cg2 ? TcCfg<256, true>::smem(p.stages, p.nbuf, head) : BN == 256 ? TcCfg<256>::smem(p.stages, p.nbuf, head) : (BN == 128 ? TcCfg<128>::smem(p.stages, p.nbuf, head)
                                                                             : TcCfg<64>::smem(p.stages, p.nbuf, head));
   if (cg2) L.grid = 2 * (p.num_tiles < ctx->n_sms / 2 ? p.num_tiles : ctx->n_sms / 2);
@@ -203,6 +205,7 @@ template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t lau
 }
 
 static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s) {
+  if (L.cg2 && L.BN == 128) return launch_bn<128, false, true>(L, s);
   if (L.cg2) return L.head ? launch_bn<256, true, true>(L, s) : launch_bn<256, false, true>(L, s);
   if (L.head) return launch_bn<256, true, false>(L, s);
   if (L.halo) return L.BN == 128 ? launch_bn<128, false, false, true>(L, s) : launch_bn<64, false, false, true>(L, s);

@@ -88,7 +88,7 @@ template <int BN, bool CG2 = false> struct TcCfg {
   }
   static constexpr int HALO_A_BYTES = 17 * 1024;     // 130 rows x 128 B, padded to the 1024-byte swizzle period
   static constexpr int smem_halo(int stages, int nbuf, int taps, int kblocks) {
-    return tc_fixed_bytes(false) + taps * kblocks * BN * 128 + stages * kblocks * HALO_A_BYTES + EG * nbuf * TC_OUT_BYTES;
+    return tc_fixed_bytes(false) + taps * kblocks * BN * 128 + stages * HALO_A_BYTES + EG * nbuf * TC_OUT_BYTES;
   }
 };
 
@@ -236,18 +236,20 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         int n_idx, t0, b0;
         decode(tile, n_idx, t0, b0);
-        T(0);
-        mbar_wait(empty_bar(stage), phase ^ 1u);
-        T(1);
-        const uint32_t sa = stage_base + stage * STAGE_BYTES;
-        if (elect_one()) {
-          mbar_arrive_expect_tx(full_bar(stage), (uint32_t)(p.kblocks * 130 * 128));
-          for (int kb = 0; kb < p.kblocks; ++kb)   // rows t0 - 1 .. t0 + 128 of the window; out-of-range rows are zero-filled
-            tma_load_4d(sa + kb * Cfg::HALO_A_BYTES, &tm_in, full_bar(stage), kb * 64, 0, t0 - 1, b0);
+        for (int kb = 0; kb < p.kblocks; ++kb) {   // one stage = the 130-row box of one 64-channel block
+          T(0);
+          mbar_wait(empty_bar(stage), phase ^ 1u);
+          T(1);
+          const uint32_t sa = stage_base + stage * STAGE_BYTES;
+          if (elect_one()) {
+            mbar_arrive_expect_tx(full_bar(stage), 130 * 128);
+            // rows t0 - 1 .. t0 + 128 of the window; out-of-range rows are zero-filled
+            tma_load_4d(sa, &tm_in, full_bar(stage), kb * 64, 0, t0 - 1, b0);
+          }
+          __syncwarp();
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+          T(2);
         }
-        __syncwarp();
-        if (++stage == STAGES) { stage = 0; phase ^= 1u; }
-        T(2);
       }
       if (lane == 0) Tflush(0);
     } else {
@@ -301,29 +303,28 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
         if (HALO) {
-          mbar_wait(full_bar(stage), phase);
-          T(2);
-          tc_fence_after();
-          const uint32_t sa = stage_base + stage * STAGE_BYTES;
-          uint32_t first = 0;
-          if (elect_one()) {
-          for (int d = 0; d < p.taps; ++d)
-            for (int kb = 0; kb < p.kblocks; ++kb) {
-              // tap d: rows d .. d + 127 of the 130-row box = descriptor start shifted by d rows of 128 B
-              uint64_t da = umma_desc_sw128(sa + kb * Cfg::HALO_A_BYTES + d * 128);
-              if (p.desc_base_offset) da |= (uint64_t)(d & 7) << 49;
-              const uint64_t db = umma_desc_sw128(w_base + (uint32_t)((d * p.kblocks + kb) * BN * 128));
+          for (int kb = 0; kb < p.kblocks; ++kb) {
+            T(0);
+            mbar_wait(full_bar(stage), phase);
+            T(2);
+            tc_fence_after();
+            if (elect_one()) {
+              const uint32_t a_lo = umma_desc_lo(stage_base + stage * STAGE_BYTES);
+              const uint32_t b_lo = umma_desc_lo(w_base + (uint32_t)(kb * BN * 128));
+              const uint32_t b_tap = (uint32_t)(p.kblocks * BN * 128) >> 4;   // weights [tap][kblock][BN rows][128 B]
+              // tap d: rows d .. d + 127 of the 130-row box = descriptor start shifted by d rows of 128 B (8 units)
 #pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                umma_bf16(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, first);
-                first = 1u;
+              for (int m = 0; m < 12; ++m) {
+                const uint32_t al = a_lo + (m / 4) * 8 + (m % 4) * 2, bl = b_lo + (m / 4) * b_tap + (m % 4) * 2;
+                if (m == 0 && kb == 0) umma_bf16_lohi<false>(d_tmem, al, bl, idesc);
+                else umma_bf16_lohi<true>(d_tmem, al, bl, idesc);
               }
+              umma_commit(empty_bar(stage));
             }
-          umma_commit(empty_bar(stage));
+            __syncwarp();
+            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+            T(3);
           }
-          __syncwarp();
-          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
-          T(3);
         }
         for (int it = 0; it < (HALO ? 0 : kiters); ++it) {
           T(0);
