@@ -376,6 +376,9 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       cudaEventRecord(lev[0], ctx->stream);
     }
     af_prof_begin(ctx, AFRAME_PROF_STEM);
+    // (a tcgen05 formulation of the stem -- three K = 16 MMAs on an im2col tile, pool = max of three accumulators -- was
+    //  built and measured: no faster end to end than this fp32 CUDA-core kernel under the power cap, and less accurate
+    //  because its operands are bf16; it was dropped)
     st = af_launch_stem_bf16(ctx, w->layers[0], w->layers[1], reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz,
                              in_bf16, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1));
     af_prof_end(ctx, AFRAME_PROF_STEM, 1);
