@@ -225,7 +225,7 @@ def latency_run(af, torch, ctx_stream, weights_blob, n_updates, n_warm_scored=10
     upd = torch.from_numpy(np.ascontiguousarray(x.reshape(2, total, STRIDE).transpose(1, 0, 2))).pin_memory()
     dev_in = torch.empty((2, STRIDE), dtype=torch.float32, device="cuda")
     host_out = torch.zeros(2, dtype=torch.float32).pin_memory()
-    wall, dev = [], []
+    wall, dev, kind = [], [], []
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with torch.cuda.stream(ctx_stream):
         for u in range(total):
@@ -242,10 +242,20 @@ def latency_run(af, torch, ctx_stream, weights_blob, n_updates, n_warm_scored=10
             if timed:
                 wall.append(time.perf_counter() - t0)
                 dev.append(ev0.elapsed_time(ev1) * 1e-3)
+                n_now = (u + 1) * STRIDE                       # what this update did besides whitening + scoring
+                kind.append(2 if (n_now >= PSD_LEN and (n_now - PSD_LEN) % 16384 == 0) else (1 if n_now % 2048 == 0 else 0))
     n_scored = int(st.n_scores.item())
     assert n_scored == 1 and np.isfinite(float(host_out[0]))
     wall, dev = np.asarray(wall) * 1e3, np.asarray(dev) * 1e3
+    kind = np.asarray(kind)
+    classes = {}
+    for k, name in ((0, "plain"), (1, "with_welch_segment"), (2, "with_psd_and_filter_update")):
+        sel = kind == k
+        if sel.any():
+            classes[name] = {"share": float(sel.mean()), "p50_ms": float(np.percentile(wall[sel], 50)),
+                             "max_ms": float(wall[sel].max())}
     out = {"workload": "configs[4]: 128 new samples/detector per update, batch 1, bf16 config-1 network",
+           "by_update_kind": classes,
            "updates": int(n_updates), "p50_ms": float(np.percentile(wall, 50)), "p99_ms": float(np.percentile(wall, 99)),
            "device_p50_ms": float(np.percentile(dev, 50)), "device_p99_ms": float(np.percentile(dev, 99)),
            "mean_ms": float(wall.mean()), "timing": "host wall-clock: pinned H2D of the update + aframe_stream_step + "

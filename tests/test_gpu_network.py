@@ -106,3 +106,37 @@ def test_bf16_path_refuses_tables_it_cannot_run(af, config0):
     with pytest.raises(af.AframeError) as e:
         ctx.forward(w, torch.from_numpy(config0["wins"]).cuda())
     assert e.value.status == af.EUNSUPPORTED                     # fails loudly, no silent fallback
+
+
+def test_full_batch_launch_configuration_sampled_against_oracle(af, config1):
+    """The launch configuration bench.py times (4096-window chunks, ragged tail, windows taken in place from a bf16
+    whitened stream at stride 128): sampled scores against the float64 oracle (rule T3), and the big batch against the
+    same windows scored in small batches (bit for bit: a window's score does not depend on its batch)."""
+    n_win = 4096 + 37
+    rng = np.random.default_rng(7)
+    white = rng.standard_normal((2, (n_win - 1) * 128 + 3072)).astype(np.float32)
+    wd = torch.from_numpy(white).cuda().to(torch.bfloat16).contiguous()
+    ctx = af.Context(precision=af.BF16)
+    w = ctx.load_weights(config1["blob"])
+    big = ctx.forward_strided(w, wd, 0, n_win)
+    assert big.shape == (n_win,) and bool(torch.isfinite(big).all())
+    picks = [0, 1, 2047, 4095, 4096, n_win - 1]
+    for i in picks:
+        small = ctx.forward_strided(w, wd, i * 128, 1)
+        assert torch.equal(small[0], big[i])
+    w64 = wd.float().cpu().numpy().astype(np.float64)
+    wins = np.stack([w64[:, i * 128: i * 128 + 3072] for i in picks])
+    ref = onet.forward(config1["net"], wins)
+    assert rel_err(big[picks].cpu().numpy(), ref) <= 2e-2
+
+
+def test_forward_rejects_bad_arguments(af, config1):
+    ctx = af.Context(precision=af.BF16)
+    w = ctx.load_weights(config1["blob"])
+    with pytest.raises(af.AframeError) as e:
+        ctx.forward(w, torch.empty((0, 2, 3072), device="cuda"))
+    assert e.value.status == af.EINVAL
+    other = af.Context(precision=af.BF16)
+    with pytest.raises(af.AframeError) as e:
+        other.forward(w, torch.zeros((1, 2, 3072), device="cuda"))
+    assert e.value.status == af.ESTATE
