@@ -168,3 +168,34 @@ def test_score_timeslides_device_host_and_oracle(af):
     with pytest.raises(af.AframeError) as e:
         ctx.score_timeslides(w, xd, 0, n_win + 2000, shifts, batch=batch)
     assert e.value.status == af.ESHAPE
+
+
+@pytest.mark.parametrize("stride", [512, 32])
+def test_other_inference_rates(af, stride):
+    """NEXT-3 (the paper infers at 4 Hz = stride 512; P:174 studies 1..64 Hz): the streaming state and the strided
+    forward at other strides, tiny network in fp32, against the oracle (flags exactly, scores to rule T2)."""
+    tc = tiny_config()
+    n_updates = 131072 // stride + tc["kernel_len"] // stride + (4 if stride == 512 else 40)
+    x = coloured_noise(n_updates * stride, seed=1002)
+    cfg = ost.StreamConfig(kernel_len=tc["kernel_len"], n_design=4096, stride=stride)
+    blob = make_weight_blob(**tc)
+    so = ost.StreamOracle(cfg, net=onet.parse_blob(blob))
+    ref = [so.step(x[:, u * stride:(u + 1) * stride].astype(np.float64)) for u in range(n_updates)]
+    ctx = af.Context(n_design=4096, kernel_len=tc["kernel_len"], stride=stride, precision=af.FP32)
+    w = ctx.load_weights(blob)
+    st = ctx.stream_create(w)
+    upd = torch.from_numpy(np.ascontiguousarray(x.reshape(2, n_updates, stride).transpose(1, 0, 2))).cuda()
+    flags, scores = [], []
+    for u in range(n_updates):
+        st.step(upd[u])
+        flags.append(int(st.n_scores.item())); scores.append(float(st.score.item()))
+    st.close()
+    flags, scores = np.asarray(flags), np.asarray(scores)
+    np.testing.assert_array_equal(flags, [0 if r is None else 1 for r in ref])
+    want = np.array([r for r in ref if r is not None])
+    assert len(want) >= 4 and rel_err(scores[flags == 1], want) <= 1e-4
+    # offline: rolling whitening + windows in place at this stride = the streamed windows
+    white = ctx.whiten_rolling(torch.from_numpy(x).cuda()).contiguous()
+    n_win = (white.shape[1] - tc["kernel_len"]) // stride + 1
+    off = ctx.forward_strided(w, white, 0, n_win).cpu().numpy()
+    assert n_win == len(want) and rel_err(off, want) <= 1e-4
