@@ -145,7 +145,6 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.head_part = head ? head_part : nullptr;
   p.head_slabs = l.t_out / 32;
   p.nb = nb;
-  p.dbg = env_int("AFRAME_TC_DBG", 0);
   p.dbg_out = nullptr;
   if (env_int("AFRAME_TC_PROF", 0)) {       // experiment: per-role cycle counters, 32 slots per layer, read back by the caller
     static long long* d_prof = nullptr;
@@ -168,7 +167,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   else                        { p.stages = r ? 5 : 6; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
   p.w_bytes = halo ? l.k * p.kblocks * BN * 128 : 0;
   p.stage_bytes = halo ? TcCfg<64>::HALO_A_BYTES : 0;     // one stage = one 64-channel block
-  p.desc_base_offset = env_int("AFRAME_DESC_BO", 0);
+
   L.BN = BN;
   L.head = head;
   L.cg2 = cg2;

@@ -58,12 +58,12 @@ struct TcConvParams {
   int64_t nb;                // windows in this launch (head variant bounds check)
   // HALO variant (k = 3, stride 1, whole 128-row tiles inside one window): the folded weights of the layer stay resident
   // in shared memory (w_bytes) and ONE (128 + 2)-row input box per 64-channel block serves all three taps: tap d reads
-  // the tile through a shared-memory descriptor whose start address is shifted by d rows (d * 128 B).
+  // the tile through a shared-memory descriptor whose start address is shifted by d rows (d * 128 B).  Measured on B200:
+  // the 128-byte swizzle is applied to the absolute shared-memory address, so the shifted start needs no other change
+  // (setting the descriptor's base-offset field to the shift gives wrong results).
   int w_bytes;               // resident weight region (0 unless HALO)
   int stage_bytes;           // bytes per main-loop stage
-  int desc_base_offset;      // experiment: set the descriptor's base-offset field to the row shift (d & 7)
   long long* dbg_out;        // timing experiments: per-role cycle counters of CTA 0 (null = off)
-  int dbg;                   // timing experiments only (wrong results): 1 = no TMA loads, 2 = epilogue drains TMEM only
 };
 
 // shared-memory carve-up (bytes from the 1024-aligned start of dynamic shared memory):
@@ -267,9 +267,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             T(1);
             const uint32_t sa = stage_base + stage * STAGE_BYTES;
             if (elect_one()) {
-              if (p.dbg & 1) {
-                if (rank == 0) mbar_arrive(full_bar(stage));
-              } else if (CG2) {
+              if (CG2) {
                 // both CTAs load their own A rows and their half of B; all bytes are counted on the leader's barrier
                 if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * Cfg::STAGE_BYTES);
                 const uint32_t lbar = lfull0 + 8u * stage;
@@ -336,7 +334,6 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           if (elect_one()) {
 #pragma unroll
           for (int k = 0; k < 4; ++k) { // 4 x (K = 16 bf16 = 32 B) inside the 128-byte swizzle row
-            if (p.dbg & 8) continue;
             if (CG2) umma_bf16_cg2(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
             else umma_bf16(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
           }
@@ -435,7 +432,6 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             else mbar_arrive(tempty_bar(acc));
           }
         }
-        if (p.dbg & 2) { if (p.has_res) mbar_wait(res_bar(g, buf), (j / NBUF) & 1u); named_bar_sync(1 + g, 128); continue; }
         if (p.has_res) mbar_wait(res_bar(g, buf), (j / NBUF) & 1u);
         T(5);
         const float4* bias4 = reinterpret_cast<const float4*>(s_bias + n0 + c * 64);
@@ -461,7 +457,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           T(6);
           fence_proxy_async_smem();                // generic-proxy writes -> visible to the TMA store
           named_bar_sync(1 + g, 128);
-          if (leader && !(p.dbg & 4)) {
+          if (leader) {
             tma_store_4d(&tm_out, sbuf, n0 + c * 64, 0, t0, b0);
             tma_store_commit();
           }
