@@ -40,7 +40,7 @@ def parse_blob(blob: bytes):
         l = dict(kind=kind, c_in=c_in, c_out=c_out, k=k, stride=stride, pad=pad, relu=relu,
                  input_from=inp, residual_from=res)
         if kind == KIND_CONV:
-            n_stat = c_out if norm_kind == 0 else n_groups
+            n_stat = c_out if norm_kind == 0 else (n_groups if norm_kind == 1 else 0)
             l["W"] = data[pos: pos + c_out * c_in * k].reshape(c_out, c_in, k); pos += c_out * c_in * k
             l["gamma"] = data[pos: pos + c_out]; pos += c_out
             l["beta"] = data[pos: pos + c_out]; pos += c_out
@@ -59,6 +59,18 @@ def stat_index(c_out, norm_kind, n_groups):
     """Channel -> index of its statistics: c (per-channel) or c // (C / n_groups) (reading B6)."""
     c = np.arange(c_out)
     return c if norm_kind == 0 else c // (c_out // n_groups)
+
+
+def group_norm_live(z, gamma, beta, n_groups, eps):
+    """True GroupNorm ("replace standard Batch Normalization layers with Group Normalization"; NEXT-2): per window
+    and per group of C / n_groups consecutive channels, mean and (biased) variance over the group's channels and all
+    time steps; y = (z - mu) / sqrt(var + eps) * gamma_c + beta_c.   z [B][C][T]."""
+    b, c, t = z.shape
+    zg = z.reshape(b, n_groups, (c // n_groups) * t)
+    mu = zg.mean(axis=2, keepdims=True)
+    var = ((zg - mu) ** 2).mean(axis=2, keepdims=True)
+    y = ((zg - mu) / np.sqrt(var + eps)).reshape(b, c, t)
+    return y * gamma[None, :, None] + beta[None, :, None]
 
 
 def fold_norm(layer, norm_kind, n_groups, eps):
@@ -130,7 +142,9 @@ def forward(net, windows, folded=True, act_round=None, weight_round=None, keep=F
     for li, l in enumerate(net["layers"]):
         src = x0 if l["input_from"] < 0 else outs[l["input_from"]]
         if l["kind"] == KIND_CONV:
-            if folded:
+            if nk == 2:                            # true GroupNorm: nothing to fold
+                y = group_norm_live(conv1d(src, l["W"], l["stride"], l["pad"]), l["gamma"], l["beta"], ng, eps)
+            elif folded:
                 w, bias = fold_norm(l, nk, ng, eps)
                 if weight_round is not None and l["input_from"] >= 0:
                     w = weight_round(w)

@@ -10,7 +10,8 @@ the oracle and the CUDA library each fold the norm themselves.
 Blob format (little endian), version 1
 --------------------------------------
 header, 32 bytes : u32 magic 'AFRW' (0x57524641), u32 version=1, u32 n_layers,
-                   u32 norm_kind (0 = per-channel statistics, 1 = per-group statistics),
+                   u32 norm_kind (0 = frozen per-channel statistics, 1 = frozen per-group statistics,
+                                  2 = true GroupNorm: statistics computed per window at inference, NEXT-2),
                    u32 n_groups (norm_kind 1 only), f32 eps, u32 in_channels, u32 reserved
 layer table      : n_layers x 12 x i32:
                    kind (0 conv+norm, 1 maxpool, 2 head = global-avg-pool + linear),
@@ -19,7 +20,7 @@ layer table      : n_layers x 12 x i32:
                    residual_from (-1 = none; added after the norm, before the ReLU),
                    3 reserved
 payload (f32)    : per conv layer, in table order: W[c_out][c_in][k], gamma[c_out], beta[c_out],
-                   mean[n_stat], var[n_stat]   (n_stat = c_out or n_groups)
+                   mean[n_stat], var[n_stat]   (n_stat = c_out or n_groups; norm_kind 2: n_stat = 0, no statistics stored)
                    per head layer: w[c_in], b[1]
 """
 from __future__ import annotations
@@ -31,7 +32,7 @@ import numpy as np
 
 MAGIC = 0x57524641
 KIND_CONV, KIND_MAXPOOL, KIND_HEAD = 0, 1, 2
-NORM_CHANNEL, NORM_GROUP = 0, 1
+NORM_CHANNEL, NORM_GROUP, NORM_GROUP_LIVE = 0, 1, 2
 
 
 @dataclass
@@ -82,6 +83,12 @@ def full_config():
                 norm_kind=NORM_GROUP, n_groups=8, seed=1, kernel_len=3072)
 
 
+def tiny_config_live_gn():
+    """NEXT-2: the tiny network with true GroupNorm (8 groups, statistics per window at inference)."""
+    return dict(table=resnet_layer_table(2, 8, 7, [1, 1, 1, 1], [8, 16, 32, 64]),
+                norm_kind=NORM_GROUP_LIVE, n_groups=8, seed=2, kernel_len=2048)
+
+
 def make_weight_blob(table, norm_kind, n_groups, seed, eps=1e-5, in_channels=2, **_unused) -> bytes:
     """He-normal (fan-in) conv weights, frozen norm statistics (reading B6/B7), head w ~ N(0, 1/C)."""
     rng = np.random.Generator(np.random.PCG64(seed))
@@ -94,7 +101,7 @@ def make_weight_blob(table, norm_kind, n_groups, seed, eps=1e-5, in_channels=2, 
     for i, l in enumerate(table):
         tab[i, :9] = [l.kind, l.c_in, l.c_out, l.k, l.stride, l.pad, l.relu, l.input_from, l.residual_from]
         if l.kind == KIND_CONV:
-            n_stat = l.c_out if norm_kind == NORM_CHANNEL else n_groups
+            n_stat = l.c_out if norm_kind == NORM_CHANNEL else (n_groups if norm_kind == NORM_GROUP else 0)
             w = rng.standard_normal((l.c_out, l.c_in, l.k)) * np.sqrt(2.0 / (l.c_in * l.k))
             gamma = 1.0 + 0.1 * rng.standard_normal(l.c_out)
             beta = 0.1 * rng.standard_normal(l.c_out)

@@ -146,3 +146,33 @@ def test_round_bf16_matches_torch():
     x = RNG.standard_normal(1000) * 10
     ref = torch.from_numpy(x).float().bfloat16().double().numpy()
     np.testing.assert_array_equal(onet.round_bf16(x), ref)
+
+
+def test_live_group_norm_matches_library_and_is_scale_invariant():
+    """NEXT-2 pin: oracle.group_norm_live = torch.nn.functional.group_norm (library routine); the normalised output does
+    not change when the window's pre-norm tensor is rescaled (eps -> 0)."""
+    import torch
+    from oracle import network as onet
+    rng = np.random.default_rng(5)
+    z = rng.standard_normal((3, 16, 40))
+    gamma, beta = rng.standard_normal(16), rng.standard_normal(16)
+    got = onet.group_norm_live(z, gamma, beta, 8, 1e-5)
+    ref = torch.nn.functional.group_norm(torch.from_numpy(z), 8, torch.from_numpy(gamma), torch.from_numpy(beta), 1e-5).numpy()
+    np.testing.assert_allclose(got, ref, rtol=1e-12, atol=1e-12)
+    np.testing.assert_allclose(onet.group_norm_live(z * 37.0, gamma, beta, 8, 0.0), onet.group_norm_live(z, gamma, beta, 8, 0.0),
+                               rtol=1e-10, atol=1e-10)
+
+
+def test_live_group_norm_network_runs_and_differs_from_folded():
+    from oracle import network as onet
+    from synthdata import make_weight_blob, tiny_config_live_gn
+    cfg = tiny_config_live_gn()
+    net = onet.parse_blob(make_weight_blob(**cfg))
+    assert net["norm_kind"] == 2 and net["layers"][0]["mean"].size == 0
+    rng = np.random.default_rng(6)
+    x = rng.standard_normal((2, 2, 2048))
+    s = onet.forward(net, x)
+    assert s.shape == (2,) and np.all(np.isfinite(s))
+    # per-window statistics: scaling one window's input leaves its score (almost) unchanged, unlike a frozen norm
+    s2 = onet.forward(net, x * np.array([1.0, 8.0])[:, None, None])
+    assert abs(s2[1] - s[1]) < 1e-3 * max(1.0, abs(s[1])) and s2[0] == s[0]
