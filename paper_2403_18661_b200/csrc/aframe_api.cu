@@ -233,6 +233,8 @@ AF_API void aframe_weights_free(aframe_weights* w) {
   for (float* p : w->d_w32) cudaFree(p);
   for (__nv_bfloat16* p : w->d_w16) cudaFree(p);
   for (float* p : w->d_bias) cudaFree(p);
+  for (float* p : w->d_gamma) cudaFree(p);
+  for (float* p : w->d_beta) cudaFree(p);
   cudaFree(w->d_head_w);
   cudaGetLastError();
   delete w;
@@ -247,8 +249,8 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
   if (hd[0] != 0x57524641u || hd[1] != 1u) return af_fail(ctx, AFRAME_EINVAL, "bad weight blob magic/version");
   const uint32_t n_layers = hd[2], norm_kind = hd[3], n_groups = hd[4], in_ch = hd[6];
   float eps; memcpy(&eps, &hd[5], 4);
-  if (n_layers == 0 || n_layers > 4096 || norm_kind > 1) return af_fail(ctx, AFRAME_EINVAL, "bad weight blob header");
-  if (norm_kind == 1 && n_groups == 0) return af_fail(ctx, AFRAME_EINVAL, "group norm with zero groups");
+  if (n_layers == 0 || n_layers > 4096 || norm_kind > 2) return af_fail(ctx, AFRAME_EINVAL, "bad weight blob header");
+  if (norm_kind >= 1 && n_groups == 0) return af_fail(ctx, AFRAME_EINVAL, "group norm with zero groups");
   if ((int)in_ch != ctx->cfg.n_channels) return af_fail(ctx, AFRAME_ESHAPE, "blob in_channels != cfg.n_channels");
   const size_t tab_off = 32, pay_off = 32 + (size_t)n_layers * 48;
   if (bytes < pay_off) return af_fail(ctx, AFRAME_ESHAPE, "weight blob shorter than its layer table");
@@ -265,6 +267,11 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
   w->d_w32.assign(n_layers, nullptr);
   w->d_w16.assign(n_layers, nullptr);
   w->d_bias.assign(n_layers, nullptr);
+  w->d_gamma.assign(n_layers, nullptr);
+  w->d_beta.assign(n_layers, nullptr);
+  w->live_gn = norm_kind == 2;
+  w->n_groups = (int)n_groups;
+  w->gn_eps = eps;
   aframe_status st = AFRAME_OK;
   size_t pos = 0;
   auto fail = [&](aframe_status s, const char* msg) { st = af_fail(ctx, s, msg); };
@@ -302,8 +309,8 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
       const LayerDesc& rs = w->layers[l.residual_from];
       if (rs.kind == 2 || rs.c_out != l.c_out || rs.t_out != l.t_out) { fail(AFRAME_ESHAPE, "layer table: residual shape mismatch"); break; }
     }
-    const int n_stat = norm_kind == 0 ? l.c_out : (int)n_groups;
-    if (norm_kind == 1 && l.c_out % (int)n_groups) { fail(AFRAME_ESHAPE, "c_out not divisible by n_groups"); break; }
+    const int n_stat = norm_kind == 0 ? l.c_out : (norm_kind == 1 ? (int)n_groups : 0);
+    if (norm_kind >= 1 && l.c_out % (int)n_groups) { fail(AFRAME_ESHAPE, "c_out not divisible by n_groups"); break; }
     const size_t nw = (size_t)l.c_out * l.c_in * l.k;
     if (pos + nw + 2 * (size_t)l.c_out + 2 * (size_t)n_stat > n_pay) { fail(AFRAME_ESHAPE, "weight blob payload too short"); break; }
     const float* W = pay + pos;
@@ -317,8 +324,9 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
     std::vector<__nv_bfloat16> w16(nw);
     for (int co = 0; co < l.c_out; ++co) {
       const int g = norm_kind == 0 ? co : co / (l.c_out / (int)n_groups);
-      const double a = (double)gamma[co] / sqrt((double)var[g] + (double)eps);
-      bias[co] = (float)((double)beta[co] - (double)mean[g] * a);
+      // frozen norm: fold; true GroupNorm: the conv stays as it is (the norm kernels apply gamma / beta)
+      const double a = norm_kind == 2 ? 1.0 : (double)gamma[co] / sqrt((double)var[g] + (double)eps);
+      bias[co] = norm_kind == 2 ? 0.f : (float)((double)beta[co] - (double)mean[g] * a);
       for (int ci = 0; ci < l.c_in; ++ci)
         for (int d = 0; d < l.k; ++d) {
           const float v = (float)((double)W[((size_t)co * l.c_in + ci) * l.k + d] * a);
@@ -331,12 +339,18 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
     if (cudaMemcpy(w->d_w32[i], w32.data(), sizeof(float) * nw, cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(w->d_w16[i], w16.data(), 2 * nw, cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(w->d_bias[i], bias.data(), sizeof(float) * l.c_out, cudaMemcpyHostToDevice) != cudaSuccess) { fail(AFRAME_ECUDA, "weight upload failed"); break; }
+    if (norm_kind == 2) {
+      if (cudaMalloc(&w->d_gamma[i], sizeof(float) * l.c_out) != cudaSuccess || cudaMalloc(&w->d_beta[i], sizeof(float) * l.c_out) != cudaSuccess) { fail(AFRAME_ENOMEM, "device allocation failed"); break; }
+      if (cudaMemcpy(w->d_gamma[i], gamma, sizeof(float) * l.c_out, cudaMemcpyHostToDevice) != cudaSuccess ||
+          cudaMemcpy(w->d_beta[i], beta, sizeof(float) * l.c_out, cudaMemcpyHostToDevice) != cudaSuccess) { fail(AFRAME_ECUDA, "weight upload failed"); break; }
+    }
   }
   if (st == AFRAME_OK && w->head_layer < 0) st = af_fail(ctx, AFRAME_ESHAPE, "layer table has no head");
   if (st == AFRAME_OK && pos != n_pay) st = af_fail(ctx, AFRAME_ESHAPE, "weight blob payload size mismatch");
   if (st == AFRAME_OK && cudaDeviceSynchronize() != cudaSuccess) st = af_fail(ctx, AFRAME_ECUDA, "sync after weight upload failed");
   if (st != AFRAME_OK) { cudaGetLastError(); aframe_weights_free(w); return st; }
   af_tc_check(ctx, w);
+  if (w->live_gn) { w->tc_ok = false; w->tc_reason = "true GroupNorm (norm_kind 2) is built on the fp32 path only"; }
   *out = w;
   return AFRAME_OK;
 }

@@ -35,6 +35,11 @@ struct aframe_weights {
   float* d_head_w = nullptr;          // [c_in]
   float head_b = 0.f;
   int head_layer = -1;
+  // NEXT-2: true GroupNorm (blob norm_kind 2): statistics per window at inference, fp32 path only
+  bool live_gn = false;
+  int n_groups = 0;
+  float gn_eps = 0.f;
+  std::vector<float*> d_gamma, d_beta;   // per conv layer [c_out] (live_gn only)
   bool tc_ok = false;                 // bf16 tensor-core path available for this table
   std::string tc_reason;
 };

@@ -98,6 +98,47 @@ __global__ void __launch_bounds__(256) conv_fp32_kernel(const ConvArgs a) {
   }
 }
 
+// NEXT-2, true GroupNorm: per (window, group) mean and biased variance over the group's channels and all time
+// steps of the conv output z [B][T][C]; then y = (z - mu) rstd gamma_c + beta_c (+ residual) (ReLU), in place.
+__global__ void __launch_bounds__(256) gn_stats_kernel(const float* __restrict__ z, int T, int C, int G, float eps,
+                                                       float2* __restrict__ stats /*[B][G] (mu, rstd)*/) {
+  __shared__ double rs[8], rq[8];
+  const int64_t b = blockIdx.x;
+  const int g = blockIdx.y;
+  const int cg = C / G;
+  const float* zb = z + b * (int64_t)T * C + g * cg;
+  double s = 0.0, q = 0.0;
+  for (int i = threadIdx.x; i < T * cg; i += blockDim.x) {
+    const double v = (double)zb[(int64_t)(i / cg) * C + (i % cg)];
+    s += v; q += v * v;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); q += __shfl_xor_sync(0xffffffffu, q, o); }
+  if ((threadIdx.x & 31) == 0) { rs[threadIdx.x >> 5] = s; rq[threadIdx.x >> 5] = q; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double ts = 0.0, tq = 0.0;
+    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) { ts += rs[i]; tq += rq[i]; }
+    const double n = (double)T * cg, mu = ts / n;
+    const double var = tq / n - mu * mu;
+    stats[b * G + g] = make_float2((float)mu, (float)(1.0 / sqrt((var > 0.0 ? var : 0.0) + (double)eps)));
+  }
+}
+
+__global__ void gn_apply_kernel(float* __restrict__ z, const float2* __restrict__ stats, const float* __restrict__ gamma,
+                                const float* __restrict__ beta, const float* __restrict__ res, int64_t total, int T, int C,
+                                int G, int relu) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int c = (int)(i % C);
+  const int64_t b = i / ((int64_t)T * C);
+  const float2 st = stats[b * G + c / (C / G)];
+  float v = (z[i] - st.x) * st.y * gamma[c] + beta[c];
+  if (res) v += res[i];
+  if (relu) v = fmaxf(v, 0.f);
+  z[i] = v;
+}
+
 __global__ void maxpool_fp32_kernel(const float* __restrict__ in, float* __restrict__ out, int64_t total, int T_in,
                                     int T_out, int C, int k, int stride, int pad) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -184,7 +225,8 @@ aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const vo
   af_make_plan(w, false, plan);
   const int64_t chunk = 128;
   const size_t slot_bytes = plan.slot_elems * sizeof(float) * (size_t)(B < chunk ? B : chunk);
-  aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots);
+  const size_t stats_bytes = w->live_gn ? sizeof(float2) * (size_t)chunk * w->n_groups : 0;
+  aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots + stats_bytes);
   if (st != AFRAME_OK) return st;
   char* base = reinterpret_cast<char*>(ctx->ws_act.ptr);
   const int n = (int)w->layers.size();
@@ -197,10 +239,11 @@ aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const vo
       if (l.kind == 0) {
         ConvArgs a;
         a.w = w->d_w32[i]; a.bias = w->d_bias[i];
-        a.res = l.residual_from >= 0 ? reinterpret_cast<float*>(base + slot_bytes * plan.slot[l.residual_from]) : nullptr;
+        const float* res_ptr = l.residual_from >= 0 ? reinterpret_cast<float*>(base + slot_bytes * plan.slot[l.residual_from]) : nullptr;
+        a.res = w->live_gn ? nullptr : res_ptr;          // true GroupNorm: residual and ReLU come after the norm
         a.out = dst; a.rows = nb * l.t_out;
         a.T_in = l.t_in; a.T_out = l.t_out; a.C_in = l.c_in; a.C_out = l.c_out;
-        a.k = l.k; a.stride = l.stride; a.pad = l.pad; a.relu = l.relu;
+        a.k = l.k; a.stride = l.stride; a.pad = l.pad; a.relu = w->live_gn ? 0 : l.relu;
         dim3 grid((unsigned)((a.rows + 63) / 64), (unsigned)((l.c_out + 63) / 64));
         const int pk = l.input_from < 0 ? AFRAME_PROF_STEM : AFRAME_PROF_CONV;
         af_prof_begin(ctx, pk);
@@ -217,6 +260,16 @@ aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const vo
         }
         af_prof_end(ctx, pk, 1);
         AF_LAUNCH_CHECK(ctx);
+        if (w->live_gn) {
+          float2* stats = reinterpret_cast<float2*>(base + slot_bytes * plan.n_slots);
+          gn_stats_kernel<<<dim3((unsigned)nb, (unsigned)w->n_groups), 256, 0, ctx->stream>>>(dst, l.t_out, l.c_out, w->n_groups,
+                                                                                             w->gn_eps, stats);
+          AF_LAUNCH_CHECK(ctx);
+          const int64_t total = nb * l.t_out * l.c_out;
+          gn_apply_kernel<<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(dst, stats, w->d_gamma[i], w->d_beta[i], res_ptr,
+                                                                                    total, l.t_out, l.c_out, w->n_groups, l.relu);
+          AF_LAUNCH_CHECK(ctx);
+        }
       } else if (l.kind == 1) {
         if (!src) return af_fail(ctx, AFRAME_EUNSUPPORTED, "max-pool directly on the network input is not supported");
         const int64_t total = nb * l.t_out * l.c_out;

@@ -140,3 +140,23 @@ def test_forward_rejects_bad_arguments(af, config1):
     with pytest.raises(af.AframeError) as e:
         other.forward(w, torch.zeros((1, 2, 3072), device="cuda"))
     assert e.value.status == af.ESTATE
+
+
+def test_true_group_norm_fp32_matches_oracle(af, config0):
+    """NEXT-2: GroupNorm statistics computed per window at inference (blob norm_kind 2) on the fp32 path against
+    the oracle (rule T2); the bf16 tensor-core path refuses such a table loudly."""
+    from synthdata import tiny_config_live_gn
+    cfg = tiny_config_live_gn()
+    blob = make_weight_blob(**cfg)
+    wins = config0["wins"][:16].copy()
+    wins[3] *= 5.0                                              # statistics are per window: a rescaled window is fine
+    ref = onet.forward(onet.parse_blob(blob), wins)
+    ctx = af.Context(n_design=4096, kernel_len=2048, precision=af.FP32)
+    w = ctx.load_weights(blob)
+    got = ctx.forward(w, torch.from_numpy(wins).cuda()).cpu().numpy()
+    assert rel_err(got, ref) <= 1e-4
+    ctx16 = af.Context(n_design=4096, kernel_len=2048, precision=af.BF16)
+    w16 = ctx16.load_weights(blob)
+    with pytest.raises(af.AframeError) as e:
+        ctx16.forward(w16, torch.from_numpy(wins).cuda())
+    assert e.value.status == af.EUNSUPPORTED
