@@ -391,7 +391,11 @@ def run_ours(args):
         gbs = args.steps * 2 * n_out_block * (4 + 2) / (wh_ms * 1e-3) / 1e9      # fp32 in + bf16 out per sample
         out["roofline_whiten"] = {"kernel": "whiten_os_kernel", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"],
                                   "unit": "GB/s", "frac": gbs / peaks["hbm"], "traffic": None,
-                                  "algorithmic": "4 B in + 2 B (bf16) out per whitened sample per channel"}
+                                  "algorithmic": "4 B in + 2 B (bf16) out per whitened sample per channel",
+                                  # the binding resource: two 4096-point complex FFTs + untangle per 6144
+                                  # valid samples = 94 flop per sample, against 148 SMs x 128 lanes x 2 x 1.965 GHz
+                                  "alu": {"bound": "alu", "achieved": 94.0 * gbs / 6.0 / 1e3, "peak": 148 * 128 * 2 * 1.965e9 / 1e12,
+                                          "unit": "TFLOP/s fp32", "frac": (94.0 * gbs / 6.0 / 1e3) / (148 * 128 * 2 * 1.965e9 / 1e12)}}
     we_ms = stages["welch"][0]
     if we_ms > 0:
         gbs = args.steps * 2 * n_raw * 4 / (we_ms * 1e-3) / 1e9                   # every raw sample enters the PSD once
