@@ -26,6 +26,7 @@ struct aframe_stream_state {
   // so the same graph serves every update).
   cudaGraphExec_t graph = nullptr;
   const float* g_in = nullptr; float* g_scores = nullptr; int32_t* g_n = nullptr;
+  void* g_ws = nullptr;          // activation workspace the captured launches point into
   int64_t g_launches = 0;        // kernels per replay
   int64_t replays = 0;
 };
@@ -184,7 +185,9 @@ AF_API aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samp
   if (!stream_graph_enabled() || ctx->prof_on || ctx->layer_ms || cap != cudaStreamCaptureStatusNone ||
       ctx->stream == nullptr || ctx->stream == cudaStreamLegacy)
     return stream_step_enqueue(ctx, d_new_samples, st, d_scores, d_n_scores);
-  if (!st->graph || st->g_in != d_new_samples || st->g_scores != d_scores || st->g_n != d_n_scores) {
+  // (a larger forward on the same context may have re-allocated the activation workspace since the capture)
+  if (!st->graph || st->g_in != d_new_samples || st->g_scores != d_scores || st->g_n != d_n_scores ||
+      st->g_ws != ctx->ws_act.ptr) {
     if (st->graph) { cudaGraphExecDestroy(st->graph); st->graph = nullptr; }
     const int64_t l0 = ctx->launches;
     AF_CUDA(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
@@ -199,6 +202,7 @@ AF_API aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samp
     cudaGraphDestroy(g);
     if (e != cudaSuccess) { st->graph = nullptr; cudaGetLastError(); return af_fail(ctx, AFRAME_ECUDA, "graph instantiation failed: %s", cudaGetErrorString(e)); }
     st->g_in = d_new_samples; st->g_scores = d_scores; st->g_n = d_n_scores;
+    st->g_ws = ctx->ws_act.ptr;
   }
   AF_CUDA(ctx, cudaGraphLaunch(st->graph, ctx->stream));
   ctx->launches += st->g_launches;

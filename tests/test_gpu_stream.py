@@ -124,6 +124,20 @@ def test_stream_graph_replay_equals_direct_launches(af):
             torch.cuda.current_stream().synchronize()
         out[name] = (scores, st.uses_graph)
         st.close()
+    # a large forward on the graph context re-allocates its activation workspace: the next update must re-capture
+    big = ctx.forward(w, torch.randn(64, 2, 3072, device="cuda"))
+    st2 = ctx.stream_create(w)
+    with torch.cuda.stream(stream):
+        for u in range(3):
+            buf.copy_(upd[u], non_blocking=True)
+            st2.step(buf)
+        ctx.forward(w, torch.randn(700, 2, 3072, device="cuda"))       # grows the workspace
+        for u in range(3, 6):
+            buf.copy_(upd[u], non_blocking=True)
+            st2.step(buf)
+        stream.synchronize()
+    assert int(st2.n_scores.item()) == 0 and bool(torch.isfinite(big).all())
+    st2.close()
     assert out["graph"][1] and not out["direct"][1]
     assert out["graph"][0] == out["direct"][0] and all(f == 1 for f, _ in out["graph"][0])
 
