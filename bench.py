@@ -378,7 +378,10 @@ def run_ours(args):
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": {"kernel": "conv_tc_kernel<BN> (35 residual-stage convolutions, tcgen05 implicit GEMM)",
                      "bound": "tensor", "achieved": conv_tflops, "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
-                     "frac": conv_tflops / peaks["bf16_sustained"], "traffic": None,
+                     "frac": conv_tflops / peaks["bf16_sustained"],
+                     # dram__bytes_read.sum + dram__bytes_write.sum of the 32 conv launches of one 4096-window batch under
+                     # ncu --set full (profiles/r01c_conv_full.md): 28.9 GB, i.e. per launch on average
+                     "traffic": 28.9e9 / 32,
                      "peak_kind": "sustained bf16 cuBLAS, " + peaks["source"], "launches": int(conv_launches),
                      "avg_launch_ms": conv_ms / max(conv_launches, 1),
                      "algorithmic": "2 x 1069.5 MMAC per window x windows scored, over the summed CUDA-event time of "

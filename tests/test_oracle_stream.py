@@ -9,6 +9,28 @@ from synthdata import coloured_noise
 FS = 2048
 
 
+def _golden():
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                name, value = line.split()[:2]
+                out[name] = float(value)
+    return out
+
+
+def test_golden_paper_constants_are_mutually_consistent_and_match_the_defaults():
+    g = _golden()
+    assert g["training_window"] == g["training_psd_length"] + g["training_whitened_length"]          # 10.5 = 8 + 2.5
+    assert g["training_whitened_length"] - 2 * g["whitening_crop_per_edge"] == g["kernel_length"]    # 2.5 - 1 = 1.5
+    assert g["window_shift"] == 1.0 / g["inference_rate"]
+    assert g["kernel_length"] - g["window_shift"] == g["window_overlap"]
+    cfg = ost.StreamConfig()
+    assert cfg.fs == g["sample_rate"] and cfg.kernel_len == g["kernel_length"] * cfg.fs
+    assert cfg.filter_len == 2 * g["whitening_crop_per_edge"] * cfg.fs and cfg.psd_len == g["inference_psd_length"] * cfg.fs
+
+
 def test_paper_geometry_constants():
     # 10.5 s = 8 s PSD + 2.5 s whitened; 0.5 s cropped per edge -> 1.5 s analysed
     assert 10.5 * FS == 8 * FS + 2.5 * FS
