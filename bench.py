@@ -407,6 +407,23 @@ def run_ours(args):
                                  "algorithmic": "4 B per raw sample per channel (each sample is in two 50 %-overlapped "
                                                 "segments; the second read is an L2 hit); DESIGN.md section 5 derives the fp32-ALU "
                                                 "bound that caps both FFT kernels below the HBM roofline"}
+    # NEXT-1: 1 s top-hat integration + 8 s clustering of the step's scores, on the device
+    with torch.cuda.stream(stream):
+        for _ in range(3):
+            ctx.postprocess(scores_dev)
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record(stream)
+        for _ in range(20):
+            integ, tval, tidx = ctx.postprocess(scores_dev)
+        p1.record(stream)
+        stream.synchronize()
+    pp_ms = p0.elapsed_time(p1) / 20
+    pp_bytes = scores_dev.numel() * 8 + scores_dev.numel() * 4 + tval.numel() * 12     # scores in, integrated out + in, triggers out
+    out["postprocess"] = {"kernel": "tophat_kernel + cluster_max_kernel (NEXT-1)", "ms_per_step": pp_ms,
+                          "scores": int(scores_dev.numel()), "triggers": int(tval.numel()), "bound": "hbm",
+                          "achieved": pp_bytes / (pp_ms * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
+                          "frac": pp_bytes / (pp_ms * 1e-3) / 1e9 / peaks["hbm"],
+                          "note": "2 launches over 2 MB of scores: launch-latency bound, 0.001 % of a step"}
     if args.latency_updates > 0 and world == 1:
         out["latency"] = latency_run(af, torch, stream, blob, args.latency_updates)
     if not args.no_cpu_baseline:
