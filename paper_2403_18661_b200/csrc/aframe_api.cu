@@ -350,7 +350,6 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
   if (st == AFRAME_OK && cudaDeviceSynchronize() != cudaSuccess) st = af_fail(ctx, AFRAME_ECUDA, "sync after weight upload failed");
   if (st != AFRAME_OK) { cudaGetLastError(); aframe_weights_free(w); return st; }
   af_tc_check(ctx, w);
-  if (w->live_gn) { w->tc_ok = false; w->tc_reason = "true GroupNorm (norm_kind 2) is built on the fp32 path only"; }
   *out = w;
   return AFRAME_OK;
 }

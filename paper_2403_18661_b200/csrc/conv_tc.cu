@@ -86,6 +86,9 @@ aframe_status af_tc_check(aframe_ctx* ctx, aframe_weights* w) {
     if (l.kind == 1) { w->tc_reason = "max-pool after the stem is not built on the bf16 path"; return AFRAME_OK; }
     if (l.kind == 0 && !tc_layer_ok(l, w->tc_reason)) return AFRAME_OK;
   }
+  if (w->live_gn && (w->n_groups < 1 || w->n_groups > 32 || 64 % w->n_groups || (64 / w->n_groups) % 2)) {
+    w->tc_reason = "true GroupNorm on the bf16 path needs an even number of stem channels per group"; return AFRAME_OK;
+  }
   w->tc_ok = true;
   return AFRAME_OK;
 }
@@ -139,7 +142,8 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.num_tiles = (int)((cg2 ? (m_tiles + 1) / 2 : m_tiles) * p.n_tiles);
   p.div_n = tc_fastdiv((uint32_t)p.n_tiles);
   p.div_t = tc_fastdiv((uint32_t)p.t_blks);
-  p.relu = l.relu; p.has_res = res != nullptr;
+  // true GroupNorm (NEXT-2): the conv stores its plain output; norm, residual and ReLU follow in af_launch_gn_bf16
+  p.relu = w->live_gn ? 0 : l.relu; p.has_res = res != nullptr;
   p.c_out = l.c_out;
   p.head_w = head ? w->d_head_w : nullptr;
   p.head_part = head ? head_part : nullptr;
@@ -327,12 +331,13 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     for (int i = 0; only_consumer && i < n - 1; ++i)
       if (w->layers[i].input_from == src || w->layers[i].residual_from == src) only_consumer = false;
     if (only_consumer && w->layers[src].c_out % 256 == 0 && w->layers[src].c_out <= 512 && tile_t_box(w->layers[src].t_out) % 32 == 0 &&
-        env_int("AFRAME_FUSE_HEAD", 1)) {
+        env_int("AFRAME_FUSE_HEAD", 1) && !w->live_gn) {
       fuse = src;
       n_part = (w->layers[src].t_out / 32) * (w->layers[src].c_out / 64);
     }
   }
-  const size_t part_bytes = (sizeof(float) * (size_t)n_part * chunk + 1023) & ~(size_t)1023;
+  const size_t part_bytes = w->live_gn ? ((sizeof(float2) * (size_t)w->n_groups * chunk + 1023) & ~(size_t)1023)   // (mu, rstd)
+                                       : ((sizeof(float) * (size_t)n_part * chunk + 1023) & ~(size_t)1023);
   aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots + part_bytes);
   if (st != AFRAME_OK) return st;
   char* base = reinterpret_cast<char*>(ctx->ws_act.ptr);
@@ -353,7 +358,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       pc->launches.resize(n);
       pc->blocks.resize(n);
       pc->fused_with.assign(n, -1);
-      if (env_int("AFRAME_FUSE_BLOCK", 1))
+      if (env_int("AFRAME_FUSE_BLOCK", 1) && !w->live_gn)
         for (int i = 2; i < n; ++i) {
           const int ib = pc->fused_with[i] < 0 ? fusable_block(w, i) : -1;
           if (ib < 0) continue;
@@ -363,7 +368,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       for (int i = 2; i < n; ++i) {
         const LayerDesc& l = w->layers[i];
         if (l.kind != 0 || pc->fused_with[i] >= 0) continue;
-        if (!build_launch(ctx, w, i, slot_ptr(l.input_from), l.residual_from >= 0 ? slot_ptr(l.residual_from) : nullptr,
+        if (!build_launch(ctx, w, i, slot_ptr(l.input_from), l.residual_from >= 0 && !w->live_gn ? slot_ptr(l.residual_from) : nullptr,
                           slot_ptr(i), nb, i == fuse, head_part, pc->launches[i])) { caches.pop_back(); return AFRAME_ECUDA; }
       }
     }
@@ -378,8 +383,10 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     // (a tcgen05 formulation of the stem -- three K = 16 MMAs on an im2col tile, pool = max of three accumulators -- was
     //  built and measured: no faster end to end than this fp32 CUDA-core kernel under the power cap, and less accurate
     //  because its operands are bf16; it was dropped)
+    float2* gn_stats = reinterpret_cast<float2*>(head_part);     // live GroupNorm: the scratch after the slots holds (mu, rstd)
+    const StemGn sgn{gn_stats, w->d_gamma[0], w->d_beta[0], w->n_groups, w->gn_eps};
     st = af_launch_stem_bf16(ctx, w->layers[0], w->layers[1], reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz,
-                             in_bf16, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1));
+                             in_bf16, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1), w->live_gn ? &sgn : nullptr);
     af_prof_end(ctx, AFRAME_PROF_STEM, 1);
     if (st != AFRAME_OK) return st;
     int n_conv = 0;
@@ -402,6 +409,11 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         cudaError_t e = pc->fused_with[i] >= 0 ? launch_block(pc->blocks[i], ctx->stream) : launch_conv(L, ctx->stream);
         ctx->launches++;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
+        if (w->live_gn) {
+          st = af_launch_gn_bf16(ctx, slot_ptr(i), l.residual_from >= 0 ? slot_ptr(l.residual_from) : nullptr, l.t_out, l.c_out,
+                                 w->n_groups, w->gn_eps, w->d_gamma[i], w->d_beta[i], l.relu, nb, gn_stats);
+          if (st != AFRAME_OK) return st;
+        }
       } else if (l.kind == 2) {
         af_prof_end(ctx, AFRAME_PROF_CONV, n_conv);
         n_conv = 0;

@@ -1,0 +1,127 @@
+// NEXT-2, true GroupNorm on the bf16 path ("GroupNorm ... whose statistics are computed per sample at inference").
+// The tensor-core conv stores its plain output z (no bias, no ReLU, no residual) as bf16 [B][T][C]; these two kernels
+// then compute, per (window, group), the mean and biased variance over the group's channels and all T positions and
+// apply y = (z - mu) rstd gamma_c + beta_c (+ residual) (ReLU) in place.  Both are pure HBM streams: 16-byte accesses,
+// one CTA per window for the statistics, one thread per 8 channels for the apply.
+#include "common.cuh"
+#include "stem.h"
+
+__device__ __forceinline__ void gn_unpack8(const uint4 v, float* f) {
+  const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v);
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const float2 t = __bfloat1622float2(h[j]);
+    f[2 * j] = t.x; f[2 * j + 1] = t.y;
+  }
+}
+
+// Fast path: C/8 divides 256 (so a thread always sees the same 8 channels) and a group is a whole number of octets.
+__global__ void __launch_bounds__(256)
+gn_stats_bf16_kernel(const __nv_bfloat16* __restrict__ z, int T, int C, int G, float eps, float2* __restrict__ stats) {
+  __shared__ double rs[256], rq[256];
+  const int64_t b = blockIdx.x;
+  const int opr = C / 8;                               // octets per row
+  const int n_oct = T * opr;
+  const uint4* zb = reinterpret_cast<const uint4*>(z + b * (int64_t)T * C);
+  double S = 0.0, Q = 0.0;
+#pragma unroll 4
+  for (int i = threadIdx.x; i < n_oct; i += 256) {
+    float f[8];
+    gn_unpack8(zb[i], f);
+    float s = 0.f, q = 0.f;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { s += f[j]; q = fmaf(f[j], f[j], q); }
+    S += (double)s; Q += (double)q;
+  }
+  rs[threadIdx.x] = S; rq[threadIdx.x] = Q;
+  __syncthreads();
+  if ((int)threadIdx.x < G) {
+    const int opg = (C / G) / 8;                       // octets per group
+    double ts = 0.0, tq = 0.0;
+    for (int t = 0; t < 256; ++t)
+      if ((t % opr) / opg == (int)threadIdx.x) { ts += rs[t]; tq += rq[t]; }
+    const double n = (double)T * (C / G), mu = ts / n;
+    const double var = tq / n - mu * mu;
+    stats[b * G + threadIdx.x] = make_float2((float)mu, (float)(1.0 / sqrt((var > 0.0 ? var : 0.0) + (double)eps)));
+  }
+}
+
+// General shapes: one CTA per (window, group), scalar loads.
+__global__ void __launch_bounds__(256)
+gn_stats_bf16_generic_kernel(const __nv_bfloat16* __restrict__ z, int T, int C, int G, float eps, float2* __restrict__ stats) {
+  __shared__ double rs[8], rq[8];
+  const int64_t b = blockIdx.x;
+  const int g = blockIdx.y;
+  const int cg = C / G;
+  const __nv_bfloat16* zb = z + b * (int64_t)T * C + g * cg;
+  double s = 0.0, q = 0.0;
+  for (int i = threadIdx.x; i < T * cg; i += blockDim.x) {
+    const double v = (double)__bfloat162float(zb[(int64_t)(i / cg) * C + (i % cg)]);
+    s += v; q += v * v;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); q += __shfl_xor_sync(0xffffffffu, q, o); }
+  if ((threadIdx.x & 31) == 0) { rs[threadIdx.x >> 5] = s; rq[threadIdx.x >> 5] = q; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double ts = 0.0, tq = 0.0;
+    for (int i = 0; i < 8; ++i) { ts += rs[i]; tq += rq[i]; }
+    const double n = (double)T * cg, mu = ts / n;
+    const double var = tq / n - mu * mu;
+    stats[b * G + g] = make_float2((float)mu, (float)(1.0 / sqrt((var > 0.0 ? var : 0.0) + (double)eps)));
+  }
+}
+
+template <bool RES>
+__global__ void __launch_bounds__(256)
+gn_apply_bf16_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ stats, const float* __restrict__ gamma,
+                     const float* __restrict__ beta, const __nv_bfloat16* __restrict__ res, int64_t n_oct, int T, int C,
+                     int G, int relu) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_oct) return;
+  const int opr = C / 8;
+  const int c0 = (int)(i % opr) * 8;
+  const int64_t b = i / ((int64_t)T * opr);
+  const int cg = C / G;
+  uint4* zp = reinterpret_cast<uint4*>(z) + i;
+  float f[8], r[8];
+  gn_unpack8(*zp, f);
+  if (RES) gn_unpack8(reinterpret_cast<const uint4*>(res)[i], r);
+  const float4 g0 = *reinterpret_cast<const float4*>(gamma + c0), g1 = *reinterpret_cast<const float4*>(gamma + c0 + 4);
+  const float4 b0 = *reinterpret_cast<const float4*>(beta + c0), b1 = *reinterpret_cast<const float4*>(beta + c0 + 4);
+  const float gm[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
+  const float bt[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+  uint4 o;
+  __nv_bfloat162* oh = reinterpret_cast<__nv_bfloat162*>(&o);
+#pragma unroll
+  for (int j = 0; j < 8; j += 2) {
+    float v[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const float2 st = stats[b * G + (c0 + j + k) / cg];
+      float y = fmaf(f[j + k] - st.x, st.y * gm[j + k], bt[j + k]);
+      if (RES) y += r[j + k];
+      if (relu) y = fmaxf(y, 0.f);
+      v[k] = y;
+    }
+    oh[j / 2] = __floats2bfloat162_rn(v[0], v[1]);
+  }
+  *zp = o;
+}
+
+aframe_status af_launch_gn_bf16(aframe_ctx* ctx, __nv_bfloat16* z, const __nv_bfloat16* res, int T, int C, int G, float eps,
+                                const float* gamma, const float* beta, int relu, int64_t nb, float2* stats) {
+  if (C % 8 || G < 1 || C % G) return af_fail(ctx, AFRAME_EUNSUPPORTED, "bf16 GroupNorm: channels must be a multiple of 8 and of n_groups");
+  const int opr = C / 8, cg = C / G;
+  if (256 % opr == 0 && cg % 8 == 0 && G <= 256)
+    gn_stats_bf16_kernel<<<(unsigned)nb, 256, 0, ctx->stream>>>(z, T, C, G, eps, stats);
+  else
+    gn_stats_bf16_generic_kernel<<<dim3((unsigned)nb, (unsigned)G), 256, 0, ctx->stream>>>(z, T, C, G, eps, stats);
+  AF_LAUNCH_CHECK(ctx);
+  const int64_t n_oct = nb * T * opr;
+  const unsigned blocks = (unsigned)((n_oct + 255) / 256);
+  if (res) gn_apply_bf16_kernel<true><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, res, n_oct, T, C, G, relu);
+  else gn_apply_bf16_kernel<false><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, nullptr, n_oct, T, C, G, relu);
+  AF_LAUNCH_CHECK(ctx);
+  return AFRAME_OK;
+}

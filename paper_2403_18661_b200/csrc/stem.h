@@ -3,6 +3,14 @@
 
 struct StemOff { int64_t v[AF_MAX_CH]; };   // per-channel element offset of a window's first sample
 
+// true GroupNorm of the stem (NEXT-2): scratch for the per-window statistics and the affine parameters
+struct StemGn { float2* stats; const float* gamma; const float* beta; int G; float eps; };
+
 aframe_status af_launch_stem_bf16(aframe_ctx* ctx, const LayerDesc& conv, const LayerDesc& pool, const void* d_in,
                                   int in_bf16, int64_t sB, const int64_t* choff, const float* d_w, const float* d_bias,
-                                  int64_t B, __nv_bfloat16* d_out);
+                                  int64_t B, __nv_bfloat16* d_out, const StemGn* gn = nullptr);
+
+// true GroupNorm after a tensor-core conv (NEXT-2): statistics per (window, group), then normalise + affine (+ residual)
+// (ReLU) in place on the bf16 tensor z [nb][T][C]; stats is scratch for nb * G float2.
+aframe_status af_launch_gn_bf16(aframe_ctx* ctx, __nv_bfloat16* z, const __nv_bfloat16* res, int T, int C, int G, float eps,
+                                const float* gamma, const float* beta, int relu, int64_t nb, float2* stats);

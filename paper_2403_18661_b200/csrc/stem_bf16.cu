@@ -15,10 +15,13 @@ __device__ __forceinline__ float stem_ld(const void* p, int64_t i) {
 // of TP/8 consecutive pooled positions.  Each conv position is computed once per run (the pool's shared position is
 // carried in a register), the input slides through registers as float4s, and a warp stores one 128-byte line per
 // pooled position.
-template <bool IN_BF16, int TP>
+// GN (NEXT-2, true GroupNorm): the conv output is normalised with the window's own statistics before ReLU and pool,
+// v = acc * sc + sh with sc = rstd_g gamma_c, sh = beta_c - mu_g rstd_g gamma_c (stats from stem_gn_stats_kernel).
+template <bool IN_BF16, int TP, bool GN>
 __global__ void __launch_bounds__(256)
 stem_pool_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const float* __restrict__ w /*[7][2][64]*/,
-                 const float* __restrict__ bias, int T_in, int T_pool, __nv_bfloat16* __restrict__ out) {
+                 const float* __restrict__ bias, int T_in, int T_pool, __nv_bfloat16* __restrict__ out,
+                 const float2* __restrict__ stats, const float* __restrict__ gamma, const float* __restrict__ beta, int G) {
   constexpr int KW = 7, CIN = 2, C_OUT = 64;
   constexpr int RUN = TP / 8;
   constexpr int NX = 4 * TP + 16;                    // samples x[4 tp0 - 8 .. 4 tp0 + 4 TP + 8) per channel
@@ -41,6 +44,13 @@ stem_pool_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const flo
       w0[d][c] = ww.x; w1[d][c] = ww.y;
     }
   const float2 bs = *reinterpret_cast<const float2*>(bias + 2 * lane);
+  float sc0 = 1.f, sc1 = 1.f, sh0 = 0.f, sh1 = 0.f;
+  if (GN) {
+    const int cg = C_OUT / G;
+    const float2 st0 = stats[b * G + (2 * lane) / cg], st1 = stats[b * G + (2 * lane + 1) / cg];
+    sc0 = st0.y * gamma[2 * lane]; sc1 = st1.y * gamma[2 * lane + 1];
+    sh0 = beta[2 * lane] - st0.x * sc0; sh1 = beta[2 * lane + 1] - st1.x * sc1;
+  }
   __syncthreads();
 
   const int tl0 = warp * RUN;                        // first pooled position (local) of this warp's run
@@ -66,6 +76,7 @@ stem_pool_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const flo
         p0 = fmaf(w0[d][c], xv, p0); p1 = fmaf(w1[d][c], xv, p1);
       }
     }
+    if (GN) { p0 = fmaf(p0, sc0, sh0); p1 = fmaf(p1, sc1, sh1); }
     p0 = fmaxf(p0, 0.f); p1 = fmaxf(p1, 0.f);
   }
   __nv_bfloat162* o = reinterpret_cast<__nv_bfloat162*>(out + ((int64_t)b * T_pool + tp0 + tl0) * C_OUT) + lane;
@@ -84,6 +95,7 @@ stem_pool_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const flo
         a0 = fmaf(w0[d][c], r[c][1 + d], a0); a1 = fmaf(w1[d][c], r[c][1 + d], a1);
         c0 = fmaf(w0[d][c], r[c][3 + d], c0); c1 = fmaf(w1[d][c], r[c][3 + d], c1);
       }
+    if (GN) { a0 = fmaf(a0, sc0, sh0); a1 = fmaf(a1, sc1, sh1); c0 = fmaf(c0, sc0, sh0); c1 = fmaf(c1, sc1, sh1); }
     c0 = fmaxf(c0, 0.f); c1 = fmaxf(c1, 0.f);
     const float m0 = fmaxf(fmaxf(p0, a0), c0), m1 = fmaxf(fmaxf(p1, a1), c1);   // ReLU folded: p, c >= 0
     if (tp0 + tl0 + i < T_pool) o[(int64_t)i * (C_OUT / 2)] = __floats2bfloat162_rn(m0, m1);
@@ -95,9 +107,77 @@ stem_pool_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const flo
   }
 }
 
+// NEXT-2: per (window, group) mean and 1/sqrt(var + eps) of the stem conv output (biased variance over the group's
+// channels and all T_conv positions), computed without storing the conv output.  One CTA per window; lane <->
+// channel pair, each warp walks pairs of conv positions (2u, 2u+1), which read x[4u-3 .. 4u+5].
+template <bool IN_BF16>
+__global__ void __launch_bounds__(256)
+stem_gn_stats_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const float* __restrict__ w /*[7][2][64]*/,
+                     const float* __restrict__ bias, int T_in, int G, float eps, float2* __restrict__ stats) {
+  constexpr int KW = 7, CIN = 2, C_OUT = 64;
+  extern __shared__ __align__(16) float xs_dyn[];     // [CIN][T_in + 8], xs[c][n] = x[c][n - 4]
+  __shared__ double red_s[8][32], red_q[8][32];
+  const int NX = T_in + 8;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int64_t b = blockIdx.x;
+  for (int i = tid; i < CIN * NX; i += 256) {
+    const int c = i / NX, n = i - c * NX;
+    const int t = n - 4;
+    xs_dyn[i] = (t >= 0 && t < T_in) ? stem_ld<IN_BF16>(in, b * sB + off.v[c] + t) : 0.f;
+  }
+  float w0[KW][CIN], w1[KW][CIN];
+#pragma unroll
+  for (int d = 0; d < KW; ++d)
+#pragma unroll
+    for (int c = 0; c < CIN; ++c) {
+      const float2 ww = *reinterpret_cast<const float2*>(w + (d * CIN + c) * C_OUT + 2 * lane);
+      w0[d][c] = ww.x; w1[d][c] = ww.y;
+    }
+  const float2 bs = *reinterpret_cast<const float2*>(bias + 2 * lane);
+  __syncthreads();
+  double S = 0.0, Q = 0.0;                             // both channels of the pair are in the same group (C_OUT / G even)
+  const int n_pairs = T_in / 4;
+  for (int u0 = warp * 32; u0 < n_pairs; u0 += 8 * 32) {
+    float s = 0.f, q = 0.f;                            // fp32 over a run of 32 position pairs, double across runs
+    const int u1 = u0 + 32 < n_pairs ? u0 + 32 : n_pairs;
+    for (int u = u0; u < u1; ++u) {
+      float r[CIN][12];                                // x[4u-4 .. 4u+8)
+#pragma unroll
+      for (int c = 0; c < CIN; ++c)
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          const float4 v = *reinterpret_cast<const float4*>(&xs_dyn[c * NX + 4 * u + 4 * k]);
+          r[c][4 * k] = v.x; r[c][4 * k + 1] = v.y; r[c][4 * k + 2] = v.z; r[c][4 * k + 3] = v.w;
+        }
+      float a0 = bs.x, a1 = bs.y, c0 = bs.x, c1 = bs.y;
+#pragma unroll
+      for (int c = 0; c < CIN; ++c)
+#pragma unroll
+        for (int d = 0; d < KW; ++d) {
+          a0 = fmaf(w0[d][c], r[c][1 + d], a0); a1 = fmaf(w1[d][c], r[c][1 + d], a1);
+          c0 = fmaf(w0[d][c], r[c][3 + d], c0); c1 = fmaf(w1[d][c], r[c][3 + d], c1);
+        }
+      s += (a0 + a1) + (c0 + c1);
+      q = fmaf(a0, a0, q); q = fmaf(a1, a1, q); q = fmaf(c0, c0, q); q = fmaf(c1, c1, q);
+    }
+    S += (double)s; Q += (double)q;
+  }
+  red_s[warp][lane] = S; red_q[warp][lane] = Q;
+  __syncthreads();
+  if (tid < G) {
+    const int lg = (C_OUT / G) / 2;                    // lanes per group
+    double ts = 0.0, tq = 0.0;
+    for (int wv = 0; wv < 8; ++wv)
+      for (int l = tid * lg; l < (tid + 1) * lg; ++l) { ts += red_s[wv][l]; tq += red_q[wv][l]; }
+    const double n = (double)(T_in / 2) * (C_OUT / G), mu = ts / n;
+    const double var = tq / n - mu * mu;
+    stats[b * G + tid] = make_float2((float)mu, (float)(1.0 / sqrt((var > 0.0 ? var : 0.0) + (double)eps)));
+  }
+}
+
 aframe_status af_launch_stem_bf16(aframe_ctx* ctx, const LayerDesc& conv, const LayerDesc& pool, const void* d_in,
                                   int in_bf16, int64_t sB, const int64_t* choff, const float* d_w, const float* d_bias,
-                                  int64_t B, __nv_bfloat16* d_out) {
+                                  int64_t B, __nv_bfloat16* d_out, const StemGn* gn) {
   if (!(conv.k == 7 && conv.c_in == 2 && conv.c_out == 64 && conv.stride == 2 && conv.pad == 3 && conv.relu &&
         pool.k == 3 && pool.stride == 2 && pool.pad == 1))
     return af_fail(ctx, AFRAME_EUNSUPPORTED, "bf16 stem: only conv(2->64,k7,s2,p3)+ReLU+maxpool(k3,s2,p1) is built");
@@ -107,10 +187,26 @@ aframe_status af_launch_stem_bf16(aframe_ctx* ctx, const LayerDesc& conv, const 
   StemOff off;
   for (int c = 0; c < AF_MAX_CH; ++c) off.v[c] = c < conv.c_in ? choff[c] : 0;
   dim3 grid((unsigned)((pool.t_out + TP - 1) / TP), (unsigned)B);
-  if (in_bf16)
-    stem_pool_kernel<true, TP><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out);
+  if (gn) {
+    const size_t smem = sizeof(float) * 2 * (size_t)(conv.t_in + 8);
+    if (gn->G < 1 || gn->G > 32 || 64 % gn->G || (64 / gn->G) % 2 || smem > 48 * 1024)
+      return af_fail(ctx, AFRAME_EUNSUPPORTED, "bf16 stem with true GroupNorm: needs an even number of channels per group and kernel_len <= 6136");
+    if (in_bf16) {
+      stem_gn_stats_kernel<true><<<(unsigned)B, 256, smem, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, gn->G, gn->eps, gn->stats);
+      stem_pool_kernel<true, TP, true><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
+                                                                      gn->stats, gn->gamma, gn->beta, gn->G);
+    } else {
+      stem_gn_stats_kernel<false><<<(unsigned)B, 256, smem, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, gn->G, gn->eps, gn->stats);
+      stem_pool_kernel<false, TP, true><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
+                                                                       gn->stats, gn->gamma, gn->beta, gn->G);
+    }
+    ctx->launches++;
+  } else if (in_bf16)
+    stem_pool_kernel<true, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
+                                                                     nullptr, nullptr, nullptr, 1);
   else
-    stem_pool_kernel<false, TP><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out);
+    stem_pool_kernel<false, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
+                                                                      nullptr, nullptr, nullptr, 1);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }

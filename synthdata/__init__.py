@@ -14,6 +14,6 @@ no whitening, no convolution, no norm fold).  It only produces inputs:
 from .noise import analytic_psd, coloured_noise, SIGMA_X_ANALYTIC  # noqa: F401
 from .chirps import newtonian_chirp, inject_chirps, ChirpParams  # noqa: F401
 from .weights import (  # noqa: F401
-    LayerSpec, resnet_layer_table, make_weight_blob, tiny_config, full_config, tiny_config_live_gn,
+    LayerSpec, resnet_layer_table, make_weight_blob, tiny_config, full_config, tiny_config_live_gn, full_config_live_gn,
     KIND_CONV, KIND_MAXPOOL, KIND_HEAD, NORM_CHANNEL, NORM_GROUP, NORM_GROUP_LIVE,
 )

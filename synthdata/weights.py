@@ -89,6 +89,12 @@ def tiny_config_live_gn():
                 norm_kind=NORM_GROUP_LIVE, n_groups=8, seed=2, kernel_len=2048)
 
 
+def full_config_live_gn():
+    """NEXT-2 at full size: the configs[1] network with true GroupNorm (8 groups, statistics per window)."""
+    return dict(table=resnet_layer_table(2, 64, 7, [3, 4, 6, 3], [64, 128, 256, 512]),
+                norm_kind=NORM_GROUP_LIVE, n_groups=8, seed=3, kernel_len=3072)
+
+
 def make_weight_blob(table, norm_kind, n_groups, seed, eps=1e-5, in_channels=2, **_unused) -> bytes:
     """He-normal (fan-in) conv weights, frozen norm statistics (reading B6/B7), head w ~ N(0, 1/C)."""
     rng = np.random.Generator(np.random.PCG64(seed))

@@ -157,6 +157,34 @@ def test_true_group_norm_fp32_matches_oracle(af, config0):
     assert rel_err(got, ref) <= 1e-4
     ctx16 = af.Context(n_design=4096, kernel_len=2048, precision=af.BF16)
     w16 = ctx16.load_weights(blob)
-    with pytest.raises(af.AframeError) as e:
+    with pytest.raises(af.AframeError) as e:                    # widths 8..64 do not tile onto the tensor-core kernel
         ctx16.forward(w16, torch.from_numpy(wins).cuda())
     assert e.value.status == af.EUNSUPPORTED
+
+
+def test_true_group_norm_full_size_fp32_and_bf16(af, config1):
+    """NEXT-2 at configs[1] size: the ResNet54 table with live GroupNorm.  fp32 path within T2 of the oracle; bf16
+    tensor-core path (plain conv output stored as bf16, statistics + affine + residual + ReLU in the GroupNorm kernels)
+    within T3 and rank-preserving; smaller ragged batches give the same scores bit for bit."""
+    from synthdata import full_config_live_gn
+    blob = make_weight_blob(**full_config_live_gn())
+    wins = config1["wins"][:48].copy()
+    wins[5] *= 7.0                                              # per-window statistics: the scale of a window drops out ...
+    wins[6] = wins[5] / 7.0                                     # ... up to eps, so these two score (almost) alike
+    ref = onet.forward(onet.parse_blob(blob), wins)
+    assert abs(ref[5] - ref[6]) <= 1e-3 * np.abs(ref).max()
+    x = torch.from_numpy(wins).cuda()
+    ctx = af.Context(precision=af.FP32)
+    got32 = ctx.forward(ctx.load_weights(blob), x[:8]).cpu().numpy()
+    assert rel_err(got32, ref[:8]) <= 1e-4
+    ctx16 = af.Context(precision=af.BF16)
+    w16 = ctx16.load_weights(blob)
+    got = ctx16.forward(w16, x).cpu().numpy().astype(np.float64)
+    err = rel_err(got, ref)
+    rho = scipy.stats.spearmanr(got, ref).statistic
+    print(f"live GroupNorm bf16: rel err {err:.3e}, spearman {rho:.5f}")
+    assert err <= 2e-2
+    assert rho >= 0.99
+    for nb in (1, 37):
+        part = ctx16.forward(w16, x[:nb]).cpu().numpy()
+        assert np.array_equal(part, got[:nb].astype(np.float32))
