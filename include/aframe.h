@@ -111,7 +111,9 @@ aframe_status aframe_whiten_rolling(aframe_ctx* ctx, const float* d_strain, int6
 /* ---- weights (readings B1-B7) ----------------------------------------------------------
  * host_blob: the version-1 blob documented in synthdata/weights.py (header, layer table, UNFOLDED
  * fp32 parameters).  The library validates the table against cfg (AFRAME_ESHAPE), folds the frozen
- * norm into (W', b') in double precision, and uploads fp32 and bf16 (K-major) copies.  Synchronises. */
+ * norm into (W', b') in double precision, and uploads fp32 and bf16 (K-major) copies.  Synchronises.
+ * Blob norm_kind 2 (NEXT-2, P:39 true GroupNorm) carries no frozen statistics: nothing is folded, and
+ * aframe_forward computes mean / variance per window and group on the device after every conv. */
 aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob, size_t bytes, aframe_weights** out);
 void          aframe_weights_free(aframe_weights* w);
 

@@ -35,13 +35,27 @@ def periodogram(seg, fs, window):
     return p
 
 
-def welch(x, fs=2048.0, nfft=4096, hop=2048):
-    """P[k], k = 0..nfft/2, in x-units^2/Hz: mean over the J segments x[hop j : hop j + nfft]."""
+def median_bias(n):
+    """NEXT-3 variant (the paper does not name its averaging, reading A1 is the mean): the median of
+    n periodogram values of Gaussian noise (chi-squared with 2 degrees of freedom, i.e. exponential) underestimates
+    their mean by sum_{i=1}^{m} (-1)^(i+1) / i, m = n for odd n and n - 1 for even n (-> ln 2)."""
+    m = n if n % 2 else n - 1
+    return sum((1.0 if i % 2 else -1.0) / i for i in range(1, m + 1))
+
+
+def welch(x, fs=2048.0, nfft=4096, hop=2048, average="mean"):
+    """P[k], k = 0..nfft/2, in x-units^2/Hz: mean (reading A1) over the J segments x[hop j : hop j + nfft], or, for
+    average="median", their per-bin median divided by median_bias(J)."""
     x = np.asarray(x, dtype=np.float64)
     j_total = segment_count(x.shape[-1], nfft, hop)
     if j_total < 1:
         raise ValueError("need at least one full segment")
     w = hann_periodic(nfft)
+    if average == "median":
+        pg = np.stack([periodogram(x[..., hop * j: hop * j + nfft], fs, w) for j in range(j_total)])
+        return np.median(pg, axis=0) / median_bias(j_total)
+    if average != "mean":
+        raise ValueError("average must be 'mean' or 'median'")
     acc = np.zeros(x.shape[:-1] + (nfft // 2 + 1,), dtype=np.float64)
     for j in range(j_total):
         acc += periodogram(x[..., hop * j: hop * j + nfft], fs, w)
