@@ -62,6 +62,9 @@ typedef struct {
   int64_t  psd_update;        /* 16384 = new PSD every 8 s (BASELINE.json configs[2])            */
   int32_t  strain_scale_log2; /* 70                                                              */
   int32_t  precision;         /* aframe_precision of the network path                            */
+  int32_t  welch_average;     /* 0 = mean over segments (reading A1, default); 1 = per-bin median
+                                 divided by its bias for n segments (NEXT-3 variant; n <= 255)   */
+  int32_t  reserved_;         /* must be 0                                                       */
 } aframe_config;
 
 typedef struct aframe_ctx aframe_ctx;
@@ -82,7 +85,8 @@ const char*   aframe_last_error(const aframe_ctx* ctx);   /* ctx may be NULL: re
  * d_strain: [C][ld] fp32 raw strain, channel c at d_strain + c*ld, n_samples valid per channel
  *           (n_samples >= welch_nfft, else AFRAME_ESHAPE).
  * d_psd   : [C][welch_nfft/2+1] fp32, one-sided density, SCALED units, mean over the
- *           floor((n_samples-nfft)/hop)+1 Hann-windowed, mean-detrended segments. */
+ *           floor((n_samples-nfft)/hop)+1 Hann-windowed, mean-detrended segments (cfg.welch_average
+ *           = 1: their per-bin median over its bias; at most 255 segments, else AFRAME_EUNSUPPORTED). */
 aframe_status aframe_psd_welch(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
                                float* d_psd);
 
@@ -107,6 +111,28 @@ aframe_status aframe_filter_taps(aframe_ctx* ctx, float* d_taps);
 aframe_status aframe_whiten_rolling(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
                                     void* d_out, int64_t ld_out, aframe_precision out_dtype,
                                     int64_t* h_n_out);
+
+/* ---- NEXT-4  training-time whitening batch -------------------------------------------------
+ * "The length of each noise window sampled from disk is 10.5 s.  The first 8 s is used to estimate the
+ * power spectral density (PSD) used for whitening.  The remaining 2.5 s of the window is whitened [...]
+ * 0.5 s of data is corrupted on both ends of the window and removed."  Every (element, detector) row gets
+ * its OWN Welch PSD (from its first n_psd samples), its own filter (O-2) and is whitened (O-3) over its
+ * remaining n_samples - n_psd samples.
+ * d_strain: [n_batch][C][n_samples] fp32, contiguous.  d_out: [n_batch][C][n_samples - n_psd - filter_len]
+ * fp32 or bf16, contiguous (the paper's shapes: n_samples 21504, n_psd 16384 -> 3072 = kernel_len).
+ * AFRAME_ESHAPE if n_psd < welch_nfft, n_samples - n_psd <= filter_len or n_batch * C > 65535. */
+aframe_status aframe_whiten_batch(aframe_ctx* ctx, const float* d_strain, int64_t n_batch, int64_t n_samples,
+                                  int64_t n_psd, void* d_out, aframe_precision out_dtype);
+
+/* ---- NEXT-4  false-alarm rate of events against a background ------------------------
+ * "a false alarm rate (FAR) can be assigned to injected events by dividing the number of background
+ * events with detection statistic greater than the event of interest, with livetime analyzed."
+ * d_background: [n_bg] fp32 detection statistics of the background triggers (timeslides), any order.
+ * d_events    : [n_ev] fp32.   d_counts: [n_ev] int64, number of background values STRICTLY greater
+ * (NaN compares false).  d_far: [n_ev] fp64 = counts / livetime_s in 1/s, or NULL.  n_bg = 0 gives
+ * zeros; n_ev = 0 is a no-op.  AFRAME_EINVAL if livetime_s <= 0 while d_far != NULL. */
+aframe_status aframe_far(aframe_ctx* ctx, const float* d_background, int64_t n_bg, const float* d_events,
+                         int64_t n_ev, double livetime_s, int64_t* d_counts, double* d_far);
 
 /* ---- weights (readings B1-B7) ----------------------------------------------------------
  * host_blob: the version-1 blob documented in synthdata/weights.py (header, layer table, UNFOLDED

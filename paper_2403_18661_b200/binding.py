@@ -31,7 +31,8 @@ class aframe_config(C.Structure):
                 ("welch_nfft", C.c_int32), ("welch_hop", C.c_int32), ("filter_len", C.c_int32),
                 ("n_design", C.c_int32), ("f_lo", C.c_double), ("f_hi", C.c_double),
                 ("kernel_len", C.c_int32), ("stride", C.c_int32), ("psd_len", C.c_int64),
-                ("psd_update", C.c_int64), ("strain_scale_log2", C.c_int32), ("precision", C.c_int32)]
+                ("psd_update", C.c_int64), ("strain_scale_log2", C.c_int32), ("precision", C.c_int32),
+                ("welch_average", C.c_int32), ("reserved_", C.c_int32)]
 
 
 EXPORTS = {
@@ -54,6 +55,8 @@ EXPORTS = {
     "aframe_stream_destroy": (None, [C.c_void_p]),
     "aframe_stream_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "aframe_launch_count": (C.c_int64, [C.c_void_p]),
+    "aframe_whiten_batch": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_int]),
+    "aframe_far": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_void_p]),
     "aframe_postprocess": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_int32, C.c_int32,
                                      C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]),
     "aframe_stream_graph_replays": (C.c_int64, [C.c_void_p]),
@@ -251,6 +254,30 @@ class Context:
                                                 _ptr(integ), _ptr(val), _ptr(idx), C.byref(nt)))
         assert nt.value == n_trig
         return integ, val, idx
+
+    # ---- NEXT-4
+    def whiten_batch(self, strain, n_psd, out_dtype=torch.float32):
+        """strain [B][C][n] float32 CUDA -> [B][C][n - n_psd - filter_len]: own PSD (first n_psd samples) per row."""
+        _need(strain, torch.float32, "strain")
+        b, c, n = strain.shape
+        if c != self.cfg.n_channels:
+            raise ValueError("strain must be [B][n_channels][n]")
+        n_out = n - int(n_psd) - self.cfg.filter_len
+        out = torch.empty((b, c, max(n_out, 1)), dtype=out_dtype, device=strain.device)
+        prec = BF16 if out_dtype == torch.bfloat16 else FP32
+        self._check(self.lib.aframe_whiten_batch(self.handle, _ptr(strain), b, n, int(n_psd), _ptr(out), prec))
+        return out
+
+    def far(self, background, events, livetime_s):
+        """counts[i] = #{background > events[i]} (int64), far = counts / livetime_s (float64, 1/s)."""
+        _need(events, torch.float32, "events")
+        if background.numel():
+            _need(background, torch.float32, "background")
+        counts = torch.empty((events.numel(),), dtype=torch.int64, device=events.device)
+        far = torch.empty((events.numel(),), dtype=torch.float64, device=events.device)
+        self._check(self.lib.aframe_far(self.handle, _ptr(background) if background.numel() else None, background.numel(),
+                                        _ptr(events), events.numel(), float(livetime_s), _ptr(counts), _ptr(far)))
+        return counts, far
 
     # ---- per-stage device timing
     def profile(self, enable: bool):

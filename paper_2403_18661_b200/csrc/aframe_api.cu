@@ -69,6 +69,8 @@ AF_API aframe_status aframe_create(const aframe_config* cfg, void* cuda_stream, 
   if (cfg->psd_len % cfg->stride) return AFRAME_ESHAPE;
   if (cfg->strain_scale_log2 < -120 || cfg->strain_scale_log2 > 120) return AFRAME_EINVAL;
   if (cfg->precision != AFRAME_FP32 && cfg->precision != AFRAME_BF16) return AFRAME_EINVAL;
+  if ((cfg->welch_average != 0 && cfg->welch_average != 1) || cfg->reserved_ != 0) return AFRAME_EINVAL;
+  if (cfg->welch_average == 1 && (cfg->psd_len - cfg->welch_nfft) / cfg->welch_hop + 1 > 255) return AFRAME_EUNSUPPORTED;
 
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return AFRAME_EUNSUPPORTED; }
@@ -172,6 +174,37 @@ AF_API aframe_status aframe_whiten(aframe_ctx* ctx, const float* d_strain, int64
   if (st != AFRAME_OK) return st;
   if (n_out <= 0) return AFRAME_OK;
   return af_launch_whiten_os(ctx, d_strain, n_samples, ld, H, 0, n_out, n_out, 1, d_out, ld_out, out_dtype == AFRAME_BF16);
+}
+
+// ---- NEXT-4: training-time whitening batch --------------------------------------------------
+AF_API aframe_status aframe_whiten_batch(aframe_ctx* ctx, const float* d_strain, int64_t n_batch, int64_t n_samples,
+                                             int64_t n_psd, void* d_out, aframe_precision out_dtype) {
+  if (!ctx) return AFRAME_EINVAL;
+  if (!d_strain || !d_out) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
+  if (out_dtype != AFRAME_FP32 && out_dtype != AFRAME_BF16) return af_fail(ctx, AFRAME_EINVAL, "bad out_dtype");
+  const aframe_config& cfg = ctx->cfg;
+  if (n_batch < 1) return af_fail(ctx, AFRAME_EINVAL, "n_batch < 1");
+  const int64_t rows = n_batch * cfg.n_channels;
+  const int64_t n_w = n_samples - n_psd, n_out = n_w - cfg.filter_len;
+  if (n_psd < cfg.welch_nfft || n_out <= 0 || rows > 65535)
+    return af_fail(ctx, AFRAME_ESHAPE, "whiten_batch: n_psd < welch_nfft, n_samples - n_psd <= filter_len, or n_batch * C > 65535");
+  const int64_t n_seg = (n_psd - cfg.welch_nfft) / cfg.welch_hop + 1;
+  const int F = cfg.welch_nfft / 2 + 1;
+  aframe_status st = af_ws_reserve(ctx, ctx->ws_psd, sizeof(float) * (size_t)rows * n_seg * F);
+  if (st != AFRAME_OK) return st;
+  st = af_ws_reserve(ctx, ctx->ws_filt, sizeof(float) * (size_t)rows * (F + AF_NOS / 2 + 1));
+  if (st != AFRAME_OK) return st;
+  float* pg = reinterpret_cast<float*>(ctx->ws_psd.ptr);
+  float* psd = reinterpret_cast<float*>(ctx->ws_filt.ptr);
+  float* H = psd + (size_t)rows * F;
+  ctx->n_ch_batch = (int)rows;               // the launchers below treat every (element, detector) row as a channel
+  st = af_launch_welch_periodograms(ctx, d_strain, n_samples, 0, n_seg, pg);
+  if (st == AFRAME_OK) st = af_launch_psd_mean(ctx, pg, n_seg, 0, 1, n_seg, psd);
+  if (st == AFRAME_OK) st = af_launch_filter_design(ctx, psd, 1, H, nullptr);
+  if (st == AFRAME_OK)
+    st = af_launch_whiten_os(ctx, d_strain + n_psd, n_w, n_samples, H, 0, n_out, n_out, 1, d_out, n_out, out_dtype == AFRAME_BF16);
+  ctx->n_ch_batch = 0;
+  return st;
 }
 
 AF_API aframe_status aframe_filter_taps(aframe_ctx* ctx, float* d_taps) {

@@ -78,7 +78,11 @@ struct aframe_ctx {
   std::vector<cudaEvent_t> prof_pool;
   cudaEvent_t prof_open[AFRAME_PROF_KINDS] = {};
   float* layer_ms = nullptr;   // aframe_profile_layers: per-layer device time of the next forward (host array), else null
+  int n_ch_batch = 0;          // aframe_whiten_batch: rows (element x detector) the signal launchers treat as channels
 };
+
+// rows the Welch / design / whitening launchers run over: the configured detectors, or a training batch's B*C rows
+static inline int af_nch(const aframe_ctx* ctx) { return ctx->n_ch_batch > 0 ? ctx->n_ch_batch : ctx->cfg.n_channels; }
 
 // Stage timing: af_prof_begin records an event before the first launch of a stage, af_prof_end one after
 // its last launch; aframe_profile_read sums the elapsed times per stage.  No-ops unless profiling is on.

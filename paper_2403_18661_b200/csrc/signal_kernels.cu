@@ -94,6 +94,28 @@ __global__ void psd_mean_kernel(const float* __restrict__ pgram, int64_t n_seg_t
   psd[((int64_t)e * C + c) * F + k] = (float)(acc / n_avg);
 }
 
+// NEXT-3 variant: per-bin MEDIAN of the n_avg periodograms (n_avg <= 255) times 1 / median_bias(n_avg) (computed on the
+// host in double).  One thread per bin: insertion sort of its column in local memory; even n_avg averages the two
+// middle values.  The order in which the periodograms sit in the ring does not matter.
+__global__ void psd_median_kernel(const float* __restrict__ pgram, int64_t n_seg_total, int64_t seg_step, int n_avg,
+                                  int F, int C, float inv_bias, float* __restrict__ psd, StreamGate gate) {
+  if (gate.d_n != nullptr && !gate.psd_due()) return;
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t e = blockIdx.y;
+  const int c = blockIdx.z;
+  if (k >= F) return;
+  const float* p = pgram + ((int64_t)c * n_seg_total + e * seg_step) * F + k;
+  float v[255];
+  for (int j = 0; j < n_avg; ++j) {
+    const float x = p[(int64_t)j * F];
+    int i = j;
+    while (i > 0 && v[i - 1] > x) { v[i] = v[i - 1]; --i; }
+    v[i] = x;
+  }
+  const float med = (n_avg & 1) ? v[n_avg / 2] : 0.5f * (v[n_avg / 2 - 1] + v[n_avg / 2]);
+  psd[((int64_t)e * C + c) * F + k] = med * inv_bias;
+}
+
 // --------------------------------------------------------------------------------------------------
 // Filter design (double).  One CTA per (epoch, channel).
 //   A[k] = 1/sqrt(P_d[k] fs/2) in band; g = irfft_{N_d}(A) (A real & even -> one complex FFT, real part);
@@ -267,7 +289,7 @@ aframe_status af_launch_welch_periodograms(aframe_ctx* ctx, const float* d_strai
   const float scale = ldexpf(1.0f, cfg.strain_scale_log2);
   const double sum_w2 = 0.375 * nfft;                 // sum of the periodic Hann window squared
   const float norm = (float)(1.0 / (cfg.fs * sum_w2));
-  dim3 grid((unsigned)(gate_in ? 1 : n_seg), (unsigned)cfg.n_channels);
+  dim3 grid((unsigned)(gate_in ? 1 : n_seg), (unsigned)af_nch(ctx));
   af_prof_begin(ctx, AFRAME_PROF_WELCH);
 #define AF_WELCH_CASE(N)                                                                                            \
   case N:                                                                                                           \
@@ -289,9 +311,17 @@ aframe_status af_launch_psd_mean(aframe_ctx* ctx, const float* d_pgram, int64_t 
   StreamGate gate = gate_in ? *gate_in : StreamGate();
   if (n_epochs <= 0) return AFRAME_OK;
   const int F = ctx->cfg.welch_nfft / 2 + 1;
-  dim3 grid((F + 127) / 128, (unsigned)n_epochs, (unsigned)ctx->cfg.n_channels);
+  dim3 grid((F + 127) / 128, (unsigned)n_epochs, (unsigned)af_nch(ctx));
   af_prof_begin(ctx, AFRAME_PROF_WELCH);
-  psd_mean_kernel<<<grid, 128, 0, ctx->stream>>>(d_pgram, n_seg_total, seg_step, (int)n_avg, F, ctx->cfg.n_channels, d_psd, gate);
+  if (ctx->cfg.welch_average == 1) {
+    if (n_avg > 255) return af_fail(ctx, AFRAME_EUNSUPPORTED, "median Welch: more than 255 segments");
+    const int64_t m = (n_avg & 1) ? n_avg : n_avg - 1;
+    double bias = 0.0;                                 // sum_{i=1}^{m} (-1)^(i+1) / i
+    for (int64_t i = 1; i <= m; ++i) bias += ((i & 1) ? 1.0 : -1.0) / (double)i;
+    psd_median_kernel<<<grid, 128, 0, ctx->stream>>>(d_pgram, n_seg_total, seg_step, (int)n_avg, F, af_nch(ctx),
+                                                     (float)(1.0 / bias), d_psd, gate);
+  } else
+    psd_mean_kernel<<<grid, 128, 0, ctx->stream>>>(d_pgram, n_seg_total, seg_step, (int)n_avg, F, af_nch(ctx), d_psd, gate);
   af_prof_end(ctx, AFRAME_PROF_WELCH, 1);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
@@ -305,7 +335,7 @@ aframe_status af_launch_filter_design(aframe_ctx* ctx, const float* d_psd, int64
   StreamGate gate = gate_in ? *gate_in : StreamGate();
   const aframe_config& cfg = ctx->cfg;
   const size_t smem = filter_design_smem(cfg.filter_len);
-  dim3 grid((unsigned)n_epochs, (unsigned)cfg.n_channels);
+  dim3 grid((unsigned)n_epochs, (unsigned)af_nch(ctx));
   const int F_w = cfg.welch_nfft / 2 + 1;
   af_prof_begin(ctx, AFRAME_PROF_DESIGN);
 #define AF_FD_CASE(N)                                                                                                \
@@ -315,7 +345,7 @@ aframe_status af_launch_filter_design(aframe_ctx* ctx, const float* d_psd, int64
       AF_CUDA(ctx, cudaFuncSetAttribute(filter_design_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
       attr_set = true;                                                                                               \
     }                                                                                                                \
-    filter_design_kernel<N><<<grid, 512, smem, ctx->stream>>>(d_psd, F_w, cfg.n_channels, cfg.fs, cfg.f_lo, cfg.f_hi, \
+    filter_design_kernel<N><<<grid, 512, smem, ctx->stream>>>(d_psd, F_w, af_nch(ctx), cfg.fs, cfg.f_lo, cfg.f_hi, \
                                                              cfg.filter_len, ctx->d_tw64, d_H, d_taps, gate);        \
   } break;
   switch (cfg.n_design) {
@@ -336,13 +366,13 @@ aframe_status af_launch_whiten_os(aframe_ctx* ctx, const float* d_strain, int64_
   const int valid = AF_NOS - cfg.filter_len;
   const int bpe = (int)((epoch_len + valid - 1) / valid);
   const float scale = ldexpf(1.0f, cfg.strain_scale_log2);
-  dim3 grid((unsigned)(n_epochs * bpe), (unsigned)cfg.n_channels);
+  dim3 grid((unsigned)(n_epochs * bpe), (unsigned)af_nch(ctx));
   af_prof_begin(ctx, AFRAME_PROF_WHITEN);
   if (out_bf16)
-    whiten_os_kernel<true><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, cfg.n_channels, in0, out_total,
+    whiten_os_kernel<true><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, af_nch(ctx), in0, out_total,
                                                           epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
   else
-    whiten_os_kernel<false><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, cfg.n_channels, in0, out_total,
+    whiten_os_kernel<false><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, af_nch(ctx), in0, out_total,
                                                            epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
   af_prof_end(ctx, AFRAME_PROF_WHITEN, 1);
   AF_LAUNCH_CHECK(ctx);
