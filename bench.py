@@ -57,6 +57,7 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=4096, help="windows per launch sequence (configs[3]: 4096)")
     ap.add_argument("--latency-updates", type=int, default=10000, help="configs[4] timed updates (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the device timings of the SURVEY 8(f) rows")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
 
@@ -424,6 +425,8 @@ def run_ours(args):
                           "achieved": pp_bytes / (pp_ms * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
                           "frac": pp_bytes / (pp_ms * 1e-3) / 1e9 / peaks["hbm"],
                           "note": "2 launches over 2 MB of scores: launch-latency bound, 0.001 % of a step"}
+    if world == 1 and not args.no_next_rows:
+        out["next_rows"] = next_rows(af, torch, stream, peaks)
     if args.latency_updates > 0 and world == 1:
         out["latency"] = latency_run(af, torch, stream, blob, args.latency_updates)
     if not args.no_cpu_baseline:
@@ -435,6 +438,53 @@ def run_ours(args):
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def next_rows(af, torch, stream, peaks):
+    """Device-timed figures for the SURVEY 8(f) rows built beyond the hot path (context, not the headline)."""
+    from synthdata import coloured_noise, full_config_live_gn
+
+    def timed(fn, reps):
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                fn()
+            e1.record(stream)
+            stream.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    res = {}
+    with torch.cuda.stream(stream):
+        ctx = af.Context(stream=stream, precision=af.BF16)
+        # NEXT-4, P:102: one training batch, 384 x 2 x 10.5 s, own PSD per row, bf16 kernels out
+        row = torch.from_numpy(coloured_noise(21504, 9001)).cuda()
+        xb = (row[None] * (1.0 + torch.arange(384, device="cuda")[:, None, None] % 5)).contiguous()
+        ms = timed(lambda: ctx.whiten_batch(xb, 16384, out_dtype=torch.bfloat16), 10)
+        nbytes = xb.numel() * 4 + 384 * 2 * 3072 * 2
+        res["whiten_batch"] = {"workload": "384 x 2 x 21504 samples (P:102)", "ms": ms, "batches_per_s": 1e3 / ms,
+                               "achieved": nbytes / (ms * 1e-3) / 1e9, "unit": "GB/s", "frac": nbytes / (ms * 1e-3) / 1e9 / peaks["hbm"],
+                               "note": "768 fp64 filter designs (one CTA each) dominate; 4 launches"}
+        # NEXT-4, P:200/P:219: FAR of 10 000 events against one year of 8 s triggers
+        g = torch.Generator(device="cuda").manual_seed(5)
+        bg = torch.randn(3_944_700, device="cuda", generator=g)
+        ev = torch.randn(10_000, device="cuda", generator=g)
+        ms = timed(lambda: ctx.far(bg, ev, 365.25 * 86400.0), 10)
+        res["far"] = {"workload": "3 944 700 background triggers (1 yr / 8 s) x 10 000 events", "ms": ms,
+                      "pairs_per_s": bg.numel() * ev.numel() / (ms * 1e-3), "bound": "alu",
+                      "note": "exact all-pairs strict compare, 2 instructions per pair"}
+        # NEXT-2, P:39: the ResNet54 table with true GroupNorm on the tcgen05 path
+        cfgd = full_config_live_gn()
+        from synthdata import make_weight_blob
+        wg = ctx.load_weights(make_weight_blob(**cfgd))
+        xw = torch.randn(4096, 2, 3072, device="cuda")
+        ms = timed(lambda: ctx.forward(wg, xw), 5)
+        res["live_group_norm"] = {"workload": "4096 windows, ResNet54 with per-window GroupNorm statistics", "ms": ms,
+                                  "windows_per_s": 4096 / (ms * 1e-3),
+                                  "note": "HBM-bound by the statistics + apply passes after every conv (DESIGN.md NEXT-2)"}
+    return res
 
 
 def main():
