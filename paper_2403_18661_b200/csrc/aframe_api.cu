@@ -266,6 +266,7 @@ AF_API void aframe_weights_free(aframe_weights* w) {
   for (float* p : w->d_w32) cudaFree(p);
   for (__nv_bfloat16* p : w->d_w16) cudaFree(p);
   for (float* p : w->d_bias) cudaFree(p);
+  for (float* p : w->d_bias_sc) cudaFree(p);
   for (float* p : w->d_gamma) cudaFree(p);
   for (float* p : w->d_beta) cudaFree(p);
   cudaFree(w->d_head_w);
@@ -300,6 +301,8 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
   w->d_w32.assign(n_layers, nullptr);
   w->d_w16.assign(n_layers, nullptr);
   w->d_bias.assign(n_layers, nullptr);
+  w->d_bias_sc.assign(n_layers, nullptr);
+  std::vector<std::vector<float>> h_bias(n_layers);
   w->d_gamma.assign(n_layers, nullptr);
   w->d_beta.assign(n_layers, nullptr);
   w->live_gn = norm_kind == 2;
@@ -372,11 +375,23 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
     if (cudaMemcpy(w->d_w32[i], w32.data(), sizeof(float) * nw, cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(w->d_w16[i], w16.data(), 2 * nw, cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(w->d_bias[i], bias.data(), sizeof(float) * l.c_out, cudaMemcpyHostToDevice) != cudaSuccess) { fail(AFRAME_ECUDA, "weight upload failed"); break; }
+    h_bias[i] = bias;
     if (norm_kind == 2) {
       if (cudaMalloc(&w->d_gamma[i], sizeof(float) * l.c_out) != cudaSuccess || cudaMalloc(&w->d_beta[i], sizeof(float) * l.c_out) != cudaSuccess) { fail(AFRAME_ENOMEM, "device allocation failed"); break; }
       if (cudaMemcpy(w->d_gamma[i], gamma, sizeof(float) * l.c_out, cudaMemcpyHostToDevice) != cudaSuccess ||
           cudaMemcpy(w->d_beta[i], beta, sizeof(float) * l.c_out, cudaMemcpyHostToDevice) != cudaSuccess) { fail(AFRAME_ECUDA, "weight upload failed"); break; }
     }
+  }
+  // bias of a conv with its 1x1 projection shortcut folded in (the tcgen05 path runs the projection as extra K blocks)
+  for (uint32_t i = 0; i < n_layers && st == AFRAME_OK; ++i) {
+    const LayerDesc& l = w->layers[i];
+    if (l.kind != 0 || l.residual_from < 0) continue;
+    const LayerDesc& r = w->layers[l.residual_from];
+    if (r.kind != 0 || r.k != 1 || r.c_out != l.c_out) continue;
+    std::vector<float> b(l.c_out);
+    for (int c = 0; c < l.c_out; ++c) b[c] = h_bias[i][c] + h_bias[l.residual_from][c];
+    if (cudaMalloc(&w->d_bias_sc[i], sizeof(float) * l.c_out) != cudaSuccess) { fail(AFRAME_ENOMEM, "device allocation failed"); break; }
+    if (cudaMemcpy(w->d_bias_sc[i], b.data(), sizeof(float) * l.c_out, cudaMemcpyHostToDevice) != cudaSuccess) { fail(AFRAME_ECUDA, "weight upload failed"); break; }
   }
   if (st == AFRAME_OK && w->head_layer < 0) st = af_fail(ctx, AFRAME_ESHAPE, "layer table has no head");
   if (st == AFRAME_OK && pos != n_pay) st = af_fail(ctx, AFRAME_ESHAPE, "weight blob payload size mismatch");

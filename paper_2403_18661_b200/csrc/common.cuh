@@ -32,6 +32,7 @@ struct aframe_weights {
   std::vector<float*> d_w32;          // [k][c_in][c_out] fp32 (N contiguous) for the CUDA-core path
   std::vector<__nv_bfloat16*> d_w16;  // [k][c_out][c_in] bf16 (K-major) for the tcgen05 path
   std::vector<float*> d_bias;         // [c_out] fp32 folded bias
+  std::vector<float*> d_bias_sc;      // conv whose residual is a 1x1 projection conv: its bias + the projection's (else null)
   float* d_head_w = nullptr;          // [c_in]
   float head_b = 0.f;
   int head_layer = -1;

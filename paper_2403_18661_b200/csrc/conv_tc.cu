@@ -30,7 +30,7 @@ static bool encode_map(aframe_ctx* ctx, CUtensorMap* m, const void* ptr, int ran
 }
 
 struct TcLaunch {
-  CUtensorMap tm_in, tm_w, tm_out, tm_res;
+  CUtensorMap tm_in, tm_w, tm_out, tm_res, tm_scw;
   TcConvParams p;
   int BN, grid, smem;
   bool head, cg2, halo;
@@ -93,9 +93,11 @@ aframe_status af_tc_check(aframe_ctx* ctx, aframe_weights* w) {
   return AFRAME_OK;
 }
 
+// sc >= 0: layer sc is the 1x1 projection conv whose output is this layer's residual; it runs inside this launch as extra
+// K blocks on its own input sc_in (res must then be null)
 static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const __nv_bfloat16* in,
                          const __nv_bfloat16* res, __nv_bfloat16* out, int64_t nb, bool head, float* head_part,
-                         TcLaunch& L) {
+                         TcLaunch& L, int sc = -1, const __nv_bfloat16* sc_in = nullptr) {
   const LayerDesc& l = w->layers[li];
   const int BN = l.c_out >= 256 ? 256 : l.c_out;
   const int cg2_mode = env_int("AFRAME_CG2", 1);                 // 1: CTA pairs (cta_group::2) for the N = 256 layers; 2: also N = 128
@@ -123,10 +125,23 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
     const uint64_t str[3] = {(uint64_t)l.c_out * 2, (uint64_t)l.c_out * 2, (uint64_t)l.t_out * l.c_out * 2};
     const uint32_t box[4] = {64, 1, (uint32_t)T_box, (uint32_t)B_box};
     if (!encode_map(ctx, &L.tm_out, out, 4, dims, str, box)) return false;
-    if (!encode_map(ctx, &L.tm_res, res ? res : out, 4, dims, str, box)) return false;
+    if (sc < 0 && !encode_map(ctx, &L.tm_res, res ? res : out, 4, dims, str, box)) return false;
+  }
+  L.tm_scw = L.tm_w;
+  if (sc >= 0) {
+    const LayerDesc& q = w->layers[sc];
+    const uint64_t dims[4] = {(uint64_t)q.c_in, (uint64_t)q.stride, (uint64_t)(q.t_in / q.stride), (uint64_t)nb};
+    const uint64_t str[3] = {(uint64_t)q.c_in * 2, (uint64_t)q.stride * q.c_in * 2, (uint64_t)q.t_in * q.c_in * 2};
+    const uint32_t box[4] = {64, 1, (uint32_t)T_box, (uint32_t)B_box};
+    if (!encode_map(ctx, &L.tm_res, sc_in, 4, dims, str, box)) return false;
+    const uint64_t wd[3] = {(uint64_t)q.c_in, (uint64_t)q.c_out, 1};
+    const uint64_t ws[2] = {(uint64_t)q.c_in * 2, (uint64_t)q.c_out * q.c_in * 2};
+    const uint32_t wb[3] = {64, (uint32_t)(cg2 ? BN / 2 : BN), 1};
+    if (!encode_map(ctx, &L.tm_scw, w->d_w16[sc], 3, wd, ws, wb)) return false;
   }
   TcConvParams& p = L.p;
-  p.bias = w->d_bias[li];
+  p.bias = sc >= 0 ? w->d_bias_sc[li] : w->d_bias[li];
+  p.sc_kblocks = sc >= 0 ? w->layers[sc].c_in / 64 : 0;
   p.taps = l.k; p.pad = l.pad; p.P = P;
   for (int d = 0; d < 3; ++d) {
     const int sft = d - l.pad;
@@ -165,18 +180,19 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   else if (cg2 && l.k * p.kblocks < 12) { p.stages = 5; p.nbuf = 2; p.pf = r ? 1 : 0; }   // short K: the epilogue is the critical path
   else if (cg2)               { p.stages = r ? 5 : 6; p.nbuf = r ? 2 : 1; p.pf = r ? 1 : 0; }
   else if (BN == 256)         { p.stages = 3; p.nbuf = 2; p.pf = r ? 1 : 0; }
+  else if (halo && BN == 128 && sc >= 0) { p.stages = 3; p.nbuf = 1; p.pf = 0; }   // 96 + 16 KB of weights + 3 x 17 KB + 2 x 16 KB
   else if (halo && BN == 128) { p.stages = 3; p.nbuf = 2; p.pf = r ? 1 : 0; }   // 96 KB of weights + 3 x 17 KB + 4 x 16 KB
   else if (halo)              { p.stages = r ? 6 : 8; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
   else if (BN == 128)         { p.stages = r ? 4 : 5; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
   else                        { p.stages = r ? 5 : 6; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }
-  p.w_bytes = halo ? l.k * p.kblocks * BN * 128 : 0;
+  p.w_bytes = halo ? (l.k * p.kblocks + p.sc_kblocks) * BN * 128 : 0;
   p.stage_bytes = halo ? TcCfg<64>::HALO_A_BYTES : 0;     // one stage = one 64-channel block
 
   L.BN = BN;
   L.head = head;
   L.cg2 = cg2;
   L.halo = halo;
-  L.smem = (cg2 && BN == 128) ? TcCfg<128, true>::smem(p.stages, p.nbuf, false) : halo ? (BN == 128 ? TcCfg<128>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks) : TcCfg<64>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks))
+  L.smem = (cg2 && BN == 128) ? TcCfg<128, true>::smem(p.stages, p.nbuf, false) : halo ? (BN == 128 ? TcCfg<128>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks) : TcCfg<64>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks)) + p.sc_kblocks * BN * 128
          : cg2 ? TcCfg<256, true>::smem(p.stages, p.nbuf, head) : BN == 256 ? TcCfg<256>::smem(p.stages, p.nbuf, head) : (BN == 128 ? TcCfg<128>::smem(p.stages, p.nbuf, head)
                                                                             : TcCfg<64>::smem(p.stages, p.nbuf, head));
   if (cg2) L.grid = 2 * (p.num_tiles < ctx->n_sms / 2 ? p.num_tiles : ctx->n_sms / 2);
@@ -204,7 +220,7 @@ template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t lau
   at[1].val.programmaticStreamSerializationAllowed = 1;
   static const int pdl = env_int("AFRAME_PDL", 1);
   cfg.attrs = at; cfg.numAttrs = pdl ? 2 : 1;
-  return cudaLaunchKernelEx(&cfg, kern, L.tm_in, L.tm_w, L.tm_out, L.tm_res, L.p);
+  return cudaLaunchKernelEx(&cfg, kern, L.tm_in, L.tm_w, L.tm_out, L.tm_res, L.tm_scw, L.p);
 }
 
 static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s) {
@@ -296,6 +312,8 @@ struct TcPlanCache {
   std::vector<TcLaunch> launches;   // indexed by layer
   std::vector<TcBlockLaunch> blocks;  // indexed by the block's SECOND layer
   std::vector<int> fused_with;        // per layer: index of the partner layer if the pair runs fused, else -1
+  std::vector<int> sc_of;             // per layer: the projection-shortcut conv that runs inside it (else -1)
+  std::vector<char> skip;             // per layer: runs inside another launch
 };
 static std::map<aframe_ctx*, std::vector<TcPlanCache>> g_cache;
 
@@ -358,6 +376,24 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       pc->launches.resize(n);
       pc->blocks.resize(n);
       pc->fused_with.assign(n, -1);
+      pc->sc_of.assign(n, -1);
+      pc->skip.assign(n, 0);
+      // projection shortcut (1x1 conv, no ReLU, read only as layer i's residual): folded into layer i as extra K blocks,
+      // which saves its launch, the write of its output and the residual read (the accumulation also stays in fp32)
+      if (env_int("AFRAME_FUSE_SC", 1) && !w->live_gn)
+        for (int i = 2; i < n; ++i) {
+          const LayerDesc& l = w->layers[i];
+          const int r = l.residual_from;
+          if (l.kind != 0 || r < 2 || i == fuse || !w->d_bias_sc[i]) continue;
+          const LayerDesc& q = w->layers[r];
+          bool ok = q.kind == 0 && q.k == 1 && q.pad == 0 && !q.relu && q.residual_from < 0 && q.c_in % 64 == 0 &&
+                    q.t_out == l.t_out && q.c_out == l.c_out && q.t_in % q.stride == 0 && q.input_from >= 1 &&
+                    l.k * (l.c_in / 64) + q.c_in / 64 <= 64;
+          for (int j = 0; ok && j < n; ++j)
+            if (j != i && (w->layers[j].input_from == r || w->layers[j].residual_from == r)) ok = false;
+          if (w->layers[i].input_from == r) ok = false;
+          if (ok) { pc->sc_of[i] = r; pc->skip[r] = 1; }
+        }
       if (env_int("AFRAME_FUSE_BLOCK", 1) && !w->live_gn)
         for (int i = 2; i < n; ++i) {
           const int ib = pc->fused_with[i] < 0 ? fusable_block(w, i) : -1;
@@ -367,9 +403,13 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         }
       for (int i = 2; i < n; ++i) {
         const LayerDesc& l = w->layers[i];
-        if (l.kind != 0 || pc->fused_with[i] >= 0) continue;
-        if (!build_launch(ctx, w, i, slot_ptr(l.input_from), l.residual_from >= 0 && !w->live_gn ? slot_ptr(l.residual_from) : nullptr,
-                          slot_ptr(i), nb, i == fuse, head_part, pc->launches[i])) { caches.pop_back(); return AFRAME_ECUDA; }
+        if (l.kind != 0 || pc->fused_with[i] >= 0 || pc->skip[i]) continue;
+        const int sc = pc->sc_of[i];
+        if (!build_launch(ctx, w, i, slot_ptr(l.input_from),
+                          l.residual_from >= 0 && !w->live_gn && sc < 0 ? slot_ptr(l.residual_from) : nullptr, slot_ptr(i), nb,
+                          i == fuse, head_part, pc->launches[i], sc, sc >= 0 ? slot_ptr(w->layers[sc].input_from) : nullptr)) {
+          caches.pop_back(); return AFRAME_ECUDA;
+        }
       }
     }
     const size_t esz = in_bf16 ? 2 : 4;
@@ -395,6 +435,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       const LayerDesc& l = w->layers[i];
       struct Rec { aframe_ctx* c; std::vector<cudaEvent_t>& v; int i; ~Rec() { if (c->layer_ms) cudaEventRecord(v[i + 1], c->stream); } } rec{ctx, lev, i};
       if (l.kind == 0 && pc->fused_with[i] > i) continue;      // first conv of a fused block: runs with its partner
+      if (pc->skip[i]) continue;                               // projection shortcut: runs inside the conv it feeds
       if (l.kind == 0) {
         // Alternate the direction in which consecutive launches walk their tiles: a layer then starts with the rows its
         // producer wrote LAST, which are still in L2 (walking every layer forwards evicts exactly the lines that are

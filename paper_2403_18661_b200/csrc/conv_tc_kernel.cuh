@@ -61,6 +61,10 @@ struct TcConvParams {
   // the tile through a shared-memory descriptor whose start address is shifted by d rows (d * 128 B).  Measured on B200:
   // the 128-byte swizzle is applied to the absolute shared-memory address, so the shifted start needs no other change
   // (setting the descriptor's base-offset field to the shift gives wrong results).
+  // fused projection shortcut: out += W_sc x_sc, sc_kblocks extra K blocks after the taps, read through tm_res (the
+  // strided 1x1 view of the block input) and tm_scw; then has_res = 0 and bias holds b + b_sc.  HALO keeps the shortcut
+  // weights resident after the main ones.
+  int sc_kblocks;
   int w_bytes;               // resident weight region (0 unless HALO)
   int stage_bytes;           // bytes per main-loop stage
   long long* dbg_out;        // timing experiments: per-role cycle counters of CTA 0 (null = off)
@@ -139,8 +143,8 @@ __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4
 template <int BN, bool HEAD, bool CG2, bool HALO>
 __global__ void __launch_bounds__(TcCfg<BN, CG2>::THREADS, 1)
 conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 rows */, const __grid_constant__ CUtensorMap tm_w,
-               const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_res,
-               const TcConvParams p) {
+               const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_res /* or shortcut input */,
+               const __grid_constant__ CUtensorMap tm_scw /* shortcut weights */, const TcConvParams p) {
   using Cfg = TcCfg<BN, CG2>;
   constexpr int EG = Cfg::EG;
   constexpr bool SPLIT = Cfg::SPLIT;
@@ -184,7 +188,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     mbar_init(w_bar, 1);
     for (int g = 0; g < EG; ++g)
       for (int b = 0; b < MAXBUF; ++b) mbar_init(res_bar(g, b), 1);
-    if (p.has_res) tma_prefetch_desc(&tm_res);
+    if (p.has_res || p.sc_kblocks) tma_prefetch_desc(&tm_res);
+    if (p.sc_kblocks) tma_prefetch_desc(&tm_scw);
     fence_mbar_init();
   }
   if (warp == 1) { if (CG2) tmem_alloc_cg2(tmem_slot, 512); else tmem_alloc(tmem_slot, 512); }
@@ -203,7 +208,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
   pdl_launch_dependents();
   if (!(HALO && warp == 0)) pdl_wait();            // (the halo producer first issues its weight loads, see below)
 
-  const int kiters = p.taps * p.kblocks;
+  const int kiters = p.taps * p.kblocks + p.sc_kblocks;
   // cycle accounting for experiments (CTA 0 only): T(slot) adds the cycles since the previous T() of this thread
   const bool prof = p.dbg_out != nullptr && blockIdx.x == 0;
   long long tprev = prof ? clock64() : 0, tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -229,6 +234,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         for (int d = 0; d < p.taps; ++d)
           for (int kb = 0; kb < p.kblocks; ++kb)
             tma_load_3d(w_base + (uint32_t)((d * p.kblocks + kb) * BN * 128), &tm_w, w_bar, kb * 64, 0, d);
+        for (int kb = 0; kb < p.sc_kblocks; ++kb)
+          tma_load_3d(w_base + (uint32_t)((p.taps * p.kblocks + kb) * BN * 128), &tm_scw, w_bar, kb * 64, 0, 0);
       }
       __syncwarp();
       pdl_wait();                                  // the activations below are the previous layer's output
@@ -249,6 +256,15 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
           T(2);
+        }
+        for (int kb = 0; kb < p.sc_kblocks; ++kb) {   // shortcut: the 128 rows x_sc[t0 ..] of one 64-channel block
+          mbar_wait(empty_bar(stage), phase ^ 1u);
+          if (elect_one()) {
+            mbar_arrive_expect_tx(full_bar(stage), 128 * 128);
+            tma_load_4d(stage_base + stage * STAGE_BYTES, &tm_res, full_bar(stage), kb * 64, 0, t0, b0);
+          }
+          __syncwarp();
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
       }
       if (lane == 0) Tflush(0);
@@ -283,6 +299,24 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             T(2);
           }
+        }
+        for (int kb = 0; kb < p.sc_kblocks; ++kb) {   // fused projection shortcut: A from the strided block input
+          mbar_wait(empty_bar(stage), phase ^ 1u);
+          const uint32_t sa = stage_base + stage * STAGE_BYTES;
+          if (elect_one()) {
+            if (CG2) {
+              if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * Cfg::STAGE_BYTES);
+              const uint32_t lbar = lfull0 + 8u * stage;
+              tma_load_4d_cg2(sa, &tm_res, lbar, kb * 64, 0, t0, b0);
+              tma_load_3d_cg2(sa + Cfg::A_BYTES, &tm_scw, lbar, kb * 64, n0 + (int)rank * Cfg::B_ROWS, 0);
+            } else {
+              mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
+              tma_load_4d(sa, &tm_res, full_bar(stage), kb * 64, 0, t0, b0);
+              tma_load_3d(sa + Cfg::A_BYTES, &tm_scw, full_bar(stage), kb * 64, n0, 0);
+            }
+          }
+          __syncwarp();
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
       }
       if (lane == 0) Tflush(0);
@@ -322,6 +356,19 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             __syncwarp();
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             T(3);
+          }
+          for (int kb = 0; kb < p.sc_kblocks; ++kb) {   // shortcut K block: plain 128-row tile, its resident weights
+            mbar_wait(full_bar(stage), phase);
+            tc_fence_after();
+            if (elect_one()) {
+              const uint32_t a_lo = umma_desc_lo(stage_base + stage * STAGE_BYTES);
+              const uint32_t b_lo = umma_desc_lo(w_base + (uint32_t)((p.taps * p.kblocks + kb) * BN * 128));
+#pragma unroll
+              for (int m = 0; m < 4; ++m) umma_bf16_lohi<true>(d_tmem, a_lo + m * 2, b_lo + m * 2, idesc);
+              umma_commit(empty_bar(stage));
+            }
+            __syncwarp();
+            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
           }
         }
         for (int it = 0; it < (HALO ? 0 : kiters); ++it) {

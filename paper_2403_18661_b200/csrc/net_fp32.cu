@@ -196,6 +196,10 @@ bool af_make_plan(const aframe_weights* w, bool fuse_stem_pool, NetPlan& plan) {
     const LayerDesc& l = w->layers[i];
     if (l.input_from >= 0) last_use[l.input_from] = i;
     if (l.residual_from >= 0) last_use[l.residual_from] = i;
+    // a 1x1 projection shortcut may run INSIDE the conv it feeds (conv_tc.cu): that conv then reads the projection's input
+    if (l.kind == 0 && l.residual_from >= 0 && w->layers[l.residual_from].kind == 0 && w->layers[l.residual_from].k == 1 &&
+        w->layers[l.residual_from].input_from >= 0)
+      last_use[w->layers[l.residual_from].input_from] = i;
   }
   std::vector<int> slot_free_at;   // layer index after which the slot is free (-1 = free now)
   plan.n_slots = 0;
