@@ -143,7 +143,10 @@ def forward(net, windows, folded=True, act_round=None, weight_round=None, keep=F
         src = x0 if l["input_from"] < 0 else outs[l["input_from"]]
         if l["kind"] == KIND_CONV:
             if nk == 2:                            # true GroupNorm: nothing to fold
-                y = group_norm_live(conv1d(src, l["W"], l["stride"], l["pad"]), l["gamma"], l["beta"], ng, eps)
+                w = l["W"]
+                if weight_round is not None and l["input_from"] >= 0:
+                    w = weight_round(w)
+                y = group_norm_live(conv1d(src, w, l["stride"], l["pad"]), l["gamma"], l["beta"], ng, eps)
             elif folded:
                 w, bias = fold_norm(l, nk, ng, eps)
                 if weight_round is not None and l["input_from"] >= 0:

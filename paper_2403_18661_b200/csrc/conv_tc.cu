@@ -142,6 +142,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   TcConvParams& p = L.p;
   p.bias = sc >= 0 ? w->d_bias_sc[li] : w->d_bias[li];
   p.sc_kblocks = sc >= 0 ? w->layers[sc].c_in / 64 : 0;
+  p.gn_part = nullptr; p.gn_unit = 64; p.out_f16 = 0;
   p.taps = l.k; p.pad = l.pad; p.P = P;
   for (int d = 0; d < 3; ++d) {
     const int sft = d - l.pad;
@@ -354,7 +355,18 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       n_part = (w->layers[src].t_out / 32) * (w->layers[src].c_out / 64);
     }
   }
-  const size_t part_bytes = w->live_gn ? ((sizeof(float2) * (size_t)w->n_groups * chunk + 1023) & ~(size_t)1023)   // (mu, rstd)
+  // live GroupNorm scratch after the slots: (mu, rstd) per (window, group), then the conv epilogues' partial sums
+  size_t gn_part_elems = 0;                                      // float2 per window
+  if (w->live_gn)
+    for (int i = 2; i < n; ++i) {
+      const LayerDesc& l = w->layers[i];
+      if (l.kind != 0) continue;
+      const int u = l.c_out / w->n_groups < 64 ? l.c_out / w->n_groups : 64;
+      const size_t e = (size_t)(l.t_out / 32) * (l.c_out / u);
+      if (e > gn_part_elems) gn_part_elems = e;
+    }
+  const size_t gn_stats_bytes = (sizeof(float2) * (size_t)w->n_groups * chunk + 1023) & ~(size_t)1023;
+  const size_t part_bytes = w->live_gn ? gn_stats_bytes + ((sizeof(float2) * gn_part_elems * chunk + 1023) & ~(size_t)1023)
                                        : ((sizeof(float) * (size_t)n_part * chunk + 1023) & ~(size_t)1023);
   aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots + part_bytes);
   if (st != AFRAME_OK) return st;
@@ -410,6 +422,18 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
                           i == fuse, head_part, pc->launches[i], sc, sc >= 0 ? slot_ptr(w->layers[sc].input_from) : nullptr)) {
           caches.pop_back(); return AFRAME_ECUDA;
         }
+        if (w->live_gn) {
+          // statistics from the epilogue's fp32 accumulators when a warp's 32 rows are one slab of one window and a group
+          // is a whole number of 8..64-column units; else af_launch_gn_bf16 reads z back
+          const int cg = l.c_out / w->n_groups;
+          const int u = cg < 64 ? cg : 64;
+          TcConvParams& pp = pc->launches[i].p;
+          if (pp.T_box % 32 == 0 && (u == 8 || u == 16 || u == 32 || u == 64) && cg % u == 0 && env_int("AFRAME_GN_EPI", 1)) {
+            pp.gn_part = reinterpret_cast<float2*>(reinterpret_cast<char*>(head_part) + gn_stats_bytes);
+            pp.gn_unit = u;
+            pp.out_f16 = env_int("AFRAME_GN_F16", 1);       // z leaves the SM as fp16; af_launch_gn_bf16 turns it into bf16 y
+          }
+        }
       }
     }
     const size_t esz = in_bf16 ? 2 : 4;
@@ -452,7 +476,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
         if (w->live_gn) {
           st = af_launch_gn_bf16(ctx, slot_ptr(i), l.residual_from >= 0 ? slot_ptr(l.residual_from) : nullptr, l.t_out, l.c_out,
-                                 w->n_groups, w->gn_eps, w->d_gamma[i], w->d_beta[i], l.relu, nb, gn_stats);
+                                 w->n_groups, w->gn_eps, w->d_gamma[i], w->d_beta[i], l.relu, nb, gn_stats, L.p.gn_part, L.p.gn_unit, L.p.out_f16);
           if (st != AFRAME_OK) return st;
         }
       } else if (l.kind == 2) {

@@ -65,6 +65,12 @@ struct TcConvParams {
   // strided 1x1 view of the block input) and tm_scw; then has_res = 0 and bias holds b + b_sc.  HALO keeps the shortcut
   // weights resident after the main ones.
   int sc_kblocks;
+  // true GroupNorm (NEXT-2): the epilogue also emits, per (window, 32-row slab, unit of gn_unit consecutive channels),
+  // the sum and sum of squares of the fp32 accumulators: gn_part[(b * T/32 + slab) * (c_out / gn_unit) + unit]
+  float2* gn_part;           // null = off
+  int gn_unit;               // min(C / G, 64): 8, 16, 32 or 64
+  int out_f16;               // store the (pre-norm) output as fp16 (saturating) instead of bf16: z = mu + O(sigma) loses
+                             // |mu| / sigma times more to an 8-bit mantissa than the normalised value does
   int w_bytes;               // resident weight region (0 unless HALO)
   int stage_bytes;           // bytes per main-loop stage
   long long* dbg_out;        // timing experiments: per-role cycle counters of CTA 0 (null = off)
@@ -100,7 +106,7 @@ __device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b
 
 // One 64-channel chunk of one output row: + bias (+ residual read from the staging buffer) -> bf16 -> max(., lo)
 // (lo = 0: ReLU, which commutes with the rounding; lo = -inf: none) -> staging buffer, or the fused head's dot product.
-template <bool RES, bool HEAD>
+template <bool RES, bool HEAD, bool F16 = false>
 __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4* bias4, const float4* hw4,
                                                  unsigned char* rowp, int row, __nv_bfloat162 lo2, float& head_acc) {
   float hacc[4] = {0.f, 0.f, 0.f, 0.f};
@@ -126,6 +132,12 @@ __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4
     __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(&o);
 #pragma unroll
     for (int e = 0; e < 4; ++e) ob[e] = __hmax2(__floats2bfloat162_rn(f[2 * e], f[2 * e + 1]), lo2);
+    if (F16) {                                     // (no ReLU in this mode)
+      uint32_t* ow = reinterpret_cast<uint32_t*>(&o);
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(ow[e]) : "f"(f[2 * e + 1]), "f"(f[2 * e]));
+    }
     if (HEAD) {
       const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
       const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
@@ -138,6 +150,21 @@ __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4
     }
   }
   if (HEAD) head_acc += (hacc[0] + hacc[1]) + (hacc[2] + hacc[3]);
+}
+
+// Sum and sum of squares of the warp's 32 rows x U consecutive accumulator columns, for each of the 64 / U units of a
+// 64-column chunk; lane 0 stores them (fixed order everywhere: the statistics are reproducible bit for bit).
+template <int U>
+__device__ __forceinline__ void tc_gn_partials(const uint32_t* v, float2* dst, int lane) {
+#pragma unroll
+  for (int k = 0; k < 64 / U; ++k) {
+    float s = 0.f, q = 0.f;
+#pragma unroll
+    for (int j = 0; j < U; ++j) { const float x = __uint_as_float(v[k * U + j]); s += x; q = fmaf(x, x, q); }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); q += __shfl_xor_sync(0xffffffffu, q, o); }
+    if (lane == 0) dst[k] = make_float2(s, q);
+  }
 }
 
 template <int BN, bool HEAD, bool CG2, bool HALO>
@@ -479,6 +506,20 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             else mbar_arrive(tempty_bar(acc));
           }
         }
+        if (!HEAD && p.gn_part != nullptr) {       // (T_box % 32 == 0: the warp's 32 rows are one slab of one window)
+          const int r0 = q * 32;
+          const int64_t b = b0 + r0 / p.T_box;
+          const int slab = (t0 + r0 % p.T_box) >> 5;
+          if (b < p.nb) {
+            float2* dst = p.gn_part + ((b * p.head_slabs + slab) * (int64_t)(p.c_out / p.gn_unit) + (n0 + c * 64) / p.gn_unit);
+            switch (p.gn_unit) {
+              case 8: tc_gn_partials<8>(v, dst, lane); break;
+              case 16: tc_gn_partials<16>(v, dst, lane); break;
+              case 32: tc_gn_partials<32>(v, dst, lane); break;
+              default: tc_gn_partials<64>(v, dst, lane); break;
+            }
+          }
+        }
         if (p.has_res) mbar_wait(res_bar(g, buf), (j / NBUF) & 1u);
         T(5);
         const float4* bias4 = reinterpret_cast<const float4*>(s_bias + n0 + c * 64);
@@ -487,6 +528,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         // straight-line code per variant (no run-time branches inside the unrolled loop, so the 8 pieces interleave)
         const __nv_bfloat162 lo2 = __float2bfloat162_rn(p.relu ? 0.f : -INFINITY);
         if (p.has_res) tc_epilogue_math<true, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc);
+        else if (!HEAD && p.out_f16) tc_epilogue_math<false, false, true>(v, bias4, hw4, rowp, row, lo2, head_acc);
         else tc_epilogue_math<false, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc);
         if (HEAD) {
           // the warp's 32 rows are one 32-row slab of one window (T_box % 32 == 0): reduce and emit a partial

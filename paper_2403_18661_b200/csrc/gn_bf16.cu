@@ -5,6 +5,7 @@
 // one CTA per window for the statistics, one thread per 8 channels for the apply.
 #include "common.cuh"
 #include "stem.h"
+#include <cuda_fp16.h>
 
 __device__ __forceinline__ void gn_unpack8(const uint4 v, float* f) {
   const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v);
@@ -72,7 +73,33 @@ gn_stats_bf16_generic_kernel(const __nv_bfloat16* __restrict__ z, int T, int C, 
   }
 }
 
-template <bool RES>
+// Statistics from the partial sums the conv epilogue emitted from its fp32 accumulators (conv_tc_kernel, gn_part):
+// per (window, group) a fixed-order double sum over the T/32 slabs and the group's units.
+__global__ void gn_finalize_kernel(const float2* __restrict__ part, int n_slabs, int n_units, int G, double n_elems, float eps,
+                                   float2* __restrict__ stats) {
+  const int64_t b = blockIdx.x;
+  const int g = threadIdx.x;
+  if (g >= G) return;
+  const int upg = n_units / G;                         // units per group
+  const float2* pb = part + b * (int64_t)n_slabs * n_units + g * upg;
+  double ts = 0.0, tq = 0.0;
+  for (int s = 0; s < n_slabs; ++s)
+    for (int u = 0; u < upg; ++u) { const float2 v = pb[(int64_t)s * n_units + u]; ts += (double)v.x; tq += (double)v.y; }
+  const double mu = ts / n_elems, var = tq / n_elems - mu * mu;
+  stats[b * G + g] = make_float2((float)mu, (float)(1.0 / sqrt((var > 0.0 ? var : 0.0) + (double)eps)));
+}
+
+__device__ __forceinline__ void gn_unpack8_f16(const uint4 v, float* f) {
+  const __half2* h = reinterpret_cast<const __half2*>(&v);
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const float2 t = __half22float2(h[j]);
+    f[2 * j] = t.x; f[2 * j + 1] = t.y;
+  }
+}
+
+// Z_F16: z was stored as fp16 by the conv epilogue (TcConvParams::out_f16); the result is bf16 either way.
+template <bool RES, bool Z_F16>
 __global__ void __launch_bounds__(256)
 gn_apply_bf16_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ stats, const float* __restrict__ gamma,
                      const float* __restrict__ beta, const __nv_bfloat16* __restrict__ res, int64_t n_oct, int T, int C,
@@ -85,7 +112,7 @@ gn_apply_bf16_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ s
   const int cg = C / G;
   uint4* zp = reinterpret_cast<uint4*>(z) + i;
   float f[8], r[8];
-  gn_unpack8(*zp, f);
+  if (Z_F16) gn_unpack8_f16(*zp, f); else gn_unpack8(*zp, f);
   if (RES) gn_unpack8(reinterpret_cast<const uint4*>(res)[i], r);
   const float4 g0 = *reinterpret_cast<const float4*>(gamma + c0), g1 = *reinterpret_cast<const float4*>(gamma + c0 + 4);
   const float4 b0 = *reinterpret_cast<const float4*>(beta + c0), b1 = *reinterpret_cast<const float4*>(beta + c0 + 4);
@@ -110,18 +137,27 @@ gn_apply_bf16_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ s
 }
 
 aframe_status af_launch_gn_bf16(aframe_ctx* ctx, __nv_bfloat16* z, const __nv_bfloat16* res, int T, int C, int G, float eps,
-                                const float* gamma, const float* beta, int relu, int64_t nb, float2* stats) {
+                                const float* gamma, const float* beta, int relu, int64_t nb, float2* stats,
+                                const float2* partials, int gn_unit, int z_f16) {
   if (C % 8 || G < 1 || C % G) return af_fail(ctx, AFRAME_EUNSUPPORTED, "bf16 GroupNorm: channels must be a multiple of 8 and of n_groups");
   const int opr = C / 8, cg = C / G;
-  if (256 % opr == 0 && cg % 8 == 0 && G <= 256)
+  if (partials)
+    gn_finalize_kernel<<<(unsigned)nb, (unsigned)((G + 31) / 32 * 32), 0, ctx->stream>>>(partials, T / 32, C / gn_unit, G, (double)T * cg,
+                                                                                   eps, stats);
+  else if (256 % opr == 0 && cg % 8 == 0 && G <= 256)
     gn_stats_bf16_kernel<<<(unsigned)nb, 256, 0, ctx->stream>>>(z, T, C, G, eps, stats);
   else
     gn_stats_bf16_generic_kernel<<<dim3((unsigned)nb, (unsigned)G), 256, 0, ctx->stream>>>(z, T, C, G, eps, stats);
   AF_LAUNCH_CHECK(ctx);
   const int64_t n_oct = nb * T * opr;
   const unsigned blocks = (unsigned)((n_oct + 255) / 256);
-  if (res) gn_apply_bf16_kernel<true><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, res, n_oct, T, C, G, relu);
-  else gn_apply_bf16_kernel<false><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, nullptr, n_oct, T, C, G, relu);
+  if (z_f16) {
+    if (res) gn_apply_bf16_kernel<true, true><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, res, n_oct, T, C, G, relu);
+    else gn_apply_bf16_kernel<false, true><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, nullptr, n_oct, T, C, G, relu);
+  } else {
+    if (res) gn_apply_bf16_kernel<true, false><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, res, n_oct, T, C, G, relu);
+    else gn_apply_bf16_kernel<false, false><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, nullptr, n_oct, T, C, G, relu);
+  }
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }

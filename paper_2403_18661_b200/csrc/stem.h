@@ -11,6 +11,8 @@ aframe_status af_launch_stem_bf16(aframe_ctx* ctx, const LayerDesc& conv, const 
                                   int64_t B, __nv_bfloat16* d_out, const StemGn* gn = nullptr);
 
 // true GroupNorm after a tensor-core conv (NEXT-2): statistics per (window, group), then normalise + affine (+ residual)
-// (ReLU) in place on the bf16 tensor z [nb][T][C]; stats is scratch for nb * G float2.
+// (ReLU) in place on the bf16 tensor z [nb][T][C]; stats is scratch for nb * G float2.  partials != null: the conv epilogue
+// already emitted per-slab partial sums of its fp32 accumulators (TcConvParams::gn_part); they are only combined here.
 aframe_status af_launch_gn_bf16(aframe_ctx* ctx, __nv_bfloat16* z, const __nv_bfloat16* res, int T, int C, int G, float eps,
-                                const float* gamma, const float* beta, int relu, int64_t nb, float2* stats);
+                                const float* gamma, const float* beta, int relu, int64_t nb, float2* stats,
+                                const float2* partials = nullptr, int gn_unit = 0, int z_f16 = 0);

@@ -182,9 +182,16 @@ def test_true_group_norm_full_size_fp32_and_bf16(af, config1):
     got = ctx16.forward(w16, x).cpu().numpy().astype(np.float64)
     err = rel_err(got, ref)
     rho = scipy.stats.spearmanr(got, ref).statistic
-    print(f"live GroupNorm bf16: rel err {err:.3e}, spearman {rho:.5f}")
+    # rule T4 in context: this randomly initialised live-GN network squeezes its scores into a 2 % band, so even the ideal
+    # bf16 evaluation (oracle with bf16 weights and one bf16 rounding per layer output) does not reach 0.999 here
+    net = onet.parse_blob(blob)
+    ideal = onet.forward(net, wins, act_round=onet.round_bf16, weight_round=onet.round_bf16)
+    rho_ideal = scipy.stats.spearmanr(ideal, ref).statistic
+    print(f"live GroupNorm bf16: rel err {err:.3e}, spearman {rho:.5f} (ideal-bf16 ceiling {rho_ideal:.5f}, "
+          f"its rel err {rel_err(ideal, ref):.3e})")
     assert err <= 2e-2
-    assert rho >= 0.99
+    assert rho >= rho_ideal - 3e-3
+    assert rel_err(got, ideal) <= 1e-2
     for nb in (1, 37):
         part = ctx16.forward(w16, x[:nb]).cpu().numpy()
         assert np.array_equal(part, got[:nb].astype(np.float32))
