@@ -380,9 +380,9 @@ def run_ours(args):
         "roofline": {"kernel": "conv_tc_kernel<BN> (35 residual-stage convolutions, tcgen05 implicit GEMM)",
                      "bound": "tensor", "achieved": conv_tflops, "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
                      "frac": conv_tflops / peaks["bf16_sustained"],
-                     # dram__bytes_read.sum + dram__bytes_write.sum of the 32 conv launches of one 4096-window batch under
-                     # ncu --set full (profiles/r01c_conv_full.md): 28.9 GB, i.e. per launch on average
-                     "traffic": 28.9e9 / 32,
+                     # dram__bytes_read.sum + dram__bytes_write.sum of the 29 conv launches of one 4096-window batch under
+                     # ncu --set full (profiles/r01d_conv_full.md): 16.5 + 10.1 GB, i.e. per launch on average
+                     "traffic": 26.66e9 / 29,
                      "peak_kind": "sustained bf16 cuBLAS, " + peaks["source"], "launches": int(conv_launches),
                      "avg_launch_ms": conv_ms / max(conv_launches, 1),
                      "algorithmic": "2 x 1069.5 MMAC per window x windows scored, over the summed CUDA-event time of "
