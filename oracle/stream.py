@@ -42,6 +42,7 @@ class StreamConfig:
     stride: int = 128
     psd_len: int = 131072
     psd_update: int = 16384
+    welch_average: str = "mean"      # NEXT-3 variant: "median" (oracle/psd.py)
 
 
 def unfold(y, kernel_len, stride, first=0, shifts=None, n_windows=None):
@@ -81,7 +82,7 @@ def epoch_of_sample(m, cfg: StreamConfig):
 def epoch_filter(x, e, cfg: StreamConfig):
     """Filter of PSD epoch e: Welch over x[n_e - psd_len : n_e], n_e = psd_len + e psd_update."""
     n_e = cfg.psd_len + e * cfg.psd_update
-    p = _psd.welch(x[n_e - cfg.psd_len: n_e], cfg.fs, cfg.welch_nfft, cfg.welch_hop)
+    p = _psd.welch(x[n_e - cfg.psd_len: n_e], cfg.fs, cfg.welch_nfft, cfg.welch_hop, cfg.welch_average)
     return _wh.design_filter(p, cfg.fs, cfg.welch_nfft, cfg.n_design, cfg.filter_len, cfg.f_lo, cfg.f_hi)
 
 
@@ -127,7 +128,8 @@ class StreamOracle:
         n, half = self.n, cfg.filter_len // 2
         if n >= cfg.psd_len and (n - cfg.psd_len) % cfg.psd_update == 0:
             self.h = [
-                _wh.design_filter(_psd.welch(self.raw[c, n - cfg.psd_len: n], cfg.fs, cfg.welch_nfft, cfg.welch_hop),
+                _wh.design_filter(_psd.welch(self.raw[c, n - cfg.psd_len: n], cfg.fs, cfg.welch_nfft, cfg.welch_hop,
+                                             cfg.welch_average),
                                   cfg.fs, cfg.welch_nfft, cfg.n_design, cfg.filter_len, cfg.f_lo, cfg.f_hi)
                 for c in range(self.c)]
             self.n_psd_updates += 1

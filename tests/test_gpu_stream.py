@@ -213,3 +213,53 @@ def test_other_inference_rates(af, stride):
     n_win = (white.shape[1] - tc["kernel_len"]) // stride + 1
     off = ctx.forward_strided(w, white, 0, n_win).cpu().numpy()
     assert n_win == len(want) and rel_err(off, want) <= 1e-4
+
+
+@pytest.mark.parametrize("average", ["mean", "median"])
+def test_eight_second_psd_and_median_variants_in_the_streaming_state(af, average):
+    """NEXT-3: the 8 s PSD of P:102 (psd_len 16384 = 7 segments) refreshed every 2 s, with the mean or the median over the
+    segments, through the streaming state and the rolling offline call, tiny network in fp32, against the oracle."""
+    tc = tiny_config()
+    psd_len, psd_update = 16384, 4096
+    n_updates = (psd_len + tc["kernel_len"] + 3 * psd_update) // S + 5
+    x = coloured_noise(n_updates * S, seed=1003)
+    x[1, 20000] += 2e-19                                          # a glitch inside several PSD epochs
+    cfg = ost.StreamConfig(kernel_len=tc["kernel_len"], n_design=4096, psd_len=psd_len, psd_update=psd_update,
+                           welch_average=average)
+    blob = make_weight_blob(**tc)
+    so = ost.StreamOracle(cfg, net=onet.parse_blob(blob))
+    ref = [so.step(x[:, u * S:(u + 1) * S].astype(np.float64)) for u in range(n_updates)]
+    assert so.n_psd_updates >= 4
+    ctx = af.Context(n_design=4096, kernel_len=tc["kernel_len"], psd_len=psd_len, psd_update=psd_update,
+                     welch_average=1 if average == "median" else 0, precision=af.FP32)
+    w = ctx.load_weights(blob)
+    flags, scores = _run_stream(af, ctx, w, x, n_updates)
+    np.testing.assert_array_equal(flags, [0 if r is None else 1 for r in ref])
+    want = np.array([r for r in ref if r is not None])
+    assert len(want) > 3 * psd_update // S and rel_err(scores[flags == 1], want) <= 1e-4
+    white = ctx.whiten_rolling(torch.from_numpy(x).cuda()).contiguous()
+    n_win = (white.shape[1] - tc["kernel_len"]) // S + 1
+    off = ctx.forward_strided(w, white, 0, n_win).cpu().numpy()
+    assert n_win == len(want) and rel_err(off, want) <= 1e-4
+
+
+def test_stride_one_windows_offline(af):
+    """NEXT-3 ("2048 Hz" online inference = one window per sample): rolling whitening and in-place windows at
+    stride 1, tiny network in fp32, against the oracle."""
+    tc = tiny_config()
+    K = tc["kernel_len"]
+    x = coloured_noise(131072 + 4096 + K, seed=1004)
+    cfg = ost.StreamConfig(kernel_len=K, n_design=4096, stride=1)
+    blob = make_weight_blob(**tc)
+    ctx = af.Context(n_design=4096, kernel_len=K, stride=1, precision=af.FP32)
+    w = ctx.load_weights(blob)
+    white = ctx.whiten_rolling(torch.from_numpy(x).cuda()).contiguous()
+    y = np.stack([ost.whiten_rolling(x[c].astype(np.float64), cfg)[0] for c in range(2)])
+    assert white.shape[1] == y.shape[1]
+    rms = np.sqrt(np.mean(y ** 2))
+    assert np.abs(white.cpu().numpy() - y).max() <= 1e-4 * rms                 # rule T1
+    n_win = 333
+    got = ctx.forward_strided(w, white, 0, n_win).cpu().numpy()
+    wins = ost.unfold(y, K, 1, n_windows=n_win)
+    ref = onet.forward(onet.parse_blob(blob), wins)
+    assert rel_err(got, ref) <= 1e-4
