@@ -396,10 +396,12 @@ def run_ours(args):
         out["roofline_whiten"] = {"kernel": "whiten_os_kernel", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"],
                                   "unit": "GB/s", "frac": gbs / peaks["hbm"], "traffic": None,
                                   "algorithmic": "4 B in + 2 B (bf16) out per whitened sample per channel",
-                                  # the binding resource: two 4096-point complex FFTs + untangle per 6144
-                                  # valid samples = 94 flop per sample, against 148 SMs x 128 lanes x 2 x 1.965 GHz
-                                  "alu": {"bound": "alu", "achieved": 94.0 * gbs / 6.0 / 1e3, "peak": 148 * 128 * 2 * 1.965e9 / 1e12,
-                                          "unit": "TFLOP/s fp32", "frac": (94.0 * gbs / 6.0 / 1e3) / (148 * 128 * 2 * 1.965e9 / 1e12)}}
+                                  # the binding resource (profiles/r01d_whiten_full.md): instruction issue.
+                                  # ncu counts 137 thread instructions per whitened sample per channel (two 4096-point complex
+                                  # FFTs, untangle and spectral multiply per 6144 valid samples); peak = 148 SMs x 128 lanes x
+                                  # 1.965 GHz thread instructions per second
+                                  "alu": {"bound": "alu", "achieved": 137.0 * gbs / 6.0 / 1e3, "peak": 148 * 128 * 1.965e9 / 1e12,
+                                          "unit": "T thread-instructions/s", "frac": (137.0 * gbs / 6.0 / 1e3) / (148 * 128 * 1.965e9 / 1e12)}}
     we_ms = stages["welch"][0]
     if we_ms > 0:
         gbs = args.steps * 2 * n_raw * 4 / (we_ms * 1e-3) / 1e9                   # every raw sample enters the PSD once
