@@ -485,7 +485,7 @@ def next_rows(af, torch, stream, peaks):
         ms = timed(lambda: ctx.forward(wg, xw), 5)
         res["live_group_norm"] = {"workload": "4096 windows, ResNet54 with per-window GroupNorm statistics", "ms": ms,
                                   "windows_per_s": 4096 / (ms * 1e-3),
-                                  "note": "HBM-bound by the statistics + apply passes after every conv (DESIGN.md NEXT-2)"}
+                                  "note": "HBM-bound by the normalise + residual + ReLU pass after every conv (DESIGN.md NEXT-2)"}
     return res
 
 

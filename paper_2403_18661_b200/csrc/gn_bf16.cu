@@ -99,11 +99,60 @@ __device__ __forceinline__ void gn_unpack8_f16(const uint4 v, float* f) {
 }
 
 // Z_F16: z was stored as fp16 by the conv epilogue (TcConvParams::out_f16); the result is bf16 either way.
+// Fast path (256 % (C/8) == 0): a CTA takes GN_ITER * 256 consecutive 8-channel octets of ONE window, so a thread always
+// sees the same 8 channels: its 8 (scale, shift) pairs -- scale = rstd_g gamma_c, shift = beta_c - mu_g scale -- are set
+// up once and every octet costs one 16-byte load (two with a residual), 8 FMAs and one 16-byte store.
+constexpr int GN_ITER = 4;
 template <bool RES, bool Z_F16>
 __global__ void __launch_bounds__(256)
 gn_apply_bf16_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ stats, const float* __restrict__ gamma,
-                     const float* __restrict__ beta, const __nv_bfloat16* __restrict__ res, int64_t n_oct, int T, int C,
-                     int G, int relu) {
+                     const float* __restrict__ beta, const __nv_bfloat16* __restrict__ res, int n_oct_win /* T * C/8 */,
+                     int segs /* CTAs per window */, int C, int G, int relu) {
+  const int b = blockIdx.x / segs, seg = blockIdx.x - b * segs;
+  const int opr = C / 8, cg = C / G;
+  const int c0 = (threadIdx.x % opr) * 8;
+  float sc[8], sh[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const float2 st = stats[(int64_t)b * G + (c0 + j) / cg];
+    sc[j] = st.y * gamma[c0 + j];
+    sh[j] = fmaf(-st.x, sc[j], beta[c0 + j]);
+  }
+  uint4* zb = reinterpret_cast<uint4*>(z) + (int64_t)b * n_oct_win;
+  const uint4* rb = RES ? reinterpret_cast<const uint4*>(res) + (int64_t)b * n_oct_win : nullptr;
+  const int i0 = seg * (GN_ITER * 256) + threadIdx.x;
+  uint4 zv[GN_ITER], rv[GN_ITER];
+#pragma unroll
+  for (int k = 0; k < GN_ITER; ++k) {
+    const int i = i0 + k * 256;
+    if (i < n_oct_win) { zv[k] = zb[i]; if (RES) rv[k] = rb[i]; }
+  }
+#pragma unroll
+  for (int k = 0; k < GN_ITER; ++k) {
+    const int i = i0 + k * 256;
+    if (i >= n_oct_win) continue;
+    float f[8], r[8];
+    if (Z_F16) gn_unpack8_f16(zv[k], f); else gn_unpack8(zv[k], f);
+    if (RES) gn_unpack8(rv[k], r);
+    uint4 o;
+    __nv_bfloat162* oh = reinterpret_cast<__nv_bfloat162*>(&o);
+#pragma unroll
+    for (int j = 0; j < 8; j += 2) {
+      float y0 = fmaf(f[j], sc[j], sh[j]), y1 = fmaf(f[j + 1], sc[j + 1], sh[j + 1]);
+      if (RES) { y0 += r[j]; y1 += r[j + 1]; }
+      if (relu) { y0 = fmaxf(y0, 0.f); y1 = fmaxf(y1, 0.f); }
+      oh[j / 2] = __floats2bfloat162_rn(y0, y1);
+    }
+    zb[i] = o;
+  }
+}
+
+// General shapes (C/8 does not divide 256): one thread per octet.
+template <bool RES, bool Z_F16>
+__global__ void __launch_bounds__(256)
+gn_apply_bf16_generic_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ stats, const float* __restrict__ gamma,
+                             const float* __restrict__ beta, const __nv_bfloat16* __restrict__ res, int64_t n_oct, int T, int C,
+                             int G, int relu) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_oct) return;
   const int opr = C / 8;
@@ -114,10 +163,6 @@ gn_apply_bf16_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ s
   float f[8], r[8];
   if (Z_F16) gn_unpack8_f16(*zp, f); else gn_unpack8(*zp, f);
   if (RES) gn_unpack8(reinterpret_cast<const uint4*>(res)[i], r);
-  const float4 g0 = *reinterpret_cast<const float4*>(gamma + c0), g1 = *reinterpret_cast<const float4*>(gamma + c0 + 4);
-  const float4 b0 = *reinterpret_cast<const float4*>(beta + c0), b1 = *reinterpret_cast<const float4*>(beta + c0 + 4);
-  const float gm[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
-  const float bt[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
   uint4 o;
   __nv_bfloat162* oh = reinterpret_cast<__nv_bfloat162*>(&o);
 #pragma unroll
@@ -126,7 +171,8 @@ gn_apply_bf16_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ s
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
       const float2 st = stats[b * G + (c0 + j + k) / cg];
-      float y = fmaf(f[j + k] - st.x, st.y * gm[j + k], bt[j + k]);
+      const float scale = st.y * gamma[c0 + j + k];
+      float y = fmaf(f[j + k], scale, fmaf(-st.x, scale, beta[c0 + j + k]));
       if (RES) y += r[j + k];
       if (relu) y = fmaxf(y, 0.f);
       v[k] = y;
@@ -150,14 +196,20 @@ aframe_status af_launch_gn_bf16(aframe_ctx* ctx, __nv_bfloat16* z, const __nv_bf
     gn_stats_bf16_generic_kernel<<<dim3((unsigned)nb, (unsigned)G), 256, 0, ctx->stream>>>(z, T, C, G, eps, stats);
   AF_LAUNCH_CHECK(ctx);
   const int64_t n_oct = nb * T * opr;
-  const unsigned blocks = (unsigned)((n_oct + 255) / 256);
-  if (z_f16) {
-    if (res) gn_apply_bf16_kernel<true, true><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, res, n_oct, T, C, G, relu);
-    else gn_apply_bf16_kernel<false, true><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, nullptr, n_oct, T, C, G, relu);
-  } else {
-    if (res) gn_apply_bf16_kernel<true, false><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, res, n_oct, T, C, G, relu);
-    else gn_apply_bf16_kernel<false, false><<<blocks, 256, 0, ctx->stream>>>(z, stats, gamma, beta, nullptr, n_oct, T, C, G, relu);
-  }
+#define AF_GN_APPLY(RES_, F16_)                                                                                          \
+  do {                                                                                                                  \
+    if (256 % opr == 0 && (int64_t)T * opr < (1 << 30)) {                                                               \
+      const int n_win = T * opr, segs = (n_win + GN_ITER * 256 - 1) / (GN_ITER * 256);                                  \
+      gn_apply_bf16_kernel<RES_, F16_><<<(unsigned)(nb * segs), 256, 0, ctx->stream>>>(z, stats, gamma, beta, res, n_win, \
+                                                                                       segs, C, G, relu);               \
+    } else {                                                                                                            \
+      gn_apply_bf16_generic_kernel<RES_, F16_><<<(unsigned)((n_oct + 255) / 256), 256, 0, ctx->stream>>>(               \
+          z, stats, gamma, beta, res, n_oct, T, C, G, relu);                                                            \
+    }                                                                                                                   \
+  } while (0)
+  if (z_f16) { if (res) AF_GN_APPLY(true, true); else AF_GN_APPLY(false, true); }
+  else { if (res) AF_GN_APPLY(true, false); else AF_GN_APPLY(false, false); }
+#undef AF_GN_APPLY
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }
