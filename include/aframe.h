@@ -17,6 +17,8 @@
  *    returns a context-owned, NUL-terminated description of the last failure.
  *  - No CPU fallback exists: on a device that is not compute capability 10.x aframe_create
  *    returns AFRAME_EUNSUPPORTED.
+ *  - Threads: a context and the weights / stream objects created from it may be used by one host
+ *    thread at a time; different contexts share no mutable state and may be used concurrently.
  *  - NaN/Inf in the inputs propagate to the outputs; they are not trapped.
  *  - Strain is pre-scaled on load by the exact power of two 2^strain_scale_log2 (reading A9:
  *    a PSD of ~1e-46 is below the smallest fp32 denormal).  PSDs handed out by the library are

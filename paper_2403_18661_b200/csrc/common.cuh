@@ -79,6 +79,7 @@ struct aframe_ctx {
   std::vector<cudaEvent_t> prof_pool;
   cudaEvent_t prof_open[AFRAME_PROF_KINDS] = {};
   float* layer_ms = nullptr;   // aframe_profile_layers: per-layer device time of the next forward (host array), else null
+  void* tc_cache = nullptr;    // conv_tc.cu: cached tensor maps / launch plans of the bf16 path (af_tc_forget frees it)
   int n_ch_batch = 0;          // aframe_whiten_batch: rows (element x detector) the signal launchers treat as channels
 };
 

@@ -7,6 +7,7 @@
 #include "common.cuh"
 #include "net_plan.h"
 #include "stem.h"
+#include <atomic>
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -32,7 +33,7 @@ static bool encode_map(aframe_ctx* ctx, CUtensorMap* m, const void* ptr, int ran
 struct TcLaunch {
   CUtensorMap tm_in, tm_w, tm_out, tm_res, tm_scw;
   TcConvParams p;
-  int BN, grid, smem;
+  int BN, grid, smem, device;
   bool head, cg2, halo;
 };
 
@@ -190,6 +191,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.stage_bytes = halo ? TcCfg<64>::HALO_A_BYTES : 0;     // one stage = one 64-channel block
 
   L.BN = BN;
+  L.device = ctx->device;
   L.head = head;
   L.cg2 = cg2;
   L.halo = halo;
@@ -202,12 +204,13 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
 }
 
 template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t launch_bn(const TcLaunch& L, cudaStream_t s) {
-  static bool attr = false;
+  static std::atomic<uint64_t> attr_done{0};          // bit d: the attribute is set on device d (it is per device)
   auto kern = conv_tc_kernel<BN, HEAD, CG2, HALO>;
-  if (!attr) {
+  const uint64_t bit = 1ull << (L.device & 63);
+  if (!(attr_done.load(std::memory_order_acquire) & bit)) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448);
     if (e != cudaSuccess) return e;
-    attr = true;
+    attr_done.fetch_or(bit, std::memory_order_release);
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)L.grid);
@@ -237,7 +240,7 @@ static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s) {
 struct TcBlockLaunch {
   CUtensorMap tm_x, tm_wa, tm_wb, tm_out;
   TcBlockParams p;
-  int grid = 0, smem = 0;
+  int grid = 0, smem = 0, device = 0;
 };
 
 // Layer i is the first conv of a basic block the fused kernel can run: 64 -> 64 -> 64 channels, k3 s1 p1, ReLU after each,
@@ -281,16 +284,18 @@ static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia,
     if (const char* f = getenv("AFRAME_TCB_PROF_PTR")) { FILE* fp = fopen(f, "w"); if (fp) { fprintf(fp, "%llu\n", (unsigned long long)(uintptr_t)d_prof); fclose(fp); } }
   }
   L.smem = tcb_smem(p.nx, p.ny, p.no);
+  L.device = ctx->device;
   L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
   return true;
 }
 
 static cudaError_t launch_block(const TcBlockLaunch& L, cudaStream_t s) {
-  static bool attr = false;
-  if (!attr) {
+  static std::atomic<uint64_t> attr_done{0};
+  const uint64_t bit = 1ull << (L.device & 63);
+  if (!(attr_done.load(std::memory_order_acquire) & bit)) {
     cudaError_t e = cudaFuncSetAttribute(conv_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448);
     if (e != cudaSuccess) return e;
-    attr = true;
+    attr_done.fetch_or(bit, std::memory_order_release);
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)L.grid);
@@ -316,9 +321,11 @@ struct TcPlanCache {
   std::vector<int> sc_of;             // per layer: the projection-shortcut conv that runs inside it (else -1)
   std::vector<char> skip;             // per layer: runs inside another launch
 };
-static std::map<aframe_ctx*, std::vector<TcPlanCache>> g_cache;
-
-void af_tc_forget(aframe_ctx* ctx) { g_cache.erase(ctx); }
+// the launch plans live in the context (ctx->tc_cache), so contexts never share mutable state
+void af_tc_forget(aframe_ctx* ctx) {
+  delete static_cast<std::vector<TcPlanCache>*>(ctx->tc_cache);
+  ctx->tc_cache = nullptr;
+}
 
 static int64_t tc_chunk_windows() {
   static int64_t v = 0;
@@ -373,7 +380,8 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   char* base = reinterpret_cast<char*>(ctx->ws_act.ptr);
   float* head_part = reinterpret_cast<float*>(base + slot_bytes * plan.n_slots);
   auto slot_ptr = [&](int layer) { return reinterpret_cast<__nv_bfloat16*>(base + slot_bytes * plan.slot[layer]); };
-  std::vector<TcPlanCache>& caches = g_cache[ctx];
+  if (!ctx->tc_cache) ctx->tc_cache = new std::vector<TcPlanCache>();
+  std::vector<TcPlanCache>& caches = *static_cast<std::vector<TcPlanCache>*>(ctx->tc_cache);
 
   for (int64_t b0 = 0; b0 < B; b0 += chunk) {
     const int64_t nb = (B - b0 < chunk) ? (B - b0) : chunk;

@@ -5,6 +5,7 @@
 //  O-3 ("whitened in the frequency-domain, and transformed back to time-domain")
 //                                  whiten_os_kernel: rFFT -> multiply by real H -> irFFT, valid part stored
 #include "fft.cuh"
+#include <atomic>
 
 // --------------------------------------------------------------------------------------------------
 // Welch: one CTA per (segment, channel).  NFFT real samples -> M = NFFT/2 complex FFT -> |X|^2.
@@ -340,10 +341,11 @@ aframe_status af_launch_filter_design(aframe_ctx* ctx, const float* d_psd, int64
   af_prof_begin(ctx, AFRAME_PROF_DESIGN);
 #define AF_FD_CASE(N)                                                                                                \
   case N: {                                                                                                          \
-    static bool attr_set = false;                                                                                    \
-    if (!attr_set) {                                                                                                 \
+    static std::atomic<uint64_t> attr_done{0};           /* bit d: set on device d (the attribute is per device) */  \
+    const uint64_t bit = 1ull << (ctx->device & 63);                                                                 \
+    if (!(attr_done.load(std::memory_order_acquire) & bit)) {                                                        \
       AF_CUDA(ctx, cudaFuncSetAttribute(filter_design_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-      attr_set = true;                                                                                               \
+      attr_done.fetch_or(bit, std::memory_order_release);                                                            \
     }                                                                                                                \
     filter_design_kernel<N><<<grid, 512, smem, ctx->stream>>>(d_psd, F_w, af_nch(ctx), cfg.fs, cfg.f_lo, cfg.f_hi, \
                                                              cfg.filter_len, ctx->d_tw64, d_H, d_taps, gate);        \
