@@ -263,3 +263,44 @@ def test_stride_one_windows_offline(af):
     wins = ost.unfold(y, K, 1, n_windows=n_win)
     ref = onet.forward(onet.parse_blob(blob), wins)
     assert rel_err(got, ref) <= 1e-4
+
+
+def test_bench_step_at_full_size_sampled_against_oracle(af):
+    """BASELINE.json configs[3] in the launch configuration bench.py times: one 4096 s block of two-detector strain (plus
+    its 64 s PSD history), 8 timeslides x 65 536 windows, batches of 4096 windows, through aframe_score_timeslides.
+    The float64 oracle (rolling whitening with the epoch's own Welch PSD + network) recomputes a seeded sample of the
+    524 288 scores one by one: the first and last valid window of each slide, windows on both sides of PSD-epoch
+    boundaries, and pseudo-random ones (rule T3); all scores must be finite."""
+    import bench
+    fc = full_config()
+    n_win, n_raw = bench.block_geometry(4096)
+    shifts = [k * FS for k in range(1, bench.N_SLIDES + 1)]
+    x = bench.make_block(7, n_raw)
+    blob = make_weight_blob(**fc)
+    ctx = af.Context(precision=af.BF16)
+    w = ctx.load_weights(blob)
+    scores = ctx.score_timeslides(w, torch.from_numpy(x).cuda(), 0, n_win, shifts, batch=4096)
+    assert scores.shape == (bench.N_SLIDES, n_win) and bool(torch.isfinite(scores).all())
+    scores = scores.cpu().numpy()
+
+    cfg = ost.StreamConfig()
+    m0 = cfg.psd_len - S - cfg.filter_len // 2                  # raw index of whitened sample 0 (reading C1)
+    rng = np.random.default_rng(20240318)
+    picks = [(k, 0) for k in (0, 7)] + [(k, n_win - 1) for k in (0, 3, 7)]
+    # windows whose samples straddle the switch to PSD epoch e (raw index where epoch e starts: reading C2)
+    for e in (1, 97, 255):
+        m_switch = cfg.psd_len + e * cfg.psd_update - S - cfg.filter_len // 2
+        i = (m_switch - m0) // S
+        picks += [(2, i - 30), (5, i - 1), (5, i)]
+    picks += [(int(rng.integers(0, 8)), int(rng.integers(0, n_win))) for _ in range(40)]
+    x64 = x.astype(np.float64)
+    net = onet.parse_blob(blob)
+    wins = []
+    for k, i in picks:
+        a = m0 + i * S
+        h1, _ = ost.whiten_rolling(x64[0], cfg, m_lo=a, m_hi=a + 3072)
+        l1, _ = ost.whiten_rolling(x64[1], cfg, m_lo=a + shifts[k], m_hi=a + shifts[k] + 3072)
+        wins.append(np.stack([h1, l1]))
+    want = onet.forward(net, np.stack(wins))
+    got = np.array([scores[k, i] for k, i in picks], dtype=np.float64)
+    assert rel_err(got, want) <= 2e-2
