@@ -195,3 +195,34 @@ def test_true_group_norm_full_size_fp32_and_bf16(af, config1):
     for nb in (1, 37):
         part = ctx16.forward(w16, x[:nb]).cpu().numpy()
         assert np.array_equal(part, got[:nb].astype(np.float32))
+
+
+@pytest.mark.parametrize("kernel_len", [2048, 4096, 2560])
+def test_bf16_path_other_window_lengths(af, kernel_len):
+    """The tensor-core path is not specialised to K = 3072: the config-1 table on 1 s, 2 s and 1.25 s windows (stage lengths
+    512..64, 1024..128 and 640..80: other tile shapes, windows-per-tile counts and fused-block tile counts)."""
+    cfg = dict(full_config(), kernel_len=kernel_len)
+    blob = make_weight_blob(**cfg)
+    rng = np.random.default_rng(kernel_len)
+    wins = rng.standard_normal((5, 2, kernel_len)).astype(np.float32)
+    ref = onet.forward(onet.parse_blob(blob), wins)
+    ctx = af.Context(kernel_len=kernel_len, precision=af.BF16)
+    got = ctx.forward(ctx.load_weights(blob), torch.from_numpy(wins).cuda()).cpu().numpy()
+    assert rel_err(got, ref) <= 2e-2
+    ctx32 = af.Context(kernel_len=kernel_len, precision=af.FP32)
+    got32 = ctx32.forward(ctx32.load_weights(blob), torch.from_numpy(wins[:2]).cuda()).cpu().numpy()
+    assert rel_err(got32, ref[:2]) <= 1e-4
+
+
+def test_live_group_norm_bf16_fallback_statistics_path(af):
+    """True GroupNorm on 1.25 s windows: the last stage has 80 rows per window (16-row tiles, 8 windows per tile), where
+    the conv epilogue cannot emit per-window partial sums and the statistics are read back from z instead."""
+    from synthdata import full_config_live_gn
+    cfg = dict(full_config_live_gn(), kernel_len=2560)
+    blob = make_weight_blob(**cfg)
+    rng = np.random.default_rng(5)
+    wins = rng.standard_normal((11, 2, 2560)).astype(np.float32)
+    ref = onet.forward(onet.parse_blob(blob), wins)
+    ctx = af.Context(kernel_len=2560, precision=af.BF16)
+    got = ctx.forward(ctx.load_weights(blob), torch.from_numpy(wins).cuda()).cpu().numpy()
+    assert rel_err(got, ref) <= 2e-2
