@@ -77,9 +77,15 @@ def rank_block_ids(rank, n_blocks):
     return [rank * 1000 + j for j in range(n_blocks)]
 
 
+def use_dist(world):
+    """One rank per GPU under torchrun; AFRAME_BENCH_FORCE_DIST=1 also runs the NCCL plumbing with a single rank (how the
+    multi-rank path is exercised on a one-GPU box)."""
+    return world > 1 or os.environ.get("AFRAME_BENCH_FORCE_DIST") == "1"
+
+
 def max_over_ranks(t, world):
     """Element-wise max over ranks of a float64 tensor (the only collective of the run; timing, not data)."""
-    if world > 1:
+    if use_dist(world):
         import torch.distributed as dist
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return t
@@ -282,11 +288,13 @@ def run_ours(args):
     if not os.path.exists(af.LIB_PATH):
         ge.build()
     torch.cuda.set_device(local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if use_dist(world):
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29533")
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local_rank))
 
     def barrier():
-        if world > 1:
+        if use_dist(world):
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -355,7 +363,7 @@ def run_ours(args):
                "h2d_bytes_per_step": int(blocks_host[0].numel() * 4), "d2h_bytes_per_step": int(scores_host.numel() * 4),
                "api": "aframe_score_timeslides_host (pinned host buffers; H2D + D2H inside the call)"}
     if rank != 0:
-        if world > 1:
+        if use_dist(world):
             dist.destroy_process_group()
         return
 
@@ -438,7 +446,7 @@ def run_ours(args):
                                "sample": "float64 oracle: Welch+design+whitening of 66 s x 2 ch and the ResNet forward on "
                                          "256 windows of the same stream; rates combined for 8 timeslides"}
     print(json.dumps(out))
-    if world > 1:
+    if use_dist(world):
         dist.destroy_process_group()
 
 
