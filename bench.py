@@ -410,6 +410,13 @@ def run_ours(args):
                                   # 1.965 GHz thread instructions per second
                                   "alu": {"bound": "alu", "achieved": 137.0 * gbs / 6.0 / 1e3, "peak": 148 * 128 * 1.965e9 / 1e12,
                                           "unit": "T thread-instructions/s", "frac": (137.0 * gbs / 6.0 / 1e3) / (148 * 128 * 1.965e9 / 1e12)}}
+    st_ms = stages["stem"][0]
+    if st_ms > 0:
+        tf = 2.0 * 1536 * 64 * 14 * windows / world / (st_ms * 1e-3) / 1e12      # conv k7 s2, 2 -> 64 channels, 1536 positions
+        out["roofline_stem"] = {"kernel": "stem_pool_kernel", "bound": "alu", "achieved": tf, "peak": 148 * 128 * 2 * 1.965e9 / 1e12,
+                                "unit": "TFLOP/s fp32", "frac": tf / (148 * 128 * 2 * 1.965e9 / 1e12),
+                                "algorithmic": "2.75 MFLOP per window (K = 14 is not a tensor-core shape: fp32 FFMA on CUDA cores); "
+                                               "peak = 148 SMs x 128 lanes x 2 x 1.965 GHz; profiles/r01d_stem_full.md"}
     we_ms = stages["welch"][0]
     if we_ms > 0:
         gbs = args.steps * 2 * n_raw * 4 / (we_ms * 1e-3) / 1e9                   # every raw sample enters the PSD once
