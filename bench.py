@@ -412,11 +412,19 @@ def run_ours(args):
                                           "unit": "T thread-instructions/s", "frac": (137.0 * gbs / 6.0 / 1e3) / (148 * 128 * 1.965e9 / 1e12)}}
     st_ms = stages["stem"][0]
     if st_ms > 0:
-        tf = 2.0 * 1536 * 64 * 14 * windows / world / (st_ms * 1e-3) / 1e12      # conv k7 s2, 2 -> 64 channels, 1536 positions
-        out["roofline_stem"] = {"kernel": "stem_pool_kernel", "bound": "alu", "achieved": tf, "peak": 148 * 128 * 2 * 1.965e9 / 1e12,
-                                "unit": "TFLOP/s fp32", "frac": tf / (148 * 128 * 2 * 1.965e9 / 1e12),
-                                "algorithmic": "2.75 MFLOP per window (K = 14 is not a tensor-core shape: fp32 FFMA on CUDA cores); "
-                                               "peak = 148 SMs x 128 lanes x 2 x 1.965 GHz; profiles/r01d_stem_full.md"}
+        # shared stem: per 4096-window chunk the stem runs once over the chunk's stream (64 new conv positions per window)
+        # plus 7 conv positions per window for the three edge rows; each position is 64 channels x 14 MACs
+        chunk = 4096
+        n_chunks = args.steps * N_SLIDES * (-(-n_win // chunk))
+        pos = args.steps * N_SLIDES * ((n_win - (-(-n_win // chunk))) * 64 + (-(-n_win // chunk)) * 1536 + 7 * n_win)
+        tf = 2.0 * 64 * 14 * pos / (st_ms * 1e-3) / 1e12
+        out["roofline_stem"] = {"kernel": "stem_pool_kernel (whole stream) + stem_edge_kernel", "bound": "alu", "achieved": tf,
+                                "peak": 148 * 128 * 2 * 1.965e9 / 1e12, "unit": "TFLOP/s fp32",
+                                "frac": tf / (148 * 128 * 2 * 1.965e9 / 1e12), "launches": int(2 * n_chunks),
+                                "algorithmic": "overlapping windows share their stem: 71 conv positions (64 new + 7 edge) x 64 channels x "
+                                               "14 MACs per window instead of 1536; two ~15 us launches per 4096 windows, so this "
+                                               "stage is launch-bound and 0.5 % of the step (per-window kernel at 4096 windows: "
+                                               "profiles/r01d_stem_full.md, 50 % of the FFMA peak)"}
     we_ms = stages["welch"][0]
     if we_ms > 0:
         gbs = args.steps * 2 * n_raw * 4 / (we_ms * 1e-3) / 1e9                   # every raw sample enters the PSD once

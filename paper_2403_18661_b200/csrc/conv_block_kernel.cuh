@@ -29,6 +29,9 @@ struct TcBlockParams {
   TcFastDiv div_tw;      // by tiles_per_win
   int nx, ny, no;        // ring depths
   int reverse;           // walk the tiles from the last to the first
+  // shared stem (stem_bf16.cu): tm_x is a strided view of the stem of the whole stream; rows 0, 1 and T - 1 of every window
+  // are overwritten in shared memory with the window's own edge rows [windows][3][64] before the tile is used (null = off)
+  const __nv_bfloat16* edge;
   long long* dbg_out;    // timing experiments: per-role cycle counters of CTA 0 (null = off)
 };
 
@@ -60,6 +63,7 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
   auto b_empty = [&](int s) { return bar2 + 8u * (6 + s); };
   const uint32_t w_bar = bar2 + 8u * 8;
   const uint32_t tmem_slot = w_bar + 8u;
+  auto x_tma = [&](int s) { return tmem_slot + 8u + 8u * s; };   // edge mode: TMA completion, before the patch
   float* s_ba = reinterpret_cast<float*>(smem_raw + 512);
   float* s_bb = s_ba + 64;
   const uint32_t wa_base = base + TCB_FIXED, wb_base = wa_base + TCB_W_BYTES;
@@ -70,7 +74,7 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tm_x); tma_prefetch_desc(&tm_wa); tma_prefetch_desc(&tm_wb); tma_prefetch_desc(&tm_out);
-    for (int s = 0; s < NX; ++s) { mbar_init(x_full(s), 1); mbar_init(x_empty(s), 2); }   // MMA_a commit + epilogue B
+    for (int s = 0; s < NX; ++s) { mbar_init(x_full(s), 1); mbar_init(x_empty(s), 2); mbar_init(x_tma(s), 1); }   // x_empty: MMA_a commit + epilogue B
     for (int s = 0; s < NY; ++s) { mbar_init(y_full(s), 4); mbar_init(y_empty(s), 1); }   // 4 epilogue-A warps | MMA_b commit
     for (int s = 0; s < 2; ++s) {
       mbar_init(a_full(s), 1); mbar_init(a_empty(s), 4);
@@ -110,6 +114,7 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
     }
     __syncwarp();
     pdl_wait();                                    // x is the previous layer's output
+    if (p.edge == nullptr) {
     int slot = 0; uint32_t ph = 0;
     for (int tile = first; tile < p.num_tiles; tile += step) {
       int b, t0;
@@ -124,6 +129,46 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
       __syncwarp();
       if (++slot == NX) { slot = 0; ph ^= 1u; }
       T(2);
+    }
+    } else {
+      // edge mode: issue whatever slot is free, and hand a tile to the MMA warp (x_full) once its TMA has landed and the
+      // window's own rows 0, 1, T - 1 -- where the box holds them -- have been written over the stream's values
+      int n_my = 0;
+      for (int tile = first; tile < p.num_tiles; tile += step) ++n_my;
+      int slot = 0, fslot = 0, n_issued = 0, n_final = 0;
+      uint32_t ph = 0, fph = 0;
+      while (n_final < n_my) {
+        bool did = false;
+        if (n_issued < n_my && __all_sync(0xffffffffu, mbar_test(x_empty(slot), ph ^ 1u))) {
+          int b, t0;
+          decode(first + n_issued * step, b, t0);
+          if (elect_one()) {
+            mbar_arrive_expect_tx(x_tma(slot), 130 * 128);
+            tma_load_3d(xs_base + slot * TCB_SLOT, &tm_x, x_tma(slot), 0, t0 - 2, b);
+          }
+          __syncwarp();
+          if (++slot == NX) { slot = 0; ph ^= 1u; }
+          ++n_issued; did = true;
+        }
+        if (n_final < n_issued && __all_sync(0xffffffffu, mbar_test(x_tma(fslot), fph))) {
+          int b, t0;
+          decode(first + n_final * step, b, t0);
+          const int k = lane >> 3, jj = lane & 7;          // lanes 8k .. 8k+7: edge row k, 16-byte piece jj
+          const int t = k < 2 ? k : p.T - 1;
+          const int xr = t - t0 + 2;                       // row of the box that holds window row t
+          if (k < 3 && xr >= 0 && xr < 130 && !(k == 1 && p.T < 2)) {
+            const uint4 v = *reinterpret_cast<const uint4*>(p.edge + ((int64_t)b * 3 + k) * 64 + jj * 8);
+            *reinterpret_cast<uint4*>(smem_raw + (xs_base - base) + fslot * TCB_SLOT + xr * 128 + ((jj ^ (xr & 7)) << 4)) = v;
+          }
+          fence_proxy_async_smem();                        // generic-proxy writes -> visible to the tensor core's reads
+          __syncwarp();
+          if (elect_one()) mbar_arrive(x_full(fslot));
+          __syncwarp();
+          if (++fslot == NX) { fslot = 0; fph ^= 1u; }
+          ++n_final; did = true;
+        }
+        if (!did) __nanosleep(20);
+      }
     }
     if (lane == 0) Tflush(0);
   } else if (warp == 1) {

@@ -257,16 +257,20 @@ static int fusable_block(const aframe_weights* w, int i) {
   return i + 1;
 }
 
+// row_shift > 0: x is the stem of the whole stream (shared stem): window b starts row_shift rows after window b - 1, and
+// edge holds every window's own rows 0, 1, T - 1
 static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia, int ib, const __nv_bfloat16* x,
-                               __nv_bfloat16* out, int64_t nb, TcBlockLaunch& L) {
+                               __nv_bfloat16* out, int64_t nb, TcBlockLaunch& L, int64_t row_shift = 0,
+                               const __nv_bfloat16* edge = nullptr) {
   const LayerDesc& a = w->layers[ia];
   const int T = a.t_out;
   const uint64_t dims[3] = {64, (uint64_t)T, (uint64_t)nb};
   const uint64_t str[2] = {128, (uint64_t)T * 128};
+  const uint64_t str_x[2] = {128, (uint64_t)(row_shift > 0 ? row_shift : T) * 128};
   const uint32_t box_x[3] = {64, 130, 1}, box_o[3] = {64, TCB_ROWS, 1}, box_w[3] = {64, 64, 1};
   const uint64_t wd[3] = {64, 64, 3};
   const uint64_t ws[2] = {128, 64 * 128};
-  if (!encode_map(ctx, &L.tm_x, x, 3, dims, str, box_x) || !encode_map(ctx, &L.tm_out, out, 3, dims, str, box_o) ||
+  if (!encode_map(ctx, &L.tm_x, x, 3, dims, str_x, box_x) || !encode_map(ctx, &L.tm_out, out, 3, dims, str, box_o) ||
       !encode_map(ctx, &L.tm_wa, w->d_w16[ia], 3, wd, ws, box_w) || !encode_map(ctx, &L.tm_wb, w->d_w16[ib], 3, wd, ws, box_w))
     return false;
   TcBlockParams& p = L.p;
@@ -276,6 +280,7 @@ static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia,
   p.num_tiles = (int)(nb * p.tiles_per_win);
   p.div_tw = tc_fastdiv((uint32_t)p.tiles_per_win);
   p.nx = 6; p.ny = 2; p.no = 1;
+  p.edge = row_shift > 0 ? edge : nullptr;
   p.dbg_out = nullptr;
   if (env_int("AFRAME_TC_PROF", 0)) {
     static long long* d_prof = nullptr;
@@ -318,6 +323,8 @@ struct TcPlanCache {
   std::vector<TcLaunch> launches;   // indexed by layer
   std::vector<TcBlockLaunch> blocks;  // indexed by the block's SECOND layer
   std::vector<int> fused_with;        // per layer: index of the partner layer if the pair runs fused, else -1
+  int64_t win_stride = 0;             // input window spacing the plans were built for (shared stem)
+  bool shared_stem = false;           // stem of the whole stream + edge rows instead of one stem per window
   std::vector<int> sc_of;             // per layer: the projection-shortcut conv that runs inside it (else -1)
   std::vector<char> skip;             // per layer: runs inside another launch
 };
@@ -387,12 +394,12 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     const int64_t nb = (B - b0 < chunk) ? (B - b0) : chunk;
     TcPlanCache* pc = nullptr;
     for (auto& c : caches)
-      if (c.w == w && c.base == base && c.nb == nb && c.slot_bytes == slot_bytes) { pc = &c; break; }
+      if (c.w == w && c.base == base && c.nb == nb && c.slot_bytes == slot_bytes && c.win_stride == sB) { pc = &c; break; }
     if (!pc) {
       if (caches.size() > 8) caches.clear();
       caches.emplace_back();
       pc = &caches.back();
-      pc->w = w; pc->base = base; pc->nb = nb; pc->slot_bytes = slot_bytes;
+      pc->w = w; pc->base = base; pc->nb = nb; pc->slot_bytes = slot_bytes; pc->win_stride = sB;
       pc->launches.resize(n);
       pc->blocks.resize(n);
       pc->fused_with.assign(n, -1);
@@ -418,7 +425,17 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         for (int i = 2; i < n; ++i) {
           const int ib = pc->fused_with[i] < 0 ? fusable_block(w, i) : -1;
           if (ib < 0) continue;
-          if (!build_block_launch(ctx, w, i, ib, slot_ptr(w->layers[i].input_from), slot_ptr(ib), nb, pc->blocks[ib])) { caches.pop_back(); return AFRAME_ECUDA; }
+          // Shared stem: overlapping in-place windows (spacing a multiple of 4 samples, shorter than the window) whose
+          // stem output is read only by this fused block: the stem runs ONCE over the whole stream, the block reads the
+          // windows as strided views of it and patches the three rows per window that see the window's own zero padding.
+          bool shared = i == 2 && w->layers[2].input_from == 1 && w->layers[ib].residual_from == 1 && nb >= 2 && sB % 4 == 0 &&
+                        sB < w->layers[0].t_in && env_int("AFRAME_SHARED_STEM", 1) != 0;
+          for (int j = 2; shared && j < n; ++j)
+            if (j != 2 && j != ib && (w->layers[j].input_from == 1 || w->layers[j].residual_from == 1)) shared = false;
+          const int64_t row_shift = shared ? sB / 4 : 0;
+          const __nv_bfloat16* edge = slot_ptr(1) + ((nb - 1) * row_shift + w->layers[1].t_out) * 64;
+          if (!build_block_launch(ctx, w, i, ib, slot_ptr(w->layers[i].input_from), slot_ptr(ib), nb, pc->blocks[ib], row_shift, edge)) { caches.pop_back(); return AFRAME_ECUDA; }
+          if (shared) pc->shared_stem = true;
           pc->fused_with[i] = ib; pc->fused_with[ib] = i;
         }
       for (int i = 2; i < n; ++i) {
@@ -457,6 +474,11 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     //  because its operands are bf16; it was dropped)
     float2* gn_stats = reinterpret_cast<float2*>(head_part);     // live GroupNorm: the scratch after the slots holds (mu, rstd)
     const StemGn sgn{gn_stats, w->d_gamma[0], w->d_beta[0], w->n_groups, w->gn_eps};
+    if (pc->shared_stem)
+      st = af_launch_stem_stream_bf16(ctx, w->layers[0], w->layers[1], reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz,
+                                      in_bf16, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1),
+                                      slot_ptr(1) + ((nb - 1) * (sB / 4) + w->layers[1].t_out) * 64);
+    else
     st = af_launch_stem_bf16(ctx, w->layers[0], w->layers[1], reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz,
                              in_bf16, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1), w->live_gn ? &sgn : nullptr);
     af_prof_end(ctx, AFRAME_PROF_STEM, 1);

@@ -10,6 +10,11 @@ aframe_status af_launch_stem_bf16(aframe_ctx* ctx, const LayerDesc& conv, const 
                                   int in_bf16, int64_t sB, const int64_t* choff, const float* d_w, const float* d_bias,
                                   int64_t B, __nv_bfloat16* d_out, const StemGn* gn = nullptr);
 
+// shared stem of overlapping in-place windows (see stem_bf16.cu): stem of the whole stream + per-window edge rows
+aframe_status af_launch_stem_stream_bf16(aframe_ctx* ctx, const LayerDesc& conv, const LayerDesc& pool, const void* d_in,
+                                         int in_bf16, int64_t win_stride, const int64_t* choff, const float* d_w,
+                                         const float* d_bias, int64_t nb, __nv_bfloat16* d_stream, __nv_bfloat16* d_edge);
+
 // true GroupNorm after a tensor-core conv (NEXT-2): statistics per (window, group), then normalise + affine (+ residual)
 // (ReLU) in place on the bf16 tensor z [nb][T][C]; stats is scratch for nb * G float2.  partials != null: the conv epilogue
 // already emitted per-slab partial sums of its fp32 accumulators (TcConvParams::gn_part); they are only combined here.

@@ -175,6 +175,80 @@ stem_gn_stats_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const
   }
 }
 
+// Shared stem (overlapping windows): rows 0, 1 and T_pool - 1 of every window are the only pooled rows that see the
+// window's own zero padding; everything else equals the stem of the whole stream (af_launch_stem_stream_bf16).  One warp
+// per window, lane <-> channel pair; the FMA order is the one of stem_pool_kernel, so the values are bit-identical to
+// what the per-window kernel stores.  edge: [nb][3][64] bf16 (rows 0, 1, T_pool - 1).
+template <bool IN_BF16>
+__global__ void __launch_bounds__(128)
+stem_edge_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const float* __restrict__ w /*[7][2][64]*/,
+                 const float* __restrict__ bias, int T_in, int T_pool, int64_t nb, __nv_bfloat16* __restrict__ edge) {
+  constexpr int KW = 7, CIN = 2, C_OUT = 64;
+  const int lane = threadIdx.x & 31;
+  const int64_t b = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (b >= nb) return;
+  float w0[KW][CIN], w1[KW][CIN];
+#pragma unroll
+  for (int d = 0; d < KW; ++d)
+#pragma unroll
+    for (int c = 0; c < CIN; ++c) {
+      const float2 ww = *reinterpret_cast<const float2*>(w + (d * CIN + c) * C_OUT + 2 * lane);
+      w0[d][c] = ww.x; w1[d][c] = ww.y;
+    }
+  const float2 bs = *reinterpret_cast<const float2*>(bias + 2 * lane);
+  const int T_conv = T_in / 2;
+#pragma unroll 1
+  for (int k = 0; k < 3; ++k) {
+    const int u = k < 2 ? k : T_pool - 1;
+    float m0 = 0.f, m1 = 0.f;                          // ReLU folded into the max
+#pragma unroll 1
+    for (int t = 2 * u - 1; t <= 2 * u + 1; ++t) {
+      if (t < 0 || t >= T_conv) continue;              // pool padding never wins
+      float a0 = bs.x, a1 = bs.y;
+#pragma unroll
+      for (int c = 0; c < CIN; ++c)
+#pragma unroll
+        for (int d = 0; d < KW; ++d) {
+          const int x = 2 * t - 3 + d;
+          const float xv = (x >= 0 && x < T_in) ? stem_ld<IN_BF16>(in, b * sB + off.v[c] + x) : 0.f;
+          a0 = fmaf(w0[d][c], xv, a0); a1 = fmaf(w1[d][c], xv, a1);
+        }
+      m0 = fmaxf(m0, a0); m1 = fmaxf(m1, a1);
+    }
+    reinterpret_cast<__nv_bfloat162*>(edge + (b * 3 + k) * C_OUT)[lane] = __floats2bfloat162_rn(m0, m1);
+  }
+}
+
+// Shared stem: the windows of one launch are K-sample views at a spacing of win_stride samples (a multiple of 4) into
+// one whitened stream, so their pooled stem outputs are views at a spacing of win_stride / 4 rows into the stem of the
+// whole stream, except for the three rows above.  d_stream: [(nb - 1) * win_stride / 4 + T_pool][64] bf16.
+aframe_status af_launch_stem_stream_bf16(aframe_ctx* ctx, const LayerDesc& conv, const LayerDesc& pool, const void* d_in,
+                                         int in_bf16, int64_t win_stride, const int64_t* choff, const float* d_w,
+                                         const float* d_bias, int64_t nb, __nv_bfloat16* d_stream, __nv_bfloat16* d_edge) {
+  constexpr int TP = 128;
+  StemOff off;
+  for (int c = 0; c < AF_MAX_CH; ++c) off.v[c] = c < conv.c_in ? choff[c] : 0;
+  const int64_t T_in = (nb - 1) * win_stride + conv.t_in;
+  if (T_in > (1ll << 30)) return af_fail(ctx, AFRAME_ESHAPE, "shared stem: stream longer than 2^30 samples");
+  const int T_pool = (int)(T_in / 4);
+  dim3 grid((unsigned)((T_pool + TP - 1) / TP), 1);
+  if (in_bf16) {
+    stem_pool_kernel<true, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, 0, off, d_w, d_bias, (int)T_in, T_pool, d_stream,
+                                                                     nullptr, nullptr, nullptr, 1);
+    AF_LAUNCH_CHECK(ctx);
+    stem_edge_kernel<true><<<(unsigned)((nb + 3) / 4), 128, 0, ctx->stream>>>(d_in, win_stride, off, d_w, d_bias, conv.t_in,
+                                                                              pool.t_out, nb, d_edge);
+  } else {
+    stem_pool_kernel<false, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, 0, off, d_w, d_bias, (int)T_in, T_pool, d_stream,
+                                                                      nullptr, nullptr, nullptr, 1);
+    AF_LAUNCH_CHECK(ctx);
+    stem_edge_kernel<false><<<(unsigned)((nb + 3) / 4), 128, 0, ctx->stream>>>(d_in, win_stride, off, d_w, d_bias, conv.t_in,
+                                                                               pool.t_out, nb, d_edge);
+  }
+  AF_LAUNCH_CHECK(ctx);
+  return AFRAME_OK;
+}
+
 aframe_status af_launch_stem_bf16(aframe_ctx* ctx, const LayerDesc& conv, const LayerDesc& pool, const void* d_in,
                                   int in_bf16, int64_t sB, const int64_t* choff, const float* d_w, const float* d_bias,
                                   int64_t B, __nv_bfloat16* d_out, const StemGn* gn) {
