@@ -32,6 +32,9 @@ struct TcBlockParams {
   // shared stem (stem_bf16.cu): tm_x is a strided view of the stem of the whole stream; rows 0, 1 and T - 1 of every window
   // are overwritten in shared memory with the window's own edge rows [windows][3][64] before the tile is used (null = off)
   const __nv_bfloat16* edge;
+  // shared stage (conv_tc.cu): a batch of short windows stored back to back, zero_valid data rows + separator rows per
+  // zero_period rows: y1 is forced to zero on the separators so that they act as each short window's zero padding
+  int zero_period, zero_valid;   // 0 = off
   long long* dbg_out;    // timing experiments: per-role cycle counters of CTA 0 (null = off)
 };
 
@@ -255,7 +258,8 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
         __syncwarp();
         if (lane == 0) mbar_arrive(a_empty(as));
         const int t = t0 - 1 + row;                // y1 row held by this thread
-        const bool inside = t >= 0 && t < p.T;
+        bool inside = t >= 0 && t < p.T;
+        if (p.zero_period > 0 && inside) inside = (t % p.zero_period) < p.zero_valid;
         T(2);
         mbar_wait(y_empty(ys), (uint32_t)(((i / NY) & 1) ^ 1));   // MMA_b of the tile that last used the slot is done
         T(3);

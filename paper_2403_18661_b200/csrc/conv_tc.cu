@@ -261,9 +261,9 @@ static int fusable_block(const aframe_weights* w, int i) {
 // edge holds every window's own rows 0, 1, T - 1
 static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia, int ib, const __nv_bfloat16* x,
                                __nv_bfloat16* out, int64_t nb, TcBlockLaunch& L, int64_t row_shift = 0,
-                               const __nv_bfloat16* edge = nullptr) {
+                               const __nv_bfloat16* edge = nullptr, int T_override = 0, int zero_period = 0, int zero_valid = 0) {
   const LayerDesc& a = w->layers[ia];
-  const int T = a.t_out;
+  const int T = T_override > 0 ? T_override : a.t_out;
   const uint64_t dims[3] = {64, (uint64_t)T, (uint64_t)nb};
   const uint64_t str[2] = {128, (uint64_t)T * 128};
   const uint64_t str_x[2] = {128, (uint64_t)(row_shift > 0 ? row_shift : T) * 128};
@@ -281,6 +281,8 @@ static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia,
   p.div_tw = tc_fastdiv((uint32_t)p.tiles_per_win);
   p.nx = 6; p.ny = 2; p.no = 1;
   p.edge = row_shift > 0 ? edge : nullptr;
+  p.zero_period = zero_period; p.zero_valid = zero_valid;
+  p.reverse = 0;
   p.dbg_out = nullptr;
   if (env_int("AFRAME_TC_PROF", 0)) {
     static long long* d_prof = nullptr;
@@ -315,6 +317,53 @@ static cudaError_t launch_block(const TcBlockLaunch& L, cudaStream_t s) {
   return cudaLaunchKernelEx(&cfg, conv_block_kernel, L.tm_x, L.tm_wa, L.tm_wb, L.tm_out, L.p);
 }
 
+// ---- shared first stage -----------------------------------------------------------------------------------------
+// Windows spaced row_shift rows apart in the stem's stream overlap, and so do the outputs of every stride-1 'same' conv
+// that follows: a row is identical in all windows that hold it EXCEPT in the windows where it lies within reach of that
+// window's zero padding (each conv widens this edge by one row per side).  The fused blocks of the 64-channel stage
+// therefore run (1) once over the whole stream and (2) over a batch of 2 short windows per window -- its first and last
+// S1_ROWS rows, with the true edge rows of the previous block -- which yields the edge rows exactly; s1_stitch_kernel
+// then writes the per-window tensor the next stage reads.  Same kernel, same per-row arithmetic: bit-identical results.
+constexpr int S1_ROWS = 16;                 // rows of a short window (needs 2 K + 4 <= S1_ROWS - 2 for K blocks)
+constexpr int S1_PERIOD = S1_ROWS + 2;      // + 2 separator rows (zero input, y1 forced to zero)
+
+// X[m][r] for short window m = 2 b + tail, r < S1_PERIOD: window row t = r (head) or T - S1_ROWS + r (tail), taken from
+// the previous block's edge results where the row is an edge row there, else from the previous block's stream.
+__global__ void s1_gather_kernel(uint4* __restrict__ X, const uint4* __restrict__ S_prev, const uint4* __restrict__ Y_prev,
+                                 const uint4* __restrict__ E0, int64_t nb, int T, int64_t row_shift, int c_head, int c_tail) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= 2 * nb * S1_PERIOD * 8) return;
+  const int j = (int)(i & 7);
+  const int64_t mr = i >> 3;
+  const int r = (int)(mr % S1_PERIOD);
+  const int64_t m = mr / S1_PERIOD, b = m >> 1;
+  const bool tail = (m & 1) != 0;
+  uint4 v = make_uint4(0u, 0u, 0u, 0u);
+  if (r < S1_ROWS) {
+    const int t = tail ? T - S1_ROWS + r : r;
+    const bool from_edge = tail ? (t >= T - c_tail) : (t < c_head);
+    if (from_edge) v = E0 ? E0[(b * 3 + (tail ? 2 : t)) * 8 + j] : Y_prev[(m * S1_PERIOD + r) * 8 + j];
+    else v = S_prev[(b * row_shift + t) * 8 + j];
+  }
+  X[i] = v;
+}
+
+// out[b][t] = the last block's edge result where t is an edge row of window b, else its stream row
+__global__ void s1_stitch_kernel(uint4* __restrict__ out, const uint4* __restrict__ S, const uint4* __restrict__ Y, int64_t nb,
+                                 int T, int64_t row_shift, int c_head, int c_tail) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nb * T * 8) return;
+  const int j = (int)(i & 7);
+  const int64_t bt = i >> 3;
+  const int t = (int)(bt % T);
+  const int64_t b = bt / T;
+  uint4 v;
+  if (t < c_head) v = Y[((2 * b) * S1_PERIOD + t) * 8 + j];
+  else if (t >= T - c_tail) v = Y[((2 * b + 1) * S1_PERIOD + (t - (T - S1_ROWS))) * 8 + j];
+  else v = S[(b * row_shift + t) * 8 + j];
+  out[i] = v;
+}
+
 struct TcPlanCache {
   const aframe_weights* w = nullptr;
   void* base = nullptr;
@@ -325,6 +374,8 @@ struct TcPlanCache {
   std::vector<int> fused_with;        // per layer: index of the partner layer if the pair runs fused, else -1
   int64_t win_stride = 0;             // input window spacing the plans were built for (shared stem)
   bool shared_stem = false;           // stem of the whole stream + edge rows instead of one stem per window
+  int s1_blocks = 0;                  // > 0: the first s1_blocks fused blocks run in shared form (see s1_gather_kernel)
+  std::vector<TcBlockLaunch> s1_stream, s1_edge;
   std::vector<int> sc_of;             // per layer: the projection-shortcut conv that runs inside it (else -1)
   std::vector<char> skip;             // per layer: runs inside another launch
 };
@@ -345,6 +396,23 @@ static int64_t tc_chunk_windows() {
     if (v < 1) v = 4096;
   }
   return v;
+}
+
+// Number of leading fused 64-channel blocks that form a chain on the pooled stem output (layers 2,3 | 4,5 | ...): the
+// blocks the shared first stage can take over.
+static int s1_chain_blocks(const aframe_weights* w) {
+  const int n = (int)w->layers.size();
+  int k = 0, prev = 1;
+  for (int i = 2; i + 1 < n && k < 5; i += 2) {
+    if (fusable_block(w, i) != i + 1 || w->layers[i].input_from != prev || w->layers[i + 1].residual_from != prev) break;
+    bool other = false;                              // the block input must have no reader outside the block
+    for (int j = 2; j < n; ++j)
+      if (j != i && j != i + 1 && (w->layers[j].input_from == prev || w->layers[j].residual_from == prev)) other = true;
+    if (other) break;
+    prev = i + 1;
+    ++k;
+  }
+  return k;
 }
 
 aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_bf16, int64_t sB,
@@ -382,9 +450,20 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   const size_t gn_stats_bytes = (sizeof(float2) * (size_t)w->n_groups * chunk + 1023) & ~(size_t)1023;
   const size_t part_bytes = w->live_gn ? gn_stats_bytes + ((sizeof(float2) * gn_part_elems * chunk + 1023) & ~(size_t)1023)
                                        : ((sizeof(float) * (size_t)n_part * chunk + 1023) & ~(size_t)1023);
-  aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots + part_bytes);
+  // shared first stage (see s1_gather_kernel): K streams + one gathered input + K edge results per chunk
+  const int s1_k = s1_chain_blocks(w);
+  const bool s1_on = s1_k > 0 && sB % 4 == 0 && sB < w->layers[0].t_in && chunk >= 2 && !w->live_gn &&
+                     w->layers[1].t_out >= 2 * S1_ROWS && env_int("AFRAME_SHARED_STEM", 1) && env_int("AFRAME_SHARED_S1", 1) &&
+                     env_int("AFRAME_FUSE_BLOCK", 1);
+  const size_t s1_stream_bytes = s1_on ? ((((size_t)(chunk - 1) * (sB / 4) + w->layers[1].t_out) * 128 + 1023) & ~(size_t)1023) : 0;
+  const size_t s1_edge_bytes = s1_on ? (((size_t)2 * chunk * S1_PERIOD * 128 + 1023) & ~(size_t)1023) : 0;
+  const size_t s1_bytes = (size_t)s1_k * s1_stream_bytes + (size_t)(s1_k + 1) * s1_edge_bytes;
+  aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots + part_bytes + s1_bytes);
   if (st != AFRAME_OK) return st;
   char* base = reinterpret_cast<char*>(ctx->ws_act.ptr);
+  char* s1_base = base + slot_bytes * plan.n_slots + part_bytes;
+  auto s1_stream_ptr = [&](int k) { return reinterpret_cast<__nv_bfloat16*>(s1_base + (size_t)(k - 1) * s1_stream_bytes); };             // S_k, k = 1..K
+  auto s1_edge_ptr = [&](int k) { return reinterpret_cast<__nv_bfloat16*>(s1_base + (size_t)s1_k * s1_stream_bytes + (size_t)k * s1_edge_bytes); };  // X (k = 0), Y_k
   float* head_part = reinterpret_cast<float*>(base + slot_bytes * plan.n_slots);
   auto slot_ptr = [&](int layer) { return reinterpret_cast<__nv_bfloat16*>(base + slot_bytes * plan.slot[layer]); };
   if (!ctx->tc_cache) ctx->tc_cache = new std::vector<TcPlanCache>();
@@ -438,6 +517,22 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           if (shared) pc->shared_stem = true;
           pc->fused_with[i] = ib; pc->fused_with[ib] = i;
         }
+      if (s1_on && pc->shared_stem && nb >= 2) {
+        const int T1 = w->layers[1].t_out;
+        const int64_t R0 = (nb - 1) * (sB / 4) + T1;
+        pc->s1_stream.resize(s1_k + 1);
+        pc->s1_edge.resize(s1_k + 1);
+        bool ok = R0 < (1ll << 30) && 2 * nb * S1_PERIOD < (1ll << 30);
+        for (int k = 1; ok && k <= s1_k; ++k) {
+          const int ia = 2 * k, ib = 2 * k + 1;
+          ok = build_block_launch(ctx, w, ia, ib, k == 1 ? slot_ptr(1) : s1_stream_ptr(k - 1), s1_stream_ptr(k), 1, pc->s1_stream[k], 0,
+                                  nullptr, (int)R0) &&
+               build_block_launch(ctx, w, ia, ib, s1_edge_ptr(0), s1_edge_ptr(k), 1, pc->s1_edge[k], 0, nullptr,
+                                  (int)(2 * nb * S1_PERIOD), S1_PERIOD, S1_ROWS);
+        }
+        if (!ok) { caches.pop_back(); return AFRAME_ECUDA; }
+        pc->s1_blocks = s1_k;
+      }
       for (int i = 2; i < n; ++i) {
         const LayerDesc& l = w->layers[i];
         if (l.kind != 0 || pc->fused_with[i] >= 0 || pc->skip[i]) continue;
@@ -485,9 +580,35 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     if (st != AFRAME_OK) return st;
     int n_conv = 0;
     if (ctx->layer_ms) { cudaEventRecord(lev[1], ctx->stream); cudaEventRecord(lev[2], ctx->stream); }
+    if (pc->s1_blocks > 0) {
+      // shared first stage: per block one pass over the stream and one over the short edge windows, then the stitch
+      af_prof_begin(ctx, AFRAME_PROF_CONV);
+      const int T1 = w->layers[1].t_out, K = pc->s1_blocks;
+      const int64_t shift = sB / 4;
+      const uint4* E0 = reinterpret_cast<const uint4*>(slot_ptr(1) + ((nb - 1) * shift + T1) * 64);
+      for (int k = 1; k <= K; ++k) {
+        cudaError_t e = launch_block(pc->s1_stream[k], ctx->stream);
+        ctx->launches++; ++n_conv;
+        if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_block (stream) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
+        const int64_t n_g = 2 * nb * S1_PERIOD * 8;
+        s1_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
+            reinterpret_cast<uint4*>(s1_edge_ptr(0)), reinterpret_cast<const uint4*>(k == 1 ? slot_ptr(1) : s1_stream_ptr(k - 1)),
+            k == 1 ? nullptr : reinterpret_cast<const uint4*>(s1_edge_ptr(k - 1)), k == 1 ? E0 : nullptr, nb, T1, shift, 2 * k, 2 * k - 1);
+        AF_LAUNCH_CHECK(ctx);
+        e = launch_block(pc->s1_edge[k], ctx->stream);
+        ctx->launches++;
+        if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_block (edge) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
+      }
+      const int64_t n_s = nb * T1 * 8;
+      s1_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
+          reinterpret_cast<uint4*>(slot_ptr(2 * K + 1)), reinterpret_cast<const uint4*>(s1_stream_ptr(K)),
+          reinterpret_cast<const uint4*>(s1_edge_ptr(K)), nb, T1, shift, 2 * K + 2, 2 * K + 1);
+      AF_LAUNCH_CHECK(ctx);
+    }
     for (int i = 2; i < n; ++i) {
       const LayerDesc& l = w->layers[i];
       struct Rec { aframe_ctx* c; std::vector<cudaEvent_t>& v; int i; ~Rec() { if (c->layer_ms) cudaEventRecord(v[i + 1], c->stream); } } rec{ctx, lev, i};
+      if (i < 2 + 2 * pc->s1_blocks) continue;                 // ran in shared form above
       if (l.kind == 0 && pc->fused_with[i] > i) continue;      // first conv of a fused block: runs with its partner
       if (pc->skip[i]) continue;                               // projection shortcut: runs inside the conv it feeds
       if (l.kind == 0) {
