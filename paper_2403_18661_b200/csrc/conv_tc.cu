@@ -96,10 +96,14 @@ aframe_status af_tc_check(aframe_ctx* ctx, aframe_weights* w) {
 
 // sc >= 0: layer sc is the 1x1 projection conv whose output is this layer's residual; it runs inside this launch as extra
 // K blocks on its own input sc_in (res must then be null)
+// ov != null (shared stages): the launch runs the layer on ONE long window of ov->t_out output rows (a stream, or a batch of
+// short windows with zeroed separator rows) instead of nb windows of the table's length
+struct TcShapeOverride { int t_out; int zero_period, zero_valid; };
 static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const __nv_bfloat16* in,
                          const __nv_bfloat16* res, __nv_bfloat16* out, int64_t nb, bool head, float* head_part,
-                         TcLaunch& L, int sc = -1, const __nv_bfloat16* sc_in = nullptr) {
-  const LayerDesc& l = w->layers[li];
+                         TcLaunch& L, int sc = -1, const __nv_bfloat16* sc_in = nullptr, const TcShapeOverride* ov = nullptr) {
+  LayerDesc l = w->layers[li];
+  if (ov) { nb = 1; l.t_out = ov->t_out; l.t_in = ov->t_out * l.stride; }
   const int BN = l.c_out >= 256 ? 256 : l.c_out;
   const int cg2_mode = env_int("AFRAME_CG2", 1);                 // 1: CTA pairs (cta_group::2) for the N = 256 layers; 2: also N = 128
   const bool cg2 = (BN == 256 && cg2_mode != 0) || (BN == 128 && cg2_mode >= 2);
@@ -130,7 +134,8 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   }
   L.tm_scw = L.tm_w;
   if (sc >= 0) {
-    const LayerDesc& q = w->layers[sc];
+    LayerDesc q = w->layers[sc];
+    if (ov) { q.t_out = ov->t_out; q.t_in = ov->t_out * q.stride; }
     const uint64_t dims[4] = {(uint64_t)q.c_in, (uint64_t)q.stride, (uint64_t)(q.t_in / q.stride), (uint64_t)nb};
     const uint64_t str[3] = {(uint64_t)q.c_in * 2, (uint64_t)q.stride * q.c_in * 2, (uint64_t)q.t_in * q.c_in * 2};
     const uint32_t box[4] = {64, 1, (uint32_t)T_box, (uint32_t)B_box};
@@ -144,6 +149,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.bias = sc >= 0 ? w->d_bias_sc[li] : w->d_bias[li];
   p.sc_kblocks = sc >= 0 ? w->layers[sc].c_in / 64 : 0;
   p.gn_part = nullptr; p.gn_unit = 64; p.out_f16 = 0;
+  p.zero_period = ov ? ov->zero_period : 0; p.zero_valid = ov ? ov->zero_valid : 0;
   p.taps = l.k; p.pad = l.pad; p.P = P;
   for (int d = 0; d < 3; ++d) {
     const int sft = d - l.pad;
@@ -364,6 +370,52 @@ __global__ void s1_stitch_kernel(uint4* __restrict__ out, const uint4* __restric
   out[i] = v;
 }
 
+// ---- shared second stage ---------------------------------------------------------------------------------------------
+// The stage that follows (stride-2 entry conv + 1x1 projection + stride-1 convs) is shift-equivariant in the same way at
+// half the row spacing.  Its layers run unchanged (conv_tc_kernel) on (1) the stream, as one long window, and (2) a batch
+// of two short windows per window -- the first / last S2_ROWS output rows, i.e. 2 S2_ROWS input rows -- separated by zeroed
+// rows (TcConvParams::zero_period), then s2_stitch_kernel writes the per-window tensor the next stage reads.
+constexpr int S2_ROWS = 30;                 // output rows of a short window at the stage's resolution
+constexpr int S2_PERIOD = 32;               // + 2 separator rows: four short windows per 128-row tile
+
+// Input of the short windows at the previous stage's resolution: [2 nb][2 S2_PERIOD rows][64 ch]; local row r < 2 S2_ROWS
+// is window row r (head) or T1 - 2 S2_ROWS + r (tail), from the first stage's edge results where it is an edge row there
+// (rows < c_head or >= T1 - c_tail), else from its stream; the other rows are zero.
+__global__ void s2_gather_kernel(uint4* __restrict__ X, const uint4* __restrict__ S, const uint4* __restrict__ Y, int64_t nb,
+                                 int64_t n_short /* short windows incl. padding */, int T1, int64_t row_shift, int c_head, int c_tail) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_short * (2 * S2_PERIOD) * 8) return;
+  const int j = (int)(i & 7);
+  const int64_t mr = i >> 3;
+  const int r = (int)(mr % (2 * S2_PERIOD));
+  const int64_t m = mr / (2 * S2_PERIOD), b = m >> 1;
+  const bool tail = (m & 1) != 0;
+  uint4 v = make_uint4(0u, 0u, 0u, 0u);
+  if (r < 2 * S2_ROWS && b < nb) {
+    const int t = tail ? T1 - 2 * S2_ROWS + r : r;
+    if (!tail && t < c_head) v = Y[(m * S1_PERIOD + t) * 8 + j];
+    else if (tail && t >= T1 - c_tail) v = Y[(m * S1_PERIOD + (t - (T1 - S1_ROWS))) * 8 + j];
+    else v = S[(b * row_shift + t) * 8 + j];
+  }
+  X[i] = v;
+}
+
+// out[b][t][C]: edge result where t is an edge row of window b (t < c_head or t >= T2 - c_tail), else the stream row
+__global__ void s2_stitch_kernel(uint4* __restrict__ out, const uint4* __restrict__ S, const uint4* __restrict__ Y, int64_t nb,
+                                 int T2, int pieces /* C / 8 */, int64_t row_shift, int c_head, int c_tail) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nb * T2 * pieces) return;
+  const int j = (int)(i % pieces);
+  const int64_t bt = i / pieces;
+  const int t = (int)(bt % T2);
+  const int64_t b = bt / T2;
+  uint4 v;
+  if (t < c_head) v = Y[((2 * b) * S2_PERIOD + t) * pieces + j];
+  else if (t >= T2 - c_tail) v = Y[((2 * b + 1) * S2_PERIOD + (t - (T2 - S2_ROWS))) * pieces + j];
+  else v = S[(b * row_shift + t) * pieces + j];
+  out[i] = v;
+}
+
 struct TcPlanCache {
   const aframe_weights* w = nullptr;
   void* base = nullptr;
@@ -376,6 +428,9 @@ struct TcPlanCache {
   bool shared_stem = false;           // stem of the whole stream + edge rows instead of one stem per window
   int s1_blocks = 0;                  // > 0: the first s1_blocks fused blocks run in shared form (see s1_gather_kernel)
   std::vector<TcBlockLaunch> s1_stream, s1_edge;
+  std::vector<int> s2_layers;         // non-empty: these layers (entry conv, then the stride-1 convs) run in shared form
+  std::vector<TcLaunch> s2_stream, s2_edge;   // parallel to s2_layers
+  int s2_head = 0, s2_tail = 0;       // edge rows of the stage's output per window
   std::vector<int> sc_of;             // per layer: the projection-shortcut conv that runs inside it (else -1)
   std::vector<char> skip;             // per layer: runs inside another launch
 };
@@ -413,6 +468,42 @@ static int s1_chain_blocks(const aframe_weights* w) {
     ++k;
   }
   return k;
+}
+
+// Layers of the stage after the shared first stage, if it has the form the shared second stage handles: entry conv k3 s2
+// (i0), projection k1 s2 (i0 + 1, folded into i0 + 2), then stride-1 k3 convs in basic blocks, all with the same width.
+// Returns the layers that launch, in order (i0, i0 + 2, i0 + 3, ...); empty if the pattern does not match.
+static std::vector<int> s2_chain_layers(const aframe_weights* w, int i0) {
+  std::vector<int> out;
+  const int n = (int)w->layers.size();
+  if (i0 + 2 >= n - 1) return out;
+  const int prev = i0 - 1;
+  const LayerDesc& e = w->layers[i0];
+  const LayerDesc& q = w->layers[i0 + 1];
+  const LayerDesc& f = w->layers[i0 + 2];
+  auto conv3 = [&](const LayerDesc& l, int stride) { return l.kind == 0 && l.k == 3 && l.stride == stride && l.pad == 1 && l.relu && l.c_out == e.c_out; };
+  if (!conv3(e, 2) || e.input_from != prev || e.residual_from >= 0 || e.c_out > 128) return out;
+  if (!(q.kind == 0 && q.k == 1 && q.stride == 2 && q.pad == 0 && !q.relu && q.input_from == prev && q.residual_from < 0 && q.c_out == e.c_out)) return out;
+  if (!conv3(f, 1) || f.input_from != i0 || f.residual_from != i0 + 1 || !w->d_bias_sc[i0 + 2]) return out;
+  for (int j = 2; j < n; ++j)                     // the first stage's output feeds only the entry conv and the projection
+    if (j != i0 && j != i0 + 1 && (w->layers[j].input_from == prev || w->layers[j].residual_from == prev)) return out;
+  out.push_back(i0); out.push_back(i0 + 2);
+  int blk_in = i0 + 2;
+  for (int j = i0 + 3; j + 1 < n - 1; j += 2) {
+    const LayerDesc& a = w->layers[j];
+    const LayerDesc& b = w->layers[j + 1];
+    if (!conv3(a, 1) || !conv3(b, 1) || a.input_from != blk_in || a.residual_from >= 0 || b.input_from != j || b.residual_from != blk_in) break;
+    out.push_back(j); out.push_back(j + 1);
+    blk_in = j + 1;
+  }
+  // every tensor inside the chain is read only inside the chain (the last one is stitched for whoever reads it)
+  const int last = out.back();
+  for (int j = 2; j < n; ++j) {
+    if (j >= i0 && j <= last) continue;
+    const int a = w->layers[j].input_from, r = w->layers[j].residual_from;
+    if ((a >= i0 && a < last) || (r >= i0 && r < last)) { out.clear(); return out; }
+  }
+  return out;
 }
 
 aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_bf16, int64_t sB,
@@ -455,14 +546,44 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   const bool s1_on = s1_k > 0 && sB % 4 == 0 && sB < w->layers[0].t_in && chunk >= 2 && !w->live_gn &&
                      w->layers[1].t_out >= 2 * S1_ROWS && env_int("AFRAME_SHARED_STEM", 1) && env_int("AFRAME_SHARED_S1", 1) &&
                      env_int("AFRAME_FUSE_BLOCK", 1);
-  const size_t s1_stream_bytes = s1_on ? ((((size_t)(chunk - 1) * (sB / 4) + w->layers[1].t_out) * 128 + 1023) & ~(size_t)1023) : 0;
+  // shared second stage (see s2_gather_kernel): per launched layer one stream and one edge-batch tensor, plus the gathered input
+  auto up128 = [](int64_t v) { return (v + 127) / 128 * 128; };
+  std::vector<int> s2_list;
+  int s2_i0 = 0, s2_T2 = 0, s2_C = 0, s2_head = 0, s2_tail = 0;
+  if (s1_on && (sB / 4) % 2 == 0 && env_int("AFRAME_SHARED_S2", 1) && env_int("AFRAME_FUSE_SC", 1)) {
+    s2_i0 = 2 + 2 * s1_k;
+    s2_list = s2_chain_layers(w, s2_i0);
+    if (!s2_list.empty()) {
+      const int T1 = w->layers[1].t_out, h1 = 2 * s1_k + 2, t1 = 2 * s1_k + 1, n2 = (int)s2_list.size() - 1;
+      s2_T2 = w->layers[s2_i0].t_out; s2_C = w->layers[s2_i0].c_out;
+      s2_head = h1 / 2 + 1 + n2;                                    // rows within reach of the window's zero padding ...
+      s2_tail = s2_T2 - (T1 - t1 - 1 + 1) / 2 + n2;                 // ... at the start and at the end of the stage's output
+      const bool fits = s2_head + n2 <= S2_ROWS && s2_tail + n2 + 1 <= S2_ROWS && s2_T2 >= S2_ROWS && T1 >= 2 * S2_ROWS &&
+                        T1 == 2 * s2_T2 && h1 <= S1_ROWS - 2 && t1 <= S1_ROWS - 2 && s2_C % 64 == 0;
+      if (!fits) s2_list.clear();
+    }
+  }
+  const bool s2_on = !s2_list.empty();
+  const int64_t s2_rows_stream = s2_on ? up128((chunk - 1) * (sB / 8) + s2_T2) : 0;    // R2p at the largest chunk
+  const int64_t s2_rows_edge = s2_on ? up128(2 * chunk * S2_PERIOD) : 0;
+  const int64_t s1_rows = (chunk - 1) * (sB / 4) + w->layers[1].t_out;
+  const size_t s1_stream_bytes = s1_on ? (((size_t)(s2_on && 2 * s2_rows_stream > s1_rows ? 2 * s2_rows_stream : s1_rows) * 128 + 1023) & ~(size_t)1023) : 0;
   const size_t s1_edge_bytes = s1_on ? (((size_t)2 * chunk * S1_PERIOD * 128 + 1023) & ~(size_t)1023) : 0;
   const size_t s1_bytes = (size_t)s1_k * s1_stream_bytes + (size_t)(s1_k + 1) * s1_edge_bytes;
-  aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots + part_bytes + s1_bytes);
+  const size_t s2_stream_bytes = s2_on ? (((size_t)s2_rows_stream * s2_C * 2 + 1023) & ~(size_t)1023) : 0;
+  const size_t s2_edge_bytes = s2_on ? (((size_t)s2_rows_edge * s2_C * 2 + 1023) & ~(size_t)1023) : 0;
+  const size_t s2_x_bytes = s2_on ? (((size_t)2 * s2_rows_edge * 128 + 1023) & ~(size_t)1023) : 0;
+  const size_t s2_bytes = s2_list.size() * (s2_stream_bytes + s2_edge_bytes) + s2_x_bytes;
+  aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots + part_bytes + s1_bytes + s2_bytes);
   if (st != AFRAME_OK) return st;
   char* base = reinterpret_cast<char*>(ctx->ws_act.ptr);
   char* s1_base = base + slot_bytes * plan.n_slots + part_bytes;
   auto s1_stream_ptr = [&](int k) { return reinterpret_cast<__nv_bfloat16*>(s1_base + (size_t)(k - 1) * s1_stream_bytes); };             // S_k, k = 1..K
+  char* s2_base = s1_base + s1_bytes;
+  auto s2_x_ptr = [&]() { return reinterpret_cast<__nv_bfloat16*>(s2_base); };
+  auto s2_buf = [&](int pass, int idx) {           // pass 0: stream, 1: edge batch; idx: position in s2_list
+    return reinterpret_cast<__nv_bfloat16*>(s2_base + s2_x_bytes + (size_t)idx * (s2_stream_bytes + s2_edge_bytes) + (pass ? s2_stream_bytes : 0));
+  };
   auto s1_edge_ptr = [&](int k) { return reinterpret_cast<__nv_bfloat16*>(s1_base + (size_t)s1_k * s1_stream_bytes + (size_t)k * s1_edge_bytes); };  // X (k = 0), Y_k
   float* head_part = reinterpret_cast<float*>(base + slot_bytes * plan.n_slots);
   auto slot_ptr = [&](int layer) { return reinterpret_cast<__nv_bfloat16*>(base + slot_bytes * plan.slot[layer]); };
@@ -532,6 +653,30 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         }
         if (!ok) { caches.pop_back(); return AFRAME_ECUDA; }
         pc->s1_blocks = s1_k;
+        if (s2_on) {
+          const int64_t rows[2] = {up128((nb - 1) * (sB / 8) + s2_T2), up128(2 * nb * S2_PERIOD)};
+          const __nv_bfloat16* src[2] = {s1_stream_ptr(s1_k), s2_x_ptr()};
+          auto idx_of = [&](int layer) { for (size_t q = 0; q < s2_list.size(); ++q) if (s2_list[q] == layer) return (int)q; return -1; };
+          pc->s2_stream.resize(s2_list.size());
+          pc->s2_edge.resize(s2_list.size());
+          for (size_t q = 0; ok && q < s2_list.size(); ++q) {
+            const int li = s2_list[q];
+            const LayerDesc& l = w->layers[li];
+            for (int pass = 0; ok && pass < 2; ++pass) {
+              const TcShapeOverride ov{(int)rows[pass], pass ? S2_PERIOD : 0, pass ? S2_ROWS : 0};
+              const bool entry = li == s2_i0;
+              const int sc = pc->sc_of[li];
+              const __nv_bfloat16* in = entry ? src[pass] : s2_buf(pass, idx_of(l.input_from));
+              const __nv_bfloat16* res = (l.residual_from >= 0 && sc < 0) ? s2_buf(pass, idx_of(l.residual_from)) : nullptr;
+              ok = (entry || idx_of(l.input_from) >= 0) && (res == nullptr || idx_of(l.residual_from) >= 0) &&
+                   build_launch(ctx, w, li, in, res, s2_buf(pass, (int)q), 1, false, nullptr, pass ? pc->s2_edge[q] : pc->s2_stream[q],
+                                sc, sc >= 0 ? src[pass] : nullptr, &ov);
+            }
+          }
+          if (!ok) { caches.pop_back(); return AFRAME_ECUDA; }
+          pc->s2_layers = s2_list;
+          pc->s2_head = s2_head; pc->s2_tail = s2_tail;
+        }
       }
       for (int i = 2; i < n; ++i) {
         const LayerDesc& l = w->layers[i];
@@ -599,16 +744,42 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         ctx->launches++;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_block (edge) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
       }
-      const int64_t n_s = nb * T1 * 8;
-      s1_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
-          reinterpret_cast<uint4*>(slot_ptr(2 * K + 1)), reinterpret_cast<const uint4*>(s1_stream_ptr(K)),
-          reinterpret_cast<const uint4*>(s1_edge_ptr(K)), nb, T1, shift, 2 * K + 2, 2 * K + 1);
-      AF_LAUNCH_CHECK(ctx);
+      if (pc->s2_layers.empty()) {
+        const int64_t n_s = nb * T1 * 8;
+        s1_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
+            reinterpret_cast<uint4*>(slot_ptr(2 * K + 1)), reinterpret_cast<const uint4*>(s1_stream_ptr(K)),
+            reinterpret_cast<const uint4*>(s1_edge_ptr(K)), nb, T1, shift, 2 * K + 2, 2 * K + 1);
+        AF_LAUNCH_CHECK(ctx);
+      } else {
+        // shared second stage: its layers read the first stage's stream and edge results directly (no stitch in between)
+        const int64_t n_short = up128(2 * nb * S2_PERIOD) / S2_PERIOD;
+        const int64_t n_g = n_short * (2 * S2_PERIOD) * 8;
+        s2_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
+            reinterpret_cast<uint4*>(s2_x_ptr()), reinterpret_cast<const uint4*>(s1_stream_ptr(K)),
+            reinterpret_cast<const uint4*>(s1_edge_ptr(K)), nb, n_short, T1, shift, 2 * K + 2, 2 * K + 1);
+        AF_LAUNCH_CHECK(ctx);
+        for (size_t q = 0; q < pc->s2_layers.size(); ++q)
+          for (int pass = 0; pass < 2; ++pass) {
+            TcLaunch& L2 = pass ? pc->s2_edge[q] : pc->s2_stream[q];
+            L2.p.reverse = 0;
+            cudaError_t e = launch_conv(L2, ctx->stream);
+            ctx->launches++; ++n_conv;
+            if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (shared stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
+          }
+        const int last = pc->s2_layers.back(), q_last = (int)pc->s2_layers.size() - 1;
+        const int T2 = w->layers[last].t_out, pieces = w->layers[last].c_out / 8;
+        const int64_t n_s = nb * T2 * pieces;
+        s2_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
+            reinterpret_cast<uint4*>(slot_ptr(last)), reinterpret_cast<const uint4*>(s2_buf(0, q_last)),
+            reinterpret_cast<const uint4*>(s2_buf(1, q_last)), nb, T2, pieces, shift / 2, pc->s2_head, pc->s2_tail);
+        AF_LAUNCH_CHECK(ctx);
+      }
     }
     for (int i = 2; i < n; ++i) {
       const LayerDesc& l = w->layers[i];
       struct Rec { aframe_ctx* c; std::vector<cudaEvent_t>& v; int i; ~Rec() { if (c->layer_ms) cudaEventRecord(v[i + 1], c->stream); } } rec{ctx, lev, i};
       if (i < 2 + 2 * pc->s1_blocks) continue;                 // ran in shared form above
+      if (!pc->s2_layers.empty() && i <= pc->s2_layers.back()) continue;
       if (l.kind == 0 && pc->fused_with[i] > i) continue;      // first conv of a fused block: runs with its partner
       if (pc->skip[i]) continue;                               // projection shortcut: runs inside the conv it feeds
       if (l.kind == 0) {

@@ -69,6 +69,9 @@ struct TcConvParams {
   // the sum and sum of squares of the fp32 accumulators: gn_part[(b * T/32 + slab) * (c_out / gn_unit) + unit]
   float2* gn_part;           // null = off
   int gn_unit;               // min(C / G, 64): 8, 16, 32 or 64
+  // shared stages (conv_tc.cu): the launch covers a batch of short windows stored back to back; output rows t with
+  // t % zero_period >= zero_valid are separators and are stored as zero (they are the short windows' zero padding)
+  int zero_period, zero_valid;   // 0 = off
   int out_f16;               // store the (pre-norm) output as fp16 (saturating) instead of bf16: z = mu + O(sigma) loses
                              // |mu| / sigma times more to an 8-bit mantissa than the normalised value does
   int w_bytes;               // resident weight region (0 unless HALO)
@@ -108,7 +111,8 @@ __device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b
 // (lo = 0: ReLU, which commutes with the rounding; lo = -inf: none) -> staging buffer, or the fused head's dot product.
 template <bool RES, bool HEAD, bool F16 = false>
 __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4* bias4, const float4* hw4,
-                                                 unsigned char* rowp, int row, __nv_bfloat162 lo2, float& head_acc) {
+                                                 unsigned char* rowp, int row, __nv_bfloat162 lo2, float& head_acc,
+                                                 bool zero_row = false) {
   float hacc[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
   for (int jj = 0; jj < 8; ++jj) {                 // 8 pieces of 8 channels (16 B of bf16)
@@ -138,6 +142,7 @@ __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4
       for (int e = 0; e < 4; ++e)
         asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(ow[e]) : "f"(f[2 * e + 1]), "f"(f[2 * e]));
     }
+    if (zero_row) o = make_uint4(0u, 0u, 0u, 0u);
     if (HEAD) {
       const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
       const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
@@ -527,9 +532,10 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         unsigned char* rowp = gen_base + (sbuf - base) + row * 128;
         // straight-line code per variant (no run-time branches inside the unrolled loop, so the 8 pieces interleave)
         const __nv_bfloat162 lo2 = __float2bfloat162_rn(p.relu ? 0.f : -INFINITY);
-        if (p.has_res) tc_epilogue_math<true, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc);
+        const bool zero_row = p.zero_period > 0 && ((t0 + row % p.T_box) % p.zero_period) >= p.zero_valid;
+        if (p.has_res) tc_epilogue_math<true, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row);
         else if (!HEAD && p.out_f16) tc_epilogue_math<false, false, true>(v, bias4, hw4, rowp, row, lo2, head_acc);
-        else tc_epilogue_math<false, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc);
+        else tc_epilogue_math<false, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row);
         if (HEAD) {
           // the warp's 32 rows are one 32-row slab of one window (T_box % 32 == 0): reduce and emit a partial
           float s = head_acc;
