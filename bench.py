@@ -394,10 +394,11 @@ def run_ours(args):
                      "peak_kind": "sustained bf16 cuBLAS, " + peaks["source"], "launches": int(conv_launches),
                      "avg_launch_ms": conv_ms / max(conv_launches, 1),
                      "algorithmic": "2 x 1069.5 MMAC per window x windows scored (the method's work per window), over the "
-                                    "summed CUDA-event time of the conv launches on the library's stream; the 64-channel stage "
-                                    "(56.6 MMAC) is computed once per stream plus two 18-row edge windows per window, so the "
-                                    "tensor cores EXECUTE 0.952 of these FLOPs (DESIGN.md section 5, shared first stage)",
-                     "executed_frac_of_algorithmic": 0.952},
+                                    "summed CUDA-event time of the conv launches on the library's stream; the 64- and "
+                                    "128-channel stages (56.6 + 144.7 MMAC) are computed once per stream plus two short edge "
+                                    "windows per window, so the tensor cores EXECUTE 0.845 of these FLOPs (DESIGN.md section 5, "
+                                    "shared first / second stage)",
+                     "executed_frac_of_algorithmic": 0.845},
         "stages": {k: {"ms": v[0], "launches": v[1], "share": v[0] / ms_total} for k, v in stages.items()},
     }
     wh_ms = stages["whiten"][0]
