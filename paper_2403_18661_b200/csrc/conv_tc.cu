@@ -378,24 +378,26 @@ __global__ void s1_stitch_kernel(uint4* __restrict__ out, const uint4* __restric
 constexpr int S2_ROWS = 30;                 // output rows of a short window at the stage's resolution
 constexpr int S2_PERIOD = 32;               // + 2 separator rows: four short windows per 128-row tile
 
-// Input of the short windows at the previous stage's resolution: [2 nb][2 S2_PERIOD rows][64 ch]; local row r < 2 S2_ROWS
-// is window row r (head) or T1 - 2 S2_ROWS + r (tail), from the first stage's edge results where it is an edge row there
-// (rows < c_head or >= T1 - c_tail), else from its stream; the other rows are zero.
-__global__ void s2_gather_kernel(uint4* __restrict__ X, const uint4* __restrict__ S, const uint4* __restrict__ Y, int64_t nb,
-                                 int64_t n_short /* short windows incl. padding */, int T1, int64_t row_shift, int c_head, int c_tail) {
+// Input of a stage's short windows at the previous stage's resolution: [short windows][2 S2_PERIOD rows][pieces * 8 ch];
+// local row r < 2 S2_ROWS is window row r (head) or Tp - 2 S2_ROWS + r (tail), taken from the previous stage's edge batch
+// (period src_period, src_rows data rows per short window) where it is an edge row there (rows < c_head or >= Tp - c_tail),
+// else from the previous stage's stream; the other rows are zero.
+__global__ void sh_gather_kernel(uint4* __restrict__ X, const uint4* __restrict__ S, const uint4* __restrict__ Y, int64_t nb,
+                                 int64_t n_short /* short windows incl. padding */, int Tp, int pieces, int64_t row_shift,
+                                 int src_period, int src_rows, int c_head, int c_tail) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_short * (2 * S2_PERIOD) * 8) return;
-  const int j = (int)(i & 7);
-  const int64_t mr = i >> 3;
+  if (i >= n_short * (2 * S2_PERIOD) * pieces) return;
+  const int j = (int)(i % pieces);
+  const int64_t mr = i / pieces;
   const int r = (int)(mr % (2 * S2_PERIOD));
   const int64_t m = mr / (2 * S2_PERIOD), b = m >> 1;
   const bool tail = (m & 1) != 0;
   uint4 v = make_uint4(0u, 0u, 0u, 0u);
   if (r < 2 * S2_ROWS && b < nb) {
-    const int t = tail ? T1 - 2 * S2_ROWS + r : r;
-    if (!tail && t < c_head) v = Y[(m * S1_PERIOD + t) * 8 + j];
-    else if (tail && t >= T1 - c_tail) v = Y[(m * S1_PERIOD + (t - (T1 - S1_ROWS))) * 8 + j];
-    else v = S[(b * row_shift + t) * 8 + j];
+    const int t = tail ? Tp - 2 * S2_ROWS + r : r;
+    if (!tail && t < c_head) v = Y[(m * src_period + t) * pieces + j];
+    else if (tail && t >= Tp - c_tail) v = Y[(m * src_period + (t - (Tp - src_rows))) * pieces + j];
+    else v = S[(b * row_shift + t) * pieces + j];
   }
   X[i] = v;
 }
@@ -428,9 +430,13 @@ struct TcPlanCache {
   bool shared_stem = false;           // stem of the whole stream + edge rows instead of one stem per window
   int s1_blocks = 0;                  // > 0: the first s1_blocks fused blocks run in shared form (see s1_gather_kernel)
   std::vector<TcBlockLaunch> s1_stream, s1_edge;
-  std::vector<int> s2_layers;         // non-empty: these layers (entry conv, then the stride-1 convs) run in shared form
-  std::vector<TcLaunch> s2_stream, s2_edge;   // parallel to s2_layers
-  int s2_head = 0, s2_tail = 0;       // edge rows of the stage's output per window
+  struct SharedStagePlan {
+    std::vector<int> layers;          // these layers (entry conv, then the stride-1 convs) run in shared form
+    std::vector<TcLaunch> stream, edge;   // parallel to layers
+    int T = 0, C = 0, C_in = 0, head = 0, tail = 0;   // output rows / channels, input channels, edge rows per window
+    int64_t shift = 0;                // rows between consecutive windows
+  };
+  std::vector<SharedStagePlan> sh;    // the stages after the first that run in shared form, in order
   std::vector<int> sc_of;             // per layer: the projection-shortcut conv that runs inside it (else -1)
   std::vector<char> skip;             // per layer: runs inside another launch
 };
@@ -482,7 +488,7 @@ static std::vector<int> s2_chain_layers(const aframe_weights* w, int i0) {
   const LayerDesc& q = w->layers[i0 + 1];
   const LayerDesc& f = w->layers[i0 + 2];
   auto conv3 = [&](const LayerDesc& l, int stride) { return l.kind == 0 && l.k == 3 && l.stride == stride && l.pad == 1 && l.relu && l.c_out == e.c_out; };
-  if (!conv3(e, 2) || e.input_from != prev || e.residual_from >= 0 || e.c_out > 128) return out;
+  if (!conv3(e, 2) || e.input_from != prev || e.residual_from >= 0) return out;
   if (!(q.kind == 0 && q.k == 1 && q.stride == 2 && q.pad == 0 && !q.relu && q.input_from == prev && q.residual_from < 0 && q.c_out == e.c_out)) return out;
   if (!conv3(f, 1) || f.input_from != i0 || f.residual_from != i0 + 1 || !w->d_bias_sc[i0 + 2]) return out;
   for (int j = 2; j < n; ++j)                     // the first stage's output feeds only the entry conv and the projection
@@ -546,43 +552,66 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   const bool s1_on = s1_k > 0 && sB % 4 == 0 && sB < w->layers[0].t_in && chunk >= 2 && !w->live_gn &&
                      w->layers[1].t_out >= 2 * S1_ROWS && env_int("AFRAME_SHARED_STEM", 1) && env_int("AFRAME_SHARED_S1", 1) &&
                      env_int("AFRAME_FUSE_BLOCK", 1);
-  // shared second stage (see s2_gather_kernel): per launched layer one stream and one edge-batch tensor, plus the gathered input
+  // shared later stages (see sh_gather_kernel): per launched layer one stream and one edge-batch tensor, plus the gathered input
   auto up128 = [](int64_t v) { return (v + 127) / 128 * 128; };
-  std::vector<int> s2_list;
-  int s2_i0 = 0, s2_T2 = 0, s2_C = 0, s2_head = 0, s2_tail = 0;
-  if (s1_on && (sB / 4) % 2 == 0 && env_int("AFRAME_SHARED_S2", 1) && env_int("AFRAME_FUSE_SC", 1)) {
-    s2_i0 = 2 + 2 * s1_k;
-    s2_list = s2_chain_layers(w, s2_i0);
-    if (!s2_list.empty()) {
-      const int T1 = w->layers[1].t_out, h1 = 2 * s1_k + 2, t1 = 2 * s1_k + 1, n2 = (int)s2_list.size() - 1;
-      s2_T2 = w->layers[s2_i0].t_out; s2_C = w->layers[s2_i0].c_out;
-      s2_head = h1 / 2 + 1 + n2;                                    // rows within reach of the window's zero padding ...
-      s2_tail = s2_T2 - (T1 - t1 - 1 + 1) / 2 + n2;                 // ... at the start and at the end of the stage's output
-      const bool fits = s2_head + n2 <= S2_ROWS && s2_tail + n2 + 1 <= S2_ROWS && s2_T2 >= S2_ROWS && T1 >= 2 * S2_ROWS &&
-                        T1 == 2 * s2_T2 && h1 <= S1_ROWS - 2 && t1 <= S1_ROWS - 2 && s2_C % 64 == 0;
-      if (!fits) s2_list.clear();
+  struct SharedStage {
+    std::vector<int> list;            // layers that launch, entry conv first
+    int i0 = 0, T = 0, C = 0, C_in = 0, head = 0, tail = 0;
+    int64_t shift = 0;                // rows between consecutive windows at this stage's resolution
+    int64_t rows_stream = 0, rows_edge = 0;
+    size_t stream_bytes = 0, edge_bytes = 0, x_bytes = 0, off = 0;
+  };
+  std::vector<SharedStage> shs;
+  if (s1_on && env_int("AFRAME_SHARED_S2", 1) && env_int("AFRAME_FUSE_SC", 1)) {
+    int i0 = 2 + 2 * s1_k, Tp = w->layers[1].t_out, hp = 2 * s1_k + 2, tp = 2 * s1_k + 1;
+    int64_t shift_p = sB / 4;
+    const int max_stages = env_int("AFRAME_SHARED_STAGES", 2);
+    while ((int)shs.size() < max_stages && shift_p % 2 == 0) {
+      SharedStage g;
+      g.list = s2_chain_layers(w, i0);
+      if (g.list.empty()) break;
+      if (fuse >= i0 && fuse <= g.list.back()) break;             // the stage that ends in the fused head stays per window
+      const int n2 = (int)g.list.size() - 1;
+      g.i0 = i0; g.T = w->layers[i0].t_out; g.C = w->layers[i0].c_out; g.C_in = w->layers[i0].c_in;
+      g.shift = shift_p / 2;
+      g.head = hp / 2 + 1 + n2;                                   // rows within reach of the window's zero padding ...
+      g.tail = g.T - (Tp - tp) / 2 + n2;                          // ... at the start and at the end of the stage's output
+      const int src_rows = shs.empty() ? S1_ROWS : S2_ROWS;
+      const bool fits = g.head + n2 <= S2_ROWS && g.tail + n2 + 1 <= S2_ROWS && g.T >= S2_ROWS && Tp >= 2 * S2_ROWS && Tp == 2 * g.T &&
+                        hp <= src_rows - 2 && tp <= src_rows - 2 && g.C % 64 == 0 && g.C_in % 64 == 0;
+      if (!fits) break;
+      g.rows_stream = up128((chunk - 1) * g.shift + g.T);
+      g.rows_edge = up128(2 * chunk * S2_PERIOD);
+      shs.push_back(g);
+      i0 = g.list.back() + 1; Tp = g.T; hp = g.head; tp = g.tail; shift_p = g.shift;
     }
   }
-  const bool s2_on = !s2_list.empty();
-  const int64_t s2_rows_stream = s2_on ? up128((chunk - 1) * (sB / 8) + s2_T2) : 0;    // R2p at the largest chunk
-  const int64_t s2_rows_edge = s2_on ? up128(2 * chunk * S2_PERIOD) : 0;
+  const bool s2_on = !shs.empty();
   const int64_t s1_rows = (chunk - 1) * (sB / 4) + w->layers[1].t_out;
-  const size_t s1_stream_bytes = s1_on ? (((size_t)(s2_on && 2 * s2_rows_stream > s1_rows ? 2 * s2_rows_stream : s1_rows) * 128 + 1023) & ~(size_t)1023) : 0;
+  const size_t s1_stream_bytes = s1_on ? (((size_t)(s2_on && 2 * shs[0].rows_stream > s1_rows ? 2 * shs[0].rows_stream : s1_rows) * 128 + 1023) & ~(size_t)1023) : 0;
   const size_t s1_edge_bytes = s1_on ? (((size_t)2 * chunk * S1_PERIOD * 128 + 1023) & ~(size_t)1023) : 0;
   const size_t s1_bytes = (size_t)s1_k * s1_stream_bytes + (size_t)(s1_k + 1) * s1_edge_bytes;
-  const size_t s2_stream_bytes = s2_on ? (((size_t)s2_rows_stream * s2_C * 2 + 1023) & ~(size_t)1023) : 0;
-  const size_t s2_edge_bytes = s2_on ? (((size_t)s2_rows_edge * s2_C * 2 + 1023) & ~(size_t)1023) : 0;
-  const size_t s2_x_bytes = s2_on ? (((size_t)2 * s2_rows_edge * 128 + 1023) & ~(size_t)1023) : 0;
-  const size_t s2_bytes = s2_list.size() * (s2_stream_bytes + s2_edge_bytes) + s2_x_bytes;
+  size_t s2_bytes = 0;
+  for (size_t g = 0; g < shs.size(); ++g) {
+    SharedStage& h = shs[g];
+    // a stage's stream is also read by the next stage's entry conv, over twice that stage's (padded) row count
+    const int64_t alloc_rows = g + 1 < shs.size() && 2 * shs[g + 1].rows_stream > h.rows_stream ? 2 * shs[g + 1].rows_stream : h.rows_stream;
+    h.stream_bytes = ((size_t)alloc_rows * h.C * 2 + 1023) & ~(size_t)1023;
+    h.edge_bytes = ((size_t)h.rows_edge * h.C * 2 + 1023) & ~(size_t)1023;
+    h.x_bytes = ((size_t)2 * h.rows_edge * h.C_in * 2 + 1023) & ~(size_t)1023;
+    h.off = s2_bytes;
+    s2_bytes += h.x_bytes + h.list.size() * (h.stream_bytes + h.edge_bytes);
+  }
   aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots + part_bytes + s1_bytes + s2_bytes);
   if (st != AFRAME_OK) return st;
   char* base = reinterpret_cast<char*>(ctx->ws_act.ptr);
   char* s1_base = base + slot_bytes * plan.n_slots + part_bytes;
   auto s1_stream_ptr = [&](int k) { return reinterpret_cast<__nv_bfloat16*>(s1_base + (size_t)(k - 1) * s1_stream_bytes); };             // S_k, k = 1..K
   char* s2_base = s1_base + s1_bytes;
-  auto s2_x_ptr = [&]() { return reinterpret_cast<__nv_bfloat16*>(s2_base); };
-  auto s2_buf = [&](int pass, int idx) {           // pass 0: stream, 1: edge batch; idx: position in s2_list
-    return reinterpret_cast<__nv_bfloat16*>(s2_base + s2_x_bytes + (size_t)idx * (s2_stream_bytes + s2_edge_bytes) + (pass ? s2_stream_bytes : 0));
+  auto sh_x_ptr = [&](int g) { return reinterpret_cast<__nv_bfloat16*>(s2_base + shs[g].off); };
+  auto sh_buf = [&](int g, int pass, int idx) {    // pass 0: stream, 1: edge batch; idx: position in the stage's list
+    const SharedStage& h = shs[g];
+    return reinterpret_cast<__nv_bfloat16*>(s2_base + h.off + h.x_bytes + (size_t)idx * (h.stream_bytes + h.edge_bytes) + (pass ? h.stream_bytes : 0));
   };
   auto s1_edge_ptr = [&](int k) { return reinterpret_cast<__nv_bfloat16*>(s1_base + (size_t)s1_k * s1_stream_bytes + (size_t)k * s1_edge_bytes); };  // X (k = 0), Y_k
   float* head_part = reinterpret_cast<float*>(base + slot_bytes * plan.n_slots);
@@ -653,30 +682,33 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         }
         if (!ok) { caches.pop_back(); return AFRAME_ECUDA; }
         pc->s1_blocks = s1_k;
-        if (s2_on) {
-          const int64_t rows[2] = {up128((nb - 1) * (sB / 8) + s2_T2), up128(2 * nb * S2_PERIOD)};
-          const __nv_bfloat16* src[2] = {s1_stream_ptr(s1_k), s2_x_ptr()};
-          auto idx_of = [&](int layer) { for (size_t q = 0; q < s2_list.size(); ++q) if (s2_list[q] == layer) return (int)q; return -1; };
-          pc->s2_stream.resize(s2_list.size());
-          pc->s2_edge.resize(s2_list.size());
-          for (size_t q = 0; ok && q < s2_list.size(); ++q) {
-            const int li = s2_list[q];
+        pc->sh.resize(shs.size());
+        for (size_t g = 0; ok && g < shs.size(); ++g) {
+          const SharedStage& h = shs[g];
+          TcPlanCache::SharedStagePlan& P = pc->sh[g];
+          const int64_t rows[2] = {up128((nb - 1) * h.shift + h.T), up128(2 * nb * S2_PERIOD)};
+          const __nv_bfloat16* src[2] = {g == 0 ? s1_stream_ptr(s1_k) : sh_buf((int)g - 1, 0, (int)shs[g - 1].list.size() - 1), sh_x_ptr((int)g)};
+          auto idx_of = [&](int layer) { for (size_t q = 0; q < h.list.size(); ++q) if (h.list[q] == layer) return (int)q; return -1; };
+          P.stream.resize(h.list.size());
+          P.edge.resize(h.list.size());
+          for (size_t q = 0; ok && q < h.list.size(); ++q) {
+            const int li = h.list[q];
             const LayerDesc& l = w->layers[li];
             for (int pass = 0; ok && pass < 2; ++pass) {
               const TcShapeOverride ov{(int)rows[pass], pass ? S2_PERIOD : 0, pass ? S2_ROWS : 0};
-              const bool entry = li == s2_i0;
+              const bool entry = li == h.i0;
               const int sc = pc->sc_of[li];
-              const __nv_bfloat16* in = entry ? src[pass] : s2_buf(pass, idx_of(l.input_from));
-              const __nv_bfloat16* res = (l.residual_from >= 0 && sc < 0) ? s2_buf(pass, idx_of(l.residual_from)) : nullptr;
+              const __nv_bfloat16* in = entry ? src[pass] : sh_buf((int)g, pass, idx_of(l.input_from));
+              const __nv_bfloat16* res = (l.residual_from >= 0 && sc < 0) ? sh_buf((int)g, pass, idx_of(l.residual_from)) : nullptr;
               ok = (entry || idx_of(l.input_from) >= 0) && (res == nullptr || idx_of(l.residual_from) >= 0) &&
-                   build_launch(ctx, w, li, in, res, s2_buf(pass, (int)q), 1, false, nullptr, pass ? pc->s2_edge[q] : pc->s2_stream[q],
+                   build_launch(ctx, w, li, in, res, sh_buf((int)g, pass, (int)q), 1, false, nullptr, pass ? P.edge[q] : P.stream[q],
                                 sc, sc >= 0 ? src[pass] : nullptr, &ov);
             }
           }
-          if (!ok) { caches.pop_back(); return AFRAME_ECUDA; }
-          pc->s2_layers = s2_list;
-          pc->s2_head = s2_head; pc->s2_tail = s2_tail;
+          P.layers = h.list;
+          P.T = h.T; P.C = h.C; P.C_in = h.C_in; P.head = h.head; P.tail = h.tail; P.shift = h.shift;
         }
+        if (!ok) { caches.pop_back(); return AFRAME_ECUDA; }
       }
       for (int i = 2; i < n; ++i) {
         const LayerDesc& l = w->layers[i];
@@ -744,42 +776,50 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         ctx->launches++;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_block (edge) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
       }
-      if (pc->s2_layers.empty()) {
+      if (pc->sh.empty()) {
         const int64_t n_s = nb * T1 * 8;
         s1_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
             reinterpret_cast<uint4*>(slot_ptr(2 * K + 1)), reinterpret_cast<const uint4*>(s1_stream_ptr(K)),
             reinterpret_cast<const uint4*>(s1_edge_ptr(K)), nb, T1, shift, 2 * K + 2, 2 * K + 1);
         AF_LAUNCH_CHECK(ctx);
-      } else {
-        // shared second stage: its layers read the first stage's stream and edge results directly (no stitch in between)
+      }
+      // shared later stages: each reads the previous stage's stream and edge results directly; only the last one is stitched
+      for (size_t g = 0; g < pc->sh.size(); ++g) {
+        TcPlanCache::SharedStagePlan& P = pc->sh[g];
         const int64_t n_short = up128(2 * nb * S2_PERIOD) / S2_PERIOD;
-        const int64_t n_g = n_short * (2 * S2_PERIOD) * 8;
-        s2_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
-            reinterpret_cast<uint4*>(s2_x_ptr()), reinterpret_cast<const uint4*>(s1_stream_ptr(K)),
-            reinterpret_cast<const uint4*>(s1_edge_ptr(K)), nb, n_short, T1, shift, 2 * K + 2, 2 * K + 1);
+        const int pieces_in = P.C_in / 8;
+        const int64_t n_g = n_short * (2 * S2_PERIOD) * pieces_in;
+        const int q_prev = g ? (int)pc->sh[g - 1].layers.size() - 1 : 0;
+        sh_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
+            reinterpret_cast<uint4*>(sh_x_ptr((int)g)),
+            reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 0, q_prev) : s1_stream_ptr(K)),
+            reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 1, q_prev) : s1_edge_ptr(K)), nb, n_short, 2 * P.T, pieces_in,
+            2 * P.shift, g ? S2_PERIOD : S1_PERIOD, g ? S2_ROWS : S1_ROWS, g ? pc->sh[g - 1].head : 2 * K + 2,
+            g ? pc->sh[g - 1].tail : 2 * K + 1);
         AF_LAUNCH_CHECK(ctx);
-        for (size_t q = 0; q < pc->s2_layers.size(); ++q)
+        for (size_t q = 0; q < P.layers.size(); ++q)
           for (int pass = 0; pass < 2; ++pass) {
-            TcLaunch& L2 = pass ? pc->s2_edge[q] : pc->s2_stream[q];
+            TcLaunch& L2 = pass ? P.edge[q] : P.stream[q];
             L2.p.reverse = 0;
             cudaError_t e = launch_conv(L2, ctx->stream);
             ctx->launches++; ++n_conv;
             if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (shared stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
           }
-        const int last = pc->s2_layers.back(), q_last = (int)pc->s2_layers.size() - 1;
-        const int T2 = w->layers[last].t_out, pieces = w->layers[last].c_out / 8;
-        const int64_t n_s = nb * T2 * pieces;
-        s2_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
-            reinterpret_cast<uint4*>(slot_ptr(last)), reinterpret_cast<const uint4*>(s2_buf(0, q_last)),
-            reinterpret_cast<const uint4*>(s2_buf(1, q_last)), nb, T2, pieces, shift / 2, pc->s2_head, pc->s2_tail);
-        AF_LAUNCH_CHECK(ctx);
+        if (g + 1 == pc->sh.size()) {
+          const int last = P.layers.back(), q_last = (int)P.layers.size() - 1, pieces = P.C / 8;
+          const int64_t n_s = nb * P.T * pieces;
+          s2_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
+              reinterpret_cast<uint4*>(slot_ptr(last)), reinterpret_cast<const uint4*>(sh_buf((int)g, 0, q_last)),
+              reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)), nb, P.T, pieces, P.shift, P.head, P.tail);
+          AF_LAUNCH_CHECK(ctx);
+        }
       }
     }
     for (int i = 2; i < n; ++i) {
       const LayerDesc& l = w->layers[i];
       struct Rec { aframe_ctx* c; std::vector<cudaEvent_t>& v; int i; ~Rec() { if (c->layer_ms) cudaEventRecord(v[i + 1], c->stream); } } rec{ctx, lev, i};
       if (i < 2 + 2 * pc->s1_blocks) continue;                 // ran in shared form above
-      if (!pc->s2_layers.empty() && i <= pc->s2_layers.back()) continue;
+      if (!pc->sh.empty() && i <= pc->sh.back().layers.back()) continue;
       if (l.kind == 0 && pc->fused_with[i] > i) continue;      // first conv of a fused block: runs with its partner
       if (pc->skip[i]) continue;                               // projection shortcut: runs inside the conv it feeds
       if (l.kind == 0) {
