@@ -418,6 +418,43 @@ __global__ void s2_stitch_kernel(uint4* __restrict__ out, const uint4* __restric
   out[i] = v;
 }
 
+// Fused-head partials for a stage that ran in shared form: the same numbers, summed in the same order, as the HEAD variant
+// of conv_tc_kernel emits from its epilogue (one warp = one 32-row slab of one window x one 64-channel chunk; lane = row),
+// read from the stage's stream or edge batch; head_finish_kernel then sums them as usual.  Nothing is stitched.
+__global__ void __launch_bounds__(256)
+sh_head_partial_kernel(const uint4* __restrict__ S, const uint4* __restrict__ Y, const float* __restrict__ head_w,
+                       float* __restrict__ head_part, int64_t nb, int T, int C, int64_t row_shift, int c_head, int c_tail) {
+  const int lane = threadIdx.x & 31;
+  const int chunks = C / 64, slabs = T / 32, pieces = C / 8;
+  const int64_t wi = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (wi >= nb * slabs * chunks) return;
+  const int c = (int)(wi % chunks);
+  const int slab = (int)((wi / chunks) % slabs);
+  const int64_t b = wi / ((int64_t)chunks * slabs);
+  const int t = slab * 32 + lane;
+  const uint4* rowp;
+  if (t < c_head) rowp = Y + ((2 * b) * S2_PERIOD + t) * pieces;
+  else if (t >= T - c_tail) rowp = Y + ((2 * b + 1) * S2_PERIOD + (t - (T - S2_ROWS))) * pieces;
+  else rowp = S + (b * row_shift + t) * pieces;
+  const float4* hw4 = reinterpret_cast<const float4*>(head_w + c * 64);
+  float hacc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int jj = 0; jj < 8; ++jj) {
+    const uint4 o = rowp[c * 8 + jj];
+    const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
+    const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
+    hacc[0] = fmaf(__uint_as_float(ow[0] << 16), hA.x, hacc[0]); hacc[1] = fmaf(__uint_as_float(ow[0] & 0xffff0000u), hA.y, hacc[1]);
+    hacc[2] = fmaf(__uint_as_float(ow[1] << 16), hA.z, hacc[2]); hacc[3] = fmaf(__uint_as_float(ow[1] & 0xffff0000u), hA.w, hacc[3]);
+    hacc[0] = fmaf(__uint_as_float(ow[2] << 16), hB.x, hacc[0]); hacc[1] = fmaf(__uint_as_float(ow[2] & 0xffff0000u), hB.y, hacc[1]);
+    hacc[2] = fmaf(__uint_as_float(ow[3] << 16), hB.z, hacc[2]); hacc[3] = fmaf(__uint_as_float(ow[3] & 0xffff0000u), hB.w, hacc[3]);
+  }
+  float sum = 0.f;
+  sum += (hacc[0] + hacc[1]) + (hacc[2] + hacc[3]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+  if (lane == 0) head_part[(b * slabs + slab) * chunks + c] = sum;
+}
+
 struct TcPlanCache {
   const aframe_weights* w = nullptr;
   void* base = nullptr;
@@ -437,6 +474,7 @@ struct TcPlanCache {
     int64_t shift = 0;                // rows between consecutive windows
   };
   std::vector<SharedStagePlan> sh;    // the stages after the first that run in shared form, in order
+  bool sh_head = false;               // the last shared stage feeds the fused head: sh_head_partial_kernel instead of a stitch
   std::vector<int> sc_of;             // per layer: the projection-shortcut conv that runs inside it (else -1)
   std::vector<char> skip;             // per layer: runs inside another launch
 };
@@ -562,15 +600,21 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     size_t stream_bytes = 0, edge_bytes = 0, x_bytes = 0, off = 0;
   };
   std::vector<SharedStage> shs;
+  bool sh_head_on = false;
   if (s1_on && env_int("AFRAME_SHARED_S2", 1) && env_int("AFRAME_FUSE_SC", 1)) {
     int i0 = 2 + 2 * s1_k, Tp = w->layers[1].t_out, hp = 2 * s1_k + 2, tp = 2 * s1_k + 1;
     int64_t shift_p = sB / 4;
-    const int max_stages = env_int("AFRAME_SHARED_STAGES", 2);
-    while ((int)shs.size() < max_stages && shift_p % 2 == 0) {
+    const int max_stages = env_int("AFRAME_SHARED_STAGES", 3);
+    while ((int)shs.size() < max_stages && shift_p % 2 == 0 && !sh_head_on) {
       SharedStage g;
       g.list = s2_chain_layers(w, i0);
       if (g.list.empty()) break;
-      if (fuse >= i0 && fuse <= g.list.back()) break;             // the stage that ends in the fused head stays per window
+      if (fuse >= i0 && fuse <= g.list.back()) {
+        // the stage that ends in the fused head: its last conv stores like any other and sh_head_partial_kernel emits the
+        // head's partial sums; needs whole 32-row slabs and the head as the only reader
+        if (fuse != g.list.back() || w->layers[fuse].t_out % 32 != 0) break;
+        sh_head_on = true;
+      }
       const int n2 = (int)g.list.size() - 1;
       g.i0 = i0; g.T = w->layers[i0].t_out; g.C = w->layers[i0].c_out; g.C_in = w->layers[i0].c_in;
       g.shift = shift_p / 2;
@@ -579,7 +623,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       const int src_rows = shs.empty() ? S1_ROWS : S2_ROWS;
       const bool fits = g.head + n2 <= S2_ROWS && g.tail + n2 + 1 <= S2_ROWS && g.T >= S2_ROWS && Tp >= 2 * S2_ROWS && Tp == 2 * g.T &&
                         hp <= src_rows - 2 && tp <= src_rows - 2 && g.C % 64 == 0 && g.C_in % 64 == 0;
-      if (!fits) break;
+      if (!fits) { sh_head_on = false; break; }
       g.rows_stream = up128((chunk - 1) * g.shift + g.T);
       g.rows_edge = up128(2 * chunk * S2_PERIOD);
       shs.push_back(g);
@@ -709,6 +753,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           P.T = h.T; P.C = h.C; P.C_in = h.C_in; P.head = h.head; P.tail = h.tail; P.shift = h.shift;
         }
         if (!ok) { caches.pop_back(); return AFRAME_ECUDA; }
+        pc->sh_head = sh_head_on;
       }
       for (int i = 2; i < n; ++i) {
         const LayerDesc& l = w->layers[i];
@@ -805,7 +850,14 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             ctx->launches++; ++n_conv;
             if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (shared stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
           }
-        if (g + 1 == pc->sh.size()) {
+        if (g + 1 == pc->sh.size() && pc->sh_head) {
+          const int q_last = (int)P.layers.size() - 1;
+          const int64_t n_warps = nb * (P.T / 32) * (P.C / 64);
+          sh_head_partial_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(
+              reinterpret_cast<const uint4*>(sh_buf((int)g, 0, q_last)), reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)),
+              w->d_head_w, head_part, nb, P.T, P.C, P.shift, P.head, P.tail);
+          AF_LAUNCH_CHECK(ctx);
+        } else if (g + 1 == pc->sh.size()) {
           const int last = P.layers.back(), q_last = (int)P.layers.size() - 1, pieces = P.C / 8;
           const int64_t n_s = nb * P.T * pieces;
           s2_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
