@@ -372,8 +372,8 @@ def run_ours(args):
     win_rank = args.steps * N_SLIDES * n_win
     conv_tflops = 2.0 * MMAC_CONV * win_rank / (conv_ms * 1e-3) / 1e12 if conv_ms > 0 else 0.0
     # Windows 128 samples apart share every activation row that is out of reach of their own zero padding, and the library
-    # computes stages 1-3 that way (shared stages): per 4096-window chunk a stage runs over the chunk's
-    # stream (rows padded to whole tiles) plus two short edge windows per window (18 rows in stage 1, 32 in stages 2-3).
+    # computes all four stages that way (shared stages): per 4096-window chunk a stage runs over the chunk's
+    # stream (rows padded to whole tiles) plus two short edge windows per window (18 rows in stage 1, 32 in stages 2-4).
     # executed = the MMACs the tensor cores really perform per window; MMAC_CONV is the method's (algorithmic) figure.
     def _up128(v):
         return (v + 127) // 128 * 128
@@ -381,9 +381,10 @@ def run_ours(args):
     _f1 = (((_nb - 1) * 32 + 768) / _nb + 36) / 768
     _f2 = (_up128((_nb - 1) * 16 + 384) / _nb + 64) / 384
     _f3 = (_up128((_nb - 1) * 8 + 192) / _nb + 64) / 192
+    _f4 = (_up128((_nb - 1) * 4 + 96) / _nb + 64) / 96
     shared_on = all(os.environ.get(k, "1") != "0" for k in ("AFRAME_SHARED_STEM", "AFRAME_SHARED_S1", "AFRAME_SHARED_S2")) \
-        and os.environ.get("AFRAME_SHARED_STAGES", "2") == "2" and args.batch == 4096
-    mmac_exec = MMAC_CONV - 56.6e6 * (1 - _f1) - 144.7e6 * (1 - _f2) - 440.4e6 * (1 - _f3) if shared_on else MMAC_CONV
+        and os.environ.get("AFRAME_SHARED_STAGES", "3") == "3" and args.batch == 4096
+    mmac_exec = (MMAC_CONV - 56.6e6 * (1 - _f1) - 144.7e6 * (1 - _f2) - 440.4e6 * (1 - _f3) - 427.8e6 * (1 - _f4)) if shared_on else MMAC_CONV
     exec_tflops = conv_tflops * mmac_exec / MMAC_CONV
     out = {
         "metric": "analysed strain-seconds per second (whitened + scored, all timeslides)",
@@ -411,7 +412,7 @@ def run_ours(args):
                      "algorithmic": "achieved = EXECUTED tensor FLOPs (2 x executed MMAC per window x windows scored) over the "
                                     "summed CUDA-event time of the conv launches on the library's stream.  The method's work is "
                                     "2 x 1069.5 MMAC per window (algorithmic_tflops counts that); overlapping windows share the "
-                                    "interior rows of stages 1-3, which are computed once per stream plus two short edge windows "
+                                    "interior rows of every stage, which are computed once per stream plus two short edge windows "
                                     "per window, so only executed_frac_of_algorithmic of those FLOPs are performed"},
         "stages": {k: {"ms": v[0], "launches": v[1], "share": v[0] / ms_total} for k, v in stages.items()},
     }
