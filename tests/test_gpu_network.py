@@ -226,3 +226,24 @@ def test_live_group_norm_bf16_fallback_statistics_path(af):
     ctx = af.Context(kernel_len=2560, precision=af.BF16)
     got = ctx.forward(ctx.load_weights(blob), torch.from_numpy(wins).cuda()).cpu().numpy()
     assert rel_err(got, ref) <= 2e-2
+
+
+@pytest.mark.parametrize("stride,n_win", [(128, 2), (128, 3), (128, 37), (128, 301), (512, 5), (512, 64), (32, 150), (64, 33),
+                                          (4, 40), (100, 21), (8, 500)])
+def test_shared_stages_equal_the_per_window_path_bit_for_bit(af, config1, stride, n_win):
+    """Overlapping in-place windows run in shared form (each stage once over the stream + two short edge windows per window,
+    DESIGN.md section 5) when their spacing allows it; explicit [B][2][K] windows always take the per-window path.  Same
+    kernels, same per-row arithmetic: the scores must be identical bit for bit, for chunk sizes 2, 3, odd, ragged, and for
+    spacings that allow all stages (128, 512, 64, 32), only some (8), none but the stem (4) or nothing at all (100)."""
+    rng = np.random.default_rng(stride * 1000 + n_win)
+    white = torch.from_numpy(rng.standard_normal((2, (n_win - 1) * stride + 3072 + 2048)).astype(np.float32)).cuda().bfloat16()
+    import math
+    unit = math.lcm(2048, stride)                                # the configuration wants PSD lengths in whole strides and hops
+    ctx = af.Context(precision=af.BF16, stride=stride, psd_update=unit * -(-16384 // unit), psd_len=unit * -(-131072 // unit))
+    w = ctx.load_weights(config1["blob"])
+    shared = ctx.forward_strided(w, white.contiguous(), 0, n_win, chan_shift=[0, 2048])
+    wins = torch.stack([torch.stack([white[0, i * stride: i * stride + 3072], white[1, 2048 + i * stride: 2048 + i * stride + 3072]])
+                        for i in range(n_win)]).float().contiguous()
+    ref = ctx.forward(w, wins)
+    assert bool(torch.isfinite(shared).all())
+    assert torch.equal(shared, ref)
