@@ -98,7 +98,7 @@ aframe_status af_tc_check(aframe_ctx* ctx, aframe_weights* w) {
 // K blocks on its own input sc_in (res must then be null)
 // ov != null (shared stages): the launch runs the layer on ONE long window of ov->t_out output rows (a stream, or a batch of
 // short windows with zeroed separator rows) instead of nb windows of the table's length
-struct TcShapeOverride { int t_out; int zero_period, zero_valid; };
+struct TcShapeOverride { int t_out; int zero_period, zero_valid, zero_origin; };
 static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const __nv_bfloat16* in,
                          const __nv_bfloat16* res, __nv_bfloat16* out, int64_t nb, bool head, float* head_part,
                          TcLaunch& L, int sc = -1, const __nv_bfloat16* sc_in = nullptr, const TcShapeOverride* ov = nullptr) {
@@ -149,7 +149,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.bias = sc >= 0 ? w->d_bias_sc[li] : w->d_bias[li];
   p.sc_kblocks = sc >= 0 ? w->layers[sc].c_in / 64 : 0;
   p.gn_part = nullptr; p.gn_unit = 64; p.out_f16 = 0;
-  p.zero_period = ov ? ov->zero_period : 0; p.zero_valid = ov ? ov->zero_valid : 0;
+  p.zero_period = ov ? ov->zero_period : 0; p.zero_valid = ov ? ov->zero_valid : 0; p.zero_origin = ov ? ov->zero_origin : 0;
   p.taps = l.k; p.pad = l.pad; p.P = P;
   for (int d = 0; d < 3; ++d) {
     const int sft = d - l.pad;
@@ -384,15 +384,23 @@ constexpr int S2_PERIOD = 32;               // + 2 separator rows: four short wi
 // else from the previous stage's stream; the other rows are zero.
 __global__ void sh_gather_kernel(uint4* __restrict__ X, const uint4* __restrict__ S, const uint4* __restrict__ Y, int64_t nb,
                                  int64_t n_short /* short windows incl. padding */, int Tp, int pieces, int64_t row_shift,
-                                 int src_period, int src_rows, int c_head, int c_tail) {
+                                 int src_period, int src_rows, int c_head, int c_tail, int64_t copy_rows, int64_t valid_rows) {
+  // X = [copy_rows rows: the previous stage's stream (its first valid_rows rows; the last 4 rows zero: they are the first short
+  //      window's padding at this resolution) | n_short short windows of 2 S2_PERIOD rows]
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_short * (2 * S2_PERIOD) * pieces) return;
+  if (i >= (copy_rows + n_short * (2 * S2_PERIOD)) * pieces) return;
   const int j = (int)(i % pieces);
-  const int64_t mr = i / pieces;
+  const int64_t row = i / pieces;
+  uint4 v = make_uint4(0u, 0u, 0u, 0u);
+  if (row < copy_rows) {
+    if (row < valid_rows && row < copy_rows - 4) v = S[row * pieces + j];
+    X[i] = v;
+    return;
+  }
+  const int64_t mr = row - copy_rows;
   const int r = (int)(mr % (2 * S2_PERIOD));
   const int64_t m = mr / (2 * S2_PERIOD), b = m >> 1;
   const bool tail = (m & 1) != 0;
-  uint4 v = make_uint4(0u, 0u, 0u, 0u);
   if (r < 2 * S2_ROWS && b < nb) {
     const int t = tail ? Tp - 2 * S2_ROWS + r : r;
     if (!tail && t < c_head) v = Y[(m * src_period + t) * pieces + j];
@@ -632,19 +640,17 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   }
   const bool s2_on = !shs.empty();
   const int64_t s1_rows = (chunk - 1) * (sB / 4) + w->layers[1].t_out;
-  const size_t s1_stream_bytes = s1_on ? (((size_t)(s2_on && 2 * shs[0].rows_stream > s1_rows ? 2 * shs[0].rows_stream : s1_rows) * 128 + 1023) & ~(size_t)1023) : 0;
+  const size_t s1_stream_bytes = s1_on ? (((size_t)s1_rows * 128 + 1023) & ~(size_t)1023) : 0;
   const size_t s1_edge_bytes = s1_on ? (((size_t)2 * chunk * S1_PERIOD * 128 + 1023) & ~(size_t)1023) : 0;
   const size_t s1_bytes = (size_t)s1_k * s1_stream_bytes + (size_t)(s1_k + 1) * s1_edge_bytes;
   size_t s2_bytes = 0;
   for (size_t g = 0; g < shs.size(); ++g) {
     SharedStage& h = shs[g];
-    // a stage's stream is also read by the next stage's entry conv, over twice that stage's (padded) row count
-    const int64_t alloc_rows = g + 1 < shs.size() && 2 * shs[g + 1].rows_stream > h.rows_stream ? 2 * shs[g + 1].rows_stream : h.rows_stream;
-    h.stream_bytes = ((size_t)alloc_rows * h.C * 2 + 1023) & ~(size_t)1023;
-    h.edge_bytes = ((size_t)h.rows_edge * h.C * 2 + 1023) & ~(size_t)1023;
-    h.x_bytes = ((size_t)2 * h.rows_edge * h.C_in * 2 + 1023) & ~(size_t)1023;
+    // one tensor per layer: [stream rows | edge-batch rows], and the entry conv's input at twice the rows
+    h.stream_bytes = ((size_t)(h.rows_stream + h.rows_edge) * h.C * 2 + 1023) & ~(size_t)1023;
+    h.x_bytes = ((size_t)2 * (h.rows_stream + h.rows_edge) * h.C_in * 2 + 1023) & ~(size_t)1023;
     h.off = s2_bytes;
-    s2_bytes += h.x_bytes + h.list.size() * (h.stream_bytes + h.edge_bytes);
+    s2_bytes += h.x_bytes + h.list.size() * h.stream_bytes;
   }
   aframe_status st = af_ws_reserve(ctx, ctx->ws_act, slot_bytes * plan.n_slots + part_bytes + s1_bytes + s2_bytes);
   if (st != AFRAME_OK) return st;
@@ -653,9 +659,11 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   auto s1_stream_ptr = [&](int k) { return reinterpret_cast<__nv_bfloat16*>(s1_base + (size_t)(k - 1) * s1_stream_bytes); };             // S_k, k = 1..K
   char* s2_base = s1_base + s1_bytes;
   auto sh_x_ptr = [&](int g) { return reinterpret_cast<__nv_bfloat16*>(s2_base + shs[g].off); };
-  auto sh_buf = [&](int g, int pass, int idx) {    // pass 0: stream, 1: edge batch; idx: position in the stage's list
+  int64_t cur_nb = chunk;                          // windows of the chunk being planned / launched (row counts depend on it)
+  auto sh_rows_stream = [&](int g) { return up128((cur_nb - 1) * shs[g].shift + shs[g].T); };
+  auto sh_buf = [&](int g, int pass, int idx) {    // pass 0: the tensor (stream part first), 1: its edge-batch part; idx: position in the list
     const SharedStage& h = shs[g];
-    return reinterpret_cast<__nv_bfloat16*>(s2_base + h.off + h.x_bytes + (size_t)idx * (h.stream_bytes + h.edge_bytes) + (pass ? h.stream_bytes : 0));
+    return reinterpret_cast<__nv_bfloat16*>(s2_base + h.off + h.x_bytes + (size_t)idx * h.stream_bytes) + (pass ? sh_rows_stream(g) * h.C : 0);
   };
   auto s1_edge_ptr = [&](int k) { return reinterpret_cast<__nv_bfloat16*>(s1_base + (size_t)s1_k * s1_stream_bytes + (size_t)k * s1_edge_bytes); };  // X (k = 0), Y_k
   float* head_part = reinterpret_cast<float*>(base + slot_bytes * plan.n_slots);
@@ -665,6 +673,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
 
   for (int64_t b0 = 0; b0 < B; b0 += chunk) {
     const int64_t nb = (B - b0 < chunk) ? (B - b0) : chunk;
+    cur_nb = nb;
     TcPlanCache* pc = nullptr;
     for (auto& c : caches)
       if (c.w == w && c.base == base && c.nb == nb && c.slot_bytes == slot_bytes && c.win_stride == sB) { pc = &c; break; }
@@ -730,24 +739,22 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         for (size_t g = 0; ok && g < shs.size(); ++g) {
           const SharedStage& h = shs[g];
           TcPlanCache::SharedStagePlan& P = pc->sh[g];
-          const int64_t rows[2] = {up128((nb - 1) * h.shift + h.T), up128(2 * nb * S2_PERIOD)};
-          const __nv_bfloat16* src[2] = {g == 0 ? s1_stream_ptr(s1_k) : sh_buf((int)g - 1, 0, (int)shs[g - 1].list.size() - 1), sh_x_ptr((int)g)};
+          const int64_t rows_s = up128((nb - 1) * h.shift + h.T), rows_tot = rows_s + up128(2 * nb * S2_PERIOD);
           auto idx_of = [&](int layer) { for (size_t q = 0; q < h.list.size(); ++q) if (h.list[q] == layer) return (int)q; return -1; };
           P.stream.resize(h.list.size());
-          P.edge.resize(h.list.size());
+          ok = rows_tot < (1ll << 30);
           for (size_t q = 0; ok && q < h.list.size(); ++q) {
+            // one launch per layer over [stream | short windows]: the mask starts at the short windows (and their leading padding)
             const int li = h.list[q];
             const LayerDesc& l = w->layers[li];
-            for (int pass = 0; ok && pass < 2; ++pass) {
-              const TcShapeOverride ov{(int)rows[pass], pass ? S2_PERIOD : 0, pass ? S2_ROWS : 0};
-              const bool entry = li == h.i0;
-              const int sc = pc->sc_of[li];
-              const __nv_bfloat16* in = entry ? src[pass] : sh_buf((int)g, pass, idx_of(l.input_from));
-              const __nv_bfloat16* res = (l.residual_from >= 0 && sc < 0) ? sh_buf((int)g, pass, idx_of(l.residual_from)) : nullptr;
-              ok = (entry || idx_of(l.input_from) >= 0) && (res == nullptr || idx_of(l.residual_from) >= 0) &&
-                   build_launch(ctx, w, li, in, res, sh_buf((int)g, pass, (int)q), 1, false, nullptr, pass ? P.edge[q] : P.stream[q],
-                                sc, sc >= 0 ? src[pass] : nullptr, &ov);
-            }
+            const TcShapeOverride ov{(int)rows_tot, S2_PERIOD, S2_ROWS, (int)rows_s};
+            const bool entry = li == h.i0;
+            const int sc = pc->sc_of[li];
+            const __nv_bfloat16* in = entry ? sh_x_ptr((int)g) : sh_buf((int)g, 0, idx_of(l.input_from));
+            const __nv_bfloat16* res = (l.residual_from >= 0 && sc < 0) ? sh_buf((int)g, 0, idx_of(l.residual_from)) : nullptr;
+            ok = (entry || idx_of(l.input_from) >= 0) && (res == nullptr || idx_of(l.residual_from) >= 0) &&
+                 build_launch(ctx, w, li, in, res, sh_buf((int)g, 0, (int)q), 1, false, nullptr, P.stream[q], sc,
+                              sc >= 0 ? sh_x_ptr((int)g) : nullptr, &ov);
           }
           P.layers = h.list;
           P.T = h.T; P.C = h.C; P.C_in = h.C_in; P.head = h.head; P.tail = h.tail; P.shift = h.shift;
@@ -833,23 +840,23 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         TcPlanCache::SharedStagePlan& P = pc->sh[g];
         const int64_t n_short = up128(2 * nb * S2_PERIOD) / S2_PERIOD;
         const int pieces_in = P.C_in / 8;
-        const int64_t n_g = n_short * (2 * S2_PERIOD) * pieces_in;
+        const int64_t copy_rows = 2 * sh_rows_stream((int)g);
+        const int64_t n_g = (copy_rows + n_short * (2 * S2_PERIOD)) * pieces_in;
         const int q_prev = g ? (int)pc->sh[g - 1].layers.size() - 1 : 0;
         sh_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
             reinterpret_cast<uint4*>(sh_x_ptr((int)g)),
             reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 0, q_prev) : s1_stream_ptr(K)),
             reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 1, q_prev) : s1_edge_ptr(K)), nb, n_short, 2 * P.T, pieces_in,
             2 * P.shift, g ? S2_PERIOD : S1_PERIOD, g ? S2_ROWS : S1_ROWS, g ? pc->sh[g - 1].head : 2 * K + 2,
-            g ? pc->sh[g - 1].tail : 2 * K + 1);
+            g ? pc->sh[g - 1].tail : 2 * K + 1, copy_rows, g ? sh_rows_stream((int)g - 1) : (nb - 1) * shift + T1);
         AF_LAUNCH_CHECK(ctx);
-        for (size_t q = 0; q < P.layers.size(); ++q)
-          for (int pass = 0; pass < 2; ++pass) {
-            TcLaunch& L2 = pass ? P.edge[q] : P.stream[q];
-            L2.p.reverse = 0;
-            cudaError_t e = launch_conv(L2, ctx->stream);
-            ctx->launches++; ++n_conv;
-            if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (shared stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
-          }
+        for (size_t q = 0; q < P.layers.size(); ++q) {
+          TcLaunch& L2 = P.stream[q];
+          L2.p.reverse = 0;
+          cudaError_t e = launch_conv(L2, ctx->stream);
+          ctx->launches++; ++n_conv;
+          if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (shared stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
+        }
         if (g + 1 == pc->sh.size() && pc->sh_head) {
           const int q_last = (int)P.layers.size() - 1;
           const int64_t n_warps = nb * (P.T / 32) * (P.C / 64);

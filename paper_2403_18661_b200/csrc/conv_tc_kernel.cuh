@@ -72,6 +72,8 @@ struct TcConvParams {
   // shared stages (conv_tc.cu): the launch covers a batch of short windows stored back to back; output rows t with
   // t % zero_period >= zero_valid are separators and are stored as zero (they are the short windows' zero padding)
   int zero_period, zero_valid;   // 0 = off
+  int zero_origin;               // the batch of short windows starts at this row (rows before it, a stream, are not masked,
+                                 // except the two rows just before it, which are the first short window's padding)
   int out_f16;               // store the (pre-norm) output as fp16 (saturating) instead of bf16: z = mu + O(sigma) loses
                              // |mu| / sigma times more to an 8-bit mantissa than the normalised value does
   int w_bytes;               // resident weight region (0 unless HALO)
@@ -532,7 +534,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         unsigned char* rowp = gen_base + (sbuf - base) + row * 128;
         // straight-line code per variant (no run-time branches inside the unrolled loop, so the 8 pieces interleave)
         const __nv_bfloat162 lo2 = __float2bfloat162_rn(p.relu ? 0.f : -INFINITY);
-        const bool zero_row = p.zero_period > 0 && ((t0 + row % p.T_box) % p.zero_period) >= p.zero_valid;
+        const int t_row = t0 + row % p.T_box;
+        const bool zero_row = p.zero_period > 0 && t_row >= p.zero_origin - 2 &&
+                              ((t_row - p.zero_origin + p.zero_period) % p.zero_period) >= p.zero_valid;
         if (p.has_res) tc_epilogue_math<true, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row);
         else if (!HEAD && p.out_f16) tc_epilogue_math<false, false, true>(v, bias4, hw4, rowp, row, lo2, head_acc);
         else tc_epilogue_math<false, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row);
