@@ -375,8 +375,8 @@ __global__ void s1_stitch_kernel(uint4* __restrict__ out, const uint4* __restric
 // half the row spacing.  Its layers run unchanged (conv_tc_kernel) on (1) the stream, as one long window, and (2) a batch
 // of two short windows per window -- the first / last S2_ROWS output rows, i.e. 2 S2_ROWS input rows -- separated by zeroed
 // rows (TcConvParams::zero_period), then s2_stitch_kernel writes the per-window tensor the next stage reads.
-constexpr int S2_ROWS = 30;                 // output rows of a short window at the stage's resolution
-constexpr int S2_PERIOD = 32;               // + 2 separator rows: four short windows per 128-row tile
+// A stage's short windows hold `rows` output rows (the smallest count that keeps every edge row out of reach of the short
+// window's artificial end: edge rows + convs after the entry conv) and repeat every `period` = rows + 2 rows (2 separators).
 
 // Input of a stage's short windows at the previous stage's resolution: [short windows][2 S2_PERIOD rows][pieces * 8 ch];
 // local row r < 2 S2_ROWS is window row r (head) or Tp - 2 S2_ROWS + r (tail), taken from the previous stage's edge batch
@@ -384,11 +384,12 @@ constexpr int S2_PERIOD = 32;               // + 2 separator rows: four short wi
 // else from the previous stage's stream; the other rows are zero.
 __global__ void sh_gather_kernel(uint4* __restrict__ X, const uint4* __restrict__ S, const uint4* __restrict__ Y, int64_t nb,
                                  int64_t n_short /* short windows incl. padding */, int Tp, int pieces, int64_t row_shift,
-                                 int src_period, int src_rows, int c_head, int c_tail, int64_t copy_rows, int64_t valid_rows) {
+                                 int src_period, int src_rows, int c_head, int c_tail, int64_t copy_rows, int64_t valid_rows,
+                                 int rows, int period, int64_t edge_rows_in /* rows of the short-window part of X */) {
   // X = [copy_rows rows: the previous stage's stream (its first valid_rows rows; the last 4 rows zero: they are the first short
   //      window's padding at this resolution) | n_short short windows of 2 S2_PERIOD rows]
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= (copy_rows + n_short * (2 * S2_PERIOD)) * pieces) return;
+  if (i >= (copy_rows + edge_rows_in) * pieces) return;
   const int j = (int)(i % pieces);
   const int64_t row = i / pieces;
   uint4 v = make_uint4(0u, 0u, 0u, 0u);
@@ -398,11 +399,11 @@ __global__ void sh_gather_kernel(uint4* __restrict__ X, const uint4* __restrict_
     return;
   }
   const int64_t mr = row - copy_rows;
-  const int r = (int)(mr % (2 * S2_PERIOD));
-  const int64_t m = mr / (2 * S2_PERIOD), b = m >> 1;
+  const int r = (int)(mr % (2 * period));
+  const int64_t m = mr / (2 * period), b = m >> 1;
   const bool tail = (m & 1) != 0;
-  if (r < 2 * S2_ROWS && b < nb) {
-    const int t = tail ? Tp - 2 * S2_ROWS + r : r;
+  if (r < 2 * rows && b < nb && m < n_short) {
+    const int t = tail ? Tp - 2 * rows + r : r;
     if (!tail && t < c_head) v = Y[(m * src_period + t) * pieces + j];
     else if (tail && t >= Tp - c_tail) v = Y[(m * src_period + (t - (Tp - src_rows))) * pieces + j];
     else v = S[(b * row_shift + t) * pieces + j];
@@ -412,7 +413,7 @@ __global__ void sh_gather_kernel(uint4* __restrict__ X, const uint4* __restrict_
 
 // out[b][t][C]: edge result where t is an edge row of window b (t < c_head or t >= T2 - c_tail), else the stream row
 __global__ void s2_stitch_kernel(uint4* __restrict__ out, const uint4* __restrict__ S, const uint4* __restrict__ Y, int64_t nb,
-                                 int T2, int pieces /* C / 8 */, int64_t row_shift, int c_head, int c_tail) {
+                                 int T2, int pieces /* C / 8 */, int64_t row_shift, int c_head, int c_tail, int rows, int period) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= nb * T2 * pieces) return;
   const int j = (int)(i % pieces);
@@ -420,8 +421,8 @@ __global__ void s2_stitch_kernel(uint4* __restrict__ out, const uint4* __restric
   const int t = (int)(bt % T2);
   const int64_t b = bt / T2;
   uint4 v;
-  if (t < c_head) v = Y[((2 * b) * S2_PERIOD + t) * pieces + j];
-  else if (t >= T2 - c_tail) v = Y[((2 * b + 1) * S2_PERIOD + (t - (T2 - S2_ROWS))) * pieces + j];
+  if (t < c_head) v = Y[((2 * b) * period + t) * pieces + j];
+  else if (t >= T2 - c_tail) v = Y[((2 * b + 1) * period + (t - (T2 - rows))) * pieces + j];
   else v = S[(b * row_shift + t) * pieces + j];
   out[i] = v;
 }
@@ -431,7 +432,8 @@ __global__ void s2_stitch_kernel(uint4* __restrict__ out, const uint4* __restric
 // read from the stage's stream or edge batch; head_finish_kernel then sums them as usual.  Nothing is stitched.
 __global__ void __launch_bounds__(256)
 sh_head_partial_kernel(const uint4* __restrict__ S, const uint4* __restrict__ Y, const float* __restrict__ head_w,
-                       float* __restrict__ head_part, int64_t nb, int T, int C, int64_t row_shift, int c_head, int c_tail) {
+                       float* __restrict__ head_part, int64_t nb, int T, int C, int64_t row_shift, int c_head, int c_tail,
+                       int rows, int period) {
   const int lane = threadIdx.x & 31;
   const int chunks = C / 64, slabs = T / 32, pieces = C / 8;
   const int64_t wi = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -441,8 +443,8 @@ sh_head_partial_kernel(const uint4* __restrict__ S, const uint4* __restrict__ Y,
   const int64_t b = wi / ((int64_t)chunks * slabs);
   const int t = slab * 32 + lane;
   const uint4* rowp;
-  if (t < c_head) rowp = Y + ((2 * b) * S2_PERIOD + t) * pieces;
-  else if (t >= T - c_tail) rowp = Y + ((2 * b + 1) * S2_PERIOD + (t - (T - S2_ROWS))) * pieces;
+  if (t < c_head) rowp = Y + ((2 * b) * period + t) * pieces;
+  else if (t >= T - c_tail) rowp = Y + ((2 * b + 1) * period + (t - (T - rows))) * pieces;
   else rowp = S + (b * row_shift + t) * pieces;
   const float4* hw4 = reinterpret_cast<const float4*>(head_w + c * 64);
   float hacc[4] = {0.f, 0.f, 0.f, 0.f};
@@ -479,6 +481,7 @@ struct TcPlanCache {
     std::vector<int> layers;          // these layers (entry conv, then the stride-1 convs) run in shared form
     std::vector<TcLaunch> stream, edge;   // parallel to layers
     int T = 0, C = 0, C_in = 0, head = 0, tail = 0;   // output rows / channels, input channels, edge rows per window
+    int rows = 0, period = 0;         // short window: data rows, data + separator rows
     int64_t shift = 0;                // rows between consecutive windows
   };
   std::vector<SharedStagePlan> sh;    // the stages after the first that run in shared form, in order
@@ -603,6 +606,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   struct SharedStage {
     std::vector<int> list;            // layers that launch, entry conv first
     int i0 = 0, T = 0, C = 0, C_in = 0, head = 0, tail = 0;
+    int rows = 0, period = 0;         // short window: data rows, data + 2 separator rows
     int64_t shift = 0;                // rows between consecutive windows at this stage's resolution
     int64_t rows_stream = 0, rows_edge = 0;
     size_t stream_bytes = 0, edge_bytes = 0, x_bytes = 0, off = 0;
@@ -628,12 +632,15 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       g.shift = shift_p / 2;
       g.head = hp / 2 + 1 + n2;                                   // rows within reach of the window's zero padding ...
       g.tail = g.T - (Tp - tp) / 2 + n2;                          // ... at the start and at the end of the stage's output
-      const int src_rows = shs.empty() ? S1_ROWS : S2_ROWS;
-      const bool fits = g.head + n2 <= S2_ROWS && g.tail + n2 + 1 <= S2_ROWS && g.T >= S2_ROWS && Tp >= 2 * S2_ROWS && Tp == 2 * g.T &&
-                        hp <= src_rows - 2 && tp <= src_rows - 2 && g.C % 64 == 0 && g.C_in % 64 == 0;
+      const int src_rows = shs.empty() ? S1_ROWS : shs.back().rows;
+      g.rows = g.head + n2 > g.tail + n2 + 1 ? g.head + n2 : g.tail + n2 + 1;
+      if (env_int("AFRAME_SHARED_ROWS", 0) > g.rows) g.rows = env_int("AFRAME_SHARED_ROWS", 0);    // (experiments: longer short windows)
+      g.period = g.rows + 2;
+      const bool fits = g.T >= g.rows && Tp >= 2 * g.rows && Tp == 2 * g.T && hp <= src_rows - 2 && tp <= src_rows - 2 &&
+                        g.C % 64 == 0 && g.C_in % 64 == 0;
       if (!fits) { sh_head_on = false; break; }
       g.rows_stream = up128((chunk - 1) * g.shift + g.T);
-      g.rows_edge = up128(2 * chunk * S2_PERIOD);
+      g.rows_edge = up128(2 * chunk * g.period);
       shs.push_back(g);
       i0 = g.list.back() + 1; Tp = g.T; hp = g.head; tp = g.tail; shift_p = g.shift;
     }
@@ -739,7 +746,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         for (size_t g = 0; ok && g < shs.size(); ++g) {
           const SharedStage& h = shs[g];
           TcPlanCache::SharedStagePlan& P = pc->sh[g];
-          const int64_t rows_s = up128((nb - 1) * h.shift + h.T), rows_tot = rows_s + up128(2 * nb * S2_PERIOD);
+          const int64_t rows_s = up128((nb - 1) * h.shift + h.T), rows_tot = rows_s + up128(2 * nb * h.period);
           auto idx_of = [&](int layer) { for (size_t q = 0; q < h.list.size(); ++q) if (h.list[q] == layer) return (int)q; return -1; };
           P.stream.resize(h.list.size());
           ok = rows_tot < (1ll << 30);
@@ -747,7 +754,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             // one launch per layer over [stream | short windows]: the mask starts at the short windows (and their leading padding)
             const int li = h.list[q];
             const LayerDesc& l = w->layers[li];
-            const TcShapeOverride ov{(int)rows_tot, S2_PERIOD, S2_ROWS, (int)rows_s};
+            const TcShapeOverride ov{(int)rows_tot, h.period, h.rows, (int)rows_s};
             const bool entry = li == h.i0;
             const int sc = pc->sc_of[li];
             const __nv_bfloat16* in = entry ? sh_x_ptr((int)g) : sh_buf((int)g, 0, idx_of(l.input_from));
@@ -757,7 +764,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
                               sc >= 0 ? sh_x_ptr((int)g) : nullptr, &ov);
           }
           P.layers = h.list;
-          P.T = h.T; P.C = h.C; P.C_in = h.C_in; P.head = h.head; P.tail = h.tail; P.shift = h.shift;
+          P.T = h.T; P.C = h.C; P.C_in = h.C_in; P.head = h.head; P.tail = h.tail; P.shift = h.shift; P.rows = h.rows; P.period = h.period;
         }
         if (!ok) { caches.pop_back(); return AFRAME_ECUDA; }
         pc->sh_head = sh_head_on;
@@ -838,17 +845,18 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       // shared later stages: each reads the previous stage's stream and edge results directly; only the last one is stitched
       for (size_t g = 0; g < pc->sh.size(); ++g) {
         TcPlanCache::SharedStagePlan& P = pc->sh[g];
-        const int64_t n_short = up128(2 * nb * S2_PERIOD) / S2_PERIOD;
+        const int64_t n_short = 2 * nb, edge_rows_in = 2 * up128(2 * nb * P.period);
         const int pieces_in = P.C_in / 8;
         const int64_t copy_rows = 2 * sh_rows_stream((int)g);
-        const int64_t n_g = (copy_rows + n_short * (2 * S2_PERIOD)) * pieces_in;
+        const int64_t n_g = (copy_rows + edge_rows_in) * pieces_in;
         const int q_prev = g ? (int)pc->sh[g - 1].layers.size() - 1 : 0;
         sh_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
             reinterpret_cast<uint4*>(sh_x_ptr((int)g)),
             reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 0, q_prev) : s1_stream_ptr(K)),
             reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 1, q_prev) : s1_edge_ptr(K)), nb, n_short, 2 * P.T, pieces_in,
-            2 * P.shift, g ? S2_PERIOD : S1_PERIOD, g ? S2_ROWS : S1_ROWS, g ? pc->sh[g - 1].head : 2 * K + 2,
-            g ? pc->sh[g - 1].tail : 2 * K + 1, copy_rows, g ? sh_rows_stream((int)g - 1) : (nb - 1) * shift + T1);
+            2 * P.shift, g ? pc->sh[g - 1].period : S1_PERIOD, g ? pc->sh[g - 1].rows : S1_ROWS, g ? pc->sh[g - 1].head : 2 * K + 2,
+            g ? pc->sh[g - 1].tail : 2 * K + 1, copy_rows, g ? sh_rows_stream((int)g - 1) : (nb - 1) * shift + T1, P.rows, P.period,
+            edge_rows_in);
         AF_LAUNCH_CHECK(ctx);
         for (size_t q = 0; q < P.layers.size(); ++q) {
           TcLaunch& L2 = P.stream[q];
@@ -862,14 +870,14 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           const int64_t n_warps = nb * (P.T / 32) * (P.C / 64);
           sh_head_partial_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(
               reinterpret_cast<const uint4*>(sh_buf((int)g, 0, q_last)), reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)),
-              w->d_head_w, head_part, nb, P.T, P.C, P.shift, P.head, P.tail);
+              w->d_head_w, head_part, nb, P.T, P.C, P.shift, P.head, P.tail, P.rows, P.period);
           AF_LAUNCH_CHECK(ctx);
         } else if (g + 1 == pc->sh.size()) {
           const int last = P.layers.back(), q_last = (int)P.layers.size() - 1, pieces = P.C / 8;
           const int64_t n_s = nb * P.T * pieces;
           s2_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
               reinterpret_cast<uint4*>(slot_ptr(last)), reinterpret_cast<const uint4*>(sh_buf((int)g, 0, q_last)),
-              reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)), nb, P.T, pieces, P.shift, P.head, P.tail);
+              reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)), nb, P.T, pieces, P.shift, P.head, P.tail, P.rows, P.period);
           AF_LAUNCH_CHECK(ctx);
         }
       }
