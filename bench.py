@@ -324,6 +324,7 @@ def run_ours(args):
             step_dev(j)
         barrier()
         launches0 = ctx.launch_count()
+        macs0 = ctx.tensor_macs()
         ctx.profile(True)
         sampler = ClockSampler(local_rank)
         sampler.start()
@@ -338,6 +339,7 @@ def run_ours(args):
         stages = ctx.profile_read()
         ctx.profile(False)
         launches = ctx.launch_count() - launches0
+        macs_exec = ctx.tensor_macs() - macs0
         assert torch.isfinite(scores_dev).all()
 
         # ---- end to end: pinned host strain in, scores out, copies inside the timed region -------------
@@ -373,18 +375,10 @@ def run_ours(args):
     conv_tflops = 2.0 * MMAC_CONV * win_rank / (conv_ms * 1e-3) / 1e12 if conv_ms > 0 else 0.0
     # Windows 128 samples apart share every activation row that is out of reach of their own zero padding, and the library
     # computes all four stages that way (shared stages): per 4096-window chunk a stage runs over the chunk's
-    # stream (rows padded to whole tiles) plus two short edge windows per window (18 rows in stage 1, 32 in stages 2-4).
-    # executed = the MMACs the tensor cores really perform per window; MMAC_CONV is the method's (algorithmic) figure.
-    def _up128(v):
-        return (v + 127) // 128 * 128
-    _nb = 4096
-    _f1 = (((_nb - 1) * 32 + 768) / _nb + 36) / 768
-    _f2 = (_up128((_nb - 1) * 16 + 384) / _nb + 64) / 384
-    _f3 = (_up128((_nb - 1) * 8 + 192) / _nb + 64) / 192
-    _f4 = (_up128((_nb - 1) * 4 + 96) / _nb + 64) / 96
-    shared_on = all(os.environ.get(k, "1") != "0" for k in ("AFRAME_SHARED_STEM", "AFRAME_SHARED_S1", "AFRAME_SHARED_S2")) \
-        and os.environ.get("AFRAME_SHARED_STAGES", "3") == "3" and args.batch == 4096
-    mmac_exec = (MMAC_CONV - 56.6e6 * (1 - _f1) - 144.7e6 * (1 - _f2) - 440.4e6 * (1 - _f3) - 427.8e6 * (1 - _f4)) if shared_on else MMAC_CONV
+    # stream (rows padded to whole tiles) plus two short edge windows per window.  executed = the MACs the tensor cores really
+    # perform, counted by the library per launch from its tile counts (aframe_tensor_macs); MMAC_CONV is the method's
+    # (algorithmic) figure per window.
+    mmac_exec = macs_exec / win_rank
     exec_tflops = conv_tflops * mmac_exec / MMAC_CONV
     out = {
         "metric": "analysed strain-seconds per second (whitened + scored, all timeslides)",

@@ -214,6 +214,12 @@ int64_t aframe_stream_graph_replays(const aframe_stream_state* st);
 /* Number of kernels the library has launched on this context since creation (for bench accounting). */
 int64_t aframe_launch_count(const aframe_ctx* ctx);
 
+/* Multiply-accumulates the bf16 tensor-core convolutions (a-7) of this context have issued since creation: per launch,
+ * (rows of all its MMA tiles, padding and separator rows included) x C_out x K.  Windows that overlap in time share the
+ * interior rows of every stage, so this is less than the method's 1069.5 MMAC per window; bench.py
+ * reports the tensor-core rate from this count, not from the algorithmic figure. */
+double aframe_tensor_macs(const aframe_ctx* ctx);
+
 /* ---- per-stage device timing (measurement aid) ------------------------------------------
  * aframe_profile(ctx, 1) clears the counters and makes every later call bracket each stage of the path
  * with a pair of CUDA events on the context's stream; aframe_profile(ctx, 0) stops.  aframe_profile_read

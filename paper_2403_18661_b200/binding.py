@@ -55,6 +55,7 @@ EXPORTS = {
     "aframe_stream_destroy": (None, [C.c_void_p]),
     "aframe_stream_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "aframe_launch_count": (C.c_int64, [C.c_void_p]),
+    "aframe_tensor_macs": (C.c_double, [C.c_void_p]),
     "aframe_whiten_batch": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_int]),
     "aframe_far": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_void_p]),
     "aframe_postprocess": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_int32, C.c_int32,
@@ -157,6 +158,9 @@ class Context:
 
     def launch_count(self):
         return int(self.lib.aframe_launch_count(self.handle))
+
+    def tensor_macs(self):
+        return float(self.lib.aframe_tensor_macs(self.handle))
 
     # ---- O-1
     def psd_welch(self, strain: torch.Tensor, out: torch.Tensor | None = None):

@@ -139,6 +139,7 @@ AF_API void aframe_destroy(aframe_ctx* ctx) {
 
 AF_API const char* aframe_last_error(const aframe_ctx* ctx) { return ctx ? ctx->err : kNoCtx; }
 AF_API int64_t aframe_launch_count(const aframe_ctx* ctx) { return ctx ? ctx->launches : 0; }
+AF_API double aframe_tensor_macs(const aframe_ctx* ctx) { return ctx ? ctx->tc_macs : 0.0; }
 
 // ---- O-1 ------------------------------------------------------------------------------------------
 AF_API aframe_status aframe_psd_welch(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,

@@ -62,6 +62,7 @@ struct aframe_ctx {
   int n_sms = 148;
   char err[512];
   int64_t launches = 0;
+  double tc_macs = 0.0;        // multiply-accumulates issued to the tensor cores so far (conv_tc.cu; aframe_tensor_macs)
   // tables
   float2* d_tw32 = nullptr;    // exp(-2 pi i q / 8192), q < 8192
   double2* d_tw64 = nullptr;

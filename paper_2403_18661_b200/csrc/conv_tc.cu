@@ -35,6 +35,7 @@ struct TcLaunch {
   TcConvParams p;
   int BN, grid, smem, device;
   bool head, cg2, halo;
+  double macs = 0.0;   // multiply-accumulates the launch issues to the tensor cores (whole tiles, padding rows included)
 };
 
 // score[b] = (sum of the fused-head partials of window b) / T + bias   (deterministic: fixed summation order)
@@ -98,16 +99,24 @@ aframe_status af_tc_check(aframe_ctx* ctx, aframe_weights* w) {
 // K blocks on its own input sc_in (res must then be null)
 // ov != null (shared stages): the launch runs the layer on ONE long window of ov->t_out output rows (a stream, or a batch of
 // short windows with zeroed separator rows) instead of nb windows of the table's length
-struct TcShapeOverride { int t_out; int zero_period, zero_valid, zero_origin; };
+// ov->e_nbp > 0 (packed edge batch, see TcConvParams::edge_nbp): 2 e_nbp short windows of e_P rows, one e_tbox-row box each
+struct TcShapeOverride {
+  int t_out; int zero_period, zero_valid, zero_origin;
+  int e_nbp = 0, e_P = 0, e_tbox = 0, e_T = 0, e_head = 0, e_tail = 0;
+  int64_t e_shift = 0, e_nb = 0;
+  const __nv_bfloat16* e_stream = nullptr;
+};
 static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const __nv_bfloat16* in,
                          const __nv_bfloat16* res, __nv_bfloat16* out, int64_t nb, bool head, float* head_part,
                          TcLaunch& L, int sc = -1, const __nv_bfloat16* sc_in = nullptr, const TcShapeOverride* ov = nullptr) {
   LayerDesc l = w->layers[li];
-  if (ov) { nb = 1; l.t_out = ov->t_out; l.t_in = ov->t_out * l.stride; }
+  const bool packed = ov && ov->e_nbp > 0;
+  if (packed) { nb = 2 * ov->e_nbp; l.t_out = ov->e_P; l.t_in = ov->e_P * l.stride; }
+  else if (ov) { nb = 1; l.t_out = ov->t_out; l.t_in = ov->t_out * l.stride; }
   const int BN = l.c_out >= 256 ? 256 : l.c_out;
   const int cg2_mode = env_int("AFRAME_CG2", 1);                 // 1: CTA pairs (cta_group::2) for the N = 256 layers; 2: also N = 128
   const bool cg2 = (BN == 256 && cg2_mode != 0) || (BN == 128 && cg2_mode >= 2);
-  const int T_box = tile_t_box(l.t_out), B_box = 128 / T_box;
+  const int T_box = packed ? ov->e_tbox : tile_t_box(l.t_out), B_box = 128 / T_box;
   const int P = l.stride;
   const bool has_res = res != nullptr;
   // resident weights + one halo box per tile (see TcConvParams): stride-1 k3 layers whose tiles stay inside a window
@@ -135,7 +144,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   L.tm_scw = L.tm_w;
   if (sc >= 0) {
     LayerDesc q = w->layers[sc];
-    if (ov) { q.t_out = ov->t_out; q.t_in = ov->t_out * q.stride; }
+    if (ov) { q.t_out = l.t_out; q.t_in = l.t_out * q.stride; }
     const uint64_t dims[4] = {(uint64_t)q.c_in, (uint64_t)q.stride, (uint64_t)(q.t_in / q.stride), (uint64_t)nb};
     const uint64_t str[3] = {(uint64_t)q.c_in * 2, (uint64_t)q.stride * q.c_in * 2, (uint64_t)q.t_in * q.c_in * 2};
     const uint32_t box[4] = {64, 1, (uint32_t)T_box, (uint32_t)B_box};
@@ -159,10 +168,17 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.kblocks = l.c_in / 64;
   p.n_tiles = l.c_out / BN;
   p.T_box = T_box; p.B_box = B_box;
-  p.t_blks = l.t_out / T_box;
+  p.t_blks = packed ? 1 : l.t_out / T_box;
+  p.edge_nbp = packed ? ov->e_nbp : 0;
+  p.edge_t0_tail = packed ? ov->e_P - T_box : 0;
+  p.edge_T = packed ? ov->e_T : 0; p.edge_P = packed ? ov->e_P : 0;
+  p.edge_head = packed ? ov->e_head : 0; p.edge_tail = packed ? ov->e_tail : 0;
+  p.edge_shift = packed ? ov->e_shift : 0;
+  p.edge_stream = packed ? reinterpret_cast<const uint4*>(ov->e_stream) : nullptr;
   const int64_t b_blks = (nb + B_box - 1) / B_box;
   const int64_t m_tiles = b_blks * p.t_blks;
   p.num_tiles = (int)((cg2 ? (m_tiles + 1) / 2 : m_tiles) * p.n_tiles);
+  L.macs = (double)(cg2 ? 2 * ((m_tiles + 1) / 2) : m_tiles) * 128.0 * l.c_out * 64.0 * (l.k * (l.c_in / 64) + (sc >= 0 ? w->layers[sc].c_in / 64 : 0));
   p.div_n = tc_fastdiv((uint32_t)p.n_tiles);
   p.div_t = tc_fastdiv((uint32_t)p.t_blks);
   // true GroupNorm (NEXT-2): the conv stores its plain output; norm, residual and ReLU follow in af_launch_gn_bf16
@@ -171,7 +187,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.head_w = head ? w->d_head_w : nullptr;
   p.head_part = head ? head_part : nullptr;
   p.head_slabs = l.t_out / 32;
-  p.nb = nb;
+  p.nb = packed ? ov->e_nb : nb;
   p.dbg_out = nullptr;
   if (env_int("AFRAME_TC_PROF", 0)) {       // experiment: per-role cycle counters, 32 slots per layer, read back by the caller
     static long long* d_prof = nullptr;
@@ -247,6 +263,7 @@ struct TcBlockLaunch {
   CUtensorMap tm_x, tm_wa, tm_wb, tm_out;
   TcBlockParams p;
   int grid = 0, smem = 0, device = 0;
+  double macs = 0.0;   // as TcLaunch::macs (two convs, 128-row MMAs per 126-row tile)
 };
 
 // Layer i is the first conv of a basic block the fused kernel can run: 64 -> 64 -> 64 channels, k3 s1 p1, ReLU after each,
@@ -299,6 +316,7 @@ static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia,
   L.smem = tcb_smem(p.nx, p.ny, p.no);
   L.device = ctx->device;
   L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
+  L.macs = 2.0 * p.num_tiles * 128.0 * 64.0 * 192.0;
   return true;
 }
 
@@ -411,9 +429,42 @@ __global__ void sh_gather_kernel(uint4* __restrict__ X, const uint4* __restrict_
   X[i] = v;
 }
 
+// Packed edge batch (stages on the CTA-pair path, see TcConvParams::edge_nbp): X = [copy_rows rows: the previous stage's stream |
+// nbp slots of P2 rows: the first P2 rows of every window | nbp slots: the last P2 rows of every window], each row taken from
+// the previous stage's edge batch where it is an edge row there, else from its stream.
+__global__ void shp_gather_kernel(uint4* __restrict__ X, const uint4* __restrict__ S, const uint4* __restrict__ Y, int64_t nb,
+                                  int64_t nbp, int Tp, int pieces, int64_t row_shift, int64_t src_stride, int64_t src_tail0,
+                                  int src_trow, int c_head, int c_tail, int64_t copy_rows, int64_t valid_rows, int P2) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (copy_rows + 2 * nbp * P2) * pieces) return;
+  const int j = (int)(i % pieces);
+  const int64_t row = i / pieces;
+  uint4 v = make_uint4(0u, 0u, 0u, 0u);
+  if (row < copy_rows) {
+    if (row < valid_rows) v = S[row * pieces + j];
+    X[i] = v;
+    return;
+  }
+  const int64_t mr = row - copy_rows;
+  const int r = (int)(mr % P2);
+  const int64_t m = mr / P2;
+  const bool tail = m >= nbp;
+  const int64_t b = tail ? m - nbp : m;
+  if (b < nb) {
+    const int t = tail ? Tp - P2 + r : r;
+    if (!tail && t < c_head) v = Y[(b * src_stride + t) * pieces + j];
+    else if (tail && t >= Tp - c_tail) v = Y[(src_tail0 + b * src_stride + (t - src_trow)) * pieces + j];
+    else v = S[(b * row_shift + t) * pieces + j];
+  }
+  X[i] = v;
+}
+
 // out[b][t][C]: edge result where t is an edge row of window b (t < c_head or t >= T2 - c_tail), else the stream row
+// (edge batch addressing, both layouts: window b's first rows start at row b * e_stride, its last rows at e_tail0 + b * e_stride,
+//  where local row 0 is window row e_trow)
 __global__ void s2_stitch_kernel(uint4* __restrict__ out, const uint4* __restrict__ S, const uint4* __restrict__ Y, int64_t nb,
-                                 int T2, int pieces /* C / 8 */, int64_t row_shift, int c_head, int c_tail, int rows, int period) {
+                                 int T2, int pieces /* C / 8 */, int64_t row_shift, int c_head, int c_tail, int64_t e_stride,
+                                 int64_t e_tail0, int e_trow) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= nb * T2 * pieces) return;
   const int j = (int)(i % pieces);
@@ -421,8 +472,8 @@ __global__ void s2_stitch_kernel(uint4* __restrict__ out, const uint4* __restric
   const int t = (int)(bt % T2);
   const int64_t b = bt / T2;
   uint4 v;
-  if (t < c_head) v = Y[((2 * b) * period + t) * pieces + j];
-  else if (t >= T2 - c_tail) v = Y[((2 * b + 1) * period + (t - (T2 - rows))) * pieces + j];
+  if (t < c_head) v = Y[(b * e_stride + t) * pieces + j];
+  else if (t >= T2 - c_tail) v = Y[(e_tail0 + b * e_stride + (t - e_trow)) * pieces + j];
   else v = S[(b * row_shift + t) * pieces + j];
   out[i] = v;
 }
@@ -433,7 +484,7 @@ __global__ void s2_stitch_kernel(uint4* __restrict__ out, const uint4* __restric
 __global__ void __launch_bounds__(256)
 sh_head_partial_kernel(const uint4* __restrict__ S, const uint4* __restrict__ Y, const float* __restrict__ head_w,
                        float* __restrict__ head_part, int64_t nb, int T, int C, int64_t row_shift, int c_head, int c_tail,
-                       int rows, int period) {
+                       int64_t e_stride, int64_t e_tail0, int e_trow) {
   const int lane = threadIdx.x & 31;
   const int chunks = C / 64, slabs = T / 32, pieces = C / 8;
   const int64_t wi = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -443,8 +494,8 @@ sh_head_partial_kernel(const uint4* __restrict__ S, const uint4* __restrict__ Y,
   const int64_t b = wi / ((int64_t)chunks * slabs);
   const int t = slab * 32 + lane;
   const uint4* rowp;
-  if (t < c_head) rowp = Y + ((2 * b) * period + t) * pieces;
-  else if (t >= T - c_tail) rowp = Y + ((2 * b + 1) * period + (t - (T - rows))) * pieces;
+  if (t < c_head) rowp = Y + (b * e_stride + t) * pieces;
+  else if (t >= T - c_tail) rowp = Y + (e_tail0 + b * e_stride + (t - e_trow)) * pieces;
   else rowp = S + (b * row_shift + t) * pieces;
   const float4* hw4 = reinterpret_cast<const float4*>(head_w + c * 64);
   float hacc[4] = {0.f, 0.f, 0.f, 0.f};
@@ -483,6 +534,10 @@ struct TcPlanCache {
     int T = 0, C = 0, C_in = 0, head = 0, tail = 0;   // output rows / channels, input channels, edge rows per window
     int rows = 0, period = 0;         // short window: data rows, data + separator rows
     int64_t shift = 0;                // rows between consecutive windows
+    bool packed = false;              // packed edge batch: separate stream / edge launches per layer (TcConvParams::edge_nbp)
+    int P = 0;                        // packed: rows per short-window slot
+    int64_t nbp = 0;                  // packed: slots per half (windows rounded up to whole boxes)
+    int64_t e_stride = 0, e_tail0 = 0; int e_trow = 0;   // edge-batch addressing of the stage's output (see s2_stitch_kernel)
   };
   std::vector<SharedStagePlan> sh;    // the stages after the first that run in shared form, in order
   bool sh_head = false;               // the last shared stage feeds the fused head: sh_head_partial_kernel instead of a stitch
@@ -610,6 +665,11 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     int64_t shift = 0;                // rows between consecutive windows at this stage's resolution
     int64_t rows_stream = 0, rows_edge = 0;
     size_t stream_bytes = 0, edge_bytes = 0, x_bytes = 0, off = 0;
+    // packed edge batch (stages whose layers run on the CTA-pair path): P rows per short-window slot, per launched layer the
+    // edge rows of its output at the window's start / end and the rows its box computes (16 or 32)
+    bool packed = false;
+    int P = 0;
+    std::vector<int> e_head, e_tail, tbox;
   };
   std::vector<SharedStage> shs;
   bool sh_head_on = false;
@@ -641,6 +701,36 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       if (!fits) { sh_head_on = false; break; }
       g.rows_stream = up128((chunk - 1) * g.shift + g.T);
       g.rows_edge = up128(2 * chunk * g.period);
+      // Packed edge batch: layer q's output differs from the stream's only in its first e_head[q] / last e_tail[q] rows (one more
+      // per conv), so a box of 16 rows per short window is enough while both stay <= 15 (the box's outermost row is computed from
+      // a row outside the box and is always replaced by the stream's value), 32 rows after that; a layer also needs 32 rows if a
+      // 32-row layer reads beyond its 16 (as input: one row further than its own edge; as residual: the same rows).
+      if (g.C % 256 == 0 && env_int("AFRAME_PACKED_EDGES", 1)) {
+        const int nl = (int)g.list.size();
+        g.e_head.resize(nl); g.e_tail.resize(nl); g.tbox.assign(nl, 16);
+        bool ok = true;
+        for (int q = 0; q < nl; ++q) {
+          g.e_head[q] = hp / 2 + 1 + q;
+          g.e_tail[q] = g.T - (Tp - tp) / 2 + q;
+          if (g.e_head[q] > 31 || g.e_tail[q] > 31) ok = false;
+          if (g.e_head[q] >= 16 || g.e_tail[q] >= 16) g.tbox[q] = 32;
+        }
+        auto idx_of = [&](int layer) { for (int q = 0; q < nl; ++q) if (g.list[q] == layer) return q; return -1; };
+        for (int q = nl - 1; ok && q >= 1; --q) {
+          if (g.tbox[q] != 32) continue;
+          const LayerDesc& l = w->layers[g.list[q]];
+          const int qi = idx_of(l.input_from), qr = l.residual_from >= 0 ? idx_of(l.residual_from) : -1;
+          if ((g.e_head[q] >= 16 || g.e_tail[q] >= 16) && qi >= 0) g.tbox[qi] = 32;
+          if ((g.e_head[q] >= 17 || g.e_tail[q] >= 17) && qr >= 0) g.tbox[qr] = 32;
+        }
+        int Pmax = 16;
+        for (int q = 0; q < nl; ++q) if (g.tbox[q] > Pmax) Pmax = g.tbox[q];
+        if (ok && g.T >= 2 * Pmax && g.e_head[nl - 1] == g.head && g.e_tail[nl - 1] == g.tail) {
+          g.packed = true; g.P = Pmax;
+          g.rows_edge = 2 * ((chunk + 7) / 8 * 8) * g.P;
+        }
+      }
+      if (!g.packed && !shs.empty() && shs.back().packed) { sh_head_on = false; break; }   // (a packed stage feeds packed stages only)
       shs.push_back(g);
       i0 = g.list.back() + 1; Tp = g.T; hp = g.head; tp = g.tail; shift_p = g.shift;
     }
@@ -750,7 +840,30 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           auto idx_of = [&](int layer) { for (size_t q = 0; q < h.list.size(); ++q) if (h.list[q] == layer) return (int)q; return -1; };
           P.stream.resize(h.list.size());
           ok = rows_tot < (1ll << 30);
-          for (size_t q = 0; ok && q < h.list.size(); ++q) {
+          P.packed = h.packed; P.P = h.P; P.nbp = (nb + 7) / 8 * 8;
+          if (h.packed) { P.e_stride = h.P; P.e_tail0 = P.nbp * h.P; P.e_trow = h.T - h.P; }
+          else { P.e_stride = 2 * h.period; P.e_tail0 = h.period; P.e_trow = h.T - h.rows; }
+          if (h.packed) P.edge.resize(h.list.size());
+          for (size_t q = 0; ok && h.packed && q < h.list.size(); ++q) {
+            // packed edge batch: per layer one launch over the stream (one long window) and one over the short-window slots
+            const int li = h.list[q];
+            const LayerDesc& l = w->layers[li];
+            const bool entry = li == h.i0;
+            const int sc = pc->sc_of[li];
+            const int qi = entry ? -1 : idx_of(l.input_from), qr = (l.residual_from >= 0 && sc < 0) ? idx_of(l.residual_from) : -1;
+            ok = (entry || qi >= 0) && (l.residual_from < 0 || sc >= 0 || qr >= 0);
+            if (!ok) break;
+            const __nv_bfloat16* x_edge = sh_x_ptr((int)g) + 2 * rows_s * h.C_in;
+            const TcShapeOverride ov_s{(int)rows_s, 0, 0, 0};
+            TcShapeOverride ov_e{0, 0, 0, 0};
+            ov_e.e_nbp = (int)P.nbp; ov_e.e_P = h.P; ov_e.e_tbox = h.tbox[q]; ov_e.e_T = h.T; ov_e.e_head = h.e_head[q]; ov_e.e_tail = h.e_tail[q];
+            ov_e.e_shift = h.shift; ov_e.e_nb = nb; ov_e.e_stream = entry ? nullptr : sh_buf((int)g, 0, (int)q);
+            ok = build_launch(ctx, w, li, entry ? sh_x_ptr((int)g) : sh_buf((int)g, 0, qi), qr >= 0 ? sh_buf((int)g, 0, qr) : nullptr,
+                              sh_buf((int)g, 0, (int)q), 1, false, nullptr, P.stream[q], sc, sc >= 0 ? sh_x_ptr((int)g) : nullptr, &ov_s) &&
+                 build_launch(ctx, w, li, entry ? x_edge : sh_buf((int)g, 1, qi), qr >= 0 ? sh_buf((int)g, 1, qr) : nullptr,
+                              sh_buf((int)g, 1, (int)q), 1, false, nullptr, P.edge[q], sc, sc >= 0 ? x_edge : nullptr, &ov_e);
+          }
+          for (size_t q = 0; ok && !h.packed && q < h.list.size(); ++q) {
             // one launch per layer over [stream | short windows]: the mask starts at the short windows (and their leading padding)
             const int li = h.list[q];
             const LayerDesc& l = w->layers[li];
@@ -824,7 +937,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       const uint4* E0 = reinterpret_cast<const uint4*>(slot_ptr(1) + ((nb - 1) * shift + T1) * 64);
       for (int k = 1; k <= K; ++k) {
         cudaError_t e = launch_block(pc->s1_stream[k], ctx->stream);
-        ctx->launches++; ++n_conv;
+        ctx->launches++; ++n_conv; ctx->tc_macs += pc->s1_stream[k].macs;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_block (stream) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
         const int64_t n_g = 2 * nb * S1_PERIOD * 8;
         s1_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
@@ -832,7 +945,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             k == 1 ? nullptr : reinterpret_cast<const uint4*>(s1_edge_ptr(k - 1)), k == 1 ? E0 : nullptr, nb, T1, shift, 2 * k, 2 * k - 1);
         AF_LAUNCH_CHECK(ctx);
         e = launch_block(pc->s1_edge[k], ctx->stream);
-        ctx->launches++;
+        ctx->launches++; ctx->tc_macs += pc->s1_edge[k].macs;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_block (edge) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
       }
       if (pc->sh.empty()) {
@@ -850,6 +963,28 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         const int64_t copy_rows = 2 * sh_rows_stream((int)g);
         const int64_t n_g = (copy_rows + edge_rows_in) * pieces_in;
         const int q_prev = g ? (int)pc->sh[g - 1].layers.size() - 1 : 0;
+        if (P.packed) {
+          const int64_t n_p = (copy_rows + 2 * P.nbp * 2 * P.P) * pieces_in;
+          const int64_t valid_prev = g ? (nb - 1) * pc->sh[g - 1].shift + pc->sh[g - 1].T : (nb - 1) * shift + T1;
+          shp_gather_kernel<<<(unsigned)((n_p + 255) / 256), 256, 0, ctx->stream>>>(
+              reinterpret_cast<uint4*>(sh_x_ptr((int)g)),
+              reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 0, q_prev) : s1_stream_ptr(K)),
+              reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 1, q_prev) : s1_edge_ptr(K)), nb, P.nbp, 2 * P.T, pieces_in,
+              2 * P.shift, g ? pc->sh[g - 1].e_stride : 2 * S1_PERIOD, g ? pc->sh[g - 1].e_tail0 : S1_PERIOD,
+              g ? pc->sh[g - 1].e_trow : T1 - S1_ROWS, g ? pc->sh[g - 1].head : 2 * K + 2, g ? pc->sh[g - 1].tail : 2 * K + 1,
+              copy_rows, valid_prev, 2 * P.P);
+          AF_LAUNCH_CHECK(ctx);
+          for (size_t q = 0; q < P.layers.size(); ++q) {
+            for (int part = 0; part < 2; ++part) {
+              TcLaunch& L2 = part ? P.edge[q] : P.stream[q];
+              L2.p.reverse = 0;
+              cudaError_t e = launch_conv(L2, ctx->stream);
+              ctx->launches++; ctx->tc_macs += L2.macs;
+              if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (packed edge stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
+            }
+            ++n_conv;
+          }
+        } else {
         sh_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
             reinterpret_cast<uint4*>(sh_x_ptr((int)g)),
             reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 0, q_prev) : s1_stream_ptr(K)),
@@ -862,22 +997,23 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           TcLaunch& L2 = P.stream[q];
           L2.p.reverse = 0;
           cudaError_t e = launch_conv(L2, ctx->stream);
-          ctx->launches++; ++n_conv;
+          ctx->launches++; ++n_conv; ctx->tc_macs += L2.macs;
           if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (shared stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
+        }
         }
         if (g + 1 == pc->sh.size() && pc->sh_head) {
           const int q_last = (int)P.layers.size() - 1;
           const int64_t n_warps = nb * (P.T / 32) * (P.C / 64);
           sh_head_partial_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(
               reinterpret_cast<const uint4*>(sh_buf((int)g, 0, q_last)), reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)),
-              w->d_head_w, head_part, nb, P.T, P.C, P.shift, P.head, P.tail, P.rows, P.period);
+              w->d_head_w, head_part, nb, P.T, P.C, P.shift, P.head, P.tail, P.e_stride, P.e_tail0, P.e_trow);
           AF_LAUNCH_CHECK(ctx);
         } else if (g + 1 == pc->sh.size()) {
           const int last = P.layers.back(), q_last = (int)P.layers.size() - 1, pieces = P.C / 8;
           const int64_t n_s = nb * P.T * pieces;
           s2_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
               reinterpret_cast<uint4*>(slot_ptr(last)), reinterpret_cast<const uint4*>(sh_buf((int)g, 0, q_last)),
-              reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)), nb, P.T, pieces, P.shift, P.head, P.tail, P.rows, P.period);
+              reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)), nb, P.T, pieces, P.shift, P.head, P.tail, P.e_stride, P.e_tail0, P.e_trow);
           AF_LAUNCH_CHECK(ctx);
         }
       }
@@ -901,7 +1037,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         af_prof_begin(ctx, AFRAME_PROF_CONV);
         ++n_conv;
         cudaError_t e = pc->fused_with[i] >= 0 ? launch_block(pc->blocks[i], ctx->stream) : launch_conv(L, ctx->stream);
-        ctx->launches++;
+        ctx->launches++; ctx->tc_macs += pc->fused_with[i] >= 0 ? pc->blocks[i].macs : L.macs;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
         if (w->live_gn) {
           st = af_launch_gn_bf16(ctx, slot_ptr(i), l.residual_from >= 0 ? slot_ptr(l.residual_from) : nullptr, l.t_out, l.c_out,

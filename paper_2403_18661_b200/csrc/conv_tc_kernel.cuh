@@ -74,6 +74,17 @@ struct TcConvParams {
   int zero_period, zero_valid;   // 0 = off
   int zero_origin;               // the batch of short windows starts at this row (rows before it, a stream, are not masked,
                                  // except the two rows just before it, which are the first short window's padding)
+  // packed edge batch (conv_tc.cu, shared stages on the CTA-pair path): the launch covers 2 edge_nbp short windows of edge_P
+  // rows each -- windows [0, edge_nbp) hold the first edge_P rows of their window (box at row 0), windows [edge_nbp, 2 edge_nbp)
+  // the last edge_P rows (box at row edge_t0_tail = edge_P - T_box) -- and one T_box-row box per short window is computed;
+  // the tensor map's zero fill is each window's own padding.  Only the rows within reach of that padding (row < edge_head or
+  // row >= edge_T - edge_tail of the window, for THIS layer's output) differ from the stream's; every other row of the box is
+  // replaced in the epilogue by the stream's value edge_stream[(b * edge_shift + row) * c_out ...] (this layer's output over
+  // the chunk's stream, written by the previous launch), so that all rows of a box are valid inputs of the next layer.
+  int edge_nbp;              // 0 = off
+  int edge_t0_tail, edge_T, edge_P, edge_head, edge_tail;
+  long long edge_shift;
+  const uint4* edge_stream;  // null: nothing is replaced (the stage's entry conv: all its input rows are valid)
   int out_f16;               // store the (pre-norm) output as fp16 (saturating) instead of bf16: z = mu + O(sigma) loses
                              // |mu| / sigma times more to an 8-bit mantissa than the normalised value does
   int w_bytes;               // resident weight region (0 unless HALO)
@@ -114,7 +125,7 @@ __device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b
 template <bool RES, bool HEAD, bool F16 = false>
 __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4* bias4, const float4* hw4,
                                                  unsigned char* rowp, int row, __nv_bfloat162 lo2, float& head_acc,
-                                                 bool zero_row = false) {
+                                                 bool zero_row = false, const uint4* copy_row = nullptr) {
   float hacc[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
   for (int jj = 0; jj < 8; ++jj) {                 // 8 pieces of 8 channels (16 B of bf16)
@@ -145,6 +156,7 @@ __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4
         asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(ow[e]) : "f"(f[2 * e + 1]), "f"(f[2 * e]));
     }
     if (zero_row) o = make_uint4(0u, 0u, 0u, 0u);
+    if (!HEAD && !F16 && copy_row != nullptr) o = copy_row[jj];
     if (HEAD) {
       const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
       const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
@@ -256,6 +268,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     const int m_idx = mp * (CG2 ? 2 : 1) + (int)rank;
     p.div_t.divmod(m_idx, bb, tb);
     t0 = tb * p.T_box; b0 = bb * p.B_box;
+    if (p.edge_nbp > 0 && b0 >= p.edge_nbp) t0 = p.edge_t0_tail;     // packed edge batch: the tails' box ends at the slot's end
   };
 
   if (warp == 0) {
@@ -537,9 +550,19 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         const int t_row = t0 + row % p.T_box;
         const bool zero_row = p.zero_period > 0 && t_row >= p.zero_origin - 2 &&
                               ((t_row - p.zero_origin + p.zero_period) % p.zero_period) >= p.zero_valid;
-        if (p.has_res) tc_epilogue_math<true, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row);
+        const uint4* copy_row = nullptr;
+        if (!HEAD && p.edge_nbp > 0 && p.edge_stream != nullptr) {
+          const int m = b0 + row / p.T_box;                      // short-window slot
+          const bool is_tail = m >= p.edge_nbp;
+          const int b = is_tail ? m - p.edge_nbp : m;
+          const int t_win = is_tail ? p.edge_T - p.edge_P + t_row : t_row;
+          const bool interior = is_tail ? t_win < p.edge_T - p.edge_tail : t_win >= p.edge_head;
+          if (interior && b < p.nb)
+            copy_row = p.edge_stream + (((long long)b * p.edge_shift + t_win) * p.c_out + n0 + c * 64) / 8;
+        }
+        if (p.has_res) tc_epilogue_math<true, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row, copy_row);
         else if (!HEAD && p.out_f16) tc_epilogue_math<false, false, true>(v, bias4, hw4, rowp, row, lo2, head_acc);
-        else tc_epilogue_math<false, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row);
+        else tc_epilogue_math<false, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row, copy_row);
         if (HEAD) {
           // the warp's 32 rows are one 32-row slab of one window (T_box % 32 == 0): reduce and emit a partial
           float s = head_acc;
