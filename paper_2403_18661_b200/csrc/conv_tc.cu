@@ -105,6 +105,7 @@ struct TcShapeOverride {
   int e_nbp = 0, e_P = 0, e_tbox = 0, e_T = 0, e_head = 0, e_tail = 0;
   int64_t e_shift = 0, e_nb = 0;
   const __nv_bfloat16* e_stream = nullptr;
+  bool head_rows = false;     // with head = true: per-row head dot products into head_part (TcConvParams::head_rows)
 };
 static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const __nv_bfloat16* in,
                          const __nv_bfloat16* res, __nv_bfloat16* out, int64_t nb, bool head, float* head_part,
@@ -187,6 +188,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.head_w = head ? w->d_head_w : nullptr;
   p.head_part = head ? head_part : nullptr;
   p.head_slabs = l.t_out / 32;
+  p.head_rows = (head && ov && ov->head_rows) ? 1 : 0; p.head_row_stride = l.t_out;
   p.nb = packed ? ov->e_nb : nb;
   p.dbg_out = nullptr;
   if (env_int("AFRAME_TC_PROF", 0)) {       // experiment: per-role cycle counters, 32 slots per layer, read back by the caller
@@ -516,6 +518,29 @@ sh_head_partial_kernel(const uint4* __restrict__ S, const uint4* __restrict__ Y,
   if (lane == 0) head_part[(b * slabs + slab) * chunks + c] = sum;
 }
 
+// The same partial sums from per-row dot products (TcConvParams::head_rows: the stage's last conv stores no activation, its
+// epilogue emits each row's dot product with the head weights per 64-channel chunk, Rs over the stream and Re over the edge
+// batch): lane = row of the slab, the 32 values are summed in the order the fused head uses.
+__global__ void __launch_bounds__(256)
+sh_head_rows_kernel(const float* __restrict__ Rs, const float* __restrict__ Re, float* __restrict__ head_part, int64_t nb, int T,
+                    int chunks, int64_t row_shift, int c_head, int c_tail, int64_t e_stride, int64_t e_tail0, int e_trow) {
+  const int lane = threadIdx.x & 31;
+  const int slabs = T / 32;
+  const int64_t wi = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (wi >= nb * slabs * chunks) return;
+  const int c = (int)(wi % chunks);
+  const int slab = (int)((wi / chunks) % slabs);
+  const int64_t b = wi / ((int64_t)chunks * slabs);
+  const int t = slab * 32 + lane;
+  float sum;
+  if (t < c_head) sum = Re[(b * e_stride + t) * chunks + c];
+  else if (t >= T - c_tail) sum = Re[(e_tail0 + b * e_stride + (t - e_trow)) * chunks + c];
+  else sum = Rs[(b * row_shift + t) * chunks + c];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+  if (lane == 0) head_part[(b * slabs + slab) * chunks + c] = sum;
+}
+
 struct TcPlanCache {
   const aframe_weights* w = nullptr;
   void* base = nullptr;
@@ -541,6 +566,7 @@ struct TcPlanCache {
   };
   std::vector<SharedStagePlan> sh;    // the stages after the first that run in shared form, in order
   bool sh_head = false;               // the last shared stage feeds the fused head: sh_head_partial_kernel instead of a stitch
+  bool sh_head_rows = false;          // ... and its last conv emits per-row head dot products (sh_head_rows_kernel)
   std::vector<int> sc_of;             // per layer: the projection-shortcut conv that runs inside it (else -1)
   std::vector<char> skip;             // per layer: runs inside another launch
 };
@@ -854,14 +880,21 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             ok = (entry || qi >= 0) && (l.residual_from < 0 || sc >= 0 || qr >= 0);
             if (!ok) break;
             const __nv_bfloat16* x_edge = sh_x_ptr((int)g) + 2 * rows_s * h.C_in;
-            const TcShapeOverride ov_s{(int)rows_s, 0, 0, 0};
+            TcShapeOverride ov_s{(int)rows_s, 0, 0, 0};
             TcShapeOverride ov_e{0, 0, 0, 0};
+            // the conv that feeds the head stores nothing: its tensor holds the per-row head dot products instead
+            // ([stream rows | edge-batch rows][C / 64] floats)
+            const bool hr = sh_head_on && g + 1 == shs.size() && q + 1 == h.list.size() && env_int("AFRAME_HEAD_ROWS", 1);
+            float* hr_s = reinterpret_cast<float*>(sh_buf((int)g, 0, (int)q));
+            float* hr_e = hr_s + rows_s * (h.C / 64);
+            ov_s.head_rows = ov_e.head_rows = hr;
+            if (hr) pc->sh_head_rows = true;
             ov_e.e_nbp = (int)P.nbp; ov_e.e_P = h.P; ov_e.e_tbox = h.tbox[q]; ov_e.e_T = h.T; ov_e.e_head = h.e_head[q]; ov_e.e_tail = h.e_tail[q];
             ov_e.e_shift = h.shift; ov_e.e_nb = nb; ov_e.e_stream = entry ? nullptr : sh_buf((int)g, 0, (int)q);
             ok = build_launch(ctx, w, li, entry ? sh_x_ptr((int)g) : sh_buf((int)g, 0, qi), qr >= 0 ? sh_buf((int)g, 0, qr) : nullptr,
-                              sh_buf((int)g, 0, (int)q), 1, false, nullptr, P.stream[q], sc, sc >= 0 ? sh_x_ptr((int)g) : nullptr, &ov_s) &&
+                              sh_buf((int)g, 0, (int)q), 1, hr, hr_s, P.stream[q], sc, sc >= 0 ? sh_x_ptr((int)g) : nullptr, &ov_s) &&
                  build_launch(ctx, w, li, entry ? x_edge : sh_buf((int)g, 1, qi), qr >= 0 ? sh_buf((int)g, 1, qr) : nullptr,
-                              sh_buf((int)g, 1, (int)q), 1, false, nullptr, P.edge[q], sc, sc >= 0 ? x_edge : nullptr, &ov_e);
+                              sh_buf((int)g, 1, (int)q), 1, hr, hr_e, P.edge[q], sc, sc >= 0 ? x_edge : nullptr, &ov_e);
           }
           for (size_t q = 0; ok && !h.packed && q < h.list.size(); ++q) {
             // one launch per layer over [stream | short windows]: the mask starts at the short windows (and their leading padding)
@@ -1001,7 +1034,15 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (shared stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
         }
         }
-        if (g + 1 == pc->sh.size() && pc->sh_head) {
+        if (g + 1 == pc->sh.size() && pc->sh_head && pc->sh_head_rows) {
+          const int q_last = (int)P.layers.size() - 1;
+          const int64_t n_warps = nb * (P.T / 32) * (P.C / 64);
+          const float* hr_s = reinterpret_cast<const float*>(sh_buf((int)g, 0, q_last));
+          sh_head_rows_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(
+              hr_s, hr_s + sh_rows_stream((int)g) * (P.C / 64), head_part, nb, P.T, P.C / 64, P.shift, P.head, P.tail, P.e_stride,
+              P.e_tail0, P.e_trow);
+          AF_LAUNCH_CHECK(ctx);
+        } else if (g + 1 == pc->sh.size() && pc->sh_head) {
           const int q_last = (int)P.layers.size() - 1;
           const int64_t n_warps = nb * (P.T / 32) * (P.C / 64);
           sh_head_partial_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(

@@ -55,6 +55,9 @@ struct TcConvParams {
   const float* head_w;
   float* head_part;
   int head_slabs;            // T_out / T_box
+  // head_rows != 0 (shared stages): head_part receives the dot product of EVERY output row's 64-channel chunk instead,
+  // head_part[((b0 + row / T_box) * head_row_stride + t) * (c_out / 64) + chunk]; sh_head_rows_kernel sums them per window slab
+  int head_rows, head_row_stride;
   int64_t nb;                // windows in this launch (head variant bounds check)
   // HALO variant (k = 3, stride 1, whole 128-row tiles inside one window): the folded weights of the layer stay resident
   // in shared memory (w_bytes) and ONE (128 + 2)-row input box per 64-channel block serves all three taps: tap d reads
@@ -567,6 +570,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           // the warp's 32 rows are one 32-row slab of one window (T_box % 32 == 0): reduce and emit a partial
           float s = head_acc;
           head_acc = 0.f;
+          if (p.head_rows) {
+            p.head_part[((long long)(b0 + row / p.T_box) * p.head_row_stride + t_row) * (p.c_out >> 6) + n_idx * CH + c] = s;
+          } else {
 #pragma unroll
           for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
           const int r0 = q * 32;
@@ -574,6 +580,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           const int slab = (t0 + r0 % p.T_box) >> 5;
           if (lane == 0 && b < p.nb)
             p.head_part[(b * p.head_slabs + slab) * (p.c_out >> 6) + n_idx * CH + c] = s;
+          }
           named_bar_sync(1 + g, 128);              // residual buffer fully read before it is refilled
         } else {
           T(6);
