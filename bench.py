@@ -379,6 +379,7 @@ def run_ours(args):
     # perform, counted by the library per launch from its tile counts (aframe_tensor_macs); MMAC_CONV is the method's
     # (algorithmic) figure per window.
     mmac_exec = macs_exec / win_rank
+    shared_on = mmac_exec < 0.9 * MMAC_CONV       # (the AFRAME_SHARED_* switches and other batch sizes run other launch plans)
     exec_tflops = conv_tflops * mmac_exec / MMAC_CONV
     out = {
         "metric": "analysed strain-seconds per second (whitened + scored, all timeslides)",
@@ -398,16 +399,17 @@ def run_ours(args):
                      "bound": "tensor", "achieved": exec_tflops, "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
                      "frac": exec_tflops / peaks["bf16_sustained"],
                      "algorithmic_tflops": conv_tflops, "executed_frac_of_algorithmic": mmac_exec / MMAC_CONV,
-                     # dram__bytes_read.sum + dram__bytes_write.sum of the 29 conv launches of one 4096-window batch under
-                     # ncu --set full of the per-window build (profiles/r01d_conv_full.md): 16.5 + 10.1 GB
-                     "traffic": 26.66e9 / 29,
+                     # dram__bytes_read.sum + dram__bytes_write.sum of the 50 conv launches of one 4096-window chunk under
+                     # ncu --set full of this build (profiles/r01i_conv_full.md): 4.22 + 1.24 GB, per launch
+                     "traffic": (5.462e9 / 50) if shared_on else (26.66e9 / 29),
                      "peak_kind": "sustained bf16 cuBLAS, " + peaks["source"], "launches": int(conv_launches),
                      "avg_launch_ms": conv_ms / max(conv_launches, 1),
                      "algorithmic": "achieved = EXECUTED tensor FLOPs (2 x executed MMAC per window x windows scored) over the "
                                     "summed CUDA-event time of the conv launches on the library's stream.  The method's work is "
                                     "2 x 1069.5 MMAC per window (algorithmic_tflops counts that); overlapping windows share the "
                                     "interior rows of every stage, which are computed once per stream plus two short edge windows "
-                                    "per window, so only executed_frac_of_algorithmic of those FLOPs are performed"},
+                                    "per window, so only executed_frac_of_algorithmic of those FLOPs are performed (counted per "
+                                    "launch by the library: aframe_tensor_macs)"},
         "stages": {k: {"ms": v[0], "launches": v[1], "share": v[0] / ms_total} for k, v in stages.items()},
     }
     wh_ms = stages["whiten"][0]

@@ -247,3 +247,40 @@ def test_shared_stages_equal_the_per_window_path_bit_for_bit(af, config1, stride
     ref = ctx.forward(w, wins)
     assert bool(torch.isfinite(shared).all())
     assert torch.equal(shared, ref)
+
+
+def test_tensor_mac_counter_matches_the_layer_table(af, config1):
+    """aframe_tensor_macs (bench.py's roofline numerator) counts, per launch, tile rows x C_out x K.  On the per-window path
+    (explicit windows, 128 of them: every conv's rows fill whole 128-row tiles) that is the layer table's own MAC count,
+    except for the 64-channel basic blocks, whose fused kernel computes 128-row MMAs per 126-row tile.  In shared form
+    (overlapping in-place windows) the count must be well below the per-window figure and above the stream-only bound."""
+    net = config1["net"]
+    ctx = af.Context(precision=af.BF16)
+    w = ctx.load_weights(config1["blob"])
+    B = 128
+    m0 = ctx.tensor_macs()
+    ctx.forward(w, torch.from_numpy(config1["wins"]).cuda())
+    torch.cuda.synchronize()
+    per_window = 0.0
+    t_of = {-1: 3072}                                            # rows of every layer's output (layer table order)
+    for i, layer in enumerate(net["layers"]):
+        t_in = t_of[layer["input_from"]]
+        if layer["kind"] == 2:                                   # head
+            break
+        t_of[i] = (t_in + 2 * layer["pad"] - layer["k"]) // layer["stride"] + 1
+        if i < 2 or layer["kind"] != 0:                          # stem conv and max-pool run on CUDA cores
+            continue
+        t_out = t_of[i]
+        rows = -(-t_out // 126) * 128 if (layer["c_in"] == 64 and layer["c_out"] == 64) else t_out
+        per_window += rows * layer["c_out"] * layer["c_in"] * layer["k"]
+    got = ctx.tensor_macs() - m0
+    assert got == pytest.approx(B * per_window, rel=1e-12)
+    # shared form: 4096 overlapping windows taken in place
+    n_win = 4096
+    white = torch.randn(2, (n_win - 1) * 128 + 3072 + 2048, device="cuda").bfloat16().contiguous()
+    m1 = ctx.tensor_macs()
+    ctx.forward_strided(w, white, 0, n_win, chan_shift=[0, 2048])
+    torch.cuda.synchronize()
+    shared = (ctx.tensor_macs() - m1) / n_win
+    algorithmic = 1069.5e6
+    assert 0.04 * algorithmic < shared < 0.5 * algorithmic      # stream alone: 128 of 3072 samples per window = 1/24
