@@ -978,7 +978,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             k == 1 ? nullptr : reinterpret_cast<const uint4*>(s1_edge_ptr(k - 1)), k == 1 ? E0 : nullptr, nb, T1, shift, 2 * k, 2 * k - 1);
         AF_LAUNCH_CHECK(ctx);
         e = launch_block(pc->s1_edge[k], ctx->stream);
-        ctx->launches++; ctx->tc_macs += pc->s1_edge[k].macs;
+        ctx->launches++; ++n_conv; ctx->tc_macs += pc->s1_edge[k].macs;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_block (edge) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
       }
       if (pc->sh.empty()) {
@@ -1012,10 +1012,9 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
               TcLaunch& L2 = part ? P.edge[q] : P.stream[q];
               L2.p.reverse = 0;
               cudaError_t e = launch_conv(L2, ctx->stream);
-              ctx->launches++; ctx->tc_macs += L2.macs;
+              ctx->launches++; ++n_conv; ctx->tc_macs += L2.macs;
               if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (packed edge stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
             }
-            ++n_conv;
           }
         } else {
         sh_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
