@@ -106,6 +106,7 @@ struct TcShapeOverride {
   int64_t e_shift = 0, e_nb = 0;
   const __nv_bfloat16* e_stream = nullptr;
   bool head_rows = false;     // with head = true: per-row head dot products into head_part (TcConvParams::head_rows)
+  bool pair_plan = false;     // one shared-memory plan for every launch of the stage, so that two of them can share a launch
 };
 static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const __nv_bfloat16* in,
                          const __nv_bfloat16* res, __nv_bfloat16* out, int64_t nb, bool head, float* head_part,
@@ -201,7 +202,8 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   // (two epilogue groups: EG * nbuf staging buffers of 16 KB; a residual tile is prefetched pf chunks ahead into the
   //  buffer its chunk's output is staged in)
   const bool r = p.has_res;
-  if (cg2 && head)            { p.stages = 5; p.nbuf = 1; p.pf = 0; }
+  if (cg2 && !head && BN == 256 && ov && ov->pair_plan) { p.stages = 5; p.nbuf = 2; p.pf = 1; }
+  else if (cg2 && head)       { p.stages = 5; p.nbuf = 1; p.pf = 0; }
   else if (cg2 && BN == 128)  { p.stages = r ? 5 : 6; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }   // 24 KB stages
   else if (cg2 && l.k * p.kblocks < 12) { p.stages = 5; p.nbuf = 2; p.pf = r ? 1 : 0; }   // short K: the epilogue is the critical path
   else if (cg2)               { p.stages = r ? 5 : 6; p.nbuf = r ? 2 : 1; p.pf = r ? 1 : 0; }
@@ -227,7 +229,8 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   return true;
 }
 
-template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t launch_bn(const TcLaunch& L, cudaStream_t s) {
+template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t launch_bn(const TcLaunch& L, cudaStream_t s,
+                                                                                   const TcLaunch* second = nullptr) {
   static std::atomic<uint64_t> attr_done{0};          // bit d: the attribute is set on device d (it is per device)
   auto kern = conv_tc_kernel<BN, HEAD, CG2, HALO>;
   const uint64_t bit = 1ull << (L.device & 63);
@@ -248,12 +251,17 @@ template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t lau
   at[1].val.programmaticStreamSerializationAllowed = 1;
   static const int pdl = env_int("AFRAME_PDL", 1);
   cfg.attrs = at; cfg.numAttrs = pdl ? 2 : 1;
-  return cudaLaunchKernelEx(&cfg, kern, L.tm_in, L.tm_w, L.tm_out, L.tm_res, L.tm_scw, L.p);
+  const TcLaunch& L1 = second ? *second : L;        // second problem of the launch (conv_tc_kernel), or none
+  TcConvParams p1 = L1.p;
+  if (!second) p1.num_tiles = 0;
+  return cudaLaunchKernelEx(&cfg, kern, L.tm_in, L.tm_w, L.tm_out, L.tm_res, L.tm_scw, L.p, L1.tm_in, L1.tm_w, L1.tm_out, L1.tm_res,
+                            L1.tm_scw, p1);
 }
 
-static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s) {
+// second != null: both problems in one launch (only the CTA-pair N = 256 storing variant is paired, see can_pair below)
+static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s, const TcLaunch* second = nullptr) {
   if (L.cg2 && L.BN == 128) return launch_bn<128, false, true>(L, s);
-  if (L.cg2) return L.head ? launch_bn<256, true, true>(L, s) : launch_bn<256, false, true>(L, s);
+  if (L.cg2) return L.head ? launch_bn<256, true, true>(L, s) : launch_bn<256, false, true>(L, s, second);
   if (L.head) return launch_bn<256, true, false>(L, s);
   if (L.halo) return L.BN == 128 ? launch_bn<128, false, false, true>(L, s) : launch_bn<64, false, false, true>(L, s);
   return L.BN == 256 ? launch_bn<256, false, false>(L, s)
@@ -888,6 +896,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             float* hr_s = reinterpret_cast<float*>(sh_buf((int)g, 0, (int)q));
             float* hr_e = hr_s + rows_s * (h.C / 64);
             ov_s.head_rows = ov_e.head_rows = hr;
+            ov_s.pair_plan = ov_e.pair_plan = true;
             if (hr) pc->sh_head_rows = true;
             ov_e.e_nbp = (int)P.nbp; ov_e.e_P = h.P; ov_e.e_tbox = h.tbox[q]; ov_e.e_T = h.T; ov_e.e_head = h.e_head[q]; ov_e.e_tail = h.e_tail[q];
             ov_e.e_shift = h.shift; ov_e.e_nb = nb; ov_e.e_stream = entry ? nullptr : sh_buf((int)g, 0, (int)q);
@@ -1007,13 +1016,33 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
               g ? pc->sh[g - 1].e_trow : T1 - S1_ROWS, g ? pc->sh[g - 1].head : 2 * K + 2, g ? pc->sh[g - 1].tail : 2 * K + 1,
               copy_rows, valid_prev, 2 * P.P);
           AF_LAUNCH_CHECK(ctx);
-          for (size_t q = 0; q < P.layers.size(); ++q) {
-            for (int part = 0; part < 2; ++part) {
-              TcLaunch& L2 = part ? P.edge[q] : P.stream[q];
-              L2.p.reverse = 0;
-              cudaError_t e = launch_conv(L2, ctx->stream);
-              ctx->launches++; ++n_conv; ctx->tc_macs += L2.macs;
-              if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (packed edge stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
+          // Launch order: stream(0) | edge(q) with stream(q + 1) as ONE launch of two problems (independent of each other: both
+          // need stream(q), and edge(q) needs edge(q - 1)) | ... | edge(last).  A stream launch alone costs 16-30 us for 1/8 of an
+          // edge launch's work (profiles/r01i_conv_full.md); as the second problem its tiles fill the edge launch's last wave.
+          static const int pair_on = env_int("AFRAME_PAIR_LAUNCH", 1);
+          const size_t nl = P.layers.size();
+          auto can_pair = [&](size_t q) {
+            if (!pair_on || q + 1 >= nl) return false;
+            const TcLaunch& a = P.edge[q];
+            const TcLaunch& b = P.stream[q + 1];
+            return a.cg2 && b.cg2 && a.BN == 256 && b.BN == 256 && !a.head && !b.head && !a.halo && !b.halo && a.p.stages == b.p.stages &&
+                   a.p.nbuf == b.p.nbuf && a.p.pf == b.p.pf && a.smem == b.smem && a.p.c_out == b.p.c_out;
+          };
+          auto launch_one = [&](TcLaunch& A, TcLaunch* B2) -> aframe_status {
+            A.p.reverse = 0;
+            if (B2) B2->p.reverse = 0;
+            cudaError_t e = launch_conv(A, ctx->stream, B2);
+            ctx->launches++; ++n_conv; ctx->tc_macs += A.macs + (B2 ? B2->macs : 0.0);
+            if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (packed edge stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
+            return AFRAME_OK;
+          };
+          if ((st = launch_one(P.stream[0], nullptr)) != AFRAME_OK) return st;
+          for (size_t q = 0; q < nl; ++q) {
+            if (can_pair(q)) {
+              if ((st = launch_one(P.edge[q], &P.stream[q + 1])) != AFRAME_OK) return st;
+            } else {
+              if ((st = launch_one(P.edge[q], nullptr)) != AFRAME_OK) return st;
+              if (q + 1 < nl && (st = launch_one(P.stream[q + 1], nullptr)) != AFRAME_OK) return st;
             }
           }
         } else {

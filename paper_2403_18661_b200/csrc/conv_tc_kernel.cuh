@@ -193,7 +193,13 @@ template <int BN, bool HEAD, bool CG2, bool HALO>
 __global__ void __launch_bounds__(TcCfg<BN, CG2>::THREADS, 1)
 conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 rows */, const __grid_constant__ CUtensorMap tm_w,
                const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_res /* or shortcut input */,
-               const __grid_constant__ CUtensorMap tm_scw /* shortcut weights */, const TcConvParams p) {
+               const __grid_constant__ CUtensorMap tm_scw /* shortcut weights */, const TcConvParams p,
+               // optional second problem (p1.num_tiles > 0; neither HALO nor HEAD): every CTA runs its tiles of the first problem,
+               // then its tiles of the second one, through the same pipelines.  The two must be independent (conv_tc.cu pairs a
+               // layer's packed edge batch with the next layer's stream) and share BN, ring depth and staging plan.
+               const __grid_constant__ CUtensorMap tm_in1, const __grid_constant__ CUtensorMap tm_w1,
+               const __grid_constant__ CUtensorMap tm_out1, const __grid_constant__ CUtensorMap tm_res1,
+               const __grid_constant__ CUtensorMap tm_scw1, const TcConvParams p1) {
   using Cfg = TcCfg<BN, CG2>;
   constexpr int EG = Cfg::EG;
   constexpr bool SPLIT = Cfg::SPLIT;
@@ -264,7 +270,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
   auto T = [&](int slot) { if (prof) { const long long t = clock64(); tacc[slot] += t - tprev; tprev = t; } };
   auto Tflush = [&](int role) { if (prof) for (int i = 0; i < 8; ++i) p.dbg_out[role * 8 + i] = tacc[i]; };
   // tile -> (n0, t0, b0): n fastest, then the T_box-row block inside a window group, then the window group
-  auto decode = [&](int tile, int& n_idx, int& t0, int& b0) {
+  auto decode = [&](const TcConvParams& p, int tile, int& n_idx, int& t0, int& b0) {
     int mp, tb, bb;
     if (p.reverse) tile = p.num_tiles - 1 - tile;
     p.div_n.divmod(tile, mp, n_idx);
@@ -292,7 +298,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       int stage = 0; uint32_t phase = 0;
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         int n_idx, t0, b0;
-        decode(tile, n_idx, t0, b0);
+        decode(p, tile, n_idx, t0, b0);
         for (int kb = 0; kb < p.kblocks; ++kb) {   // one stage = the 130-row box of one 64-channel block
           T(0);
           mbar_wait(empty_bar(stage), phase ^ 1u);
@@ -321,9 +327,11 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     } else {
       const uint32_t lfull0 = CG2 ? mapa_cluster(full_bar(0), 0) : full_bar(0);   // leader's full barriers
       int stage = 0; uint32_t phase = 0;
+      auto produce = [&](const CUtensorMap& tm_in, const CUtensorMap& tm_w, const CUtensorMap& tm_res, const CUtensorMap& tm_scw,
+                         const TcConvParams& p) {
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         int n_idx, t0, b0;
-        decode(tile, n_idx, t0, b0);
+        decode(p, tile, n_idx, t0, b0);
         const int n0 = n_idx * BN;
         for (int d = 0; d < p.taps; ++d) {
           const int toff = p.tap_toff[d], par = p.tap_par[d];
@@ -369,6 +377,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
       }
+      };
+      produce(tm_in, tm_w, tm_res, tm_scw, p);
+      if (!HEAD && p1.num_tiles > 0) produce(tm_in1, tm_w1, tm_res1, tm_scw1, p1);
       if (lane == 0) Tflush(0);
     }
   } else if (warp == 1) {
@@ -378,6 +389,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       int stage = 0; uint32_t phase = 0;
       int acc = 0; uint32_t acc_phase = 0;
       if (HALO) mbar_wait(w_bar, 0);
+      auto issue = [&](const TcConvParams& p) {
+      const int kiters = p.taps * p.kblocks + p.sc_kblocks;
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         T(0);
         mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
@@ -449,6 +462,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         if (++acc == NACC) { acc = 0; acc_phase ^= 1u; }
         T(4);
       }
+      };
+      issue(p);
+      if (!HALO && !HEAD && p1.num_tiles > 0) issue(p1);
       if (lane == 0) Tflush(1);
     }
   } else {
@@ -467,15 +483,27 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     const int c_first = SPLIT ? g : 0;
     const uint32_t tempty_leader0 = CG2 ? mapa_cluster(tempty_bar(0), 0) : tempty_bar(0);
 
+    uint32_t j = 0;                                // chunk counter of this group
+    uint32_t seq = SPLIT ? 0 : g;                  // this CTA's tile sequence number
+    uint32_t res_par = 0;                          // bit b: phase parity of this group's residual barrier b
+    const int PF = p.pf;
+    auto drain = [&](const CUtensorMap& tm_out, const CUtensorMap& tm_res, const TcConvParams& p, bool second) {
+    if (second) {
+      // the second problem's bias replaces the first one's once both groups are done with it; the leader's earlier stores
+      // must have read their staging buffers before a residual tile is prefetched into one
+      named_bar_sync(3, 128 * EG);
+      for (int i = (int)threadIdx.x - 64; i < p.c_out; i += 128 * EG) s_bias[i] = p.bias[i];
+      named_bar_sync(3, 128 * EG);
+      if (leader) tma_store_wait_read_n(0);
+    }
     // residual prefetch cursor (leader only): item pf_j of this group's (tile, chunk) sequence; the residual tile lands
     // in the staging buffer the chunk's output will be written to (added in place)
     int pf_tile = tile_first, pf_c = c_first;
-    uint32_t pf_j = 0;
-    const int PF = p.pf;
+    uint32_t pf_j = j;
     auto issue_res = [&]() {
       if (pf_tile < p.num_tiles) {
         int n_idx, t0, b0;
-        decode(pf_tile, n_idx, t0, b0);
+        decode(p, pf_tile, n_idx, t0, b0);
         const int buf = pf_j % NBUF;
         mbar_arrive_expect_tx(res_bar(g, buf), TC_OUT_BYTES);
         tma_load_4d(gbuf + buf * TC_OUT_BYTES, &tm_res, res_bar(g, buf), n_idx * BN + pf_c * 64, 0, t0, b0);
@@ -504,20 +532,18 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     auto copy_prefetch = [&](int tile_) {
       if (HEAD || p.edge_nbp == 0 || p.edge_stream == nullptr || tile_ >= p.num_tiles) return;
       int n_i, t0_, b0_;
-      decode(tile_, n_i, t0_, b0_);
+      decode(p, tile_, n_i, t0_, b0_);
       const uint4* cb = copy_base(n_i * BN, t0_, b0_);
       if (cb != nullptr)
         for (int c = c_first; c < CH; c += C_STEP) asm volatile("prefetch.global.L1 [%0];" :: "l"(cb + c * 8));
     };
     copy_prefetch(tile_first);
 
-    uint32_t j = 0;                                // chunk counter of this group
-    uint32_t seq = SPLIT ? 0 : g;                  // this CTA's tile sequence number
     for (int tile = tile_first; tile < p.num_tiles; tile += tile_step, seq += (SPLIT ? 1 : EG)) {
       const int acc = seq % NACC;
       const uint32_t acc_phase = (seq / NACC) & 1u;
       int n_idx, t0, b0;
-      decode(tile, n_idx, t0, b0);
+      decode(p, tile, n_idx, t0, b0);
       const int n0 = n_idx * BN;
       const uint4* copy_tile = copy_base(n0, t0, b0);
       copy_prefetch(tile + tile_step);
@@ -569,7 +595,10 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             }
           }
         }
-        if (p.has_res) mbar_wait(res_bar(g, buf), (j / NBUF) & 1u);
+        if (p.has_res) {                           // (own parity per buffer: with two problems not every chunk has a residual)
+          mbar_wait(res_bar(g, buf), (res_par >> buf) & 1u);
+          res_par ^= 1u << buf;
+        }
         T(5);
         const float4* bias4 = reinterpret_cast<const float4*>(s_bias + n0 + c * 64);
         const float4* hw4 = reinterpret_cast<const float4*>(s_headw + n0 + c * 64);
@@ -618,6 +647,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         }
       }
     }
+    };
+    drain(tm_out, tm_res, p, false);
+    if (!HALO && !HEAD && p1.num_tiles > 0) drain(tm_out1, tm_res1, p1, true);
     if (leader) Tflush(2 + g);
     if (leader && !HEAD) tma_store_wait_all<0>();
   }
