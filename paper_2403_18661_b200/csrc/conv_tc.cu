@@ -171,13 +171,15 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.n_tiles = l.c_out / BN;
   p.T_box = T_box; p.B_box = B_box;
   p.t_blks = packed ? 1 : l.t_out / T_box;
+  p.a_bytes = T_box * B_box * 128;
   p.edge_nbp = packed ? ov->e_nbp : 0;
+  p.edge_blks_half = packed ? (int)((ov->e_nb + B_box - 1) / B_box) : 0;
   p.edge_t0_tail = packed ? ov->e_P - T_box : 0;
   p.edge_T = packed ? ov->e_T : 0; p.edge_P = packed ? ov->e_P : 0;
   p.edge_head = packed ? ov->e_head : 0; p.edge_tail = packed ? ov->e_tail : 0;
   p.edge_shift = packed ? ov->e_shift : 0;
   p.edge_stream = packed ? reinterpret_cast<const uint4*>(ov->e_stream) : nullptr;
-  const int64_t b_blks = (nb + B_box - 1) / B_box;
+  const int64_t b_blks = packed ? 2 * ((ov->e_nb + B_box - 1) / B_box) : (nb + B_box - 1) / B_box;
   const int64_t m_tiles = b_blks * p.t_blks;
   p.num_tiles = (int)((cg2 ? (m_tiles + 1) / 2 : m_tiles) * p.n_tiles);
   L.macs = (double)(cg2 ? 2 * ((m_tiles + 1) / 2) : m_tiles) * 128.0 * l.c_out * 64.0 * (l.k * (l.c_in / 64) + (sc >= 0 ? w->layers[sc].c_in / 64 : 0));
@@ -358,6 +360,7 @@ static cudaError_t launch_block(const TcBlockLaunch& L, cudaStream_t s) {
 // therefore run (1) once over the whole stream and (2) over a batch of 2 short windows per window -- its first and last
 // S1_ROWS rows, with the true edge rows of the previous block -- which yields the edge rows exactly; s1_stitch_kernel
 // then writes the per-window tensor the next stage reads.  Same kernel, same per-row arithmetic: bit-identical results.
+constexpr int SH_SPARE_SLOTS = 16;          // packed edge batch: spare slots after each half (the last box of a half may overhang)
 constexpr int S1_ROWS = 16;                 // rows of a short window (needs 2 K + 4 <= S1_ROWS - 2 for K blocks)
 constexpr int S1_PERIOD = S1_ROWS + 2;      // + 2 separator rows (zero input, y1 forced to zero)
 
@@ -736,32 +739,23 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       g.rows_stream = up128((chunk - 1) * g.shift + g.T);
       g.rows_edge = up128(2 * chunk * g.period);
       // Packed edge batch: layer q's output differs from the stream's only in its first e_head[q] / last e_tail[q] rows (one more
-      // per conv), so a box of 16 rows per short window is enough while both stay <= 15 (the box's outermost row is computed from
-      // a row outside the box and is always replaced by the stream's value), 32 rows after that; a layer also needs 32 rows if a
-      // 32-row layer reads beyond its 16 (as input: one row further than its own edge; as residual: the same rows).
+      // per conv); its box holds those rows and the two rows next to them that the epilogue takes from the stream (the outer one
+      // is computed from a row outside the box): tbox[q] = max(e_head, e_tail) + 2 rows, floor(128 / tbox) slots per MMA tile.
       if (g.C % 256 == 0 && env_int("AFRAME_PACKED_EDGES", 1)) {
         const int nl = (int)g.list.size();
-        g.e_head.resize(nl); g.e_tail.resize(nl); g.tbox.assign(nl, 16);
+        g.e_head.resize(nl); g.e_tail.resize(nl); g.tbox.assign(nl, 0);
         bool ok = true;
+        int Pmax = 0;
         for (int q = 0; q < nl; ++q) {
           g.e_head[q] = hp / 2 + 1 + q;
           g.e_tail[q] = g.T - (Tp - tp) / 2 + q;
-          if (g.e_head[q] > 31 || g.e_tail[q] > 31) ok = false;
-          if (g.e_head[q] >= 16 || g.e_tail[q] >= 16) g.tbox[q] = 32;
+          g.tbox[q] = (g.e_head[q] > g.e_tail[q] ? g.e_head[q] : g.e_tail[q]) + 2;     // edge rows + the two copied rows
+          if (g.tbox[q] > 32) ok = false;
+          if (g.tbox[q] > Pmax) Pmax = g.tbox[q];
         }
-        auto idx_of = [&](int layer) { for (int q = 0; q < nl; ++q) if (g.list[q] == layer) return q; return -1; };
-        for (int q = nl - 1; ok && q >= 1; --q) {
-          if (g.tbox[q] != 32) continue;
-          const LayerDesc& l = w->layers[g.list[q]];
-          const int qi = idx_of(l.input_from), qr = l.residual_from >= 0 ? idx_of(l.residual_from) : -1;
-          if ((g.e_head[q] >= 16 || g.e_tail[q] >= 16) && qi >= 0) g.tbox[qi] = 32;
-          if ((g.e_head[q] >= 17 || g.e_tail[q] >= 17) && qr >= 0) g.tbox[qr] = 32;
-        }
-        int Pmax = 16;
-        for (int q = 0; q < nl; ++q) if (g.tbox[q] > Pmax) Pmax = g.tbox[q];
         if (ok && g.T >= 2 * Pmax && g.e_head[nl - 1] == g.head && g.e_tail[nl - 1] == g.tail) {
           g.packed = true; g.P = Pmax;
-          g.rows_edge = 2 * ((chunk + 7) / 8 * 8) * g.P;
+          g.rows_edge = 2 * (chunk + SH_SPARE_SLOTS) * g.P;
         }
       }
       if (!g.packed && !shs.empty() && shs.back().packed) { sh_head_on = false; break; }   // (a packed stage feeds packed stages only)
@@ -874,7 +868,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           auto idx_of = [&](int layer) { for (size_t q = 0; q < h.list.size(); ++q) if (h.list[q] == layer) return (int)q; return -1; };
           P.stream.resize(h.list.size());
           ok = rows_tot < (1ll << 30);
-          P.packed = h.packed; P.P = h.P; P.nbp = (nb + 7) / 8 * 8;
+          P.packed = h.packed; P.P = h.P; P.nbp = nb + SH_SPARE_SLOTS;
           if (h.packed) { P.e_stride = h.P; P.e_tail0 = P.nbp * h.P; P.e_trow = h.T - h.P; }
           else { P.e_stride = 2 * h.period; P.e_tail0 = h.period; P.e_trow = h.T - h.rows; }
           if (h.packed) P.edge.resize(h.list.size());

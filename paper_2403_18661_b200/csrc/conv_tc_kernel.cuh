@@ -85,8 +85,11 @@ struct TcConvParams {
   // which the next layers read as well (a conv reaches one row further, and so does the residual two layers on), are replaced
   // in the epilogue by the stream's values edge_stream[(b * edge_shift + row) * c_out ...] (this layer's output over the
   // chunk's stream, written by the previous launch); the rest of the box is never read.
-  int edge_nbp;              // 0 = off
+  int edge_nbp;              // 0 = off; else slots per half (windows + spare slots for the last box of a half)
+  int edge_blks_half;        // boxes per half: M tiles [0, edge_blks_half) are window starts, the rest window ends
   int edge_t0_tail, edge_T, edge_P, edge_head, edge_tail;
+  int a_bytes;               // bytes of one activation box (T_box * B_box rows of 128 B; 16 KB unless T_box does not divide 128:
+                             // the rest of the 128-row MMA tile is then stale shared memory, and those rows are dropped)
   long long edge_shift;
   const uint4* edge_stream;  // null: nothing is replaced (the stage's entry conv: all its input rows are valid)
   int out_f16;               // store the (pre-norm) output as fp16 (saturating) instead of bf16: z = mu + O(sigma) loses
@@ -277,7 +280,10 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     const int m_idx = mp * (CG2 ? 2 : 1) + (int)rank;
     p.div_t.divmod(m_idx, bb, tb);
     t0 = tb * p.T_box; b0 = bb * p.B_box;
-    if (p.edge_nbp > 0 && b0 >= p.edge_nbp) t0 = p.edge_t0_tail;     // packed edge batch: the tails' box ends at the slot's end
+    if (p.edge_nbp > 0 && bb >= p.edge_blks_half) {                  // packed edge batch: window ends, the box ends at the slot's end
+      b0 = p.edge_nbp + (bb - p.edge_blks_half) * p.B_box;
+      t0 = p.edge_t0_tail;
+    }
   };
 
   if (warp == 0) {
@@ -343,12 +349,12 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             if (elect_one()) {
               if (CG2) {
                 // both CTAs load their own A rows and their half of B; all bytes are counted on the leader's barrier
-                if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * Cfg::STAGE_BYTES);
+                if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * (p.a_bytes + Cfg::B_BYTES));
                 const uint32_t lbar = lfull0 + 8u * stage;
                 tma_load_4d_cg2(sa, &tm_in, lbar, kb * 64, par, t0 + toff, b0);
                 tma_load_3d_cg2(sa + Cfg::A_BYTES, &tm_w, lbar, kb * 64, n0 + (int)rank * Cfg::B_ROWS, d);
               } else {
-                mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
+                mbar_arrive_expect_tx(full_bar(stage), p.a_bytes + Cfg::B_BYTES);
                 tma_load_4d(sa, &tm_in, full_bar(stage), kb * 64, par, t0 + toff, b0);
                 tma_load_3d(sa + Cfg::A_BYTES, &tm_w, full_bar(stage), kb * 64, n0, d);
               }
@@ -363,12 +369,12 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           const uint32_t sa = stage_base + stage * STAGE_BYTES;
           if (elect_one()) {
             if (CG2) {
-              if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * Cfg::STAGE_BYTES);
+              if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * (p.a_bytes + Cfg::B_BYTES));
               const uint32_t lbar = lfull0 + 8u * stage;
               tma_load_4d_cg2(sa, &tm_res, lbar, kb * 64, 0, t0, b0);
               tma_load_3d_cg2(sa + Cfg::A_BYTES, &tm_scw, lbar, kb * 64, n0 + (int)rank * Cfg::B_ROWS, 0);
             } else {
-              mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
+              mbar_arrive_expect_tx(full_bar(stage), p.a_bytes + Cfg::B_BYTES);
               tma_load_4d(sa, &tm_res, full_bar(stage), kb * 64, 0, t0, b0);
               tma_load_3d(sa + Cfg::A_BYTES, &tm_scw, full_bar(stage), kb * 64, n0, 0);
             }
@@ -505,7 +511,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         int n_idx, t0, b0;
         decode(p, pf_tile, n_idx, t0, b0);
         const int buf = pf_j % NBUF;
-        mbar_arrive_expect_tx(res_bar(g, buf), TC_OUT_BYTES);
+        mbar_arrive_expect_tx(res_bar(g, buf), p.a_bytes);
         tma_load_4d(gbuf + buf * TC_OUT_BYTES, &tm_res, res_bar(g, buf), n_idx * BN + pf_c * 64, 0, t0, b0);
       }
       ++pf_j;
@@ -518,7 +524,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     // packed edge batch: this thread's row of tile (n0_, t0_, b0_) is taken from the stream if it is one of the two rows next to
     // the window's edge rows (the only interior rows a later layer reads): pointer to its first channel of the tile, else null
     auto copy_base = [&](int n0_, int t0_, int b0_) -> const uint4* {
-      if (HEAD || p.edge_nbp == 0 || p.edge_stream == nullptr) return nullptr;
+      if (HEAD || p.edge_nbp == 0 || p.edge_stream == nullptr || row >= p.T_box * p.B_box) return nullptr;
       const int m = b0_ + row / p.T_box;           // short-window slot
       const bool is_tail = m >= p.edge_nbp;
       const int b = is_tail ? m - p.edge_nbp : m;
@@ -624,7 +630,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           float s = head_acc;
           head_acc = 0.f;
           if (p.head_rows) {
-            p.head_part[((long long)(b0 + row / p.T_box) * p.head_row_stride + t_row) * (p.c_out >> 6) + n_idx * CH + c] = s;
+            if (row < p.T_box * p.B_box) p.head_part[((long long)(b0 + row / p.T_box) * p.head_row_stride + t_row) * (p.c_out >> 6) + n_idx * CH + c] = s;
           } else {
 #pragma unroll
           for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
