@@ -741,6 +741,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       // Packed edge batch: layer q's output differs from the stream's only in its first e_head[q] / last e_tail[q] rows (one more
       // per conv); its box holds those rows and the two rows next to them that the epilogue takes from the stream (the outer one
       // is computed from a row outside the box): tbox[q] = max(e_head, e_tail) + 2 rows, floor(128 / tbox) slots per MMA tile.
+      // (The entry conv's rows are all computed from valid input rows and the last layer's interior rows are never read: no copies.)
       if (g.C % 256 == 0 && env_int("AFRAME_PACKED_EDGES", 1)) {
         const int nl = (int)g.list.size();
         g.e_head.resize(nl); g.e_tail.resize(nl); g.tbox.assign(nl, 0);
@@ -749,7 +750,8 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         for (int q = 0; q < nl; ++q) {
           g.e_head[q] = hp / 2 + 1 + q;
           g.e_tail[q] = g.T - (Tp - tp) / 2 + q;
-          g.tbox[q] = (g.e_head[q] > g.e_tail[q] ? g.e_head[q] : g.e_tail[q]) + 2;     // edge rows + the two copied rows
+          // edge rows + the two copied rows; the stage's last layer is read at its edge rows only (next stage's gather, stitch, head)
+          g.tbox[q] = (g.e_head[q] > g.e_tail[q] ? g.e_head[q] : g.e_tail[q]) + (q + 1 < nl ? 2 : 0);
           if (g.tbox[q] > 32) ok = false;
           if (g.tbox[q] > Pmax) Pmax = g.tbox[q];
         }
@@ -893,7 +895,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             ov_s.pair_plan = ov_e.pair_plan = true;
             if (hr) pc->sh_head_rows = true;
             ov_e.e_nbp = (int)P.nbp; ov_e.e_P = h.P; ov_e.e_tbox = h.tbox[q]; ov_e.e_T = h.T; ov_e.e_head = h.e_head[q]; ov_e.e_tail = h.e_tail[q];
-            ov_e.e_shift = h.shift; ov_e.e_nb = nb; ov_e.e_stream = entry ? nullptr : sh_buf((int)g, 0, (int)q);
+            ov_e.e_shift = h.shift; ov_e.e_nb = nb; ov_e.e_stream = (entry || q + 1 == h.list.size()) ? nullptr : sh_buf((int)g, 0, (int)q);
             ok = build_launch(ctx, w, li, entry ? sh_x_ptr((int)g) : sh_buf((int)g, 0, qi), qr >= 0 ? sh_buf((int)g, 0, qr) : nullptr,
                               sh_buf((int)g, 0, (int)q), 1, hr, hr_s, P.stream[q], sc, sc >= 0 ? sh_x_ptr((int)g) : nullptr, &ov_s) &&
                  build_launch(ctx, w, li, entry ? x_edge : sh_buf((int)g, 1, qi), qr >= 0 ? sh_buf((int)g, 1, qr) : nullptr,
