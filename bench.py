@@ -400,8 +400,8 @@ def run_ours(args):
                      "frac": exec_tflops / peaks["bf16_sustained"],
                      "algorithmic_tflops": conv_tflops, "executed_frac_of_algorithmic": mmac_exec / MMAC_CONV,
                      # dram__bytes_read.sum + dram__bytes_write.sum of the 35 conv launches of one 4096-window chunk under
-                     # ncu --set full of this build (profiles/r01j_conv_full.md): 4.16 + 1.51 GB, per launch
-                     "traffic": (5.666e9 / 35) if shared_on else (26.66e9 / 29),
+                     # ncu --set full of this build (profiles/r01l_conv_full.md): 3.55 + 1.09 GB, per launch
+                     "traffic": (4.639e9 / 35) if shared_on else (26.66e9 / 29),
                      "peak_kind": "sustained bf16 cuBLAS, " + peaks["source"], "launches": int(conv_launches),
                      "avg_launch_ms": conv_ms / max(conv_launches, 1),
                      "algorithmic": "achieved = EXECUTED tensor FLOPs (2 x executed MMAC per window x windows scored) over the "
