@@ -752,7 +752,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           g.e_tail[q] = g.T - (Tp - tp) / 2 + q;
           // edge rows + the two copied rows; the stage's last layer is read at its edge rows only (next stage's gather, stitch, head)
           g.tbox[q] = (g.e_head[q] > g.e_tail[q] ? g.e_head[q] : g.e_tail[q]) + (q + 1 < nl ? 2 : 0);
-          if (g.tbox[q] > 32) ok = false;
+          if (g.tbox[q] > 32 || g.tbox[q] < 1 || 128 / g.tbox[q] > SH_SPARE_SLOTS) ok = false;   // (a half's last box overhangs by < 128 / tbox slots)
           if (g.tbox[q] > Pmax) Pmax = g.tbox[q];
         }
         if (ok && g.T >= 2 * Pmax && g.e_head[nl - 1] == g.head && g.e_tail[nl - 1] == g.tail) {
