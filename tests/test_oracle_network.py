@@ -176,3 +176,50 @@ def test_live_group_norm_network_runs_and_differs_from_folded():
     # per-window statistics: scaling one window's input leaves its score (almost) unchanged, unlike a frozen norm
     s2 = onet.forward(net, x * np.array([1.0, 8.0])[:, None, None])
     assert abs(s2[1] - s[1]) < 1e-3 * max(1.0, abs(s[1])) and s2[0] == s[0]
+
+
+def test_overlapping_windows_share_every_row_out_of_reach_of_their_padding():
+    """The identity the CUDA path's shared stages rest on, checked on the float64 oracle alone: two
+    windows cut 128 samples apart from one stream have identical activations, layer by layer, except in the rows within
+    reach of each window's own zero padding.  The reach follows from the conv definition (O-5): stem + pool leave rows
+    {0, 1} / {T - 1}; a k3 s1 conv adds one row per side; a k3 s2 conv maps e -> e // 2 + 1 and f -> T_out - (T_in - f - 1 + 1) // 2;
+    a k1 s2 conv e -> ceil(e / 2); a residual takes the larger reach.  Stage ends: 8/7, 12/11, 18/17, 15/14 rows."""
+    from synthdata import make_weight_blob, full_config
+    net = onet.parse_blob(make_weight_blob(**full_config()))
+    rng = np.random.default_rng(5)
+    stream = rng.standard_normal((2, 3072 + 128))
+    wins = np.stack([stream[:, :3072], stream[:, 128:128 + 3072]])
+    _, outs = onet.forward(net, wins, keep=True)
+    lens = onet.output_length(net, 3072)
+    reach = {}                                     # layer -> (rows at the start, rows at the end) that see the padding
+    stage_end = {}
+    for i, l in enumerate(net["layers"]):
+        if l["kind"] == onet.KIND_HEAD:
+            break
+        t_out = lens[i]
+        if l["input_from"] < 0:                    # stem conv k7 s2 p3: rows 0, 1 / the last row see the padding
+            e, f = 2, 1
+        else:
+            ei, fi = reach[l["input_from"]]
+            t_in = lens[l["input_from"]]
+            k, s, p = l["k"], l["stride"], l["pad"]
+            # output row t reads input rows s t - p ... s t - p + k - 1
+            e = max([t + 1 for t in range(t_out) if s * t - p < ei] + [0])
+            f = max([t_out - t for t in range(t_out) if s * t - p + k - 1 >= t_in - fi] + [0])
+            if l["kind"] == onet.KIND_CONV and l["residual_from"] >= 0:
+                er, fr = reach[l["residual_from"]]
+                e, f = max(e, er), max(f, fr)
+        reach[i] = (e, f)
+        stage_end[l["c_out"] if l["kind"] == onet.KIND_CONV else 64] = (e, f)
+        shift = 128 * t_out // 3072                # rows between the two windows at this resolution
+        if i == 0 or (128 * t_out) % 3072:
+            continue
+        a = outs[i][0][:, shift + e: t_out - f]    # window 0, the rows that are window 1's rows e ... t_out - shift - f
+        b = outs[i][1][:, e: t_out - shift - f]
+        scale = np.abs(outs[i]).max()
+        assert np.abs(a - b).max() <= 1e-10 * scale, (i, e, f)
+        # the bound is tight: the last row inside the reach does differ (checked where the padding's influence, which decays
+        # with every layer, is still far above rounding: the 64- and 128-channel stages)
+        if e > 0 and l["kind"] == onet.KIND_CONV and l["c_out"] <= 128:
+            assert np.abs(outs[i][0][:, shift + e - 1] - outs[i][1][:, e - 1]).max() > 1e-9 * scale, (i, e)
+    assert stage_end[64] == (8, 7) and stage_end[128] == (12, 11) and stage_end[256] == (18, 17) and stage_end[512] == (15, 14)
