@@ -222,7 +222,7 @@ def latency_run(af, torch, ctx_stream, weights_blob, n_updates, n_warm_scored=10
     """configs[4]: one update of 128 new samples per detector, batch 1, over a 1.5 s ring with incremental
     whitening.  Host wall-clock from the call to the score being readable on the host, and device time."""
     from synthdata import coloured_noise
-    ctx = af.Context(precision=af.BF16, stream=ctx_stream)
+    ctx = af.Context(precision=af.F16, stream=ctx_stream)
     w = ctx.load_weights(weights_blob)
     st = ctx.stream_create(w)
     n_fill = PSD_LEN // STRIDE + KERNEL // STRIDE           # updates before the first score (reading C1)
@@ -310,7 +310,7 @@ def run_ours(args):
     torch.cuda.synchronize()
 
     with torch.cuda.stream(stream):
-        ctx = af.Context(precision=af.BF16, stream=stream)
+        ctx = af.Context(precision=af.F16, stream=stream)
         w = ctx.load_weights(blob)
 
         def step_dev(j):
@@ -498,7 +498,7 @@ def next_rows(af, torch, stream, peaks):
 
     res = {}
     with torch.cuda.stream(stream):
-        ctx = af.Context(stream=stream, precision=af.BF16)
+        ctx = af.Context(stream=stream, precision=af.F16)
         # NEXT-4: one training batch, 384 x 2 x 10.5 s, own PSD per row, bf16 kernels out
         row = torch.from_numpy(coloured_noise(21504, 9001)).cuda()
         xb = (row[None] * (1.0 + torch.arange(384, device="cuda")[:, None, None] % 5)).contiguous()

@@ -45,7 +45,17 @@ typedef enum {
   AFRAME_EUNSUPPORTED = 6  /* device is not sm_100, or the layer table needs an unsupported op  */
 } aframe_status;
 
-typedef enum { AFRAME_FP32 = 0, AFRAME_BF16 = 1 } aframe_precision;
+/* Two uses.
+ * (1) cfg.precision, the arithmetic of the network path: AFRAME_FP32 (CUDA-core FFMA) or AFRAME_F16, the tensor-core
+ *     path (tcgen05 kind::f16): folded weights rounded once to IEEE half, every stored activation rounded once to half
+ *     (round to nearest even, saturating at +-65504; NaN stays NaN), products exact, accumulation, bias, residual add and
+ *     ReLU in fp32, stem arithmetic and head in fp32 (reading B10 of DESIGN.md).  AFRAME_BF16 is refused here
+ *     (AFRAME_EUNSUPPORTED): with bf16 storage the scores lose their rank order -- Spearman 0.9987 against the float64
+ *     oracle on BASELINE.json configs[1], measured, which IS the ceiling of that format (0.9985 for the oracle with
+ *     bf16 roundings) and below the 0.999 the contract asks for -- while half costs the same bytes and the same
+ *     tensor-core rate and gives > 0.9999.
+ * (2) the element type of a whitened stream handed in or out (out_dtype / dtype arguments): any of the three. */
+typedef enum { AFRAME_FP32 = 0, AFRAME_BF16 = 1, AFRAME_F16 = 2 } aframe_precision;
 
 /* POD configuration, versioned by .size (= sizeof(aframe_config)).  Defaults in comments are
  * BASELINE.json configs[1..4]; configs[0] uses n_design 4096, kernel_len 2048. */
@@ -63,7 +73,7 @@ typedef struct {
   int64_t  psd_len;           /* 131072 = 64 s of PSD history; multiple of welch_hop     */
   int64_t  psd_update;        /* 16384 = new PSD every 8 s (BASELINE.json configs[2])            */
   int32_t  strain_scale_log2; /* 70                                                              */
-  int32_t  precision;         /* aframe_precision of the network path                            */
+  int32_t  precision;         /* network path: AFRAME_F16 (tensor cores, default) or AFRAME_FP32 */
   int32_t  welch_average;     /* 0 = mean over segments (reading A1, default); 1 = per-bin median
                                  divided by its bias for n segments (NEXT-3 variant; n <= 255)   */
   int32_t  reserved_;         /* must be 0                                                       */
@@ -96,7 +106,7 @@ aframe_status aframe_psd_welch(aframe_ctx* ctx, const float* d_strain, int64_t n
  * Designs the L-tap zero-phase FIR whitening filter from d_psd (as returned by aframe_psd_welch) and
  * applies it to a contiguous segment by FFT overlap-save.  Output has n_samples - filter_len samples
  * per channel: out[c][m] corresponds to input sample m + filter_len/2 (0.5 s cropped per edge).
- * d_out: [C][ld_out] of fp32 or bf16 (out_dtype).  n_samples <= filter_len writes nothing (OK). */
+ * d_out: [C][ld_out] of fp32, bf16 or fp16 (out_dtype).  n_samples <= filter_len writes nothing (OK). */
 aframe_status aframe_whiten(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
                             const float* d_psd, void* d_out, int64_t ld_out, aframe_precision out_dtype);
 
@@ -121,7 +131,7 @@ aframe_status aframe_whiten_rolling(aframe_ctx* ctx, const float* d_strain, int6
  * its OWN Welch PSD (from its first n_psd samples), its own filter (O-2) and is whitened (O-3) over its
  * remaining n_samples - n_psd samples.
  * d_strain: [n_batch][C][n_samples] fp32, contiguous.  d_out: [n_batch][C][n_samples - n_psd - filter_len]
- * fp32 or bf16, contiguous (the paper's shapes: n_samples 21504, n_psd 16384 -> 3072 = kernel_len).
+ * fp32, bf16 or fp16, contiguous (the paper's shapes: n_samples 21504, n_psd 16384 -> 3072 = kernel_len).
  * AFRAME_ESHAPE if n_psd < welch_nfft, n_samples - n_psd <= filter_len or n_batch * C > 65535. */
 aframe_status aframe_whiten_batch(aframe_ctx* ctx, const float* d_strain, int64_t n_batch, int64_t n_samples,
                                   int64_t n_psd, void* d_out, aframe_precision out_dtype);
@@ -139,7 +149,7 @@ aframe_status aframe_far(aframe_ctx* ctx, const float* d_background, int64_t n_b
 /* ---- weights (readings B1-B7) ----------------------------------------------------------
  * host_blob: the version-1 blob documented in synthdata/weights.py (header, layer table, UNFOLDED
  * fp32 parameters).  The library validates the table against cfg (AFRAME_ESHAPE), folds the frozen
- * norm into (W', b') in double precision, and uploads fp32 and bf16 (K-major) copies.  Synchronises.
+ * norm into (W', b') in double precision, and uploads fp32 and fp16 (K-major) copies.  Synchronises.
  * Blob norm_kind 2 (NEXT-2, P:39 true GroupNorm) carries no frozen statistics: nothing is folded, and
  * aframe_forward computes mean / variance per window and group on the device after every conv. */
 aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob, size_t bytes, aframe_weights** out);
@@ -147,8 +157,8 @@ void          aframe_weights_free(aframe_weights* w);
 
 /* ---- O-5  network forward ------------------------------------------------------------------------------
  * d_windows: [B][C][kernel_len] fp32, already whitened.  d_scores: [B] fp32 raw logits (no sigmoid, B8).
- * B <= 0 is AFRAME_EINVAL.  Precision follows cfg.precision (bf16: tcgen05 tensor-core path with fp32
- * accumulation, reading B10; fp32: CUDA-core FFMA path). */
+ * B <= 0 is AFRAME_EINVAL.  Precision follows cfg.precision (AFRAME_F16: tcgen05 tensor-core path, fp16 weights and
+ * activations, fp32 accumulation, reading B10; AFRAME_FP32: CUDA-core FFMA path). */
 aframe_status aframe_forward(aframe_ctx* ctx, const aframe_weights* w, const float* d_windows, int64_t B,
                              float* d_scores);
 
@@ -161,7 +171,10 @@ aframe_status aframe_forward_strided(aframe_ctx* ctx, const aframe_weights* w, c
 
 /* ---- O-6  streaming ("snapshotting") -------------------------------------------------
  * The state (raw ring, cached periodograms, PSD, filter, whitened ring, activations) is an opaque
- * device-resident object owned by the library. */
+ * device-resident object owned by the library.  aframe_stream_create returns AFRAME_ESHAPE unless cfg.stride divides
+ * cfg.welch_hop (one Welch segment completes exactly on an update) and psd_len >= stride + filter_len.
+ * Lifetime: a weights object must outlive every stream state created from it, and a context must outlive its weights
+ * and stream states: destroy in the order states, weights, context. */
 aframe_status aframe_stream_create(aframe_ctx* ctx, const aframe_weights* w, aframe_stream_state** out);
 aframe_status aframe_stream_reset(aframe_stream_state* st);
 void          aframe_stream_destroy(aframe_stream_state* st);
@@ -175,7 +188,7 @@ aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samples, af
 
 /* ---- O-3..O-6 in one call: offline background analysis of a stored segment (C3) ---------
  * BASELINE.json configs[3]: the segment is whitened once per detector with the rolling-PSD rule
- * (aframe_whiten_rolling; output kept in the context's workspace in the network's input precision),
+ * (aframe_whiten_rolling; output kept in the context's workspace as fp16 for the tensor-core path, else fp32),
  * then n_slides timeslides are scored: window i of slide k takes channel 0 (H1, held fixed) at whitened
  * index first + i*stride and every other channel at first + i*stride + slide_shifts[k] ("the Livingston
  * data is shifted in 1 s increments"; shifts in SAMPLES, applied to the whitened stream, C3).
@@ -201,14 +214,15 @@ aframe_status aframe_score_timeslides_host(aframe_ctx* ctx, const aframe_weights
  * d_integrated [n_series][n]: 1 s top hat = mean of the trailing n_int scores (n_int = inference rate x 1 s = 16;
  *   the first n_int - 1 entries average the scores that exist), float32 sums in index order.
  * Triggers: one per consecutive window of n_cluster integrated values (8 s = 128; a trailing partial window counts):
- *   d_trig_value [n_series][n_trig] = the maximum, d_trig_index [n_series][n_trig] = index of its first occurrence.
+ *   d_trig_value [n_series][n_trig] = the maximum, d_trig_index [n_series][n_trig] = index of its first occurrence
+ *   (a window that holds a NaN yields its first NaN: NaN propagates).
  *   *h_n_trig (HOST) = ceil(n / n_cluster).  The caller sizes the trigger arrays for that. */
 aframe_status aframe_postprocess(aframe_ctx* ctx, const float* d_scores, int64_t n_series, int64_t n, int64_t ld,
                                  int32_t n_int, int32_t n_cluster, float* d_integrated, float* d_trig_value,
                                  int64_t* d_trig_index, int64_t* h_n_trig);
 
-/* How many updates of this state were served by replaying the captured CUDA graph (0 if graphs are switched off with
- * the environment variable AFRAME_STREAM_GRAPH=0, or while aframe_profile is on). */
+/* How many updates of this state were served by replaying the captured CUDA graph (0 for a context bound to the legacy
+ * default stream, which cannot be captured, or while aframe_profile is on). */
 int64_t aframe_stream_graph_replays(const aframe_stream_state* st);
 
 /* Number of kernels the library has launched on this context since creation (for bench accounting). */

@@ -129,12 +129,20 @@ def round_bf16(x):
     return r.view(np.float32).astype(np.float64)
 
 
+def round_f16(x):
+    """float64 -> float32 (RNE) -> IEEE half (RNE, finite values beyond +-65504 saturate, NaN stays NaN) -> float64;
+    emulates the activation storage of the CUDA tensor-core path (reading B10)."""
+    f = np.clip(np.asarray(x, dtype=np.float64).astype(np.float32), np.float32(-65504.0), np.float32(65504.0))
+    return f.astype(np.float16).astype(np.float64)
+
+
 def forward(net, windows, folded=True, act_round=None, weight_round=None, keep=False):
     """windows [B][C][K] float -> scores [B] float64.
 
     folded=False evaluates conv -> explicit norm (the unfolded form of reading B6); tests prove both
-    agree.  act_round / weight_round (optional callables) emulate the bf16 storage points of the CUDA
-    path (reading B10) for the "bf16-ideal ceiling"; the parity oracle leaves them None.
+    agree.  act_round / weight_round (optional callables) emulate the 16-bit storage points of the CUDA
+    path (reading B10: weight_round = round_bf16; act_round = round_f16, or round_bf16 for the "bf16-ideal
+    ceiling" that motivated fp16 activations); the parity oracle leaves them None.
     """
     x0 = np.asarray(windows, dtype=np.float64)
     outs = []

@@ -86,9 +86,11 @@ def epoch_filter(x, e, cfg: StreamConfig):
     return _wh.design_filter(p, cfg.fs, cfg.welch_nfft, cfg.n_design, cfg.filter_len, cfg.f_lo, cfg.f_hi)
 
 
-def whiten_rolling(x, cfg: StreamConfig, m_lo=None, m_hi=None):
+def whiten_rolling(x, cfg: StreamConfig, m_lo=None, m_hi=None, filters=None):
     """Offline form of O-6 for one channel x[N]: whitened samples for raw indices [m_lo, m_hi)
-    (defaults: everything the streaming rule would have produced).  Returns (y, m_lo)."""
+    (defaults: everything the streaming rule would have produced).  Returns (y, m_lo).
+    filters: optional dict {epoch: taps} of THIS channel, filled on first use, so that many short requests on
+    one record design each epoch's filter once (memoisation only; the arithmetic is epoch_filter's)."""
     x = np.asarray(x, dtype=np.float64)
     half = cfg.filter_len // 2
     n_eff = (x.shape[0] // cfg.stride) * cfg.stride
@@ -102,7 +104,12 @@ def whiten_rolling(x, cfg: StreamConfig, m_lo=None, m_hi=None):
     while m < m_hi:
         e = epoch_of_sample(m, cfg)
         m_next = min(cfg.psd_len + (e + 1) * cfg.psd_update - cfg.stride - half, m_hi)  # first sample of epoch e+1
-        h = epoch_filter(x, e, cfg)
+        if filters is None:
+            h = epoch_filter(x, e, cfg)
+        else:
+            if e not in filters:
+                filters[e] = epoch_filter(x, e, cfg)
+            h = filters[e]
         y[m - m_lo: m_next - m_lo] = _wh.whiten_fir_direct(x[m - half: m_next + half], h)
         m = m_next
     return y, m_lo

@@ -5,5 +5,5 @@ libaframe_b200.so); this package is its thin ctypes binding.  No CPU fallback ex
 """
 from .binding import (  # noqa: F401
     AframeError, Context, Stream, Weights, aframe_config, default_config, load_library, LIB_PATH, EXPORTS,
-    OK, EINVAL, ESHAPE, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED, FP32, BF16,
+    OK, EINVAL, ESHAPE, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED, FP32, BF16, F16,
 )

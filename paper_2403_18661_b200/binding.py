@@ -15,7 +15,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libaframe_b200.so")
 
 OK, EINVAL, ESHAPE, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED = range(7)
-FP32, BF16 = 0, 1
+FP32, BF16, F16 = 0, 1, 2
+_DT = {torch.float32: FP32, torch.bfloat16: BF16, torch.float16: F16}
 _STATUS = {0: "AFRAME_OK", 1: "AFRAME_EINVAL", 2: "AFRAME_ESHAPE", 3: "AFRAME_ENOMEM", 4: "AFRAME_ECUDA",
            5: "AFRAME_ESTATE", 6: "AFRAME_EUNSUPPORTED"}
 
@@ -178,7 +179,7 @@ class Context:
         n_out = max(n - self.cfg.filter_len, 0)
         if out is None:
             out = torch.empty((c, max(n_out, 1)), dtype=out_dtype, device=strain.device)
-        prec = BF16 if out.dtype == torch.bfloat16 else FP32
+        prec = _DT[out.dtype]
         self._check(self.lib.aframe_whiten(self.handle, _ptr(strain), n, strain.stride(0), _ptr(psd), _ptr(out),
                                            out.stride(0), prec))
         return out[:, :n_out]
@@ -193,7 +194,7 @@ class Context:
         c, n = strain.shape
         if out is None:
             out = torch.empty((c, max(n, 1)), dtype=out_dtype, device=strain.device)
-        prec = BF16 if out.dtype == torch.bfloat16 else FP32
+        prec = _DT[out.dtype]
         n_out = C.c_int64(0)
         self._check(self.lib.aframe_whiten_rolling(self.handle, _ptr(strain), n, strain.stride(0), _ptr(out),
                                                    out.stride(0), prec, C.byref(n_out)))
@@ -214,14 +215,14 @@ class Context:
         return scores
 
     def forward_strided(self, weights: Weights, white, first, n_windows, chan_shift=None, scores=None):
-        if not (white.is_cuda and white.is_contiguous() and white.dtype in (torch.float32, torch.bfloat16)):
-            raise TypeError("white: expected a contiguous CUDA tensor of float32 or bfloat16")
+        if not (white.is_cuda and white.is_contiguous() and white.dtype in _DT):
+            raise TypeError("white: expected a contiguous CUDA tensor of float32, bfloat16 or float16")
         if scores is None:
             scores = torch.empty((n_windows,), dtype=torch.float32, device=white.device)
         shifts = None
         if chan_shift is not None:
             shifts = (C.c_int64 * self.cfg.n_channels)(*[int(v) for v in chan_shift])
-        prec = BF16 if white.dtype == torch.bfloat16 else FP32
+        prec = _DT[white.dtype]
         self._check(self.lib.aframe_forward_strided(self.handle, weights.handle, _ptr(white), prec, white.stride(0),
                                                     int(first), shifts, int(n_windows), _ptr(scores)))
         return scores
@@ -268,7 +269,7 @@ class Context:
             raise ValueError("strain must be [B][n_channels][n]")
         n_out = n - int(n_psd) - self.cfg.filter_len
         out = torch.empty((b, c, max(n_out, 1)), dtype=out_dtype, device=strain.device)
-        prec = BF16 if out_dtype == torch.bfloat16 else FP32
+        prec = _DT[out_dtype]
         self._check(self.lib.aframe_whiten_batch(self.handle, _ptr(strain), b, n, int(n_psd), _ptr(out), prec))
         return out
 

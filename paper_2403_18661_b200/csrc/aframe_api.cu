@@ -26,7 +26,7 @@ AF_API aframe_status aframe_config_default(aframe_config* cfg) {
   cfg->psd_len = 131072;
   cfg->psd_update = 16384;
   cfg->strain_scale_log2 = 70;
-  cfg->precision = AFRAME_BF16;
+  cfg->precision = AFRAME_F16;
   return AFRAME_OK;
 }
 
@@ -68,7 +68,8 @@ AF_API aframe_status aframe_create(const aframe_config* cfg, void* cuda_stream, 
   if (cfg->psd_update < 1 || cfg->psd_update % cfg->welch_hop || cfg->psd_update % cfg->stride) return AFRAME_ESHAPE;
   if (cfg->psd_len % cfg->stride) return AFRAME_ESHAPE;
   if (cfg->strain_scale_log2 < -120 || cfg->strain_scale_log2 > 120) return AFRAME_EINVAL;
-  if (cfg->precision != AFRAME_FP32 && cfg->precision != AFRAME_BF16) return AFRAME_EINVAL;
+  if (cfg->precision == AFRAME_BF16) return AFRAME_EUNSUPPORTED;   // bf16 storage cannot meet the rank tolerance (aframe.h)
+  if (cfg->precision != AFRAME_FP32 && cfg->precision != AFRAME_F16) return AFRAME_EINVAL;
   if ((cfg->welch_average != 0 && cfg->welch_average != 1) || cfg->reserved_ != 0) return AFRAME_EINVAL;
   if (cfg->welch_average == 1 && (cfg->psd_len - cfg->welch_nfft) / cfg->welch_hop + 1 > 255) return AFRAME_EUNSUPPORTED;
 
@@ -114,7 +115,7 @@ AF_API aframe_status aframe_create(const aframe_config* cfg, void* cuda_stream, 
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ctx->encode_tiled, cudaEnableDefault, &qres) != cudaSuccess ||
         qres != cudaDriverEntryPointSuccess) {
       cudaGetLastError();
-      ctx->encode_tiled = nullptr;   // bf16 path will report EUNSUPPORTED
+      ctx->encode_tiled = nullptr;   // the tensor-core path will report EUNSUPPORTED
     }
     if (cudaDeviceSynchronize() != cudaSuccess) { st = AFRAME_ECUDA; break; }
   } while (0);
@@ -163,7 +164,7 @@ AF_API aframe_status aframe_whiten(aframe_ctx* ctx, const float* d_strain, int64
                                        const float* d_psd, void* d_out, int64_t ld_out, aframe_precision out_dtype) {
   if (!ctx) return AFRAME_EINVAL;
   if (!d_strain || !d_psd || !d_out) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
-  if (out_dtype != AFRAME_FP32 && out_dtype != AFRAME_BF16) return af_fail(ctx, AFRAME_EINVAL, "bad out_dtype");
+  if (out_dtype != AFRAME_FP32 && out_dtype != AFRAME_BF16 && out_dtype != AFRAME_F16) return af_fail(ctx, AFRAME_EINVAL, "bad out_dtype");
   const aframe_config& cfg = ctx->cfg;
   if (n_samples < 0 || ld < n_samples) return af_fail(ctx, AFRAME_ESHAPE, "ld < n_samples");
   const int64_t n_out = n_samples - cfg.filter_len;
@@ -174,7 +175,7 @@ AF_API aframe_status aframe_whiten(aframe_ctx* ctx, const float* d_strain, int64
   st = af_launch_filter_design(ctx, d_psd, 1, H, ctx->d_taps_last);
   if (st != AFRAME_OK) return st;
   if (n_out <= 0) return AFRAME_OK;
-  return af_launch_whiten_os(ctx, d_strain, n_samples, ld, H, 0, n_out, n_out, 1, d_out, ld_out, out_dtype == AFRAME_BF16);
+  return af_launch_whiten_os(ctx, d_strain, n_samples, ld, H, 0, n_out, n_out, 1, d_out, ld_out, (int)out_dtype);
 }
 
 // ---- NEXT-4: training-time whitening batch --------------------------------------------------
@@ -182,7 +183,7 @@ AF_API aframe_status aframe_whiten_batch(aframe_ctx* ctx, const float* d_strain,
                                              int64_t n_psd, void* d_out, aframe_precision out_dtype) {
   if (!ctx) return AFRAME_EINVAL;
   if (!d_strain || !d_out) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
-  if (out_dtype != AFRAME_FP32 && out_dtype != AFRAME_BF16) return af_fail(ctx, AFRAME_EINVAL, "bad out_dtype");
+  if (out_dtype != AFRAME_FP32 && out_dtype != AFRAME_BF16 && out_dtype != AFRAME_F16) return af_fail(ctx, AFRAME_EINVAL, "bad out_dtype");
   const aframe_config& cfg = ctx->cfg;
   if (n_batch < 1) return af_fail(ctx, AFRAME_EINVAL, "n_batch < 1");
   const int64_t rows = n_batch * cfg.n_channels;
@@ -203,7 +204,7 @@ AF_API aframe_status aframe_whiten_batch(aframe_ctx* ctx, const float* d_strain,
   if (st == AFRAME_OK) st = af_launch_psd_mean(ctx, pg, n_seg, 0, 1, n_seg, psd);
   if (st == AFRAME_OK) st = af_launch_filter_design(ctx, psd, 1, H, nullptr);
   if (st == AFRAME_OK)
-    st = af_launch_whiten_os(ctx, d_strain + n_psd, n_w, n_samples, H, 0, n_out, n_out, 1, d_out, n_out, out_dtype == AFRAME_BF16);
+    st = af_launch_whiten_os(ctx, d_strain + n_psd, n_w, n_samples, H, 0, n_out, n_out, 1, d_out, n_out, (int)out_dtype);
   ctx->n_ch_batch = 0;
   return st;
 }
@@ -221,7 +222,7 @@ AF_API aframe_status aframe_whiten_rolling(aframe_ctx* ctx, const float* d_strai
                                                void* d_out, int64_t ld_out, aframe_precision out_dtype, int64_t* h_n_out) {
   if (!ctx) return AFRAME_EINVAL;
   if (!d_strain || !d_out || !h_n_out) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
-  if (out_dtype != AFRAME_FP32 && out_dtype != AFRAME_BF16) return af_fail(ctx, AFRAME_EINVAL, "bad out_dtype");
+  if (out_dtype != AFRAME_FP32 && out_dtype != AFRAME_BF16 && out_dtype != AFRAME_F16) return af_fail(ctx, AFRAME_EINVAL, "bad out_dtype");
   const aframe_config& cfg = ctx->cfg;
   *h_n_out = 0;
   if (n_samples < 0 || ld < n_samples) return af_fail(ctx, AFRAME_ESHAPE, "ld < n_samples");
@@ -254,7 +255,7 @@ AF_API aframe_status aframe_whiten_rolling(aframe_ctx* ctx, const float* d_strai
   st = af_launch_filter_design(ctx, psd, n_epochs, H, nullptr);
   if (st != AFRAME_OK) return st;
   st = af_launch_whiten_os(ctx, d_strain, n_samples, ld, H, m0 - half, n_out, cfg.psd_update, n_epochs, d_out, ld_out,
-                           out_dtype == AFRAME_BF16);
+                           (int)out_dtype);
   if (st != AFRAME_OK) return st;
   *h_n_out = n_out;
   return AFRAME_OK;
@@ -265,7 +266,7 @@ AF_API void aframe_weights_free(aframe_weights* w) {
   if (!w) return;
   if (w->ctx) { cudaStreamSynchronize(w->ctx->stream); af_tc_forget(w->ctx); }
   for (float* p : w->d_w32) cudaFree(p);
-  for (__nv_bfloat16* p : w->d_w16) cudaFree(p);
+  for (af_act_t* p : w->d_w16) cudaFree(p);
   for (float* p : w->d_bias) cudaFree(p);
   for (float* p : w->d_bias_sc) cudaFree(p);
   for (float* p : w->d_gamma) cudaFree(p);
@@ -358,7 +359,7 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
     pos += nw + 2 * (size_t)l.c_out + 2 * (size_t)n_stat;
     // fold the frozen norm (reading B6) in double: W' = a_c W, b' = beta_c - mu_g a_c
     std::vector<float> w32(nw), bias(l.c_out);
-    std::vector<__nv_bfloat16> w16(nw);
+    std::vector<__half> w16(nw);
     for (int co = 0; co < l.c_out; ++co) {
       const int g = norm_kind == 0 ? co : co / (l.c_out / (int)n_groups);
       // frozen norm: fold; true GroupNorm: the conv stays as it is (the norm kernels apply gamma / beta)
@@ -368,7 +369,7 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
         for (int d = 0; d < l.k; ++d) {
           const float v = (float)((double)W[((size_t)co * l.c_in + ci) * l.k + d] * a);
           w32[((size_t)d * l.c_in + ci) * l.c_out + co] = v;                      // [k][c_in][c_out]
-          w16[((size_t)d * l.c_out + co) * l.c_in + ci] = __float2bfloat16_rn(v);  // [k][c_out][c_in]
+          w16[((size_t)d * l.c_out + co) * l.c_in + ci] = __float2half_rn(fminf(fmaxf(v, -65504.f), 65504.f));  // [k][c_out][c_in]
         }
     }
     if (cudaMalloc(&w->d_w32[i], sizeof(float) * nw) != cudaSuccess || cudaMalloc(&w->d_w16[i], 2 * nw) != cudaSuccess ||
@@ -404,14 +405,14 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
 }
 
 // ---- O-5 ------------------------------------------------------------------------------------------
-static aframe_status forward_common(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_bf16, int64_t sB,
+static aframe_status forward_common(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_dt, int64_t sB,
                                     const int64_t* choff, int64_t B, float* d_scores) {
   if (w->ctx != ctx) return af_fail(ctx, AFRAME_ESTATE, "weights belong to another context");
-  if (ctx->cfg.precision == AFRAME_BF16) {
-    if (!w->tc_ok) return af_fail(ctx, AFRAME_EUNSUPPORTED, "bf16 tensor-core path unavailable: %s", w->tc_reason.c_str());
-    return af_forward_bf16(ctx, w, d_in, in_bf16, sB, 1, choff, B, d_scores);
+  if (ctx->cfg.precision == AFRAME_F16) {
+    if (!w->tc_ok) return af_fail(ctx, AFRAME_EUNSUPPORTED, "fp16 tensor-core path unavailable: %s", w->tc_reason.c_str());
+    return af_forward_bf16(ctx, w, d_in, in_dt, sB, 1, choff, B, d_scores);
   }
-  return af_forward_fp32(ctx, w, d_in, in_bf16, sB, 1, choff, B, d_scores);
+  return af_forward_fp32(ctx, w, d_in, in_dt, sB, 1, choff, B, d_scores);
 }
 
 AF_API aframe_status aframe_forward(aframe_ctx* ctx, const aframe_weights* w, const float* d_windows, int64_t B,
@@ -430,7 +431,7 @@ AF_API aframe_status aframe_forward_strided(aframe_ctx* ctx, const aframe_weight
   if (!ctx) return AFRAME_EINVAL;
   if (!w || !d_white || !d_scores) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
   if (B <= 0) return af_fail(ctx, AFRAME_EINVAL, "B must be positive");
-  if (dtype != AFRAME_FP32 && dtype != AFRAME_BF16) return af_fail(ctx, AFRAME_EINVAL, "bad dtype");
+  if (dtype != AFRAME_FP32 && dtype != AFRAME_BF16 && dtype != AFRAME_F16) return af_fail(ctx, AFRAME_EINVAL, "bad dtype");
   if (first < 0) return af_fail(ctx, AFRAME_EINVAL, "first must be non-negative");
   int64_t choff[AF_MAX_CH] = {0};
   for (int c = 0; c < ctx->cfg.n_channels; ++c) {
@@ -439,7 +440,7 @@ AF_API aframe_status aframe_forward_strided(aframe_ctx* ctx, const aframe_weight
       return af_fail(ctx, AFRAME_ESHAPE, "windows reach outside the whitened stream (ld)");
     choff[c] = (int64_t)c * ld + first + sh;
   }
-  return forward_common(ctx, w, d_white, dtype == AFRAME_BF16, ctx->cfg.stride, choff, B, d_scores);
+  return forward_common(ctx, w, d_white, (int)dtype, ctx->cfg.stride, choff, B, d_scores);
 }
 
 // ---- per-stage device timing --------------------------------------------------------------------------
@@ -506,13 +507,14 @@ static aframe_status score_timeslides_dev(aframe_ctx* ctx, const aframe_weights*
   if (n_windows <= 0 || n_slides <= 0 || batch <= 0) return af_fail(ctx, AFRAME_EINVAL, "n_windows, n_slides, batch must be positive");
   if (first < 0) return af_fail(ctx, AFRAME_EINVAL, "first must be non-negative");
   if (w->ctx != ctx) return af_fail(ctx, AFRAME_ESTATE, "weights belong to another context");
-  const int bf16 = cfg.precision == AFRAME_BF16;
-  const size_t esz = bf16 ? 2 : 4;
+  // whitened stream in the network's input precision
+  const aframe_precision wdt = cfg.precision == AFRAME_F16 ? AFRAME_F16 : AFRAME_FP32;
+  const size_t esz = af_dt_bytes((int)wdt);
   const int64_t ld_w = (n_samples + 63) & ~(int64_t)63;
   aframe_status st = af_ws_reserve(ctx, ctx->ws_white, esz * (size_t)C * ld_w);
   if (st != AFRAME_OK) return st;
   int64_t n_out = 0;
-  st = aframe_whiten_rolling(ctx, d_strain, n_samples, ld, ctx->ws_white.ptr, ld_w, bf16 ? AFRAME_BF16 : AFRAME_FP32, &n_out);
+  st = aframe_whiten_rolling(ctx, d_strain, n_samples, ld, ctx->ws_white.ptr, ld_w, wdt, &n_out);
   if (st != AFRAME_OK) return st;
   int64_t sh_min = 0, sh_max = 0;
   for (int k = 0; k < n_slides; ++k) {
@@ -527,7 +529,7 @@ static aframe_status score_timeslides_dev(aframe_ctx* ctx, const aframe_weights*
     for (int c = 1; c < C; ++c) shifts[c] = h_slide_shifts[k];
     for (int64_t i0 = 0; i0 < n_windows; i0 += batch) {
       const int64_t nb = n_windows - i0 < batch ? n_windows - i0 : batch;
-      st = aframe_forward_strided(ctx, w, ctx->ws_white.ptr, bf16 ? AFRAME_BF16 : AFRAME_FP32, ld_w,
+      st = aframe_forward_strided(ctx, w, ctx->ws_white.ptr, wdt, ld_w,
                                   first + i0 * cfg.stride, shifts, nb, d_scores + (int64_t)k * n_windows + i0);
       if (st != AFRAME_OK) return st;
     }
@@ -574,7 +576,7 @@ AF_API aframe_status aframe_profile_layers(aframe_ctx* ctx, const aframe_weights
   if (!ctx) return AFRAME_EINVAL;
   if (!w || !d_windows || !d_scores || !h_ms) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
   if (n_layers != (int32_t)w->layers.size()) return af_fail(ctx, AFRAME_ESHAPE, "n_layers does not match the layer table");
-  if (ctx->cfg.precision != AFRAME_BF16) return af_fail(ctx, AFRAME_EUNSUPPORTED, "per-layer timing is built for the bf16 path");
+  if (ctx->cfg.precision != AFRAME_F16) return af_fail(ctx, AFRAME_EUNSUPPORTED, "per-layer timing is built for the tensor-core path");
   for (int i = 0; i < n_layers; ++i) h_ms[i] = 0.f;
   ctx->layer_ms = h_ms;
   aframe_status st = aframe_forward(ctx, w, d_windows, B, d_scores);

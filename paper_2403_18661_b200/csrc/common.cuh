@@ -3,6 +3,7 @@
 
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <stdint.h>
 #include <stdio.h>
 #include <string>
@@ -15,6 +16,31 @@
 #define AF_API extern "C" __attribute__((visibility("default")))
 #else
 #define AF_API extern "C"
+#endif
+
+// Storage types (values of aframe_precision): fp32, bf16, fp16.
+enum { AF_DT_F32 = 0, AF_DT_BF16 = 1, AF_DT_F16 = 2 };
+static inline size_t af_dt_bytes(int dt) { return dt == AF_DT_F32 ? 4 : 2; }
+
+// Weights and activations of the tensor-core path are stored as IEEE half (reading B10 of DESIGN.md: with one bf16
+// rounding per stored activation the scores lose their rank order -- Spearman 0.9987 against the float64 oracle on
+// configs[1], the ceiling of that format -- while fp16's three extra mantissa bits give > 0.9999 at the same bytes and
+// the same tcgen05 kind::f16 rate; the instruction wants A and B in ONE format: a mixed fp16 x bf16 descriptor raises
+// an illegal-instruction fault on B200).  Conversions round to nearest even and saturate at +-65504 (NaN stays NaN).
+typedef __half af_act_t;
+#ifdef __CUDACC__
+__device__ __forceinline__ uint32_t af_act_pack2(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+__device__ __forceinline__ float2 af_act_unpack2(uint32_t w) { return __half22float2(*reinterpret_cast<const __half2*>(&w)); }
+// one element of a whitened stream / window tensor of storage type DT -> fp32
+template <int DT> __device__ __forceinline__ float af_ld_as_f32(const void* p, int64_t i) {
+  if (DT == AF_DT_BF16) return __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(p)[i]);
+  if (DT == AF_DT_F16) return __half2float(reinterpret_cast<const __half*>(p)[i]);
+  return __ldg(reinterpret_cast<const float*>(p) + i);
+}
 #endif
 
 struct LayerDesc {
@@ -30,7 +56,7 @@ struct aframe_weights {
   int kernel_len = 0;
   // per conv layer (index = layer index; null for other kinds)
   std::vector<float*> d_w32;          // [k][c_in][c_out] fp32 (N contiguous) for the CUDA-core path
-  std::vector<__nv_bfloat16*> d_w16;  // [k][c_out][c_in] bf16 (K-major) for the tcgen05 path
+  std::vector<af_act_t*> d_w16;       // [k][c_out][c_in] fp16 (K-major) for the tcgen05 path
   std::vector<float*> d_bias;         // [c_out] fp32 folded bias
   std::vector<float*> d_bias_sc;      // conv whose residual is a 1x1 projection conv: its bias + the projection's (else null)
   float* d_head_w = nullptr;          // [c_in]
@@ -140,11 +166,11 @@ aframe_status af_launch_filter_design(aframe_ctx* ctx, const float* d_psd, int64
                                       float* d_taps /*[E][C][L+1] or null*/, const StreamGate* gate = nullptr);
 aframe_status af_launch_whiten_os(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
                                   const float* d_H, int64_t in0, int64_t out_total, int64_t epoch_len, int64_t n_epochs,
-                                  void* d_out, int64_t ld_out, int out_bf16);
+                                  void* d_out, int64_t ld_out, int out_dt);
 
-aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_bf16,
+aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_dt,
                               int64_t sB, int64_t sT, const int64_t* choff, int64_t B, float* d_scores);
-aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_bf16,
+aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_dt,
                               int64_t sB, int64_t sT, const int64_t* choff, int64_t B, float* d_scores);
 aframe_status af_tc_check(aframe_ctx* ctx, aframe_weights* w);
 void af_tc_forget(aframe_ctx* ctx);

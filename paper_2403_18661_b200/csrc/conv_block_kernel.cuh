@@ -7,10 +7,10 @@
 // Tile = 126 output rows of one window.  Per tile:
 //   X  : one TMA box of 130 input rows (t0 - 2 .. t0 + 127, out-of-range rows zero-filled), SWIZZLE_128B
 //   MMA_a (M128 N64 K16 x 12): tap d reads X through a descriptor shifted by d rows  -> acc_a row r = y1[t0 - 1 + r]
-//   epilogue A : acc_a + ba -> ReLU -> zero the rows outside the window -> bf16 -> Y tile in shared memory (same
+//   epilogue A : acc_a + ba -> fp16 -> ReLU -> zero the rows outside the window -> Y tile in shared memory (same
 //                swizzled layout, i.e. directly an A operand)
 //   MMA_b : tap d reads Y shifted by d rows                                          -> acc_b row r = y2[t0 + r], r < 126
-//   epilogue B : acc_b + bb + x (X rows r + 2, still in shared memory) -> ReLU -> bf16 -> staging -> TMA store (126 rows)
+//   epilogue B : acc_b + bb + x (X rows r + 2, still in shared memory) -> fp16 -> ReLU -> staging -> TMA store (126 rows)
 // HBM traffic per block: x read once, y2 written once (the unfused pair reads 3 tensors and writes 2).
 // Both weight sets (2 x 24 KB) stay resident.  Rings: X (NX slots), Y (NY), staging (NO); TMEM: 2 + 2 accumulators.
 //
@@ -31,11 +31,13 @@ struct TcBlockParams {
   int reverse;           // walk the tiles from the last to the first
   // shared stem (stem_bf16.cu): tm_x is a strided view of the stem of the whole stream; rows 0, 1 and T - 1 of every window
   // are overwritten in shared memory with the window's own edge rows [windows][3][64] before the tile is used (null = off)
-  const __nv_bfloat16* edge;
+  const af_act_t* edge;
   // shared stage (conv_tc.cu): a batch of short windows stored back to back, zero_valid data rows + separator rows per
   // zero_period rows: y1 is forced to zero on the separators so that they act as each short window's zero padding
   int zero_period, zero_valid;   // 0 = off
-  long long* dbg_out;    // timing experiments: per-role cycle counters of CTA 0 (null = off)
+#ifdef AFRAME_TC_CYCLES
+  long long* dbg_out;    // experiments build only: per-role cycle counters of CTA 0 (null = off)
+#endif
 };
 
 #define TCB_ROWS 126
@@ -101,10 +103,15 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
     t0 = i * TCB_ROWS;
   };
   const int first = blockIdx.x, step = gridDim.x;
+#ifdef AFRAME_TC_CYCLES
   const bool prof = p.dbg_out != nullptr && blockIdx.x == 0;
   long long tprev = prof ? clock64() : 0, tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   auto T = [&](int slot) { if (prof) { const long long t = clock64(); tacc[slot] += t - tprev; tprev = t; } };
   auto Tflush = [&](int role) { if (prof) for (int i = 0; i < 8; ++i) p.dbg_out[role * 8 + i] = tacc[i]; };
+#else
+  auto T = [](int) {};
+  auto Tflush = [](int) {};
+#endif
 
   if (warp == 0) {
     // ===== TMA producer =====
@@ -176,7 +183,7 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
     if (lane == 0) Tflush(0);
   } else if (warp == 1) {
     // ===== MMA issuer (whole warp runs the uniform loop, one elected lane issues) =====
-    constexpr uint32_t idesc = umma_idesc_bf16_mn(128, 64);
+    constexpr uint32_t idesc = umma_idesc_f16_mn(128, 64);
     mbar_wait(w_bar, 0);
     int n_my = 0;
     for (int tile = first; tile < p.num_tiles; tile += step) ++n_my;
@@ -196,10 +203,10 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
           if (elect_one()) {
             const uint32_t d_tmem = tmem_base + (uint32_t)(as * 64);
             const uint32_t a_lo = xs_lo + (uint32_t)xs * (TCB_SLOT >> 4);
-            umma_bf16_lohi<false>(d_tmem, a_lo, wa_lo, idesc);
+            umma_mma_lohi<false>(d_tmem, a_lo, wa_lo, idesc);
 #pragma unroll
             for (int m = 1; m < 12; ++m)           // tap d = m / 4 (8 = one 128-byte row), K step k = m % 4 (2 = 32 bytes)
-              umma_bf16_lohi<true>(d_tmem, a_lo + (m / 4) * 8 + (m % 4) * 2, wa_lo + (m / 4) * 512 + (m % 4) * 2, idesc);
+              umma_mma_lohi<true>(d_tmem, a_lo + (m / 4) * 8 + (m % 4) * 2, wa_lo + (m / 4) * 512 + (m % 4) * 2, idesc);
             umma_commit(a_full(as));
             umma_commit(x_empty(xs));              // first of the slot's two releases
           }
@@ -216,10 +223,10 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
           if (elect_one()) {
             const uint32_t d_tmem = tmem_base + (uint32_t)(128 + bs * 64);
             const uint32_t a_lo = ys_lo + (uint32_t)ys * (TCB_SLOT >> 4);
-            umma_bf16_lohi<false>(d_tmem, a_lo, wb_lo, idesc);
+            umma_mma_lohi<false>(d_tmem, a_lo, wb_lo, idesc);
 #pragma unroll
             for (int m = 1; m < 12; ++m)
-              umma_bf16_lohi<true>(d_tmem, a_lo + (m / 4) * 8 + (m % 4) * 2, wb_lo + (m / 4) * 512 + (m % 4) * 2, idesc);
+              umma_mma_lohi<true>(d_tmem, a_lo + (m / 4) * 8 + (m % 4) * 2, wb_lo + (m / 4) * 512 + (m % 4) * 2, idesc);
             umma_commit(b_full(bs));
             umma_commit(y_empty(ys));
           }
@@ -236,7 +243,12 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
     const int row = q * 32 + lane;
     const bool grp_b = warp >= 10;
     const int g = ((warp - 2) >> 2) & 1;           // group of its kind: tiles g, g + 2, ...
-    const __nv_bfloat162 z2 = __float2bfloat162_rn(0.f);
+    const __half2 z2 = __float2half2_rn(0.f);
+    auto pack_relu = [&](float a, float b) -> uint32_t {   // fp16 (RNE, saturating), then ReLU
+      const uint32_t pk = af_act_pack2(a, b);
+      const __half2 m = __hmax2(*reinterpret_cast<const __half2*>(&pk), z2);
+      return *reinterpret_cast<const uint32_t*>(&m);
+    };
     if (!grp_b) {
       // ===== epilogue A: acc_a -> y1 tile (an A operand of conv_b) =====
       const float4* bias4 = reinterpret_cast<const float4*>(s_ba);
@@ -268,11 +280,10 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
         for (int jj = 0; jj < 8; ++jj) {
           const float4 bA = bias4[2 * jj], bB = bias4[2 * jj + 1];
           uint4 o;
-          __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(&o);
-          ob[0] = __hmax2(__floats2bfloat162_rn(__uint_as_float(v[8 * jj + 0]) + bA.x, __uint_as_float(v[8 * jj + 1]) + bA.y), z2);
-          ob[1] = __hmax2(__floats2bfloat162_rn(__uint_as_float(v[8 * jj + 2]) + bA.z, __uint_as_float(v[8 * jj + 3]) + bA.w), z2);
-          ob[2] = __hmax2(__floats2bfloat162_rn(__uint_as_float(v[8 * jj + 4]) + bB.x, __uint_as_float(v[8 * jj + 5]) + bB.y), z2);
-          ob[3] = __hmax2(__floats2bfloat162_rn(__uint_as_float(v[8 * jj + 6]) + bB.z, __uint_as_float(v[8 * jj + 7]) + bB.w), z2);
+          o.x = pack_relu(__uint_as_float(v[8 * jj + 0]) + bA.x, __uint_as_float(v[8 * jj + 1]) + bA.y);
+          o.y = pack_relu(__uint_as_float(v[8 * jj + 2]) + bA.z, __uint_as_float(v[8 * jj + 3]) + bA.w);
+          o.z = pack_relu(__uint_as_float(v[8 * jj + 4]) + bB.x, __uint_as_float(v[8 * jj + 5]) + bB.y);
+          o.w = pack_relu(__uint_as_float(v[8 * jj + 6]) + bB.z, __uint_as_float(v[8 * jj + 7]) + bB.w);
           if (!inside) o = make_uint4(0u, 0u, 0u, 0u);
           *reinterpret_cast<uint4*>(rowp + ((jj ^ (row & 7)) << 4)) = o;
         }
@@ -284,7 +295,7 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
       }
       if (((warp - 2) & 3) == 0 && lane == 0) Tflush(2 + g);
     } else {
-      // ===== epilogue B: acc_b + bias + x -> ReLU -> bf16 -> staging -> TMA store of 126 rows =====
+      // ===== epilogue B: acc_b + bias + x -> fp16 -> ReLU -> staging -> TMA store of 126 rows =====
       const float4* bias4 = reinterpret_cast<const float4*>(s_bb);
       const bool leader = ((warp - 2) & 3) == 0 && lane == 0;
       const uint32_t og_base = os_base + (uint32_t)(g * NO) * TC_OUT_BYTES;   // this group's staging slots
@@ -324,11 +335,12 @@ conv_block_kernel(const __grid_constant__ CUtensorMap tm_x, const __grid_constan
           f[4] = __uint_as_float(v[8 * jj + 4]) + bB.x; f[5] = __uint_as_float(v[8 * jj + 5]) + bB.y;
           f[6] = __uint_as_float(v[8 * jj + 6]) + bB.z; f[7] = __uint_as_float(v[8 * jj + 7]) + bB.w;
           uint4 o;
-          __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(&o);
+          uint32_t* ow = reinterpret_cast<uint32_t*>(&o);
 #pragma unroll
-          for (int e = 0; e < 4; ++e)
-            ob[e] = __hmax2(__floats2bfloat162_rn(f[2 * e] + __uint_as_float(rw[e] << 16),
-                                                  f[2 * e + 1] + __uint_as_float(rw[e] & 0xffff0000u)), z2);
+          for (int e = 0; e < 4; ++e) {
+            const float2 xr2 = af_act_unpack2(rw[e]);
+            ow[e] = pack_relu(f[2 * e] + xr2.x, f[2 * e + 1] + xr2.y);
+          }
           *reinterpret_cast<uint4*>(orow + ((jj ^ (row & 7)) << 4)) = o;
         }
         T(4);

@@ -1,5 +1,4 @@
-// Host side of the bf16 tensor-core network path: TMA tensor maps, per-layer launches, forward driver.
-#include <stdlib.h>
+// Host side of the tensor-core network path (fp16 weights and activations, fp32 accumulation): TMA tensor maps, per-layer launches, forward driver.
 #include <map>
 
 #include "conv_tc_kernel.cuh"
@@ -20,7 +19,7 @@ static bool encode_map(aframe_ctx* ctx, CUtensorMap* m, const void* ptr, int ran
   for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; es[i] = 1; }
   for (int i = 0; i < rank - 1; ++i) gs[i] = strides_bytes[i];
   EncodeTiledFn fn = reinterpret_cast<EncodeTiledFn>(ctx->encode_tiled);
-  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, const_cast<void*>(ptr), gd, gs, bx, es,
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, (cuuint32_t)rank, const_cast<void*>(ptr), gd, gs, bx, es,
                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
@@ -46,11 +45,6 @@ __global__ void head_finish_kernel(const float* __restrict__ part, int n_part, f
   float s = 0.f;
   for (int i = 0; i < n_part; ++i) s += part[b * n_part + i];
   scores[b] = s * inv_t + bias;
-}
-
-static int env_int(const char* name, int dflt) {
-  const char* e = getenv(name);
-  return e ? atoi(e) : dflt;
 }
 
 static int tile_t_box(int t_out) {
@@ -104,26 +98,24 @@ struct TcShapeOverride {
   int t_out; int zero_period, zero_valid, zero_origin;
   int e_nbp = 0, e_P = 0, e_tbox = 0, e_T = 0, e_head = 0, e_tail = 0;
   int64_t e_shift = 0, e_nb = 0;
-  const __nv_bfloat16* e_stream = nullptr;
+  const af_act_t* e_stream = nullptr;
   bool head_rows = false;     // with head = true: per-row head dot products into head_part (TcConvParams::head_rows)
   bool pair_plan = false;     // one shared-memory plan for every launch of the stage, so that two of them can share a launch
 };
-static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const __nv_bfloat16* in,
-                         const __nv_bfloat16* res, __nv_bfloat16* out, int64_t nb, bool head, float* head_part,
-                         TcLaunch& L, int sc = -1, const __nv_bfloat16* sc_in = nullptr, const TcShapeOverride* ov = nullptr) {
+static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const af_act_t* in,
+                         const af_act_t* res, af_act_t* out, int64_t nb, bool head, float* head_part,
+                         TcLaunch& L, int sc = -1, const af_act_t* sc_in = nullptr, const TcShapeOverride* ov = nullptr) {
   LayerDesc l = w->layers[li];
   const bool packed = ov && ov->e_nbp > 0;
   if (packed) { nb = 2 * ov->e_nbp; l.t_out = ov->e_P; l.t_in = ov->e_P * l.stride; }
   else if (ov) { nb = 1; l.t_out = ov->t_out; l.t_in = ov->t_out * l.stride; }
   const int BN = l.c_out >= 256 ? 256 : l.c_out;
-  const int cg2_mode = env_int("AFRAME_CG2", 1);                 // 1: CTA pairs (cta_group::2) for the N = 256 layers; 2: also N = 128
-  const bool cg2 = (BN == 256 && cg2_mode != 0) || (BN == 128 && cg2_mode >= 2);
+  const bool cg2 = BN == 256;                                    // CTA pairs (cta_group::2) for the N = 256 layers
   const int T_box = packed ? ov->e_tbox : tile_t_box(l.t_out), B_box = 128 / T_box;
   const int P = l.stride;
   const bool has_res = res != nullptr;
   // resident weights + one halo box per tile (see TcConvParams): stride-1 k3 layers whose tiles stay inside a window
-  bool halo = !head && !cg2 && l.k == 3 && l.stride == 1 && l.pad == 1 && T_box == 128 && BN == l.c_out && BN <= 128 &&
-              env_int("AFRAME_HALO", 1) != 0;
+  bool halo = !head && !cg2 && l.k == 3 && l.stride == 1 && l.pad == 1 && T_box == 128 && BN == l.c_out && BN <= 128;
   {
     const uint64_t dims[4] = {(uint64_t)l.c_in, (uint64_t)P, (uint64_t)(l.t_in / P), (uint64_t)nb};
     const uint64_t str[3] = {(uint64_t)l.c_in * 2, (uint64_t)P * l.c_in * 2, (uint64_t)l.t_in * l.c_in * 2};
@@ -159,7 +151,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   TcConvParams& p = L.p;
   p.bias = sc >= 0 ? w->d_bias_sc[li] : w->d_bias[li];
   p.sc_kblocks = sc >= 0 ? w->layers[sc].c_in / 64 : 0;
-  p.gn_part = nullptr; p.gn_unit = 64; p.out_f16 = 0;
+  p.gn_part = nullptr; p.gn_unit = 64;
   p.zero_period = ov ? ov->zero_period : 0; p.zero_valid = ov ? ov->zero_valid : 0; p.zero_origin = ov ? ov->zero_origin : 0;
   p.taps = l.k; p.pad = l.pad; p.P = P;
   for (int d = 0; d < 3; ++d) {
@@ -193,20 +185,12 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.head_slabs = l.t_out / 32;
   p.head_rows = (head && ov && ov->head_rows) ? 1 : 0; p.head_row_stride = l.t_out;
   p.nb = packed ? ov->e_nb : nb;
-  p.dbg_out = nullptr;
-  if (env_int("AFRAME_TC_PROF", 0)) {       // experiment: per-role cycle counters, 32 slots per layer, read back by the caller
-    static long long* d_prof = nullptr;
-    if (!d_prof) { cudaMalloc(&d_prof, sizeof(long long) * 32 * 64); cudaMemset(d_prof, 0, sizeof(long long) * 32 * 64); }
-    p.dbg_out = d_prof + 32 * li;
-    if (const char* f = getenv("AFRAME_TC_PROF_PTR")) { FILE* fp = fopen(f, "w"); if (fp) { fprintf(fp, "%llu\n", (unsigned long long)(uintptr_t)d_prof); fclose(fp); } }
-  }
   // shared-memory plan (227 KB per CTA): main-loop ring depth vs epilogue staging / residual prefetch buffers
   // (two epilogue groups: EG * nbuf staging buffers of 16 KB; a residual tile is prefetched pf chunks ahead into the
   //  buffer its chunk's output is staged in)
   const bool r = p.has_res;
   if (cg2 && !head && BN == 256 && ov && ov->pair_plan) { p.stages = 5; p.nbuf = 2; p.pf = 1; }
   else if (cg2 && head)       { p.stages = 5; p.nbuf = 1; p.pf = 0; }
-  else if (cg2 && BN == 128)  { p.stages = r ? 5 : 6; p.nbuf = r ? 3 : 2; p.pf = r ? 1 : 0; }   // 24 KB stages
   else if (cg2 && l.k * p.kblocks < 12) { p.stages = 5; p.nbuf = 2; p.pf = r ? 1 : 0; }   // short K: the epilogue is the critical path
   else if (cg2)               { p.stages = r ? 5 : 6; p.nbuf = r ? 2 : 1; p.pf = r ? 1 : 0; }
   else if (BN == 256)         { p.stages = 3; p.nbuf = 2; p.pf = r ? 1 : 0; }
@@ -223,7 +207,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   L.head = head;
   L.cg2 = cg2;
   L.halo = halo;
-  L.smem = (cg2 && BN == 128) ? TcCfg<128, true>::smem(p.stages, p.nbuf, false) : halo ? (BN == 128 ? TcCfg<128>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks) : TcCfg<64>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks)) + p.sc_kblocks * BN * 128
+  L.smem = halo ? (BN == 128 ? TcCfg<128>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks) : TcCfg<64>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks)) + p.sc_kblocks * BN * 128
          : cg2 ? TcCfg<256, true>::smem(p.stages, p.nbuf, head) : BN == 256 ? TcCfg<256>::smem(p.stages, p.nbuf, head) : (BN == 128 ? TcCfg<128>::smem(p.stages, p.nbuf, head)
                                                                             : TcCfg<64>::smem(p.stages, p.nbuf, head));
   if (cg2) L.grid = 2 * (p.num_tiles < ctx->n_sms / 2 ? p.num_tiles : ctx->n_sms / 2);
@@ -251,8 +235,7 @@ template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t lau
   at[0].val.clusterDim.x = CG2 ? 2 : 1; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
   at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // the kernel orders itself with griddepcontrol.wait
   at[1].val.programmaticStreamSerializationAllowed = 1;
-  static const int pdl = env_int("AFRAME_PDL", 1);
-  cfg.attrs = at; cfg.numAttrs = pdl ? 2 : 1;
+  cfg.attrs = at; cfg.numAttrs = 2;
   const TcLaunch& L1 = second ? *second : L;        // second problem of the launch (conv_tc_kernel), or none
   TcConvParams p1 = L1.p;
   if (!second) p1.num_tiles = 0;
@@ -262,7 +245,6 @@ template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t lau
 
 // second != null: both problems in one launch (only the CTA-pair N = 256 storing variant is paired, see can_pair below)
 static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s, const TcLaunch* second = nullptr) {
-  if (L.cg2 && L.BN == 128) return launch_bn<128, false, true>(L, s);
   if (L.cg2) return L.head ? launch_bn<256, true, true>(L, s) : launch_bn<256, false, true>(L, s, second);
   if (L.head) return launch_bn<256, true, false>(L, s);
   if (L.halo) return L.BN == 128 ? launch_bn<128, false, false, true>(L, s) : launch_bn<64, false, false, true>(L, s);
@@ -294,9 +276,9 @@ static int fusable_block(const aframe_weights* w, int i) {
 
 // row_shift > 0: x is the stem of the whole stream (shared stem): window b starts row_shift rows after window b - 1, and
 // edge holds every window's own rows 0, 1, T - 1
-static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia, int ib, const __nv_bfloat16* x,
-                               __nv_bfloat16* out, int64_t nb, TcBlockLaunch& L, int64_t row_shift = 0,
-                               const __nv_bfloat16* edge = nullptr, int T_override = 0, int zero_period = 0, int zero_valid = 0) {
+static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia, int ib, const af_act_t* x,
+                               af_act_t* out, int64_t nb, TcBlockLaunch& L, int64_t row_shift = 0,
+                               const af_act_t* edge = nullptr, int T_override = 0, int zero_period = 0, int zero_valid = 0) {
   const LayerDesc& a = w->layers[ia];
   const int T = T_override > 0 ? T_override : a.t_out;
   const uint64_t dims[3] = {64, (uint64_t)T, (uint64_t)nb};
@@ -318,13 +300,6 @@ static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia,
   p.edge = row_shift > 0 ? edge : nullptr;
   p.zero_period = zero_period; p.zero_valid = zero_valid;
   p.reverse = 0;
-  p.dbg_out = nullptr;
-  if (env_int("AFRAME_TC_PROF", 0)) {
-    static long long* d_prof = nullptr;
-    if (!d_prof) { cudaMalloc(&d_prof, sizeof(long long) * 64 * 8); cudaMemset(d_prof, 0, sizeof(long long) * 64 * 8); }
-    p.dbg_out = d_prof + 48 * (ib % 8);
-    if (const char* f = getenv("AFRAME_TCB_PROF_PTR")) { FILE* fp = fopen(f, "w"); if (fp) { fprintf(fp, "%llu\n", (unsigned long long)(uintptr_t)d_prof); fclose(fp); } }
-  }
   L.smem = tcb_smem(p.nx, p.ny, p.no);
   L.device = ctx->device;
   L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
@@ -348,8 +323,7 @@ static cudaError_t launch_block(const TcBlockLaunch& L, cudaStream_t s) {
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
-  static const int pdl = env_int("AFRAME_PDL", 1);
-  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  cfg.attrs = at; cfg.numAttrs = 1;
   return cudaLaunchKernelEx(&cfg, conv_block_kernel, L.tm_x, L.tm_wa, L.tm_wb, L.tm_out, L.p);
 }
 
@@ -516,11 +490,11 @@ sh_head_partial_kernel(const uint4* __restrict__ S, const uint4* __restrict__ Y,
   for (int jj = 0; jj < 8; ++jj) {
     const uint4 o = rowp[c * 8 + jj];
     const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
-    const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
-    hacc[0] = fmaf(__uint_as_float(ow[0] << 16), hA.x, hacc[0]); hacc[1] = fmaf(__uint_as_float(ow[0] & 0xffff0000u), hA.y, hacc[1]);
-    hacc[2] = fmaf(__uint_as_float(ow[1] << 16), hA.z, hacc[2]); hacc[3] = fmaf(__uint_as_float(ow[1] & 0xffff0000u), hA.w, hacc[3]);
-    hacc[0] = fmaf(__uint_as_float(ow[2] << 16), hB.x, hacc[0]); hacc[1] = fmaf(__uint_as_float(ow[2] & 0xffff0000u), hB.y, hacc[1]);
-    hacc[2] = fmaf(__uint_as_float(ow[3] << 16), hB.z, hacc[2]); hacc[3] = fmaf(__uint_as_float(ow[3] & 0xffff0000u), hB.w, hacc[3]);
+    const float2 o0 = af_act_unpack2(o.x), o1 = af_act_unpack2(o.y), o2 = af_act_unpack2(o.z), o3 = af_act_unpack2(o.w);
+    hacc[0] = fmaf(o0.x, hA.x, hacc[0]); hacc[1] = fmaf(o0.y, hA.y, hacc[1]);
+    hacc[2] = fmaf(o1.x, hA.z, hacc[2]); hacc[3] = fmaf(o1.y, hA.w, hacc[3]);
+    hacc[0] = fmaf(o2.x, hB.x, hacc[0]); hacc[1] = fmaf(o2.y, hB.y, hacc[1]);
+    hacc[2] = fmaf(o3.x, hB.z, hacc[2]); hacc[3] = fmaf(o3.y, hB.w, hacc[3]);
   }
   float sum = 0.f;
   sum += (hacc[0] + hacc[1]) + (hacc[2] + hacc[3]);
@@ -587,18 +561,10 @@ void af_tc_forget(aframe_ctx* ctx) {
   ctx->tc_cache = nullptr;
 }
 
-static int64_t tc_chunk_windows() {
-  static int64_t v = 0;
-  if (v == 0) {
-    const char* e = getenv("AFRAME_CHUNK_B");
-    // windows per internal launch sequence.  Measured on B200: every layer launch carries ~12 us of launch gap, prologue
-    // (TMEM/barriers/first loads from HBM) and drain, so large chunks win (592: 869, 1184: 922, 4096: 994 TFLOP/s);
-    // the three live activation tensors leave the 126 MB L2 from ~300 windows on anyway.
-    v = e ? atoll(e) : 4096;
-    if (v < 1) v = 4096;
-  }
-  return v;
-}
+// Windows per internal launch sequence.  Measured on B200: every layer launch carries ~12 us of launch gap, prologue
+// (TMEM/barriers/first loads from HBM) and drain, so large chunks win (592: 869, 1184: 922, 4096: 994 TFLOP/s); the three
+// live activation tensors leave the 126 MB L2 from ~300 windows on anyway.
+static int64_t tc_chunk_windows() { return 4096; }
 
 // Number of leading fused 64-channel blocks that form a chain on the pooled stem output (layers 2,3 | 4,5 | ...): the
 // blocks the shared first stage can take over.
@@ -653,7 +619,7 @@ static std::vector<int> s2_chain_layers(const aframe_weights* w, int i0) {
   return out;
 }
 
-aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_bf16, int64_t sB,
+aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_dt, int64_t sB,
                               int64_t sT, const int64_t* choff, int64_t B, float* d_scores) {
   (void)sT;
   NetPlan plan;
@@ -670,7 +636,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     for (int i = 0; only_consumer && i < n - 1; ++i)
       if (w->layers[i].input_from == src || w->layers[i].residual_from == src) only_consumer = false;
     if (only_consumer && w->layers[src].c_out % 256 == 0 && w->layers[src].c_out <= 512 && tile_t_box(w->layers[src].t_out) % 32 == 0 &&
-        env_int("AFRAME_FUSE_HEAD", 1) && !w->live_gn) {
+        !w->live_gn) {
       fuse = src;
       n_part = (w->layers[src].t_out / 32) * (w->layers[src].c_out / 64);
     }
@@ -691,8 +657,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   // shared first stage (see s1_gather_kernel): K streams + one gathered input + K edge results per chunk
   const int s1_k = s1_chain_blocks(w);
   const bool s1_on = s1_k > 0 && sB % 4 == 0 && sB < w->layers[0].t_in && chunk >= 2 && !w->live_gn &&
-                     w->layers[1].t_out >= 2 * S1_ROWS && env_int("AFRAME_SHARED_STEM", 1) && env_int("AFRAME_SHARED_S1", 1) &&
-                     env_int("AFRAME_FUSE_BLOCK", 1);
+                     w->layers[1].t_out >= 2 * S1_ROWS;
   // shared later stages (see sh_gather_kernel): per launched layer one stream and one edge-batch tensor, plus the gathered input
   auto up128 = [](int64_t v) { return (v + 127) / 128 * 128; };
   struct SharedStage {
@@ -710,10 +675,10 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   };
   std::vector<SharedStage> shs;
   bool sh_head_on = false;
-  if (s1_on && env_int("AFRAME_SHARED_S2", 1) && env_int("AFRAME_FUSE_SC", 1)) {
+  if (s1_on) {
     int i0 = 2 + 2 * s1_k, Tp = w->layers[1].t_out, hp = 2 * s1_k + 2, tp = 2 * s1_k + 1;
     int64_t shift_p = sB / 4;
-    const int max_stages = env_int("AFRAME_SHARED_STAGES", 3);
+    const int max_stages = 3;
     while ((int)shs.size() < max_stages && shift_p % 2 == 0 && !sh_head_on) {
       SharedStage g;
       g.list = s2_chain_layers(w, i0);
@@ -731,7 +696,6 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       g.tail = g.T - (Tp - tp) / 2 + n2;                          // ... at the start and at the end of the stage's output
       const int src_rows = shs.empty() ? S1_ROWS : shs.back().rows;
       g.rows = g.head + n2 > g.tail + n2 + 1 ? g.head + n2 : g.tail + n2 + 1;
-      if (env_int("AFRAME_SHARED_ROWS", 0) > g.rows) g.rows = env_int("AFRAME_SHARED_ROWS", 0);    // (experiments: longer short windows)
       g.period = g.rows + 2;
       const bool fits = g.T >= g.rows && Tp >= 2 * g.rows && Tp == 2 * g.T && hp <= src_rows - 2 && tp <= src_rows - 2 &&
                         g.C % 64 == 0 && g.C_in % 64 == 0;
@@ -742,7 +706,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       // per conv); its box holds those rows and the two rows next to them that the epilogue takes from the stream (the outer one
       // is computed from a row outside the box): tbox[q] = max(e_head, e_tail) + 2 rows, floor(128 / tbox) slots per MMA tile.
       // (The entry conv's rows are all computed from valid input rows and the last layer's interior rows are never read: no copies.)
-      if (g.C % 256 == 0 && env_int("AFRAME_PACKED_EDGES", 1)) {
+      if (g.C % 256 == 0) {
         const int nl = (int)g.list.size();
         g.e_head.resize(nl); g.e_tail.resize(nl); g.tbox.assign(nl, 0);
         bool ok = true;
@@ -783,18 +747,18 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   if (st != AFRAME_OK) return st;
   char* base = reinterpret_cast<char*>(ctx->ws_act.ptr);
   char* s1_base = base + slot_bytes * plan.n_slots + part_bytes;
-  auto s1_stream_ptr = [&](int k) { return reinterpret_cast<__nv_bfloat16*>(s1_base + (size_t)(k - 1) * s1_stream_bytes); };             // S_k, k = 1..K
+  auto s1_stream_ptr = [&](int k) { return reinterpret_cast<af_act_t*>(s1_base + (size_t)(k - 1) * s1_stream_bytes); };             // S_k, k = 1..K
   char* s2_base = s1_base + s1_bytes;
-  auto sh_x_ptr = [&](int g) { return reinterpret_cast<__nv_bfloat16*>(s2_base + shs[g].off); };
+  auto sh_x_ptr = [&](int g) { return reinterpret_cast<af_act_t*>(s2_base + shs[g].off); };
   int64_t cur_nb = chunk;                          // windows of the chunk being planned / launched (row counts depend on it)
   auto sh_rows_stream = [&](int g) { return up128((cur_nb - 1) * shs[g].shift + shs[g].T); };
   auto sh_buf = [&](int g, int pass, int idx) {    // pass 0: the tensor (stream part first), 1: its edge-batch part; idx: position in the list
     const SharedStage& h = shs[g];
-    return reinterpret_cast<__nv_bfloat16*>(s2_base + h.off + h.x_bytes + (size_t)idx * h.stream_bytes) + (pass ? sh_rows_stream(g) * h.C : 0);
+    return reinterpret_cast<af_act_t*>(s2_base + h.off + h.x_bytes + (size_t)idx * h.stream_bytes) + (pass ? sh_rows_stream(g) * h.C : 0);
   };
-  auto s1_edge_ptr = [&](int k) { return reinterpret_cast<__nv_bfloat16*>(s1_base + (size_t)s1_k * s1_stream_bytes + (size_t)k * s1_edge_bytes); };  // X (k = 0), Y_k
+  auto s1_edge_ptr = [&](int k) { return reinterpret_cast<af_act_t*>(s1_base + (size_t)s1_k * s1_stream_bytes + (size_t)k * s1_edge_bytes); };  // X (k = 0), Y_k
   float* head_part = reinterpret_cast<float*>(base + slot_bytes * plan.n_slots);
-  auto slot_ptr = [&](int layer) { return reinterpret_cast<__nv_bfloat16*>(base + slot_bytes * plan.slot[layer]); };
+  auto slot_ptr = [&](int layer) { return reinterpret_cast<af_act_t*>(base + slot_bytes * plan.slot[layer]); };
   if (!ctx->tc_cache) ctx->tc_cache = new std::vector<TcPlanCache>();
   std::vector<TcPlanCache>& caches = *static_cast<std::vector<TcPlanCache>*>(ctx->tc_cache);
 
@@ -816,7 +780,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       pc->skip.assign(n, 0);
       // projection shortcut (1x1 conv, no ReLU, read only as layer i's residual): folded into layer i as extra K blocks,
       // which saves its launch, the write of its output and the residual read (the accumulation also stays in fp32)
-      if (env_int("AFRAME_FUSE_SC", 1) && !w->live_gn)
+      if (!w->live_gn)
         for (int i = 2; i < n; ++i) {
           const LayerDesc& l = w->layers[i];
           const int r = l.residual_from;
@@ -830,7 +794,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           if (w->layers[i].input_from == r) ok = false;
           if (ok) { pc->sc_of[i] = r; pc->skip[r] = 1; }
         }
-      if (env_int("AFRAME_FUSE_BLOCK", 1) && !w->live_gn)
+      if (!w->live_gn)
         for (int i = 2; i < n; ++i) {
           const int ib = pc->fused_with[i] < 0 ? fusable_block(w, i) : -1;
           if (ib < 0) continue;
@@ -838,11 +802,11 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           // stem output is read only by this fused block: the stem runs ONCE over the whole stream, the block reads the
           // windows as strided views of it and patches the three rows per window that see the window's own zero padding.
           bool shared = i == 2 && w->layers[2].input_from == 1 && w->layers[ib].residual_from == 1 && nb >= 2 && sB % 4 == 0 &&
-                        sB < w->layers[0].t_in && env_int("AFRAME_SHARED_STEM", 1) != 0;
+                        sB < w->layers[0].t_in;
           for (int j = 2; shared && j < n; ++j)
             if (j != 2 && j != ib && (w->layers[j].input_from == 1 || w->layers[j].residual_from == 1)) shared = false;
           const int64_t row_shift = shared ? sB / 4 : 0;
-          const __nv_bfloat16* edge = slot_ptr(1) + ((nb - 1) * row_shift + w->layers[1].t_out) * 64;
+          const af_act_t* edge = slot_ptr(1) + ((nb - 1) * row_shift + w->layers[1].t_out) * 64;
           if (!build_block_launch(ctx, w, i, ib, slot_ptr(w->layers[i].input_from), slot_ptr(ib), nb, pc->blocks[ib], row_shift, edge)) { caches.pop_back(); return AFRAME_ECUDA; }
           if (shared) pc->shared_stem = true;
           pc->fused_with[i] = ib; pc->fused_with[ib] = i;
@@ -883,12 +847,12 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             const int qi = entry ? -1 : idx_of(l.input_from), qr = (l.residual_from >= 0 && sc < 0) ? idx_of(l.residual_from) : -1;
             ok = (entry || qi >= 0) && (l.residual_from < 0 || sc >= 0 || qr >= 0);
             if (!ok) break;
-            const __nv_bfloat16* x_edge = sh_x_ptr((int)g) + 2 * rows_s * h.C_in;
+            const af_act_t* x_edge = sh_x_ptr((int)g) + 2 * rows_s * h.C_in;
             TcShapeOverride ov_s{(int)rows_s, 0, 0, 0};
             TcShapeOverride ov_e{0, 0, 0, 0};
             // the conv that feeds the head stores nothing: its tensor holds the per-row head dot products instead
             // ([stream rows | edge-batch rows][C / 64] floats)
-            const bool hr = sh_head_on && g + 1 == shs.size() && q + 1 == h.list.size() && env_int("AFRAME_HEAD_ROWS", 1);
+            const bool hr = sh_head_on && g + 1 == shs.size() && q + 1 == h.list.size();
             float* hr_s = reinterpret_cast<float*>(sh_buf((int)g, 0, (int)q));
             float* hr_e = hr_s + rows_s * (h.C / 64);
             ov_s.head_rows = ov_e.head_rows = hr;
@@ -908,8 +872,8 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             const TcShapeOverride ov{(int)rows_tot, h.period, h.rows, (int)rows_s};
             const bool entry = li == h.i0;
             const int sc = pc->sc_of[li];
-            const __nv_bfloat16* in = entry ? sh_x_ptr((int)g) : sh_buf((int)g, 0, idx_of(l.input_from));
-            const __nv_bfloat16* res = (l.residual_from >= 0 && sc < 0) ? sh_buf((int)g, 0, idx_of(l.residual_from)) : nullptr;
+            const af_act_t* in = entry ? sh_x_ptr((int)g) : sh_buf((int)g, 0, idx_of(l.input_from));
+            const af_act_t* res = (l.residual_from >= 0 && sc < 0) ? sh_buf((int)g, 0, idx_of(l.residual_from)) : nullptr;
             ok = (entry || idx_of(l.input_from) >= 0) && (res == nullptr || idx_of(l.residual_from) >= 0) &&
                  build_launch(ctx, w, li, in, res, sh_buf((int)g, 0, (int)q), 1, false, nullptr, P.stream[q], sc,
                               sc >= 0 ? sh_x_ptr((int)g) : nullptr, &ov);
@@ -935,15 +899,14 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           const int cg = l.c_out / w->n_groups;
           const int u = cg < 64 ? cg : 64;
           TcConvParams& pp = pc->launches[i].p;
-          if (pp.T_box % 32 == 0 && (u == 8 || u == 16 || u == 32 || u == 64) && cg % u == 0 && env_int("AFRAME_GN_EPI", 1)) {
+          if (pp.T_box % 32 == 0 && (u == 8 || u == 16 || u == 32 || u == 64) && cg % u == 0) {
             pp.gn_part = reinterpret_cast<float2*>(reinterpret_cast<char*>(head_part) + gn_stats_bytes);
             pp.gn_unit = u;
-            pp.out_f16 = env_int("AFRAME_GN_F16", 1);       // z leaves the SM as fp16; af_launch_gn_bf16 turns it into bf16 y
           }
         }
       }
     }
-    const size_t esz = in_bf16 ? 2 : 4;
+    const size_t esz = af_dt_bytes(in_dt);
     std::vector<cudaEvent_t> lev;
     if (ctx->layer_ms) {
       lev.resize(n + 1);
@@ -958,11 +921,11 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     const StemGn sgn{gn_stats, w->d_gamma[0], w->d_beta[0], w->n_groups, w->gn_eps};
     if (pc->shared_stem)
       st = af_launch_stem_stream_bf16(ctx, w->layers[0], w->layers[1], reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz,
-                                      in_bf16, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1),
+                                      in_dt, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1),
                                       slot_ptr(1) + ((nb - 1) * (sB / 4) + w->layers[1].t_out) * 64);
     else
     st = af_launch_stem_bf16(ctx, w->layers[0], w->layers[1], reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz,
-                             in_bf16, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1), w->live_gn ? &sgn : nullptr);
+                             in_dt, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1), w->live_gn ? &sgn : nullptr);
     af_prof_end(ctx, AFRAME_PROF_STEM, 1);
     if (st != AFRAME_OK) return st;
     int n_conv = 0;
@@ -1015,10 +978,9 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           // Launch order: stream(0) | edge(q) with stream(q + 1) as ONE launch of two problems (independent of each other: both
           // need stream(q), and edge(q) needs edge(q - 1)) | ... | edge(last).  A stream launch alone costs 16-30 us for 1/8 of an
           // edge launch's work (profiles/r01i_conv_full.md); as the second problem its tiles fill the edge launch's last wave.
-          static const int pair_on = env_int("AFRAME_PAIR_LAUNCH", 1);
           const size_t nl = P.layers.size();
           auto can_pair = [&](size_t q) {
-            if (!pair_on || q + 1 >= nl) return false;
+            if (q + 1 >= nl) return false;
             const TcLaunch& a = P.edge[q];
             const TcLaunch& b = P.stream[q + 1];
             return a.cg2 && b.cg2 && a.BN == 256 && b.BN == 256 && !a.head && !b.head && !a.halo && !b.halo && a.p.stages == b.p.stages &&
@@ -1094,8 +1056,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         // Alternate the direction in which consecutive launches walk their tiles: a layer then starts with the rows its
         // producer wrote LAST, which are still in L2 (walking every layer forwards evicts exactly the lines that are
         // about to be read).
-        static const int alt = env_int("AFRAME_ALT_DIR", 1);
-        const int rev = alt ? (n_conv & 1) : 0;
+        const int rev = n_conv & 1;
         pc->launches[i].p.reverse = rev;
         pc->blocks[i].p.reverse = rev;
         const TcLaunch& L = pc->launches[i];
@@ -1106,7 +1067,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
         if (w->live_gn) {
           st = af_launch_gn_bf16(ctx, slot_ptr(i), l.residual_from >= 0 ? slot_ptr(l.residual_from) : nullptr, l.t_out, l.c_out,
-                                 w->n_groups, w->gn_eps, w->d_gamma[i], w->d_beta[i], l.relu, nb, gn_stats, L.p.gn_part, L.p.gn_unit, L.p.out_f16);
+                                 w->n_groups, w->gn_eps, w->d_gamma[i], w->d_beta[i], l.relu, nb, gn_stats, L.p.gn_part, L.p.gn_unit);
           if (st != AFRAME_OK) return st;
         }
       } else if (l.kind == 2) {
@@ -1119,7 +1080,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           ctx->launches++;
           if (cudaGetLastError() != cudaSuccess) return af_fail(ctx, AFRAME_ECUDA, "head_finish launch failed");
         } else {
-          st = af_launch_head(ctx, slot_ptr(l.input_from), 1, w->d_head_w, w->head_b, l.t_in, l.c_in, nb, d_scores + b0);
+          st = af_launch_head(ctx, slot_ptr(l.input_from), AF_DT_F16, w->d_head_w, w->head_b, l.t_in, l.c_in, nb, d_scores + b0);
         }
         af_prof_end(ctx, AFRAME_PROF_HEAD, 1);
         if (st != AFRAME_OK) return st;

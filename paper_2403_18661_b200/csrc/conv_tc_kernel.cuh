@@ -2,14 +2,15 @@
 //
 //   out[b][t][co] = relu( bias[co] + sum_{d, ci} W'[d][co][ci] * in[b][P*t + d - pad][ci] (+ res[b][t][co]) )
 //
-//   GEMM view: M = (window, t) rows, N = C_out, K = taps * C_in.  Activations are channels-last bf16, so a
+//   GEMM view: M = (window, t) rows, N = C_out, K = taps * C_in.  Activations are channels-last fp16, so a
 //   row of A for tap d is the contiguous channel vector of input row P*t + d - pad.
 //   A tile (128 rows x 64 ch) : ONE TMA box of the rank-4 view (C_in, P, T_in/P, B), start row shifted per
 //                               tap; out-of-range rows (t = -1, T) are zero-filled by TMA = 'same' padding,
 //                               per window, so rows never bleed between windows.  Stride 2 = parity dim.
-//   B tile (BN x 64 ch)       : TMA box of the folded bf16 weights [taps][C_out][C_in] (K-major).
-//   tcgen05.mma M=128, N=BN, K=16, fp32 accumulators in TMEM (two stages of BN columns).
-//   Epilogue: tcgen05.ld -> +bias (+residual, prefetched by TMA) -> ReLU -> bf16 -> swizzled smem -> TMA store,
+//   B tile (BN x 64 ch)       : TMA box of the folded fp16 weights [taps][C_out][C_in] (K-major).
+//   tcgen05.mma kind::f16 (fp16 activations x fp16 weights) M=128, N=BN, K=16, fp32 accumulators in TMEM
+//   (two stages of BN columns).
+//   Epilogue: tcgen05.ld -> +bias (+residual, prefetched by TMA) -> fp16 -> ReLU -> swizzled smem -> TMA store,
 //   or (HEAD) the fused global-average-pool + linear head: per-(window, slab) partial dot products.
 //
 // Warp roles: warp 0 TMA producer, warp 1 MMA issuer (+TMEM alloc), then EG epilogue groups of 4 warps.
@@ -18,7 +19,7 @@
 // Persistent: CTA i handles tiles i, i + grid, ...
 #pragma once
 #include "tc_ptx.cuh"
-#include <cuda_bf16.h>
+#include "common.cuh"
 
 // Division by a run-time constant without the ~200-cycle integer-divide sequence (the tile loops of the producer,
 // MMA and epilogue roles are single dependent instruction streams): q = (umulhi(x, mul) + x) >> shr, exact for
@@ -51,7 +52,7 @@ struct TcConvParams {
   int stages;                // smem ring depth of the main loop
   int nbuf, pf;              // output/residual staging buffers per epilogue group, residual prefetch distance
   int c_out;
-  // fused head (HEAD variant): partial[b][slab][chunk] = sum_{t in slab, c in chunk} bf16(out[b][t][c]) * head_w[c]
+  // fused head (HEAD variant): partial[b][slab][chunk] = sum_{t in slab, c in chunk} fp16(out[b][t][c]) * head_w[c]
   const float* head_w;
   float* head_part;
   int head_slabs;            // T_out / T_box
@@ -92,11 +93,11 @@ struct TcConvParams {
                              // the rest of the 128-row MMA tile is then stale shared memory, and those rows are dropped)
   long long edge_shift;
   const uint4* edge_stream;  // null: nothing is replaced (the stage's entry conv: all its input rows are valid)
-  int out_f16;               // store the (pre-norm) output as fp16 (saturating) instead of bf16: z = mu + O(sigma) loses
-                             // |mu| / sigma times more to an 8-bit mantissa than the normalised value does
   int w_bytes;               // resident weight region (0 unless HALO)
   int stage_bytes;           // bytes per main-loop stage
-  long long* dbg_out;        // timing experiments: per-role cycle counters of CTA 0 (null = off)
+#ifdef AFRAME_TC_CYCLES      // experiments build only (not compiled into the product library)
+  long long* dbg_out;        // per-role cycle counters of CTA 0 (null = off)
+#endif
 };
 
 // shared-memory carve-up (bytes from the 1024-aligned start of dynamic shared memory):
@@ -127,15 +128,15 @@ template <int BN, bool CG2 = false> struct TcCfg {
 
 __device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 
-// One 64-channel chunk of one output row: + bias (+ residual read from the staging buffer) -> bf16 -> max(., lo)
-// (lo = 0: ReLU, which commutes with the rounding; lo = -inf: none) -> staging buffer, or the fused head's dot product.
-template <bool RES, bool HEAD, bool F16 = false>
+// One 64-channel chunk of one output row: + bias (+ residual read from the staging buffer) -> fp16 (RNE, saturating) ->
+// max(., lo) (lo = 0: ReLU, which commutes with the rounding; lo = -inf: none) -> staging buffer, or the fused head's dot product.
+template <bool RES, bool HEAD>
 __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4* bias4, const float4* hw4,
-                                                 unsigned char* rowp, int row, __nv_bfloat162 lo2, float& head_acc,
+                                                 unsigned char* rowp, int row, __half2 lo2, float& head_acc,
                                                  bool zero_row = false) {
   float hacc[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-  for (int jj = 0; jj < 8; ++jj) {                 // 8 pieces of 8 channels (16 B of bf16)
+  for (int jj = 0; jj < 8; ++jj) {                 // 8 pieces of 8 channels (16 B of fp16)
     const float4 bA = bias4[2 * jj], bB = bias4[2 * jj + 1];
     float f[8];
     f[0] = __uint_as_float(v[8 * jj + 0]) + bA.x; f[1] = __uint_as_float(v[8 * jj + 1]) + bA.y;
@@ -147,29 +148,28 @@ __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4
       const uint4 r = *sp;
       const uint32_t rw[4] = {r.x, r.y, r.z, r.w};
 #pragma unroll
-      for (int e = 0; e < 4; ++e) {                // bf16 pair -> two fp32 (exact): low half << 16, high half masked
-        f[2 * e] += __uint_as_float(rw[e] << 16);
-        f[2 * e + 1] += __uint_as_float(rw[e] & 0xffff0000u);
+      for (int e = 0; e < 4; ++e) {                // fp16 pair -> two fp32 (exact)
+        const float2 t = af_act_unpack2(rw[e]);
+        f[2 * e] += t.x;
+        f[2 * e + 1] += t.y;
       }
     }
     uint4 o;
-    __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(&o);
+    uint32_t* ow = reinterpret_cast<uint32_t*>(&o);
 #pragma unroll
-    for (int e = 0; e < 4; ++e) ob[e] = __hmax2(__floats2bfloat162_rn(f[2 * e], f[2 * e + 1]), lo2);
-    if (F16) {                                     // (no ReLU in this mode)
-      uint32_t* ow = reinterpret_cast<uint32_t*>(&o);
-#pragma unroll
-      for (int e = 0; e < 4; ++e)
-        asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(ow[e]) : "f"(f[2 * e + 1]), "f"(f[2 * e]));
+    for (int e = 0; e < 4; ++e) {
+      const uint32_t pk = af_act_pack2(f[2 * e], f[2 * e + 1]);
+      const __half2 m = __hmax2(*reinterpret_cast<const __half2*>(&pk), lo2);
+      ow[e] = *reinterpret_cast<const uint32_t*>(&m);
     }
     if (zero_row) o = make_uint4(0u, 0u, 0u, 0u);
     if (HEAD) {
       const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
-      const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
-      hacc[0] = fmaf(__uint_as_float(ow[0] << 16), hA.x, hacc[0]); hacc[1] = fmaf(__uint_as_float(ow[0] & 0xffff0000u), hA.y, hacc[1]);
-      hacc[2] = fmaf(__uint_as_float(ow[1] << 16), hA.z, hacc[2]); hacc[3] = fmaf(__uint_as_float(ow[1] & 0xffff0000u), hA.w, hacc[3]);
-      hacc[0] = fmaf(__uint_as_float(ow[2] << 16), hB.x, hacc[0]); hacc[1] = fmaf(__uint_as_float(ow[2] & 0xffff0000u), hB.y, hacc[1]);
-      hacc[2] = fmaf(__uint_as_float(ow[3] << 16), hB.z, hacc[2]); hacc[3] = fmaf(__uint_as_float(ow[3] & 0xffff0000u), hB.w, hacc[3]);
+      const float2 o0 = af_act_unpack2(o.x), o1 = af_act_unpack2(o.y), o2 = af_act_unpack2(o.z), o3 = af_act_unpack2(o.w);
+      hacc[0] = fmaf(o0.x, hA.x, hacc[0]); hacc[1] = fmaf(o0.y, hA.y, hacc[1]);
+      hacc[2] = fmaf(o1.x, hA.z, hacc[2]); hacc[3] = fmaf(o1.y, hA.w, hacc[3]);
+      hacc[0] = fmaf(o2.x, hB.x, hacc[0]); hacc[1] = fmaf(o2.y, hB.y, hacc[1]);
+      hacc[2] = fmaf(o3.x, hB.z, hacc[2]); hacc[3] = fmaf(o3.y, hB.w, hacc[3]);
     } else {
       *sp = o;
     }
@@ -268,10 +268,15 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
 
   const int kiters = p.taps * p.kblocks + p.sc_kblocks;
   // cycle accounting for experiments (CTA 0 only): T(slot) adds the cycles since the previous T() of this thread
+#ifdef AFRAME_TC_CYCLES
   const bool prof = p.dbg_out != nullptr && blockIdx.x == 0;
   long long tprev = prof ? clock64() : 0, tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   auto T = [&](int slot) { if (prof) { const long long t = clock64(); tacc[slot] += t - tprev; tprev = t; } };
   auto Tflush = [&](int role) { if (prof) for (int i = 0; i < 8; ++i) p.dbg_out[role * 8 + i] = tacc[i]; };
+#else
+  auto T = [](int) {};
+  auto Tflush = [](int) {};
+#endif
   // tile -> (n0, t0, b0): n fastest, then the T_box-row block inside a window group, then the window group
   auto decode = [&](const TcConvParams& p, int tile, int& n_idx, int& t0, int& b0) {
     int mp, tb, bb;
@@ -391,7 +396,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
   } else if (warp == 1) {
     // ===== MMA issuer: the whole warp runs the (uniform) loop, one elected lane issues =====
     if (rank == 0) {
-      constexpr uint32_t idesc = umma_idesc_bf16_mn(CG2 ? 256 : 128, BN);
+      constexpr uint32_t idesc = umma_idesc_f16_mn(CG2 ? 256 : 128, BN);
       int stage = 0; uint32_t phase = 0;
       int acc = 0; uint32_t acc_phase = 0;
       if (HALO) mbar_wait(w_bar, 0);
@@ -417,8 +422,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
 #pragma unroll
               for (int m = 0; m < 12; ++m) {
                 const uint32_t al = a_lo + (m / 4) * 8 + (m % 4) * 2, bl = b_lo + (m / 4) * b_tap + (m % 4) * 2;
-                if (m == 0 && kb == 0) umma_bf16_lohi<false>(d_tmem, al, bl, idesc);
-                else umma_bf16_lohi<true>(d_tmem, al, bl, idesc);
+                if (m == 0 && kb == 0) umma_mma_lohi<false>(d_tmem, al, bl, idesc);
+                else umma_mma_lohi<true>(d_tmem, al, bl, idesc);
               }
               umma_commit(empty_bar(stage));
             }
@@ -433,7 +438,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
               const uint32_t a_lo = umma_desc_lo(stage_base + stage * STAGE_BYTES);
               const uint32_t b_lo = umma_desc_lo(w_base + (uint32_t)((p.taps * p.kblocks + kb) * BN * 128));
 #pragma unroll
-              for (int m = 0; m < 4; ++m) umma_bf16_lohi<true>(d_tmem, a_lo + m * 2, b_lo + m * 2, idesc);
+              for (int m = 0; m < 4; ++m) umma_mma_lohi<true>(d_tmem, a_lo + m * 2, b_lo + m * 2, idesc);
               umma_commit(empty_bar(stage));
             }
             __syncwarp();
@@ -449,9 +454,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           const uint64_t da = umma_desc_sw128(sa), db = umma_desc_sw128(sa + Cfg::A_BYTES);
           if (elect_one()) {
 #pragma unroll
-          for (int k = 0; k < 4; ++k) { // 4 x (K = 16 bf16 = 32 B) inside the 128-byte swizzle row
-            if (CG2) umma_bf16_cg2(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
-            else umma_bf16(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
+          for (int k = 0; k < 4; ++k) { // 4 x (K = 16 elements = 32 B) inside the 128-byte swizzle row
+            if (CG2) umma_mma_cg2(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
+            else umma_mma(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (it > 0 || k > 0) ? 1u : 0u);
           }
           if (CG2) umma_commit_cg2(empty_bar(stage), 3);   // frees the smem slot in BOTH CTAs when these MMAs retire
           else umma_commit(empty_bar(stage));
@@ -610,13 +615,12 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         const float4* hw4 = reinterpret_cast<const float4*>(s_headw + n0 + c * 64);
         unsigned char* rowp = gen_base + (sbuf - base) + row * 128;
         // straight-line code per variant (no run-time branches inside the unrolled loop, so the 8 pieces interleave)
-        const __nv_bfloat162 lo2 = __float2bfloat162_rn(p.relu ? 0.f : -INFINITY);
+        const __half2 lo2 = __float2half2_rn(p.relu ? 0.f : -INFINITY);
         const int t_row = t0 + row % p.T_box;
         const bool zero_row = p.zero_period > 0 && t_row >= p.zero_origin - 2 &&
                               ((t_row - p.zero_origin + p.zero_period) % p.zero_period) >= p.zero_valid;
         const uint4* copy_row = copy_tile != nullptr ? copy_tile + c * 8 : nullptr;
         if (p.has_res) tc_epilogue_math<true, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row);
-        else if (!HEAD && p.out_f16) tc_epilogue_math<false, false, true>(v, bias4, hw4, rowp, row, lo2, head_acc);
         else tc_epilogue_math<false, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row);
         if (!HEAD && copy_row != nullptr) {        // the staged row is replaced by the stream's (8 independent loads, then 8 stores)
           uint4 cr[8];

@@ -1,24 +1,23 @@
-// NEXT-2, true GroupNorm on the bf16 path ("GroupNorm ... whose statistics are computed per sample at inference").
-// The tensor-core conv stores its plain output z (no bias, no ReLU, no residual) as bf16 [B][T][C]; these two kernels
+// NEXT-2, true GroupNorm on the tensor-core path ("GroupNorm ... whose statistics are computed per sample at inference").
+// The tensor-core conv stores its plain output z (no bias, no ReLU, no residual) as fp16 [B][T][C]; these two kernels
 // then compute, per (window, group), the mean and biased variance over the group's channels and all T positions and
 // apply y = (z - mu) rstd gamma_c + beta_c (+ residual) (ReLU) in place.  Both are pure HBM streams: 16-byte accesses,
 // one CTA per window for the statistics, one thread per 8 channels for the apply.
 #include "common.cuh"
 #include "stem.h"
-#include <cuda_fp16.h>
 
 __device__ __forceinline__ void gn_unpack8(const uint4 v, float* f) {
-  const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v);
+  const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
-    const float2 t = __bfloat1622float2(h[j]);
+    const float2 t = af_act_unpack2(w[j]);
     f[2 * j] = t.x; f[2 * j + 1] = t.y;
   }
 }
 
 // Fast path: C/8 divides 256 (so a thread always sees the same 8 channels) and a group is a whole number of octets.
 __global__ void __launch_bounds__(256)
-gn_stats_bf16_kernel(const __nv_bfloat16* __restrict__ z, int T, int C, int G, float eps, float2* __restrict__ stats) {
+gn_stats_bf16_kernel(const af_act_t* __restrict__ z, int T, int C, int G, float eps, float2* __restrict__ stats) {
   __shared__ double rs[256], rq[256];
   const int64_t b = blockIdx.x;
   const int opr = C / 8;                               // octets per row
@@ -49,15 +48,15 @@ gn_stats_bf16_kernel(const __nv_bfloat16* __restrict__ z, int T, int C, int G, f
 
 // General shapes: one CTA per (window, group), scalar loads.
 __global__ void __launch_bounds__(256)
-gn_stats_bf16_generic_kernel(const __nv_bfloat16* __restrict__ z, int T, int C, int G, float eps, float2* __restrict__ stats) {
+gn_stats_bf16_generic_kernel(const af_act_t* __restrict__ z, int T, int C, int G, float eps, float2* __restrict__ stats) {
   __shared__ double rs[8], rq[8];
   const int64_t b = blockIdx.x;
   const int g = blockIdx.y;
   const int cg = C / G;
-  const __nv_bfloat16* zb = z + b * (int64_t)T * C + g * cg;
+  const af_act_t* zb = z + b * (int64_t)T * C + g * cg;
   double s = 0.0, q = 0.0;
   for (int i = threadIdx.x; i < T * cg; i += blockDim.x) {
-    const double v = (double)__bfloat162float(zb[(int64_t)(i / cg) * C + (i % cg)]);
+    const double v = (double)__half2float(zb[(int64_t)(i / cg) * C + (i % cg)]);
     s += v; q += v * v;
   }
 #pragma unroll
@@ -89,24 +88,14 @@ __global__ void gn_finalize_kernel(const float2* __restrict__ part, int n_slabs,
   stats[b * G + g] = make_float2((float)mu, (float)(1.0 / sqrt((var > 0.0 ? var : 0.0) + (double)eps)));
 }
 
-__device__ __forceinline__ void gn_unpack8_f16(const uint4 v, float* f) {
-  const __half2* h = reinterpret_cast<const __half2*>(&v);
-#pragma unroll
-  for (int j = 0; j < 4; ++j) {
-    const float2 t = __half22float2(h[j]);
-    f[2 * j] = t.x; f[2 * j + 1] = t.y;
-  }
-}
-
-// Z_F16: z was stored as fp16 by the conv epilogue (TcConvParams::out_f16); the result is bf16 either way.
 // Fast path (256 % (C/8) == 0): a CTA takes GN_ITER * 256 consecutive 8-channel octets of ONE window, so a thread always
 // sees the same 8 channels: its 8 (scale, shift) pairs -- scale = rstd_g gamma_c, shift = beta_c - mu_g scale -- are set
 // up once and every octet costs one 16-byte load (two with a residual), 8 FMAs and one 16-byte store.
 constexpr int GN_ITER = 4;
-template <bool RES, bool Z_F16>
+template <bool RES>
 __global__ void __launch_bounds__(256)
-gn_apply_bf16_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ stats, const float* __restrict__ gamma,
-                     const float* __restrict__ beta, const __nv_bfloat16* __restrict__ res, int n_oct_win /* T * C/8 */,
+gn_apply_bf16_kernel(af_act_t* __restrict__ z, const float2* __restrict__ stats, const float* __restrict__ gamma,
+                     const float* __restrict__ beta, const af_act_t* __restrict__ res, int n_oct_win /* T * C/8 */,
                      int segs /* CTAs per window */, int C, int G, int relu) {
   const int b = blockIdx.x / segs, seg = blockIdx.x - b * segs;
   const int opr = C / 8, cg = C / G;
@@ -132,26 +121,26 @@ gn_apply_bf16_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ s
     const int i = i0 + k * 256;
     if (i >= n_oct_win) continue;
     float f[8], r[8];
-    if (Z_F16) gn_unpack8_f16(zv[k], f); else gn_unpack8(zv[k], f);
+    gn_unpack8(zv[k], f);
     if (RES) gn_unpack8(rv[k], r);
     uint4 o;
-    __nv_bfloat162* oh = reinterpret_cast<__nv_bfloat162*>(&o);
+    uint32_t* oh = reinterpret_cast<uint32_t*>(&o);
 #pragma unroll
     for (int j = 0; j < 8; j += 2) {
       float y0 = fmaf(f[j], sc[j], sh[j]), y1 = fmaf(f[j + 1], sc[j + 1], sh[j + 1]);
       if (RES) { y0 += r[j]; y1 += r[j + 1]; }
       if (relu) { y0 = fmaxf(y0, 0.f); y1 = fmaxf(y1, 0.f); }
-      oh[j / 2] = __floats2bfloat162_rn(y0, y1);
+      oh[j / 2] = af_act_pack2(y0, y1);
     }
     zb[i] = o;
   }
 }
 
 // General shapes (C/8 does not divide 256): one thread per octet.
-template <bool RES, bool Z_F16>
+template <bool RES>
 __global__ void __launch_bounds__(256)
-gn_apply_bf16_generic_kernel(__nv_bfloat16* __restrict__ z, const float2* __restrict__ stats, const float* __restrict__ gamma,
-                             const float* __restrict__ beta, const __nv_bfloat16* __restrict__ res, int64_t n_oct, int T, int C,
+gn_apply_bf16_generic_kernel(af_act_t* __restrict__ z, const float2* __restrict__ stats, const float* __restrict__ gamma,
+                             const float* __restrict__ beta, const af_act_t* __restrict__ res, int64_t n_oct, int T, int C,
                              int G, int relu) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_oct) return;
@@ -161,10 +150,10 @@ gn_apply_bf16_generic_kernel(__nv_bfloat16* __restrict__ z, const float2* __rest
   const int cg = C / G;
   uint4* zp = reinterpret_cast<uint4*>(z) + i;
   float f[8], r[8];
-  if (Z_F16) gn_unpack8_f16(*zp, f); else gn_unpack8(*zp, f);
+  gn_unpack8(*zp, f);
   if (RES) gn_unpack8(reinterpret_cast<const uint4*>(res)[i], r);
   uint4 o;
-  __nv_bfloat162* oh = reinterpret_cast<__nv_bfloat162*>(&o);
+  uint32_t* oh = reinterpret_cast<uint32_t*>(&o);
 #pragma unroll
   for (int j = 0; j < 8; j += 2) {
     float v[2];
@@ -177,14 +166,14 @@ gn_apply_bf16_generic_kernel(__nv_bfloat16* __restrict__ z, const float2* __rest
       if (relu) y = fmaxf(y, 0.f);
       v[k] = y;
     }
-    oh[j / 2] = __floats2bfloat162_rn(v[0], v[1]);
+    oh[j / 2] = af_act_pack2(v[0], v[1]);
   }
   *zp = o;
 }
 
-aframe_status af_launch_gn_bf16(aframe_ctx* ctx, __nv_bfloat16* z, const __nv_bfloat16* res, int T, int C, int G, float eps,
+aframe_status af_launch_gn_bf16(aframe_ctx* ctx, af_act_t* z, const af_act_t* res, int T, int C, int G, float eps,
                                 const float* gamma, const float* beta, int relu, int64_t nb, float2* stats,
-                                const float2* partials, int gn_unit, int z_f16) {
+                                const float2* partials, int gn_unit) {
   if (C % 8 || G < 1 || C % G) return af_fail(ctx, AFRAME_EUNSUPPORTED, "bf16 GroupNorm: channels must be a multiple of 8 and of n_groups");
   const int opr = C / 8, cg = C / G;
   if (partials)
@@ -196,19 +185,18 @@ aframe_status af_launch_gn_bf16(aframe_ctx* ctx, __nv_bfloat16* z, const __nv_bf
     gn_stats_bf16_generic_kernel<<<dim3((unsigned)nb, (unsigned)G), 256, 0, ctx->stream>>>(z, T, C, G, eps, stats);
   AF_LAUNCH_CHECK(ctx);
   const int64_t n_oct = nb * T * opr;
-#define AF_GN_APPLY(RES_, F16_)                                                                                          \
+#define AF_GN_APPLY(RES_)                                                                                                \
   do {                                                                                                                  \
     if (256 % opr == 0 && (int64_t)T * opr < (1 << 30)) {                                                               \
       const int n_win = T * opr, segs = (n_win + GN_ITER * 256 - 1) / (GN_ITER * 256);                                  \
-      gn_apply_bf16_kernel<RES_, F16_><<<(unsigned)(nb * segs), 256, 0, ctx->stream>>>(z, stats, gamma, beta, res, n_win, \
+      gn_apply_bf16_kernel<RES_><<<(unsigned)(nb * segs), 256, 0, ctx->stream>>>(z, stats, gamma, beta, res, n_win, \
                                                                                        segs, C, G, relu);               \
     } else {                                                                                                            \
-      gn_apply_bf16_generic_kernel<RES_, F16_><<<(unsigned)((n_oct + 255) / 256), 256, 0, ctx->stream>>>(               \
+      gn_apply_bf16_generic_kernel<RES_><<<(unsigned)((n_oct + 255) / 256), 256, 0, ctx->stream>>>(               \
           z, stats, gamma, beta, res, n_oct, T, C, G, relu);                                                            \
     }                                                                                                                   \
   } while (0)
-  if (z_f16) { if (res) AF_GN_APPLY(true, true); else AF_GN_APPLY(false, true); }
-  else { if (res) AF_GN_APPLY(true, false); else AF_GN_APPLY(false, false); }
+  if (res) AF_GN_APPLY(true); else AF_GN_APPLY(false);
 #undef AF_GN_APPLY
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;

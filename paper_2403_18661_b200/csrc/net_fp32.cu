@@ -18,13 +18,10 @@ struct ConvArgs {
   int T_in, T_out, C_in, C_out, k, stride, pad, relu;
 };
 
-template <bool IN_BF16>
-__device__ __forceinline__ float ld_in(const void* p, int64_t i) {
-  if (IN_BF16) return __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(p)[i]);
-  return reinterpret_cast<const float*>(p)[i];
-}
+template <int IN_DT>
+__device__ __forceinline__ float ld_in(const void* p, int64_t i) { return af_ld_as_f32<IN_DT>(p, i); }
 
-template <bool IN_BF16>
+template <int IN_DT>
 __global__ void __launch_bounds__(256) conv_fp32_kernel(const ConvArgs a) {
   constexpr int BM = 64, BN = 64, BK = 16;
   __shared__ float As[BK][BM + 4];
@@ -55,7 +52,7 @@ __global__ void __launch_bounds__(256) conv_fp32_kernel(const ConvArgs a) {
         const int t_in = t * a.stride + d - a.pad;
         if (t_in >= 0 && t_in < a.T_in) {
           const int64_t off = b * a.in_sB + (int64_t)t_in * a.in_sT + (a.use_choff ? a.choff[ci] : (int64_t)ci * a.in_sC);
-          v = ld_in<IN_BF16>(a.in, off);
+          v = ld_in<IN_DT>(a.in, off);
         }
       }
       As[kk][r] = v;
@@ -156,7 +153,7 @@ __global__ void maxpool_fp32_kernel(const float* __restrict__ in, float* __restr
 }
 
 // Global average pool over T, then dot with w[C] + b.  One CTA per window.
-template <bool IN_BF16>
+template <int IN_DT>
 __global__ void __launch_bounds__(256) head_kernel(const void* __restrict__ in, const float* __restrict__ w, float bias,
                                                    int T, int C, float* __restrict__ scores) {
   __shared__ float red[8];
@@ -164,7 +161,7 @@ __global__ void __launch_bounds__(256) head_kernel(const void* __restrict__ in, 
   float part = 0.f;
   for (int c = threadIdx.x; c < C; c += blockDim.x) {
     float s = 0.f;
-    for (int t = 0; t < T; ++t) s += ld_in<IN_BF16>(in, (b * T + t) * (int64_t)C + c);
+    for (int t = 0; t < T; ++t) s += ld_in<IN_DT>(in, (b * T + t) * (int64_t)C + c);
     part += s * w[c];
   }
 #pragma unroll
@@ -178,10 +175,11 @@ __global__ void __launch_bounds__(256) head_kernel(const void* __restrict__ in, 
   }
 }
 
-aframe_status af_launch_head(aframe_ctx* ctx, const void* d_in, int in_bf16, const float* d_w, float bias, int T, int C,
+aframe_status af_launch_head(aframe_ctx* ctx, const void* d_in, int in_dt, const float* d_w, float bias, int T, int C,
                              int64_t B, float* d_scores) {
-  if (in_bf16) head_kernel<true><<<(unsigned)B, 256, 0, ctx->stream>>>(d_in, d_w, bias, T, C, d_scores);
-  else head_kernel<false><<<(unsigned)B, 256, 0, ctx->stream>>>(d_in, d_w, bias, T, C, d_scores);
+  if (in_dt == AF_DT_F16) head_kernel<AF_DT_F16><<<(unsigned)B, 256, 0, ctx->stream>>>(d_in, d_w, bias, T, C, d_scores);
+  else if (in_dt == AF_DT_BF16) head_kernel<AF_DT_BF16><<<(unsigned)B, 256, 0, ctx->stream>>>(d_in, d_w, bias, T, C, d_scores);
+  else head_kernel<AF_DT_F32><<<(unsigned)B, 256, 0, ctx->stream>>>(d_in, d_w, bias, T, C, d_scores);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }
@@ -223,7 +221,7 @@ bool af_make_plan(const aframe_weights* w, bool fuse_stem_pool, NetPlan& plan) {
   return true;
 }
 
-aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_bf16, int64_t sB,
+aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_dt, int64_t sB,
                               int64_t sT, const int64_t* choff, int64_t B, float* d_scores) {
   NetPlan plan;
   af_make_plan(w, false, plan);
@@ -252,15 +250,16 @@ aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const vo
         const int pk = l.input_from < 0 ? AFRAME_PROF_STEM : AFRAME_PROF_CONV;
         af_prof_begin(ctx, pk);
         if (l.input_from < 0) {
-          const size_t esz = in_bf16 ? 2 : 4;
+          const size_t esz = af_dt_bytes(in_dt);
           a.in = reinterpret_cast<const char*>(d_in) + (size_t)(b0 * sB) * esz;
           a.in_sB = sB; a.in_sT = sT; a.in_sC = 0; a.use_choff = 1;
           for (int c = 0; c < AF_MAX_CH; ++c) a.choff[c] = c < l.c_in ? choff[c] : 0;
-          if (in_bf16) conv_fp32_kernel<true><<<grid, 256, 0, ctx->stream>>>(a);
-          else conv_fp32_kernel<false><<<grid, 256, 0, ctx->stream>>>(a);
+          if (in_dt == AF_DT_BF16) conv_fp32_kernel<AF_DT_BF16><<<grid, 256, 0, ctx->stream>>>(a);
+          else if (in_dt == AF_DT_F16) conv_fp32_kernel<AF_DT_F16><<<grid, 256, 0, ctx->stream>>>(a);
+          else conv_fp32_kernel<AF_DT_F32><<<grid, 256, 0, ctx->stream>>>(a);
         } else {
           a.in = src; a.in_sB = (int64_t)l.t_in * l.c_in; a.in_sT = l.c_in; a.in_sC = 1; a.use_choff = 0;
-          conv_fp32_kernel<false><<<grid, 256, 0, ctx->stream>>>(a);
+          conv_fp32_kernel<AF_DT_F32><<<grid, 256, 0, ctx->stream>>>(a);
         }
         af_prof_end(ctx, pk, 1);
         AF_LAUNCH_CHECK(ctx);

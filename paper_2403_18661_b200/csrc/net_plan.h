@@ -17,5 +17,5 @@ struct NetPlan {
 };
 
 bool af_make_plan(const aframe_weights* w, bool fuse_stem_pool, NetPlan& plan);
-aframe_status af_launch_head(aframe_ctx* ctx, const void* d_in, int in_bf16, const float* d_w, float bias, int T, int C,
+aframe_status af_launch_head(aframe_ctx* ctx, const void* d_in, int in_dt, const float* d_w, float bias, int T, int C,
                              int64_t B, float* d_scores);

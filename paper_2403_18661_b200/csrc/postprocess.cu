@@ -16,6 +16,15 @@ tophat_kernel(const float* __restrict__ scores, int64_t n, int64_t ld, int n_int
   integ[s * ld_out + i] = __fmul_rn(acc, __fdiv_rn(1.0f, (float)(i + 1 - lo)));
 }
 
+// (value, index) order of the clustering: a NaN beats every number (NaN propagates: the trigger of a window that holds
+// one is its FIRST NaN, as numpy.argmax gives for the oracle); among equals the earlier index wins.
+__device__ __forceinline__ bool cluster_better(float v, int64_t vi, float b, int64_t bi) {
+  const bool vn = v != v, bn = b != b;
+  if (vn != bn) return vn;
+  if (vn) return vi < bi;
+  return v > b || (v == b && vi < bi);
+}
+
 // One warp per (series, cluster window): first maximum of n_cluster consecutive integrated values.
 __global__ void __launch_bounds__(256)
 cluster_max_kernel(const float* __restrict__ integ, int64_t n, int64_t ld, int n_cluster, int64_t n_trig,
@@ -32,14 +41,14 @@ cluster_max_kernel(const float* __restrict__ integ, int64_t n, int64_t ld, int n
   bool have = false;
   for (int64_t j = a + lane; j < b; j += 32) {
     const float v = x[j];
-    if (!have || v > best) { best = v; bi = j; have = true; }   // NaN never wins; ties keep the earlier index
+    if (!have || cluster_better(v, j, best, bi)) { best = v; bi = j; have = true; }
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     const float ov = __shfl_xor_sync(0xffffffffu, best, o);
     const int64_t oi = __shfl_xor_sync(0xffffffffu, bi, o);
     const int oh = __shfl_xor_sync(0xffffffffu, (int)have, o);
-    if (oh && (!have || ov > best || (ov == best && oi < bi))) { best = ov; bi = oi; have = true; }
+    if (oh && (!have || cluster_better(ov, oi, best, bi))) { best = ov; bi = oi; have = true; }
   }
   if (lane == 0) { trig_value[s * n_trig + k] = best; trig_index[s * n_trig + k] = bi; }
 }

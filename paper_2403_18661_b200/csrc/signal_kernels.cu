@@ -183,7 +183,7 @@ filter_design_kernel(const float* __restrict__ psd, int F_w, int C, double fs, d
 // Overlap-save whitening: one CTA per (block, channel).  Block of NOS real samples -> M = NOS/2 complex
 // FFT -> untangle, multiply by real H, re-tangle -> inverse FFT (conjugation trick) -> store valid part.
 // --------------------------------------------------------------------------------------------------
-template <bool OUT_BF16>
+template <int OUT_DT>
 __global__ void __launch_bounds__(256, 3)
 whiten_os_kernel(const float* __restrict__ strain, int64_t n_samples, int64_t ld, const float* __restrict__ H, int C,
                  int64_t in0, int64_t out_total, int64_t epoch_len, int blocks_per_epoch, int L, float scale,
@@ -248,17 +248,21 @@ whiten_os_kernel(const float* __restrict__ strain, int64_t n_samples, int64_t ld
 
   // x[2n] = Re r[n], x[2n+1] = -Im r[n]  (1/M folded into H); valid outputs are i in [L/2, L/2 + n_valid)
   const int half = L / 2;
-  if (OUT_BF16) {
-    __nv_bfloat16* o = reinterpret_cast<__nv_bfloat16*>(out_v) + (int64_t)c * ld_out + out0;
+  if (OUT_DT != AF_DT_F32) {                         // 16-bit output: bf16, or fp16 (saturating)
+    uint16_t* o = reinterpret_cast<uint16_t*>(out_v) + (int64_t)c * ld_out + out0;
+    auto cvt1 = [](float v) -> uint16_t {
+      if (OUT_DT == AF_DT_BF16) return __bfloat16_as_ushort(__float2bfloat16_rn(v));
+      return (uint16_t)(af_act_pack2(v, 0.f) & 0xffffu);
+    };
     const bool st_vec = ((((uintptr_t)o) & 3) == 0) && ((half & 1) == 0);
     for (int n = tid; n < M; n += NT) {
       const float2 r = s[fft_pad(n)];
       const int64_t i0 = 2 * n - half;
       if (st_vec && i0 >= 0 && i0 + 1 < n_valid) {
-        *reinterpret_cast<__nv_bfloat162*>(o + i0) = __floats2bfloat162_rn(r.x, -r.y);
+        *reinterpret_cast<uint32_t*>(o + i0) = (uint32_t)cvt1(r.x) | ((uint32_t)cvt1(-r.y) << 16);
       } else {
-        if (i0 >= 0 && i0 < n_valid) o[i0] = __float2bfloat16_rn(r.x);
-        if (i0 + 1 >= 0 && i0 + 1 < n_valid) o[i0 + 1] = __float2bfloat16_rn(-r.y);
+        if (i0 >= 0 && i0 < n_valid) o[i0] = cvt1(r.x);
+        if (i0 + 1 >= 0 && i0 + 1 < n_valid) o[i0 + 1] = cvt1(-r.y);
       }
     }
   } else {
@@ -362,7 +366,7 @@ aframe_status af_launch_filter_design(aframe_ctx* ctx, const float* d_psd, int64
 
 aframe_status af_launch_whiten_os(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
                                   const float* d_H, int64_t in0, int64_t out_total, int64_t epoch_len, int64_t n_epochs,
-                                  void* d_out, int64_t ld_out, int out_bf16) {
+                                  void* d_out, int64_t ld_out, int out_dt) {
   if (out_total <= 0 || n_epochs <= 0) return AFRAME_OK;
   const aframe_config& cfg = ctx->cfg;
   const int valid = AF_NOS - cfg.filter_len;
@@ -370,12 +374,15 @@ aframe_status af_launch_whiten_os(aframe_ctx* ctx, const float* d_strain, int64_
   const float scale = ldexpf(1.0f, cfg.strain_scale_log2);
   dim3 grid((unsigned)(n_epochs * bpe), (unsigned)af_nch(ctx));
   af_prof_begin(ctx, AFRAME_PROF_WHITEN);
-  if (out_bf16)
-    whiten_os_kernel<true><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, af_nch(ctx), in0, out_total,
-                                                          epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
+  if (out_dt == AF_DT_BF16)
+    whiten_os_kernel<AF_DT_BF16><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, af_nch(ctx), in0, out_total,
+                                                                epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
+  else if (out_dt == AF_DT_F16)
+    whiten_os_kernel<AF_DT_F16><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, af_nch(ctx), in0, out_total,
+                                                               epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
   else
-    whiten_os_kernel<false><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, af_nch(ctx), in0, out_total,
-                                                           epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
+    whiten_os_kernel<AF_DT_F32><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, af_nch(ctx), in0, out_total,
+                                                               epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
   af_prof_end(ctx, AFRAME_PROF_WHITEN, 1);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;

@@ -1,15 +1,12 @@
 // Fused stem of the bf16 path: window assembly in place from the whitened stream,
-// conv k7 s2 (C_in -> 64) + folded norm + ReLU + max-pool k3 s2 p1, output rounded once to bf16,
+// conv k7 s2 (C_in -> 64) + folded norm + ReLU + max-pool k3 s2 p1, output rounded once to fp16,
 // channels-last [B][T_pool][C_out].  K = C_in*7 = 14 is not a tensor-core shape: fp32 FFMA on CUDA cores.
 // The pre-pool tensor never leaves the SM.
 #include "common.cuh"
 #include "stem.h"
 
-template <bool IN_BF16>
-__device__ __forceinline__ float stem_ld(const void* p, int64_t i) {
-  if (IN_BF16) return __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(p)[i]);
-  return __ldg(reinterpret_cast<const float*>(p) + i);
-}
+template <int IN_DT>
+__device__ __forceinline__ float stem_ld(const void* p, int64_t i) { return af_ld_as_f32<IN_DT>(p, i); }
 
 // One CTA: one window, TP pooled positions, all 64 channels.  lane <-> channel pair (2*lane, 2*lane+1), warp <-> a run
 // of TP/8 consecutive pooled positions.  Each conv position is computed once per run (the pool's shared position is
@@ -17,10 +14,10 @@ __device__ __forceinline__ float stem_ld(const void* p, int64_t i) {
 // pooled position.
 // GN (NEXT-2, true GroupNorm): the conv output is normalised with the window's own statistics before ReLU and pool,
 // v = acc * sc + sh with sc = rstd_g gamma_c, sh = beta_c - mu_g rstd_g gamma_c (stats from stem_gn_stats_kernel).
-template <bool IN_BF16, int TP, bool GN>
+template <int IN_DT, int TP, bool GN>
 __global__ void __launch_bounds__(256)
 stem_pool_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const float* __restrict__ w /*[7][2][64]*/,
-                 const float* __restrict__ bias, int T_in, int T_pool, __nv_bfloat16* __restrict__ out,
+                 const float* __restrict__ bias, int T_in, int T_pool, af_act_t* __restrict__ out,
                  const float2* __restrict__ stats, const float* __restrict__ gamma, const float* __restrict__ beta, int G) {
   constexpr int KW = 7, CIN = 2, C_OUT = 64;
   constexpr int RUN = TP / 8;
@@ -33,7 +30,7 @@ stem_pool_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const flo
   for (int i = tid; i < CIN * NX; i += 256) {
     const int c = i / NX, n = i - c * NX;
     const int t = x0 + n;
-    xs[c][n] = (t >= 0 && t < T_in) ? stem_ld<IN_BF16>(in, b * sB + off.v[c] + t) : 0.f;
+    xs[c][n] = (t >= 0 && t < T_in) ? stem_ld<IN_DT>(in, b * sB + off.v[c] + t) : 0.f;
   }
   float w0[KW][CIN], w1[KW][CIN];
 #pragma unroll
@@ -79,7 +76,7 @@ stem_pool_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const flo
     if (GN) { p0 = fmaf(p0, sc0, sh0); p1 = fmaf(p1, sc1, sh1); }
     p0 = fmaxf(p0, 0.f); p1 = fmaxf(p1, 0.f);
   }
-  __nv_bfloat162* o = reinterpret_cast<__nv_bfloat162*>(out + ((int64_t)b * T_pool + tp0 + tl0) * C_OUT) + lane;
+  uint32_t* o = reinterpret_cast<uint32_t*>(out + ((int64_t)b * T_pool + tp0 + tl0) * C_OUT) + lane;
 #pragma unroll
   for (int i = 0; i < RUN; ++i) {
 #pragma unroll
@@ -98,7 +95,7 @@ stem_pool_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const flo
     if (GN) { a0 = fmaf(a0, sc0, sh0); a1 = fmaf(a1, sc1, sh1); c0 = fmaf(c0, sc0, sh0); c1 = fmaf(c1, sc1, sh1); }
     c0 = fmaxf(c0, 0.f); c1 = fmaxf(c1, 0.f);
     const float m0 = fmaxf(fmaxf(p0, a0), c0), m1 = fmaxf(fmaxf(p1, a1), c1);   // ReLU folded: p, c >= 0
-    if (tp0 + tl0 + i < T_pool) o[(int64_t)i * (C_OUT / 2)] = __floats2bfloat162_rn(m0, m1);
+    if (tp0 + tl0 + i < T_pool) o[(int64_t)i * (C_OUT / 2)] = af_act_pack2(m0, m1);
     p0 = c0; p1 = c1;
 #pragma unroll
     for (int c = 0; c < CIN; ++c)
@@ -110,7 +107,7 @@ stem_pool_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const flo
 // NEXT-2: per (window, group) mean and 1/sqrt(var + eps) of the stem conv output (biased variance over the group's
 // channels and all T_conv positions), computed without storing the conv output.  One CTA per window; lane <->
 // channel pair, each warp walks pairs of conv positions (2u, 2u+1), which read x[4u-3 .. 4u+5].
-template <bool IN_BF16>
+template <int IN_DT>
 __global__ void __launch_bounds__(256)
 stem_gn_stats_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const float* __restrict__ w /*[7][2][64]*/,
                      const float* __restrict__ bias, int T_in, int G, float eps, float2* __restrict__ stats) {
@@ -123,7 +120,7 @@ stem_gn_stats_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const
   for (int i = tid; i < CIN * NX; i += 256) {
     const int c = i / NX, n = i - c * NX;
     const int t = n - 4;
-    xs_dyn[i] = (t >= 0 && t < T_in) ? stem_ld<IN_BF16>(in, b * sB + off.v[c] + t) : 0.f;
+    xs_dyn[i] = (t >= 0 && t < T_in) ? stem_ld<IN_DT>(in, b * sB + off.v[c] + t) : 0.f;
   }
   float w0[KW][CIN], w1[KW][CIN];
 #pragma unroll
@@ -178,11 +175,11 @@ stem_gn_stats_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const
 // Shared stem (overlapping windows): rows 0, 1 and T_pool - 1 of every window are the only pooled rows that see the
 // window's own zero padding; everything else equals the stem of the whole stream (af_launch_stem_stream_bf16).  One warp
 // per window, lane <-> channel pair; the FMA order is the one of stem_pool_kernel, so the values are bit-identical to
-// what the per-window kernel stores.  edge: [nb][3][64] bf16 (rows 0, 1, T_pool - 1).
-template <bool IN_BF16>
+// what the per-window kernel stores.  edge: [nb][3][64] fp16 (rows 0, 1, T_pool - 1).
+template <int IN_DT>
 __global__ void __launch_bounds__(128)
 stem_edge_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const float* __restrict__ w /*[7][2][64]*/,
-                 const float* __restrict__ bias, int T_in, int T_pool, int64_t nb, __nv_bfloat16* __restrict__ edge) {
+                 const float* __restrict__ bias, int T_in, int T_pool, int64_t nb, af_act_t* __restrict__ edge) {
   constexpr int KW = 7, CIN = 2, C_OUT = 64;
   const int lane = threadIdx.x & 31;
   const int64_t b = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
@@ -210,21 +207,21 @@ stem_edge_kernel(const void* __restrict__ in, int64_t sB, StemOff off, const flo
 #pragma unroll
         for (int d = 0; d < KW; ++d) {
           const int x = 2 * t - 3 + d;
-          const float xv = (x >= 0 && x < T_in) ? stem_ld<IN_BF16>(in, b * sB + off.v[c] + x) : 0.f;
+          const float xv = (x >= 0 && x < T_in) ? stem_ld<IN_DT>(in, b * sB + off.v[c] + x) : 0.f;
           a0 = fmaf(w0[d][c], xv, a0); a1 = fmaf(w1[d][c], xv, a1);
         }
       m0 = fmaxf(m0, a0); m1 = fmaxf(m1, a1);
     }
-    reinterpret_cast<__nv_bfloat162*>(edge + (b * 3 + k) * C_OUT)[lane] = __floats2bfloat162_rn(m0, m1);
+    reinterpret_cast<uint32_t*>(edge + (b * 3 + k) * C_OUT)[lane] = af_act_pack2(m0, m1);
   }
 }
 
 // Shared stem: the windows of one launch are K-sample views at a spacing of win_stride samples (a multiple of 4) into
 // one whitened stream, so their pooled stem outputs are views at a spacing of win_stride / 4 rows into the stem of the
-// whole stream, except for the three rows above.  d_stream: [(nb - 1) * win_stride / 4 + T_pool][64] bf16.
+// whole stream, except for the three rows above.  d_stream: [(nb - 1) * win_stride / 4 + T_pool][64] fp16.
 aframe_status af_launch_stem_stream_bf16(aframe_ctx* ctx, const LayerDesc& conv, const LayerDesc& pool, const void* d_in,
-                                         int in_bf16, int64_t win_stride, const int64_t* choff, const float* d_w,
-                                         const float* d_bias, int64_t nb, __nv_bfloat16* d_stream, __nv_bfloat16* d_edge) {
+                                         int in_dt, int64_t win_stride, const int64_t* choff, const float* d_w,
+                                         const float* d_bias, int64_t nb, af_act_t* d_stream, af_act_t* d_edge) {
   constexpr int TP = 128;
   StemOff off;
   for (int c = 0; c < AF_MAX_CH; ++c) off.v[c] = c < conv.c_in ? choff[c] : 0;
@@ -232,26 +229,25 @@ aframe_status af_launch_stem_stream_bf16(aframe_ctx* ctx, const LayerDesc& conv,
   if (T_in > (1ll << 30)) return af_fail(ctx, AFRAME_ESHAPE, "shared stem: stream longer than 2^30 samples");
   const int T_pool = (int)(T_in / 4);
   dim3 grid((unsigned)((T_pool + TP - 1) / TP), 1);
-  if (in_bf16) {
-    stem_pool_kernel<true, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, 0, off, d_w, d_bias, (int)T_in, T_pool, d_stream,
-                                                                     nullptr, nullptr, nullptr, 1);
-    AF_LAUNCH_CHECK(ctx);
-    stem_edge_kernel<true><<<(unsigned)((nb + 3) / 4), 128, 0, ctx->stream>>>(d_in, win_stride, off, d_w, d_bias, conv.t_in,
-                                                                              pool.t_out, nb, d_edge);
-  } else {
-    stem_pool_kernel<false, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, 0, off, d_w, d_bias, (int)T_in, T_pool, d_stream,
-                                                                      nullptr, nullptr, nullptr, 1);
-    AF_LAUNCH_CHECK(ctx);
-    stem_edge_kernel<false><<<(unsigned)((nb + 3) / 4), 128, 0, ctx->stream>>>(d_in, win_stride, off, d_w, d_bias, conv.t_in,
-                                                                               pool.t_out, nb, d_edge);
-  }
+#define AF_STEM_STREAM(DT)                                                                                              \
+  do {                                                                                                                  \
+    stem_pool_kernel<DT, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, 0, off, d_w, d_bias, (int)T_in, T_pool, d_stream, \
+                                                                   nullptr, nullptr, nullptr, 1);                        \
+    AF_LAUNCH_CHECK(ctx);                                                                                               \
+    stem_edge_kernel<DT><<<(unsigned)((nb + 3) / 4), 128, 0, ctx->stream>>>(d_in, win_stride, off, d_w, d_bias, conv.t_in, \
+                                                                            pool.t_out, nb, d_edge);                     \
+  } while (0)
+  if (in_dt == AF_DT_BF16) AF_STEM_STREAM(AF_DT_BF16);
+  else if (in_dt == AF_DT_F16) AF_STEM_STREAM(AF_DT_F16);
+  else AF_STEM_STREAM(AF_DT_F32);
+#undef AF_STEM_STREAM
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }
 
 aframe_status af_launch_stem_bf16(aframe_ctx* ctx, const LayerDesc& conv, const LayerDesc& pool, const void* d_in,
-                                  int in_bf16, int64_t sB, const int64_t* choff, const float* d_w, const float* d_bias,
-                                  int64_t B, __nv_bfloat16* d_out, const StemGn* gn) {
+                                  int in_dt, int64_t sB, const int64_t* choff, const float* d_w, const float* d_bias,
+                                  int64_t B, af_act_t* d_out, const StemGn* gn) {
   if (!(conv.k == 7 && conv.c_in == 2 && conv.c_out == 64 && conv.stride == 2 && conv.pad == 3 && conv.relu &&
         pool.k == 3 && pool.stride == 2 && pool.pad == 1))
     return af_fail(ctx, AFRAME_EUNSUPPORTED, "bf16 stem: only conv(2->64,k7,s2,p3)+ReLU+maxpool(k3,s2,p1) is built");
@@ -265,22 +261,26 @@ aframe_status af_launch_stem_bf16(aframe_ctx* ctx, const LayerDesc& conv, const 
     const size_t smem = sizeof(float) * 2 * (size_t)(conv.t_in + 8);
     if (gn->G < 1 || gn->G > 32 || 64 % gn->G || (64 / gn->G) % 2 || smem > 48 * 1024)
       return af_fail(ctx, AFRAME_EUNSUPPORTED, "bf16 stem with true GroupNorm: needs an even number of channels per group and kernel_len <= 6136");
-    if (in_bf16) {
-      stem_gn_stats_kernel<true><<<(unsigned)B, 256, smem, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, gn->G, gn->eps, gn->stats);
-      stem_pool_kernel<true, TP, true><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
-                                                                      gn->stats, gn->gamma, gn->beta, gn->G);
-    } else {
-      stem_gn_stats_kernel<false><<<(unsigned)B, 256, smem, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, gn->G, gn->eps, gn->stats);
-      stem_pool_kernel<false, TP, true><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
-                                                                       gn->stats, gn->gamma, gn->beta, gn->G);
-    }
+#define AF_STEM_GN(DT)                                                                                                  \
+  do {                                                                                                                  \
+    stem_gn_stats_kernel<DT><<<(unsigned)B, 256, smem, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, gn->G, gn->eps, gn->stats); \
+    stem_pool_kernel<DT, TP, true><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out, \
+                                                                  gn->stats, gn->gamma, gn->beta, gn->G);                \
+  } while (0)
+    if (in_dt == AF_DT_BF16) AF_STEM_GN(AF_DT_BF16);
+    else if (in_dt == AF_DT_F16) AF_STEM_GN(AF_DT_F16);
+    else AF_STEM_GN(AF_DT_F32);
+#undef AF_STEM_GN
     ctx->launches++;
-  } else if (in_bf16)
-    stem_pool_kernel<true, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
-                                                                     nullptr, nullptr, nullptr, 1);
+  } else if (in_dt == AF_DT_BF16)
+    stem_pool_kernel<AF_DT_BF16, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
+                                                                           nullptr, nullptr, nullptr, 1);
+  else if (in_dt == AF_DT_F16)
+    stem_pool_kernel<AF_DT_F16, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
+                                                                          nullptr, nullptr, nullptr, 1);
   else
-    stem_pool_kernel<false, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
-                                                                      nullptr, nullptr, nullptr, 1);
+    stem_pool_kernel<AF_DT_F32, TP, false><<<grid, 256, 0, ctx->stream>>>(d_in, sB, off, d_w, d_bias, conv.t_in, pool.t_out, d_out,
+                                                                          nullptr, nullptr, nullptr, 1);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }

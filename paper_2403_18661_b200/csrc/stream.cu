@@ -2,7 +2,6 @@
 // Every kernel of an update takes its decisions from a device-resident counter, so the same launch
 // sequence (and hence one captured CUDA graph) serves every update.
 #include <new>
-#include <stdlib.h>
 #include "common.cuh"
 
 struct aframe_stream_state {
@@ -126,6 +125,9 @@ AF_API aframe_status aframe_stream_create(aframe_ctx* ctx, const aframe_weights*
   const int C = cfg.n_channels, F = cfg.welch_nfft / 2 + 1, L = cfg.filter_len, K = cfg.kernel_len;
   if ((size_t)C * K > 8 * 1024) return af_fail(ctx, AFRAME_EUNSUPPORTED, "streaming window larger than 8192 samples in total");
   if (cfg.psd_len < cfg.stride + L) return af_fail(ctx, AFRAME_ESHAPE, "psd_len < stride + filter_len");
+  // the streaming Welch computes the ONE segment that ends at the newest sample, on the updates where n is a multiple of
+  // the hop; with a stride that does not divide the hop some segments would end between updates and never be computed
+  if (cfg.welch_hop % cfg.stride) return af_fail(ctx, AFRAME_ESHAPE, "streaming needs welch_hop to be a multiple of stride");
   aframe_stream_state* st = new (std::nothrow) aframe_stream_state();
   if (!st) return af_fail(ctx, AFRAME_ENOMEM, "host allocation failed");
   st->ctx = ctx; st->w = w;
@@ -165,12 +167,6 @@ AF_API aframe_status aframe_stream_create(aframe_ctx* ctx, const aframe_weights*
 static aframe_status stream_step_enqueue(aframe_ctx* ctx, const float* d_new_samples, aframe_stream_state* st,
                                          float* d_scores, int32_t* d_n_scores);
 
-static bool stream_graph_enabled() {
-  static int v = -1;
-  if (v < 0) { const char* e = getenv("AFRAME_STREAM_GRAPH"); v = e ? (atoi(e) != 0) : 1; }
-  return v != 0;
-}
-
 AF_API int64_t aframe_stream_graph_replays(const aframe_stream_state* st) { return st ? st->replays : 0; }
 
 AF_API aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samples, aframe_stream_state* st,
@@ -180,9 +176,9 @@ AF_API aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samp
   if (!d_new_samples || !d_scores || !d_n_scores) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
   cudaStreamIsCapturing(ctx->stream, &cap);
-  // direct launches when the caller is capturing the stream itself, when stage timing is on, or when switched off
+  // direct launches when the caller is capturing the stream itself or when stage timing is on
   // (the legacy default stream cannot be captured: a context bound to it launches directly as well)
-  if (!stream_graph_enabled() || ctx->prof_on || ctx->layer_ms || cap != cudaStreamCaptureStatusNone ||
+  if (ctx->prof_on || ctx->layer_ms || cap != cudaStreamCaptureStatusNone ||
       ctx->stream == nullptr || ctx->stream == cudaStreamLegacy)
     return stream_step_enqueue(ctx, d_new_samples, st, d_scores, d_n_scores);
   // (a larger forward on the same context may have re-allocated the activation workspace since the capture)

@@ -1,5 +1,6 @@
 """GPU parity (through the C ABI) of the network forward pass against the float64 oracle.
-fp32 path: rule T2 (<= 1e-4); bf16 tensor-core path: rules T3 (<= 2e-2) and T4 (Spearman >= 0.999)."""
+fp32 path: rule T2 (<= 1e-4); tensor-core path (fp16 weights and activations, fp32 accumulation): rules T3 (<= 2e-2) and T4 (Spearman
+>= 0.999), both asserted outright."""
 import numpy as np
 import pytest
 import scipy.stats
@@ -72,36 +73,36 @@ def test_config1_fp32_scores(af, config1, batch):
     ctx = af.Context(precision=af.FP32)
     w = ctx.load_weights(config1["blob"])
     got = ctx.forward(w, torch.from_numpy(config1["wins"][:batch]).cuda()).cpu().numpy()
-    assert rel_err(got, config1["ref"][:batch]) <= 1e-4 * (1 if batch == 128 else 3)
+    assert rel_err(got, config1["ref"][:batch]) <= 1e-4            # T2 at every batch size (measured: 2e-7 .. 9e-7)
 
 
-def test_config1_bf16_scores_and_rank(af, config1):
-    ctx = af.Context(precision=af.BF16)
+def test_config1_tensor_core_scores_and_rank(af, config1):
+    ctx = af.Context(precision=af.F16)
     w = ctx.load_weights(config1["blob"])
     got = ctx.forward(w, torch.from_numpy(config1["wins"]).cuda()).cpu().numpy().astype(np.float64)
     ref = config1["ref"]
     err = rel_err(got, ref)
     rho = scipy.stats.spearmanr(got, ref).statistic
-    # bf16-ideal ceiling: the oracle with RNE-to-bf16 at exactly the CUDA path's rounding points (B10)
-    ideal = onet.forward(config1["net"], config1["wins"], act_round=onet.round_bf16, weight_round=onet.round_bf16)
+    # the oracle with the CUDA path's storage roundings (B10): fp16 weights, fp16 after every stored activation
+    ideal = onet.forward(config1["net"], config1["wins"], act_round=onet.round_f16, weight_round=onet.round_f16)
     rho_ideal = scipy.stats.spearmanr(ideal, ref).statistic
     err_vs_ideal = rel_err(got, ideal)
-    print(f"bf16: rel err {err:.3e}, spearman {rho:.5f}; ideal-bf16 ceiling {rho_ideal:.5f}; vs ideal {err_vs_ideal:.3e}")
+    print(f"tensor-core path: rel err {err:.3e}, spearman {rho:.5f}; same roundings in float64 {rho_ideal:.5f}; vs that {err_vs_ideal:.3e}")
     assert err <= 2e-2                                           # T3
-    assert err_vs_ideal <= 5e-3                                  # kernels reproduce the bf16-ideal arithmetic
-    assert rho >= min(0.999, rho_ideal - 5e-4)                   # T4 (capped by what the format allows)
+    assert err_vs_ideal <= 1e-3                                  # kernels reproduce the rounded-storage arithmetic
+    assert rho >= 0.999                                          # T4, outright
 
 
 @pytest.mark.parametrize("batch", [1, 3, 7])
-def test_config1_bf16_small_and_ragged_batches(af, config1, batch):
-    ctx = af.Context(precision=af.BF16)
+def test_config1_tensor_core_small_and_ragged_batches(af, config1, batch):
+    ctx = af.Context(precision=af.F16)
     w = ctx.load_weights(config1["blob"])
     got = ctx.forward(w, torch.from_numpy(config1["wins"][:batch]).cuda()).cpu().numpy()
     assert rel_err(got, config1["ref"][:batch]) <= 2e-2
 
 
-def test_bf16_path_refuses_tables_it_cannot_run(af, config0):
-    ctx = af.Context(n_design=4096, kernel_len=2048, precision=af.BF16)
+def test_tensor_core_path_refuses_tables_it_cannot_run(af, config0):
+    ctx = af.Context(n_design=4096, kernel_len=2048, precision=af.F16)
     w = ctx.load_weights(config0["blob"])                        # widths 8..64: not UMMA shapes
     with pytest.raises(af.AframeError) as e:
         ctx.forward(w, torch.from_numpy(config0["wins"]).cuda())
@@ -110,13 +111,13 @@ def test_bf16_path_refuses_tables_it_cannot_run(af, config0):
 
 def test_full_batch_launch_configuration_sampled_against_oracle(af, config1):
     """The launch configuration bench.py times (4096-window chunks, ragged tail, windows taken in place from a bf16
-    whitened stream at stride 128): sampled scores against the float64 oracle (rule T3), and the big batch against the
+    whitened stream (any of the three stream types may be handed in) at stride 128): sampled scores against the float64 oracle (rule T3), and the big batch against the
     same windows scored in small batches (bit for bit: a window's score does not depend on its batch)."""
     n_win = 4096 + 37
     rng = np.random.default_rng(7)
     white = rng.standard_normal((2, (n_win - 1) * 128 + 3072)).astype(np.float32)
     wd = torch.from_numpy(white).cuda().to(torch.bfloat16).contiguous()
-    ctx = af.Context(precision=af.BF16)
+    ctx = af.Context(precision=af.F16)
     w = ctx.load_weights(config1["blob"])
     big = ctx.forward_strided(w, wd, 0, n_win)
     assert big.shape == (n_win,) and bool(torch.isfinite(big).all())
@@ -131,12 +132,12 @@ def test_full_batch_launch_configuration_sampled_against_oracle(af, config1):
 
 
 def test_forward_rejects_bad_arguments(af, config1):
-    ctx = af.Context(precision=af.BF16)
+    ctx = af.Context(precision=af.F16)
     w = ctx.load_weights(config1["blob"])
     with pytest.raises(af.AframeError) as e:
         ctx.forward(w, torch.empty((0, 2, 3072), device="cuda"))
     assert e.value.status == af.EINVAL
-    other = af.Context(precision=af.BF16)
+    other = af.Context(precision=af.F16)
     with pytest.raises(af.AframeError) as e:
         other.forward(w, torch.zeros((1, 2, 3072), device="cuda"))
     assert e.value.status == af.ESTATE
@@ -144,7 +145,7 @@ def test_forward_rejects_bad_arguments(af, config1):
 
 def test_true_group_norm_fp32_matches_oracle(af, config0):
     """NEXT-2: GroupNorm statistics computed per window at inference (blob norm_kind 2) on the fp32 path against
-    the oracle (rule T2); the bf16 tensor-core path refuses such a table loudly."""
+    the oracle (rule T2); the tensor-core path refuses such a table loudly."""
     from synthdata import tiny_config_live_gn
     cfg = tiny_config_live_gn()
     blob = make_weight_blob(**cfg)
@@ -155,17 +156,17 @@ def test_true_group_norm_fp32_matches_oracle(af, config0):
     w = ctx.load_weights(blob)
     got = ctx.forward(w, torch.from_numpy(wins).cuda()).cpu().numpy()
     assert rel_err(got, ref) <= 1e-4
-    ctx16 = af.Context(n_design=4096, kernel_len=2048, precision=af.BF16)
+    ctx16 = af.Context(n_design=4096, kernel_len=2048, precision=af.F16)
     w16 = ctx16.load_weights(blob)
     with pytest.raises(af.AframeError) as e:                    # widths 8..64 do not tile onto the tensor-core kernel
         ctx16.forward(w16, torch.from_numpy(wins).cuda())
     assert e.value.status == af.EUNSUPPORTED
 
 
-def test_true_group_norm_full_size_fp32_and_bf16(af, config1):
-    """NEXT-2 at configs[1] size: the ResNet54 table with live GroupNorm.  fp32 path within T2 of the oracle; bf16
-    tensor-core path (plain conv output stored as bf16, statistics + affine + residual + ReLU in the GroupNorm kernels)
-    within T3 and rank-preserving; smaller ragged batches give the same scores bit for bit."""
+def test_true_group_norm_full_size_fp32_and_tensor_core(af, config1):
+    """NEXT-2 at configs[1] size: the ResNet54 table with live GroupNorm.  fp32 path within T2 of the oracle; tensor-core
+    path (plain conv output stored as fp16, statistics + affine + residual + ReLU in the GroupNorm kernels) within T3 and
+    T4 (Spearman >= 0.999, outright); smaller ragged batches give the same scores bit for bit."""
     from synthdata import full_config_live_gn
     blob = make_weight_blob(**full_config_live_gn())
     wins = config1["wins"][:48].copy()
@@ -177,28 +178,27 @@ def test_true_group_norm_full_size_fp32_and_bf16(af, config1):
     ctx = af.Context(precision=af.FP32)
     got32 = ctx.forward(ctx.load_weights(blob), x[:8]).cpu().numpy()
     assert rel_err(got32, ref[:8]) <= 1e-4
-    ctx16 = af.Context(precision=af.BF16)
+    ctx16 = af.Context(precision=af.F16)
     w16 = ctx16.load_weights(blob)
     got = ctx16.forward(w16, x).cpu().numpy().astype(np.float64)
     err = rel_err(got, ref)
     rho = scipy.stats.spearmanr(got, ref).statistic
-    # rule T4 in context: this randomly initialised live-GN network squeezes its scores into a 2 % band, so even the ideal
-    # bf16 evaluation (oracle with bf16 weights and one bf16 rounding per layer output) does not reach 0.999 here
+    # the oracle with the CUDA path's storage roundings (fp16 weights, fp16 after every stored tensor), for the record
     net = onet.parse_blob(blob)
-    ideal = onet.forward(net, wins, act_round=onet.round_bf16, weight_round=onet.round_bf16)
+    ideal = onet.forward(net, wins, act_round=onet.round_f16, weight_round=onet.round_f16)
     rho_ideal = scipy.stats.spearmanr(ideal, ref).statistic
-    print(f"live GroupNorm bf16: rel err {err:.3e}, spearman {rho:.5f} (ideal-bf16 ceiling {rho_ideal:.5f}, "
+    print(f"live GroupNorm, tensor-core path: rel err {err:.3e}, spearman {rho:.5f} (same roundings in float64 {rho_ideal:.5f}, "
           f"its rel err {rel_err(ideal, ref):.3e})")
-    assert err <= 2e-2
-    assert rho >= rho_ideal - 3e-3
-    assert rel_err(got, ideal) <= 1e-2
+    assert err <= 2e-2                                           # T3 (measured 1.0e-3)
+    assert rho >= 0.999                                          # T4, outright (measured 0.99957 on these 48 windows)
+    assert rel_err(got, ideal) <= 5e-3
     for nb in (1, 37):
         part = ctx16.forward(w16, x[:nb]).cpu().numpy()
         assert np.array_equal(part, got[:nb].astype(np.float32))
 
 
 @pytest.mark.parametrize("kernel_len", [2048, 4096, 2560])
-def test_bf16_path_other_window_lengths(af, kernel_len):
+def test_tensor_core_path_other_window_lengths(af, kernel_len):
     """The tensor-core path is not specialised to K = 3072: the config-1 table on 1 s, 2 s and 1.25 s windows (stage lengths
     512..64, 1024..128 and 640..80: other tile shapes, windows-per-tile counts and fused-block tile counts)."""
     cfg = dict(full_config(), kernel_len=kernel_len)
@@ -206,7 +206,7 @@ def test_bf16_path_other_window_lengths(af, kernel_len):
     rng = np.random.default_rng(kernel_len)
     wins = rng.standard_normal((5, 2, kernel_len)).astype(np.float32)
     ref = onet.forward(onet.parse_blob(blob), wins)
-    ctx = af.Context(kernel_len=kernel_len, precision=af.BF16)
+    ctx = af.Context(kernel_len=kernel_len, precision=af.F16)
     got = ctx.forward(ctx.load_weights(blob), torch.from_numpy(wins).cuda()).cpu().numpy()
     assert rel_err(got, ref) <= 2e-2
     ctx32 = af.Context(kernel_len=kernel_len, precision=af.FP32)
@@ -214,7 +214,7 @@ def test_bf16_path_other_window_lengths(af, kernel_len):
     assert rel_err(got32, ref[:2]) <= 1e-4
 
 
-def test_live_group_norm_bf16_fallback_statistics_path(af):
+def test_live_group_norm_tensor_core_fallback_statistics_path(af):
     """True GroupNorm on 1.25 s windows: the last stage has 80 rows per window (16-row tiles, 8 windows per tile), where
     the conv epilogue cannot emit per-window partial sums and the statistics are read back from z instead."""
     from synthdata import full_config_live_gn
@@ -223,7 +223,7 @@ def test_live_group_norm_bf16_fallback_statistics_path(af):
     rng = np.random.default_rng(5)
     wins = rng.standard_normal((11, 2, 2560)).astype(np.float32)
     ref = onet.forward(onet.parse_blob(blob), wins)
-    ctx = af.Context(kernel_len=2560, precision=af.BF16)
+    ctx = af.Context(kernel_len=2560, precision=af.F16)
     got = ctx.forward(ctx.load_weights(blob), torch.from_numpy(wins).cuda()).cpu().numpy()
     assert rel_err(got, ref) <= 2e-2
 
@@ -239,7 +239,7 @@ def test_shared_stages_equal_the_per_window_path_bit_for_bit(af, config1, stride
     white = torch.from_numpy(rng.standard_normal((2, (n_win - 1) * stride + 3072 + 2048)).astype(np.float32)).cuda().bfloat16()
     import math
     unit = math.lcm(2048, stride)                                # the configuration wants PSD lengths in whole strides and hops
-    ctx = af.Context(precision=af.BF16, stride=stride, psd_update=unit * -(-16384 // unit), psd_len=unit * -(-131072 // unit))
+    ctx = af.Context(precision=af.F16, stride=stride, psd_update=unit * -(-16384 // unit), psd_len=unit * -(-131072 // unit))
     w = ctx.load_weights(config1["blob"])
     shared = ctx.forward_strided(w, white.contiguous(), 0, n_win, chan_shift=[0, 2048])
     wins = torch.stack([torch.stack([white[0, i * stride: i * stride + 3072], white[1, 2048 + i * stride: 2048 + i * stride + 3072]])
@@ -255,7 +255,7 @@ def test_tensor_mac_counter_matches_the_layer_table(af, config1):
     except for the 64-channel basic blocks, whose fused kernel computes 128-row MMAs per 126-row tile.  In shared form
     (overlapping in-place windows) the count must be well below the per-window figure and above the stream-only bound."""
     net = config1["net"]
-    ctx = af.Context(precision=af.BF16)
+    ctx = af.Context(precision=af.F16)
     w = ctx.load_weights(config1["blob"])
     B = 128
     m0 = ctx.tensor_macs()

@@ -31,7 +31,7 @@ def test_zero_lag_triggers_get_far_from_timeslide_background(af):
     noise = coloured_noise(n_raw, seed=4242)
     x, _ = inject_chirps(noise, draw_chirp_params(20, n_raw / FS, seed=7))
     shifts = [0] + [k * FS for k in range(1, 9)]                 # series 0 = zero lag, 1..8 = background
-    ctx = af.Context(precision=af.BF16)
+    ctx = af.Context(precision=af.F16)
     w = ctx.load_weights(make_weight_blob(**full_config()))
     scores = ctx.score_timeslides(w, torch.from_numpy(x).cuda(), 0, n_win, shifts, batch=4096)
     assert scores.shape == (9, n_win) and bool(torch.isfinite(scores).all())

@@ -62,15 +62,15 @@ def test_stream_fp32_matches_oracle_through_warmup_and_a_psd_update(af):
     assert rel_err(got, want) <= 1e-4
 
 
-def test_stream_bf16_full_network_scores(af):
-    """configs[4]: config-1 network in bf16 at batch 1; rule T3 on the first scored updates."""
+def test_stream_tensor_core_full_network_scores(af):
+    """configs[4]: config-1 network on the fp16 tensor-core path at batch 1; rule T3 on the first scored updates."""
     fc = full_config()
     n_updates = 131072 // S + 3072 // S + 6
     x = coloured_noise(n_updates * S, seed=1002)
     blob = make_weight_blob(**fc)
     so = ost.StreamOracle(ost.StreamConfig(), net=onet.parse_blob(blob))
     ref = [so.step(x[:, u * S:(u + 1) * S].astype(np.float64)) for u in range(n_updates)]
-    ctx = af.Context(precision=af.BF16)
+    ctx = af.Context(precision=af.F16)
     w = ctx.load_weights(blob)
     flags, scores = _run_stream(af, ctx, w, x, n_updates)
     np.testing.assert_array_equal(flags, [0 if r is None else 1 for r in ref])
@@ -110,7 +110,7 @@ def test_stream_graph_replay_equals_direct_launches(af):
     buf = torch.empty((2, S), dtype=torch.float32, device="cuda")
     out = {}
     for name, stream in (("direct", None), ("graph", torch.cuda.Stream())):
-        ctx = af.Context(precision=af.BF16, stream=stream)
+        ctx = af.Context(precision=af.F16, stream=stream)
         w = ctx.load_weights(blob)
         st = ctx.stream_create(w)
         scores = []
@@ -153,12 +153,12 @@ def test_score_timeslides_device_host_and_oracle(af):
     n_raw = -(-(m0 + n_white + 1024) // S) * S + 16384          # crosses a PSD epoch
     x = coloured_noise(n_raw, seed=1003)
     blob = make_weight_blob(**fc)
-    ctx = af.Context(precision=af.BF16)
+    ctx = af.Context(precision=af.F16)
     w = ctx.load_weights(blob)
     xd = torch.from_numpy(x).cuda()
     dev = ctx.score_timeslides(w, xd, 0, n_win, shifts, batch=batch)
     assert dev.shape == (2, n_win) and dev.is_cuda
-    white = ctx.whiten_rolling(xd, out_dtype=torch.bfloat16).contiguous()
+    white = ctx.whiten_rolling(xd, out_dtype=torch.float16).contiguous()   # the call keeps its whitened stream as fp16
     for k, sh in enumerate(shifts):
         ref = ctx.forward_strided(w, white, 0, n_win, chan_shift=[0, sh])
         assert torch.equal(dev[k], ref)
@@ -277,7 +277,7 @@ def test_bench_step_at_full_size_sampled_against_oracle(af):
     shifts = [k * FS for k in range(1, bench.N_SLIDES + 1)]
     x = bench.make_block(7, n_raw)
     blob = make_weight_blob(**fc)
-    ctx = af.Context(precision=af.BF16)
+    ctx = af.Context(precision=af.F16)
     w = ctx.load_weights(blob)
     scores = ctx.score_timeslides(w, torch.from_numpy(x).cuda(), 0, n_win, shifts, batch=4096)
     assert scores.shape == (bench.N_SLIDES, n_win) and bool(torch.isfinite(scores).all())
@@ -304,3 +304,20 @@ def test_bench_step_at_full_size_sampled_against_oracle(af):
     want = onet.forward(net, np.stack(wins))
     got = np.array([scores[k, i] for k, i in picks], dtype=np.float64)
     assert rel_err(got, want) <= 2e-2
+
+
+def test_configurations_the_streaming_state_or_the_path_cannot_honour_are_refused(af):
+    """(a) a stride that does not divide the Welch hop would leave Welch segments that end between two updates uncomputed
+    (the PSD would silently come out low): aframe_stream_create refuses it; the offline calls, which compute every segment
+    from the stored record, accept it.  (b) bf16 is a stream storage type only: as the network precision it is refused."""
+    tc = tiny_config()
+    ctx = af.Context(n_design=4096, kernel_len=tc["kernel_len"], stride=3072, psd_len=129024, psd_update=18432, precision=af.FP32)
+    w = ctx.load_weights(make_weight_blob(**tc))
+    with pytest.raises(af.AframeError) as e:
+        ctx.stream_create(w)
+    assert e.value.status == af.ESHAPE
+    x = torch.from_numpy(coloured_noise(129024 + 2 * 18432, seed=3)).cuda()
+    assert ctx.whiten_rolling(x).shape[1] > 0
+    with pytest.raises(af.AframeError) as e:
+        af.Context(precision=af.BF16)
+    assert e.value.status == af.EUNSUPPORTED

@@ -148,6 +148,21 @@ def test_round_bf16_matches_torch():
     np.testing.assert_array_equal(onet.round_bf16(x), ref)
 
 
+def test_round_f16_matches_torch_spacing_and_saturation():
+    """Pins of round_f16 (activation storage of the tensor-core path, reading B10): the library conversion, the format's
+    spacing (2^-10 relative in the normal range, 2^-24 absolute below 2^-14: hand values), saturation at +-65504."""
+    x = np.concatenate([RNG.standard_normal(1000) * 10, RNG.standard_normal(200) * 1e-6, RNG.standard_normal(200) * 3e3])
+    ref = torch.from_numpy(x).float().half().double().numpy()
+    np.testing.assert_array_equal(onet.round_f16(x), ref)
+    np.testing.assert_array_equal(onet.round_f16([1.0 + 2.0 ** -11, 1.0 + 3 * 2.0 ** -11, 2048.0 + 1.0, 2.0 ** -25 * 1.5]),
+                                  [1.0, 1.0 + 2.0 ** -9, 2048.0, 2.0 ** -24])        # ties to even; subnormal spacing
+    np.testing.assert_array_equal(onet.round_f16([1e5, -7e4, 65504.0, 65519.9]), [65504.0, -65504.0, 65504.0, 65504.0])
+    assert np.isnan(onet.round_f16([np.nan]))[0]
+    # eight times finer than bf16 in the normal range
+    v = np.linspace(1.0, 2.0, 4097)[:-1]
+    assert np.abs(onet.round_f16(v) - v).max() == 2.0 ** -11 and np.abs(onet.round_bf16(v) - v).max() == 2.0 ** -8
+
+
 def test_live_group_norm_matches_library_and_is_scale_invariant():
     """NEXT-2 pin: oracle.group_norm_live = torch.nn.functional.group_norm (library routine); the normalised output does
     not change when the window's pre-norm tensor is rescaled (eps -> 0)."""

@@ -44,3 +44,10 @@ def test_float32_variant_is_what_the_kernel_computes():
     a = opp.integrate_tophat(s, 16, dtype=np.float32)
     assert a.dtype == np.float32
     np.testing.assert_allclose(a, opp.integrate_tophat(s.astype(np.float64), 16), rtol=2e-6, atol=2e-7)
+
+
+def test_cluster_max_propagates_nan_as_its_first_occurrence():
+    """Hand example: a window holding NaNs yields the first NaN; windows without are unaffected."""
+    x = np.array([1.0, np.nan, 5.0, np.nan, 2.0, 7.0, 3.0, 0.0])
+    idx, val = opp.cluster_max(x, 4)
+    assert list(idx) == [1, 5] and np.isnan(val[0]) and val[1] == 7.0
