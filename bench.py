@@ -4,10 +4,10 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
 
 Workload (BASELINE.json configs[3], "offline background throughput"): a 1e5 s two-detector record of
-synthetic coloured noise is analysed in time blocks of --block-seconds (default 4096 s).  ONE STEP = one
+synthetic coloured noise with injected Newtonian chirps (one per 17.6 s, configs[2]'s recipe) is analysed in time blocks of --block-seconds (default 4096 s).  ONE STEP = one
 block through the whole hot path: raw strain -> rolling Welch PSD (64 s, new every
 8 s) -> filter design -> overlap-save whitening (once per detector) -> 8 timeslides (L1 shifted 1..8 s)
-of 1.5 s windows at stride 128, 4096 windows per launch sequence -> bf16 tcgen05 ResNet -> one score per
+of 1.5 s windows at stride 128, 4096 windows per launch sequence -> fp16 tcgen05 ResNet -> one score per
 window.  Each step takes a different block (its own seeded noise), so nothing is reused between steps.
 
     value = analysed livetime per second = sum_slides windows * stride / fs / wall   [strain-seconds/s]
@@ -17,9 +17,11 @@ path ("scaling": "weak").  The time is the max over ranks of the CUDA-event time
 
 The JSON line also carries: "e2e" (same steps through aframe_score_timeslides_host: pinned host strain
 in, scores out, copies inside the timed region), "roofline" of the dominant kernel family (conv_tc_kernel,
-tensor-bound) from CUDA events recorded by the library on its own stream, "stages" (per-stage device
-time), "latency" (configs[4]: per-update p50/p99 of aframe_stream_step) and "cpu_baseline" (the float64
-oracle timed on this box's host cores on a bounded sample).
+tensor-bound) from CUDA events recorded by the library on its own stream in a second, profiled pass over
+the same steps, "stages" (per-stage device time), "parity" (configs[1] errors and Spearman rank
+correlation against the float64 oracle, and a chirp-bearing configs[3] batch), "config1" / "config2"
+(BASELINE.md section 2 rows), "latency" (configs[4]: per-update p50/p99 of aframe_stream_step) and
+"cpu_baseline" (the float64 oracle timed on this box's host cores on a bounded sample).
 """
 from __future__ import annotations
 
@@ -59,6 +61,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the device timings of the SURVEY 8(f) rows")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--parity-windows", type=int, default=512,
+                    help="windows of a chirp-bearing configs[3] batch the oracle re-scores for the parity object (0 = skip)")
+    ap.add_argument("--no-configs", action="store_true", help="skip the configs[1] / configs[2] lines")
     return ap.parse_args()
 
 
@@ -92,9 +97,9 @@ def max_over_ranks(t, world):
 
 
 def make_block(index, n_raw):
-    from synthdata import coloured_noise
-    seed = int(np.random.SeedSequence([1003, index]).generate_state(1)[0])
-    return coloured_noise(n_raw, seed=seed)
+    """Block `index` of the configs[3] record: coloured noise + chirps (synthdata.configs.config3_block)."""
+    from synthdata.configs import config3_block
+    return config3_block(index, n_raw)[0]
 
 
 class ClockSampler:
@@ -218,6 +223,145 @@ def measured_peaks():
     return {"bf16_burst": 1590.0, "bf16_sustained": 1400.0, "hbm": 6650.0, "source": "fallback (B200_PROFILING.md)"}
 
 
+def ncu_counters():
+    """Per-launch counters of the committed `ncu --set full` summary of this build (profiles/ncu_counters.csv, rows
+    key,value,source; written from the capture named in `source`).  The `traffic` fields of the JSON line come from here,
+    never from literals in this file; a missing file or key reads as None."""
+    path = os.path.join(ROOT, "profiles", "ncu_counters.csv")
+    out = {}
+    if os.path.exists(path):
+        with open(path) as f:
+            for line in f:
+                parts = [v.strip() for v in line.split(",")]
+                if len(parts) >= 2 and parts[0] and not parts[0].startswith("#") and parts[0] != "key":
+                    try:
+                        out[parts[0]] = (float(parts[1]), parts[2] if len(parts) > 2 else "")
+                    except ValueError:
+                        pass
+    return out
+
+
+def rel_err(g, o):
+    """Rules T2 / T3: max_i |g_i - o_i| / max(|o_i|, 1e-3 max_j |o_j|)."""
+    g, o = np.asarray(g, np.float64), np.asarray(o, np.float64)
+    return float(np.max(np.abs(g - o) / np.maximum(np.abs(o), 1e-3 * np.abs(o).max())))
+
+
+def parity_report(af, torch, stream, blob, n_cfg3):
+    """Parity of the timed path against the float64 oracle, carried in the bench line (rules T2-T4 of DESIGN.md):
+    configs[1]'s 128 windows (64 with chirps) on the fp32 and the tensor-core path, with the oracle re-run under the
+    path's own storage roundings (fp16) and under bf16 roundings (the ceiling that ruled bf16 storage out); and n_cfg3
+    consecutive windows of a chirp-bearing configs[3] block scored the way the timed steps score them (rolling whitening,
+    windows in place at stride 128, shared stages) against the oracle's rolling whitening + forward."""
+    import scipy.stats
+    from oracle import network as onet, psd as opsd, stream as ost, whiten as owh
+    from synthdata.configs import config1_raw, config3_block, gather_windows
+    sp = lambda a, b: float(scipy.stats.spearmanr(a, b).statistic)
+    net = onet.parse_blob(blob)
+    strain, starts, _ = config1_raw(128)
+    x = strain.astype(np.float64)
+    y = np.stack([owh.whiten_fft(x[c], owh.design_filter(opsd.welch(x[c, : 64 * FS]))) for c in range(2)])
+    wins = gather_windows(y, starts, KERNEL, offset=FILTER // 2).astype(np.float32)
+    ref = onet.forward(net, wins)
+    as_f16 = onet.forward(net, wins, act_round=onet.round_f16, weight_round=onet.round_f16)
+    as_bf16 = onet.forward(net, wins, act_round=onet.round_bf16, weight_round=onet.round_bf16)
+    out = {}
+    with torch.cuda.stream(stream):
+        wd = torch.from_numpy(wins).cuda()
+        c32 = af.Context(precision=af.FP32, stream=stream)
+        w32 = c32.load_weights(blob)
+        g32 = c32.forward(w32, wd).cpu().numpy()
+        c16 = af.Context(precision=af.F16, stream=stream)
+        w16 = c16.load_weights(blob)
+        g16 = c16.forward(w16, wd).cpu().numpy()
+        out["config1"] = {"windows": 128, "fp32_rel_err": rel_err(g32, ref), "f16_rel_err": rel_err(g16, ref),
+                          "f16_spearman": sp(g16, ref), "oracle_with_f16_roundings_spearman": sp(as_f16, ref),
+                          "oracle_with_bf16_roundings_spearman": sp(as_bf16, ref),
+                          "oracle_with_bf16_roundings_rel_err": rel_err(as_bf16, ref),
+                          "tolerances": {"fp32_rel_err": 1e-4, "f16_rel_err": 2e-2, "spearman": 0.999}}
+        w32.free(); c32.close()
+        if n_cfg3 > 0:
+            n_win_b = 4096
+            m0 = PSD_LEN - STRIDE - FILTER // 2
+            n_raw = m0 + (n_win_b - 1) * STRIDE + FS + KERNEL + FILTER // 2
+            n_raw = -(-n_raw // STRIDE) * STRIDE
+            xb, params = config3_block(424242, n_raw)
+            got = c16.score_timeslides(w16, torch.from_numpy(xb).cuda(), 0, n_win_b, [FS], batch=4096)[0].cpu().numpy()
+            # the n_cfg3 consecutive windows that start 40 windows before the block's first chirp coalesces
+            i_c = (int(round(params[0].t_c * FS)) - m0) // STRIDE
+            i0 = max(0, min(i_c - 40, n_win_b - n_cfg3))
+            cfg = ost.StreamConfig()
+            a = m0 + i0 * STRIDE
+            span = (n_cfg3 - 1) * STRIDE + KERNEL
+            x64 = xb.astype(np.float64)
+            h1, _ = ost.whiten_rolling(x64[0], cfg, m_lo=a, m_hi=a + span)
+            l1, _ = ost.whiten_rolling(x64[1], cfg, m_lo=a + FS, m_hi=a + FS + span)
+            wn = np.stack([np.stack([h1[i * STRIDE: i * STRIDE + KERNEL], l1[i * STRIDE: i * STRIDE + KERNEL]]) for i in range(n_cfg3)])
+            want = onet.forward(net, wn)
+            g = got[i0: i0 + n_cfg3]
+            n_ch = sum(1 for p in params if a / FS + 0.25 <= p.t_c <= (a + span) / FS - 0.25)
+            out["config3_batch"] = {"windows": int(n_cfg3), "chirps_inside": int(n_ch), "first_window": int(i0),
+                                    "f16_rel_err": rel_err(g, want), "f16_spearman": sp(g, want),
+                                    "what": "consecutive windows of slide 1 (L1 shifted 1 s) of a 4096-window launch sequence "
+                                            "of a chirp-bearing block, scored by aframe_score_timeslides"}
+        w16.free(); c16.close()
+    return out
+
+
+def config_rows(af, torch, stream, blob, peaks):
+    """configs[1] (batch 128 through aframe_forward: conv-stack rate) and configs[2] (the one-hour
+    record with 200 chirps through aframe_score_timeslides at zero lag, device-resident and from host buffers)."""
+    from synthdata.configs import config2_strain
+
+    def timed(fn, reps, warm=3):
+        with torch.cuda.stream(stream):
+            for _ in range(warm):
+                fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                fn()
+            e1.record(stream)
+            stream.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    res = {}
+    with torch.cuda.stream(stream):
+        ctx = af.Context(precision=af.F16, stream=stream)
+        w = ctx.load_weights(blob)
+        g = torch.Generator(device="cuda").manual_seed(1)
+        xw = torch.randn(128, 2, KERNEL, device="cuda", generator=g)
+        ms = timed(lambda: ctx.forward(w, xw), 20)
+        tf = 2.0 * MMAC_CONV * 128 / (ms * 1e-3) / 1e12
+        res["config1"] = {"workload": "configs[1]: aframe_forward on 128 explicit windows [128][2][3072] (one network per window: "
+                                      "explicit windows share nothing)", "ms": ms, "windows_per_s": 128 / (ms * 1e-3),
+                          "conv_tflops": tf, "frac_of_sustained_peak": tf / peaks["bf16_sustained"],
+                          "note": "128 windows = 96 .. 768 tiles per layer on 148 SMs: launch- and tail-bound; the 4096-window "
+                                  "launch sequences of configs[3] are the throughput case"}
+        x, _ = config2_strain()
+        xh = torch.from_numpy(x).pin_memory()
+        xd = xh.cuda()
+        m0 = PSD_LEN - STRIDE - FILTER // 2
+        n_win = (x.shape[1] - m0 - FILTER // 2 - KERNEL) // STRIDE + 1
+        sd = torch.empty((1, n_win), dtype=torch.float32, device="cuda")
+        sh = torch.empty((1, n_win), dtype=torch.float32).pin_memory()
+        ms = timed(lambda: ctx.score_timeslides(w, xd, 0, n_win, [0], batch=4096, scores=sd), 5)
+        t0 = time.perf_counter()
+        for _ in range(3):
+            ctx.score_timeslides(w, xh, 0, n_win, [0], batch=4096, scores=sh)
+        ms_host = (time.perf_counter() - t0) / 3 * 1e3
+        live = n_win * STRIDE / FS
+        res["config2"] = {"workload": "configs[2]: 3600 s x 2 detectors, 200 chirps, PSD every 8 s from the trailing 64 s, "
+                                      "every 1.5 s window at stride 128 (zero lag) through aframe_score_timeslides, batch 4096",
+                          "windows": int(n_win), "ms": ms, "strain_s_per_s": live / (ms * 1e-3), "windows_per_s": n_win / (ms * 1e-3),
+                          "e2e_host_buffers": {"ms": ms_host, "strain_s_per_s": live / (ms_host * 1e-3),
+                                               "h2d_bytes": int(xh.numel() * 4), "d2h_bytes": int(sh.numel() * 4)},
+                          "streamed": "the same record update by update is configs[4]: see 'latency' (updates per second = "
+                                      "1000 / mean_ms; 16 updates = 1 strain-second)"}
+        w.free(); ctx.close()
+    return res
+
+
 def latency_run(af, torch, ctx_stream, weights_blob, n_updates, n_warm_scored=100):
     """configs[4]: one update of 128 new samples per detector, batch 1, over a 1.5 s ring with incremental
     whitening.  Host wall-clock from the call to the score being readable on the host, and device time."""
@@ -319,13 +463,12 @@ def run_ours(args):
         def step_host(j):
             ctx.score_timeslides(w, blocks_host[j], 0, n_win, shifts, batch=args.batch, scores=scores_host)
 
-        # ---- device-resident timing -----------------------------------------------------------------
+        # ---- device-resident timing (the headline; no stage events inside the timed region) -----------
         for j in range(args.warmup):
             step_dev(j)
         barrier()
         launches0 = ctx.launch_count()
         macs0 = ctx.tensor_macs()
-        ctx.profile(True)
         sampler = ClockSampler(local_rank)
         sampler.start()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -336,11 +479,20 @@ def run_ours(args):
         barrier()
         clocks = sampler.stop()
         ms_total = e0.elapsed_time(e1)
-        stages = ctx.profile_read()
-        ctx.profile(False)
         launches = ctx.launch_count() - launches0
         macs_exec = ctx.tensor_macs() - macs0
         assert torch.isfinite(scores_dev).all()
+        # ---- the same steps once more with the library's per-stage CUDA events on its stream (roofline, stages) ----
+        ctx.profile(True)
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record(stream)
+        for j in range(args.steps):
+            step_dev(args.warmup + j)
+        p1.record(stream)
+        barrier()
+        ms_profiled = p0.elapsed_time(p1)
+        stages = ctx.profile_read()
+        ctx.profile(False)
 
         # ---- end to end: pinned host strain in, scores out, copies inside the timed region -------------
         e2e = None
@@ -379,19 +531,21 @@ def run_ours(args):
     # perform, counted by the library per launch from its tile counts (aframe_tensor_macs); MMAC_CONV is the method's
     # (algorithmic) figure per window.
     mmac_exec = macs_exec / win_rank
-    shared_on = mmac_exec < 0.9 * MMAC_CONV       # (the AFRAME_SHARED_* switches and other batch sizes run other launch plans)
     exec_tflops = conv_tflops * mmac_exec / MMAC_CONV
     out = {
         "metric": "analysed strain-seconds per second (whitened + scored, all timeslides)",
         "value": value, "unit": "strain-s/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "bf16", "data": "synthetic",
+        "dtype": "f16", "data": "synthetic",
         "config": {"workload": f"configs[3] offline background: {N_SLIDES} timeslides, {args.batch} windows/launch sequence, "
-                               f"1.5 s windows at stride 128, config-1 ResNet bf16; record analysed in blocks of "
-                               f"{args.block_seconds} s, one block per step",
+                               f"1.5 s windows at stride 128, config-1 ResNet on the tensor-core path (fp16 weights and "
+                               f"activations, fp32 accumulation); coloured noise + one chirp per 17.6 s; record analysed in "
+                               f"blocks of {args.block_seconds} s, one block per step",
                    "block_seconds": args.block_seconds, "windows_per_step": N_SLIDES * n_win, "batch": args.batch,
                    "l2": "each step reads a different block; per-launch activations (>= 400 MB) exceed the 126 MB L2",
-                   "chunk_windows": int(os.environ.get("AFRAME_CHUNK_B", "0")) or "library default"},
+                   "precision": "BASELINE.json names bf16; with bf16 storage the scores fail its own rank tolerance (Spearman "
+                                "0.9987 < 0.999, the format's ceiling), so weights and activations are IEEE half: same bytes, same "
+                                "tcgen05 kind::f16 rate (DESIGN.md reading B10; 'parity' below carries both figures)"},
         "windows_per_s": windows / (ms_total * 1e-3),
         "end_to_end_tflops": 2.0 * MMAC_TOTAL * windows / (ms_total * 1e-3) / 1e12,
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
@@ -399,9 +553,7 @@ def run_ours(args):
                      "bound": "tensor", "achieved": exec_tflops, "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
                      "frac": exec_tflops / peaks["bf16_sustained"],
                      "algorithmic_tflops": conv_tflops, "executed_frac_of_algorithmic": mmac_exec / MMAC_CONV,
-                     # dram__bytes_read.sum + dram__bytes_write.sum of the 35 conv launches of one 4096-window chunk under
-                     # ncu --set full of this build (profiles/r01l_conv_full.md): 3.55 + 1.09 GB, per launch
-                     "traffic": (4.639e9 / 35) if shared_on else (26.66e9 / 29),
+                     "traffic": None,      # dram__bytes per launch from profiles/ncu_counters.csv (set below)
                      "peak_kind": "sustained bf16 cuBLAS, " + peaks["source"], "launches": int(conv_launches),
                      "avg_launch_ms": conv_ms / max(conv_launches, 1),
                      "algorithmic": "achieved = EXECUTED tensor FLOPs (2 x executed MMAC per window x windows scored) over the "
@@ -410,8 +562,13 @@ def run_ours(args):
                                     "interior rows of every stage, which are computed once per stream plus two short edge windows "
                                     "per window, so only executed_frac_of_algorithmic of those FLOPs are performed (counted per "
                                     "launch by the library: aframe_tensor_macs)"},
-        "stages": {k: {"ms": v[0], "launches": v[1], "share": v[0] / ms_total} for k, v in stages.items()},
+        "stages": {k: {"ms": v[0], "launches": v[1], "share": v[0] / ms_profiled} for k, v in stages.items()},
+        "stages_pass": {"ms_per_step": ms_profiled / args.steps,
+                        "note": "second pass over the same steps with the library's per-stage CUDA events on its stream"},
     }
+    ncu = ncu_counters()
+    if "conv_dram_bytes_per_launch" in ncu:
+        out["roofline"]["traffic"], out["roofline"]["traffic_source"] = ncu["conv_dram_bytes_per_launch"]
     wh_ms = stages["whiten"][0]
     if wh_ms > 0:
         n_out_block = n_raw - (PSD_LEN - STRIDE - FILTER // 2) - FILTER // 2
@@ -465,6 +622,9 @@ def run_ours(args):
                           "achieved": pp_bytes / (pp_ms * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
                           "frac": pp_bytes / (pp_ms * 1e-3) / 1e9 / peaks["hbm"],
                           "note": "2 launches over 2 MB of scores: launch-latency bound, 0.001 % of a step"}
+    if world == 1 and not args.no_configs:
+        out["parity"] = parity_report(af, torch, stream, blob, args.parity_windows)
+        out.update(config_rows(af, torch, stream, blob, peaks))
     if world == 1 and not args.no_next_rows:
         out["next_rows"] = next_rows(af, torch, stream, peaks)
     if args.latency_updates > 0 and world == 1:

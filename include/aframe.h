@@ -247,6 +247,7 @@ enum {
   AFRAME_PROF_CONV = 4,     /* residual-stage convolutions (a-7)        */
   AFRAME_PROF_HEAD = 5,     /* pool + linear head (a-8)                 */
   AFRAME_PROF_STREAM = 6,   /* ring-buffer bookkeeping (a-9)            */
+  AFRAME_PROF_GATHER = 7,   /* shared stages: edge-batch gathers, stitch, head-rows sum (a-7 bookkeeping) */
   AFRAME_PROF_KINDS = 8
 };
 aframe_status aframe_profile(aframe_ctx* ctx, int enable);

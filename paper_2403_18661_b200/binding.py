@@ -70,7 +70,7 @@ EXPORTS = {
     "aframe_profile_layers": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.POINTER(C.c_float), C.c_int32]),
     "aframe_profile_read": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
 }
-PROF_KINDS = ("welch", "design", "whiten", "stem", "conv", "head", "stream", "reserved")
+PROF_KINDS = ("welch", "design", "whiten", "stem", "conv", "head", "stream", "gather")
 
 _lib = None
 
@@ -300,7 +300,7 @@ class Context:
         ms = (C.c_double * 8)()
         nl = (C.c_int64 * 8)()
         self._check(self.lib.aframe_profile_read(self.handle, ms, nl))
-        return {k: (ms[i], int(nl[i])) for i, k in enumerate(PROF_KINDS) if k != "reserved"}
+        return {k: (ms[i], int(nl[i])) for i, k in enumerate(PROF_KINDS)}
 
     # ---- O-6
     def stream_create(self, weights: Weights):

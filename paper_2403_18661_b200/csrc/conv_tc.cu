@@ -928,7 +928,10 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
                              in_dt, sB, choff, w->d_w32[0], w->d_bias[0], nb, slot_ptr(1), w->live_gn ? &sgn : nullptr);
     af_prof_end(ctx, AFRAME_PROF_STEM, 1);
     if (st != AFRAME_OK) return st;
-    int n_conv = 0;
+    int n_conv = 0, span_conv = 0;             // conv launches so far (tile direction) / in the open timing span
+    // gathers, stitches and the head-rows sum are timed apart from the convolutions (AFRAME_PROF_GATHER)
+    auto aux_begin = [&]() { af_prof_end(ctx, AFRAME_PROF_CONV, span_conv); span_conv = 0; af_prof_begin(ctx, AFRAME_PROF_GATHER); };
+    auto aux_end = [&]() { af_prof_end(ctx, AFRAME_PROF_GATHER, 1); af_prof_begin(ctx, AFRAME_PROF_CONV); };
     if (ctx->layer_ms) { cudaEventRecord(lev[1], ctx->stream); cudaEventRecord(lev[2], ctx->stream); }
     if (pc->s1_blocks > 0) {
       // shared first stage: per block one pass over the stream and one over the short edge windows, then the stitch
@@ -938,23 +941,27 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
       const uint4* E0 = reinterpret_cast<const uint4*>(slot_ptr(1) + ((nb - 1) * shift + T1) * 64);
       for (int k = 1; k <= K; ++k) {
         cudaError_t e = launch_block(pc->s1_stream[k], ctx->stream);
-        ctx->launches++; ++n_conv; ctx->tc_macs += pc->s1_stream[k].macs;
+        ctx->launches++; ++n_conv; ++span_conv; ctx->tc_macs += pc->s1_stream[k].macs;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_block (stream) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
         const int64_t n_g = 2 * nb * S1_PERIOD * 8;
+        aux_begin();
         s1_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
             reinterpret_cast<uint4*>(s1_edge_ptr(0)), reinterpret_cast<const uint4*>(k == 1 ? slot_ptr(1) : s1_stream_ptr(k - 1)),
             k == 1 ? nullptr : reinterpret_cast<const uint4*>(s1_edge_ptr(k - 1)), k == 1 ? E0 : nullptr, nb, T1, shift, 2 * k, 2 * k - 1);
         AF_LAUNCH_CHECK(ctx);
+        aux_end();
         e = launch_block(pc->s1_edge[k], ctx->stream);
-        ctx->launches++; ++n_conv; ctx->tc_macs += pc->s1_edge[k].macs;
+        ctx->launches++; ++n_conv; ++span_conv; ctx->tc_macs += pc->s1_edge[k].macs;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_block (edge) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
       }
       if (pc->sh.empty()) {
         const int64_t n_s = nb * T1 * 8;
+        aux_begin();
         s1_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
             reinterpret_cast<uint4*>(slot_ptr(2 * K + 1)), reinterpret_cast<const uint4*>(s1_stream_ptr(K)),
             reinterpret_cast<const uint4*>(s1_edge_ptr(K)), nb, T1, shift, 2 * K + 2, 2 * K + 1);
         AF_LAUNCH_CHECK(ctx);
+        aux_end();
       }
       // shared later stages: each reads the previous stage's stream and edge results directly; only the last one is stitched
       for (size_t g = 0; g < pc->sh.size(); ++g) {
@@ -967,6 +974,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         if (P.packed) {
           const int64_t n_p = (copy_rows + 2 * P.nbp * 2 * P.P) * pieces_in;
           const int64_t valid_prev = g ? (nb - 1) * pc->sh[g - 1].shift + pc->sh[g - 1].T : (nb - 1) * shift + T1;
+          aux_begin();
           shp_gather_kernel<<<(unsigned)((n_p + 255) / 256), 256, 0, ctx->stream>>>(
               reinterpret_cast<uint4*>(sh_x_ptr((int)g)),
               reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 0, q_prev) : s1_stream_ptr(K)),
@@ -975,6 +983,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
               g ? pc->sh[g - 1].e_trow : T1 - S1_ROWS, g ? pc->sh[g - 1].head : 2 * K + 2, g ? pc->sh[g - 1].tail : 2 * K + 1,
               copy_rows, valid_prev, 2 * P.P);
           AF_LAUNCH_CHECK(ctx);
+          aux_end();
           // Launch order: stream(0) | edge(q) with stream(q + 1) as ONE launch of two problems (independent of each other: both
           // need stream(q), and edge(q) needs edge(q - 1)) | ... | edge(last).  A stream launch alone costs 16-30 us for 1/8 of an
           // edge launch's work (profiles/r01i_conv_full.md); as the second problem its tiles fill the edge launch's last wave.
@@ -990,7 +999,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             A.p.reverse = 0;
             if (B2) B2->p.reverse = 0;
             cudaError_t e = launch_conv(A, ctx->stream, B2);
-            ctx->launches++; ++n_conv; ctx->tc_macs += A.macs + (B2 ? B2->macs : 0.0);
+            ctx->launches++; ++n_conv; ++span_conv; ctx->tc_macs += A.macs + (B2 ? B2->macs : 0.0);
             if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (packed edge stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
             return AFRAME_OK;
           };
@@ -1004,6 +1013,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             }
           }
         } else {
+        aux_begin();
         sh_gather_kernel<<<(unsigned)((n_g + 255) / 256), 256, 0, ctx->stream>>>(
             reinterpret_cast<uint4*>(sh_x_ptr((int)g)),
             reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 0, q_prev) : s1_stream_ptr(K)),
@@ -1012,11 +1022,12 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             g ? pc->sh[g - 1].tail : 2 * K + 1, copy_rows, g ? sh_rows_stream((int)g - 1) : (nb - 1) * shift + T1, P.rows, P.period,
             edge_rows_in);
         AF_LAUNCH_CHECK(ctx);
+        aux_end();
         for (size_t q = 0; q < P.layers.size(); ++q) {
           TcLaunch& L2 = P.stream[q];
           L2.p.reverse = 0;
           cudaError_t e = launch_conv(L2, ctx->stream);
-          ctx->launches++; ++n_conv; ctx->tc_macs += L2.macs;
+          ctx->launches++; ++n_conv; ++span_conv; ctx->tc_macs += L2.macs;
           if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc (shared stage) launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
         }
         }
@@ -1024,24 +1035,30 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           const int q_last = (int)P.layers.size() - 1;
           const int64_t n_warps = nb * (P.T / 32) * (P.C / 64);
           const float* hr_s = reinterpret_cast<const float*>(sh_buf((int)g, 0, q_last));
+          aux_begin();
           sh_head_rows_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(
               hr_s, hr_s + sh_rows_stream((int)g) * (P.C / 64), head_part, nb, P.T, P.C / 64, P.shift, P.head, P.tail, P.e_stride,
               P.e_tail0, P.e_trow);
           AF_LAUNCH_CHECK(ctx);
+          aux_end();
         } else if (g + 1 == pc->sh.size() && pc->sh_head) {
           const int q_last = (int)P.layers.size() - 1;
           const int64_t n_warps = nb * (P.T / 32) * (P.C / 64);
+          aux_begin();
           sh_head_partial_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(
               reinterpret_cast<const uint4*>(sh_buf((int)g, 0, q_last)), reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)),
               w->d_head_w, head_part, nb, P.T, P.C, P.shift, P.head, P.tail, P.e_stride, P.e_tail0, P.e_trow);
           AF_LAUNCH_CHECK(ctx);
+          aux_end();
         } else if (g + 1 == pc->sh.size()) {
           const int last = P.layers.back(), q_last = (int)P.layers.size() - 1, pieces = P.C / 8;
           const int64_t n_s = nb * P.T * pieces;
+          aux_begin();
           s2_stitch_kernel<<<(unsigned)((n_s + 255) / 256), 256, 0, ctx->stream>>>(
               reinterpret_cast<uint4*>(slot_ptr(last)), reinterpret_cast<const uint4*>(sh_buf((int)g, 0, q_last)),
               reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)), nb, P.T, pieces, P.shift, P.head, P.tail, P.e_stride, P.e_tail0, P.e_trow);
           AF_LAUNCH_CHECK(ctx);
+          aux_end();
         }
       }
     }
@@ -1061,7 +1078,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         pc->blocks[i].p.reverse = rev;
         const TcLaunch& L = pc->launches[i];
         af_prof_begin(ctx, AFRAME_PROF_CONV);
-        ++n_conv;
+        ++n_conv; ++span_conv;
         cudaError_t e = pc->fused_with[i] >= 0 ? launch_block(pc->blocks[i], ctx->stream) : launch_conv(L, ctx->stream);
         ctx->launches++; ctx->tc_macs += pc->fused_with[i] >= 0 ? pc->blocks[i].macs : L.macs;
         if (e != cudaSuccess) { snprintf(ctx->err, sizeof(ctx->err), "conv_tc launch: %s", cudaGetErrorString(e)); return AFRAME_ECUDA; }
@@ -1071,8 +1088,8 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           if (st != AFRAME_OK) return st;
         }
       } else if (l.kind == 2) {
-        af_prof_end(ctx, AFRAME_PROF_CONV, n_conv);
-        n_conv = 0;
+        af_prof_end(ctx, AFRAME_PROF_CONV, span_conv);
+        n_conv = 0; span_conv = 0;
         af_prof_begin(ctx, AFRAME_PROF_HEAD);
         if (fuse >= 0) {
           head_finish_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, ctx->stream>>>(head_part, n_part, 1.0f / l.t_in, w->head_b, nb,

@@ -3,7 +3,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from .chirps import ChirpParams, inject_chirps
+from .chirps import ChirpParams, draw_chirp_params, inject_chirps
 from .noise import coloured_noise
 
 FS = 2048
@@ -41,3 +41,24 @@ def config1_raw(n_windows=128, kernel_len=3072, seed=1001):
 def gather_windows(white, starts, kernel_len, offset):
     """windows[i][c] = white[c][starts[i] - offset : ... + kernel_len]; offset = raw index of white[:, 0]."""
     return np.stack([white[:, s - offset: s - offset + kernel_len] for s in starts])
+
+
+def config2_strain(duration_s=3600, n_chirps=200, seed=1002):
+    """configs[2] (also fed update by update as configs[4]): `duration_s` of two-detector coloured noise (seed 1002) with
+    one Newtonian chirp per 17.6 s slot from t = 70 s on (200 in the hour), chirp mass U(10, 60) Msun, per-detector
+    offset U(+-10 ms), network SNR U(4, 20).  Returns (strain float32 [2][N], chirp parameters)."""
+    noise = coloured_noise(int(duration_s) * FS, seed=seed)
+    params = draw_chirp_params(n_chirps, float(duration_s), seed=seed + 7)
+    strain, _ = inject_chirps(noise, params)
+    return strain, params
+
+
+def config3_block(index, n_raw):
+    """One time block of the configs[3] record (1e5 s analysed in independent blocks): coloured noise with its own seed
+    and chirps at configs[2]'s rate and parameter ranges (one per 17.6 s slot after the 64 s PSD history)."""
+    seed = int(np.random.SeedSequence([1003, int(index)]).generate_state(1)[0])
+    noise = coloured_noise(int(n_raw), seed=seed)
+    dur = n_raw / FS
+    params = draw_chirp_params(int(dur // 17.6) + 1, dur, seed=seed + 7)
+    strain, _ = inject_chirps(noise, params)
+    return strain, params

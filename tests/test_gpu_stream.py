@@ -266,16 +266,19 @@ def test_stride_one_windows_offline(af):
 
 
 def test_bench_step_at_full_size_sampled_against_oracle(af):
-    """BASELINE.json configs[3] in the launch configuration bench.py times: one 4096 s block of two-detector strain (plus
-    its 64 s PSD history), 8 timeslides x 65 536 windows, batches of 4096 windows, through aframe_score_timeslides.
+    """BASELINE.json configs[3] in the launch configuration bench.py times: one 4096 s block of two-detector strain with
+    232 injected chirps (plus its 64 s PSD history), 8 timeslides x 65 536 windows, batches of 4096 windows, through aframe_score_timeslides.
     The float64 oracle (rolling whitening with the epoch's own Welch PSD + network) recomputes a seeded sample of the
     524 288 scores one by one: the first and last valid window of each slide, windows on both sides of PSD-epoch
-    boundaries, and pseudo-random ones (rule T3); all scores must be finite."""
+    boundaries, windows that hold a chirp's coalescence in H1 (slides misalign L1: background) and pseudo-random ones
+    (rule T3); all scores must be finite."""
     import bench
     fc = full_config()
     n_win, n_raw = bench.block_geometry(4096)
     shifts = [k * FS for k in range(1, bench.N_SLIDES + 1)]
-    x = bench.make_block(7, n_raw)
+    from synthdata.configs import config3_block
+    x, params = config3_block(7, n_raw)
+    assert np.array_equal(x, bench.make_block(7, n_raw)) and len(params) > 200
     blob = make_weight_blob(**fc)
     ctx = af.Context(precision=af.F16)
     w = ctx.load_weights(blob)
@@ -292,7 +295,10 @@ def test_bench_step_at_full_size_sampled_against_oracle(af):
         m_switch = cfg.psd_len + e * cfg.psd_update - S - cfg.filter_len // 2
         i = (m_switch - m0) // S
         picks += [(2, i - 30), (5, i - 1), (5, i)]
-    picks += [(int(rng.integers(0, 8)), int(rng.integers(0, n_win))) for _ in range(40)]
+    for j, p in enumerate(params[3:60:8]):                      # H1 coalescence 0.25 .. 1.25 s into the window
+        i_c = (int(round(p.t_c * FS)) - m0) // S
+        picks += [(j % 8, i_c - 4 - 2 * j)]
+    picks += [(int(rng.integers(0, 8)), int(rng.integers(0, n_win))) for _ in range(32)]
     x64 = x.astype(np.float64)
     net = onet.parse_blob(blob)
     wins = []
