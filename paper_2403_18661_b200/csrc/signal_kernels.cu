@@ -2,8 +2,7 @@
 //
 //  O-1 (reading A1)  welch_periodogram_kernel + psd_mean_kernel
 //  O-2 (readings A3-A6)            filter_design_kernel (double precision, one CTA per epoch x channel)
-//  O-3 ("whitened in the frequency-domain, and transformed back to time-domain")
-//                                  whiten_os_kernel: rFFT -> multiply by real H -> irFFT, valid part stored
+//  (O-3, the overlap-save whitening, lives in signal_fft64.cu)
 #include "fft.cuh"
 #include <atomic>
 
@@ -180,108 +179,6 @@ filter_design_kernel(const float* __restrict__ psd, int F_w, int C, double fs, d
 }
 
 // --------------------------------------------------------------------------------------------------
-// Overlap-save whitening: one CTA per (block, channel).  Block of NOS real samples -> M = NOS/2 complex
-// FFT -> untangle, multiply by real H, re-tangle -> inverse FFT (conjugation trick) -> store valid part.
-// --------------------------------------------------------------------------------------------------
-template <int OUT_DT>
-__global__ void __launch_bounds__(256, 3)
-whiten_os_kernel(const float* __restrict__ strain, int64_t n_samples, int64_t ld, const float* __restrict__ H, int C,
-                 int64_t in0, int64_t out_total, int64_t epoch_len, int blocks_per_epoch, int L, float scale,
-                 const float2* __restrict__ tw, void* __restrict__ out_v, int64_t ld_out) {
-  constexpr int NOS = AF_NOS, M = NOS / 2, NT = 256;
-  __shared__ float2 s[fft_smem_elems(M)];
-  const int tid = threadIdx.x;
-  const int c = blockIdx.y;
-  const int64_t e = blockIdx.x / blocks_per_epoch;
-  const int sb = blockIdx.x % blocks_per_epoch;
-  const int valid = NOS - L;
-  const int64_t out0 = e * epoch_len + (int64_t)sb * valid;
-  int64_t n_valid = epoch_len - (int64_t)sb * valid;
-  if (n_valid > valid) n_valid = valid;
-  if (n_valid > out_total - out0) n_valid = out_total - out0;
-  if (n_valid <= 0) return;
-  const int64_t x0 = in0 + out0;
-  const float* x = strain + (int64_t)c * ld;
-  const float* Hc = H + (e * C + c) * (int64_t)(M + 1);
-
-  const bool vec_ok = (((uintptr_t)(x + x0)) & 7) == 0 && (x0 + NOS <= n_samples);
-  if (vec_ok) {
-    const float2* x2 = reinterpret_cast<const float2*>(x + x0);
-#pragma unroll 4
-    for (int n = tid; n < M; n += NT) {
-      const float2 v = __ldg(x2 + n);
-      s[fft_pad(n)] = make_float2(v.x * scale, v.y * scale);
-    }
-  } else {
-    for (int n = tid; n < M; n += NT) {
-      const int64_t i0 = x0 + 2 * n;
-      const float a = (i0 < n_samples) ? x[i0] * scale : 0.f;
-      const float b = (i0 + 1 < n_samples) ? x[i0 + 1] * scale : 0.f;
-      s[fft_pad(n)] = make_float2(a, b);
-    }
-  }
-  __syncthreads();
-  fft_smem<float2, M, NT>(s, tw, tid);
-
-  for (int k = tid; k <= M / 2; k += NT) {
-    const int km = (M - k) & (M - 1);
-    const float2 zk = s[fft_pad(k)], zm = s[fft_pad(km)];
-    const float2 ee = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
-    const float2 oo = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
-    const float2 w = tw[k * (AF_TW_N / NOS)];
-    const float2 wo = cmul(w, oo);
-    const float hk = Hc[k], hm = Hc[M - k];
-    const float2 yk = make_float2(hk * (ee.x + wo.x), hk * (ee.y + wo.y));     // Y[k]
-    const float2 ym = make_float2(hm * (ee.x - wo.x), hm * (ee.y - wo.y));     // conj(Y[M-k])
-    const float2 ep = make_float2(0.5f * (yk.x + ym.x), 0.5f * (yk.y + ym.y));
-    const float2 op = cmul(make_float2(0.5f * (yk.x - ym.x), 0.5f * (yk.y - ym.y)), cconj(w));
-    // Z'[k] = E' + i O';  Z'[M-k] = conj(E') + i conj(O');  store CONJUGATED for the inverse transform
-    const float2 z1 = make_float2(ep.x - op.y, ep.y + op.x);
-    s[fft_pad(k)] = cconj(z1);
-    if (k != 0 && k != M / 2) {
-      const float2 z2 = make_float2(ep.x + op.y, -ep.y + op.x);
-      s[fft_pad(km)] = cconj(z2);
-    }
-  }
-  __syncthreads();
-  fft_smem<float2, M, NT>(s, tw, tid);
-
-  // x[2n] = Re r[n], x[2n+1] = -Im r[n]  (1/M folded into H); valid outputs are i in [L/2, L/2 + n_valid)
-  const int half = L / 2;
-  if (OUT_DT != AF_DT_F32) {                         // 16-bit output: bf16, or fp16 (saturating)
-    uint16_t* o = reinterpret_cast<uint16_t*>(out_v) + (int64_t)c * ld_out + out0;
-    auto cvt1 = [](float v) -> uint16_t {
-      if (OUT_DT == AF_DT_BF16) return __bfloat16_as_ushort(__float2bfloat16_rn(v));
-      return (uint16_t)(af_act_pack2(v, 0.f) & 0xffffu);
-    };
-    const bool st_vec = ((((uintptr_t)o) & 3) == 0) && ((half & 1) == 0);
-    for (int n = tid; n < M; n += NT) {
-      const float2 r = s[fft_pad(n)];
-      const int64_t i0 = 2 * n - half;
-      if (st_vec && i0 >= 0 && i0 + 1 < n_valid) {
-        *reinterpret_cast<uint32_t*>(o + i0) = (uint32_t)cvt1(r.x) | ((uint32_t)cvt1(-r.y) << 16);
-      } else {
-        if (i0 >= 0 && i0 < n_valid) o[i0] = cvt1(r.x);
-        if (i0 + 1 >= 0 && i0 + 1 < n_valid) o[i0 + 1] = cvt1(-r.y);
-      }
-    }
-  } else {
-    float* o = reinterpret_cast<float*>(out_v) + (int64_t)c * ld_out + out0;
-    const bool st_vec = ((((uintptr_t)o) & 7) == 0) && ((half & 1) == 0);
-    for (int n = tid; n < M; n += NT) {
-      const float2 r = s[fft_pad(n)];
-      const int64_t i0 = 2 * n - half;
-      if (st_vec && i0 >= 0 && i0 + 1 < n_valid) {
-        *reinterpret_cast<float2*>(o + i0) = make_float2(r.x, -r.y);
-      } else {
-        if (i0 >= 0 && i0 < n_valid) o[i0] = r.x;
-        if (i0 + 1 >= 0 && i0 + 1 < n_valid) o[i0 + 1] = -r.y;
-      }
-    }
-  }
-}
-
-// --------------------------------------------------------------------------------------------------
 // host launchers
 // --------------------------------------------------------------------------------------------------
 aframe_status af_launch_welch_periodograms(aframe_ctx* ctx, const float* d_strain, int64_t ld, int64_t first_seg,
@@ -360,30 +257,6 @@ aframe_status af_launch_filter_design(aframe_ctx* ctx, const float* d_psd, int64
   }
 #undef AF_FD_CASE
   af_prof_end(ctx, AFRAME_PROF_DESIGN, 1);
-  AF_LAUNCH_CHECK(ctx);
-  return AFRAME_OK;
-}
-
-aframe_status af_launch_whiten_os(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
-                                  const float* d_H, int64_t in0, int64_t out_total, int64_t epoch_len, int64_t n_epochs,
-                                  void* d_out, int64_t ld_out, int out_dt) {
-  if (out_total <= 0 || n_epochs <= 0) return AFRAME_OK;
-  const aframe_config& cfg = ctx->cfg;
-  const int valid = AF_NOS - cfg.filter_len;
-  const int bpe = (int)((epoch_len + valid - 1) / valid);
-  const float scale = ldexpf(1.0f, cfg.strain_scale_log2);
-  dim3 grid((unsigned)(n_epochs * bpe), (unsigned)af_nch(ctx));
-  af_prof_begin(ctx, AFRAME_PROF_WHITEN);
-  if (out_dt == AF_DT_BF16)
-    whiten_os_kernel<AF_DT_BF16><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, af_nch(ctx), in0, out_total,
-                                                                epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
-  else if (out_dt == AF_DT_F16)
-    whiten_os_kernel<AF_DT_F16><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, af_nch(ctx), in0, out_total,
-                                                               epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
-  else
-    whiten_os_kernel<AF_DT_F32><<<grid, 256, 0, ctx->stream>>>(d_strain, n_samples, ld, d_H, af_nch(ctx), in0, out_total,
-                                                               epoch_len, bpe, cfg.filter_len, scale, ctx->d_tw32, d_out, ld_out);
-  af_prof_end(ctx, AFRAME_PROF_WHITEN, 1);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }
