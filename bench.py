@@ -308,6 +308,39 @@ def parity_report(af, torch, stream, blob, n_cfg3):
     return out
 
 
+def fft_rows(af, torch, stream, peaks):
+    """The batched real transform on its own (aframe_rfft8192 / aframe_irfft8192): 8192 rows of 8192 samples (268 MB in,
+    269 MB out per call: larger than the 126 MB L2), CUDA events on the library's stream.  Algorithmic bytes: each row is
+    read once and written once."""
+    rows = 8192
+    out = {}
+    with torch.cuda.stream(stream):
+        ctx = af.Context(precision=af.FP32, stream=stream)
+        g = torch.Generator(device="cuda").manual_seed(3)
+        x = torch.randn(rows, 8192, device="cuda", generator=g)
+        spec = torch.empty((rows, 4097, 2), dtype=torch.float32, device="cuda")
+        back = torch.empty_like(x)
+        for name, fn, nbytes in (("rfft", lambda: ctx.rfft8192(x, out=spec), x.numel() * 4 + spec.numel() * 4),
+                                 ("irfft", lambda: ctx.irfft8192(spec, out=back), x.numel() * 4 + spec.numel() * 4)):
+            for _ in range(3):
+                fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(10):
+                fn()
+            e1.record(stream)
+            stream.synchronize()
+            ms = e0.elapsed_time(e1) / 10
+            gbs = nbytes / (ms * 1e-3) / 1e9
+            out["roofline_" + name] = {"kernel": name + "8192_kernel (64 x 64 register transform, standalone)", "bound": "hbm",
+                                       "achieved": gbs, "peak": peaks["hbm"], "unit": "GB/s", "frac": gbs / peaks["hbm"],
+                                       "ms": ms, "rows": rows, "traffic": None,
+                                       "algorithmic": "8192 fp32 samples in, 4097 complex bins out per row (and back)"}
+        assert float((back - x).abs().max()) <= 1e-4
+        ctx.close()
+    return out
+
+
 def config_rows(af, torch, stream, blob, peaks):
     """configs[1] (batch 128 through aframe_forward: conv-stack rate) and configs[2] (the one-hour
     record with 200 chirps through aframe_score_timeslides at zero lag, device-resident and from host buffers)."""
@@ -522,6 +555,7 @@ def run_ours(args):
         return
 
     peaks = measured_peaks()
+    ncu = ncu_counters()
     conv_ms, conv_launches = stages["conv"]
     win_rank = args.steps * N_SLIDES * n_win
     conv_tflops = 2.0 * MMAC_CONV * win_rank / (conv_ms * 1e-3) / 1e12 if conv_ms > 0 else 0.0
@@ -566,22 +600,25 @@ def run_ours(args):
         "stages_pass": {"ms_per_step": ms_profiled / args.steps,
                         "note": "second pass over the same steps with the library's per-stage CUDA events on its stream"},
     }
-    ncu = ncu_counters()
     if "conv_dram_bytes_per_launch" in ncu:
         out["roofline"]["traffic"], out["roofline"]["traffic_source"] = ncu["conv_dram_bytes_per_launch"]
     wh_ms = stages["whiten"][0]
     if wh_ms > 0:
         n_out_block = n_raw - (PSD_LEN - STRIDE - FILTER // 2) - FILTER // 2
-        gbs = args.steps * 2 * n_out_block * (4 + 2) / (wh_ms * 1e-3) / 1e9      # fp32 in + bf16 out per sample
-        out["roofline_whiten"] = {"kernel": "whiten_os_kernel", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"],
-                                  "unit": "GB/s", "frac": gbs / peaks["hbm"], "traffic": None,
-                                  "algorithmic": "4 B in + 2 B (bf16) out per whitened sample per channel",
-                                  # the binding resource (profiles/r01d_whiten_full.md): instruction issue.
-                                  # ncu counts 137 thread instructions per whitened sample per channel (two 4096-point complex
-                                  # FFTs, untangle and spectral multiply per 6144 valid samples); peak = 148 SMs x 128 lanes x
-                                  # 1.965 GHz thread instructions per second
-                                  "alu": {"bound": "alu", "achieved": 137.0 * gbs / 6.0 / 1e3, "peak": 148 * 128 * 1.965e9 / 1e12,
-                                          "unit": "T thread-instructions/s", "frac": (137.0 * gbs / 6.0 / 1e3) / (148 * 128 * 1.965e9 / 1e12)}}
+        gbs = args.steps * 2 * n_out_block * (4 + 2) / (wh_ms * 1e-3) / 1e9      # fp32 in + fp16 out per sample
+        rw = {"kernel": "whiten_os64_kernel", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"],
+              "unit": "GB/s", "frac": gbs / peaks["hbm"], "traffic": None,
+              "algorithmic": "4 B in + 2 B (fp16) out per whitened sample per channel"}
+        if "whiten_dram_bytes_per_launch" in ncu:
+            rw["traffic"], rw["traffic_source"] = ncu["whiten_dram_bytes_per_launch"]
+        if "whiten_thread_instructions_per_sample" in ncu:
+            # what binds: instruction issue at two warps per scheduler.  Thread instructions per whitened
+            # sample from the ncu capture; peak = 148 SMs x 128 lanes x 1.965 GHz thread instructions per second
+            ipsa, src = ncu["whiten_thread_instructions_per_sample"]
+            ach = ipsa * gbs / 6.0 / 1e3
+            rw["alu"] = {"bound": "alu", "achieved": ach, "peak": 148 * 128 * 1.965e9 / 1e12, "unit": "T thread-instructions/s",
+                         "frac": ach / (148 * 128 * 1.965e9 / 1e12), "thread_instructions_per_sample": ipsa, "source": src}
+        out["roofline_whiten"] = rw
     st_ms = stages["stem"][0]
     if st_ms > 0:
         # shared stem: per 4096-window chunk the stem runs once over the chunk's stream (64 new conv positions per window)
@@ -600,11 +637,12 @@ def run_ours(args):
     we_ms = stages["welch"][0]
     if we_ms > 0:
         gbs = args.steps * 2 * n_raw * 4 / (we_ms * 1e-3) / 1e9                   # every raw sample enters the PSD once
-        out["roofline_welch"] = {"kernel": "welch_periodogram_kernel + psd_mean_kernel", "bound": "hbm", "achieved": gbs,
-                                 "peak": peaks["hbm"], "unit": "GB/s", "frac": gbs / peaks["hbm"], "traffic": None,
+        out["roofline_welch"] = {"kernel": "welch_pair_kernel + psd_group_sum_kernel + psd_mean_grouped_kernel", "bound": "hbm", "achieved": gbs,
+                                 "peak": peaks["hbm"], "unit": "GB/s", "frac": gbs / peaks["hbm"],
+                                 "traffic": ncu["welch_dram_bytes_per_launch"][0] if "welch_dram_bytes_per_launch" in ncu else None,
                                  "algorithmic": "4 B per raw sample per channel (each sample is in two 50 %-overlapped "
-                                                "segments; the second read is an L2 hit); DESIGN.md section 5 derives the fp32-ALU "
-                                                "bound that caps both FFT kernels below the HBM roofline"}
+                                                "segments, transformed as one complex pair); the stage also writes 4 B of "
+                                                "periodogram per sample and sums them per epoch"}
     # NEXT-1: 1 s top-hat integration + 8 s clustering of the step's scores, on the device
     with torch.cuda.stream(stream):
         for _ in range(3):
@@ -623,6 +661,10 @@ def run_ours(args):
                           "frac": pp_bytes / (pp_ms * 1e-3) / 1e9 / peaks["hbm"],
                           "note": "2 launches over 2 MB of scores: launch-latency bound, 0.001 % of a step"}
     if world == 1 and not args.no_configs:
+        out.update(fft_rows(af, torch, stream, peaks))
+        for key, name in (("rfft_dram_bytes_per_launch", "roofline_rfft"), ("irfft_dram_bytes_per_launch", "roofline_irfft")):
+            if key in ncu and name in out:
+                out[name]["traffic"], out[name]["traffic_source"] = ncu[key]
         out["parity"] = parity_report(af, torch, stream, blob, args.parity_windows)
         out.update(config_rows(af, torch, stream, blob, peaks))
     if world == 1 and not args.no_next_rows:

@@ -110,6 +110,16 @@ aframe_status aframe_psd_welch(aframe_ctx* ctx, const float* d_strain, int64_t n
 aframe_status aframe_whiten(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
                             const float* d_psd, void* d_out, int64_t ld_out, aframe_precision out_dtype);
 
+/* ---- the batched real transform of the overlap-save block, on its own ------------------------------------------------
+ * BASELINE.json's north_star names "a batched power-of-two real FFT/iFFT" as a subsystem; inside aframe_whiten it is fused
+ * with the spectral multiply ("whitened in the frequency-domain, and transformed back to time-domain").  These two
+ * calls run exactly its two halves, one row per 8192-sample block, so the transform can be tested and profiled alone.
+ * d_x   : [batch][8192] fp32 real rows, contiguous, 8-byte aligned.
+ * d_spec: [batch][4097][2] fp32 (re, im), the one-sided spectrum X[k] = sum_n x[n] exp(-2 pi i n k / 8192), k = 0..4096.
+ * aframe_irfft8192 carries the 1/8192 (x = irfft(rfft(x))) and ignores Im X[0] and Im X[4096].  batch = 0 is a no-op. */
+aframe_status aframe_rfft8192(aframe_ctx* ctx, const float* d_x, int64_t batch, float* d_spec);
+aframe_status aframe_irfft8192(aframe_ctx* ctx, const float* d_spec, int64_t batch, float* d_x);
+
 /* Optional read-back of the taps designed by the last aframe_whiten call on this context:
  * d_taps [C][filter_len+1] fp32, h[j + L/2], j = -L/2..L/2 (used by the parity tests of O-2). */
 aframe_status aframe_filter_taps(aframe_ctx* ctx, float* d_taps);

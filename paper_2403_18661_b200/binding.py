@@ -44,6 +44,8 @@ EXPORTS = {
     "aframe_psd_welch": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]),
     "aframe_whiten": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_int64, C.c_int]),
     "aframe_filter_taps": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "aframe_rfft8192": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]),
+    "aframe_irfft8192": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]),
     "aframe_whiten_rolling": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_int64, C.c_int,
                                         C.POINTER(C.c_int64)]),
     "aframe_weights_load": (C.c_int, [C.c_void_p, C.c_char_p, C.c_size_t, C.POINTER(C.c_void_p)]),
@@ -183,6 +185,22 @@ class Context:
         self._check(self.lib.aframe_whiten(self.handle, _ptr(strain), n, strain.stride(0), _ptr(psd), _ptr(out),
                                            out.stride(0), prec))
         return out[:, :n_out]
+
+    def rfft8192(self, x, out=None):
+        """x [batch][8192] float32 CUDA -> one-sided spectrum [batch][4097][2] (re, im)."""
+        _need(x, torch.float32, "x")
+        if out is None:
+            out = torch.empty((x.shape[0], 4097, 2), dtype=torch.float32, device=x.device)
+        self._check(self.lib.aframe_rfft8192(self.handle, _ptr(x), x.shape[0], _ptr(out)))
+        return out
+
+    def irfft8192(self, spec, out=None):
+        """spec [batch][4097][2] float32 CUDA -> [batch][8192] real rows (1/8192 included)."""
+        _need(spec, torch.float32, "spec")
+        if out is None:
+            out = torch.empty((spec.shape[0], 8192), dtype=torch.float32, device=spec.device)
+        self._check(self.lib.aframe_irfft8192(self.handle, _ptr(spec), spec.shape[0], _ptr(out)))
+        return out
 
     def filter_taps(self):
         out = torch.empty((self.cfg.n_channels, self.cfg.filter_len + 1), dtype=torch.float32, device="cuda")

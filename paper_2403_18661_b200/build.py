@@ -14,6 +14,8 @@ SOURCES = ["aframe_api.cu", "signal_kernels.cu", "signal_fft64.cu", "net_fp32.cu
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
+# extra nvcc flags for one-off experiment builds (e.g. NVCC_EXTRA=-DAFRAME_TC_CYCLES); the product build sets none
+FLAGS += [f for f in os.environ.get("NVCC_EXTRA", "").split() if f]
 
 
 def _newer(src, dst):

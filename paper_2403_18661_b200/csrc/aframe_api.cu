@@ -130,7 +130,7 @@ AF_API void aframe_destroy(aframe_ctx* ctx) {
   af_tc_forget(ctx);
   cudaFree(ctx->d_tw32); cudaFree(ctx->d_tw64); cudaFree(ctx->d_taps_last);
   cudaFree(ctx->ws_psd.ptr); cudaFree(ctx->ws_filt.ptr); cudaFree(ctx->ws_act.ptr);
-  cudaFree(ctx->ws_white.ptr); cudaFree(ctx->ws_stage.ptr);
+  cudaFree(ctx->ws_white.ptr); cudaFree(ctx->ws_stage.ptr); cudaFree(ctx->ws_groups.ptr);
   for (ProfSpan& s : ctx->prof_spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
   for (cudaEvent_t e : ctx->prof_pool) cudaEventDestroy(e);
   for (int k = 0; k < AFRAME_PROF_KINDS; ++k) if (ctx->prof_open[k]) cudaEventDestroy(ctx->prof_open[k]);
@@ -250,7 +250,14 @@ AF_API aframe_status aframe_whiten_rolling(aframe_ctx* ctx, const float* d_strai
   float* H = reinterpret_cast<float*>(reinterpret_cast<char*>(ctx->ws_filt.ptr) + psd_bytes);
   st = af_launch_welch_periodograms(ctx, d_strain, ld, 0, seg_total, pg);
   if (st != AFRAME_OK) return st;
-  st = af_launch_psd_mean(ctx, pg, seg_total, seg_step, n_epochs, n_avg, psd);
+  if (cfg.welch_average == 0 && seg_step >= 2 && n_avg >= 2 * seg_step && n_epochs >= 8) {
+    // consecutive epochs share all but seg_step of their n_avg periodograms: sum them in groups of seg_step once
+    st = af_ws_reserve(ctx, ctx->ws_groups, sizeof(float) * (size_t)C * (seg_total / seg_step) * F);
+    if (st != AFRAME_OK) return st;
+    st = af_launch_psd_mean_grouped(ctx, pg, seg_total, seg_step, n_epochs, n_avg, reinterpret_cast<float*>(ctx->ws_groups.ptr), psd);
+  } else {
+    st = af_launch_psd_mean(ctx, pg, seg_total, seg_step, n_epochs, n_avg, psd);
+  }
   if (st != AFRAME_OK) return st;
   st = af_launch_filter_design(ctx, psd, n_epochs, H, nullptr);
   if (st != AFRAME_OK) return st;

@@ -100,6 +100,7 @@ struct aframe_ctx {
   void* encode_tiled = nullptr;   // cuTensorMapEncodeTiled entry point
   Workspace ws_white;          // whitened stream of aframe_score_timeslides
   Workspace ws_stage;          // device staging of the *_host entry points
+  Workspace ws_groups;         // group sums of periodograms (aframe_whiten_rolling)
   // optional per-stage device timing (aframe_profile): CUDA-event pairs on ctx->stream
   bool prof_on = false;
   std::vector<ProfSpan> prof_spans;
@@ -167,6 +168,12 @@ aframe_status af_launch_filter_design(aframe_ctx* ctx, const float* d_psd, int64
 aframe_status af_launch_whiten_os(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
                                   const float* d_H, int64_t in0, int64_t out_total, int64_t epoch_len, int64_t n_epochs,
                                   void* d_out, int64_t ld_out, int out_dt);
+
+// signal_fft64.cu: stored records with welch_nfft 4096 take two segments per transform; many epochs take group sums
+bool af_welch_pair_applicable(const aframe_ctx* ctx, int64_t n_seg);
+aframe_status af_launch_welch_pairs(aframe_ctx* ctx, const float* d_strain, int64_t ld, int64_t n_seg, float* d_pgram);
+aframe_status af_launch_psd_mean_grouped(aframe_ctx* ctx, const float* d_pgram, int64_t n_seg_total, int64_t seg_step,
+                                         int64_t n_epochs, int64_t n_avg, float* d_groups, float* d_psd);
 
 aframe_status af_forward_fp32(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_dt,
                               int64_t sB, int64_t sT, const int64_t* choff, int64_t B, float* d_scores);

@@ -29,6 +29,23 @@ static bool encode_map(aframe_ctx* ctx, CUtensorMap* m, const void* ptr, int ran
   return true;
 }
 
+#ifdef AFRAME_TC_CYCLES
+// Experiments build only (nvcc -DAFRAME_TC_CYCLES; never part of the product library): per-role cycle counters of CTA 0,
+// 32 slots per launch plan, handed out in build order and read back through aframe_experiment_tc_cycles.
+static long long* g_tc_cycles = nullptr;
+static int g_tc_cycles_next = 0;
+static long long* tc_cycles_slot() {
+  if (!g_tc_cycles) { cudaMalloc(&g_tc_cycles, sizeof(long long) * 32 * 256); cudaMemset(g_tc_cycles, 0, sizeof(long long) * 32 * 256); }
+  return g_tc_cycles + 32 * (g_tc_cycles_next++ % 256);
+}
+AF_API int aframe_experiment_tc_cycles(long long* host_out /* [256][32] */) {
+  if (!g_tc_cycles) return 0;
+  cudaDeviceSynchronize();
+  cudaMemcpy(host_out, g_tc_cycles, sizeof(long long) * 32 * 256, cudaMemcpyDeviceToHost);
+  return g_tc_cycles_next;
+}
+#endif
+
 struct TcLaunch {
   CUtensorMap tm_in, tm_w, tm_out, tm_res, tm_scw;
   TcConvParams p;
@@ -185,6 +202,9 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.head_slabs = l.t_out / 32;
   p.head_rows = (head && ov && ov->head_rows) ? 1 : 0; p.head_row_stride = l.t_out;
   p.nb = packed ? ov->e_nb : nb;
+#ifdef AFRAME_TC_CYCLES
+  p.dbg_out = tc_cycles_slot();
+#endif
   // shared-memory plan (227 KB per CTA): main-loop ring depth vs epilogue staging / residual prefetch buffers
   // (two epilogue groups: EG * nbuf staging buffers of 16 KB; a residual tile is prefetched pf chunks ahead into the
   //  buffer its chunk's output is staged in)
@@ -208,7 +228,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   L.cg2 = cg2;
   L.halo = halo;
   L.smem = halo ? (BN == 128 ? TcCfg<128>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks) : TcCfg<64>::smem_halo(p.stages, p.nbuf, l.k, p.kblocks)) + p.sc_kblocks * BN * 128
-         : cg2 ? TcCfg<256, true>::smem(p.stages, p.nbuf, head) : BN == 256 ? TcCfg<256>::smem(p.stages, p.nbuf, head) : (BN == 128 ? TcCfg<128>::smem(p.stages, p.nbuf, head)
+         : cg2 ? TcCfg<256, true>::smem(p.stages, p.nbuf, head) : (BN == 128 ? TcCfg<128>::smem(p.stages, p.nbuf, head)
                                                                             : TcCfg<64>::smem(p.stages, p.nbuf, head));
   if (cg2) L.grid = 2 * (p.num_tiles < ctx->n_sms / 2 ? p.num_tiles : ctx->n_sms / 2);
   else L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
@@ -246,10 +266,8 @@ template <int BN, bool HEAD, bool CG2, bool HALO = false> static cudaError_t lau
 // second != null: both problems in one launch (only the CTA-pair N = 256 storing variant is paired, see can_pair below)
 static cudaError_t launch_conv(const TcLaunch& L, cudaStream_t s, const TcLaunch* second = nullptr) {
   if (L.cg2) return L.head ? launch_bn<256, true, true>(L, s) : launch_bn<256, false, true>(L, s, second);
-  if (L.head) return launch_bn<256, true, false>(L, s);
   if (L.halo) return L.BN == 128 ? launch_bn<128, false, false, true>(L, s) : launch_bn<64, false, false, true>(L, s);
-  return L.BN == 256 ? launch_bn<256, false, false>(L, s)
-                     : (L.BN == 128 ? launch_bn<128, false, false>(L, s) : launch_bn<64, false, false>(L, s));
+  return L.BN == 128 ? launch_bn<128, false, false>(L, s) : launch_bn<64, false, false>(L, s);
 }
 
 // fused basic block (conv_block_kernel): layers a (conv) and b (conv + residual from a's input)
@@ -300,6 +318,9 @@ static bool build_block_launch(aframe_ctx* ctx, const aframe_weights* w, int ia,
   p.edge = row_shift > 0 ? edge : nullptr;
   p.zero_period = zero_period; p.zero_valid = zero_valid;
   p.reverse = 0;
+#ifdef AFRAME_TC_CYCLES
+  p.dbg_out = tc_cycles_slot();
+#endif
   L.smem = tcb_smem(p.nx, p.ny, p.no);
   L.device = ctx->device;
   L.grid = p.num_tiles < ctx->n_sms ? p.num_tiles : ctx->n_sms;
@@ -465,47 +486,11 @@ __global__ void s2_stitch_kernel(uint4* __restrict__ out, const uint4* __restric
   out[i] = v;
 }
 
-// Fused-head partials for a stage that ran in shared form: the same numbers, summed in the same order, as the HEAD variant
-// of conv_tc_kernel emits from its epilogue (one warp = one 32-row slab of one window x one 64-channel chunk; lane = row),
-// read from the stage's stream or edge batch; head_finish_kernel then sums them as usual.  Nothing is stitched.
-__global__ void __launch_bounds__(256)
-sh_head_partial_kernel(const uint4* __restrict__ S, const uint4* __restrict__ Y, const float* __restrict__ head_w,
-                       float* __restrict__ head_part, int64_t nb, int T, int C, int64_t row_shift, int c_head, int c_tail,
-                       int64_t e_stride, int64_t e_tail0, int e_trow) {
-  const int lane = threadIdx.x & 31;
-  const int chunks = C / 64, slabs = T / 32, pieces = C / 8;
-  const int64_t wi = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
-  if (wi >= nb * slabs * chunks) return;
-  const int c = (int)(wi % chunks);
-  const int slab = (int)((wi / chunks) % slabs);
-  const int64_t b = wi / ((int64_t)chunks * slabs);
-  const int t = slab * 32 + lane;
-  const uint4* rowp;
-  if (t < c_head) rowp = Y + (b * e_stride + t) * pieces;
-  else if (t >= T - c_tail) rowp = Y + (e_tail0 + b * e_stride + (t - e_trow)) * pieces;
-  else rowp = S + (b * row_shift + t) * pieces;
-  const float4* hw4 = reinterpret_cast<const float4*>(head_w + c * 64);
-  float hacc[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-  for (int jj = 0; jj < 8; ++jj) {
-    const uint4 o = rowp[c * 8 + jj];
-    const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
-    const float2 o0 = af_act_unpack2(o.x), o1 = af_act_unpack2(o.y), o2 = af_act_unpack2(o.z), o3 = af_act_unpack2(o.w);
-    hacc[0] = fmaf(o0.x, hA.x, hacc[0]); hacc[1] = fmaf(o0.y, hA.y, hacc[1]);
-    hacc[2] = fmaf(o1.x, hA.z, hacc[2]); hacc[3] = fmaf(o1.y, hA.w, hacc[3]);
-    hacc[0] = fmaf(o2.x, hB.x, hacc[0]); hacc[1] = fmaf(o2.y, hB.y, hacc[1]);
-    hacc[2] = fmaf(o3.x, hB.z, hacc[2]); hacc[3] = fmaf(o3.y, hB.w, hacc[3]);
-  }
-  float sum = 0.f;
-  sum += (hacc[0] + hacc[1]) + (hacc[2] + hacc[3]);
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-  if (lane == 0) head_part[(b * slabs + slab) * chunks + c] = sum;
-}
-
-// The same partial sums from per-row dot products (TcConvParams::head_rows: the stage's last conv stores no activation, its
-// epilogue emits each row's dot product with the head weights per 64-channel chunk, Rs over the stream and Re over the edge
-// batch): lane = row of the slab, the 32 values are summed in the order the fused head uses.
+// Fused-head partials for a stage that ran in shared form: the same numbers, summed in the same order, as the HEAD variant of
+// conv_tc_kernel emits from its epilogue.  The stage's last conv stores no activation (TcConvParams::head_rows): its epilogue
+// emits each row's dot product with the head weights per head unit (the channels one epilogue thread holds), Rs over the
+// stream and Re over the edge batch; here one warp = one 32-row slab of one window x one unit, lane = row of the slab, and
+// the 32 values are summed in the order the fused head uses.  head_finish_kernel then sums the partials as usual.
 __global__ void __launch_bounds__(256)
 sh_head_rows_kernel(const float* __restrict__ Rs, const float* __restrict__ Re, float* __restrict__ head_part, int64_t nb, int T,
                     int chunks, int64_t row_shift, int c_head, int c_tail, int64_t e_stride, int64_t e_tail0, int e_trow) {
@@ -638,7 +623,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     if (only_consumer && w->layers[src].c_out % 256 == 0 && w->layers[src].c_out <= 512 && tile_t_box(w->layers[src].t_out) % 32 == 0 &&
         !w->live_gn) {
       fuse = src;
-      n_part = (w->layers[src].t_out / 32) * (w->layers[src].c_out / 64);
+      n_part = (w->layers[src].t_out / 32) * (w->layers[src].c_out / 64) * TcCfg<256, true>::EPW;   // head units of EPI_COLS channels
     }
   }
   // live GroupNorm scratch after the slots: (mu, rstd) per (window, group), then the conv epilogues' partial sums
@@ -647,7 +632,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     for (int i = 2; i < n; ++i) {
       const LayerDesc& l = w->layers[i];
       if (l.kind != 0) continue;
-      const int u = l.c_out / w->n_groups < 64 ? l.c_out / w->n_groups : 64;
+      const int u = l.c_out / w->n_groups < 32 ? l.c_out / w->n_groups : 32;   // (an upper bound on the units: 32-column units on the CTA-pair path)
       const size_t e = (size_t)(l.t_out / 32) * (l.c_out / u);
       if (e > gn_part_elems) gn_part_elems = e;
     }
@@ -854,7 +839,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             // ([stream rows | edge-batch rows][C / 64] floats)
             const bool hr = sh_head_on && g + 1 == shs.size() && q + 1 == h.list.size();
             float* hr_s = reinterpret_cast<float*>(sh_buf((int)g, 0, (int)q));
-            float* hr_e = hr_s + rows_s * (h.C / 64);
+            float* hr_e = hr_s + rows_s * (h.C / TcCfg<256, true>::EPI_COLS);
             ov_s.head_rows = ov_e.head_rows = hr;
             ov_s.pair_plan = ov_e.pair_plan = true;
             if (hr) pc->sh_head_rows = true;
@@ -897,7 +882,8 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           // statistics from the epilogue's fp32 accumulators when a warp's 32 rows are one slab of one window and a group
           // is a whole number of 8..64-column units; else af_launch_gn_bf16 reads z back
           const int cg = l.c_out / w->n_groups;
-          const int u = cg < 64 ? cg : 64;
+          const int ec = pc->launches[i].cg2 ? TcCfg<256, true>::EPI_COLS : 64;   // accumulator columns per epilogue thread
+          const int u = cg < ec ? cg : ec;
           TcConvParams& pp = pc->launches[i].p;
           if (pp.T_box % 32 == 0 && (u == 8 || u == 16 || u == 32 || u == 64) && cg % u == 0) {
             pp.gn_part = reinterpret_cast<float2*>(reinterpret_cast<char*>(head_part) + gn_stats_bytes);
@@ -1033,21 +1019,13 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         }
         if (g + 1 == pc->sh.size() && pc->sh_head && pc->sh_head_rows) {
           const int q_last = (int)P.layers.size() - 1;
-          const int64_t n_warps = nb * (P.T / 32) * (P.C / 64);
+          const int hu = P.C / TcCfg<256, true>::EPI_COLS;          // head units per row
+          const int64_t n_warps = nb * (P.T / 32) * hu;
           const float* hr_s = reinterpret_cast<const float*>(sh_buf((int)g, 0, q_last));
           aux_begin();
           sh_head_rows_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(
-              hr_s, hr_s + sh_rows_stream((int)g) * (P.C / 64), head_part, nb, P.T, P.C / 64, P.shift, P.head, P.tail, P.e_stride,
+              hr_s, hr_s + sh_rows_stream((int)g) * hu, head_part, nb, P.T, hu, P.shift, P.head, P.tail, P.e_stride,
               P.e_tail0, P.e_trow);
-          AF_LAUNCH_CHECK(ctx);
-          aux_end();
-        } else if (g + 1 == pc->sh.size() && pc->sh_head) {
-          const int q_last = (int)P.layers.size() - 1;
-          const int64_t n_warps = nb * (P.T / 32) * (P.C / 64);
-          aux_begin();
-          sh_head_partial_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(
-              reinterpret_cast<const uint4*>(sh_buf((int)g, 0, q_last)), reinterpret_cast<const uint4*>(sh_buf((int)g, 1, q_last)),
-              w->d_head_w, head_part, nb, P.T, P.C, P.shift, P.head, P.tail, P.e_stride, P.e_tail0, P.e_trow);
           AF_LAUNCH_CHECK(ctx);
           aux_end();
         } else if (g + 1 == pc->sh.size()) {

@@ -13,7 +13,8 @@
 //   Epilogue: tcgen05.ld -> +bias (+residual, prefetched by TMA) -> fp16 -> ReLU -> swizzled smem -> TMA store,
 //   or (HEAD) the fused global-average-pool + linear head: per-(window, slab) partial dot products.
 //
-// Warp roles: warp 0 TMA producer, warp 1 MMA issuer (+TMEM alloc), then EG epilogue groups of 4 warps.
+// Warp roles: warp 0 TMA producer, warp 1 MMA issuer (+TMEM alloc), then EG epilogue groups of 4 warps (CTA pairs: 8 warps,
+// two per TMEM lane quadrant, each taking half of a chunk's columns).
 // With EG = 2 the groups take alternate tiles (group g <-> TMEM accumulator stage g), which doubles the
 // epilogue rate of the small-K layers whose epilogue, not the MMA, is the critical path.
 // Persistent: CTA i handles tiles i, i + grid, ...
@@ -116,7 +117,14 @@ template <int BN, bool CG2 = false> struct TcCfg {
   static constexpr bool SPLIT = (BN == 256);         // true: both groups drain every tile (alternate 64-column chunks);
                                                      // false: the groups take alternate tiles
   static constexpr int NACC = 512 / BN;              // TMEM accumulator stages (512 columns)
-  static constexpr int THREADS = 64 + 128 * EG;
+  // Warps per TMEM lane quadrant in an epilogue group.  CTA pairs (N = 256): two, each taking 32 of a chunk's 64 columns.
+  // Their epilogue was the critical path of the 256-channel stage (12 K blocks = 3.1 us of MMA per tile against four
+  // 64-column chunks drained by 8 warps that spent their time in latency, not issue: profiles/r02_conv_stage3.md); 16
+  // warps halve the time a chunk spends in the epilogue, and 32 accumulator columns per thread fit 576 threads' registers.
+  static constexpr int EPW = CG2 ? 2 : 1;
+  static constexpr int EPI_COLS = 64 / EPW;          // accumulator columns per epilogue thread and chunk
+  static constexpr int GROUP_THREADS = 128 * EPW;
+  static constexpr int THREADS = 64 + GROUP_THREADS * EG;
   static constexpr int smem(int stages, int nbuf, bool head) {
     return tc_fixed_bytes(head) + stages * STAGE_BYTES + EG * nbuf * TC_OUT_BYTES;
   }
@@ -128,21 +136,23 @@ template <int BN, bool CG2 = false> struct TcCfg {
 
 __device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 
-// One 64-channel chunk of one output row: + bias (+ residual read from the staging buffer) -> fp16 (RNE, saturating) ->
-// max(., lo) (lo = 0: ReLU, which commutes with the rounding; lo = -inf: none) -> staging buffer, or the fused head's dot product.
-template <bool RES, bool HEAD>
+// NP x 8 channels (pieces jj0 .. jj0 + NP - 1 of a 64-channel chunk) of one output row: + bias (+ residual read from the
+// staging buffer) -> fp16 (RNE, saturating) -> max(., lo) (lo = 0: ReLU, which commutes with the rounding; lo = -inf: none)
+// -> staging buffer, or the fused head's dot product.  v holds the NP * 8 accumulator columns.
+template <bool RES, bool HEAD, int NP>
 __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4* bias4, const float4* hw4,
-                                                 unsigned char* rowp, int row, __half2 lo2, float& head_acc,
+                                                 unsigned char* rowp, int row, int jj0, __half2 lo2, float& head_acc,
                                                  bool zero_row = false) {
   float hacc[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-  for (int jj = 0; jj < 8; ++jj) {                 // 8 pieces of 8 channels (16 B of fp16)
+  for (int j = 0; j < NP; ++j) {                   // pieces of 8 channels (16 B of fp16)
+    const int jj = jj0 + j;
     const float4 bA = bias4[2 * jj], bB = bias4[2 * jj + 1];
     float f[8];
-    f[0] = __uint_as_float(v[8 * jj + 0]) + bA.x; f[1] = __uint_as_float(v[8 * jj + 1]) + bA.y;
-    f[2] = __uint_as_float(v[8 * jj + 2]) + bA.z; f[3] = __uint_as_float(v[8 * jj + 3]) + bA.w;
-    f[4] = __uint_as_float(v[8 * jj + 4]) + bB.x; f[5] = __uint_as_float(v[8 * jj + 5]) + bB.y;
-    f[6] = __uint_as_float(v[8 * jj + 6]) + bB.z; f[7] = __uint_as_float(v[8 * jj + 7]) + bB.w;
+    f[0] = __uint_as_float(v[8 * j + 0]) + bA.x; f[1] = __uint_as_float(v[8 * j + 1]) + bA.y;
+    f[2] = __uint_as_float(v[8 * j + 2]) + bA.z; f[3] = __uint_as_float(v[8 * j + 3]) + bA.w;
+    f[4] = __uint_as_float(v[8 * j + 4]) + bB.x; f[5] = __uint_as_float(v[8 * j + 5]) + bB.y;
+    f[6] = __uint_as_float(v[8 * j + 6]) + bB.z; f[7] = __uint_as_float(v[8 * j + 7]) + bB.w;
     uint4* sp = reinterpret_cast<uint4*>(rowp + ((jj ^ (row & 7)) << 4));   // 128B-swizzle position
     if (RES) {
       const uint4 r = *sp;
@@ -177,12 +187,12 @@ __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4
   if (HEAD) head_acc += (hacc[0] + hacc[1]) + (hacc[2] + hacc[3]);
 }
 
-// Sum and sum of squares of the warp's 32 rows x U consecutive accumulator columns, for each of the 64 / U units of a
-// 64-column chunk; lane 0 stores them (fixed order everywhere: the statistics are reproducible bit for bit).
-template <int U>
+// Sum and sum of squares of the warp's 32 rows x U consecutive accumulator columns, for each of the NV / U units of the
+// thread's NV columns; lane 0 stores them (fixed order everywhere: the statistics are reproducible bit for bit).
+template <int U, int NV>
 __device__ __forceinline__ void tc_gn_partials(const uint32_t* v, float2* dst, int lane) {
 #pragma unroll
-  for (int k = 0; k < 64 / U; ++k) {
+  for (int k = 0; k < NV / U; ++k) {
     float s = 0.f, q = 0.f;
 #pragma unroll
     for (int j = 0; j < U; ++j) { const float x = __uint_as_float(v[k * U + j]); s += x; q = fmaf(x, x, q); }
@@ -241,7 +251,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     for (int a = 0; a < NACC; ++a) {               // tempty: one arrival per epilogue warp that drains the stage
       mbar_init(tfull_bar(a), 1);
-      mbar_init(tempty_bar(a), (SPLIT ? 8 : 4) * (CG2 ? 2 : 1));
+      mbar_init(tempty_bar(a), (SPLIT ? 8 : 4) * Cfg::EPW * (CG2 ? 2 : 1));
     }
     mbar_init(w_bar, 1);
     for (int g = 0; g < EG; ++g)
@@ -480,11 +490,13 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     }
   } else {
     // ===== epilogue: EG groups of 4 warps, thread <-> one output row =====
+    constexpr int EPW = Cfg::EPW, GT = Cfg::GROUP_THREADS, EC = Cfg::EPI_COLS;
     const int ew = warp - 2;
-    const int g = ew >> 2;                         // epilogue group: takes this CTA's tiles g, g + EG, ...
+    const int g = ew / (4 * EPW);                  // epilogue group: takes this CTA's tiles g, g + EG, ...
     const int q = warp & 3;                        // TMEM lane quadrant this warp may access
+    const int hf = (ew % (4 * EPW)) >> 2;          // which EC columns of a chunk this warp takes (EPW = 2: two warps per quadrant)
     const int row = q * 32 + lane;
-    const bool leader = ((ew & 3) == 0) && lane == 0;
+    const bool leader = ((ew % (4 * EPW)) == 0) && lane == 0;
     const int NBUF = p.nbuf > 0 ? p.nbuf : 1;      // (the fused head stages nothing)
     const uint32_t gbuf = out_base + (uint32_t)(g * NBUF) * TC_OUT_BYTES;
     constexpr int CH = BN / 64;
@@ -502,9 +514,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     if (second) {
       // the second problem's bias replaces the first one's once both groups are done with it; the leader's earlier stores
       // must have read their staging buffers before a residual tile is prefetched into one
-      named_bar_sync(3, 128 * EG);
-      for (int i = (int)threadIdx.x - 64; i < p.c_out; i += 128 * EG) s_bias[i] = p.bias[i];
-      named_bar_sync(3, 128 * EG);
+      named_bar_sync(3, GT * EG);
+      for (int i = (int)threadIdx.x - 64; i < p.c_out; i += GT * EG) s_bias[i] = p.bias[i];
+      named_bar_sync(3, GT * EG);
       if (leader) tma_store_wait_read_n(0);
     }
     // residual prefetch cursor (leader only): item pf_j of this group's (tile, chunk) sequence; the residual tile lands
@@ -576,12 +588,12 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           }
         }
         T(2);
-        named_bar_sync(1 + g, 128);
+        named_bar_sync(1 + g, GT);
         T(3);
-        uint32_t v[64];
-        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN + c * 64);
+        uint32_t v[EC];
+        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN + c * 64 + hf * EC);
         tmem_ld32(taddr, v);
-        tmem_ld32(taddr + 32, v + 32);
+        if (EC == 64) tmem_ld32(taddr + 32, v + 32);
         tmem_ld_wait();
         T(4);
         if (c + C_STEP >= CH) {                    // this group's part of the accumulator is drained: hand it back to the (leader's) MMA warp
@@ -596,13 +608,13 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           const int r0 = q * 32;
           const int64_t b = b0 + r0 / p.T_box;
           const int slab = (t0 + r0 % p.T_box) >> 5;
-          if (b < p.nb) {
-            float2* dst = p.gn_part + ((b * p.head_slabs + slab) * (int64_t)(p.c_out / p.gn_unit) + (n0 + c * 64) / p.gn_unit);
+          if (b < p.nb) {                          // (gn_unit <= EC: conv_tc.cu)
+            float2* dst = p.gn_part + ((b * p.head_slabs + slab) * (int64_t)(p.c_out / p.gn_unit) + (n0 + c * 64 + hf * EC) / p.gn_unit);
             switch (p.gn_unit) {
-              case 8: tc_gn_partials<8>(v, dst, lane); break;
-              case 16: tc_gn_partials<16>(v, dst, lane); break;
-              case 32: tc_gn_partials<32>(v, dst, lane); break;
-              default: tc_gn_partials<64>(v, dst, lane); break;
+              case 8: tc_gn_partials<8, EC>(v, dst, lane); break;
+              case 16: tc_gn_partials<16, EC>(v, dst, lane); break;
+              case 32: tc_gn_partials<32, EC>(v, dst, lane); break;
+              default: tc_gn_partials<EC, EC>(v, dst, lane); break;
             }
           }
         }
@@ -620,21 +632,24 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         const bool zero_row = p.zero_period > 0 && t_row >= p.zero_origin - 2 &&
                               ((t_row - p.zero_origin + p.zero_period) % p.zero_period) >= p.zero_valid;
         const uint4* copy_row = copy_tile != nullptr ? copy_tile + c * 8 : nullptr;
-        if (p.has_res) tc_epilogue_math<true, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row);
-        else tc_epilogue_math<false, HEAD>(v, bias4, hw4, rowp, row, lo2, head_acc, zero_row);
-        if (!HEAD && copy_row != nullptr) {        // the staged row is replaced by the stream's (8 independent loads, then 8 stores)
-          uint4 cr[8];
+        constexpr int NP = EC / 8;
+        if (p.has_res) tc_epilogue_math<true, HEAD, NP>(v, bias4, hw4, rowp, row, hf * NP, lo2, head_acc, zero_row);
+        else tc_epilogue_math<false, HEAD, NP>(v, bias4, hw4, rowp, row, hf * NP, lo2, head_acc, zero_row);
+        if (!HEAD && copy_row != nullptr) {        // the staged row is replaced by the stream's (independent loads, then the stores)
+          uint4 cr[NP];
 #pragma unroll
-          for (int jj = 0; jj < 8; ++jj) cr[jj] = __ldg(copy_row + jj);
+          for (int j = 0; j < NP; ++j) cr[j] = __ldg(copy_row + hf * NP + j);
 #pragma unroll
-          for (int jj = 0; jj < 8; ++jj) *reinterpret_cast<uint4*>(rowp + ((jj ^ (row & 7)) << 4)) = cr[jj];
+          for (int j = 0; j < NP; ++j) *reinterpret_cast<uint4*>(rowp + (((hf * NP + j) ^ (row & 7)) << 4)) = cr[j];
         }
         if (HEAD) {
           // the warp's 32 rows are one 32-row slab of one window (T_box % 32 == 0): reduce and emit a partial
           float s = head_acc;
           head_acc = 0.f;
+          // head units: EC channels (one per epilogue warp of a quadrant), c_out / EC of them per row
+          const int hu = (n_idx * CH + c) * EPW + hf, n_hu = (p.c_out >> 6) * EPW;
           if (p.head_rows) {
-            if (row < p.T_box * p.B_box) p.head_part[((long long)(b0 + row / p.T_box) * p.head_row_stride + t_row) * (p.c_out >> 6) + n_idx * CH + c] = s;
+            if (row < p.T_box * p.B_box) p.head_part[((long long)(b0 + row / p.T_box) * p.head_row_stride + t_row) * n_hu + hu] = s;
           } else {
 #pragma unroll
           for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
@@ -642,13 +657,13 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           const int64_t b = b0 + r0 / p.T_box;
           const int slab = (t0 + r0 % p.T_box) >> 5;
           if (lane == 0 && b < p.nb)
-            p.head_part[(b * p.head_slabs + slab) * (p.c_out >> 6) + n_idx * CH + c] = s;
+            p.head_part[(b * p.head_slabs + slab) * n_hu + hu] = s;
           }
-          named_bar_sync(1 + g, 128);              // residual buffer fully read before it is refilled
+          named_bar_sync(1 + g, GT);               // residual buffer fully read before it is refilled
         } else {
           T(6);
           fence_proxy_async_smem();                // generic-proxy writes -> visible to the TMA store
-          named_bar_sync(1 + g, 128);
+          named_bar_sync(1 + g, GT);
           if (leader) {
             tma_store_4d(&tm_out, sbuf, n0 + c * 64, 0, t0, b0);
             tma_store_commit();

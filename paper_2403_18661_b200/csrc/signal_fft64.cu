@@ -233,3 +233,281 @@ aframe_status af_launch_whiten_os(aframe_ctx* ctx, const float* d_strain, int64_
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
 }
+
+// --------------------------------------------------------------------------------------------------
+// Welch periodograms of a stored record, two segments per transform (welch_nfft = 4096 only).
+// Segments 2q and 2q + 1 (50 % overlap: they share 2048 samples) are mean-detrended, Hann-windowed and transformed
+// TOGETHER as z = a + i b; their spectra are A[k] = (Z[k] + conj Z[N-k]) / 2, B[k] = (Z[k] - conj Z[N-k]) / (2 i), and only the
+// squared magnitudes are needed: no untangling multiply.  Work item = (segment pair, channel).
+// --------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(W64_THREADS, 2)
+welch_pair_kernel(const float* __restrict__ strain, int64_t ld, int64_t n_seg, int64_t seg_stride_out, int C, int64_t n_items,
+                  float scale, float norm, const float2* __restrict__ tw, float* __restrict__ pgram) {
+  constexpr int N = 4096, HOP = 2048, F = N / 2 + 1;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float2* tab = reinterpret_cast<float2*>(smem_raw);
+  const int tid = threadIdx.x, g = tid >> 6, t = tid & 63, lane = tid & 31, wq = (tid >> 5) & 1;
+  float2* tile = tab + 4096 + g * F64_TILE;
+  __shared__ float2 red[2][2];
+  f64_fill_tab(tab, tw, tid, W64_THREADS);
+  __syncthreads();
+  const int bar = 1 + g;
+  const float2 wt = __ldg(tw + 2 * t);           // (cos, -sin)(2 pi t / 4096)
+  const int64_t n_pairs = (n_seg + 1) / 2;
+
+  for (int64_t item = (int64_t)blockIdx.x * 2 + g; item < n_items; item += (int64_t)gridDim.x * 2) {
+    const int c = (int)(item % C);
+    const int64_t q = item / C;
+    const bool has_b = 2 * q + 1 < n_seg;
+    const float* x = strain + (int64_t)c * ld + 2 * q * HOP;
+    // thread t holds samples 64 m + t of the 6144 the pair covers: a[n1] = X[n1], b[n1] = X[n1 + 32]
+    float xs[96];
+#pragma unroll
+    for (int m = 0; m < 64; ++m) xs[m] = __ldg(x + 64 * m + t) * scale;
+#pragma unroll
+    for (int m = 64; m < 96; ++m) xs[m] = has_b ? __ldg(x + 64 * m + t) * scale : 0.f;
+    // detrend = 'constant' (reading A1): each segment's own mean
+    float sa = 0.f, sm = 0.f, sb = 0.f;
+#pragma unroll
+    for (int m = 0; m < 32; ++m) { sa += xs[m]; sm += xs[m + 32]; sb += xs[m + 64]; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      sa += __shfl_xor_sync(0xffffffffu, sa, o); sm += __shfl_xor_sync(0xffffffffu, sm, o); sb += __shfl_xor_sync(0xffffffffu, sb, o);
+    }
+    if (lane == 0) red[g][wq] = make_float2(sa + sm, sm + sb);
+    f64_bar(bar);
+    const float mean_a = (red[g][0].x + red[g][1].x) * (1.0f / N), mean_b = (red[g][0].y + red[g][1].y) * (1.0f / N);
+    // periodic Hann w[n] = 0.5 - 0.5 cos(2 pi n / 4096), n = 64 n1 + t: cos(u + v) with u = 2 pi n1 / 64 a constant
+    float2 v[64];
+#pragma unroll
+    for (int n1 = 0; n1 < 64; ++n1) {
+      const float2 cs = w64_cs(n1);
+      const float w = fmaf(-0.5f * cs.x, wt.x, fmaf(-0.5f * cs.y, wt.y, 0.5f));   // wt.y = -sin
+      v[n1] = make_float2((xs[n1] - mean_a) * w, has_b ? (xs[n1 + 32] - mean_b) * w : 0.f);
+    }
+    fft64<-1>(v);
+    f64_twiddle_store<-1>(v, tile, tab, t);
+    f64_bar(bar);
+    f64_load_row(v, tile, t);
+    fft64<-1>(v);
+    mirror_publish(v, tile, t, bar);
+    float* oa = pgram + ((int64_t)c * seg_stride_out + 2 * q) * F;
+    float* ob = oa + F;
+#pragma unroll
+    for (int k2 = 0; k2 < 32; ++k2) {
+      const float2 zk = v[k2], zq = *mirror_slot(tile, t, k2);
+      const float ar = zk.x + zq.x, ai = zk.y - zq.y, br = zk.x - zq.x, bi = zk.y + zq.y;
+      const float nk = (k2 == 0 && t == 0) ? 0.25f * norm : 0.5f * norm;           // one-sided: doubled except k = 0, N/2
+      const int k = t + 64 * k2;
+      oa[k] = (ar * ar + ai * ai) * nk;
+      if (has_b) ob[k] = (br * br + bi * bi) * nk;
+    }
+    if (t == 0) {                                // k = N/2 is its own mirror: A = Re Z, B = Im Z
+      oa[N / 2] = v[32].x * v[32].x * norm;
+      if (has_b) ob[N / 2] = v[32].y * v[32].y * norm;
+    }
+    f64_bar(bar);                                // the tile and `red` are free for the next item
+  }
+  (void)n_pairs;
+}
+
+// G[c][j][k] = sum of the `step` consecutive periodograms j step .. j step + step - 1.  fp32: a sum of n_avg = 63 positive
+// terms taken as 7 group sums of 8 plus 7 single terms is good to a few 1e-7 relative, against the 1e-4 of rule T1.
+__global__ void psd_group_sum_kernel(const float* __restrict__ pgram, int64_t n_seg_total, int step, int64_t n_groups, int F,
+                                     float* __restrict__ G) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t j = blockIdx.y;
+  const int c = blockIdx.z;
+  if (k >= F) return;
+  const float* p = pgram + ((int64_t)c * n_seg_total + j * step) * F + k;
+  float acc = 0.f;
+#pragma unroll 8
+  for (int i = 0; i < step; ++i, p += F) acc += *p;
+  G[((int64_t)c * n_groups + j) * F + k] = acc;
+}
+// PSD of epoch e = mean of the n_avg periodograms from segment e step on = (n_avg / step whole groups + the rest) / n_avg
+__global__ void psd_mean_grouped_kernel(const float* __restrict__ pgram, const float* __restrict__ G, int64_t n_seg_total,
+                                        int64_t n_groups, int step, int n_avg, int F, int C, float inv_n, float* __restrict__ psd) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t e = blockIdx.y;
+  const int c = blockIdx.z;
+  if (k >= F) return;
+  const int n_full = n_avg / step, n_rest = n_avg - n_full * step;
+  const float* gp = G + ((int64_t)c * n_groups + e) * F + k;
+  const float* p = pgram + ((int64_t)c * n_seg_total + e * step + (int64_t)n_full * step) * F + k;
+  float a0 = 0.f, a1 = 0.f;
+#pragma unroll 8
+  for (int j = 0; j < n_full; ++j, gp += F) a0 += *gp;
+#pragma unroll 8
+  for (int i = 0; i < n_rest; ++i, p += F) a1 += *p;
+  psd[((int64_t)e * C + c) * F + k] = (a0 + a1) * inv_n;
+}
+
+static std::atomic<uint64_t> g_welch_pair_attr{0};
+
+// Periodograms of segments [0, n_seg) of a stored record (welch_nfft 4096): returns false if this path does not apply.
+bool af_welch_pair_applicable(const aframe_ctx* ctx, int64_t n_seg) {
+  return ctx->cfg.welch_nfft == 4096 && ctx->cfg.welch_hop == 2048 && n_seg >= 2;
+}
+aframe_status af_launch_welch_pairs(aframe_ctx* ctx, const float* d_strain, int64_t ld, int64_t n_seg, float* d_pgram) {
+  const aframe_config& cfg = ctx->cfg;
+  const int C = af_nch(ctx);
+  const float scale = ldexpf(1.0f, cfg.strain_scale_log2);
+  const float norm = (float)(1.0 / (cfg.fs * 0.375 * cfg.welch_nfft));   // 1 / (fs sum w^2), periodic Hann
+  const int64_t n_items = ((n_seg + 1) / 2) * C;
+  const int64_t want = (n_items + 1) / 2, cap = 2 * (int64_t)ctx->n_sms;
+  aframe_status st = w64_set_smem(ctx, welch_pair_kernel, g_welch_pair_attr);
+  if (st != AFRAME_OK) return st;
+  af_prof_begin(ctx, AFRAME_PROF_WELCH);
+  welch_pair_kernel<<<(unsigned)(want < cap ? want : cap), W64_THREADS, W64_SMEM, ctx->stream>>>(
+      d_strain, ld, n_seg, n_seg, C, n_items, scale, norm, ctx->d_tw32, d_pgram);
+  af_prof_end(ctx, AFRAME_PROF_WELCH, 1);
+  AF_LAUNCH_CHECK(ctx);
+  return AFRAME_OK;
+}
+
+// Mean PSD per epoch through group sums (reads n_avg / step + n_avg % step values per bin and epoch instead of n_avg).
+// d_groups: scratch of C * n_groups * F floats, n_groups = n_seg_total / step.
+aframe_status af_launch_psd_mean_grouped(aframe_ctx* ctx, const float* d_pgram, int64_t n_seg_total, int64_t seg_step,
+                                         int64_t n_epochs, int64_t n_avg, float* d_groups, float* d_psd) {
+  const int F = ctx->cfg.welch_nfft / 2 + 1, C = af_nch(ctx);
+  const int64_t n_groups = n_seg_total / seg_step;
+  af_prof_begin(ctx, AFRAME_PROF_WELCH);
+  psd_group_sum_kernel<<<dim3((F + 127) / 128, (unsigned)n_groups, (unsigned)C), 128, 0, ctx->stream>>>(
+      d_pgram, n_seg_total, (int)seg_step, n_groups, F, d_groups);
+  AF_LAUNCH_CHECK(ctx);
+  psd_mean_grouped_kernel<<<dim3((F + 127) / 128, (unsigned)n_epochs, (unsigned)C), 128, 0, ctx->stream>>>(
+      d_pgram, d_groups, n_seg_total, n_groups, (int)seg_step, (int)n_avg, F, C, (float)(1.0 / (double)n_avg), d_psd);
+  af_prof_end(ctx, AFRAME_PROF_WELCH, 2);
+  AF_LAUNCH_CHECK(ctx);
+  return AFRAME_OK;
+}
+
+// --------------------------------------------------------------------------------------------------
+// The plain batched real transform of 8192 samples and its inverse (aframe_rfft8192 / aframe_irfft8192): the two halves
+// of the whitening kernel without the spectral multiply, one work item per row.
+//   rfft : x[8192] real -> X[0..4096] complex, X[k] = sum_n x[n] exp(-2 pi i n k / 8192)
+//   irfft: X[0..4096] -> x[8192] real, with the 1/8192 (Im X[0], Im X[4096] are ignored)
+// --------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(W64_THREADS, 2)
+rfft8192_kernel(const float* __restrict__ x_in, int64_t n_items, const float2* __restrict__ tw, float2* __restrict__ spec) {
+  constexpr int M = W64_M;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float2* tab = reinterpret_cast<float2*>(smem_raw);
+  const int tid = threadIdx.x, g = tid >> 6, t = tid & 63;
+  float2* tile = tab + 4096 + g * F64_TILE;
+  f64_fill_tab(tab, tw, tid, W64_THREADS);
+  __syncthreads();
+  const int bar = 1 + g;
+  const float2 wt = __ldg(tw + t);               // W_8192^t
+  for (int64_t item = (int64_t)blockIdx.x * 2 + g; item < n_items; item += (int64_t)gridDim.x * 2) {
+    const float2* x2 = reinterpret_cast<const float2*>(x_in + item * AF_NOS);
+    float2* X = spec + item * (M + 1);
+    float2 v[64];
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+      if (pass == 0) {
+#pragma unroll
+        for (int b = 0; b < 8; ++b)
+#pragma unroll
+          for (int a = 0; a < 8; ++a) v[8 * a + b] = __ldg(x2 + 64 * (8 * a + b) + t);
+      } else {
+        f64_load_row(v, tile, t);
+      }
+      fft64<-1>(v);
+      if (pass == 0) { f64_twiddle_store<-1>(v, tile, tab, t); f64_bar(bar); }
+    }
+    mirror_publish(v, tile, t, bar);
+#pragma unroll
+    for (int k2 = 0; k2 < 32; ++k2) {
+      const int k = t + 64 * k2;
+      const float2 w = f64_cmul_cs<-1>(wt, w128_cs(k2));
+      const float2 zk = v[k2], zq = *mirror_slot(tile, t, k2);
+      const float2 ee = make_float2(zk.x + zq.x, zk.y - zq.y);          // 2 E
+      const float2 oo = make_float2(zk.y + zq.y, zq.x - zk.x);          // 2 O
+      const float2 wo = f64_cmul<false>(oo, w);
+      X[k] = make_float2(0.5f * (ee.x + wo.x), 0.5f * (ee.y + wo.y));              // X[k] = E + W^k O
+      X[M - k] = make_float2(0.5f * (ee.x - wo.x), -0.5f * (ee.y - wo.y));         // X[M - k] = conj(E - W^k O)
+    }
+    if (t == 0) X[M / 2] = make_float2(v[32].x, -v[32].y);                         // its own mirror: conj(Z[M/2])
+    f64_bar(bar);
+  }
+}
+
+__global__ void __launch_bounds__(W64_THREADS, 2)
+irfft8192_kernel(const float2* __restrict__ spec, int64_t n_items, const float2* __restrict__ tw, float* __restrict__ x_out) {
+  constexpr int M = W64_M;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float2* tab = reinterpret_cast<float2*>(smem_raw);
+  const int tid = threadIdx.x, g = tid >> 6, t = tid & 63;
+  float2* tile = tab + 4096 + g * F64_TILE;
+  f64_fill_tab(tab, tw, tid, W64_THREADS);
+  __syncthreads();
+  const int bar = 1 + g;
+  const float2 wt = __ldg(tw + t);
+  const float sc = 0.5f / M;                     // the pair's half and the 1/M of the inverse
+  for (int64_t item = (int64_t)blockIdx.x * 2 + g; item < n_items; item += (int64_t)gridDim.x * 2) {
+    const float2* X = spec + item * (M + 1);
+    float2 v[64];
+    // pack: Z'[k] = X_E[k] + i X_O[k], kept conjugated for the forward code (IFFT(y) = conj(FFT(conj(y))))
+#pragma unroll
+    for (int k2 = 0; k2 < 32; ++k2) {
+      const int k = t + 64 * k2;
+      const float2 w = f64_cmul_cs<-1>(wt, w128_cs(k2));
+      float2 yk = __ldg(X + k), ym = __ldg(X + M - k);
+      if (k == 0) { yk.y = 0.f; ym.y = 0.f; }
+      ym.y = -ym.y;                              // conj(X[M - k])
+      const float2 ep = make_float2(sc * (yk.x + ym.x), sc * (yk.y + ym.y));
+      const float2 op = f64_cmul<true>(make_float2(sc * (yk.x - ym.x), sc * (yk.y - ym.y)), w);
+      v[k2] = make_float2(ep.x - op.y, -(ep.y + op.x));
+      *mirror_slot(tile, t, k2) = make_float2(ep.x + op.y, ep.y - op.x);
+    }
+    if (t == 0) { const float2 xm = __ldg(X + M / 2); tile[32] = make_float2(xm.x * (1.0f / M), xm.y * (1.0f / M)); }
+    f64_bar(bar);
+#pragma unroll
+    for (int k2 = 32; k2 < 64; ++k2) v[k2] = tile[t * F64_ROW + k2];
+    f64_bar(bar);
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+      if (pass == 1) f64_load_row(v, tile, t);
+      fft64<-1>(v);
+      if (pass == 0) { f64_twiddle_store<-1>(v, tile, tab, t); f64_bar(bar); }
+    }
+    float2* o = reinterpret_cast<float2*>(x_out + item * AF_NOS);
+#pragma unroll
+    for (int n1 = 0; n1 < 64; ++n1) o[64 * n1 + t] = make_float2(v[n1].x, -v[n1].y);
+    f64_bar(bar);
+  }
+}
+
+static std::atomic<uint64_t> g_rfft_attr{0}, g_irfft_attr{0};
+
+AF_API aframe_status aframe_rfft8192(aframe_ctx* ctx, const float* d_x, int64_t batch, float* d_spec) {
+  if (!ctx) return AFRAME_EINVAL;
+  if (!d_x || !d_spec) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
+  if (batch < 0) return af_fail(ctx, AFRAME_EINVAL, "negative batch");
+  if (batch == 0) return AFRAME_OK;
+  if ((reinterpret_cast<uintptr_t>(d_x) | reinterpret_cast<uintptr_t>(d_spec)) & 7) return af_fail(ctx, AFRAME_EINVAL, "rfft8192: pointers must be 8-byte aligned");
+  aframe_status st = w64_set_smem(ctx, rfft8192_kernel, g_rfft_attr);
+  if (st != AFRAME_OK) return st;
+  const int64_t want = (batch + 1) / 2, cap = 2 * (int64_t)ctx->n_sms;
+  rfft8192_kernel<<<(unsigned)(want < cap ? want : cap), W64_THREADS, W64_SMEM, ctx->stream>>>(d_x, batch, ctx->d_tw32,
+                                                                                             reinterpret_cast<float2*>(d_spec));
+  AF_LAUNCH_CHECK(ctx);
+  return AFRAME_OK;
+}
+
+AF_API aframe_status aframe_irfft8192(aframe_ctx* ctx, const float* d_spec, int64_t batch, float* d_x) {
+  if (!ctx) return AFRAME_EINVAL;
+  if (!d_x || !d_spec) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
+  if (batch < 0) return af_fail(ctx, AFRAME_EINVAL, "negative batch");
+  if (batch == 0) return AFRAME_OK;
+  if ((reinterpret_cast<uintptr_t>(d_x) | reinterpret_cast<uintptr_t>(d_spec)) & 7) return af_fail(ctx, AFRAME_EINVAL, "irfft8192: pointers must be 8-byte aligned");
+  aframe_status st = w64_set_smem(ctx, irfft8192_kernel, g_irfft_attr);
+  if (st != AFRAME_OK) return st;
+  const int64_t want = (batch + 1) / 2, cap = 2 * (int64_t)ctx->n_sms;
+  irfft8192_kernel<<<(unsigned)(want < cap ? want : cap), W64_THREADS, W64_SMEM, ctx->stream>>>(reinterpret_cast<const float2*>(d_spec),
+                                                                                              batch, ctx->d_tw32, d_x);
+  AF_LAUNCH_CHECK(ctx);
+  return AFRAME_OK;
+}

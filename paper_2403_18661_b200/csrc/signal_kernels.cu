@@ -184,6 +184,7 @@ filter_design_kernel(const float* __restrict__ psd, int F_w, int C, double fs, d
 aframe_status af_launch_welch_periodograms(aframe_ctx* ctx, const float* d_strain, int64_t ld, int64_t first_seg,
                                            int64_t n_seg, float* d_pgram, const StreamGate* gate_in) {
   if (n_seg <= 0) return AFRAME_OK;
+  if (!gate_in && first_seg == 0 && af_welch_pair_applicable(ctx, n_seg)) return af_launch_welch_pairs(ctx, d_strain, ld, n_seg, d_pgram);
   StreamGate gate = gate_in ? *gate_in : StreamGate();
   if (gate_in) { first_seg = 0; }
   const aframe_config& cfg = ctx->cfg;

@@ -123,3 +123,31 @@ def test_rolling_whitening_shorter_than_warmup_writes_nothing(af):
     x = coloured_noise(100000, seed=3)
     ctx = af.Context(precision=af.FP32)
     assert ctx.whiten_rolling(torch.from_numpy(x).cuda()).shape == (2, 0)
+
+
+@pytest.mark.parametrize("batch", [1, 2, 7, 600])
+def test_batched_rfft_and_irfft_of_the_overlap_save_block(af, batch):
+    """aframe_rfft8192 / aframe_irfft8192 (the two halves of the whitening kernel without the spectral multiply) against
+    the oracle's radix-2 FFT (itself pinned to the naive DFT): one-sided spectrum incl. DC, Nyquist and the self-mirrored
+    bin 2048; the inverse on a spectrum with non-zero imaginary parts at DC / Nyquist (ignored); round trip."""
+    from oracle import fft as offt
+    rng = np.random.default_rng(batch)
+    x = rng.standard_normal((batch, 8192)).astype(np.float32)
+    x[0, :] += 3.0                                               # a DC term
+    ctx = af.Context(precision=af.FP32)
+    xd = torch.from_numpy(x).cuda()
+    spec = ctx.rfft8192(xd)
+    got = spec.cpu().numpy().astype(np.float64)
+    got = got[..., 0] + 1j * got[..., 1]
+    rows = list(range(min(batch, 3))) + ([batch - 1] if batch > 3 else [])
+    ref = offt.rfft(x[rows].astype(np.float64))
+    scale = np.sqrt(np.mean(np.abs(ref) ** 2))
+    assert np.abs(got[rows] - ref).max() <= 2e-6 * scale         # fp32 transform of 8192 points
+    back = ctx.irfft8192(spec).cpu().numpy()
+    assert np.abs(back - x).max() <= 2e-6 * np.abs(x).max()
+    s = (rng.standard_normal((len(rows), 4097)) + 1j * rng.standard_normal((len(rows), 4097)))
+    sd = torch.from_numpy(np.stack([s.real, s.imag], axis=-1).astype(np.float32)).cuda().contiguous()
+    y = ctx.irfft8192(sd).cpu().numpy().astype(np.float64)
+    s32 = sd.cpu().numpy().astype(np.float64)
+    yref = offt.irfft(s32[..., 0] + 1j * s32[..., 1], 8192)
+    assert np.abs(y - yref).max() <= 2e-6 * np.sqrt(np.mean(yref ** 2)) * 10
