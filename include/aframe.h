@@ -183,8 +183,12 @@ aframe_status aframe_forward_strided(aframe_ctx* ctx, const aframe_weights* w, c
  * The state (raw ring, cached periodograms, PSD, filter, whitened ring, activations) is an opaque
  * device-resident object owned by the library.  aframe_stream_create returns AFRAME_ESHAPE unless cfg.stride divides
  * cfg.welch_hop (one Welch segment completes exactly on an update) and psd_len >= stride + filter_len.
- * Lifetime: a weights object must outlive every stream state created from it, and a context must outlive its weights
- * and stream states: destroy in the order states, weights, context. */
+ * Lifetime: the natural order is states, weights, context.  Other orders are safe: aframe_destroy releases the device
+ * resources of the weights and stream states that are still alive and leaves them as dead shells, and aframe_weights_free
+ * does the same to the stream states built on those weights; a dead shell only accepts its own free / destroy call
+ * (aframe_stream_step on one returns AFRAME_ESTATE, a forward with dead weights AFRAME_ESTATE).
+ * aframe_stream_step replays one captured CUDA graph per (d_new_samples, d_scores, d_n_scores) triple and keeps the four
+ * most recently used: a caller should cycle through at most four sets of buffers. */
 aframe_status aframe_stream_create(aframe_ctx* ctx, const aframe_weights* w, aframe_stream_state** out);
 aframe_status aframe_stream_reset(aframe_stream_state* st);
 void          aframe_stream_destroy(aframe_stream_state* st);
@@ -230,6 +234,28 @@ aframe_status aframe_score_timeslides_host(aframe_ctx* ctx, const aframe_weights
 aframe_status aframe_postprocess(aframe_ctx* ctx, const float* d_scores, int64_t n_series, int64_t n, int64_t ld,
                                  int32_t n_int, int32_t n_cluster, float* d_integrated, float* d_trig_value,
                                  int64_t* d_trig_index, int64_t* h_n_trig);
+
+/* ---- how overlapping windows are planned (diagnostic; host arithmetic only, needs no device and no context) ------------
+ * Windows taken in place at a spacing of window_spacing samples share every activation row that is out of reach of their own
+ * zero padding: the tensor-core path runs each stage once over the stream of a launch sequence plus, per
+ * window, the rows within reach of the padding.  This call reports that plan for a weight blob (version 1, as for
+ * aframe_weights_load): *first_stage_blocks = basic blocks of the 64-channel stage run in shared form (0: none), then one
+ * record per later stage in shared form.  In a packed stage, launched layer q computes per window one box of tbox[q] rows at
+ * each end (its e_head[q] / e_tail[q] edge rows plus the two rows the epilogue copies from the stream), floor(128 / tbox[q])
+ * boxes per 128-row MMA tile, in slots of P rows; the last box of a half may overhang into the spare_slots slots that follow.
+ * AFRAME_EINVAL / AFRAME_ESHAPE for bad arguments or a bad table. */
+typedef struct {
+  int32_t first_layer, n_layers;   /* table index of the stage's entry conv; layers that launch (<= 16 are described) */
+  int32_t T, C;                    /* rows per window and channels of the stage's output                             */
+  int32_t head, tail;              /* rows at a window's start / end within reach of its zero padding, stage output  */
+  int32_t packed;                  /* 1: packed edge batch (CTA-pair kernels); 0: fixed-length short windows         */
+  int32_t P;                       /* packed: rows per slot; else data rows of a short window                        */
+  int32_t spare_slots;             /* packed: slots after each half                                                   */
+  int32_t e_head[16], e_tail[16], tbox[16];
+} aframe_stage_plan;
+aframe_status aframe_describe_shared_plan(const void* host_blob, size_t bytes, int32_t kernel_len, int32_t n_channels,
+                                          int32_t window_spacing, int64_t n_windows, int32_t* first_stage_blocks,
+                                          aframe_stage_plan* stages, int32_t max_stages, int32_t* n_stages);
 
 /* How many updates of this state were served by replaying the captured CUDA graph (0 for a context bound to the legacy
  * default stream, which cannot be captured, or while aframe_profile is on). */

@@ -36,6 +36,12 @@ class aframe_config(C.Structure):
                 ("welch_average", C.c_int32), ("reserved_", C.c_int32)]
 
 
+class aframe_stage_plan(C.Structure):
+    _fields_ = [("first_layer", C.c_int32), ("n_layers", C.c_int32), ("T", C.c_int32), ("C", C.c_int32), ("head", C.c_int32),
+                ("tail", C.c_int32), ("packed", C.c_int32), ("P", C.c_int32), ("spare_slots", C.c_int32),
+                ("e_head", C.c_int32 * 16), ("e_tail", C.c_int32 * 16), ("tbox", C.c_int32 * 16)]
+
+
 EXPORTS = {
     "aframe_config_default": (C.c_int, [C.POINTER(aframe_config)]),
     "aframe_create": (C.c_int, [C.POINTER(aframe_config), C.c_void_p, C.POINTER(C.c_void_p)]),
@@ -64,6 +70,8 @@ EXPORTS = {
     "aframe_postprocess": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_int32, C.c_int32,
                                      C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]),
     "aframe_stream_graph_replays": (C.c_int64, [C.c_void_p]),
+    "aframe_describe_shared_plan": (C.c_int, [C.c_char_p, C.c_size_t, C.c_int32, C.c_int32, C.c_int32, C.c_int64, C.POINTER(C.c_int32),
+                                              C.POINTER(aframe_stage_plan), C.c_int32, C.POINTER(C.c_int32)]),
     "aframe_score_timeslides": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_int64,
                                           C.POINTER(C.c_int64), C.c_int32, C.c_int64, C.c_void_p]),
     "aframe_score_timeslides_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64,
@@ -90,6 +98,25 @@ def load_library():
             fn.restype, fn.argtypes = res, args
         _lib = lib
     return _lib
+
+
+def describe_shared_plan(blob: bytes, kernel_len=3072, n_channels=2, window_spacing=128, n_windows=4096):
+    """aframe_describe_shared_plan (host arithmetic only: works without a GPU).  Returns (first_stage_blocks, [stage dicts])."""
+    lib = load_library()
+    s1 = C.c_int32(0)
+    n = C.c_int32(0)
+    arr = (aframe_stage_plan * 8)()
+    st = lib.aframe_describe_shared_plan(blob, len(blob), int(kernel_len), int(n_channels), int(window_spacing), int(n_windows),
+                                         C.byref(s1), arr, 8, C.byref(n))
+    if st != OK:
+        raise AframeError(st, "aframe_describe_shared_plan")
+    out = []
+    for i in range(n.value):
+        a = arr[i]
+        nl = min(a.n_layers, 16)
+        out.append(dict(first_layer=a.first_layer, n_layers=a.n_layers, T=a.T, C=a.C, head=a.head, tail=a.tail, packed=bool(a.packed),
+                        P=a.P, spare_slots=a.spare_slots, e_head=list(a.e_head[:nl]), e_tail=list(a.e_tail[:nl]), tbox=list(a.tbox[:nl])))
+    return s1.value, out
 
 
 def default_config(**overrides) -> aframe_config:

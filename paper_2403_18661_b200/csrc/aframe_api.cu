@@ -127,6 +127,11 @@ AF_API aframe_status aframe_create(const aframe_config* cfg, void* cuda_stream, 
 AF_API void aframe_destroy(aframe_ctx* ctx) {
   if (!ctx) return;
   cudaStreamSynchronize(ctx->stream);
+  // children that outlive their context are released here and left as dead shells (aframe.h, "Lifetime")
+  for (aframe_stream_state* st : ctx->live_streams) af_stream_release(st);
+  ctx->live_streams.clear();
+  for (aframe_weights* w : ctx->live_weights) { af_weights_release(w); w->ctx = nullptr; }
+  ctx->live_weights.clear();
   af_tc_forget(ctx);
   cudaFree(ctx->d_tw32); cudaFree(ctx->d_tw64); cudaFree(ctx->d_taps_last);
   cudaFree(ctx->ws_psd.ptr); cudaFree(ctx->ws_filt.ptr); cudaFree(ctx->ws_act.ptr);
@@ -269,35 +274,96 @@ AF_API aframe_status aframe_whiten_rolling(aframe_ctx* ctx, const float* d_strai
 }
 
 // ---- weights --------------------------------------------------------------------------------------
+void af_weights_release(aframe_weights* w) {
+  for (float*& p : w->d_w32) { cudaFree(p); p = nullptr; }
+  for (af_act_t*& p : w->d_w16) { cudaFree(p); p = nullptr; }
+  for (float*& p : w->d_bias) { cudaFree(p); p = nullptr; }
+  for (float*& p : w->d_bias_sc) { cudaFree(p); p = nullptr; }
+  for (float*& p : w->d_gamma) { cudaFree(p); p = nullptr; }
+  for (float*& p : w->d_beta) { cudaFree(p); p = nullptr; }
+  cudaFree(w->d_head_w); w->d_head_w = nullptr;
+  cudaGetLastError();
+}
+
 AF_API void aframe_weights_free(aframe_weights* w) {
   if (!w) return;
-  if (w->ctx) { cudaStreamSynchronize(w->ctx->stream); af_tc_forget(w->ctx); }
-  for (float* p : w->d_w32) cudaFree(p);
-  for (af_act_t* p : w->d_w16) cudaFree(p);
-  for (float* p : w->d_bias) cudaFree(p);
-  for (float* p : w->d_bias_sc) cudaFree(p);
-  for (float* p : w->d_gamma) cudaFree(p);
-  for (float* p : w->d_beta) cudaFree(p);
-  cudaFree(w->d_head_w);
-  cudaGetLastError();
+  if (aframe_ctx* ctx = w->ctx) {                     // (a dead shell, released by aframe_destroy, has no context)
+    cudaStreamSynchronize(ctx->stream);
+    af_tc_forget(ctx);
+    // stream states built on these weights can no longer step: released, and aframe_stream_step answers AFRAME_ESTATE
+    for (aframe_stream_state* st : ctx->live_streams)
+      if (af_stream_weights(st) == w) af_stream_release(st);
+    for (size_t i = 0; i < ctx->live_weights.size(); ++i)
+      if (ctx->live_weights[i] == w) { ctx->live_weights.erase(ctx->live_weights.begin() + i); break; }
+    af_weights_release(w);
+  }
   delete w;
+}
+
+// Header and layer table of a version-1 blob (synthdata/weights.py): validation and shape inference on the host, no CUDA call.
+// hdr receives the eight header words; *why a static description of the first problem found.
+aframe_status af_parse_layer_table(const void* host_blob, size_t bytes, int kernel_len, int n_channels,
+                                   std::vector<LayerDesc>& layers, uint32_t hdr[8], const char** why) {
+  static const char* ok = "";
+  *why = ok;
+  if (bytes < 32) { *why = "weight blob shorter than its header"; return AFRAME_ESHAPE; }
+  memcpy(hdr, host_blob, 32);
+  if (hdr[0] != 0x57524641u || hdr[1] != 1u) { *why = "bad weight blob magic/version"; return AFRAME_EINVAL; }
+  const uint32_t n_layers = hdr[2], norm_kind = hdr[3], n_groups = hdr[4], in_ch = hdr[6];
+  if (n_layers == 0 || n_layers > 4096 || norm_kind > 2) { *why = "bad weight blob header"; return AFRAME_EINVAL; }
+  if (norm_kind >= 1 && n_groups == 0) { *why = "group norm with zero groups"; return AFRAME_EINVAL; }
+  if ((int)in_ch != n_channels) { *why = "blob in_channels != cfg.n_channels"; return AFRAME_ESHAPE; }
+  if (bytes < 32 + (size_t)n_layers * 48) { *why = "weight blob shorter than its layer table"; return AFRAME_ESHAPE; }
+  const int32_t* tab = reinterpret_cast<const int32_t*>(reinterpret_cast<const char*>(host_blob) + 32);
+  layers.assign(n_layers, LayerDesc());
+  int head_layer = -1;
+  for (uint32_t i = 0; i < n_layers; ++i) {
+    const int32_t* r = tab + (size_t)i * 12;
+    LayerDesc& l = layers[i];
+    l.kind = r[0]; l.c_in = r[1]; l.c_out = r[2]; l.k = r[3]; l.stride = r[4]; l.pad = r[5]; l.relu = r[6];
+    l.input_from = r[7]; l.residual_from = r[8];
+    if (l.kind < 0 || l.kind > 2 || l.c_in < 1 || l.c_out < 1 || l.k < 1 || l.stride < 1 || l.pad < 0) { *why = "layer table: bad field"; return AFRAME_ESHAPE; }
+    if (l.input_from >= (int)i || l.residual_from >= (int)i || l.input_from < -1 || l.residual_from < -1) { *why = "layer table: forward reference"; return AFRAME_ESHAPE; }
+    const int c_src = l.input_from < 0 ? (int)in_ch : layers[l.input_from].c_out;
+    const int t_src = l.input_from < 0 ? kernel_len : layers[l.input_from].t_out;
+    if (l.input_from >= 0 && layers[l.input_from].kind == 2) { *why = "layer table: input from a head"; return AFRAME_ESHAPE; }
+    if (c_src != l.c_in) { *why = "layer table: c_in does not match its input"; return AFRAME_ESHAPE; }
+    l.t_in = t_src;
+    if (l.kind == 2) {
+      l.t_out = 1;
+      if (l.c_out != 1) { *why = "head must have one output"; return AFRAME_ESHAPE; }
+      if (head_layer >= 0 || i != n_layers - 1) { *why = "exactly one head, as the last layer"; return AFRAME_ESHAPE; }
+      head_layer = (int)i;
+      continue;
+    }
+    if (l.t_in + 2 * l.pad < l.k) { *why = "layer table: kernel longer than its padded input"; return AFRAME_ESHAPE; }
+    l.t_out = (l.t_in + 2 * l.pad - l.k) / l.stride + 1;
+    if (l.kind == 1) {
+      if (l.c_out != l.c_in || l.residual_from >= 0) { *why = "max-pool must keep the channel count"; return AFRAME_ESHAPE; }
+      continue;
+    }
+    if (l.residual_from >= 0) {
+      const LayerDesc& rs = layers[l.residual_from];
+      if (rs.kind == 2 || rs.c_out != l.c_out || rs.t_out != l.t_out) { *why = "layer table: residual shape mismatch"; return AFRAME_ESHAPE; }
+    }
+    if (norm_kind >= 1 && l.c_out % (int)n_groups) { *why = "c_out not divisible by n_groups"; return AFRAME_ESHAPE; }
+  }
+  if (head_layer < 0) { *why = "layer table has no head"; return AFRAME_ESHAPE; }
+  return AFRAME_OK;
 }
 
 AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob, size_t bytes, aframe_weights** out) {
   if (!ctx) return AFRAME_EINVAL;
   if (!host_blob || !out) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
   *out = nullptr;
-  if (bytes < 32) return af_fail(ctx, AFRAME_ESHAPE, "weight blob shorter than its header");
-  const uint32_t* hd = reinterpret_cast<const uint32_t*>(host_blob);
-  if (hd[0] != 0x57524641u || hd[1] != 1u) return af_fail(ctx, AFRAME_EINVAL, "bad weight blob magic/version");
+  uint32_t hd[8];
+  std::vector<LayerDesc> table;
+  const char* why = "";
+  const aframe_status pst = af_parse_layer_table(host_blob, bytes, ctx->cfg.kernel_len, ctx->cfg.n_channels, table, hd, &why);
+  if (pst != AFRAME_OK) return af_fail(ctx, pst, "%s", why);
   const uint32_t n_layers = hd[2], norm_kind = hd[3], n_groups = hd[4], in_ch = hd[6];
   float eps; memcpy(&eps, &hd[5], 4);
-  if (n_layers == 0 || n_layers > 4096 || norm_kind > 2) return af_fail(ctx, AFRAME_EINVAL, "bad weight blob header");
-  if (norm_kind >= 1 && n_groups == 0) return af_fail(ctx, AFRAME_EINVAL, "group norm with zero groups");
-  if ((int)in_ch != ctx->cfg.n_channels) return af_fail(ctx, AFRAME_ESHAPE, "blob in_channels != cfg.n_channels");
-  const size_t tab_off = 32, pay_off = 32 + (size_t)n_layers * 48;
-  if (bytes < pay_off) return af_fail(ctx, AFRAME_ESHAPE, "weight blob shorter than its layer table");
-  const int32_t* tab = reinterpret_cast<const int32_t*>(reinterpret_cast<const char*>(host_blob) + tab_off);
+  const size_t pay_off = 32 + (size_t)n_layers * 48;
   const float* pay = reinterpret_cast<const float*>(reinterpret_cast<const char*>(host_blob) + pay_off);
   const size_t n_pay = (bytes - pay_off) / 4;
 
@@ -306,7 +372,7 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
   w->ctx = ctx;
   w->in_channels = (int)in_ch;
   w->kernel_len = ctx->cfg.kernel_len;
-  w->layers.resize(n_layers);
+  w->layers = table;
   w->d_w32.assign(n_layers, nullptr);
   w->d_w16.assign(n_layers, nullptr);
   w->d_bias.assign(n_layers, nullptr);
@@ -321,21 +387,8 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
   size_t pos = 0;
   auto fail = [&](aframe_status s, const char* msg) { st = af_fail(ctx, s, msg); };
   for (uint32_t i = 0; i < n_layers && st == AFRAME_OK; ++i) {
-    const int32_t* r = tab + (size_t)i * 12;
-    LayerDesc& l = w->layers[i];
-    l.kind = r[0]; l.c_in = r[1]; l.c_out = r[2]; l.k = r[3]; l.stride = r[4]; l.pad = r[5]; l.relu = r[6];
-    l.input_from = r[7]; l.residual_from = r[8];
-    if (l.kind < 0 || l.kind > 2 || l.c_in < 1 || l.c_out < 1 || l.k < 1 || l.stride < 1 || l.pad < 0) { fail(AFRAME_ESHAPE, "layer table: bad field"); break; }
-    if (l.input_from >= (int)i || l.residual_from >= (int)i || l.input_from < -1 || l.residual_from < -1) { fail(AFRAME_ESHAPE, "layer table: forward reference"); break; }
-    const int c_src = l.input_from < 0 ? (int)in_ch : w->layers[l.input_from].c_out;
-    const int t_src = l.input_from < 0 ? ctx->cfg.kernel_len : w->layers[l.input_from].t_out;
-    if (l.input_from >= 0 && w->layers[l.input_from].kind == 2) { fail(AFRAME_ESHAPE, "layer table: input from a head"); break; }
-    if (c_src != l.c_in) { fail(AFRAME_ESHAPE, "layer table: c_in does not match its input"); break; }
-    l.t_in = t_src;
+    LayerDesc& l = w->layers[i];               // (validated, shapes inferred: af_parse_layer_table)
     if (l.kind == 2) {
-      l.t_out = 1;
-      if (l.c_out != 1) { fail(AFRAME_ESHAPE, "head must have one output"); break; }
-      if (w->head_layer >= 0 || i != n_layers - 1) { fail(AFRAME_ESHAPE, "exactly one head, as the last layer"); break; }
       if (pos + l.c_in + 1 > n_pay) { fail(AFRAME_ESHAPE, "weight blob payload too short"); break; }
       w->head_layer = (int)i;
       w->head_b = pay[pos + l.c_in];
@@ -344,18 +397,8 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
       pos += l.c_in + 1;
       continue;
     }
-    if (l.t_in + 2 * l.pad < l.k) { fail(AFRAME_ESHAPE, "layer table: kernel longer than its padded input"); break; }
-    l.t_out = (l.t_in + 2 * l.pad - l.k) / l.stride + 1;
-    if (l.kind == 1) {
-      if (l.c_out != l.c_in || l.residual_from >= 0) { fail(AFRAME_ESHAPE, "max-pool must keep the channel count"); break; }
-      continue;
-    }
-    if (l.residual_from >= 0) {
-      const LayerDesc& rs = w->layers[l.residual_from];
-      if (rs.kind == 2 || rs.c_out != l.c_out || rs.t_out != l.t_out) { fail(AFRAME_ESHAPE, "layer table: residual shape mismatch"); break; }
-    }
+    if (l.kind == 1) continue;
     const int n_stat = norm_kind == 0 ? l.c_out : (norm_kind == 1 ? (int)n_groups : 0);
-    if (norm_kind >= 1 && l.c_out % (int)n_groups) { fail(AFRAME_ESHAPE, "c_out not divisible by n_groups"); break; }
     const size_t nw = (size_t)l.c_out * l.c_in * l.k;
     if (pos + nw + 2 * (size_t)l.c_out + 2 * (size_t)n_stat > n_pay) { fail(AFRAME_ESHAPE, "weight blob payload too short"); break; }
     const float* W = pay + pos;
@@ -405,8 +448,9 @@ AF_API aframe_status aframe_weights_load(aframe_ctx* ctx, const void* host_blob,
   if (st == AFRAME_OK && w->head_layer < 0) st = af_fail(ctx, AFRAME_ESHAPE, "layer table has no head");
   if (st == AFRAME_OK && pos != n_pay) st = af_fail(ctx, AFRAME_ESHAPE, "weight blob payload size mismatch");
   if (st == AFRAME_OK && cudaDeviceSynchronize() != cudaSuccess) st = af_fail(ctx, AFRAME_ECUDA, "sync after weight upload failed");
-  if (st != AFRAME_OK) { cudaGetLastError(); aframe_weights_free(w); return st; }
+  if (st != AFRAME_OK) { cudaGetLastError(); af_weights_release(w); delete w; return st; }
   af_tc_check(ctx, w);
+  ctx->live_weights.push_back(w);
   *out = w;
   return AFRAME_OK;
 }

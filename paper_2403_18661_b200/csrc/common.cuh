@@ -109,7 +109,15 @@ struct aframe_ctx {
   float* layer_ms = nullptr;   // aframe_profile_layers: per-layer device time of the next forward (host array), else null
   void* tc_cache = nullptr;    // conv_tc.cu: cached tensor maps / launch plans of the bf16 path (af_tc_forget frees it)
   int n_ch_batch = 0;          // aframe_whiten_batch: rows (element x detector) the signal launchers treat as channels
+  // objects created from this context that are still alive: aframe_destroy releases their device resources and marks
+  // them dead (ctx = nullptr), after which aframe_weights_free / aframe_stream_destroy only delete the host shell
+  std::vector<aframe_weights*> live_weights;
+  std::vector<aframe_stream_state*> live_streams;
 };
+
+void af_weights_release(aframe_weights* w);             // device arrays of a weights object (aframe_api.cu)
+void af_stream_release(aframe_stream_state* st);        // device blob and captured graphs of a stream state (stream.cu)
+const aframe_weights* af_stream_weights(const aframe_stream_state* st);
 
 // rows the Welch / design / whitening launchers run over: the configured detectors, or a training batch's B*C rows
 static inline int af_nch(const aframe_ctx* ctx) { return ctx->n_ch_batch > 0 ? ctx->n_ch_batch : ctx->cfg.n_channels; }

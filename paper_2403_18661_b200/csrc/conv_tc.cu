@@ -1,5 +1,6 @@
 // Host side of the tensor-core network path (fp16 weights and activations, fp32 accumulation): TMA tensor maps, per-layer launches, forward driver.
 #include <map>
+#include <string.h>
 
 #include "conv_tc_kernel.cuh"
 #include "conv_block_kernel.cuh"
@@ -280,16 +281,26 @@ struct TcBlockLaunch {
 
 // Layer i is the first conv of a basic block the fused kernel can run: 64 -> 64 -> 64 channels, k3 s1 p1, ReLU after each,
 // the second conv adds the block input, and nothing else reads the intermediate tensor.
-static int fusable_block(const aframe_weights* w, int i) {
-  const int n = (int)w->layers.size();
+static int fusable_block(const std::vector<LayerDesc>& layers, int i) {
+  const int n = (int)layers.size();
   if (i < 2 || i + 1 >= n) return -1;
-  const LayerDesc& a = w->layers[i];
-  const LayerDesc& b = w->layers[i + 1];
+  const LayerDesc& a = layers[i];
+  const LayerDesc& b = layers[i + 1];
   auto conv3 = [](const LayerDesc& l) { return l.kind == 0 && l.k == 3 && l.stride == 1 && l.pad == 1 && l.relu && l.c_in == 64 && l.c_out == 64; };
   if (!conv3(a) || !conv3(b) || a.residual_from >= 0 || b.input_from != i || b.residual_from != a.input_from) return -1;
   for (int j = 0; j < n; ++j)
-    if (j != i + 1 && (w->layers[j].input_from == i || w->layers[j].residual_from == i)) return -1;
+    if (j != i + 1 && (layers[j].input_from == i || layers[j].residual_from == i)) return -1;
   return i + 1;
+}
+static int fusable_block(const aframe_weights* w, int i) { return fusable_block(w->layers, i); }
+
+// Layer i adds the output of a 1x1 projection conv of the same width (aframe_weights_load then keeps the sum of the two
+// folded biases in d_bias_sc[i], and the projection can run inside layer i as extra K blocks)
+static bool has_projection_residual(const std::vector<LayerDesc>& layers, int i) {
+  const LayerDesc& l = layers[i];
+  if (l.kind != 0 || l.residual_from < 0) return false;
+  const LayerDesc& r = layers[l.residual_from];
+  return r.kind == 0 && r.k == 1 && r.c_out == l.c_out;
 }
 
 // row_shift > 0: x is the stem of the whole stream (shared stem): window b starts row_shift rows after window b - 1, and
@@ -553,14 +564,14 @@ static int64_t tc_chunk_windows() { return 4096; }
 
 // Number of leading fused 64-channel blocks that form a chain on the pooled stem output (layers 2,3 | 4,5 | ...): the
 // blocks the shared first stage can take over.
-static int s1_chain_blocks(const aframe_weights* w) {
-  const int n = (int)w->layers.size();
+static int s1_chain_blocks(const std::vector<LayerDesc>& layers) {
+  const int n = (int)layers.size();
   int k = 0, prev = 1;
   for (int i = 2; i + 1 < n && k < 5; i += 2) {
-    if (fusable_block(w, i) != i + 1 || w->layers[i].input_from != prev || w->layers[i + 1].residual_from != prev) break;
+    if (fusable_block(layers, i) != i + 1 || layers[i].input_from != prev || layers[i + 1].residual_from != prev) break;
     bool other = false;                              // the block input must have no reader outside the block
     for (int j = 2; j < n; ++j)
-      if (j != i && j != i + 1 && (w->layers[j].input_from == prev || w->layers[j].residual_from == prev)) other = true;
+      if (j != i && j != i + 1 && (layers[j].input_from == prev || layers[j].residual_from == prev)) other = true;
     if (other) break;
     prev = i + 1;
     ++k;
@@ -571,25 +582,25 @@ static int s1_chain_blocks(const aframe_weights* w) {
 // Layers of the stage after the shared first stage, if it has the form the shared second stage handles: entry conv k3 s2
 // (i0), projection k1 s2 (i0 + 1, folded into i0 + 2), then stride-1 k3 convs in basic blocks, all with the same width.
 // Returns the layers that launch, in order (i0, i0 + 2, i0 + 3, ...); empty if the pattern does not match.
-static std::vector<int> s2_chain_layers(const aframe_weights* w, int i0) {
+static std::vector<int> s2_chain_layers(const std::vector<LayerDesc>& layers, int i0) {
   std::vector<int> out;
-  const int n = (int)w->layers.size();
+  const int n = (int)layers.size();
   if (i0 + 2 >= n - 1) return out;
   const int prev = i0 - 1;
-  const LayerDesc& e = w->layers[i0];
-  const LayerDesc& q = w->layers[i0 + 1];
-  const LayerDesc& f = w->layers[i0 + 2];
+  const LayerDesc& e = layers[i0];
+  const LayerDesc& q = layers[i0 + 1];
+  const LayerDesc& f = layers[i0 + 2];
   auto conv3 = [&](const LayerDesc& l, int stride) { return l.kind == 0 && l.k == 3 && l.stride == stride && l.pad == 1 && l.relu && l.c_out == e.c_out; };
   if (!conv3(e, 2) || e.input_from != prev || e.residual_from >= 0) return out;
   if (!(q.kind == 0 && q.k == 1 && q.stride == 2 && q.pad == 0 && !q.relu && q.input_from == prev && q.residual_from < 0 && q.c_out == e.c_out)) return out;
-  if (!conv3(f, 1) || f.input_from != i0 || f.residual_from != i0 + 1 || !w->d_bias_sc[i0 + 2]) return out;
+  if (!conv3(f, 1) || f.input_from != i0 || f.residual_from != i0 + 1 || !has_projection_residual(layers, i0 + 2)) return out;
   for (int j = 2; j < n; ++j)                     // the first stage's output feeds only the entry conv and the projection
-    if (j != i0 && j != i0 + 1 && (w->layers[j].input_from == prev || w->layers[j].residual_from == prev)) return out;
+    if (j != i0 && j != i0 + 1 && (layers[j].input_from == prev || layers[j].residual_from == prev)) return out;
   out.push_back(i0); out.push_back(i0 + 2);
   int blk_in = i0 + 2;
   for (int j = i0 + 3; j + 1 < n - 1; j += 2) {
-    const LayerDesc& a = w->layers[j];
-    const LayerDesc& b = w->layers[j + 1];
+    const LayerDesc& a = layers[j];
+    const LayerDesc& b = layers[j + 1];
     if (!conv3(a, 1) || !conv3(b, 1) || a.input_from != blk_in || a.residual_from >= 0 || b.input_from != j || b.residual_from != blk_in) break;
     out.push_back(j); out.push_back(j + 1);
     blk_in = j + 1;
@@ -598,10 +609,141 @@ static std::vector<int> s2_chain_layers(const aframe_weights* w, int i0) {
   const int last = out.back();
   for (int j = 2; j < n; ++j) {
     if (j >= i0 && j <= last) continue;
-    const int a = w->layers[j].input_from, r = w->layers[j].residual_from;
+    const int a = layers[j].input_from, r = layers[j].residual_from;
     if ((a >= i0 && a < last) || (r >= i0 && r < last)) { out.clear(); return out; }
   }
   return out;
+}
+
+
+// ---- the shared-stage plan: host arithmetic only (no CUDA call), so that it can be unit-tested without a device --------
+constexpr int TC_MAX_SHARED_STAGES = 3;
+struct SharedStage {
+  std::vector<int> list;            // layers that launch, entry conv first
+  int i0 = 0, T = 0, C = 0, C_in = 0, head = 0, tail = 0;
+  int rows = 0, period = 0;         // short window: data rows, data + 2 separator rows
+  int64_t shift = 0;                // rows between consecutive windows at this stage's resolution
+  int64_t rows_stream = 0, rows_edge = 0;
+  size_t stream_bytes = 0, edge_bytes = 0, x_bytes = 0, off = 0;
+  // packed edge batch (stages whose layers run on the CTA-pair path): P rows per short-window slot, per launched layer the
+  // edge rows of its output at the window's start / end and the rows its box computes
+  bool packed = false;
+  int P = 0;
+  std::vector<int> e_head, e_tail, tbox;
+};
+struct SharedPlan {
+  int fuse = -1;                    // conv whose epilogue runs the head (else -1)
+  int s1_k = 0;                     // fused 64-channel blocks on the pooled stem output
+  bool s1_on = false;               // ... that run in shared form
+  bool sh_head_on = false;          // the last shared stage ends in the fused head
+  std::vector<SharedStage> stages;  // the shared stages after the first
+};
+static int64_t tc_up128(int64_t v) { return (v + 127) / 128 * 128; }
+
+// layers: the table with t_in / t_out filled; sB: window spacing in samples; chunk: windows per launch sequence
+static SharedPlan tc_plan_shared(const std::vector<LayerDesc>& layers, bool live_gn, int64_t sB, int64_t chunk) {
+  SharedPlan pl;
+  const int n = (int)layers.size();
+  {
+    // fused head: the conv feeding the head (and nothing else) pools + dots in its epilogue and stores nothing
+    const LayerDesc& h = layers[n - 1];
+    const int src = h.input_from;
+    bool only_consumer = src >= 2 && layers[src].kind == 0;
+    for (int i = 0; only_consumer && i < n - 1; ++i)
+      if (layers[i].input_from == src || layers[i].residual_from == src) only_consumer = false;
+    if (only_consumer && layers[src].c_out % 256 == 0 && layers[src].c_out <= 512 && tile_t_box(layers[src].t_out) % 32 == 0 && !live_gn)
+      pl.fuse = src;
+  }
+  pl.s1_k = s1_chain_blocks(layers);
+  pl.s1_on = pl.s1_k > 0 && sB % 4 == 0 && sB < layers[0].t_in && chunk >= 2 && !live_gn && layers[1].t_out >= 2 * S1_ROWS;
+  if (!pl.s1_on) return pl;
+  std::vector<SharedStage>& shs = pl.stages;
+  int i0 = 2 + 2 * pl.s1_k, Tp = layers[1].t_out, hp = 2 * pl.s1_k + 2, tp = 2 * pl.s1_k + 1;
+  int64_t shift_p = sB / 4;
+  while ((int)shs.size() < TC_MAX_SHARED_STAGES && shift_p % 2 == 0 && !pl.sh_head_on) {
+    SharedStage g;
+    g.list = s2_chain_layers(layers, i0);
+    if (g.list.empty()) break;
+    if (pl.fuse >= i0 && pl.fuse <= g.list.back()) {
+      // the stage that ends in the fused head: its last conv emits per-row head dot products (sh_head_rows_kernel);
+      // needs whole 32-row slabs and the head as the only reader
+      if (pl.fuse != g.list.back() || layers[pl.fuse].t_out % 32 != 0) break;
+      pl.sh_head_on = true;
+    }
+    const int n2 = (int)g.list.size() - 1;
+    g.i0 = i0; g.T = layers[i0].t_out; g.C = layers[i0].c_out; g.C_in = layers[i0].c_in;
+    g.shift = shift_p / 2;
+    g.head = hp / 2 + 1 + n2;                                   // rows within reach of the window's zero padding ...
+    g.tail = g.T - (Tp - tp) / 2 + n2;                          // ... at the start and at the end of the stage's output
+    const int src_rows = shs.empty() ? S1_ROWS : shs.back().rows;
+    g.rows = g.head + n2 > g.tail + n2 + 1 ? g.head + n2 : g.tail + n2 + 1;
+    g.period = g.rows + 2;
+    // (head + tail <= T: a row taken from the window's first rows must be out of reach of the padding at its END, which the
+    //  short window at the start does not see, and vice versa; short windows at both ends of short windows would overlap)
+    const bool fits = g.T >= g.rows && Tp >= 2 * g.rows && Tp == 2 * g.T && hp <= src_rows - 2 && tp <= src_rows - 2 &&
+                      g.C % 64 == 0 && g.C_in % 64 == 0 && g.head + g.tail <= g.T;
+    if (!fits) { pl.sh_head_on = false; break; }
+    g.rows_stream = tc_up128((chunk - 1) * g.shift + g.T);
+    g.rows_edge = tc_up128(2 * chunk * g.period);
+    // Packed edge batch: layer q's output differs from the stream's only in its first e_head[q] / last e_tail[q] rows (one more
+    // per conv); its box holds those rows and the two rows next to them that the epilogue takes from the stream (the outer one
+    // is computed from a row outside the box): tbox[q] = max(e_head, e_tail) + 2 rows, floor(128 / tbox) slots per MMA tile.
+    // (The entry conv's rows are all computed from valid input rows and the last layer's interior rows are never read: no copies.)
+    if (g.C % 256 == 0) {
+      const int nl = (int)g.list.size();
+      g.e_head.resize(nl); g.e_tail.resize(nl); g.tbox.assign(nl, 0);
+      bool ok = true;
+      int Pmax = 0;
+      for (int q = 0; q < nl; ++q) {
+        g.e_head[q] = hp / 2 + 1 + q;
+        g.e_tail[q] = g.T - (Tp - tp) / 2 + q;
+        // edge rows + the two copied rows; the stage's last layer is read at its edge rows only (next stage's gather, stitch, head)
+        g.tbox[q] = (g.e_head[q] > g.e_tail[q] ? g.e_head[q] : g.e_tail[q]) + (q + 1 < nl ? 2 : 0);
+        if (g.tbox[q] > 32 || g.tbox[q] < 1 || 128 / g.tbox[q] > SH_SPARE_SLOTS) ok = false;   // (a half's last box overhangs by < 128 / tbox slots)
+        if (g.tbox[q] > Pmax) Pmax = g.tbox[q];
+      }
+      if (ok && g.T >= 2 * Pmax && g.e_head[nl - 1] == g.head && g.e_tail[nl - 1] == g.tail) {
+        g.packed = true; g.P = Pmax;
+        g.rows_edge = 2 * (chunk + SH_SPARE_SLOTS) * g.P;
+      }
+    }
+    if (!g.packed && !shs.empty() && shs.back().packed) { pl.sh_head_on = false; break; }   // (a packed stage feeds packed stages only)
+    shs.push_back(g);
+    i0 = g.list.back() + 1; Tp = g.T; hp = g.head; tp = g.tail; shift_p = g.shift;
+  }
+  return pl;
+}
+
+aframe_status af_parse_layer_table(const void* host_blob, size_t bytes, int kernel_len, int n_channels,
+                                   std::vector<LayerDesc>& layers, uint32_t hdr[8], const char** why);   // aframe_api.cu
+
+// Host-only description of the plan above for a weight blob and a window spacing (include/aframe.h).
+AF_API aframe_status aframe_describe_shared_plan(const void* host_blob, size_t bytes, int32_t kernel_len, int32_t n_channels,
+                                                 int32_t window_spacing, int64_t n_windows, int32_t* first_stage_blocks,
+                                                 aframe_stage_plan* stages, int32_t max_stages, int32_t* n_stages) {
+  if (!host_blob || !first_stage_blocks || !n_stages || (max_stages > 0 && !stages) || kernel_len < 1 || window_spacing < 1 ||
+      n_windows < 1 || max_stages < 0) return AFRAME_EINVAL;
+  std::vector<LayerDesc> layers;
+  uint32_t hdr[8];
+  const char* why = "";
+  const aframe_status st = af_parse_layer_table(host_blob, bytes, kernel_len, n_channels, layers, hdr, &why);
+  if (st != AFRAME_OK) return st;
+  *first_stage_blocks = 0; *n_stages = 0;
+  if (layers.size() < 3 || layers[0].kind != 0 || layers[1].kind != 1) return AFRAME_OK;   // not a stem + pool table: nothing is shared
+  const int64_t chunk = n_windows < tc_chunk_windows() ? n_windows : tc_chunk_windows();
+  const SharedPlan pl = tc_plan_shared(layers, hdr[3] == 2, window_spacing, chunk);
+  *first_stage_blocks = pl.s1_on ? pl.s1_k : 0;
+  for (const SharedStage& g : pl.stages) {
+    if (*n_stages >= max_stages) break;
+    aframe_stage_plan& o = stages[(*n_stages)++];
+    memset(&o, 0, sizeof(o));
+    o.first_layer = g.i0; o.n_layers = (int32_t)g.list.size(); o.T = g.T; o.C = g.C; o.head = g.head; o.tail = g.tail;
+    o.packed = g.packed ? 1 : 0; o.P = g.packed ? g.P : g.rows; o.spare_slots = g.packed ? SH_SPARE_SLOTS : 0;
+    for (int q = 0; q < o.n_layers && q < 16; ++q) {
+      o.e_head[q] = g.packed ? g.e_head[q] : 0; o.e_tail[q] = g.packed ? g.e_tail[q] : 0; o.tbox[q] = g.packed ? g.tbox[q] : 0;
+    }
+  }
+  return AFRAME_OK;
 }
 
 aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const void* d_in, int in_dt, int64_t sB,
@@ -612,20 +754,9 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   const int64_t chunk = tc_chunk_windows() < B ? tc_chunk_windows() : B;
   const size_t slot_bytes = ((plan.slot_elems * 2 * (size_t)chunk) + 1023) & ~(size_t)1023;
   const int n = (int)w->layers.size();
-  // fused head: the conv feeding the head (and nothing else) pools + dots in its epilogue and stores nothing
-  int fuse = -1, n_part = 0;
-  {
-    const LayerDesc& h = w->layers[n - 1];
-    const int src = h.input_from;
-    bool only_consumer = src >= 2 && w->layers[src].kind == 0;
-    for (int i = 0; only_consumer && i < n - 1; ++i)
-      if (w->layers[i].input_from == src || w->layers[i].residual_from == src) only_consumer = false;
-    if (only_consumer && w->layers[src].c_out % 256 == 0 && w->layers[src].c_out <= 512 && tile_t_box(w->layers[src].t_out) % 32 == 0 &&
-        !w->live_gn) {
-      fuse = src;
-      n_part = (w->layers[src].t_out / 32) * (w->layers[src].c_out / 64) * TcCfg<256, true>::EPW;   // head units of EPI_COLS channels
-    }
-  }
+  SharedPlan shp = tc_plan_shared(w->layers, w->live_gn, sB, chunk);
+  const int fuse = shp.fuse;
+  const int n_part = fuse >= 0 ? (w->layers[fuse].t_out / 32) * (w->layers[fuse].c_out / 64) * TcCfg<256, true>::EPW : 0;   // head units of EPI_COLS channels
   // live GroupNorm scratch after the slots: (mu, rstd) per (window, group), then the conv epilogues' partial sums
   size_t gn_part_elems = 0;                                      // float2 per window
   if (w->live_gn)
@@ -639,81 +770,13 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
   const size_t gn_stats_bytes = (sizeof(float2) * (size_t)w->n_groups * chunk + 1023) & ~(size_t)1023;
   const size_t part_bytes = w->live_gn ? gn_stats_bytes + ((sizeof(float2) * gn_part_elems * chunk + 1023) & ~(size_t)1023)
                                        : ((sizeof(float) * (size_t)n_part * chunk + 1023) & ~(size_t)1023);
-  // shared first stage (see s1_gather_kernel): K streams + one gathered input + K edge results per chunk
-  const int s1_k = s1_chain_blocks(w);
-  const bool s1_on = s1_k > 0 && sB % 4 == 0 && sB < w->layers[0].t_in && chunk >= 2 && !w->live_gn &&
-                     w->layers[1].t_out >= 2 * S1_ROWS;
-  // shared later stages (see sh_gather_kernel): per launched layer one stream and one edge-batch tensor, plus the gathered input
-  auto up128 = [](int64_t v) { return (v + 127) / 128 * 128; };
-  struct SharedStage {
-    std::vector<int> list;            // layers that launch, entry conv first
-    int i0 = 0, T = 0, C = 0, C_in = 0, head = 0, tail = 0;
-    int rows = 0, period = 0;         // short window: data rows, data + 2 separator rows
-    int64_t shift = 0;                // rows between consecutive windows at this stage's resolution
-    int64_t rows_stream = 0, rows_edge = 0;
-    size_t stream_bytes = 0, edge_bytes = 0, x_bytes = 0, off = 0;
-    // packed edge batch (stages whose layers run on the CTA-pair path): P rows per short-window slot, per launched layer the
-    // edge rows of its output at the window's start / end and the rows its box computes (16 or 32)
-    bool packed = false;
-    int P = 0;
-    std::vector<int> e_head, e_tail, tbox;
-  };
-  std::vector<SharedStage> shs;
-  bool sh_head_on = false;
-  if (s1_on) {
-    int i0 = 2 + 2 * s1_k, Tp = w->layers[1].t_out, hp = 2 * s1_k + 2, tp = 2 * s1_k + 1;
-    int64_t shift_p = sB / 4;
-    const int max_stages = 3;
-    while ((int)shs.size() < max_stages && shift_p % 2 == 0 && !sh_head_on) {
-      SharedStage g;
-      g.list = s2_chain_layers(w, i0);
-      if (g.list.empty()) break;
-      if (fuse >= i0 && fuse <= g.list.back()) {
-        // the stage that ends in the fused head: its last conv stores like any other and sh_head_partial_kernel emits the
-        // head's partial sums; needs whole 32-row slabs and the head as the only reader
-        if (fuse != g.list.back() || w->layers[fuse].t_out % 32 != 0) break;
-        sh_head_on = true;
-      }
-      const int n2 = (int)g.list.size() - 1;
-      g.i0 = i0; g.T = w->layers[i0].t_out; g.C = w->layers[i0].c_out; g.C_in = w->layers[i0].c_in;
-      g.shift = shift_p / 2;
-      g.head = hp / 2 + 1 + n2;                                   // rows within reach of the window's zero padding ...
-      g.tail = g.T - (Tp - tp) / 2 + n2;                          // ... at the start and at the end of the stage's output
-      const int src_rows = shs.empty() ? S1_ROWS : shs.back().rows;
-      g.rows = g.head + n2 > g.tail + n2 + 1 ? g.head + n2 : g.tail + n2 + 1;
-      g.period = g.rows + 2;
-      const bool fits = g.T >= g.rows && Tp >= 2 * g.rows && Tp == 2 * g.T && hp <= src_rows - 2 && tp <= src_rows - 2 &&
-                        g.C % 64 == 0 && g.C_in % 64 == 0;
-      if (!fits) { sh_head_on = false; break; }
-      g.rows_stream = up128((chunk - 1) * g.shift + g.T);
-      g.rows_edge = up128(2 * chunk * g.period);
-      // Packed edge batch: layer q's output differs from the stream's only in its first e_head[q] / last e_tail[q] rows (one more
-      // per conv); its box holds those rows and the two rows next to them that the epilogue takes from the stream (the outer one
-      // is computed from a row outside the box): tbox[q] = max(e_head, e_tail) + 2 rows, floor(128 / tbox) slots per MMA tile.
-      // (The entry conv's rows are all computed from valid input rows and the last layer's interior rows are never read: no copies.)
-      if (g.C % 256 == 0) {
-        const int nl = (int)g.list.size();
-        g.e_head.resize(nl); g.e_tail.resize(nl); g.tbox.assign(nl, 0);
-        bool ok = true;
-        int Pmax = 0;
-        for (int q = 0; q < nl; ++q) {
-          g.e_head[q] = hp / 2 + 1 + q;
-          g.e_tail[q] = g.T - (Tp - tp) / 2 + q;
-          // edge rows + the two copied rows; the stage's last layer is read at its edge rows only (next stage's gather, stitch, head)
-          g.tbox[q] = (g.e_head[q] > g.e_tail[q] ? g.e_head[q] : g.e_tail[q]) + (q + 1 < nl ? 2 : 0);
-          if (g.tbox[q] > 32 || g.tbox[q] < 1 || 128 / g.tbox[q] > SH_SPARE_SLOTS) ok = false;   // (a half's last box overhangs by < 128 / tbox slots)
-          if (g.tbox[q] > Pmax) Pmax = g.tbox[q];
-        }
-        if (ok && g.T >= 2 * Pmax && g.e_head[nl - 1] == g.head && g.e_tail[nl - 1] == g.tail) {
-          g.packed = true; g.P = Pmax;
-          g.rows_edge = 2 * (chunk + SH_SPARE_SLOTS) * g.P;
-        }
-      }
-      if (!g.packed && !shs.empty() && shs.back().packed) { sh_head_on = false; break; }   // (a packed stage feeds packed stages only)
-      shs.push_back(g);
-      i0 = g.list.back() + 1; Tp = g.T; hp = g.head; tp = g.tail; shift_p = g.shift;
-    }
-  }
+  // shared first stage (see s1_gather_kernel): K streams + one gathered input + K edge results per chunk; shared later
+  // stages (see sh_gather_kernel): per launched layer one stream and one edge-batch tensor, plus the gathered input
+  const int s1_k = shp.s1_k;
+  const bool s1_on = shp.s1_on;
+  auto up128 = [](int64_t v) { return tc_up128(v); };
+  std::vector<SharedStage>& shs = shp.stages;
+  const bool sh_head_on = shp.sh_head_on;
   const bool s2_on = !shs.empty();
   const int64_t s1_rows = (chunk - 1) * (sB / 4) + w->layers[1].t_out;
   const size_t s1_stream_bytes = s1_on ? (((size_t)s1_rows * 128 + 1023) & ~(size_t)1023) : 0;
@@ -769,7 +832,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         for (int i = 2; i < n; ++i) {
           const LayerDesc& l = w->layers[i];
           const int r = l.residual_from;
-          if (l.kind != 0 || r < 2 || i == fuse || !w->d_bias_sc[i]) continue;
+          if (l.kind != 0 || r < 2 || i == fuse || !has_projection_residual(w->layers, i) || !w->d_bias_sc[i]) continue;
           const LayerDesc& q = w->layers[r];
           bool ok = q.kind == 0 && q.k == 1 && q.pad == 0 && !q.relu && q.residual_from < 0 && q.c_in % 64 == 0 &&
                     q.t_out == l.t_out && q.c_out == l.c_out && q.t_in % q.stride == 0 && q.input_from >= 1 &&

@@ -22,13 +22,30 @@ struct aframe_stream_state {
   float* d_new = nullptr;        // [C][stride]
   // One update = one CUDA graph launch: the launch sequence is captured the first time a given triple of caller
   // pointers is seen and replayed afterwards (every decision of an update is taken on the device from the counters,
-  // so the same graph serves every update).
-  cudaGraphExec_t graph = nullptr;
-  const float* g_in = nullptr; float* g_scores = nullptr; int32_t* g_n = nullptr;
-  void* g_ws = nullptr;          // activation workspace the captured launches point into
+  // so the same graph serves every update).  A caller that alternates between a few buffers keeps one graph per triple
+  // (least recently used of AF_STREAM_GRAPHS is replaced).
+  struct Graph {
+    cudaGraphExec_t exec = nullptr;
+    const float* in = nullptr; float* scores = nullptr; int32_t* n = nullptr;
+    void* ws = nullptr;          // activation workspace the captured launches point into
+    int64_t last_use = 0;
+  };
+  static constexpr int AF_STREAM_GRAPHS = 4;
+  Graph graphs[AF_STREAM_GRAPHS];
   int64_t g_launches = 0;        // kernels per replay
-  int64_t replays = 0;
+  int64_t replays = 0, steps = 0;
 };
+
+const aframe_weights* af_stream_weights(const aframe_stream_state* st) { return st->w; }
+
+// Device resources of a state (after the context's stream has been synchronised); the host shell stays valid and dead.
+void af_stream_release(aframe_stream_state* st) {
+  for (auto& g : st->graphs) { if (g.exec) cudaGraphExecDestroy(g.exec); g = aframe_stream_state::Graph(); }
+  cudaFree(st->blob);
+  st->blob = nullptr;
+  cudaGetLastError();
+  st->ctx = nullptr; st->w = nullptr;
+}
 
 // Append `stride` samples per channel to the ring and advance the counter.  One CTA.
 __global__ void stream_ingest_kernel(const float* __restrict__ fresh, int C, int stride, float* __restrict__ raw,
@@ -108,11 +125,12 @@ AF_API aframe_status aframe_stream_reset(aframe_stream_state* st) {
 
 AF_API void aframe_stream_destroy(aframe_stream_state* st) {
   if (!st) return;
-  if (st->ctx) cudaStreamSynchronize(st->ctx->stream);
-  if (st->graph) cudaGraphExecDestroy(st->graph);
-  cudaFree(st->blob);
-  cudaGetLastError();
-  st->ctx = nullptr;
+  if (aframe_ctx* ctx = st->ctx) {                    // (a dead shell, released with its context or weights, has none)
+    cudaStreamSynchronize(ctx->stream);
+    for (size_t i = 0; i < ctx->live_streams.size(); ++i)
+      if (ctx->live_streams[i] == st) { ctx->live_streams.erase(ctx->live_streams.begin() + i); break; }
+    af_stream_release(st);
+  }
   delete st;
 }
 
@@ -159,7 +177,8 @@ AF_API aframe_status aframe_stream_create(aframe_ctx* ctx, const aframe_weights*
   if (rs == AFRAME_OK) rs = aframe_forward(ctx, w, st->d_white, 1, d_tmp);
   if (rs == AFRAME_OK && cudaStreamSynchronize(ctx->stream) != cudaSuccess) rs = af_fail(ctx, AFRAME_ECUDA, "stream warm-up forward failed");
   cudaFree(d_tmp);
-  if (rs != AFRAME_OK) { cudaGetLastError(); aframe_stream_destroy(st); return rs; }
+  if (rs != AFRAME_OK) { cudaGetLastError(); af_stream_release(st); delete st; return rs; }
+  ctx->live_streams.push_back(st);
   *out = st;
   return AFRAME_OK;
 }
@@ -172,7 +191,7 @@ AF_API int64_t aframe_stream_graph_replays(const aframe_stream_state* st) { retu
 AF_API aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samples, aframe_stream_state* st,
                                         float* d_scores, int32_t* d_n_scores) {
   if (!ctx) return AFRAME_EINVAL;
-  if (!st || st->ctx != ctx) return af_fail(ctx, AFRAME_ESTATE, "stream state is destroyed or belongs to another context");
+  if (!st || st->ctx != ctx || !st->w) return af_fail(ctx, AFRAME_ESTATE, "stream state is released (its weights or context are gone) or belongs to another context");
   if (!d_new_samples || !d_scores || !d_n_scores) return af_fail(ctx, AFRAME_EINVAL, "null pointer");
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
   cudaStreamIsCapturing(ctx->stream, &cap);
@@ -181,10 +200,22 @@ AF_API aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samp
   if (ctx->prof_on || ctx->layer_ms || cap != cudaStreamCaptureStatusNone ||
       ctx->stream == nullptr || ctx->stream == cudaStreamLegacy)
     return stream_step_enqueue(ctx, d_new_samples, st, d_scores, d_n_scores);
-  // (a larger forward on the same context may have re-allocated the activation workspace since the capture)
-  if (!st->graph || st->g_in != d_new_samples || st->g_scores != d_scores || st->g_n != d_n_scores ||
-      st->g_ws != ctx->ws_act.ptr) {
-    if (st->graph) { cudaGraphExecDestroy(st->graph); st->graph = nullptr; }
+  // the graph captured for these pointers (a larger forward on the same context may have re-allocated the activation
+  // workspace since: then it is stale and captured again)
+  st->steps++;
+  aframe_stream_state::Graph* hit = nullptr;
+  aframe_stream_state::Graph* lru = nullptr;          // an empty slot if there is one, else the least recently used
+  for (auto& g : st->graphs) {
+    if (g.exec && g.in == d_new_samples && g.scores == d_scores && g.n == d_n_scores) hit = &g;
+    if (!lru || (lru->exec && (!g.exec || g.last_use < lru->last_use))) lru = &g;
+  }
+  if (hit && hit->ws != ctx->ws_act.ptr) { lru = hit; hit = nullptr; }
+  if (!hit) {
+    if (lru->exec) {                                  // (it may still be in flight)
+      AF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+      cudaGraphExecDestroy(lru->exec);
+      *lru = aframe_stream_state::Graph();
+    }
     const int64_t l0 = ctx->launches;
     AF_CUDA(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
     aframe_status rs = stream_step_enqueue(ctx, d_new_samples, st, d_scores, d_n_scores);
@@ -194,13 +225,15 @@ AF_API aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samp
     ctx->launches = l0;
     if (rs != AFRAME_OK) { if (g) cudaGraphDestroy(g); cudaGetLastError(); return rs; }
     if (e != cudaSuccess || !g) { cudaGetLastError(); return af_fail(ctx, AFRAME_ECUDA, "stream capture failed: %s", cudaGetErrorString(e)); }
-    e = cudaGraphInstantiate(&st->graph, g, 0);
+    e = cudaGraphInstantiate(&lru->exec, g, 0);
     cudaGraphDestroy(g);
-    if (e != cudaSuccess) { st->graph = nullptr; cudaGetLastError(); return af_fail(ctx, AFRAME_ECUDA, "graph instantiation failed: %s", cudaGetErrorString(e)); }
-    st->g_in = d_new_samples; st->g_scores = d_scores; st->g_n = d_n_scores;
-    st->g_ws = ctx->ws_act.ptr;
+    if (e != cudaSuccess) { lru->exec = nullptr; cudaGetLastError(); return af_fail(ctx, AFRAME_ECUDA, "graph instantiation failed: %s", cudaGetErrorString(e)); }
+    lru->in = d_new_samples; lru->scores = d_scores; lru->n = d_n_scores;
+    lru->ws = ctx->ws_act.ptr;
+    hit = lru;
   }
-  AF_CUDA(ctx, cudaGraphLaunch(st->graph, ctx->stream));
+  hit->last_use = st->steps;
+  AF_CUDA(ctx, cudaGraphLaunch(hit->exec, ctx->stream));
   ctx->launches += st->g_launches;
   st->replays++;
   return AFRAME_OK;

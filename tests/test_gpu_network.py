@@ -249,6 +249,35 @@ def test_shared_stages_equal_the_per_window_path_bit_for_bit(af, config1, stride
     assert torch.equal(shared, ref)
 
 
+@pytest.mark.parametrize("kernel_len", [512, 768, 1024, 1280, 2048, 2560, 4096])
+def test_shared_stages_at_other_window_lengths(af, kernel_len):
+    """Windows in place at stride 128 for short and long windows: the planner shares fewer stages where a stage's rows are
+    too few for its edge rows (at 512 / 768 samples a window's first and last edge rows would meet in the 256- / 512-channel
+    stage); what it shares must equal the per-window path -- bit for bit where both run the same kernel variant per layer
+    (128-channel stage of a multiple of 128 rows: resident-weight halo tiles on both paths), else to rounding, because the
+    per-window tiles of a shorter stage go through the tap-major kernel, which adds the same products in another order --
+    and the oracle within rule T3."""
+    cfg = dict(full_config(), kernel_len=kernel_len)
+    blob = make_weight_blob(**cfg)
+    n_win = 70
+    rng = np.random.default_rng(kernel_len + 1)
+    white = torch.from_numpy(rng.standard_normal((2, (n_win - 1) * 128 + kernel_len + 2048)).astype(np.float32)).cuda().half()
+    ctx = af.Context(precision=af.F16, kernel_len=kernel_len)
+    w = ctx.load_weights(blob)
+    shared = ctx.forward_strided(w, white.contiguous(), 0, n_win, chan_shift=[0, 2048])
+    wins = torch.stack([torch.stack([white[0, i * 128: i * 128 + kernel_len], white[1, 2048 + i * 128: 2048 + i * 128 + kernel_len]])
+                        for i in range(n_win)]).float().contiguous()
+    ref = ctx.forward(w, wins)
+    assert bool(torch.isfinite(shared).all())
+    if (kernel_len // 8) % 128 == 0:
+        assert torch.equal(shared, ref)
+    else:
+        assert rel_err(shared.cpu().numpy(), ref.cpu().numpy()) <= 2e-3     # (measured 1e-3: one fp16 ulp is 5e-4)
+    picks = [0, 1, n_win // 2, n_win - 1]
+    want = onet.forward(onet.parse_blob(blob), wins[picks].cpu().numpy().astype(np.float64))
+    assert rel_err(shared[picks].cpu().numpy(), want) <= 2e-2
+
+
 def test_tensor_mac_counter_matches_the_layer_table(af, config1):
     """aframe_tensor_macs (bench.py's roofline numerator) counts, per launch, tile rows x C_out x K.  On the per-window path
     (explicit windows, 128 of them: every conv's rows fill whole 128-row tiles) that is the layer table's own MAC count,

@@ -327,3 +327,44 @@ def test_configurations_the_streaming_state_or_the_path_cannot_honour_are_refuse
     with pytest.raises(af.AframeError) as e:
         af.Context(precision=af.BF16)
     assert e.value.status == af.EUNSUPPORTED
+
+
+def test_objects_may_be_destroyed_in_any_order_and_graphs_are_kept_per_buffer(af):
+    """Lifetime (aframe.h): closing the context first, or freeing the weights under a live stream state, leaves dead shells
+    that only accept their own free / destroy call; a caller that alternates between buffers keeps one graph per buffer
+    (all but the first update per buffer are replays) and gets the same scores as with a single buffer."""
+    tc = tiny_config()
+    blob = make_weight_blob(**tc)
+    n_updates = 131072 // S + tc["kernel_len"] // S + 6
+    x = coloured_noise(n_updates * S, seed=21)
+    upd = torch.from_numpy(np.ascontiguousarray(x.reshape(2, n_updates, S).transpose(1, 0, 2))).cuda()
+    stream = torch.cuda.Stream()
+    out = {}
+    with torch.cuda.stream(stream):
+        for n_buf in (1, 3):
+            ctx = af.Context(n_design=4096, kernel_len=tc["kernel_len"], precision=af.FP32, stream=stream)
+            w = ctx.load_weights(blob)
+            st = ctx.stream_create(w)
+            bufs = [torch.empty((2, S), dtype=torch.float32, device="cuda") for _ in range(n_buf)]
+            scores = []
+            for u in range(n_updates):
+                b = bufs[u % n_buf]
+                b.copy_(upd[u], non_blocking=True)
+                st.step(b)
+                if u >= n_updates - 6:
+                    stream.synchronize()
+                    scores.append((int(st.n_scores.item()), float(st.score.item())))
+            stream.synchronize()
+            replays = int(ctx.lib.aframe_stream_graph_replays(st.handle))
+            assert replays == n_updates                         # every update went through a graph; captures: n_buf
+            out[n_buf] = scores
+            if n_buf == 1:
+                ctx.close()                                     # context first: children become dead shells
+                st.close(); w.free()
+            else:
+                w.free()                                        # weights under a live state: the state is released
+                with pytest.raises(af.AframeError) as e:
+                    st.step(bufs[0])
+                assert e.value.status == af.ESTATE
+                st.close(); ctx.close()
+    assert out[1] == out[3] and all(f == 1 for f, _ in out[1])
