@@ -117,6 +117,12 @@ struct TcShapeOverride {
   int e_nbp = 0, e_P = 0, e_tbox = 0, e_T = 0, e_head = 0, e_tail = 0;
   int64_t e_shift = 0, e_nb = 0;
   const af_act_t* e_stream = nullptr;
+  // packed stages read their stage input in place: in_rows > 0: the (stream) launch's input tensor holds in_rows rows
+  // (rows past them read as zero); e_Pin > 0: the edge launch's input slots hold e_Pin rows (the stage-input slots of the
+  // entry conv and of the conv with the folded projection are only as long as those two layers reach)
+  // (main: the layer's own input; sc: the input of the projection folded into it)
+  int64_t in_rows = 0, in_rows_sc = 0;
+  int e_Pin = 0, e_Pin_sc = 0;
   bool head_rows = false;     // with head = true: per-row head dot products into head_part (TcConvParams::head_rows)
   bool pair_plan = false;     // one shared-memory plan for every launch of the stage, so that two of them can share a launch
 };
@@ -127,6 +133,8 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   const bool packed = ov && ov->e_nbp > 0;
   if (packed) { nb = 2 * ov->e_nbp; l.t_out = ov->e_P; l.t_in = ov->e_P * l.stride; }
   else if (ov) { nb = 1; l.t_out = ov->t_out; l.t_in = ov->t_out * l.stride; }
+  // rows of the input tensor as the tensor map sees them (out-of-range rows are zero-filled by TMA)
+  const int64_t in_rows = packed && ov->e_Pin > 0 ? ov->e_Pin : (ov && ov->in_rows > 0 ? ov->in_rows : l.t_in);
   const int BN = l.c_out >= 256 ? 256 : l.c_out;
   const bool cg2 = BN == 256;                                    // CTA pairs (cta_group::2) for the N = 256 layers
   const int T_box = packed ? ov->e_tbox : tile_t_box(l.t_out), B_box = 128 / T_box;
@@ -135,8 +143,8 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   // resident weights + one halo box per tile (see TcConvParams): stride-1 k3 layers whose tiles stay inside a window
   bool halo = !head && !cg2 && l.k == 3 && l.stride == 1 && l.pad == 1 && T_box == 128 && BN == l.c_out && BN <= 128;
   {
-    const uint64_t dims[4] = {(uint64_t)l.c_in, (uint64_t)P, (uint64_t)(l.t_in / P), (uint64_t)nb};
-    const uint64_t str[3] = {(uint64_t)l.c_in * 2, (uint64_t)P * l.c_in * 2, (uint64_t)l.t_in * l.c_in * 2};
+    const uint64_t dims[4] = {(uint64_t)l.c_in, (uint64_t)P, (uint64_t)(in_rows / P), (uint64_t)nb};
+    const uint64_t str[3] = {(uint64_t)l.c_in * 2, (uint64_t)P * l.c_in * 2, (uint64_t)in_rows * l.c_in * 2};
     const uint32_t box[4] = {64, 1, (uint32_t)(halo ? T_box + 2 : T_box), (uint32_t)B_box};
     if (!encode_map(ctx, &L.tm_in, in, 4, dims, str, box)) return false;
   }
@@ -157,8 +165,9 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   if (sc >= 0) {
     LayerDesc q = w->layers[sc];
     if (ov) { q.t_out = l.t_out; q.t_in = l.t_out * q.stride; }
-    const uint64_t dims[4] = {(uint64_t)q.c_in, (uint64_t)q.stride, (uint64_t)(q.t_in / q.stride), (uint64_t)nb};
-    const uint64_t str[3] = {(uint64_t)q.c_in * 2, (uint64_t)q.stride * q.c_in * 2, (uint64_t)q.t_in * q.c_in * 2};
+    const int64_t sc_rows = packed && ov->e_Pin_sc > 0 ? ov->e_Pin_sc : (ov && ov->in_rows_sc > 0 ? ov->in_rows_sc : q.t_in);
+    const uint64_t dims[4] = {(uint64_t)q.c_in, (uint64_t)q.stride, (uint64_t)(sc_rows / q.stride), (uint64_t)nb};
+    const uint64_t str[3] = {(uint64_t)q.c_in * 2, (uint64_t)q.stride * q.c_in * 2, (uint64_t)sc_rows * q.c_in * 2};
     const uint32_t box[4] = {64, 1, (uint32_t)T_box, (uint32_t)B_box};
     if (!encode_map(ctx, &L.tm_res, sc_in, 4, dims, str, box)) return false;
     const uint64_t wd[3] = {(uint64_t)q.c_in, (uint64_t)q.c_out, 1};
@@ -185,6 +194,10 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.edge_nbp = packed ? ov->e_nbp : 0;
   p.edge_blks_half = packed ? (int)((ov->e_nb + B_box - 1) / B_box) : 0;
   p.edge_t0_tail = packed ? ov->e_P - T_box : 0;
+  // ... and where a tail box starts in the slots it READS (in output-row units of this layer): slots of the previous layer's
+  // output are as long as this layer's; stage-input slots (e_Pin rows at the previous stage's resolution) are shorter
+  p.edge_t0_tail_in = packed ? (int)(in_rows / P) - T_box : 0;
+  p.edge_t0_tail_sc = packed && sc >= 0 ? (int)((ov->e_Pin_sc > 0 ? ov->e_Pin_sc : w->layers[sc].stride * ov->e_P) / w->layers[sc].stride) - T_box : 0;
   p.edge_T = packed ? ov->e_T : 0; p.edge_P = packed ? ov->e_P : 0;
   p.edge_head = packed ? ov->e_head : 0; p.edge_tail = packed ? ov->e_tail : 0;
   p.edge_shift = packed ? ov->e_shift : 0;
@@ -202,6 +215,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.head_part = head ? head_part : nullptr;
   p.head_slabs = l.t_out / 32;
   p.head_rows = (head && ov && ov->head_rows) ? 1 : 0; p.head_row_stride = l.t_out;
+  p.head_rows_total = (long long)l.t_out * nb;
   p.nb = packed ? ov->e_nb : nb;
 #ifdef AFRAME_TC_CYCLES
   p.dbg_out = tc_cycles_slot();
@@ -503,8 +517,9 @@ __global__ void s2_stitch_kernel(uint4* __restrict__ out, const uint4* __restric
 // stream and Re over the edge batch; here one warp = one 32-row slab of one window x one unit, lane = row of the slab, and
 // the 32 values are summed in the order the fused head uses.  head_finish_kernel then sums the partials as usual.
 __global__ void __launch_bounds__(256)
-sh_head_rows_kernel(const float* __restrict__ Rs, const float* __restrict__ Re, float* __restrict__ head_part, int64_t nb, int T,
-                    int chunks, int64_t row_shift, int c_head, int c_tail, int64_t e_stride, int64_t e_tail0, int e_trow) {
+sh_head_rows_kernel(const float* __restrict__ Rs, int64_t rows_s, const float* __restrict__ Re, int64_t rows_e,
+                    float* __restrict__ head_part, int64_t nb, int T, int chunks, int64_t row_shift, int c_head, int c_tail,
+                    int64_t e_stride, int64_t e_tail0, int e_trow) {
   const int lane = threadIdx.x & 31;
   const int slabs = T / 32;
   const int64_t wi = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -514,9 +529,9 @@ sh_head_rows_kernel(const float* __restrict__ Rs, const float* __restrict__ Re, 
   const int64_t b = wi / ((int64_t)chunks * slabs);
   const int t = slab * 32 + lane;
   float sum;
-  if (t < c_head) sum = Re[(b * e_stride + t) * chunks + c];
-  else if (t >= T - c_tail) sum = Re[(e_tail0 + b * e_stride + (t - e_trow)) * chunks + c];
-  else sum = Rs[(b * row_shift + t) * chunks + c];
+  if (t < c_head) sum = Re[c * rows_e + b * e_stride + t];
+  else if (t >= T - c_tail) sum = Re[c * rows_e + e_tail0 + b * e_stride + (t - e_trow)];
+  else sum = Rs[c * rows_s + b * row_shift + t];
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
   if (lane == 0) head_part[(b * slabs + slab) * chunks + c] = sum;
@@ -560,7 +575,7 @@ void af_tc_forget(aframe_ctx* ctx) {
 // Windows per internal launch sequence.  Measured on B200: every layer launch carries ~12 us of launch gap, prologue
 // (TMEM/barriers/first loads from HBM) and drain, so large chunks win (592: 869, 1184: 922, 4096: 994 TFLOP/s); the three
 // live activation tensors leave the 126 MB L2 from ~300 windows on anyway.
-static int64_t tc_chunk_windows() { return 4096; }
+static int64_t tc_chunk_windows() { return 8192; }
 
 // Number of leading fused 64-channel blocks that form a chain on the pooled stem output (layers 2,3 | 4,5 | ...): the
 // blocks the shared first stage can take over.
@@ -628,7 +643,7 @@ struct SharedStage {
   // packed edge batch (stages whose layers run on the CTA-pair path): P rows per short-window slot, per launched layer the
   // edge rows of its output at the window's start / end and the rows its box computes
   bool packed = false;
-  int P = 0;
+  int P = 0, P_in = 0;              // rows per slot of the layers' outputs / of the gathered stage input
   std::vector<int> e_head, e_tail, tbox;
 };
 struct SharedPlan {
@@ -787,7 +802,11 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     SharedStage& h = shs[g];
     // one tensor per layer: [stream rows | edge-batch rows], and the entry conv's input at twice the rows
     h.stream_bytes = ((size_t)(h.rows_stream + h.rows_edge) * h.C * 2 + 1023) & ~(size_t)1023;
-    h.x_bytes = ((size_t)2 * (h.rows_stream + h.rows_edge) * h.C_in * 2 + 1023) & ~(size_t)1023;
+    // the stage input: packed stages read the previous stage's stream in place and gather only the slots their first two
+    // layers reach (P_in rows per slot at the previous stage's resolution); other stages gather [stream | short windows]
+    h.P_in = h.packed ? 2 * (h.tbox.size() > 1 ? h.tbox[1] : h.tbox[0] + 1) : 0;
+    h.x_bytes = h.packed ? (((size_t)2 * (chunk + SH_SPARE_SLOTS) * h.P_in * h.C_in * 2 + 1023) & ~(size_t)1023)
+                         : (((size_t)2 * (h.rows_stream + h.rows_edge) * h.C_in * 2 + 1023) & ~(size_t)1023);
     h.off = s2_bytes;
     s2_bytes += h.x_bytes + h.list.size() * h.stream_bytes;
   }
@@ -895,9 +914,15 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             const int qi = entry ? -1 : idx_of(l.input_from), qr = (l.residual_from >= 0 && sc < 0) ? idx_of(l.residual_from) : -1;
             ok = (entry || qi >= 0) && (l.residual_from < 0 || sc >= 0 || qr >= 0);
             if (!ok) break;
-            const af_act_t* x_edge = sh_x_ptr((int)g) + 2 * rows_s * h.C_in;
+            // stage input: the previous stage's stream in place (its valid rows; the rest reads as zero), and the gathered slots
+            const int q_prev = g ? (int)shs[g - 1].list.size() - 1 : 0;
+            const af_act_t* x_stream = g ? sh_buf((int)g - 1, 0, q_prev) : s1_stream_ptr(s1_k);
+            const af_act_t* x_edge = sh_x_ptr((int)g);
             TcShapeOverride ov_s{(int)rows_s, 0, 0, 0};
             TcShapeOverride ov_e{0, 0, 0, 0};
+            const int64_t valid_prev = (g ? (nb - 1) * shs[g - 1].shift + shs[g - 1].T : (nb - 1) * (sB / 4) + w->layers[1].t_out) & ~(int64_t)1;
+            if (entry) { ov_s.in_rows = valid_prev; ov_e.e_Pin = h.P_in; }
+            if (sc >= 0) { ov_s.in_rows_sc = valid_prev; ov_e.e_Pin_sc = h.P_in; }
             // the conv that feeds the head stores nothing: its tensor holds the per-row head dot products instead
             // ([stream rows | edge-batch rows][C / 64] floats)
             const bool hr = sh_head_on && g + 1 == shs.size() && q + 1 == h.list.size();
@@ -908,8 +933,8 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             if (hr) pc->sh_head_rows = true;
             ov_e.e_nbp = (int)P.nbp; ov_e.e_P = h.P; ov_e.e_tbox = h.tbox[q]; ov_e.e_T = h.T; ov_e.e_head = h.e_head[q]; ov_e.e_tail = h.e_tail[q];
             ov_e.e_shift = h.shift; ov_e.e_nb = nb; ov_e.e_stream = (entry || q + 1 == h.list.size()) ? nullptr : sh_buf((int)g, 0, (int)q);
-            ok = build_launch(ctx, w, li, entry ? sh_x_ptr((int)g) : sh_buf((int)g, 0, qi), qr >= 0 ? sh_buf((int)g, 0, qr) : nullptr,
-                              sh_buf((int)g, 0, (int)q), 1, hr, hr_s, P.stream[q], sc, sc >= 0 ? sh_x_ptr((int)g) : nullptr, &ov_s) &&
+            ok = build_launch(ctx, w, li, entry ? x_stream : sh_buf((int)g, 0, qi), qr >= 0 ? sh_buf((int)g, 0, qr) : nullptr,
+                              sh_buf((int)g, 0, (int)q), 1, hr, hr_s, P.stream[q], sc, sc >= 0 ? x_stream : nullptr, &ov_s) &&
                  build_launch(ctx, w, li, entry ? x_edge : sh_buf((int)g, 1, qi), qr >= 0 ? sh_buf((int)g, 1, qr) : nullptr,
                               sh_buf((int)g, 1, (int)q), 1, hr, hr_e, P.edge[q], sc, sc >= 0 ? x_edge : nullptr, &ov_e);
           }
@@ -1021,8 +1046,8 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         const int64_t n_g = (copy_rows + edge_rows_in) * pieces_in;
         const int q_prev = g ? (int)pc->sh[g - 1].layers.size() - 1 : 0;
         if (P.packed) {
-          const int64_t n_p = (copy_rows + 2 * P.nbp * 2 * P.P) * pieces_in;
-          const int64_t valid_prev = g ? (nb - 1) * pc->sh[g - 1].shift + pc->sh[g - 1].T : (nb - 1) * shift + T1;
+          const int P_in = shs[g].P_in;
+          const int64_t n_p = (2 * P.nbp * P_in) * pieces_in;
           aux_begin();
           shp_gather_kernel<<<(unsigned)((n_p + 255) / 256), 256, 0, ctx->stream>>>(
               reinterpret_cast<uint4*>(sh_x_ptr((int)g)),
@@ -1030,7 +1055,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
               reinterpret_cast<const uint4*>(g ? sh_buf((int)g - 1, 1, q_prev) : s1_edge_ptr(K)), nb, P.nbp, 2 * P.T, pieces_in,
               2 * P.shift, g ? pc->sh[g - 1].e_stride : 2 * S1_PERIOD, g ? pc->sh[g - 1].e_tail0 : S1_PERIOD,
               g ? pc->sh[g - 1].e_trow : T1 - S1_ROWS, g ? pc->sh[g - 1].head : 2 * K + 2, g ? pc->sh[g - 1].tail : 2 * K + 1,
-              copy_rows, valid_prev, 2 * P.P);
+              0, 0, P_in);
           AF_LAUNCH_CHECK(ctx);
           aux_end();
           // Launch order: stream(0) | edge(q) with stream(q + 1) as ONE launch of two problems (independent of each other: both
@@ -1044,8 +1069,10 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             return a.cg2 && b.cg2 && a.BN == 256 && b.BN == 256 && !a.head && !b.head && !a.halo && !b.halo && a.p.stages == b.p.stages &&
                    a.p.nbuf == b.p.nbuf && a.p.pf == b.p.pf && a.smem == b.smem && a.p.c_out == b.p.c_out;
           };
-          auto launch_one = [&](TcLaunch& A, TcLaunch* B2) -> aframe_status {
-            A.p.reverse = 0;
+          // consecutive edge launches walk their tiles in opposite directions: layer q + 1 starts on the slots layer q wrote
+          // last, which are still in L2 (an edge-batch tensor is 100-135 MB, the L2 126 MB)
+          auto launch_one = [&](TcLaunch& A, TcLaunch* B2, int rev = 0) -> aframe_status {
+            A.p.reverse = rev;
             if (B2) B2->p.reverse = 0;
             cudaError_t e = launch_conv(A, ctx->stream, B2);
             ctx->launches++; ++n_conv; ++span_conv; ctx->tc_macs += A.macs + (B2 ? B2->macs : 0.0);
@@ -1055,9 +1082,9 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           if ((st = launch_one(P.stream[0], nullptr)) != AFRAME_OK) return st;
           for (size_t q = 0; q < nl; ++q) {
             if (can_pair(q)) {
-              if ((st = launch_one(P.edge[q], &P.stream[q + 1])) != AFRAME_OK) return st;
+              if ((st = launch_one(P.edge[q], &P.stream[q + 1], (int)(q & 1))) != AFRAME_OK) return st;
             } else {
-              if ((st = launch_one(P.edge[q], nullptr)) != AFRAME_OK) return st;
+              if ((st = launch_one(P.edge[q], nullptr, (int)(q & 1))) != AFRAME_OK) return st;
               if (q + 1 < nl && (st = launch_one(P.stream[q + 1], nullptr)) != AFRAME_OK) return st;
             }
           }
@@ -1087,8 +1114,8 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
           const float* hr_s = reinterpret_cast<const float*>(sh_buf((int)g, 0, q_last));
           aux_begin();
           sh_head_rows_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(
-              hr_s, hr_s + sh_rows_stream((int)g) * hu, head_part, nb, P.T, hu, P.shift, P.head, P.tail, P.e_stride,
-              P.e_tail0, P.e_trow);
+              hr_s, sh_rows_stream((int)g), hr_s + sh_rows_stream((int)g) * hu, 2 * P.nbp * P.P, head_part, nb, P.T, hu, P.shift,
+              P.head, P.tail, P.e_stride, P.e_tail0, P.e_trow);
           AF_LAUNCH_CHECK(ctx);
           aux_end();
         } else if (g + 1 == pc->sh.size()) {

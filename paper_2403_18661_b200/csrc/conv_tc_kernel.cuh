@@ -57,9 +57,11 @@ struct TcConvParams {
   const float* head_w;
   float* head_part;
   int head_slabs;            // T_out / T_box
-  // head_rows != 0 (shared stages): head_part receives the dot product of EVERY output row's 64-channel chunk instead,
-  // head_part[((b0 + row / T_box) * head_row_stride + t) * (c_out / 64) + chunk]; sh_head_rows_kernel sums them per window slab
+  // head_rows != 0 (shared stages): head_part receives the dot product of EVERY output row with each head unit instead
+  // (unit-major, so that a warp's 32 rows are 32 consecutive floats on both sides):
+  // head_part[unit * head_rows_total + (b0 + row / T_box) * head_row_stride + t]; sh_head_rows_kernel sums them per window slab
   int head_rows, head_row_stride;
+  long long head_rows_total;
   int64_t nb;                // windows in this launch (head variant bounds check)
   // HALO variant (k = 3, stride 1, whole 128-row tiles inside one window): the folded weights of the layer stay resident
   // in shared memory (w_bytes) and ONE (128 + 2)-row input box per 64-channel block serves all three taps: tap d reads
@@ -90,6 +92,7 @@ struct TcConvParams {
   int edge_nbp;              // 0 = off; else slots per half (windows + spare slots for the last box of a half)
   int edge_blks_half;        // boxes per half: M tiles [0, edge_blks_half) are window starts, the rest window ends
   int edge_t0_tail, edge_T, edge_P, edge_head, edge_tail;
+  int edge_t0_tail_in, edge_t0_tail_sc;   // start of a tail box in the slots it reads (main input / fused-projection input)
   int a_bytes;               // bytes of one activation box (T_box * B_box rows of 128 B; 16 KB unless T_box does not divide 128:
                              // the rest of the 128-row MMA tile is then stale shared memory, and those rows are dropped)
   long long edge_shift;
@@ -354,6 +357,10 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         int n_idx, t0, b0;
         decode(p, tile, n_idx, t0, b0);
         const int n0 = n_idx * BN;
+        // packed edge batch, tail boxes: the slots this launch reads may be shorter than the slots it writes
+        const bool tail_box = p.edge_nbp > 0 && b0 >= p.edge_nbp;
+        const int t0s = tail_box ? p.edge_t0_tail_sc : t0;
+        if (tail_box) t0 = p.edge_t0_tail_in;
         for (int d = 0; d < p.taps; ++d) {
           const int toff = p.tap_toff[d], par = p.tap_par[d];
           for (int kb = 0; kb < p.kblocks; ++kb) {
@@ -386,11 +393,11 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             if (CG2) {
               if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * (p.a_bytes + Cfg::B_BYTES));
               const uint32_t lbar = lfull0 + 8u * stage;
-              tma_load_4d_cg2(sa, &tm_res, lbar, kb * 64, 0, t0, b0);
+              tma_load_4d_cg2(sa, &tm_res, lbar, kb * 64, 0, t0s, b0);
               tma_load_3d_cg2(sa + Cfg::A_BYTES, &tm_scw, lbar, kb * 64, n0 + (int)rank * Cfg::B_ROWS, 0);
             } else {
               mbar_arrive_expect_tx(full_bar(stage), p.a_bytes + Cfg::B_BYTES);
-              tma_load_4d(sa, &tm_res, full_bar(stage), kb * 64, 0, t0, b0);
+              tma_load_4d(sa, &tm_res, full_bar(stage), kb * 64, 0, t0s, b0);
               tma_load_3d(sa + Cfg::A_BYTES, &tm_scw, full_bar(stage), kb * 64, n0, 0);
             }
           }
@@ -649,7 +656,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           // head units: EC channels (one per epilogue warp of a quadrant), c_out / EC of them per row
           const int hu = (n_idx * CH + c) * EPW + hf, n_hu = (p.c_out >> 6) * EPW;
           if (p.head_rows) {
-            if (row < p.T_box * p.B_box) p.head_part[((long long)(b0 + row / p.T_box) * p.head_row_stride + t_row) * n_hu + hu] = s;
+            // (rows past the tensor -- the peer CTA's half of a last, partial pair tile -- have no place in a unit's row array)
+            const long long hr = (long long)(b0 + row / p.T_box) * p.head_row_stride + t_row;
+            if (row < p.T_box * p.B_box && t_row < p.head_row_stride && hr < p.head_rows_total) p.head_part[hu * p.head_rows_total + hr] = s;
           } else {
 #pragma unroll
           for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
