@@ -76,7 +76,8 @@ typedef struct {
   int32_t  precision;         /* network path: AFRAME_F16 (tensor cores, default) or AFRAME_FP32 */
   int32_t  welch_average;     /* 0 = mean over segments (reading A1, default); 1 = per-bin median
                                  divided by its bias for n segments (NEXT-3 variant; n <= 255)   */
-  int32_t  reserved_;         /* must be 0                                                       */
+  int32_t  stream_full_forward; /* aframe_stream_step: 0 (default) = the incremental network where the configuration
+                                 allows it (see aframe_stream_incremental); 1 = one full forward of the window per update */
 } aframe_config;
 
 typedef struct aframe_ctx aframe_ctx;
@@ -260,6 +261,25 @@ aframe_status aframe_describe_shared_plan(const void* host_blob, size_t bytes, i
 /* How many updates of this state were served by replaying the captured CUDA graph (0 for a context bound to the legacy
  * default stream, which cannot be captured, or while aframe_profile is on). */
 int64_t aframe_stream_graph_replays(const aframe_stream_state* st);
+
+/* 0 if this state runs one full forward of the window per update; else the number of CTAs of the cluster that runs the
+ * incremental network ("snapshotting" taken through the network: windows of consecutive updates share every activation
+ * row that is out of reach of their own zero padding, so an update computes, per layer, only stride / (samples per row) new
+ * rows plus the window's first and last few rows -- at most 48 rows instead of 768 ... 96).  Used when cfg.precision is
+ * AFRAME_F16 with a folded norm, the table is stem conv k7 s2 + ReLU + max-pool k3 s2 p1, k1 / k3 convs, head, cfg.stride is
+ * a multiple of the network's total downsampling (32 for config-1) and at most 128, and cfg.stream_full_forward is 0.
+ * Same roundings as the full forward (fp16 weights, one fp16 rounding per stored activation, fp32 accumulation), another
+ * summation order: scores agree with it to ~1e-3 relative, not bit for bit. */
+int32_t aframe_stream_incremental(const aframe_stream_state* st);
+
+/* Host-only arithmetic (no CUDA call): rows the incremental network computes per update and layer for a weight blob and an
+ * update stride.  For layer i of the blob's table (the head excluded): t_out[i] rows per window, of which the first
+ * head_rows[i] and the last tail_rows[i] are within reach of the window's own zero padding (an output row is such a row iff
+ * it reads padding or such a row of its input), and new_rows[i] = stride / (samples per row) rows enter per update.
+ * *n_layers = 0 if the table or the stride does not qualify (see aframe_stream_incremental); arrays hold max_layers entries. */
+aframe_status aframe_describe_stream_plan(const void* host_blob, size_t bytes, int32_t kernel_len, int32_t n_channels,
+                                          int32_t stride, int32_t max_layers, int32_t* n_layers, int32_t* t_out,
+                                          int32_t* head_rows, int32_t* tail_rows, int32_t* new_rows);
 
 /* Number of kernels the library has launched on this context since creation (for bench accounting). */
 int64_t aframe_launch_count(const aframe_ctx* ctx);

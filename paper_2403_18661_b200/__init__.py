@@ -4,6 +4,6 @@ The product is the C-ABI library declared in include/aframe.h (built from csrc/ 
 libaframe_b200.so); this package is its thin ctypes binding.  No CPU fallback exists.
 """
 from .binding import (  # noqa: F401
-    AframeError, Context, Stream, Weights, aframe_config, default_config, describe_shared_plan, load_library, LIB_PATH, EXPORTS,
+    AframeError, Context, Stream, Weights, aframe_config, default_config, describe_shared_plan, describe_stream_plan, load_library, LIB_PATH, EXPORTS,
     OK, EINVAL, ESHAPE, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED, FP32, BF16, F16,
 )

@@ -33,7 +33,7 @@ class aframe_config(C.Structure):
                 ("n_design", C.c_int32), ("f_lo", C.c_double), ("f_hi", C.c_double),
                 ("kernel_len", C.c_int32), ("stride", C.c_int32), ("psd_len", C.c_int64),
                 ("psd_update", C.c_int64), ("strain_scale_log2", C.c_int32), ("precision", C.c_int32),
-                ("welch_average", C.c_int32), ("reserved_", C.c_int32)]
+                ("welch_average", C.c_int32), ("stream_full_forward", C.c_int32)]
 
 
 class aframe_stage_plan(C.Structure):
@@ -70,6 +70,9 @@ EXPORTS = {
     "aframe_postprocess": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_int32, C.c_int32,
                                      C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]),
     "aframe_stream_graph_replays": (C.c_int64, [C.c_void_p]),
+    "aframe_stream_incremental": (C.c_int32, [C.c_void_p]),
+    "aframe_describe_stream_plan": (C.c_int, [C.c_char_p, C.c_size_t, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int32),
+                                              C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]),
     "aframe_describe_shared_plan": (C.c_int, [C.c_char_p, C.c_size_t, C.c_int32, C.c_int32, C.c_int32, C.c_int64, C.POINTER(C.c_int32),
                                               C.POINTER(aframe_stage_plan), C.c_int32, C.POINTER(C.c_int32)]),
     "aframe_score_timeslides": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_int64,
@@ -117,6 +120,19 @@ def describe_shared_plan(blob: bytes, kernel_len=3072, n_channels=2, window_spac
         out.append(dict(first_layer=a.first_layer, n_layers=a.n_layers, T=a.T, C=a.C, head=a.head, tail=a.tail, packed=bool(a.packed),
                         P=a.P, spare_slots=a.spare_slots, e_head=list(a.e_head[:nl]), e_tail=list(a.e_tail[:nl]), tbox=list(a.tbox[:nl])))
     return s1.value, out
+
+
+def describe_stream_plan(blob: bytes, kernel_len=3072, n_channels=2, stride=128):
+    """aframe_describe_stream_plan (host arithmetic only).  Returns a list of dicts (t_out, head, tail, new) per layer, [] if
+    the table / stride does not qualify for the incremental network."""
+    lib = load_library()
+    n = C.c_int32(0)
+    cap = 256
+    arrs = [(C.c_int32 * cap)() for _ in range(4)]
+    st = lib.aframe_describe_stream_plan(blob, len(blob), int(kernel_len), int(n_channels), int(stride), cap, C.byref(n), *arrs)
+    if st != OK:
+        raise AframeError(st, "aframe_describe_stream_plan")
+    return [dict(t_out=arrs[0][i], head=arrs[1][i], tail=arrs[2][i], new=arrs[3][i]) for i in range(min(n.value, cap))]
 
 
 def default_config(**overrides) -> aframe_config:
@@ -367,6 +383,11 @@ class Stream:
     @property
     def uses_graph(self):
         return int(self.ctx.lib.aframe_stream_graph_replays(self.handle)) > 0
+
+    @property
+    def incremental(self):
+        """CTAs of the cluster that runs the incremental network, 0 = one full forward per update."""
+        return int(self.ctx.lib.aframe_stream_incremental(self.handle))
 
     def step(self, new_samples: torch.Tensor):
         """Enqueue one update; results land in self.score / self.n_scores (device tensors)."""

@@ -3,6 +3,7 @@
 // sequence (and hence one captured CUDA graph) serves every update.
 #include <new>
 #include "common.cuh"
+#include "stream_net.h"
 
 struct aframe_stream_state {
   aframe_ctx* ctx = nullptr;
@@ -20,6 +21,7 @@ struct aframe_stream_state {
   float* d_taps = nullptr;       // [C][L+1]
   float* d_white = nullptr;      // [C][K] newest K whitened samples, oldest first
   float* d_new = nullptr;        // [C][stride]
+  af_stream_net* net = nullptr;  // incremental network (stream_net.cu); null: one full forward per update
   // One update = one CUDA graph launch: the launch sequence is captured the first time a given triple of caller
   // pointers is seen and replayed afterwards (every decision of an update is taken on the device from the counters,
   // so the same graph serves every update).  A caller that alternates between a few buffers keeps one graph per triple
@@ -43,6 +45,8 @@ void af_stream_release(aframe_stream_state* st) {
   for (auto& g : st->graphs) { if (g.exec) cudaGraphExecDestroy(g.exec); g = aframe_stream_state::Graph(); }
   cudaFree(st->blob);
   st->blob = nullptr;
+  af_stream_net_free(st->net);
+  st->net = nullptr;
   cudaGetLastError();
   st->ctx = nullptr; st->w = nullptr;
 }
@@ -120,6 +124,7 @@ static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 AF_API aframe_status aframe_stream_reset(aframe_stream_state* st) {
   if (!st || !st->ctx) return AFRAME_ESTATE;
   AF_CUDA(st->ctx, cudaMemsetAsync(st->blob, 0, st->blob_bytes, st->ctx->stream));
+  if (st->net) return af_stream_net_reset(st->ctx, st->net);
   return AFRAME_OK;
 }
 
@@ -169,12 +174,19 @@ AF_API aframe_status aframe_stream_create(aframe_ctx* ctx, const aframe_weights*
   st->d_taps = reinterpret_cast<float*>(st->blob + o_taps);
   st->d_white = reinterpret_cast<float*>(st->blob + o_w);
   st->d_new = reinterpret_cast<float*>(st->blob + o_new);
-  aframe_status rs = aframe_stream_reset(st);
+  // the incremental network where the configuration allows it (cfg.stream_full_forward = 0, folded tensor-core path, a
+  // stride that is a multiple of the network's total downsampling and at most 128 samples)
+  aframe_status rs = AFRAME_OK;
+  if (!cfg.stream_full_forward) {
+    const char* why = "";
+    rs = af_stream_net_create(ctx, w, &st->net, &why);
+  }
+  if (rs == AFRAME_OK) rs = aframe_stream_reset(st);
   // one untimed forward at B = 1 sizes the activation workspace, builds the tensor maps and sets the
   // kernels' shared-memory attributes, so that aframe_stream_step never allocates (graph capturable)
   float* d_tmp = nullptr;
   if (rs == AFRAME_OK && cudaMalloc(&d_tmp, sizeof(float)) != cudaSuccess) { cudaGetLastError(); rs = AFRAME_ENOMEM; }
-  if (rs == AFRAME_OK) rs = aframe_forward(ctx, w, st->d_white, 1, d_tmp);
+  if (rs == AFRAME_OK && !st->net) rs = aframe_forward(ctx, w, st->d_white, 1, d_tmp);
   if (rs == AFRAME_OK && cudaStreamSynchronize(ctx->stream) != cudaSuccess) rs = af_fail(ctx, AFRAME_ECUDA, "stream warm-up forward failed");
   cudaFree(d_tmp);
   if (rs != AFRAME_OK) { cudaGetLastError(); af_stream_release(st); delete st; return rs; }
@@ -187,6 +199,7 @@ static aframe_status stream_step_enqueue(aframe_ctx* ctx, const float* d_new_sam
                                          float* d_scores, int32_t* d_n_scores);
 
 AF_API int64_t aframe_stream_graph_replays(const aframe_stream_state* st) { return st ? st->replays : 0; }
+AF_API int32_t aframe_stream_incremental(const aframe_stream_state* st) { return st && st->net ? af_stream_net_cluster(st->net) : 0; }
 
 AF_API aframe_status aframe_stream_step(aframe_ctx* ctx, const float* d_new_samples, aframe_stream_state* st,
                                         float* d_scores, int32_t* d_n_scores) {
@@ -260,5 +273,6 @@ static aframe_status stream_step_enqueue(aframe_ctx* ctx, const float* d_new_sam
   AF_LAUNCH_CHECK(ctx);
   stream_slide_kernel<<<1, 1024, 0, ctx->stream>>>(st->d_white, st->d_new, C, K, s, st->d_n, st->d_has_filter, d_n_scores);
   AF_LAUNCH_CHECK(ctx);
+  if (st->net) return af_stream_net_launch(ctx, st->net, st->d_white, st->d_n, st->d_has_filter, d_n_scores, d_scores);
   return aframe_forward(ctx, st->w, st->d_white, 1, d_scores);
 }

@@ -368,3 +368,77 @@ def test_objects_may_be_destroyed_in_any_order_and_graphs_are_kept_per_buffer(af
                 assert e.value.status == af.ESTATE
                 st.close(); ctx.close()
     assert out[1] == out[3] and all(f == 1 for f, _ in out[1])
+
+
+@pytest.mark.parametrize("stride", [128, 64, 32])
+def test_incremental_network_equals_a_full_forward_per_update_and_the_oracle(af, stride):
+    """configs[4] with the incremental network (stream_net.cu: per update and layer only the new stream rows and the window's
+    head / tail rows, one cluster kernel) against (a) the same state running one full forward of the window per update
+    (cfg.stream_full_forward = 1: same fp16 roundings, other summation order) on every scored update, through two PSD updates
+    and a reset, and (b) the float64 oracle (rule T3) on a sample of the updates.  8 s PSD refreshed every 2 s keeps
+    the warm-up short."""
+    fc = full_config()
+    psd_len, psd_update, K = 16384, 4096, fc["kernel_len"]
+    n_updates = (psd_len + K + 2 * psd_update) // stride + 40
+    x = coloured_noise(n_updates * stride, seed=1004)
+    x[0, psd_len + 3000: psd_len + 3400] += 4e-21 * np.sin(np.arange(400) * 0.3)      # something that is not noise
+    blob = make_weight_blob(**fc)
+    upd = torch.from_numpy(np.ascontiguousarray(x.reshape(2, n_updates, stride).transpose(1, 0, 2))).cuda()
+    res = {}
+    stream = torch.cuda.Stream()                                 # (the legacy default stream cannot be captured into a graph)
+    for full in (0, 1):
+        with torch.cuda.stream(stream):
+            ctx = af.Context(precision=af.F16, stride=stride, psd_len=psd_len, psd_update=psd_update, stream_full_forward=full,
+                             stream=stream)
+            w = ctx.load_weights(blob)
+            st = ctx.stream_create(w)
+            assert (st.incremental == 0) == (full == 1) and st.incremental in (0, 8, 16)
+            out = torch.zeros((2, n_updates, 2), dtype=torch.float32, device="cuda")
+            buf = torch.empty((2, stride), dtype=torch.float32, device="cuda")
+            for rep in range(2 if full == 0 else 1):             # the incremental state again after a reset
+                if rep:
+                    st.reset()
+                for u in range(n_updates):
+                    buf.copy_(upd[u], non_blocking=True)
+                    st.step(buf)
+                    out[rep, u, 0].copy_(st.score[0], non_blocking=True)
+                    out[rep, u, 1].copy_(st.n_scores[0], non_blocking=True)
+            stream.synchronize()
+            assert st.uses_graph
+            res[full] = out.cpu().numpy()
+            st.close()
+    inc, ful = res[0], res[1]
+    np.testing.assert_array_equal(inc[0, :, 1], ful[0, :, 1])
+    scored = inc[0, :, 1] == 1
+    np.testing.assert_array_equal(inc[0, :, 1], inc[1, :, 1])    # reset reproduces the run bit for bit
+    np.testing.assert_array_equal(inc[0, scored, 0], inc[1, scored, 0])
+    first = int(np.argmax(scored))
+    assert first == psd_len // stride - 1 + K // stride - 1 and scored[first:].all()
+    assert rel_err(inc[0, scored, 0], ful[0, scored, 0]) <= 2e-3
+    # oracle on every 8th scored update and on the updates around the PSD switches
+    cfg = ost.StreamConfig(stride=stride, psd_len=psd_len, psd_update=psd_update)
+    m0 = ost.first_whitened_index(cfg)
+    picks = sorted(set(range(first, n_updates, 8)) | {u for u in range(first, n_updates) if ((u + 1) * stride) % psd_update < 3 * stride})
+    x64 = x.astype(np.float64)
+    filters = [{}, {}]
+    wins = np.empty((len(picks), 2, K))
+    for j, u in enumerate(picks):
+        a = m0 + (u - first) * stride
+        for c in range(2):
+            wins[j, c], _ = ost.whiten_rolling(x64[c], cfg, m_lo=a, m_hi=a + K, filters=filters[c])
+    want = onet.forward(onet.parse_blob(blob), wins)
+    assert len(picks) >= 20 and rel_err(inc[0, picks, 0], want) <= 2e-2 and rel_err(ful[0, picks, 0], want) <= 2e-2
+
+
+def test_incremental_network_is_not_used_where_it_does_not_apply(af):
+    fc, tc = full_config(), tiny_config()
+    ctx = af.Context(precision=af.F16, stride=512)               # more than 48 rows per layer and update
+    w = ctx.load_weights(make_weight_blob(**fc))
+    st = ctx.stream_create(w)
+    assert st.incremental == 0
+    st.close()
+    ctx = af.Context(n_design=4096, kernel_len=tc["kernel_len"], precision=af.FP32)   # fp32 CUDA-core path
+    w = ctx.load_weights(make_weight_blob(**tc))
+    st = ctx.stream_create(w)
+    assert st.incremental == 0
+    st.close()
