@@ -142,9 +142,10 @@ def test_batched_rfft_and_irfft_of_the_overlap_save_block(af, batch):
     rows = list(range(min(batch, 3))) + ([batch - 1] if batch > 3 else [])
     ref = offt.rfft(x[rows].astype(np.float64))
     scale = np.sqrt(np.mean(np.abs(ref) ** 2))
-    # fp32 transform of 8192 points: 2e-6 of the spectrum's rms, plus one fp32 ulp of the bin itself (the DC bin of row 0
-    # is 3 * 8192 = 2.4e4, whose ulp alone is 2e-3; with one row the rms does not hide it)
-    assert (np.abs(got[rows] - ref) <= 2e-6 * scale + 1.2e-7 * np.abs(ref)).all()
+    # fp32 transform of 8192 points: 2e-6 of the spectrum's rms, plus one fp32 ulp of the row's LARGEST bin (the DC bin of row
+    # 0 is 3 * 8192 = 2.4e4, whose ulp alone is 2e-3, and partial sums of that size pass through the butterflies the Nyquist
+    # bin shares with it: measured 1.1e-3 at DC, 8.9e-4 at Nyquist; with one row the rms does not hide it)
+    assert (np.abs(got[rows] - ref) <= 2e-6 * scale + 1.2e-7 * np.abs(ref).max(axis=-1, keepdims=True)).all()
     back = ctx.irfft8192(spec).cpu().numpy()
     assert np.abs(back - x).max() <= 2e-6 * np.abs(x).max()
     s = (rng.standard_normal((len(rows), 4097)) + 1j * rng.standard_normal((len(rows), 4097)))
