@@ -103,6 +103,19 @@ const char*   aframe_last_error(const aframe_ctx* ctx);   /* ctx may be NULL: re
 aframe_status aframe_psd_welch(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
                                float* d_psd);
 
+/* The same PSD (same kernels, bit-identical result) for callers that may not allocate device memory -- code under CUDA-graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc: the periodogram scratch is a file-scope device array of
+ * aframe_psd_welch_static_max_floats() = 2 * 64 * 2049 floats (1.0 MiB, held by every GPU that loads the library until
+ * the process exits), so the call performs no cudaMalloc / cudaFree and calls no allocating routine.
+ * AFRAME_ESHAPE (with the sizes in aframe_last_error) if n_channels * segments * (welch_nfft / 2 + 1) exceeds that;
+ * AFRAME_ESTATE if the context's device is not the current device.  Arguments as aframe_psd_welch.
+ * The array is shared by every call, context and stream on the device and keeps the last call's contents (nothing in it has
+ * to start at zero: a call writes every periodogram before it reads it); calls that overlap on the GPU race on it, so
+ * serialise them (one stream, or events between streams). */
+aframe_status aframe_psd_welch_static(aframe_ctx* ctx, const float* d_strain, int64_t n_samples, int64_t ld,
+                                      float* d_psd);
+int64_t       aframe_psd_welch_static_max_floats(void);
+
 /* ---- O-2/O-3  filter design + whitening (readings A3-A6) -----------------------------
  * Designs the L-tap zero-phase FIR whitening filter from d_psd (as returned by aframe_psd_welch) and
  * applies it to a contiguous segment by FFT overlap-save.  Output has n_samples - filter_len samples

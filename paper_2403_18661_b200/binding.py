@@ -48,6 +48,8 @@ EXPORTS = {
     "aframe_destroy": (None, [C.c_void_p]),
     "aframe_last_error": (C.c_char_p, [C.c_void_p]),
     "aframe_psd_welch": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]),
+    "aframe_psd_welch_static": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]),
+    "aframe_psd_welch_static_max_floats": (C.c_int64, []),
     "aframe_whiten": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_int64, C.c_int]),
     "aframe_filter_taps": (C.c_int, [C.c_void_p, C.c_void_p]),
     "aframe_rfft8192": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]),
@@ -215,6 +217,16 @@ class Context:
         if out is None:
             out = torch.empty((c, self.n_freq), dtype=torch.float32, device=strain.device)
         self._check(self.lib.aframe_psd_welch(self.handle, _ptr(strain), n, strain.stride(0), _ptr(out)))
+        return out
+
+    def psd_welch_static(self, strain: torch.Tensor, out: torch.Tensor):
+        """aframe_psd_welch_static: the same PSD with its scratch in a fixed device array (the call allocates nothing, so
+        `out` is the caller's)."""
+        _need(strain, torch.float32, "strain"); _need(out, torch.float32, "out")
+        c, n = strain.shape
+        if tuple(out.shape) != (c, self.n_freq) or not out.is_contiguous():
+            raise ValueError("out must be a contiguous [C][welch_nfft / 2 + 1] tensor")
+        self._check(self.lib.aframe_psd_welch_static(self.handle, _ptr(strain), n, strain.stride(0), _ptr(out)))
         return out
 
     # ---- O-2 / O-3

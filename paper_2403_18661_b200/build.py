@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libaframe_b200.so")
-SOURCES = ["aframe_api.cu", "signal_kernels.cu", "signal_fft64.cu", "net_fp32.cu", "stem_bf16.cu", "gn_bf16.cu", "conv_tc.cu", "stream.cu", "stream_net.cu", "postprocess.cu"]
+SOURCES = ["aframe_api.cu", "signal_kernels.cu", "signal_fft64.cu", "net_fp32.cu", "stem_bf16.cu", "gn_bf16.cu", "conv_tc.cu", "stream.cu", "stream_net.cu", "postprocess.cu", "psd_static.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
