@@ -448,6 +448,10 @@ def latency_run(af, torch, ctx_stream, weights_blob, n_updates, n_warm_scored=10
            "mean_ms": float(wall.mean()), "timing": "host wall-clock: pinned H2D of the update + aframe_stream_step + "
            "D2H of the score + stream sync; device: CUDA events around aframe_stream_step",
            "graph": bool(getattr(st, "uses_graph", False)),
+           "incremental_network": {"cluster_ctas": int(st.incremental),
+                                   "what": "0 = one full forward of the window per update; else the update computes, per layer, only "
+                                           "the new stream rows and the window's head / tail rows (<= 48 rows) in one cluster kernel "
+                                           "(stream_net.cu); the graph then holds 7 kernels instead of 40"},
            "realtime_factor": float((stride / FS) / (wall.mean() * 1e-3))}
     st.close(); w.free(); ctx.close()
     return out

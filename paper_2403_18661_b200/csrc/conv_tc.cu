@@ -208,6 +208,7 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   L.macs = (double)(cg2 ? 2 * ((m_tiles + 1) / 2) : m_tiles) * 128.0 * l.c_out * 64.0 * (l.k * (l.c_in / 64) + (sc >= 0 ? w->layers[sc].c_in / 64 : 0));
   p.div_n = tc_fastdiv((uint32_t)p.n_tiles);
   p.div_t = tc_fastdiv((uint32_t)p.t_blks);
+  p.div_tbox = tc_fastdiv((uint32_t)T_box);
   // true GroupNorm (NEXT-2): the conv stores its plain output; norm, residual and ReLU follow in af_launch_gn_bf16
   p.relu = w->live_gn ? 0 : l.relu; p.has_res = res != nullptr;
   p.c_out = l.c_out;

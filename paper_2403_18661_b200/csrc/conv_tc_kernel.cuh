@@ -42,6 +42,7 @@ static inline TcFastDiv tc_fastdiv(uint32_t d) {
 struct TcConvParams {
   const float* bias;
   TcFastDiv div_n, div_t;    // by n_tiles and by t_blks
+  TcFastDiv div_tbox;        // by T_box
   int tap_toff[3], tap_par[3];   // per tap: row offset and parity plane of the strided input view
   int taps, pad, P;          // kernel taps, left padding, stride
   int kblocks;               // C_in / 64
@@ -127,7 +128,13 @@ template <int BN, bool CG2 = false> struct TcCfg {
   static constexpr int EPW = CG2 ? 2 : 1;
   static constexpr int EPI_COLS = 64 / EPW;          // accumulator columns per epilogue thread and chunk
   static constexpr int GROUP_THREADS = 128 * EPW;
-  static constexpr int THREADS = 64 + GROUP_THREADS * EG;
+  // CTA pairs: one more warp per epilogue group whose only job is that group's TMA traffic (stores of staged chunks, residual
+  // prefetch).  With the group's leader thread doing it, 255 threads waited at a named barrier per chunk while one thread
+  // waited for the previous store to be read (~900 cycles), decoded the next tile and issued the residual load, and again
+  // while it issued the store (~500): profiles/r02_conv_cycles.md.  The store warp and the epilogue threads meet only at
+  // mbarriers ("staged": 256 arrivals after the chunk is written; "ready": the buffer is free again / its residual landed).
+  static constexpr int STORE_WARPS = CG2 ? EG : 0;
+  static constexpr int THREADS = 64 + GROUP_THREADS * EG + 32 * STORE_WARPS;
   static constexpr int smem(int stages, int nbuf, bool head) {
     return tc_fixed_bytes(head) + stages * STAGE_BYTES + EG * nbuf * TC_OUT_BYTES;
   }
@@ -238,6 +245,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
   auto res_bar = [&](int g, int b) { return base + 8u * (2 * STAGES + 2 * NACC + g * MAXBUF + b); };
   const uint32_t w_bar = base + 8u * (2 * STAGES + 2 * NACC + EG * MAXBUF);
   const uint32_t tmem_slot = w_bar + 8u;
+  auto staged_bar = [&](int g, int b) { return tmem_slot + 8u + 8u * (g * MAXBUF + b); };
+  constexpr bool STW = CG2 && !HEAD;               // epilogue groups served by store warps (see TcCfg::STORE_WARPS)
   float* s_bias = reinterpret_cast<float*>(gen_base + TC_BAR_BYTES);
   float* s_headw = reinterpret_cast<float*>(gen_base + 3072);
   static_assert(!HALO || (!CG2 && !HEAD), "HALO is a single-CTA, storing variant");
@@ -258,7 +267,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     }
     mbar_init(w_bar, 1);
     for (int g = 0; g < EG; ++g)
-      for (int b = 0; b < MAXBUF; ++b) mbar_init(res_bar(g, b), 1);
+      for (int b = 0; b < MAXBUF; ++b) { mbar_init(res_bar(g, b), 1); mbar_init(staged_bar(g, b), Cfg::GROUP_THREADS); }
     if (p.has_res || p.sc_kblocks) tma_prefetch_desc(&tm_res);
     if (p.sc_kblocks) tma_prefetch_desc(&tm_scw);
     fence_mbar_init();
@@ -495,6 +504,57 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       if (!HALO && !HEAD && p1.num_tiles > 0) issue(p1);
       if (lane == 0) Tflush(1);
     }
+  } else if (warp >= 2 + 4 * Cfg::EPW * EG) {
+    // ===== store warp of epilogue group g: lane 0 walks the group's (tile, chunk) sequence over both problems =====
+    // (the fused-head variant stores nothing: its store warps are idle)
+    const int g = warp - (2 + 4 * Cfg::EPW * EG);
+    if (STW && lane == 0) {
+      const int NBUF = p.nbuf > 0 ? p.nbuf : 1;
+      const uint32_t gbuf = out_base + (uint32_t)(g * NBUF) * TC_OUT_BYTES;
+      constexpr int CH = BN / 64;
+      struct Cur { int prob, tile, c; };
+      auto settle = [&](Cur& k) {                  // first valid item at or after k (prob = 2: past the end)
+        while (k.prob < 2) {
+          const TcConvParams& P = k.prob ? p1 : p;
+          if (k.tile < P.num_tiles) return;
+          ++k.prob; k.tile = worker; k.c = g;
+        }
+      };
+      auto next = [&](Cur& k) {
+        k.c += 2;
+        if (k.c >= CH) { k.c = g; k.tile += n_workers; }
+        settle(k);
+      };
+      // buffer `buf` may be written for item k: its residual tile is on its way, or (no residual) it is simply free
+      auto signal_ready = [&](const Cur& k, int buf) {
+        if (k.prob >= 2) return;
+        const TcConvParams& P = k.prob ? p1 : p;
+        if (P.has_res) {
+          int n_idx, t0, b0;
+          decode(P, k.tile, n_idx, t0, b0);
+          mbar_arrive_expect_tx(res_bar(g, buf), P.a_bytes);
+          tma_load_4d(gbuf + buf * TC_OUT_BYTES, k.prob ? &tm_res1 : &tm_res, res_bar(g, buf), n_idx * BN + k.c * 64, 0, t0, b0);
+        } else {
+          mbar_arrive(res_bar(g, buf));
+        }
+      };
+      Cur S = {0, worker, g}, A = {0, worker, g};
+      settle(S); settle(A);
+      for (int i = 0; i < NBUF; ++i) { signal_ready(A, i); next(A); }
+      for (uint32_t j = 0; S.prob < 2; ++j) {
+        const int buf = j % NBUF;
+        mbar_wait(staged_bar(g, buf), (j / NBUF) & 1u);
+        const TcConvParams& P = S.prob ? p1 : p;
+        int n_idx, t0, b0;
+        decode(P, S.tile, n_idx, t0, b0);
+        tma_store_4d(S.prob ? &tm_out1 : &tm_out, gbuf + buf * TC_OUT_BYTES, n_idx * BN + S.c * 64, 0, t0, b0);
+        tma_store_commit();
+        tma_store_wait_read_n(0);                  // the buffer has been read: item j + NBUF may have it
+        signal_ready(A, buf);
+        next(A); next(S);
+      }
+      tma_store_wait_all<0>();
+    }
   } else {
     // ===== epilogue: EG groups of 4 warps, thread <-> one output row =====
     constexpr int EPW = Cfg::EPW, GT = Cfg::GROUP_THREADS, EC = Cfg::EPI_COLS;
@@ -524,8 +584,10 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       named_bar_sync(3, GT * EG);
       for (int i = (int)threadIdx.x - 64; i < p.c_out; i += GT * EG) s_bias[i] = p.bias[i];
       named_bar_sync(3, GT * EG);
-      if (leader) tma_store_wait_read_n(0);
+      if (!STW && leader) tma_store_wait_read_n(0);
     }
+    int row_bq, row_tq;                            // this thread's row inside the tile's box
+    p.div_tbox.divmod(row, row_bq, row_tq);
     // residual prefetch cursor (leader only): item pf_j of this group's (tile, chunk) sequence; the residual tile lands
     // in the staging buffer the chunk's output will be written to (added in place)
     int pf_tile = tile_first, pf_c = c_first;
@@ -542,17 +604,17 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       pf_c += C_STEP;
       if (pf_c >= CH) { pf_c = c_first; pf_tile += tile_step; }
     };
-    if (leader && p.has_res)
+    if (!STW && leader && p.has_res)
       for (int i = 0; i < PF; ++i) issue_res();
 
     // packed edge batch: this thread's row of tile (n0_, t0_, b0_) is taken from the stream if it is one of the two rows next to
     // the window's edge rows (the only interior rows a later layer reads): pointer to its first channel of the tile, else null
     auto copy_base = [&](int n0_, int t0_, int b0_) -> const uint4* {
       if (HEAD || p.edge_nbp == 0 || p.edge_stream == nullptr || row >= p.T_box * p.B_box) return nullptr;
-      const int m = b0_ + row / p.T_box;           // short-window slot
+      const int m = b0_ + row_bq;                  // short-window slot
       const bool is_tail = m >= p.edge_nbp;
       const int b = is_tail ? m - p.edge_nbp : m;
-      const int t_win = (is_tail ? p.edge_T - p.edge_P : 0) + t0_ + row % p.T_box;
+      const int t_win = (is_tail ? p.edge_T - p.edge_P : 0) + t0_ + row_tq;
       const int d = is_tail ? p.edge_T - p.edge_tail - 1 - t_win : t_win - p.edge_head;   // 0, 1: the two rows past the edge
       if (d < 0 || d > 1 || b >= p.nb) return nullptr;
       return p.edge_stream + (((long long)b * p.edge_shift + t_win) * p.c_out + n0_) / 8;
@@ -586,6 +648,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       for (int c = c_first; c < CH; c += C_STEP, ++j) {
         const int buf = j % NBUF;
         const uint32_t sbuf = gbuf + buf * TC_OUT_BYTES;
+        if (!STW) {
         if (leader) {
           if (p.has_res) {
             if (!HEAD) tma_store_wait_read_n(NBUF - PF - 1);   // buffer of chunk j + PF is free again
@@ -596,6 +659,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         }
         T(2);
         named_bar_sync(1 + g, GT);
+        }
         T(3);
         uint32_t v[EC];
         const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN + c * 64 + hf * EC);
@@ -625,7 +689,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             }
           }
         }
-        if (p.has_res) {                           // (own parity per buffer: with two problems not every chunk has a residual)
+        if (STW) {                                 // the store warp: this chunk's buffer is free, its residual (if any) has landed
+          mbar_wait(res_bar(g, buf), (j / NBUF) & 1u);
+        } else if (p.has_res) {                    // (own parity per buffer: with two problems not every chunk has a residual)
           mbar_wait(res_bar(g, buf), (res_par >> buf) & 1u);
           res_par ^= 1u << buf;
         }
@@ -635,7 +701,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         unsigned char* rowp = gen_base + (sbuf - base) + row * 128;
         // straight-line code per variant (no run-time branches inside the unrolled loop, so the 8 pieces interleave)
         const __half2 lo2 = __float2half2_rn(p.relu ? 0.f : -INFINITY);
-        const int t_row = t0 + row % p.T_box;
+        const int t_row = t0 + row_tq;
         const bool zero_row = p.zero_period > 0 && t_row >= p.zero_origin - 2 &&
                               ((t_row - p.zero_origin + p.zero_period) % p.zero_period) >= p.zero_valid;
         const uint4* copy_row = copy_tile != nullptr ? copy_tile + c * 8 : nullptr;
@@ -672,10 +738,14 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         } else {
           T(6);
           fence_proxy_async_smem();                // generic-proxy writes -> visible to the TMA store
+          if (STW) {
+            mbar_arrive(staged_bar(g, buf));       // the store warp takes it from here
+          } else {
           named_bar_sync(1 + g, GT);
           if (leader) {
             tma_store_4d(&tm_out, sbuf, n0 + c * 64, 0, t0, b0);
             tma_store_commit();
+          }
           }
           T(7);
         }
@@ -685,7 +755,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     drain(tm_out, tm_res, p, false);
     if (!HALO && !HEAD && p1.num_tiles > 0) drain(tm_out1, tm_res1, p1, true);
     if (leader) Tflush(2 + g);
-    if (leader && !HEAD) tma_store_wait_all<0>();
+    if (!STW && leader && !HEAD) tma_store_wait_all<0>();
   }
   tc_fence_before();
   __syncthreads();

@@ -64,36 +64,56 @@ __global__ void stream_ingest_kernel(const float* __restrict__ fresh, int C, int
 }
 
 // The `stride` newest whitened samples m in [n - s - L/2, n - L/2) by direct summation of the L-1 taps
-// (0.52 MMAC per update).  One warp per output sample.
+// (0.52 MMAC per update).  One CTA = FIR_NO consecutive outputs of one channel: the L - 2 + FIR_NO ring samples they
+// touch and the taps are staged in shared memory once (ring wrap handled while staging, by a conditional subtract: the
+// first version took a 64-bit modulo per tap and cost 36 us of the update), then each warp sums FIR_NO / 8 outputs,
+// lane-strided over the taps.
+constexpr int FIR_NO = 16;
 __global__ void __launch_bounds__(256)
 stream_fir_kernel(const float* __restrict__ raw, int64_t ring_len, const float* __restrict__ taps, int L, int stride,
                   float scale, const int64_t* __restrict__ d_n, const int* __restrict__ d_has_filter,
                   float* __restrict__ fresh_white) {
   if (*d_has_filter == 0) return;
+  extern __shared__ float fir_smem[];              // [L + 1] taps, then [L - 2 + FIR_NO] samples
+  float* hs = fir_smem;
+  float* xs = fir_smem + (L + 1);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int o = blockIdx.x * 8 + warp;
-  if (o >= stride) return;
+  const int o0 = blockIdx.x * FIR_NO;
   const int c = blockIdx.y;
   const int half = L / 2;
   const int64_t n = d_n[0];
-  const int64_t m = n - stride - half + o;
+  // y[m] = sum_{i = 1}^{L - 1} h[i] x[m + half - i]; outputs m0 + o, o = o0 .. o0 + FIR_NO - 1, read samples
+  // m0 + o0 + half - (L - 1) ... m0 + o0 + FIR_NO - 1 + half - 1: xs[k] = x[first + k]
+  const int64_t m0 = n - stride - half;
+  const int64_t first = m0 + o0 + half - (L - 1);
+  const int n_x = L - 2 + FIR_NO;
   const float* x = raw + (int64_t)c * ring_len;
   const float* h = taps + (int64_t)c * (L + 1);
-  float acc0 = 0.f, acc1 = 0.f;
-  // y[m] = sum_j h[j] x[m - j], j = -(half-1)..half-1 ; tap array index i = j + half, sample m + half - i
-  for (int i = 1 + lane; i < L; i += 64) {
-    int64_t p0 = (m + half - i) % ring_len;
-    acc0 = fmaf(h[i], x[p0] * scale, acc0);
-    const int i1 = i + 32;
-    if (i1 < L) {
-      int64_t p1 = (m + half - i1) % ring_len;
-      acc1 = fmaf(h[i1], x[p1] * scale, acc1);
-    }
+  int64_t p0 = first % ring_len;                    // (one modulo per thread; first >= 0 once a filter exists: n >= psd_len >= stride + L)
+  if (p0 < 0) p0 += ring_len;
+  for (int k = threadIdx.x; k < n_x; k += 256) {
+    int64_t q = p0 + k;
+    if (q >= ring_len) q -= ring_len;
+    xs[k] = x[q] * scale;
   }
-  float acc = acc0 + acc1;
+  for (int k = threadIdx.x; k <= L; k += 256) hs[k] = h[k];
+  __syncthreads();
+  for (int oo = warp; oo < FIR_NO; oo += 8) {
+    const int o = o0 + oo;
+    if (o >= stride) break;
+    // sample of tap i for output oo: x[m0 + o + half - i] = xs[oo + (L - 1) - i]
+    float acc0 = 0.f, acc1 = 0.f;
+    const float* xo = xs + oo + (L - 1);
+    for (int i = 1 + lane; i < L; i += 64) {
+      acc0 = fmaf(hs[i], xo[-i], acc0);
+      const int i1 = i + 32;
+      if (i1 < L) acc1 = fmaf(hs[i1], xo[-i1], acc1);
+    }
+    float acc = acc0 + acc1;
 #pragma unroll
-  for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
-  if (lane == 0) fresh_white[c * stride + o] = acc;
+    for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+    if (lane == 0) fresh_white[c * stride + o] = acc;
+  }
 }
 
 // Slide the whitened window by `stride` and append the fresh samples.  One CTA (read all, sync, write).
@@ -268,7 +288,7 @@ static aframe_status stream_step_enqueue(aframe_ctx* ctx, const float* d_new_sam
   rs = af_launch_filter_design(ctx, st->d_psd, 1, st->d_H, st->d_taps, &gate);
   if (rs != AFRAME_OK) return rs;
   const float scale = ldexpf(1.0f, cfg.strain_scale_log2);
-  stream_fir_kernel<<<dim3((unsigned)((s + 7) / 8), (unsigned)C), 256, 0, ctx->stream>>>(
+  stream_fir_kernel<<<dim3((unsigned)((s + FIR_NO - 1) / FIR_NO), (unsigned)C), 256, sizeof(float) * (2 * L - 1 + FIR_NO), ctx->stream>>>(
       st->d_raw, st->ring_len, st->d_taps, L, s, scale, st->d_n, st->d_has_filter, st->d_new);
   AF_LAUNCH_CHECK(ctx);
   stream_slide_kernel<<<1, 1024, 0, ctx->stream>>>(st->d_white, st->d_new, C, K, s, st->d_n, st->d_has_filter, d_n_scores);
