@@ -36,6 +36,7 @@ constexpr int SN_PD = 12;                         // weight-fragment copies (pai
 constexpr int SN_PART_BYTES = SN_WARPS * SN_MAX_MT * 128 * 4;    // partial sums of the 16 warps
 constexpr int SN_WBUF_BYTES = SN_WARPS * SN_PD * 512;            // weight fragments in flight
 constexpr int SN_RES_BYTES = SN_THREADS * 16;                    // one residual piece per epilogue thread
+constexpr int SN_BIAS_BYTES = SN_WARPS * 8 * 4;                  // the folded bias of this CTA's output blocks
 constexpr int SN_GP = 8;                          // 16-byte pieces of the input rows per thread
 
 struct SnLayer {
@@ -154,7 +155,8 @@ __global__ void __launch_bounds__(SN_THREADS, 1) stream_net_kernel(const SnParam
   // copies cannot be sunk to their first use by the compiler, which is what happened to plain loads held in registers)
   uint4* wbuf = reinterpret_cast<uint4*>(sn_smem + SN_PART_BYTES) + warp * (SN_PD * 32) + lane;
   uint4* res_buf = reinterpret_cast<uint4*>(sn_smem + SN_PART_BYTES + SN_WBUF_BYTES);
-  unsigned char* in_tile = sn_smem + SN_PART_BYTES + SN_WBUF_BYTES + SN_RES_BYTES;
+  float* bias_buf = reinterpret_cast<float*>(sn_smem + SN_PART_BYTES + SN_WBUF_BYTES + SN_RES_BYTES);
+  unsigned char* in_tile = sn_smem + SN_PART_BYTES + SN_WBUF_BYTES + SN_RES_BYTES + SN_BIAS_BYTES;
   auto sn_prefetch = [&](int li) {
     if (li >= p.n_layers || s_layers[li].kind != 0) { sn_cp_async_commit(); return; }   // (an empty group: the epilogue counts groups)
     int np;
@@ -232,6 +234,8 @@ __global__ void __launch_bounds__(SN_THREADS, 1) stream_net_kernel(const SnParam
       sn_cp_async16(sn_smem_u32(res_buf + tid),
                     reinterpret_cast<const uint4*>(sn_row(Lr, p.arena, sn_out_row(L, m), upd * Lr.nnew)) + (rank + i * CL));
     }
+    if (tid < 2 * nbl)                             // ... and the bias of this CTA's blocks (block i = tid / 2: channels 8 (rank + i CL) ...)
+      sn_cp_async16(sn_smem_u32(bias_buf + 4 * tid), L.bias + (rank + (tid >> 1) * CL) * 8 + 4 * (tid & 1));
     sn_cp_async_commit();
 
     // gather the input rows (16-byte pieces; rows padded by 16 B: conflict-free ldmatrix)
@@ -311,20 +315,20 @@ __global__ void __launch_bounds__(SN_THREADS, 1) stream_net_kernel(const SnParam
     for (int mt = 0; mt < SN_MAX_MT; ++mt)
 #pragma unroll
       for (int j = 0; j < 4; ++j) part[((warp * SN_MAX_MT + mt) * 4 + j) * 32 + lane] = acc[mt][j];
+    sn_cp_async_wait_all();                        // this thread's residual / bias pieces have landed; after the barrier everyone's
     __syncthreads();
     SN_T(li, 2);
     sn_prefetch(li + 1);                           // the next layer's first weight fragments travel during the epilogue and the barrier
 
     // epilogue: one thread per (output row, output block): sum the K chunks in order, + bias (+ residual) -> fp16 -> ReLU
     {
-      sn_cp_async_wait_1();                        // the residual pieces have landed (the next layer's weights may still travel)
       for (int it = tid; it < n_epi; it += SN_THREADS) {
         const int m = it / nbl, i = it - m * nbl;
         const int nbo = rank + i * CL;
         const int mt = m >> 4, rr = m & 15;
         float v[8];
         {
-          const float4 b0 = __ldg(reinterpret_cast<const float4*>(L.bias + nbo * 8)), b1 = __ldg(reinterpret_cast<const float4*>(L.bias + nbo * 8) + 1);
+          const float4 b0 = reinterpret_cast<const float4*>(bias_buf)[2 * i], b1 = reinterpret_cast<const float4*>(bias_buf)[2 * i + 1];
           v[0] = b0.x; v[1] = b0.y; v[2] = b0.z; v[3] = b0.w; v[4] = b1.x; v[5] = b1.y; v[6] = b1.z; v[7] = b1.w;
         }
         // accumulator fragment of m16n8: lane = (row % 8) * 4 + col / 2, register = (row / 8) * 2 + col % 2
@@ -546,7 +550,7 @@ aframe_status af_stream_net_create(aframe_ctx* ctx, const aframe_weights* w, af_
     arena = (arena + 63) & ~63ll;
     sn->layers.push_back(L);
   }
-  sn->smem_bytes = SN_PART_BYTES + SN_WBUF_BYTES + SN_RES_BYTES + smem_in_max;
+  sn->smem_bytes = SN_PART_BYTES + SN_WBUF_BYTES + SN_RES_BYTES + SN_BIAS_BYTES + smem_in_max;
   if (sn->smem_bytes > 200 * 1024) { delete sn; *why = "input rows do not fit shared memory"; return AFRAME_OK; }
   cudaError_t ce = cudaFuncSetAttribute(stream_net_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sn->smem_bytes);
   if (ce == cudaSuccess) ce = cudaFuncSetAttribute(stream_net_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
