@@ -521,21 +521,33 @@ __global__ void __launch_bounds__(256)
 sh_head_rows_kernel(const float* __restrict__ Rs, int64_t rows_s, const float* __restrict__ Re, int64_t rows_e,
                     float* __restrict__ head_part, int64_t nb, int T, int chunks, int64_t row_shift, int c_head, int c_tail,
                     int64_t e_stride, int64_t e_tail0, int e_trow) {
+  // one warp per (window, slab), lane = row; the head units are walked in a loop (one 32-bit division per warp instead of
+  // three 64-bit ones per (window, slab, unit): the first version was bound by them)
   const int lane = threadIdx.x & 31;
   const int slabs = T / 32;
-  const int64_t wi = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
-  if (wi >= nb * slabs * chunks) return;
-  const int c = (int)(wi % chunks);
-  const int slab = (int)((wi / chunks) % slabs);
-  const int64_t b = wi / ((int64_t)chunks * slabs);
+  const unsigned wi = blockIdx.x * 8u + (threadIdx.x >> 5);
+  if (wi >= (unsigned)(nb * slabs)) return;
+  const unsigned b = wi / (unsigned)slabs;
+  const int slab = (int)(wi - b * (unsigned)slabs);
   const int t = slab * 32 + lane;
-  float sum;
-  if (t < c_head) sum = Re[c * rows_e + b * e_stride + t];
-  else if (t >= T - c_tail) sum = Re[c * rows_e + e_tail0 + b * e_stride + (t - e_trow)];
-  else sum = Rs[c * rows_s + b * row_shift + t];
+  const float* src;
+  int64_t unit_stride;
+  if (t < c_head) { src = Re + (int64_t)b * e_stride + t; unit_stride = rows_e; }
+  else if (t >= T - c_tail) { src = Re + e_tail0 + (int64_t)b * e_stride + (t - e_trow); unit_stride = rows_e; }
+  else { src = Rs + (int64_t)b * row_shift + t; unit_stride = rows_s; }
+  float* dst = head_part + ((int64_t)b * slabs + slab) * chunks;
+  for (int c0 = 0; c0 < chunks; c0 += 4) {         // four units in flight
+    float v[4];
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-  if (lane == 0) head_part[(b * slabs + slab) * chunks + c] = sum;
+    for (int k = 0; k < 4; ++k) v[k] = c0 + k < chunks ? __ldg(src + (c0 + k) * unit_stride) : 0.f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      float sum = v[k];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+      if (lane == 0 && c0 + k < chunks) dst[c0 + k] = sum;
+    }
+  }
 }
 
 struct TcPlanCache {
@@ -1111,7 +1123,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         if (g + 1 == pc->sh.size() && pc->sh_head && pc->sh_head_rows) {
           const int q_last = (int)P.layers.size() - 1;
           const int hu = P.C / TcCfg<256, true>::EPI_COLS;          // head units per row
-          const int64_t n_warps = nb * (P.T / 32) * hu;
+          const int64_t n_warps = nb * (P.T / 32);
           const float* hr_s = reinterpret_cast<const float*>(sh_buf((int)g, 0, q_last));
           aux_begin();
           sh_head_rows_kernel<<<(unsigned)((n_warps + 7) / 8), 256, 0, ctx->stream>>>(
