@@ -607,6 +607,22 @@ def run_ours(args):
         "stages_pass": {"ms_per_step": ms_profiled / args.steps,
                         "note": "second pass over the same steps with the library's per-stage CUDA events on its stream"},
     }
+    # Of the executed MACs, which ones does the method need at all?  Per window and layer: the rows that enter with a new
+    # window (128 / samples per row) plus the window's own head and tail rows (those within reach of its zero padding), from the
+    # library's host-side row plan (aframe_describe_stream_plan: the same identity, per update instead of per window).  The
+    # rest of the executed MACs are whole-tile padding, box rows computed and replaced, and separator rows.
+    try:
+        from synthdata import full_config as _fc
+        _plan = af.describe_stream_plan(blob, kernel_len=KERNEL, stride=STRIDE)
+        _tab = _fc()["table"]
+        useful = sum((r["new"] + r["head"] + r["tail"]) * l.k * l.c_in * l.c_out
+                     for i, (r, l) in enumerate(zip(_plan, _tab)) if i >= 2)
+        out["roofline"]["useful_mmac_per_window"] = useful / 1e6
+        out["roofline"]["useful_frac_of_executed"] = useful / mmac_exec if mmac_exec > 0 else None
+        out["roofline"]["useful_tflops"] = exec_tflops * useful / mmac_exec if mmac_exec > 0 else None
+    except Exception as e:                                       # (a table the incremental plan does not cover)
+        out["roofline"]["useful_frac_of_executed"] = None
+        out["roofline"]["useful_note"] = repr(e)
     if "conv_dram_bytes_per_launch" in ncu:
         out["roofline"]["traffic"], out["roofline"]["traffic_source"] = ncu["conv_dram_bytes_per_launch"]
     wh_ms = stages["whiten"][0]
