@@ -646,7 +646,7 @@ def run_ours(args):
     if st_ms > 0:
         # shared stem: per 4096-window chunk the stem runs once over the chunk's stream (64 new conv positions per window)
         # plus 7 conv positions per window for the three edge rows; each position is 64 channels x 14 MACs
-        chunk = 4096
+        chunk = args.batch
         n_chunks = args.steps * N_SLIDES * (-(-n_win // chunk))
         pos = args.steps * N_SLIDES * ((n_win - (-(-n_win // chunk))) * 64 + (-(-n_win // chunk)) * 1536 + 7 * n_win)
         tf = 2.0 * 64 * 14 * pos / (st_ms * 1e-3) / 1e12
@@ -654,7 +654,7 @@ def run_ours(args):
                                 "peak": 148 * 128 * 2 * 1.965e9 / 1e12, "unit": "TFLOP/s fp32",
                                 "frac": tf / (148 * 128 * 2 * 1.965e9 / 1e12), "launches": int(2 * n_chunks),
                                 "algorithmic": "overlapping windows share their stem: 71 conv positions (64 new + 7 edge) x 64 channels x "
-                                               "14 MACs per window instead of 1536; two ~15 us launches per 4096 windows, so this "
+                                               "14 MACs per window instead of 1536; two ~15 us launches per launch sequence, so this "
                                                "stage is launch-bound and 0.5 % of the step (per-window kernel at 4096 windows: "
                                                "profiles/r01d_stem_full.md, 50 % of the FFMA peak)"}
     we_ms = stages["welch"][0]

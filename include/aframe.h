@@ -77,7 +77,9 @@ typedef struct {
   int32_t  welch_average;     /* 0 = mean over segments (reading A1, default); 1 = per-bin median
                                  divided by its bias for n segments (NEXT-3 variant; n <= 255)   */
   int32_t  stream_full_forward; /* aframe_stream_step: 0 (default) = the incremental network where the configuration
-                                 allows it (see aframe_stream_incremental); 1 = one full forward of the window per update */
+                                 allows it (see aframe_stream_incremental), on a cluster of 16 CTAs if the device can place
+                                 one, else 8; 1 = one full forward of the window per update; 2 = the incremental network on
+                                 the portable cluster size 8 */
 } aframe_config;
 
 typedef struct aframe_ctx aframe_ctx;

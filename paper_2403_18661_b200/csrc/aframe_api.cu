@@ -70,7 +70,7 @@ AF_API aframe_status aframe_create(const aframe_config* cfg, void* cuda_stream, 
   if (cfg->strain_scale_log2 < -120 || cfg->strain_scale_log2 > 120) return AFRAME_EINVAL;
   if (cfg->precision == AFRAME_BF16) return AFRAME_EUNSUPPORTED;   // bf16 storage cannot meet the rank tolerance (aframe.h)
   if (cfg->precision != AFRAME_FP32 && cfg->precision != AFRAME_F16) return AFRAME_EINVAL;
-  if ((cfg->welch_average != 0 && cfg->welch_average != 1) || (cfg->stream_full_forward != 0 && cfg->stream_full_forward != 1)) return AFRAME_EINVAL;
+  if ((cfg->welch_average != 0 && cfg->welch_average != 1) || cfg->stream_full_forward < 0 || cfg->stream_full_forward > 2) return AFRAME_EINVAL;
   if (cfg->welch_average == 1 && (cfg->psd_len - cfg->welch_nfft) / cfg->welch_hop + 1 > 255) return AFRAME_EUNSUPPORTED;
 
   int dev = 0;

@@ -197,7 +197,7 @@ AF_API aframe_status aframe_stream_create(aframe_ctx* ctx, const aframe_weights*
   // the incremental network where the configuration allows it (cfg.stream_full_forward = 0, folded tensor-core path, a
   // stride that is a multiple of the network's total downsampling and at most 128 samples)
   aframe_status rs = AFRAME_OK;
-  if (!cfg.stream_full_forward) {
+  if (cfg.stream_full_forward != 1) {
     const char* why = "";
     rs = af_stream_net_create(ctx, w, &st->net, &why);
   }

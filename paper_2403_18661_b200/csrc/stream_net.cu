@@ -565,7 +565,7 @@ aframe_status af_stream_net_create(aframe_ctx* ctx, const aframe_weights* w, af_
     at.val.clusterDim.x = 16; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
     lc.attrs = &at; lc.numAttrs = 1;
     int n_cl = 0;
-    if (cudaOccupancyMaxActiveClusters(&n_cl, stream_net_kernel, &lc) == cudaSuccess && n_cl >= 1) sn->cluster = 16;
+    if (cfg.stream_full_forward != 2 && cudaOccupancyMaxActiveClusters(&n_cl, stream_net_kernel, &lc) == cudaSuccess && n_cl >= 1) sn->cluster = 16;
     cudaGetLastError();
   }
   // work split per layer: the CTA with the most output blocks has nbl_max of them; its 16 warps take (block, K chunk)
