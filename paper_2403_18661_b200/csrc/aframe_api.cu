@@ -257,7 +257,7 @@ AF_API aframe_status aframe_whiten_rolling(aframe_ctx* ctx, const float* d_strai
   if (st != AFRAME_OK) return st;
   if (cfg.welch_average == 0 && seg_step >= 2 && n_avg >= 2 * seg_step && n_epochs >= 8) {
     // consecutive epochs share all but seg_step of their n_avg periodograms: sum them in groups of seg_step once
-    st = af_ws_reserve(ctx, ctx->ws_groups, sizeof(float) * (size_t)C * (seg_total / seg_step) * F);
+    st = af_ws_reserve(ctx, ctx->ws_groups, 2 * sizeof(float) * (size_t)C * (seg_total / seg_step) * F);   // group sums + their first step - 1 terms
     if (st != AFRAME_OK) return st;
     st = af_launch_psd_mean_grouped(ctx, pg, seg_total, seg_step, n_epochs, n_avg, reinterpret_cast<float*>(ctx->ws_groups.ptr), psd);
   } else {

@@ -311,35 +311,47 @@ welch_pair_kernel(const float* __restrict__ strain, int64_t ld, int64_t n_seg, i
   (void)n_pairs;
 }
 
-// G[c][j][k] = sum of the `step` consecutive periodograms j step .. j step + step - 1.  fp32: a sum of n_avg = 63 positive
-// terms taken as 7 group sums of 8 plus 7 single terms is good to a few 1e-7 relative, against the 1e-4 of rule T1.
+// G[c][j][k] = sum of the `step` consecutive periodograms j step .. j step + step - 1, and Tl[c][j][k] = the sum of the first
+// step - 1 of them (the same additions in the same order, one term earlier).  fp32: a sum of n_avg = 63 positive terms taken
+// as 7 group sums of 8 plus 7 single terms is good to a few 1e-7 relative, against the 1e-4 of rule T1.
 __global__ void psd_group_sum_kernel(const float* __restrict__ pgram, int64_t n_seg_total, int step, int64_t n_groups, int F,
-                                     float* __restrict__ G) {
+                                     float* __restrict__ G, float* __restrict__ Tl) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t j = blockIdx.y;
   const int c = blockIdx.z;
   if (k >= F) return;
   const float* p = pgram + ((int64_t)c * n_seg_total + j * step) * F + k;
-  float acc = 0.f;
+  float acc = 0.f, head = 0.f;
 #pragma unroll 8
-  for (int i = 0; i < step; ++i, p += F) acc += *p;
+  for (int i = 0; i < step; ++i, p += F) {
+    if (i == step - 1) head = acc;
+    acc += *p;
+  }
   G[((int64_t)c * n_groups + j) * F + k] = acc;
+  Tl[((int64_t)c * n_groups + j) * F + k] = head;
 }
-// PSD of epoch e = mean of the n_avg periodograms from segment e step on = (n_avg / step whole groups + the rest) / n_avg
-__global__ void psd_mean_grouped_kernel(const float* __restrict__ pgram, const float* __restrict__ G, int64_t n_seg_total,
-                                        int64_t n_groups, int step, int n_avg, int F, int C, float inv_n, float* __restrict__ psd) {
+// PSD of epoch e = mean of the n_avg periodograms from segment e step on = (n_avg / step whole groups + the rest) / n_avg.
+// rest == step - 1 (63 = 7 x 8 + 7): the rest is Tl of the next group -- 8 reads per bin instead of 14, none of them from
+// the periodograms; else the single terms are read.
+__global__ void psd_mean_grouped_kernel(const float* __restrict__ pgram, const float* __restrict__ G, const float* __restrict__ Tl,
+                                        int64_t n_seg_total, int64_t n_groups, int step, int n_avg, int F, int C, float inv_n,
+                                        float* __restrict__ psd) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t e = blockIdx.y;
   const int c = blockIdx.z;
   if (k >= F) return;
   const int n_full = n_avg / step, n_rest = n_avg - n_full * step;
   const float* gp = G + ((int64_t)c * n_groups + e) * F + k;
-  const float* p = pgram + ((int64_t)c * n_seg_total + e * step + (int64_t)n_full * step) * F + k;
   float a0 = 0.f, a1 = 0.f;
 #pragma unroll 8
   for (int j = 0; j < n_full; ++j, gp += F) a0 += *gp;
+  if (n_rest == step - 1 && e + n_full < n_groups) {
+    a1 = Tl[((int64_t)c * n_groups + e + n_full) * F + k];
+  } else {
+    const float* p = pgram + ((int64_t)c * n_seg_total + e * step + (int64_t)n_full * step) * F + k;
 #pragma unroll 8
-  for (int i = 0; i < n_rest; ++i, p += F) a1 += *p;
+    for (int i = 0; i < n_rest; ++i, p += F) a1 += *p;
+  }
   psd[((int64_t)e * C + c) * F + k] = (a0 + a1) * inv_n;
 }
 
@@ -367,17 +379,18 @@ aframe_status af_launch_welch_pairs(aframe_ctx* ctx, const float* d_strain, int6
 }
 
 // Mean PSD per epoch through group sums (reads n_avg / step + n_avg % step values per bin and epoch instead of n_avg).
-// d_groups: scratch of C * n_groups * F floats, n_groups = n_seg_total / step.
+// d_groups: scratch of 2 * C * n_groups * F floats, n_groups = n_seg_total / step.
 aframe_status af_launch_psd_mean_grouped(aframe_ctx* ctx, const float* d_pgram, int64_t n_seg_total, int64_t seg_step,
                                          int64_t n_epochs, int64_t n_avg, float* d_groups, float* d_psd) {
   const int F = ctx->cfg.welch_nfft / 2 + 1, C = af_nch(ctx);
   const int64_t n_groups = n_seg_total / seg_step;
   af_prof_begin(ctx, AFRAME_PROF_WELCH);
+  float* d_tails = d_groups + (size_t)C * n_groups * F;            // (the caller reserves both halves)
   psd_group_sum_kernel<<<dim3((F + 127) / 128, (unsigned)n_groups, (unsigned)C), 128, 0, ctx->stream>>>(
-      d_pgram, n_seg_total, (int)seg_step, n_groups, F, d_groups);
+      d_pgram, n_seg_total, (int)seg_step, n_groups, F, d_groups, d_tails);
   AF_LAUNCH_CHECK(ctx);
   psd_mean_grouped_kernel<<<dim3((F + 127) / 128, (unsigned)n_epochs, (unsigned)C), 128, 0, ctx->stream>>>(
-      d_pgram, d_groups, n_seg_total, n_groups, (int)seg_step, (int)n_avg, F, C, (float)(1.0 / (double)n_avg), d_psd);
+      d_pgram, d_groups, d_tails, n_seg_total, n_groups, (int)seg_step, (int)n_avg, F, C, (float)(1.0 / (double)n_avg), d_psd);
   af_prof_end(ctx, AFRAME_PROF_WELCH, 2);
   AF_LAUNCH_CHECK(ctx);
   return AFRAME_OK;
