@@ -128,12 +128,12 @@ template <int BN, bool CG2 = false> struct TcCfg {
   static constexpr int EPW = CG2 ? 2 : 1;
   static constexpr int EPI_COLS = 64 / EPW;          // accumulator columns per epilogue thread and chunk
   static constexpr int GROUP_THREADS = 128 * EPW;
-  // CTA pairs: one more warp per epilogue group whose only job is that group's TMA traffic (stores of staged chunks, residual
+  // One more warp per epilogue group whose only job is that group's TMA traffic (stores of staged chunks, residual
   // prefetch).  With the group's leader thread doing it, 255 threads waited at a named barrier per chunk while one thread
   // waited for the previous store to be read (~900 cycles), decoded the next tile and issued the residual load, and again
   // while it issued the store (~500): profiles/r02_conv_cycles.md.  The store warp and the epilogue threads meet only at
   // mbarriers ("staged": 256 arrivals after the chunk is written; "ready": the buffer is free again / its residual landed).
-  static constexpr int STORE_WARPS = CG2 ? EG : 0;
+  static constexpr int STORE_WARPS = EG;
   static constexpr int THREADS = 64 + GROUP_THREADS * EG + 32 * STORE_WARPS;
   static constexpr int smem(int stages, int nbuf, bool head) {
     return tc_fixed_bytes(head) + stages * STAGE_BYTES + EG * nbuf * TC_OUT_BYTES;
@@ -246,7 +246,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
   const uint32_t w_bar = base + 8u * (2 * STAGES + 2 * NACC + EG * MAXBUF);
   const uint32_t tmem_slot = w_bar + 8u;
   auto staged_bar = [&](int g, int b) { return tmem_slot + 8u + 8u * (g * MAXBUF + b); };
-  constexpr bool STW = CG2 && !HEAD;               // epilogue groups served by store warps (see TcCfg::STORE_WARPS)
+  constexpr bool STW = !HEAD;                      // epilogue groups served by store warps (see TcCfg::STORE_WARPS)
   float* s_bias = reinterpret_cast<float*>(gen_base + TC_BAR_BYTES);
   float* s_headw = reinterpret_cast<float*>(gen_base + 3072);
   static_assert(!HALO || (!CG2 && !HEAD), "HALO is a single-CTA, storing variant");
@@ -512,17 +512,22 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       const int NBUF = p.nbuf > 0 ? p.nbuf : 1;
       const uint32_t gbuf = out_base + (uint32_t)(g * NBUF) * TC_OUT_BYTES;
       constexpr int CH = BN / 64;
+      // the group's items, as its epilogue threads walk them: SPLIT (N = 256): every tile of this CTA, chunks g, g + 2;
+      // else: this CTA's tiles g, g + EG, ..., every chunk
+      const int tile_step = (SPLIT ? 1 : EG) * n_workers, tile_first = worker + (SPLIT ? 0 : g) * n_workers;
+      constexpr int C_STEP = SPLIT ? 2 : 1;
+      const int c_first = SPLIT ? g : 0;
       struct Cur { int prob, tile, c; };
       auto settle = [&](Cur& k) {                  // first valid item at or after k (prob = 2: past the end)
         while (k.prob < 2) {
           const TcConvParams& P = k.prob ? p1 : p;
           if (k.tile < P.num_tiles) return;
-          ++k.prob; k.tile = worker; k.c = g;
+          ++k.prob; k.tile = tile_first; k.c = c_first;
         }
       };
       auto next = [&](Cur& k) {
-        k.c += 2;
-        if (k.c >= CH) { k.c = g; k.tile += n_workers; }
+        k.c += C_STEP;
+        if (k.c >= CH) { k.c = c_first; k.tile += tile_step; }
         settle(k);
       };
       // buffer `buf` may be written for item k: its residual tile is on its way, or (no residual) it is simply free
@@ -538,7 +543,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           mbar_arrive(res_bar(g, buf));
         }
       };
-      Cur S = {0, worker, g}, A = {0, worker, g};
+      Cur S = {0, tile_first, c_first}, A = {0, tile_first, c_first};
       settle(S); settle(A);
       for (int i = 0; i < NBUF; ++i) { signal_ready(A, i); next(A); }
       for (uint32_t j = 0; S.prob < 2; ++j) {
