@@ -14,7 +14,8 @@
 //   or (HEAD) the fused global-average-pool + linear head: per-(window, slab) partial dot products.
 //
 // Warp roles: warp 0 TMA producer, warp 1 MMA issuer (+TMEM alloc), then EG epilogue groups of 4 warps (CTA pairs: 8 warps,
-// two per TMEM lane quadrant, each taking half of a chunk's columns).
+// two per TMEM lane quadrant, each taking half of a chunk's columns), then one store warp per epilogue group (storing
+// variants): it issues the group's TMA stores and residual prefetches, so the epilogue threads never wait on a store.
 // With EG = 2 the groups take alternate tiles (group g <-> TMEM accumulator stage g), which doubles the
 // epilogue rate of the small-K layers whose epilogue, not the MMA, is the critical path.
 // Persistent: CTA i handles tiles i, i + grid, ...
