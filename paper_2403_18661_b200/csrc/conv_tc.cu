@@ -202,6 +202,18 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.edge_head = packed ? ov->e_head : 0; p.edge_tail = packed ? ov->e_tail : 0;
   p.edge_shift = packed ? ov->e_shift : 0;
   p.edge_stream = packed ? reinterpret_cast<const uint4*>(ov->e_stream) : nullptr;
+  // the two stream rows next to a slot's edge rows, as far as the box does not hold them (the store warp copies those)
+  p.edge_out = packed && ov->e_stream ? reinterpret_cast<uint4*>(out) : nullptr;
+  p.cpy_t0_head = p.cpy_n_head = p.cpy_t0_tail = p.cpy_n_tail = 0;
+  if (p.edge_out) {
+    p.cpy_t0_head = ov->e_head > T_box ? ov->e_head : T_box;
+    p.cpy_n_head = ov->e_head + 2 - p.cpy_t0_head;
+    p.cpy_t0_tail = ov->e_T - ov->e_tail - 2;
+    p.cpy_n_tail = ov->e_tail + 2 - T_box;
+    if (p.cpy_n_head < 0) p.cpy_n_head = 0;
+    if (p.cpy_n_tail < 0) p.cpy_n_tail = 0;
+    if (p.cpy_n_tail > 2) p.cpy_n_tail = 2;
+  }
   const int64_t b_blks = packed ? 2 * ((ov->e_nb + B_box - 1) / B_box) : (nb + B_box - 1) / B_box;
   const int64_t m_tiles = b_blks * p.t_blks;
   p.num_tiles = (int)((cg2 ? (m_tiles + 1) / 2 : m_tiles) * p.n_tiles);
@@ -714,9 +726,10 @@ static SharedPlan tc_plan_shared(const std::vector<LayerDesc>& layers, bool live
     g.rows_stream = tc_up128((chunk - 1) * g.shift + g.T);
     g.rows_edge = tc_up128(2 * chunk * g.period);
     // Packed edge batch: layer q's output differs from the stream's only in its first e_head[q] / last e_tail[q] rows (one more
-    // per conv); its box holds those rows and the two rows next to them that the epilogue takes from the stream (the outer one
-    // is computed from a row outside the box): tbox[q] = max(e_head, e_tail) + 2 rows, floor(128 / tbox) slots per MMA tile.
-    // (The entry conv's rows are all computed from valid input rows and the last layer's interior rows are never read: no copies.)
+    // per conv); its box holds those rows: tbox[q] = max(e_head, e_tail) (at least 8) rows, floor(128 / tbox) slots per MMA
+    // tile.  The two rows next to them, which the next two layers read as well, are the stream's: the launch's store warps copy
+    // them into the slot (with them inside the box, as before, the 256 / 512-channel stages ran 12 % more tiles) (rows of the box among them are replaced in the epilogue), so a slot is max(e_head, e_tail) + 2 rows.
+    // (The last layer's interior rows are never read: no copies.)
     if (g.C % 256 == 0) {
       const int nl = (int)g.list.size();
       g.e_head.resize(nl); g.e_tail.resize(nl); g.tbox.assign(nl, 0);
@@ -726,9 +739,11 @@ static SharedPlan tc_plan_shared(const std::vector<LayerDesc>& layers, bool live
         g.e_head[q] = hp / 2 + 1 + q;
         g.e_tail[q] = g.T - (Tp - tp) / 2 + q;
         // edge rows + the two copied rows; the stage's last layer is read at its edge rows only (next stage's gather, stitch, head)
-        g.tbox[q] = (g.e_head[q] > g.e_tail[q] ? g.e_head[q] : g.e_tail[q]) + (q + 1 < nl ? 2 : 0);
-        if (g.tbox[q] > 32 || g.tbox[q] < 1 || 128 / g.tbox[q] > SH_SPARE_SLOTS) ok = false;   // (a half's last box overhangs by < 128 / tbox slots)
-        if (g.tbox[q] > Pmax) Pmax = g.tbox[q];
+        const int e_max = g.e_head[q] > g.e_tail[q] ? g.e_head[q] : g.e_tail[q];
+        g.tbox[q] = e_max > 8 ? e_max : 8;
+        if (g.tbox[q] > 32 || e_max < 1 || 128 / g.tbox[q] > SH_SPARE_SLOTS) ok = false;   // (a half's last box overhangs by < 128 / tbox slots)
+        const int slot_rows = q + 1 < nl ? (g.tbox[q] > e_max + 2 ? g.tbox[q] : e_max + 2) : g.tbox[q];
+        if (slot_rows > Pmax) Pmax = slot_rows;
       }
       if (ok && g.T >= 2 * Pmax && g.e_head[nl - 1] == g.head && g.e_tail[nl - 1] == g.tail) {
         g.packed = true; g.P = Pmax;
@@ -945,7 +960,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             ov_s.pair_plan = ov_e.pair_plan = true;
             if (hr) pc->sh_head_rows = true;
             ov_e.e_nbp = (int)P.nbp; ov_e.e_P = h.P; ov_e.e_tbox = h.tbox[q]; ov_e.e_T = h.T; ov_e.e_head = h.e_head[q]; ov_e.e_tail = h.e_tail[q];
-            ov_e.e_shift = h.shift; ov_e.e_nb = nb; ov_e.e_stream = (entry || q + 1 == h.list.size()) ? nullptr : sh_buf((int)g, 0, (int)q);
+            ov_e.e_shift = h.shift; ov_e.e_nb = nb; ov_e.e_stream = q + 1 == h.list.size() ? nullptr : sh_buf((int)g, 0, (int)q);
             ok = build_launch(ctx, w, li, entry ? x_stream : sh_buf((int)g, 0, qi), qr >= 0 ? sh_buf((int)g, 0, qr) : nullptr,
                               sh_buf((int)g, 0, (int)q), 1, hr, hr_s, P.stream[q], sc, sc >= 0 ? x_stream : nullptr, &ov_s) &&
                  build_launch(ctx, w, li, entry ? x_edge : sh_buf((int)g, 1, qi), qr >= 0 ? sh_buf((int)g, 1, qr) : nullptr,

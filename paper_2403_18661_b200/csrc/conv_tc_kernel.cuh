@@ -88,9 +88,11 @@ struct TcConvParams {
   // the last edge_P rows (box at row edge_t0_tail = edge_P - T_box) -- and one T_box-row box per short window is computed;
   // the tensor map's zero fill is each window's own padding.  Only the rows within reach of that padding (row < edge_head or
   // row >= edge_T - edge_tail of the window, for THIS layer's output) differ from the stream's; the two rows next to them,
-  // which the next layers read as well (a conv reaches one row further, and so does the residual two layers on), are replaced
-  // in the epilogue by the stream's values edge_stream[(b * edge_shift + row) * c_out ...] (this layer's output over the
-  // chunk's stream, written by the previous launch); the rest of the box is never read.
+  // which the next layers read as well (a conv reaches one row further, and so does the residual two layers on), are the
+  // stream's values edge_stream[(b * edge_shift + row) * c_out ...] (this layer's output over the chunk's stream, written by the
+  // previous launch): rows of the box are replaced in the epilogue, rows of the slot outside the box (the box is only as long
+  // as the edge rows: T_box = max(edge_head, edge_tail)) are copied global -> global by lanes 1..31 of the store warps (edge_out, cpy_*).
+  // The rest of the box is never read.
   int edge_nbp;              // 0 = off; else slots per half (windows + spare slots for the last box of a half)
   int edge_blks_half;        // boxes per half: M tiles [0, edge_blks_half) are window starts, the rest window ends
   int edge_t0_tail, edge_T, edge_P, edge_head, edge_tail;
@@ -98,7 +100,10 @@ struct TcConvParams {
   int a_bytes;               // bytes of one activation box (T_box * B_box rows of 128 B; 16 KB unless T_box does not divide 128:
                              // the rest of the 128-row MMA tile is then stale shared memory, and those rows are dropped)
   long long edge_shift;
-  const uint4* edge_stream;  // null: nothing is replaced (the stage's entry conv: all its input rows are valid)
+  const uint4* edge_stream;  // null: nothing is replaced or copied (the stage's last layer: only its edge rows are read)
+  uint4* edge_out;           // this launch's slots [2 edge_nbp][edge_P][c_out] (the tensor behind tm_out), for those copies
+  int cpy_t0_head, cpy_n_head;   // window rows [cpy_t0, cpy_t0 + cpy_n) of a head / tail slot come from the stream and lie outside
+  int cpy_t0_tail, cpy_n_tail;   // the box (cpy_n = 0..2)
   int w_bytes;               // resident weight region (0 unless HALO)
   int stage_bytes;           // bytes per main-loop stage
 #ifdef AFRAME_TC_CYCLES      // experiments build only (not compiled into the product library)
@@ -560,6 +565,49 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         next(A); next(S);
       }
       tma_store_wait_all<0>();
+    } else if (STW && CG2) {
+      // ===== lanes 1..31 of the store warps (CTA-pair storing variant), on their own path: packed edge batch, the stream rows
+      // next to each slot's edge rows that the box does not hold (see TcConvParams::edge_out), global -> global, store warp g
+      // taking its 1/EG of the tile's columns.  Nothing in this launch reads these rows, so the path meets no barrier.
+      auto copy_rows = [&](const TcConvParams& P) {
+        if (P.edge_out == nullptr) return;
+        const int cq = P.c_out >> 3;                // uint4 per row
+        constexpr int PER_ROW = BN / 8 / EG;        // uint4 of this warp's columns per slot row (a power of two)
+        static_assert((PER_ROW & (PER_ROW - 1)) == 0, "PER_ROW");
+        for (int tile = worker; tile < P.num_tiles; tile += n_workers) {
+          int n_idx, t0, b0;
+          decode(P, tile, n_idx, t0, b0);
+          const bool tailb = b0 >= P.edge_nbp;
+          const int rows_cp = tailb ? P.cpy_n_tail : P.cpy_n_head;
+          if (rows_cp <= 0) continue;
+          const int tw0 = tailb ? P.cpy_t0_tail : P.cpy_t0_head, bfirst = tailb ? b0 - P.edge_nbp : b0;
+          const int srow0 = tw0 - (tailb ? P.edge_T - P.edge_P : 0);
+          const int col = ((n_idx * BN) >> 3) + g * PER_ROW;
+          const int total = P.B_box * rows_cp * PER_ROW;
+          constexpr int NCP = 6;
+          for (int i0 = 0; i0 < total; i0 += 31 * NCP) {
+            uint4 cr[NCP];
+            uint4* cdst[NCP];
+#pragma unroll
+            for (int k = 0; k < NCP; ++k) {
+              const int idx = i0 + (lane - 1) + 31 * k;
+              const int srow = idx / PER_ROW, ch = idx % PER_ROW;
+              const int slot = rows_cp == 2 ? srow >> 1 : srow, r = rows_cp == 2 ? srow & 1 : 0;
+              const int b = bfirst + slot;
+              cdst[k] = nullptr;
+              if (idx < total && b < P.nb) {
+                cdst[k] = P.edge_out + ((long long)(tailb ? P.edge_nbp + b : b) * P.edge_P + srow0 + r) * cq + col + ch;
+                cr[k] = __ldg(P.edge_stream + ((long long)b * P.edge_shift + tw0 + r) * cq + col + ch);
+              }
+            }
+#pragma unroll
+            for (int k = 0; k < NCP; ++k)
+              if (cdst[k] != nullptr) *cdst[k] = cr[k];
+          }
+        }
+      };
+      copy_rows(p);
+      if (!HALO && !HEAD && p1.num_tiles > 0) copy_rows(p1);
     }
   } else {
     // ===== epilogue: EG groups of 4 warps, thread <-> one output row =====

@@ -29,8 +29,9 @@ def test_config1_plan_is_the_documented_one(af, blob):
     assert [(d["T"], d["C"], d["head"], d["tail"], d["packed"]) for d in st] == [
         (384, 128, 12, 11, False), (192, 256, 18, 17, True), (96, 512, 15, 14, True)]
     assert st[0]["P"] == 19                                      # 128-channel stage: fixed 19-row short windows
-    assert st[1]["tbox"] == [9, 10, 11, 12, 13, 14, 15, 16, 17, 18, 19, 18] and st[1]["P"] == 19
-    assert st[2]["tbox"] == [12, 13, 14, 15, 16, 15] and st[2]["P"] == 16
+    # a box holds the edge rows only (at least 8); a slot also holds the two stream rows next to them, except in the last layer
+    assert st[1]["tbox"] == [8, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17, 18] and st[1]["P"] == 19
+    assert st[2]["tbox"] == [10, 11, 12, 13, 14, 15] and st[2]["P"] == 16
     assert st[1]["e_head"] == list(range(7, 19)) and st[1]["e_tail"] == list(range(6, 18))
     assert st[2]["e_head"] == list(range(10, 16)) and st[2]["e_tail"] == list(range(9, 15))
     assert all(d["spare_slots"] == 16 for d in st[1:])
@@ -62,16 +63,19 @@ def test_packed_edge_invariants_for_every_window_length(af, blob, spacing):
                 eh, et, tb = d["e_head"], d["e_tail"], d["tbox"]
                 assert eh == list(range(eh[0], eh[0] + nl)) and et == list(range(et[0], et[0] + nl))   # one more row per conv
                 assert eh[-1] == d["head"] and et[-1] == d["tail"]
+                slot_rows = []
                 for q in range(nl):
-                    assert tb[q] == max(eh[q], et[q]) + (2 if q + 1 < nl else 0)
+                    assert tb[q] == max(eh[q], et[q], 8)
                     assert 1 <= tb[q] <= 32
+                    # the slot: the box, and (all layers but the last) the two stream rows past the edge rows
+                    slot_rows.append(max(tb[q], max(eh[q], et[q]) + 2) if q + 1 < nl else tb[q])
                     boxes_per_tile = 128 // tb[q]
                     assert boxes_per_tile >= 4
                     # the last box of a half starts inside the windows and covers boxes_per_tile slots: overhang < spare slots
                     assert boxes_per_tile <= d["spare_slots"]
                     n_boxes = -(-n_windows // boxes_per_tile)
                     assert n_boxes * boxes_per_tile - n_windows < d["spare_slots"] + 1
-                assert d["P"] == max(tb) and d["T"] >= 2 * d["P"]  # the two halves of a window's slots never overlap
+                assert d["P"] == max(slot_rows) and d["T"] >= 2 * d["P"]  # the two halves of a window's slots never overlap
     if spacing in (32, 64, 128, 512):
         assert n_planned > 100
 
