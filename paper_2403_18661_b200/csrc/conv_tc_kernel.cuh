@@ -237,6 +237,9 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
   const uint32_t rank = CG2 ? cluster_ctarank() : 0u;
   const int n_workers = CG2 ? (int)(gridDim.x >> 1) : (int)gridDim.x;   // tile loops step by this
   const int worker = CG2 ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
+  // the second problem's tiles are dealt out where the first problem's round-robin stopped, so that no worker takes the odd
+  // tile of both (two problems of 5.04 and 1.74 rounds are 7 rounds, not 6 + 2)
+  const int worker1 = p1.num_tiles > 0 ? (worker + n_workers - p.num_tiles % n_workers) % n_workers : worker;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const uint32_t base = smem_u32(smem_raw);
   if (base & 1023u) __trap();                      // SWIZZLE_128B tiles need 1024-byte alignment
@@ -367,7 +370,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       const uint32_t lfull0 = CG2 ? mapa_cluster(full_bar(0), 0) : full_bar(0);   // leader's full barriers
       int stage = 0; uint32_t phase = 0;
       auto produce = [&](const CUtensorMap& tm_in, const CUtensorMap& tm_w, const CUtensorMap& tm_res, const CUtensorMap& tm_scw,
-                         const TcConvParams& p) {
+                         const TcConvParams& p, int worker) {
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         int n_idx, t0, b0;
         decode(p, tile, n_idx, t0, b0);
@@ -421,8 +424,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         }
       }
       };
-      produce(tm_in, tm_w, tm_res, tm_scw, p);
-      if (!HEAD && p1.num_tiles > 0) produce(tm_in1, tm_w1, tm_res1, tm_scw1, p1);
+      produce(tm_in, tm_w, tm_res, tm_scw, p, worker);
+      if (!HEAD && p1.num_tiles > 0) produce(tm_in1, tm_w1, tm_res1, tm_scw1, p1, worker1);
       if (lane == 0) Tflush(0);
     }
   } else if (warp == 1) {
@@ -432,7 +435,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       int stage = 0; uint32_t phase = 0;
       int acc = 0; uint32_t acc_phase = 0;
       if (HALO) mbar_wait(w_bar, 0);
-      auto issue = [&](const TcConvParams& p) {
+      auto issue = [&](const TcConvParams& p, int worker) {
       const int kiters = p.taps * p.kblocks + p.sc_kblocks;
       for (int tile = worker; tile < p.num_tiles; tile += n_workers) {
         T(0);
@@ -506,8 +509,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         T(4);
       }
       };
-      issue(p);
-      if (!HALO && !HEAD && p1.num_tiles > 0) issue(p1);
+      issue(p, worker);
+      if (!HALO && !HEAD && p1.num_tiles > 0) issue(p1, worker1);
       if (lane == 0) Tflush(1);
     }
   } else if (warp >= 2 + 4 * Cfg::EPW * EG) {
@@ -521,6 +524,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       // the group's items, as its epilogue threads walk them: SPLIT (N = 256): every tile of this CTA, chunks g, g + 2;
       // else: this CTA's tiles g, g + EG, ..., every chunk
       const int tile_step = (SPLIT ? 1 : EG) * n_workers, tile_first = worker + (SPLIT ? 0 : g) * n_workers;
+      const int tile_first1 = worker1 + (SPLIT ? 0 : g) * n_workers;
       constexpr int C_STEP = SPLIT ? 2 : 1;
       const int c_first = SPLIT ? g : 0;
       struct Cur { int prob, tile, c; };
@@ -528,7 +532,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         while (k.prob < 2) {
           const TcConvParams& P = k.prob ? p1 : p;
           if (k.tile < P.num_tiles) return;
-          ++k.prob; k.tile = tile_first; k.c = c_first;
+          ++k.prob; k.tile = tile_first1; k.c = c_first;
         }
       };
       auto next = [&](Cur& k) {
@@ -569,7 +573,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       // ===== lanes 1..31 of the store warps (CTA-pair storing variant), on their own path: packed edge batch, the stream rows
       // next to each slot's edge rows that the box does not hold (see TcConvParams::edge_out), global -> global, store warp g
       // taking its 1/EG of the tile's columns.  Nothing in this launch reads these rows, so the path meets no barrier.
-      auto copy_rows = [&](const TcConvParams& P) {
+      auto copy_rows = [&](const TcConvParams& P, int worker) {
         if (P.edge_out == nullptr) return;
         const int cq = P.c_out >> 3;                // uint4 per row
         constexpr int PER_ROW = BN / 8 / EG;        // uint4 of this warp's columns per slot row (a power of two)
@@ -606,8 +610,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
           }
         }
       };
-      copy_rows(p);
-      if (!HALO && !HEAD && p1.num_tiles > 0) copy_rows(p1);
+      copy_rows(p, worker);
+      if (!HALO && !HEAD && p1.num_tiles > 0) copy_rows(p1, worker1);
     }
   } else {
     // ===== epilogue: EG groups of 4 warps, thread <-> one output row =====
@@ -622,7 +626,6 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     const uint32_t gbuf = out_base + (uint32_t)(g * NBUF) * TC_OUT_BYTES;
     constexpr int CH = BN / 64;
     const int tile_step = (SPLIT ? 1 : EG) * n_workers;     // this group's tiles ...
-    const int tile_first = worker + (SPLIT ? 0 : g) * n_workers;
     constexpr int C_STEP = SPLIT ? 2 : 1;                   // ... and its chunks of each tile
     const int c_first = SPLIT ? g : 0;
     const uint32_t tempty_leader0 = CG2 ? mapa_cluster(tempty_bar(0), 0) : tempty_bar(0);
@@ -632,6 +635,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
     uint32_t res_par = 0;                          // bit b: phase parity of this group's residual barrier b
     const int PF = p.pf;
     auto drain = [&](const CUtensorMap& tm_out, const CUtensorMap& tm_res, const TcConvParams& p, bool second) {
+    const int tile_first = (second ? worker1 : worker) + (SPLIT ? 0 : g) * n_workers;
     if (second) {
       // the second problem's bias replaces the first one's once both groups are done with it; the leader's earlier stores
       // must have read their staging buffers before a residual tile is prefetched into one
