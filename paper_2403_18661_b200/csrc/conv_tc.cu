@@ -730,7 +730,7 @@ static SharedPlan tc_plan_shared(const std::vector<LayerDesc>& layers, bool live
     // tile.  The two rows next to them, which the next two layers read as well, are the stream's: the launch's store warps copy
     // them into the slot (with them inside the box, as before, the 256 / 512-channel stages ran 12 % more tiles) (rows of the box among them are replaced in the epilogue), so a slot is max(e_head, e_tail) + 2 rows.
     // (The last layer's interior rows are never read: no copies.)
-    if (g.C % 256 == 0) {
+    if (g.C % 128 == 0) {
       const int nl = (int)g.list.size();
       g.e_head.resize(nl); g.e_tail.resize(nl); g.tbox.assign(nl, 0);
       bool ok = true;

@@ -379,9 +379,11 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         const bool tail_box = p.edge_nbp > 0 && b0 >= p.edge_nbp;
         const int t0s = tail_box ? p.edge_t0_tail_sc : t0;
         if (tail_box) t0 = p.edge_t0_tail_in;
-        for (int d = 0; d < p.taps; ++d) {
-          const int toff = p.tap_toff[d], par = p.tap_par[d];
-          for (int kb = 0; kb < p.kblocks; ++kb) {
+        // (64-channel block outer, tap inner: the order in which the HALO variant accumulates, so that a layer gives the same
+        //  bits whichever of the two computes a row)
+        for (int kb = 0; kb < p.kblocks; ++kb) {
+          for (int d = 0; d < p.taps; ++d) {
+            const int toff = p.tap_toff[d], par = p.tap_par[d];
             T(0);
             mbar_wait(empty_bar(stage), phase ^ 1u);
             T(1);
@@ -569,7 +571,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         next(A); next(S);
       }
       tma_store_wait_all<0>();
-    } else if (STW && CG2) {
+    } else if (STW && !HALO) {
       // ===== lanes 1..31 of the store warps (CTA-pair storing variant), on their own path: packed edge batch, the stream rows
       // next to each slot's edge rows that the box does not hold (see TcConvParams::edge_out), global -> global, store warp g
       // taking its 1/EG of the tile's columns.  Nothing in this launch reads these rows, so the path meets no barrier.

@@ -27,14 +27,15 @@ def test_config1_plan_is_the_documented_one(af, blob):
     s1, st = af.describe_shared_plan(blob, 3072, 2, 128, 4096)
     assert s1 == 3                                               # three fused 64-channel blocks: edge 2k+2 / 2k+1 = 8 / 7 rows
     assert [(d["T"], d["C"], d["head"], d["tail"], d["packed"]) for d in st] == [
-        (384, 128, 12, 11, False), (192, 256, 18, 17, True), (96, 512, 15, 14, True)]
-    assert st[0]["P"] == 19                                      # 128-channel stage: fixed 19-row short windows
+        (384, 128, 12, 11, True), (192, 256, 18, 17, True), (96, 512, 15, 14, True)]
     # a box holds the edge rows only (at least 8); a slot also holds the two stream rows next to them, except in the last layer
+    assert st[0]["tbox"] == [8, 8, 8, 8, 9, 10, 11, 12] and st[0]["P"] == 13
+    assert st[0]["e_head"] == list(range(5, 13)) and st[0]["e_tail"] == list(range(4, 12))
     assert st[1]["tbox"] == [8, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17, 18] and st[1]["P"] == 19
     assert st[2]["tbox"] == [10, 11, 12, 13, 14, 15] and st[2]["P"] == 16
     assert st[1]["e_head"] == list(range(7, 19)) and st[1]["e_tail"] == list(range(6, 18))
     assert st[2]["e_head"] == list(range(10, 16)) and st[2]["e_tail"] == list(range(9, 15))
-    assert all(d["spare_slots"] == 16 for d in st[1:])
+    assert all(d["spare_slots"] == 16 for d in st)
 
 
 @pytest.mark.parametrize("spacing", [4, 8, 16, 32, 64, 100, 128, 256, 384, 512, 1024, 3072, 4096])
