@@ -117,6 +117,8 @@ struct TcShapeOverride {
   int e_nbp = 0, e_P = 0, e_tbox = 0, e_T = 0, e_head = 0, e_tail = 0;
   int64_t e_shift = 0, e_nb = 0;
   const af_act_t* e_stream = nullptr;
+  int e_keep = 0;             // > 0: the slot's first / last e_keep rows must be valid (the next stage reads them in place); else e + 2
+
   // packed stages read their stage input in place: in_rows > 0: the (stream) launch's input tensor holds in_rows rows
   // (rows past them read as zero); e_Pin > 0: the edge launch's input slots hold e_Pin rows (the stage-input slots of the
   // entry conv and of the conv with the folded projection are only as long as those two layers reach)
@@ -206,13 +208,13 @@ static bool build_launch(aframe_ctx* ctx, const aframe_weights* w, int li, const
   p.edge_out = packed && ov->e_stream ? reinterpret_cast<uint4*>(out) : nullptr;
   p.cpy_t0_head = p.cpy_n_head = p.cpy_t0_tail = p.cpy_n_tail = 0;
   if (p.edge_out) {
+    const int need_h = ov->e_keep > 0 ? ov->e_keep : ov->e_head + 2, need_t = ov->e_keep > 0 ? ov->e_keep : ov->e_tail + 2;
     p.cpy_t0_head = ov->e_head > T_box ? ov->e_head : T_box;
-    p.cpy_n_head = ov->e_head + 2 - p.cpy_t0_head;
-    p.cpy_t0_tail = ov->e_T - ov->e_tail - 2;
-    p.cpy_n_tail = ov->e_tail + 2 - T_box;
+    p.cpy_n_head = need_h - p.cpy_t0_head;
+    p.cpy_t0_tail = ov->e_T - need_t;
+    p.cpy_n_tail = need_t - (ov->e_tail > T_box ? ov->e_tail : T_box);
     if (p.cpy_n_head < 0) p.cpy_n_head = 0;
     if (p.cpy_n_tail < 0) p.cpy_n_tail = 0;
-    if (p.cpy_n_tail > 2) p.cpy_n_tail = 2;
   }
   const int64_t b_blks = packed ? 2 * ((ov->e_nb + B_box - 1) / B_box) : (nb + B_box - 1) / B_box;
   const int64_t m_tiles = b_blks * p.t_blks;
@@ -669,6 +671,8 @@ struct SharedStage {
   // edge rows of its output at the window's start / end and the rows its box computes
   bool packed = false;
   int P = 0, P_in = 0;              // rows per slot of the layers' outputs / of the gathered stage input
+  bool in_place = false;            // the stage reads the previous (packed) stage's last-layer slots in place: no gather
+  int keep = 0;                     // > 0: the next stage does; the last layer's slots hold `keep` valid rows at each end
   std::vector<int> e_head, e_tail, tbox;
 };
 struct SharedPlan {
@@ -754,6 +758,20 @@ static SharedPlan tc_plan_shared(const std::vector<LayerDesc>& layers, bool live
     shs.push_back(g);
     i0 = g.list.back() + 1; Tp = g.T; hp = g.head; tp = g.tail; shift_p = g.shift;
   }
+  // A packed stage after a packed stage reads its input slots where the previous stage's last layer wrote them: that layer's
+  // slots are made as long as the entry conv and the folded projection reach (P_in rows, an even number: the stride-2 view),
+  // its store warps copy the stream rows past the edge rows, and the gather between the two stages is not launched.
+  for (size_t g = 0; g < shs.size(); ++g) {
+    SharedStage& h = shs[g];
+    h.P_in = h.packed ? 2 * (h.tbox.size() > 1 ? h.tbox[1] : h.tbox[0] + 1) : 0;
+    if (g == 0 || !h.packed || !shs[g - 1].packed) continue;
+    SharedStage& a = shs[g - 1];
+    int P2 = a.P > h.P_in ? a.P : h.P_in;
+    P2 += P2 & 1;
+    if (a.T < 2 * P2 || a.C != h.C_in) continue;
+    a.P = P2; a.keep = h.P_in; a.rows_edge = 2 * (chunk + SH_SPARE_SLOTS) * a.P;
+    h.in_place = true;
+  }
   return pl;
 }
 
@@ -832,8 +850,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
     h.stream_bytes = ((size_t)(h.rows_stream + h.rows_edge) * h.C * 2 + 1023) & ~(size_t)1023;
     // the stage input: packed stages read the previous stage's stream in place and gather only the slots their first two
     // layers reach (P_in rows per slot at the previous stage's resolution); other stages gather [stream | short windows]
-    h.P_in = h.packed ? 2 * (h.tbox.size() > 1 ? h.tbox[1] : h.tbox[0] + 1) : 0;
-    h.x_bytes = h.packed ? (((size_t)2 * (chunk + SH_SPARE_SLOTS) * h.P_in * h.C_in * 2 + 1023) & ~(size_t)1023)
+    h.x_bytes = h.in_place ? 0 : h.packed ? (((size_t)2 * (chunk + SH_SPARE_SLOTS) * h.P_in * h.C_in * 2 + 1023) & ~(size_t)1023)
                          : (((size_t)2 * (h.rows_stream + h.rows_edge) * h.C_in * 2 + 1023) & ~(size_t)1023);
     h.off = s2_bytes;
     s2_bytes += h.x_bytes + h.list.size() * h.stream_bytes;
@@ -945,12 +962,13 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             // stage input: the previous stage's stream in place (its valid rows; the rest reads as zero), and the gathered slots
             const int q_prev = g ? (int)shs[g - 1].list.size() - 1 : 0;
             const af_act_t* x_stream = g ? sh_buf((int)g - 1, 0, q_prev) : s1_stream_ptr(s1_k);
-            const af_act_t* x_edge = sh_x_ptr((int)g);
+            const af_act_t* x_edge = h.in_place ? sh_buf((int)g - 1, 1, q_prev) : sh_x_ptr((int)g);
+            const int x_Pin = h.in_place ? shs[g - 1].P : h.P_in;
             TcShapeOverride ov_s{(int)rows_s, 0, 0, 0};
             TcShapeOverride ov_e{0, 0, 0, 0};
             const int64_t valid_prev = (g ? (nb - 1) * shs[g - 1].shift + shs[g - 1].T : (nb - 1) * (sB / 4) + w->layers[1].t_out) & ~(int64_t)1;
-            if (entry) { ov_s.in_rows = valid_prev; ov_e.e_Pin = h.P_in; }
-            if (sc >= 0) { ov_s.in_rows_sc = valid_prev; ov_e.e_Pin_sc = h.P_in; }
+            if (entry) { ov_s.in_rows = valid_prev; ov_e.e_Pin = x_Pin; }
+            if (sc >= 0) { ov_s.in_rows_sc = valid_prev; ov_e.e_Pin_sc = x_Pin; }
             // the conv that feeds the head stores nothing: its tensor holds the per-row head dot products instead
             // ([stream rows | edge-batch rows][C / 64] floats)
             const bool hr = sh_head_on && g + 1 == shs.size() && q + 1 == h.list.size();
@@ -960,7 +978,9 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
             ov_s.pair_plan = ov_e.pair_plan = true;
             if (hr) pc->sh_head_rows = true;
             ov_e.e_nbp = (int)P.nbp; ov_e.e_P = h.P; ov_e.e_tbox = h.tbox[q]; ov_e.e_T = h.T; ov_e.e_head = h.e_head[q]; ov_e.e_tail = h.e_tail[q];
-            ov_e.e_shift = h.shift; ov_e.e_nb = nb; ov_e.e_stream = q + 1 == h.list.size() ? nullptr : sh_buf((int)g, 0, (int)q);
+            ov_e.e_shift = h.shift; ov_e.e_nb = nb; const bool last_q = q + 1 == h.list.size();
+            ov_e.e_stream = last_q && h.keep == 0 ? nullptr : sh_buf((int)g, 0, (int)q);
+            ov_e.e_keep = last_q ? h.keep : 0;
             ok = build_launch(ctx, w, li, entry ? x_stream : sh_buf((int)g, 0, qi), qr >= 0 ? sh_buf((int)g, 0, qr) : nullptr,
                               sh_buf((int)g, 0, (int)q), 1, hr, hr_s, P.stream[q], sc, sc >= 0 ? x_stream : nullptr, &ov_s) &&
                  build_launch(ctx, w, li, entry ? x_edge : sh_buf((int)g, 1, qi), qr >= 0 ? sh_buf((int)g, 1, qr) : nullptr,
@@ -1076,6 +1096,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
         if (P.packed) {
           const int P_in = shs[g].P_in;
           const int64_t n_p = (2 * P.nbp * P_in) * pieces_in;
+          if (!shs[g].in_place) {
           aux_begin();
           shp_gather_kernel<<<(unsigned)((n_p + 255) / 256), 256, 0, ctx->stream>>>(
               reinterpret_cast<uint4*>(sh_x_ptr((int)g)),
@@ -1086,6 +1107,7 @@ aframe_status af_forward_bf16(aframe_ctx* ctx, const aframe_weights* w, const vo
               0, 0, P_in);
           AF_LAUNCH_CHECK(ctx);
           aux_end();
+          }
           // Launch order: stream(0) | edge(q) with stream(q + 1) as ONE launch of two problems (independent of each other: both
           // need stream(q), and edge(q) needs edge(q - 1)) | ... | edge(last).  A stream launch alone costs 16-30 us for 1/8 of an
           // edge launch's work (profiles/r01i_conv_full.md); as the second problem its tiles fill the edge launch's last wave.

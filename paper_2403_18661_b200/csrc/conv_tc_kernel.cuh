@@ -598,7 +598,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
             for (int k = 0; k < NCP; ++k) {
               const int idx = i0 + (lane - 1) + 31 * k;
               const int srow = idx / PER_ROW, ch = idx % PER_ROW;
-              const int slot = rows_cp == 2 ? srow >> 1 : srow, r = rows_cp == 2 ? srow & 1 : 0;
+              const int slot = srow / rows_cp, r = srow - slot * rows_cp;
               const int b = bfirst + slot;
               cdst[k] = nullptr;
               if (idx < total && b < P.nb) {
@@ -675,8 +675,8 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       const bool is_tail = m >= p.edge_nbp;
       const int b = is_tail ? m - p.edge_nbp : m;
       const int t_win = (is_tail ? p.edge_T - p.edge_P : 0) + t0_ + row_tq;
-      const int d = is_tail ? p.edge_T - p.edge_tail - 1 - t_win : t_win - p.edge_head;   // 0, 1: the two rows past the edge
-      if (d < 0 || d > 1 || b >= p.nb) return nullptr;
+      const int d = is_tail ? p.edge_T - p.edge_tail - 1 - t_win : t_win - p.edge_head;   // >= 0: a row of the box past the edge rows
+      if (d < 0 || b >= p.nb) return nullptr;
       return p.edge_stream + (((long long)b * p.edge_shift + t_win) * p.c_out + n0_) / 8;
     };
     // ... and is fetched into L1 one tile ahead, so that the epilogue does not wait for L2 (measured: the un-prefetched copy

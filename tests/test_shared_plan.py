@@ -29,9 +29,11 @@ def test_config1_plan_is_the_documented_one(af, blob):
     assert [(d["T"], d["C"], d["head"], d["tail"], d["packed"]) for d in st] == [
         (384, 128, 12, 11, True), (192, 256, 18, 17, True), (96, 512, 15, 14, True)]
     # a box holds the edge rows only (at least 8); a slot also holds the two stream rows next to them, except in the last layer
-    assert st[0]["tbox"] == [8, 8, 8, 8, 9, 10, 11, 12] and st[0]["P"] == 13
+    # (a packed stage that feeds a packed stage holds, in its slots, the rows the next stage's first two layers reach: 2 x
+    #  their second box, read in place)
+    assert st[0]["tbox"] == [8, 8, 8, 8, 9, 10, 11, 12] and st[0]["P"] == 16
     assert st[0]["e_head"] == list(range(5, 13)) and st[0]["e_tail"] == list(range(4, 12))
-    assert st[1]["tbox"] == [8, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17, 18] and st[1]["P"] == 19
+    assert st[1]["tbox"] == [8, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17, 18] and st[1]["P"] == 22
     assert st[2]["tbox"] == [10, 11, 12, 13, 14, 15] and st[2]["P"] == 16
     assert st[1]["e_head"] == list(range(7, 19)) and st[1]["e_tail"] == list(range(6, 18))
     assert st[2]["e_head"] == list(range(10, 16)) and st[2]["e_tail"] == list(range(9, 15))
@@ -52,7 +54,7 @@ def test_packed_edge_invariants_for_every_window_length(af, blob, spacing):
                 continue
             assert 0 <= s1 <= 5
             prev_T = kernel_len // 4
-            for d in st:
+            for si, d in enumerate(st):
                 # rows taken from one end of a window must be out of reach of the padding at the other end
                 assert d["T"] * 2 == prev_T and d["head"] >= 1 and d["tail"] >= 1 and d["head"] + d["tail"] <= d["T"]
                 prev_T = d["T"]
@@ -76,7 +78,11 @@ def test_packed_edge_invariants_for_every_window_length(af, blob, spacing):
                     assert boxes_per_tile <= d["spare_slots"]
                     n_boxes = -(-n_windows // boxes_per_tile)
                     assert n_boxes * boxes_per_tile - n_windows < d["spare_slots"] + 1
-                assert d["P"] == max(slot_rows) and d["T"] >= 2 * d["P"]  # the two halves of a window's slots never overlap
+                # ... or, if a packed stage follows, the rows its entry conv and folded projection reach (an even number)
+                nxt = st[si + 1] if si + 1 < len(st) and st[si + 1]["packed"] else None
+                p_in = 2 * (nxt["tbox"][1] if nxt["n_layers"] > 1 else nxt["tbox"][0] + 1) if nxt else 0
+                want = max(max(slot_rows), p_in)
+                assert d["P"] in (max(slot_rows), want + (want & 1)) and d["T"] >= 2 * d["P"]  # a window's two slots never overlap
     if spacing in (32, 64, 128, 512):
         assert n_planned > 100
 
