@@ -395,7 +395,7 @@ static cudaError_t launch_block(const TcBlockLaunch& L, cudaStream_t s) {
 // therefore run (1) once over the whole stream and (2) over a batch of 2 short windows per window -- its first and last
 // S1_ROWS rows, with the true edge rows of the previous block -- which yields the edge rows exactly; s1_stitch_kernel
 // then writes the per-window tensor the next stage reads.  Same kernel, same per-row arithmetic: bit-identical results.
-constexpr int SH_SPARE_SLOTS = 16;          // packed edge batch: spare slots after each half (the last box of a half may overhang)
+constexpr int SH_SPARE_SLOTS = 32;          // packed edge batch: spare slots after each half (the last box of a half may overhang)
 constexpr int S1_ROWS = 16;                 // rows of a short window (needs 2 K + 4 <= S1_ROWS - 2 for K blocks)
 constexpr int S1_PERIOD = S1_ROWS + 2;      // + 2 separator rows (zero input, y1 forced to zero)
 
@@ -730,7 +730,7 @@ static SharedPlan tc_plan_shared(const std::vector<LayerDesc>& layers, bool live
     g.rows_stream = tc_up128((chunk - 1) * g.shift + g.T);
     g.rows_edge = tc_up128(2 * chunk * g.period);
     // Packed edge batch: layer q's output differs from the stream's only in its first e_head[q] / last e_tail[q] rows (one more
-    // per conv); its box holds those rows: tbox[q] = max(e_head, e_tail) (at least 8) rows, floor(128 / tbox) slots per MMA
+    // per conv); its box holds those rows: tbox[q] = max(e_head, e_tail) (at least 4) rows, floor(128 / tbox) slots per MMA
     // tile.  The two rows next to them, which the next two layers read as well, are the stream's: the launch's store warps copy
     // them into the slot (with them inside the box, as before, the 256 / 512-channel stages ran 12 % more tiles) (rows of the box among them are replaced in the epilogue), so a slot is max(e_head, e_tail) + 2 rows.
     // (The last layer's interior rows are never read: no copies.)
@@ -744,7 +744,7 @@ static SharedPlan tc_plan_shared(const std::vector<LayerDesc>& layers, bool live
         g.e_tail[q] = g.T - (Tp - tp) / 2 + q;
         // edge rows + the two copied rows; the stage's last layer is read at its edge rows only (next stage's gather, stitch, head)
         const int e_max = g.e_head[q] > g.e_tail[q] ? g.e_head[q] : g.e_tail[q];
-        g.tbox[q] = e_max > 8 ? e_max : 8;
+        g.tbox[q] = e_max > 4 ? e_max : 4;          // (at most 32 = SH_SPARE_SLOTS boxes per tile)
         if (g.tbox[q] > 32 || e_max < 1 || 128 / g.tbox[q] > SH_SPARE_SLOTS) ok = false;   // (a half's last box overhangs by < 128 / tbox slots)
         const int slot_rows = q + 1 < nl ? (g.tbox[q] > e_max + 2 ? g.tbox[q] : e_max + 2) : g.tbox[q];
         if (slot_rows > Pmax) Pmax = slot_rows;

@@ -28,16 +28,16 @@ def test_config1_plan_is_the_documented_one(af, blob):
     assert s1 == 3                                               # three fused 64-channel blocks: edge 2k+2 / 2k+1 = 8 / 7 rows
     assert [(d["T"], d["C"], d["head"], d["tail"], d["packed"]) for d in st] == [
         (384, 128, 12, 11, True), (192, 256, 18, 17, True), (96, 512, 15, 14, True)]
-    # a box holds the edge rows only (at least 8); a slot also holds the two stream rows next to them, except in the last layer
+    # a box holds the edge rows only (at least 4); a slot also holds the two stream rows next to them, except in the last layer
     # (a packed stage that feeds a packed stage holds, in its slots, the rows the next stage's first two layers reach: 2 x
     #  their second box, read in place)
-    assert st[0]["tbox"] == [8, 8, 8, 8, 9, 10, 11, 12] and st[0]["P"] == 16
+    assert st[0]["tbox"] == [5, 6, 7, 8, 9, 10, 11, 12] and st[0]["P"] == 16
     assert st[0]["e_head"] == list(range(5, 13)) and st[0]["e_tail"] == list(range(4, 12))
-    assert st[1]["tbox"] == [8, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17, 18] and st[1]["P"] == 22
+    assert st[1]["tbox"] == [7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17, 18] and st[1]["P"] == 22
     assert st[2]["tbox"] == [10, 11, 12, 13, 14, 15] and st[2]["P"] == 16
     assert st[1]["e_head"] == list(range(7, 19)) and st[1]["e_tail"] == list(range(6, 18))
     assert st[2]["e_head"] == list(range(10, 16)) and st[2]["e_tail"] == list(range(9, 15))
-    assert all(d["spare_slots"] == 16 for d in st)
+    assert all(d["spare_slots"] == 32 for d in st)
 
 
 @pytest.mark.parametrize("spacing", [4, 8, 16, 32, 64, 100, 128, 256, 384, 512, 1024, 3072, 4096])
@@ -68,7 +68,7 @@ def test_packed_edge_invariants_for_every_window_length(af, blob, spacing):
                 assert eh[-1] == d["head"] and et[-1] == d["tail"]
                 slot_rows = []
                 for q in range(nl):
-                    assert tb[q] == max(eh[q], et[q], 8)
+                    assert tb[q] == max(eh[q], et[q], 4)
                     assert 1 <= tb[q] <= 32
                     # the slot: the box, and (all layers but the last) the two stream rows past the edge rows
                     slot_rows.append(max(tb[q], max(eh[q], et[q]) + 2) if q + 1 < nl else tb[q])
