@@ -256,15 +256,17 @@ aframe_status aframe_postprocess(aframe_ctx* ctx, const float* d_scores, int64_t
  * zero padding: the tensor-core path runs each stage once over the stream of a launch sequence plus, per
  * window, the rows within reach of the padding.  This call reports that plan for a weight blob (version 1, as for
  * aframe_weights_load): *first_stage_blocks = basic blocks of the 64-channel stage run in shared form (0: none), then one
- * record per later stage in shared form.  In a packed stage, launched layer q computes per window one box of tbox[q] rows at
- * each end (its e_head[q] / e_tail[q] edge rows plus the two rows the epilogue copies from the stream), floor(128 / tbox[q])
- * boxes per 128-row MMA tile, in slots of P rows; the last box of a half may overhang into the spare_slots slots that follow.
+ * record per later stage in shared form.  In a packed stage, launched layer q computes per window one box of tbox[q] =
+ * max(e_head[q], e_tail[q], 4) rows at each end (its edge rows), floor(128 / tbox[q]) boxes per 128-row MMA tile, in slots
+ * of P rows: the box, the two rows next to the edge rows that later layers read (copied from the stream) and, if the next
+ * stage is packed too, the rows its first two layers reach, which it reads in place (P is then even).  The last box of a half
+ * may overhang into the spare_slots slots that follow.
  * AFRAME_EINVAL / AFRAME_ESHAPE for bad arguments or a bad table. */
 typedef struct {
   int32_t first_layer, n_layers;   /* table index of the stage's entry conv; layers that launch (<= 16 are described) */
   int32_t T, C;                    /* rows per window and channels of the stage's output                             */
   int32_t head, tail;              /* rows at a window's start / end within reach of its zero padding, stage output  */
-  int32_t packed;                  /* 1: packed edge batch (CTA-pair kernels); 0: fixed-length short windows         */
+  int32_t packed;                  /* 1: packed edge batch; 0: fixed-length short windows                            */
   int32_t P;                       /* packed: rows per slot; else data rows of a short window                        */
   int32_t spare_slots;             /* packed: slots after each half                                                   */
   int32_t e_head[16], e_tail[16], tbox[16];
