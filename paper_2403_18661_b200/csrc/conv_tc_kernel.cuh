@@ -155,7 +155,7 @@ __device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b
 // NP x 8 channels (pieces jj0 .. jj0 + NP - 1 of a 64-channel chunk) of one output row: + bias (+ residual read from the
 // staging buffer) -> fp16 (RNE, saturating) -> max(., lo) (lo = 0: ReLU, which commutes with the rounding; lo = -inf: none)
 // -> staging buffer, or the fused head's dot product.  v holds the NP * 8 accumulator columns.
-template <bool RES, bool HEAD, int NP>
+template <bool RES, bool HEAD, int NP, bool ZR = true>
 __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4* bias4, const float4* hw4,
                                                  unsigned char* rowp, int row, int jj0, __half2 lo2, float& head_acc,
                                                  bool zero_row = false) {
@@ -188,7 +188,7 @@ __device__ __forceinline__ void tc_epilogue_math(const uint32_t* v, const float4
       const __half2 m = __hmax2(*reinterpret_cast<const __half2*>(&pk), lo2);
       ow[e] = *reinterpret_cast<const uint32_t*>(&m);
     }
-    if (zero_row) o = make_uint4(0u, 0u, 0u, 0u);
+    if (ZR && zero_row) o = make_uint4(0u, 0u, 0u, 0u);
     if (HEAD) {
       const float4 hA = hw4[2 * jj], hB = hw4[2 * jj + 1];
       const float2 o0 = af_act_unpack2(o.x), o1 = af_act_unpack2(o.y), o2 = af_act_unpack2(o.z), o3 = af_act_unpack2(o.w);
@@ -766,8 +766,13 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
                               ((t_row - p.zero_origin + p.zero_period) % p.zero_period) >= p.zero_valid;
         const uint4* copy_row = copy_tile != nullptr ? copy_tile + c * 8 : nullptr;
         constexpr int NP = EC / 8;
-        if (p.has_res) tc_epilogue_math<true, HEAD, NP>(v, bias4, hw4, rowp, row, hf * NP, lo2, head_acc, zero_row);
-        else tc_epilogue_math<false, HEAD, NP>(v, bias4, hw4, rowp, row, hf * NP, lo2, head_acc, zero_row);
+        if (p.zero_period > 0) {                   // (row masks exist only in the fixed-length short-window form)
+          if (p.has_res) tc_epilogue_math<true, HEAD, NP, true>(v, bias4, hw4, rowp, row, hf * NP, lo2, head_acc, zero_row);
+          else tc_epilogue_math<false, HEAD, NP, true>(v, bias4, hw4, rowp, row, hf * NP, lo2, head_acc, zero_row);
+        } else {
+          if (p.has_res) tc_epilogue_math<true, HEAD, NP, false>(v, bias4, hw4, rowp, row, hf * NP, lo2, head_acc);
+          else tc_epilogue_math<false, HEAD, NP, false>(v, bias4, hw4, rowp, row, hf * NP, lo2, head_acc);
+        }
         if (!HEAD && copy_row != nullptr) {        // the staged row is replaced by the stream's (independent loads, then the stores)
           uint4 cr[NP];
 #pragma unroll
