@@ -572,7 +572,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
       }
       tma_store_wait_all<0>();
     } else if (STW && !HALO) {
-      // ===== lanes 1..31 of the store warps (CTA-pair storing variant), on their own path: packed edge batch, the stream rows
+      // ===== lanes 1..31 of the store warps (ring variants that store), on their own path: packed edge batch, the stream rows
       // next to each slot's edge rows that the box does not hold (see TcConvParams::edge_out), global -> global, store warp g
       // taking its 1/EG of the tile's columns.  Nothing in this launch reads these rows, so the path meets no barrier.
       auto copy_rows = [&](const TcConvParams& P, int worker) {
@@ -613,7 +613,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tm_in /* HALO: box of 130 row
         }
       };
       copy_rows(p, worker);
-      if (!HALO && !HEAD && p1.num_tiles > 0) copy_rows(p1, worker1);
+      if (p1.num_tiles > 0) copy_rows(p1, worker1);
     }
   } else {
     // ===== epilogue: EG groups of 4 warps, thread <-> one output row =====
