@@ -243,28 +243,23 @@ __global__ void __launch_bounds__(SN_THREADS, 1) stream_net_kernel(const SnParam
     {
       const int ppr_log = 31 - __clz(L.c_in >> 3);  // pieces per row (c_in / 8, a power of two)
       const int total = L.in_rows << ppr_log;
-      // all loads of a thread first (independent L2 round trips), then the stores: <= SN_GP pieces per thread
-      uint4 v[SN_GP];
+      // asynchronous copies straight into shared memory (<= SN_GP pieces per thread, all in flight at once); rows outside the
+      // window are written as zeros.  (One bulk copy per row instead was measured: 2.3-2.9 us per layer against 0.9-2.2.)
 #pragma unroll
       for (int k = 0; k < SN_GP; ++k) {
         const int i = tid + k * SN_THREADS;
-        v[k] = make_uint4(0, 0, 0, 0);
         if (i < total) {
           const int j = i >> ppr_log, q = i - (j << ppr_log);
           const int s = j >= L.seg_in_base[2] ? 2 : (j >= L.seg_in_base[1] ? 1 : 0);
           const int r_first = s == 0 ? L.T_out - L.f - L.nnew : (s == 1 ? 0 : L.T_out - L.f);
           const int r_in = L.P * r_first - L.pad + (j - L.seg_in_base[s]);
-          if (r_in >= 0 && r_in < L.T_in) v[k] = sn_ldcg(reinterpret_cast<const uint4*>(sn_row(Lin, p.arena, r_in, base_in)) + q);
+          unsigned char* dst = in_tile + (size_t)j * row_bytes + q * 16;
+          if (r_in >= 0 && r_in < L.T_in) sn_cp_async16(sn_smem_u32(dst), reinterpret_cast<const uint4*>(sn_row(Lin, p.arena, r_in, base_in)) + q);
+          else *reinterpret_cast<uint4*>(dst) = make_uint4(0, 0, 0, 0);
         }
       }
-#pragma unroll
-      for (int k = 0; k < SN_GP; ++k) {
-        const int i = tid + k * SN_THREADS;
-        if (i < total) {
-          const int j = i >> ppr_log, q = i - (j << ppr_log);
-          *reinterpret_cast<uint4*>(in_tile + (size_t)j * row_bytes + q * 16) = v[k];
-        }
-      }
+      sn_cp_async_commit();
+      sn_cp_async_wait_all();
     }
     __syncthreads();
     SN_T(li, 1);
@@ -334,9 +329,10 @@ __global__ void __launch_bounds__(SN_THREADS, 1) stream_net_kernel(const SnParam
         // accumulator fragment of m16n8: lane = (row % 8) * 4 + col / 2, register = (row / 8) * 2 + col % 2
         for (int k = 0; k < L.kc; ++k) {
           const int w = i * L.kc + k;
-          const float* pp = part + (size_t)(w * SN_MAX_MT + mt) * 128;
-#pragma unroll
-          for (int j = 0; j < 8; ++j) v[j] += pp[((rr >> 3) * 2 + (j & 1)) * 32 + (rr & 7) * 4 + (j >> 1)];
+          // (the row's even columns are register (rr / 8) * 2 of four consecutive lanes, its odd columns the next register)
+          const float* pp = part + (size_t)(w * SN_MAX_MT + mt) * 128 + (rr >> 3) * 64 + (rr & 7) * 4;
+          const float4 ev = *reinterpret_cast<const float4*>(pp), od = *reinterpret_cast<const float4*>(pp + 32);
+          v[0] += ev.x; v[1] += od.x; v[2] += ev.y; v[3] += od.y; v[4] += ev.z; v[5] += od.z; v[6] += ev.w; v[7] += od.w;
         }
         const int r = sn_out_row(L, m);
         if (L.res_layer >= 0) {
