@@ -84,6 +84,8 @@ __device__ __forceinline__ uint32_t sn_cluster_size() { uint32_t r; asm volatile
 __device__ __forceinline__ void sn_cluster_sync() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+__device__ __forceinline__ void sn_cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void sn_cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 __device__ __forceinline__ void sn_ldmatrix_x4(uint32_t addr, uint32_t (&a)[4]) {
   asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];"
                : "=r"(a[0]), "=r"(a[1]), "=r"(a[2]), "=r"(a[3]) : "r"(addr));
@@ -313,7 +315,6 @@ __global__ void __launch_bounds__(SN_THREADS, 1) stream_net_kernel(const SnParam
     sn_cp_async_wait_all();                        // this thread's residual / bias pieces have landed; after the barrier everyone's
     __syncthreads();
     SN_T(li, 2);
-    sn_prefetch(li + 1);                           // the next layer's first weight fragments travel during the epilogue and the barrier
 
     // epilogue: one thread per (output row, output block): sum the K chunks in order, + bias (+ residual) -> fp16 -> ReLU
     {
@@ -368,7 +369,11 @@ __global__ void __launch_bounds__(SN_THREADS, 1) stream_net_kernel(const SnParam
       }
     }
     SN_T(li, 3);
-    sn_cluster_sync();                             // this layer's rows are visible to every CTA; shared memory is free again
+    // this layer's rows become visible to every CTA; the next layer's first weight fragments (which depend on no activation)
+    // are issued between the arrival and the wait, so that their issue time hides in the barrier's latency
+    sn_cluster_arrive();
+    sn_prefetch(li + 1);
+    sn_cluster_wait();
     SN_T(li, 4);
   }
 
