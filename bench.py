@@ -620,6 +620,9 @@ def run_ours(args):
         out["roofline"]["useful_mmac_per_window"] = useful / 1e6
         out["roofline"]["useful_frac_of_executed"] = useful / mmac_exec if mmac_exec > 0 else None
         out["roofline"]["useful_tflops"] = exec_tflops * useful / mmac_exec if mmac_exec > 0 else None
+        # the same against the peak: `frac` counts every executed FLOP, padding rows included, so it FALLS when padding is
+        # removed; this one only counts rows the method needs
+        out["roofline"]["useful_frac_of_peak"] = (exec_tflops * useful / mmac_exec / peaks["bf16_sustained"]) if mmac_exec > 0 else None
     except Exception as e:                                       # (a table the incremental plan does not cover)
         out["roofline"]["useful_frac_of_executed"] = None
         out["roofline"]["useful_note"] = repr(e)
